@@ -1,0 +1,328 @@
+"""Pins of the CPU oracle against things other than itself (all CPU, `-m "not gpu"`).
+
+Each test names the plausible oracle mistake it would catch.  Nothing here touches the CUDA path.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from tests import helpers as Hh
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+SENT = 0xA5
+
+
+def _rand_pool(rng, nbytes):
+    return rng.integers(0, 256, size=nbytes, dtype=np.uint8)
+
+
+def _geom(layout, L, H, D, NB, BS):
+    return getattr(O.PoolGeom, layout)(L, H, D, 2, NB, BS)
+
+
+# ---------------------------------------------------------------------------------------
+# element placement
+# ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("layout", ["lkbthd", "blkhtd"])
+def test_same_layout_full_blocks_equals_numpy_fancy_indexing(layout):
+    """Catches: wrong stride order, swapped src/dst table, K|V or layer axis mix-up."""
+    rng = np.random.default_rng(1)
+    L, H, D, NB, BS, n = 3, 2, 8, 11, 4, 6
+    g = _geom(layout, L, H, D, NB, BS)
+    src = _rand_pool(rng, g.span_bytes())
+    dst = np.full(g.span_bytes(), SENT, np.uint8)
+    Src = rng.permutation(NB)[:n]
+    Dst = rng.permutation(NB)[:n]
+    O.transfer(src, g, dst, g, Src, Dst, n * BS)
+    exp = np.full(g.span_bytes(), SENT, np.uint8)
+    ev = Hh.logical_view(exp, layout, L, NB, BS, H, D)
+    sv = Hh.logical_view(src, layout, L, NB, BS, H, D)
+    ev[:, :, Dst] = sv[:, :, Src]
+    assert np.array_equal(dst, exp)
+
+
+@pytest.mark.parametrize("bs_s,bs_d,src_layout,dst_layout", [
+    (4, 4, "lkbthd", "blkhtd"), (2, 8, "lkbthd", "blkhtd"), (8, 2, "blkhtd", "lkbthd"), (4, 16, "lkbthd", "lkbthd"),
+])
+def test_layout_and_block_size_conversion_equals_numpy_reshape(bs_s, bs_d, src_layout, dst_layout):
+    """Full blocks on both sides: gather -> flatten tokens -> regroup into dst blocks.
+    Catches: head/token transposition errors, wrong div/mod block size on one side."""
+    rng = np.random.default_rng(2)
+    L, H, D = 2, 3, 8
+    T = 32
+    ns, nd = T // bs_s, T // bs_d
+    NBs, NBd = ns + 3, nd + 2
+    gs, gd = _geom(src_layout, L, H, D, NBs, bs_s), _geom(dst_layout, L, H, D, NBd, bs_d)
+    src = _rand_pool(rng, gs.span_bytes())
+    dst = np.full(gd.span_bytes(), SENT, np.uint8)
+    Src, Dst = rng.permutation(NBs)[:ns], rng.permutation(NBd)[:nd]
+    O.transfer(src, gs, dst, gd, Src, Dst, T)
+    sv = Hh.logical_view(src, src_layout, L, NBs, bs_s, H, D)
+    toks = sv[:, :, Src].reshape(L, 2, T, H, D)
+    exp = np.full(gd.span_bytes(), SENT, np.uint8)
+    ev = Hh.logical_view(exp, dst_layout, L, NBd, bs_d, H, D)
+    ev[:, :, Dst] = toks.reshape(L, 2, nd, bs_d, H, D)
+    assert np.array_equal(dst, exp)
+
+
+def test_self_describing_pool_lands_where_definition_says():
+    """src rows carry their own (l,c,block,tok,h) in their first 5 words; after the move each dst row
+    named by the definition must carry the coordinates computed directly from the tables.
+    Independent of the oracle's src addressing.  Catches: off-by-one in t//BS, t%BS, wrong table side."""
+    rng = np.random.default_rng(3)
+    L, H, D, NBs, NBd, bs_s, bs_d, T = 2, 2, 8, 9, 5, 4, 8, 27
+    gs, gd = _geom("lkbthd", L, H, D, NBs, bs_s), _geom("blkhtd", L, H, D, NBd, bs_d)
+    src = np.zeros(gs.span_bytes(), np.uint8)
+    sv = Hh.logical_view(src, "lkbthd", L, NBs, bs_s, H, D)
+    l, c, b, t, h = np.meshgrid(np.arange(L), np.arange(2), np.arange(NBs), np.arange(bs_s), np.arange(H), indexing="ij")
+    for k, a in enumerate((l, c, b, t, h)):
+        sv[..., k] = a + 1
+    Src = rng.permutation(NBs)[:-(-T // bs_s)]
+    Dst = rng.permutation(NBd)[:-(-T // bs_d)]
+    dst = np.zeros(gd.span_bytes(), np.uint8)
+    O.transfer(src, gs, dst, gd, Src, Dst, T)
+    dv = Hh.logical_view(dst, "blkhtd", L, NBd, bs_d, H, D)
+    seen = 0
+    for tt in range(T):
+        for ll in range(L):
+            for cc in range(2):
+                for hh in range(H):
+                    row = dv[ll, cc, Dst[tt // bs_d], tt % bs_d, hh]
+                    assert list(row[:5]) == [ll + 1, cc + 1, Src[tt // bs_s] + 1, tt % bs_s + 1, hh + 1]
+                    seen += 1
+    # and nothing else was written (rows not named stay zero)
+    assert np.count_nonzero(dv[..., 0]) == seen
+
+
+def test_identity_tables_is_memcmp_prefix():
+    """Identity tables + identical geometry: dst prefix == src prefix byte for byte."""
+    rng = np.random.default_rng(4)
+    L, H, D, NB, BS = 1, 2, 8, 6, 4
+    g = _geom("blkhtd", 1, H, D, NB, BS)   # L=1 blkhtd: a block is one contiguous span
+    src = _rand_pool(rng, g.span_bytes())
+    dst = np.full(g.span_bytes(), SENT, np.uint8)
+    O.transfer(src, g, dst, g, np.arange(4), np.arange(4), 4 * BS)
+    n = 4 * g.s_block
+    assert dst[:n].tobytes() == src[:n].tobytes()
+    assert np.all(dst[n:] == SENT)
+
+
+@pytest.mark.parametrize("T", [0, 1, 5, 8, 9, 15])
+def test_partial_last_block_and_untouched_bytes(T):
+    """Reading A4: only t < T is copied; every other dst byte keeps the sentinel; src unchanged.
+    Catches: whole-block copies, tail spill, writes into src."""
+    rng = np.random.default_rng(5)
+    L, H, D, NB, BS = 2, 2, 8, 6, 4
+    gs, gd = _geom("lkbthd", L, H, D, NB, BS), _geom("blkhtd", L, H, D, NB, BS)
+    src = _rand_pool(rng, gs.span_bytes())
+    src0 = src.copy()
+    dst = np.full(gd.span_bytes(), SENT, np.uint8)
+    nb = -(-T // BS)
+    Src, Dst = rng.permutation(NB)[:nb], rng.permutation(NB)[:nb]
+    O.transfer(src, gs, dst, gd, Src, Dst, T)
+    assert np.array_equal(src, src0)
+    exp = np.full(gd.span_bytes(), SENT, np.uint8)
+    ev, sv = Hh.logical_view(exp, "blkhtd", L, NB, BS, H, D), Hh.logical_view(src, "lkbthd", L, NB, BS, H, D)
+    for t in range(T):
+        ev[:, :, Dst[t // BS], t % BS] = sv[:, :, Src[t // BS], t % BS]
+    assert np.array_equal(dst, exp)
+    assert np.count_nonzero(dst != SENT) <= T * gs.bytes_per_token
+
+
+def test_all_65536_bit_patterns_survive():
+    """Raw-bit fidelity: NaN payloads, -0, denormals, Inf.  Catches: any pass through a float type."""
+    L, H, D, BS = 1, 2, 64, 16
+    NB = 65536 // (2 * BS * H * D)  # 16 blocks -> 65,536 elements
+    g = _geom("lkbthd", L, H, D, NB, BS)
+    src = np.arange(65536, dtype=np.uint16).view(np.uint8).copy()
+    assert src.size == g.span_bytes()
+    dst = np.zeros_like(src)
+    perm = np.random.default_rng(6).permutation(NB)
+    O.transfer(src, g, dst, g, perm, np.arange(NB), NB * BS)
+    sv, dv = Hh.logical_view(src, "lkbthd", L, NB, BS, H, D), Hh.logical_view(dst, "lkbthd", L, NB, BS, H, D)
+    assert np.array_equal(dv, sv[:, :, perm])
+    assert np.array_equal(np.sort(dst.view(np.uint16)), np.arange(65536, dtype=np.uint16))
+
+
+def test_layer_range_and_layer_slab():
+    """Layer windows: [l0,l1) touches only those layers; a slab handed in with layer0 gives the same bytes."""
+    rng = np.random.default_rng(7)
+    L, H, D, NB, BS, T = 4, 2, 8, 5, 4, 14
+    g = _geom("lkbthd", L, H, D, NB, BS)
+    src = _rand_pool(rng, g.span_bytes())
+    Src, Dst = rng.permutation(NB)[:4], rng.permutation(NB)[:4]
+    full = np.full(g.span_bytes(), SENT, np.uint8)
+    O.transfer(src, g, full, g, Src, Dst, T)
+    part = np.full(g.span_bytes(), SENT, np.uint8)
+    O.transfer(src, g, part, g, Src, Dst, T, l0=1, l1=3)
+    assert np.array_equal(part[g.s_layer:3 * g.s_layer], full[g.s_layer:3 * g.s_layer])
+    assert np.all(part[:g.s_layer] == SENT) and np.all(part[3 * g.s_layer:] == SENT)
+    slab = np.full(g.s_layer, SENT, np.uint8)
+    O.transfer(src[2 * g.s_layer:3 * g.s_layer].copy(), g, slab, g, Src, Dst, T, l0=2, l1=3, src_layer0=2, dst_layer0=2)
+    assert np.array_equal(slab, full[2 * g.s_layer:3 * g.s_layer])
+
+
+def test_out_of_range_block_id_rejected():
+    g = _geom("lkbthd", 1, 1, 8, 4, 4)
+    src = np.zeros(g.span_bytes(), np.uint8)
+    dst = np.zeros(g.span_bytes(), np.uint8)
+    with pytest.raises(ValueError):
+        O.transfer(src, g, dst, g, [4], [0], 4)
+    with pytest.raises(ValueError):
+        O.transfer(src, g, dst, g, [0], [-1], 4)
+
+
+# ---------------------------------------------------------------------------------------
+# pack / unpack (wire format reading A12)
+# ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("layout", ["lkbthd", "blkhtd"])
+def test_pack_equals_numpy_gather_and_unpack_inverts(layout):
+    """staging[request][layer][K|V][token][head][dim].  Catches: wrong request offset, plane stride T_r,
+    token/head order in the wire format."""
+    rng = np.random.default_rng(8)
+    L, H, D, NB, BS = 2, 3, 8, 12, 4
+    g = _geom(layout, L, H, D, NB, BS)
+    src = _rand_pool(rng, g.span_bytes())
+    Ts = [7, 0, 12, 5]
+    perm = rng.permutation(NB)
+    tabs, off = [], 0
+    for T in Ts:
+        nb = -(-T // BS)
+        tabs.append(perm[off:off + nb]); off += nb
+    bpt = g.bytes_per_token
+    staging = np.full(sum(Ts) * bpt, SENT, np.uint8)
+    sv = Hh.logical_view(src, layout, L, NB, BS, H, D)
+    exp_parts, tok_off = [], 0
+    for T, tab in zip(Ts, tabs):
+        O.pack(src, g, tab, T, staging, tok_off)
+        tok_off += T
+        exp_parts.append(sv[:, :, tab].reshape(L, 2, len(tab) * BS, H, D)[:, :, :T].reshape(-1))
+    assert np.array_equal(staging.view(np.uint16), np.concatenate(exp_parts))
+    # unpack through DIFFERENT dst tables == transfer src->dst directly
+    gd = _geom("blkhtd" if layout == "lkbthd" else "lkbthd", L, H, D, NB, BS * 2)
+    dperm = rng.permutation(NB)
+    d1 = np.full(gd.span_bytes(), SENT, np.uint8)
+    d2 = np.full(gd.span_bytes(), SENT, np.uint8)
+    tok_off = doff = 0
+    for T, tab in zip(Ts, tabs):
+        nb = -(-T // (BS * 2))
+        dtab = dperm[doff:doff + nb]; doff += nb
+        O.unpack(staging, tok_off, d1, gd, dtab, T)
+        O.transfer(src, g, d2, gd, tab, dtab, T)
+        tok_off += T
+    assert np.array_equal(d1, d2)
+
+
+def test_pack_unpack_identity_and_round_trip():
+    """unpack(pack(pool,T),T) restores every named slot; transfer S->D then D->S restores src slots."""
+    rng = np.random.default_rng(9)
+    L, H, D, NB, BS, T = 2, 2, 8, 7, 4, 22
+    g = _geom("lkbthd", L, H, D, NB, BS)
+    pool = _rand_pool(rng, g.span_bytes())
+    tab = rng.permutation(NB)[:6]
+    staging = np.zeros(T * g.bytes_per_token, np.uint8)
+    O.pack(pool, g, tab, T, staging, 0)
+    back = np.full(g.span_bytes(), SENT, np.uint8)
+    O.unpack(staging, 0, back, g, tab, T)
+    pv, bv = Hh.logical_view(pool, "lkbthd", L, NB, BS, H, D), Hh.logical_view(back, "lkbthd", L, NB, BS, H, D)
+    for t in range(T):
+        assert np.array_equal(bv[:, :, tab[t // BS], t % BS], pv[:, :, tab[t // BS], t % BS])
+    assert np.count_nonzero(back != SENT) <= T * g.bytes_per_token
+    gd = _geom("blkhtd", L, H, D, 4, 8)
+    mid = np.zeros(gd.span_bytes(), np.uint8)
+    dtab = rng.permutation(4)[:3]
+    O.transfer(pool, g, mid, gd, tab, dtab, T)
+    again = np.full(g.span_bytes(), SENT, np.uint8)
+    O.transfer(mid, gd, again, g, dtab, tab, T)
+    assert np.array_equal(again, back)
+
+
+# ---------------------------------------------------------------------------------------
+# plan oracle: bidirectional segment alignment
+# ---------------------------------------------------------------------------------------
+def _expand(t):
+    return list(range(*t["arange"])) if isinstance(t, dict) else t
+
+
+def test_golden_alignment_fixtures():
+    with open(os.path.join(GOLD, "align_examples.json")) as f:
+        gold = json.load(f)
+    for case in gold["cases"]:
+        got = O.align(_expand(case["src"]), case["bs_src"], _expand(case["dst"]), case["bs_dst"], case["tokens"])
+        assert got == [tuple(x) for x in case["expect"]], case["cite"]
+        assert O.count_segments(_expand(case["src"]), case["bs_src"], _expand(case["dst"]), case["bs_dst"],
+                                case["tokens"]) == len(case["expect"])
+    for c in gold["blockwise_calls"]:
+        assert O.blockwise_calls(c["n_blocks"], c["num_layers"]) == c["expect"], c["cite"]
+
+
+def test_alignment_equals_token_level_definition_random():
+    """Oracle works on granule ids; the definition is restated here on TOKEN slots.  Catches wrong
+    granule scaling (BS/g), wrong gcd, missed break on one side, tail clamp."""
+    rng = np.random.default_rng(10)
+    for _ in range(300):
+        bs_s, bs_d = (int(x) for x in rng.choice([1, 2, 4, 8, 16], size=2))
+        T = int(rng.integers(0, 90))
+        ns, nd = -(-T // bs_s), -(-T // bs_d)
+        # tables with long-ish runs so that merges actually happen
+        def tab(n):
+            out, cur = [], int(rng.integers(0, 50))
+            for _ in range(n):
+                out.append(cur)
+                cur = cur + 1 if rng.random() < 0.7 else int(rng.integers(0, 200))
+            return out
+        S, Dd = tab(ns), tab(nd)
+        got = O.align(S, bs_s, Dd, bs_d, T)
+        exp = Hh.segments_from_cuts(Hh.cuts_by_definition(S, bs_s, Dd, bs_d, T), T)
+        assert got == exp
+        if T:
+            Hh.check_segment_invariants(got, S, bs_s, Dd, bs_d, T)
+        # one-sided (pack / unpack) plans
+        assert O.align(S, bs_s, None, 0, T) == Hh.segments_from_cuts(Hh.cuts_by_definition(S, bs_s, None, 0, T), T)
+        assert O.align(None, 0, Dd, bs_d, T) == Hh.segments_from_cuts(Hh.cuts_by_definition(None, 0, Dd, bs_d, T), T)
+
+
+def test_alignment_is_the_unique_minimal_partition_bruteforce():
+    """Exhaustive: every way to cut a tiny request; the oracle's list is THE minimal legal partition
+    (so 'number of segments == number of maximal consecutive-id runs', north_star)."""
+    for bs_s, bs_d in [(2, 2), (2, 4), (4, 2), (1, 2)]:
+        for T in (5, 8, 9):
+            ns, nd = -(-T // bs_s), -(-T // bs_d)
+            pool_s, pool_d = ns + 1, nd + 1
+            rng = np.random.default_rng(100 + T + 10 * bs_s + bs_d)
+            all_s = list(Hh.injective_tables(pool_s, ns))
+            all_d = list(Hh.injective_tables(pool_d, nd))
+            pick_s = [all_s[i] for i in rng.choice(len(all_s), size=min(12, len(all_s)), replace=False)]
+            pick_d = [all_d[i] for i in rng.choice(len(all_d), size=min(12, len(all_d)), replace=False)]
+            for S in pick_s:
+                for Dd in pick_d:
+                    best, parts = Hh.brute_force_min_partition(S, bs_s, Dd, bs_d, T)
+                    got = O.align(list(S), bs_s, list(Dd), bs_d, T)
+                    assert len(got) == best and parts == [got]
+
+
+def test_random_permutation_table_gives_one_segment_per_block():
+    """BASELINE.json configs[0]: run length 1 => 63 segments for 1000 tokens."""
+    from paper_2504_03775_b200 import synth
+    w = synth.config1_tiny()
+    r = w.requests[0]
+    assert O.count_segments(r.src_blocks, 16, r.dst_blocks, 16, r.num_tokens) == 63
+    assert O.blockwise_calls(len(r.src_blocks), w.shape.num_layers) == 252
+
+
+def test_expected_break_rate_independent_sides():
+    """Independent geometric runs (mean 2 src, mean 16 dst): P(break) = 1 - (1/2)(15/16) = 0.531."""
+    rng = np.random.default_rng(11)
+    n = 40000
+
+    def tab(p):
+        out, cur = [], 0
+        for _ in range(n):
+            out.append(cur)
+            cur = cur + 1 if rng.random() >= p else cur + 2 + int(rng.integers(0, 5))
+        return out
+    segs = O.count_segments(tab(0.5), 16, tab(1 / 16), 16, n * 16)
+    assert abs(segs / n - (1 - 0.5 * 15 / 16)) < 0.01
