@@ -1,0 +1,216 @@
+/*
+ * flowkv.h — C-ABI boundary of the B200-native FlowKV KV-cache transfer path.
+ *
+ * What the path is (arXiv 2504.03775; "P:Lnn" = /root/reference/PAPER.md line nn):
+ *   P:L69  §3.1   "transfers the KV Cache K and V from node P_p to node D_d"
+ *   P:L92  §3.3   the KV cache is paged (logical -> physical block mapping), so a request's
+ *                 cache is many small scattered chunks
+ *   P:L98-103 Eq.5  two orders of the same pool axes, (L,2,B,H) and (B,L,2,H)
+ *   P:L107 §3.3, Fig.5  "bidirectional segment alignment": compare the block-id lists
+ *                 of sender and receiver, merge ids that are memory-contiguous on BOTH sides into
+ *                 one transfer
+ * Restated for one B200 (BASELINE.json north_star): the "transfer" is a block-table driven
+ * gather / layout-convert / scatter between two pools in HBM (or a dense staging buffer in
+ * device or mapped pinned host memory), executed by ONE persistent sm_100a kernel per batch.
+ *
+ * Result that every entry point below reaches exactly (pure byte movement):
+ *   for every request r, token t in [0,T_r), layer l, c in {K,V}, head h, dim d
+ *     dst[l, c, Dst_r[t div BS_d], t mod BS_d, h, d] := src[l, c, Src_r[t div BS_s], t mod BS_s, h, d]
+ *   each side addressed as base + l*s_layer + c*s_kv + blk*s_block + tok*s_token + h*s_head + d*e.
+ *   Every other byte of dst keeps its value; src is never written.
+ *
+ * Conventions
+ *   - All functions return a flowkv_status, never throw, never abort, never call exit.
+ *   - "host" / "device" is stated for every pointer.  Pools, staging buffers and streams are
+ *     the caller's; the library never allocates, frees or reallocs them.  A plan owns only
+ *     its own small descriptor buffers (host + device).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - All validation happens in flowkv_plan(); running a plan enqueues EXACTLY ONE kernel on
+ *     the caller's stream (zero for an empty plan) and returns without synchronising.
+ *   - There is no CPU fallback and no other backend: without a CUDA device every call that
+ *     needs one returns FLOWKV_ERR_CUDA.
+ *   - Thread safety: distinct plans may be used from distinct threads; flowkv_last_error()
+ *     is thread-local.
+ */
+#ifndef FLOWKV_H_
+#define FLOWKV_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FLOWKV_VERSION 1
+
+#if defined(__GNUC__)
+#define FLOWKV_API __attribute__((visibility("default")))
+#else
+#define FLOWKV_API
+#endif
+
+typedef enum {
+  FLOWKV_OK = 0,
+  FLOWKV_ERR_INVALID_ARG = 1,      /* NULL where a pointer is required, bad enum / flag           */
+  FLOWKV_ERR_BLOCK_OOB = 2,        /* a block id is < 0 or >= num_blocks of its pool               */
+  FLOWKV_ERR_TABLE_LEN = 3,        /* n_*_blocks != ceil(num_tokens / block_size)                  */
+  FLOWKV_ERR_DST_ALIAS = 4,        /* same dst block named twice in the batch (write race)        */
+  FLOWKV_ERR_ALIGN = 5,            /* a base, stride or the row size is not a multiple of 16 B     */
+  FLOWKV_ERR_SHAPE_MISMATCH = 6,   /* src and dst pools differ in L, Hkv, Dh or elem_bytes         */
+  FLOWKV_ERR_UNSUPPORTED = 7,      /* e.g. block_size not a power of two, plan lacks the operation */
+  FLOWKV_ERR_STAGING_TOO_SMALL = 8,
+  FLOWKV_ERR_NOMEM = 9,
+  FLOWKV_ERR_CUDA = 10             /* a CUDA runtime call failed; flowkv_last_error() has its text */
+} flowkv_status;
+
+/* Pool layouts.  `dim` (head_dim elements of elem_bytes) is always innermost and contiguous.
+ *   LKBTHD  [layer][K|V][block][token][head][dim]  — Eq. 5 left side  (L,2,B,H), H=[token][head][dim]
+ *   BLKHTD  [block][layer][K|V][head][token][dim]  — Eq. 5 right side (B,L,2,H), H=[head][token][dim]
+ *   STRIDED caller fills stride_bytes[] itself (separate K and V tensors, padded blocks, ...).    */
+typedef enum {
+  FLOWKV_LAYOUT_LKBTHD = 0,
+  FLOWKV_LAYOUT_BLKHTD = 1,
+  FLOWKV_LAYOUT_STRIDED = 2
+} flowkv_layout;
+
+enum { FLOWKV_S_LAYER = 0, FLOWKV_S_KV = 1, FLOWKV_S_BLOCK = 2, FLOWKV_S_TOKEN = 3, FLOWKV_S_HEAD = 4 };
+
+/* A paged KV pool.  Caller-owned memory. */
+typedef struct {
+  void*    base;            /* DEVICE pointer to element [0,0,0,0,0,0]; 16-B aligned (32-B enables 256-bit accesses) */
+  uint32_t num_layers;      /* L                                                                    */
+  uint32_t num_kv_heads;    /* Hkv                                                                  */
+  uint32_t head_dim;        /* Dh; head_dim*elem_bytes (one "row") must be a multiple of 16 bytes   */
+  uint32_t elem_bytes;      /* e; the library is dtype-agnostic, bytes move verbatim                */
+  uint32_t num_blocks;      /* NB                                                                   */
+  uint32_t block_size;      /* BS, tokens per block; power of two                                   */
+  uint32_t layout;          /* flowkv_layout                                                        */
+  uint32_t _reserved;
+  int64_t  stride_bytes[5]; /* layer, kv, block, token, head — see FLOWKV_S_*; multiples of 16      */
+} flowkv_pool;
+
+/* One request: its length and both sides' block-id lists.
+ * HOST pointers, borrowed only for the duration of flowkv_plan(). */
+typedef struct {
+  uint32_t       num_tokens;     /* T_r; 0 is legal (contributes nothing)                          */
+  uint32_t       n_src_blocks;   /* must equal ceil(T_r / src.block_size) when src pool is given   */
+  const int32_t* src_blocks;     /* HOST; may be NULL when the plan has no src pool                */
+  const int32_t* dst_blocks;     /* HOST; may be NULL when the plan has no dst pool                */
+  uint32_t       n_dst_blocks;   /* must equal ceil(T_r / dst.block_size) when dst pool is given   */
+  uint32_t       _reserved;
+} flowkv_request;
+
+/* One aligned segment (read-only view for tests / reporting): a maximal stretch of a request whose
+ * token slots are consecutive on BOTH sides (unique, in request order then token order). */
+typedef struct {
+  uint32_t request;         /* index into reqs[]                                                    */
+  uint32_t first_token;     /* first token of the stretch within its request                        */
+  uint32_t n_tokens;
+  uint32_t src_block, src_tok_off;   /* where it starts on the src side (0,0 without a src pool)    */
+  uint32_t dst_block, dst_tok_off;   /* where it starts on the dst side (0,0 without a dst pool)    */
+  uint32_t _reserved;
+  uint64_t staging_tok_off; /* exclusive prefix sum of T over the requests before `request`         */
+} flowkv_segment;
+
+/* Plan flags */
+#define FLOWKV_CHECK_DST_ALIAS   (1u << 0)  /* reject a dst block id used twice (A9)                 */
+#define FLOWKV_PLAN_NO_TRANSFER  (1u << 1)  /* do not build the pool->pool schedule                  */
+#define FLOWKV_PLAN_NO_PACK      (1u << 2)  /* do not build the pool->staging schedule               */
+#define FLOWKV_PLAN_NO_UNPACK    (1u << 3)  /* do not build the staging->pool schedule               */
+
+/* Optional tuning; zero-initialise for defaults.  Never changes results, only the schedule. */
+typedef struct {
+  uint32_t tile_bytes;      /* max bytes one thread group copies per tile (0 = auto; pow2, 1 KiB..1 MiB) */
+  uint32_t ctas_per_sm;     /* resident CTAs per SM of the persistent grid (0 = auto)               */
+  uint32_t max_sms;         /* SM budget: grid = min(#SMs, max_sms) * ctas_per_sm (0 = all SMs; P:L92 co-run) */
+  uint32_t threads;         /* threads per CTA (0 = auto; multiple of 32, <= 1024)                  */
+  uint32_t group_threads;   /* threads that share one tile (0 = auto; 32..threads, power of two)    */
+  uint32_t variant;         /* flowkv_variant (0 = auto)                                            */
+  uint32_t tile_order;      /* 0 = auto, 1 = plane-major (all tiles of plane 0, then plane 1, ...), 2 = chunk-major */
+  uint32_t cache_hint;      /* ldst: 0 = auto, 1 = default caching, 2 = L1::no_allocate, 3 = + L2::evict_first */
+  uint32_t stages;          /* bulk: ring depth (0 = auto; 2..16)                                   */
+  uint32_t _reserved[3];
+} flowkv_tuning;
+
+typedef enum {
+  FLOWKV_VARIANT_AUTO = 0,
+  FLOWKV_VARIANT_LDST = 1,   /* register path: 128/256-bit ld.global / st.global, unrolled        */
+  FLOWKV_VARIANT_BULK = 2    /* TMA path: cp.async.bulk gmem->smem->gmem ring driven by one thread  */
+} flowkv_variant;
+
+typedef struct flowkv_plan_s flowkv_plan_t;
+
+typedef struct {
+  uint64_t n_requests, n_segments;
+  uint64_t total_tokens, payload_bytes;     /* payload = total_tokens * 2*L*Hkv*Dh*e                */
+  uint64_t staging_bytes;                   /* dense wire size == payload_bytes                     */
+  uint64_t n_chunks_transfer, n_chunks_pack, n_chunks_unpack;  /* schedule entries per plane         */
+  uint64_t plan_device_bytes;               /* descriptor bytes resident on the device              */
+  uint32_t n_planes;                        /* 2*L                                                  */
+  uint32_t mode_transfer, mode_pack, mode_unpack;   /* 0 = absent, 1 = span (contiguous), 2 = rows  */
+  uint32_t grid, threads, group_threads, tile_bytes, variant, vec_bytes;   /* launch shape in use   */
+  uint32_t tile_order, cache_hint, stages, smem_bytes;                     /* (resolved, not 0)     */
+  uint32_t num_sms;
+  uint32_t _reserved;
+} flowkv_plan_stats;
+
+/* Fill stride_bytes[] of a LKBTHD / BLKHTD pool from its shape.  STRIDED: validates only.
+ * pool: HOST pointer, read-write. */
+FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
+
+/* Build a plan: validate (a1), bidirectional segment alignment (a2), tile schedule (a3),
+ * upload (a4; one cudaMalloc + one cudaMemcpyAsync on `stream`).
+ *   src, dst : HOST pointers to pool descriptors; either may be NULL (pack-only / unpack-only).
+ *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
+ *   tuning   : HOST pointer or NULL.
+ *   out      : HOST pointer; receives the plan (caller destroys it).  Untouched on error.
+ * The plan stays valid until destroyed; pools must stay alive while it is run. */
+FLOWKV_API flowkv_status flowkv_plan(const flowkv_pool* src, const flowkv_pool* dst,
+                          const flowkv_request* reqs, uint32_t n_reqs, uint32_t flags,
+                          const flowkv_tuning* tuning, void* stream, flowkv_plan_t** out);
+
+/* Host-only variant of the same planner: no CUDA call at all (segments + stats only; the plan
+ * cannot be run).  Used by host-logic tests and multi-process sharding tests. */
+FLOWKV_API flowkv_status flowkv_plan_host(const flowkv_pool* src, const flowkv_pool* dst,
+                               const flowkv_request* reqs, uint32_t n_reqs, uint32_t flags,
+                               const flowkv_tuning* tuning, flowkv_plan_t** out);
+
+/* stats: HOST out.  segments: HOST out, receives a pointer owned by the plan (n_segments entries,
+ * valid until flowkv_plan_destroy); may be NULL. */
+FLOWKV_API flowkv_status flowkv_plan_info(const flowkv_plan_t* plan, flowkv_plan_stats* stats,
+                               const flowkv_segment** segments);
+
+/* Pool -> pool (a5).  One kernel launch on `stream`; no host synchronisation. */
+FLOWKV_API flowkv_status flowkv_transfer(const flowkv_plan_t* plan, void* stream);
+
+/* Pool -> dense staging (a6) / dense staging -> pool (a7).  Wire format (A12):
+ * [request][layer][K|V][token][head][dim], requests concatenated; request r starts at byte
+ * staging_tok_off(r) * bytes_per_token.  `staging`: DEVICE pointer, or a mapped pinned HOST
+ * pointer reachable from the device (UVA); 16-B aligned; `bytes` >= staging_bytes. */
+FLOWKV_API flowkv_status flowkv_pack(const flowkv_plan_t* plan, void* staging, uint64_t bytes, void* stream);
+FLOWKV_API flowkv_status flowkv_unpack(const flowkv_plan_t* plan, const void* staging, uint64_t bytes, void* stream);
+
+FLOWKV_API void flowkv_plan_destroy(flowkv_plan_t* plan);
+
+FLOWKV_API const char* flowkv_status_string(flowkv_status s);
+FLOWKV_API const char* flowkv_last_error(void);          /* thread-local text of the last failure          */
+
+/* Number of kernels this library has launched in this process (monotonic; for launch accounting). */
+FLOWKV_API uint64_t flowkv_launch_count(void);
+
+/* ---- comparison baselines (BASELINE.json north_star; they are NOT the product path) ----------
+ * Each issues cudaMemcpyAsync D2D copies on `stream` and writes the number issued to *n_calls.
+ * They require same-layout, token-major pools (LKBTHD or equivalent strides) and equal block sizes.
+ *   blockwise : one copy per (block, layer, K|V) — the pre-optimisation scheme of P:L92/L103;
+ *               a partial last block copies only its valid tokens.
+ *   segmentwise: one copy per (aligned segment, layer, K|V) — the paper's coalescing
+ *               with cudaMemcpyAsync in place of ncclSend/ncclRecv.                              */
+FLOWKV_API flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_pool* dst,
+                                        const flowkv_request* reqs, uint32_t n_reqs,
+                                        void* stream, uint64_t* n_calls);
+FLOWKV_API flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* plan, void* stream, uint64_t* n_calls);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLOWKV_H_ */

@@ -1,0 +1,475 @@
+// api.cpp — the C-ABI of include/flowkv.h: plan objects, upload, launches, error text.
+// Everything the hot path does on the device runs in kernels.cu; this file is host plumbing.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "flowkv_internal.h"
+
+using namespace flowkv;
+
+namespace {
+
+thread_local std::string g_last_error;
+std::atomic<uint64_t> g_launches{0};
+
+flowkv_status fail(flowkv_status s, const std::string& msg) {
+  g_last_error = msg;
+  return s;
+}
+flowkv_status fail_cuda(cudaError_t e, const char* what) {
+  g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+  return FLOWKV_ERR_CUDA;
+}
+
+bool is_pow2(uint32_t x) { return x && !(x & (x - 1)); }
+uint32_t log2u(uint32_t x) { uint32_t l = 0; while ((1u << l) < x) ++l; return l; }
+uint32_t log2_or_none(uint32_t x) { return is_pow2(x) ? log2u(x) : 0xffffffffu; }
+
+struct Op {                  // one runnable operation of a plan
+  Schedule sched;
+  const Chunk* d_chunks = nullptr;
+  LaunchShape shape{};
+  uint32_t tile_order = 0;   // resolved: 0 plane-major, 1 chunk-major
+  uint32_t max_chunk_bytes = 0;
+};
+
+}  // namespace
+
+struct flowkv_plan_s {
+  bool has_src = false, has_dst = false, on_device = false;
+  flowkv_pool src{}, dst{};
+  Geometry g{};
+  flowkv_tuning tuning{};
+  uint32_t tile_bytes = 0;
+  std::vector<flowkv_segment> segments;      // the reported alignment
+  std::vector<flowkv_segment> segs_pack, segs_unpack;
+  Op transfer, pack, unpack;
+  uint64_t n_requests = 0, total_tokens = 0;
+  void* d_buf = nullptr;
+  uint64_t d_bytes = 0;
+  int device = -1;
+  uint32_t num_sms = 0, max_smem_optin = 0;
+};
+
+namespace {
+
+// vector width every address of an operation is aligned to
+uint32_t pick_vec(const flowkv_pool* a, const flowkv_pool* b, const Geometry& g) {
+  auto ok32 = [&](const flowkv_pool* p) {
+    if (!p) return true;
+    if ((uintptr_t)p->base % 32) return false;
+    for (int i = 0; i < 5; ++i) if (p->stride_bytes[i] % 32) return false;
+    return true;
+  };
+  return (g.row_bytes % 32 == 0 && ok32(a) && ok32(b)) ? 32 : 16;
+}
+
+void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv_pool* b) {
+  const flowkv_tuning& t = pl->tuning;
+  LaunchShape& ls = op.shape;
+  const uint32_t sms = pl->num_sms ? pl->num_sms : 148;
+  const uint32_t use_sms = t.max_sms ? std::min(t.max_sms, sms) : sms;
+  ls.vec_bytes = pick_vec(a, b, pl->g);
+  ls.variant = t.variant ? t.variant : FLOWKV_VARIANT_LDST;
+  if (op.sched.mode != MODE_SPAN) ls.variant = FLOWKV_VARIANT_LDST;   // bulk handles contiguous chunks only
+  op.max_chunk_bytes = 0;
+  for (const Chunk& c : op.sched.chunks)
+    op.max_chunk_bytes = std::max(op.max_chunk_bytes, op.sched.mode == MODE_SPAN ? c.n : c.n * pl->g.tok_bytes);
+  op.tile_order = t.tile_order == 2 ? 1 : 0;
+  const uint64_t n_tiles = (uint64_t)op.sched.chunks.size() * 2 * pl->g.L;
+  if (ls.variant == FLOWKV_VARIANT_BULK) {
+    ls.threads = 32;
+    ls.group_threads = 32;
+    ls.stage_bytes = std::max<uint32_t>(op.max_chunk_bytes, 1024);
+    ls.stage_bytes = (ls.stage_bytes + 127) & ~127u;
+    const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 1;
+    const uint32_t smem_cap = (pl->max_smem_optin ? pl->max_smem_optin : 232448) - 1024;
+    const uint32_t budget = std::min<uint32_t>(smem_cap, (228u * 1024 - 2048) / ctas - 1024);
+    uint32_t stages = t.stages ? t.stages : 16;
+    stages = std::min<uint32_t>(stages, 16);
+    while (stages > 2 && (uint64_t)stages * ls.stage_bytes > budget) --stages;
+    ls.n_stages = stages;
+    ls.hint = 2;
+    ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(n_tiles, 1));
+    return;
+  }
+  ls.threads = t.threads ? t.threads : 256;
+  ls.group_threads = t.group_threads ? t.group_threads : ls.threads;
+  ls.hint = t.cache_hint ? t.cache_hint - 1 : 2;
+  ls.n_stages = 0;
+  ls.stage_bytes = 0;
+  const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 4;
+  const uint32_t groups_per_cta = ls.threads / ls.group_threads;
+  const uint64_t ctas_needed = (n_tiles + groups_per_cta - 1) / groups_per_cta;
+  ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(ctas_needed, 1));
+}
+
+flowkv_status check_tuning(const flowkv_tuning& t) {
+  if (t.tile_bytes && (!is_pow2(t.tile_bytes) || t.tile_bytes < 1024 || t.tile_bytes > (1u << 20)))
+    return fail(FLOWKV_ERR_INVALID_ARG, "tuning.tile_bytes must be a power of two in [1 KiB, 1 MiB]");
+  if (t.threads && (t.threads % 32 || t.threads > 512 || !is_pow2(t.threads)))
+    return fail(FLOWKV_ERR_INVALID_ARG, "tuning.threads must be a power of two in [32, 512]");
+  const uint32_t thr = t.threads ? t.threads : 256;
+  if (t.group_threads && (!is_pow2(t.group_threads) || t.group_threads < 32 || t.group_threads > thr))
+    return fail(FLOWKV_ERR_INVALID_ARG, "tuning.group_threads must be a power of two in [32, threads]");
+  if (t.variant > FLOWKV_VARIANT_BULK) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.variant unknown");
+  if (t.tile_order > 2) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.tile_order unknown");
+  if (t.cache_hint > 3) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.cache_hint unknown");
+  if (t.stages && (t.stages < 2 || t.stages > 16)) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.stages must be in [2,16]");
+  if (t.ctas_per_sm > 32) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.ctas_per_sm must be <= 32");
+  if (t.variant == FLOWKV_VARIANT_BULK && t.tile_bytes > (64u << 10))
+    return fail(FLOWKV_ERR_INVALID_ARG, "bulk variant: tile_bytes must be <= 64 KiB (two ring slots must fit in shared memory)");
+  return FLOWKV_OK;
+}
+
+flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs, uint32_t n_reqs,
+                        uint32_t flags, const flowkv_tuning* tuning, bool device, void* stream, flowkv_plan_t** out) {
+  if (!out) return fail(FLOWKV_ERR_INVALID_ARG, "out is NULL");
+  if (!src && !dst) return fail(FLOWKV_ERR_INVALID_ARG, "both pools are NULL");
+  if (n_reqs && !reqs) return fail(FLOWKV_ERR_INVALID_ARG, "reqs is NULL");
+  if (flags & ~(FLOWKV_CHECK_DST_ALIAS | FLOWKV_PLAN_NO_TRANSFER | FLOWKV_PLAN_NO_PACK | FLOWKV_PLAN_NO_UNPACK))
+    return fail(FLOWKV_ERR_INVALID_ARG, "unknown flag bit");
+  std::string err;
+  flowkv_status st;
+  if (src && (st = validate_pool(src, "src", err)) != FLOWKV_OK) return fail(st, err);
+  if (dst && (st = validate_pool(dst, "dst", err)) != FLOWKV_OK) return fail(st, err);
+  if (src && dst &&
+      (src->num_layers != dst->num_layers || src->num_kv_heads != dst->num_kv_heads ||
+       src->head_dim != dst->head_dim || src->elem_bytes != dst->elem_bytes))
+    return fail(FLOWKV_ERR_SHAPE_MISMATCH, "src and dst pools differ in num_layers, num_kv_heads, head_dim or elem_bytes");
+  flowkv_tuning tn{};
+  if (tuning) tn = *tuning;
+  if ((st = check_tuning(tn)) != FLOWKV_OK) return st;
+  if ((st = validate_requests(src, dst, reqs, n_reqs, flags, err)) != FLOWKV_OK) return fail(st, err);
+
+  flowkv_plan_t* pl = new (std::nothrow) flowkv_plan_s();
+  if (!pl) return fail(FLOWKV_ERR_NOMEM, "out of host memory");
+  try {
+    const flowkv_pool* any = src ? src : dst;
+    pl->has_src = src != nullptr;
+    pl->has_dst = dst != nullptr;
+    if (src) pl->src = *src;
+    if (dst) pl->dst = *dst;
+    pl->tuning = tn;
+    Geometry& g = pl->g;
+    g.L = any->num_layers; g.Hkv = any->num_kv_heads; g.Dh = any->head_dim; g.e = any->elem_bytes;
+    g.row_bytes = g.Dh * g.e;
+    g.tok_bytes = g.Hkv * g.row_bytes;
+    g.bytes_per_token = 2ull * g.L * g.tok_bytes;
+    pl->n_requests = n_reqs;
+    for (uint32_t r = 0; r < n_reqs; ++r) pl->total_tokens += reqs[r].num_tokens;
+    if ((uint64_t)g.Hkv * g.row_bytes > (1u << 24)) {
+      delete pl;
+      return fail(FLOWKV_ERR_UNSUPPORTED, "token larger than 16 MiB per plane");
+    }
+
+    if (device) {
+      cudaError_t e = cudaGetDevice(&pl->device);
+      if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaGetDevice"); }
+      int v = 0;
+      e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, pl->device);
+      if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaDeviceGetAttribute"); }
+      pl->num_sms = (uint32_t)v;
+      pl->max_smem_optin = bulk_max_smem();
+    } else {
+      pl->num_sms = 148;
+    }
+
+    // tile size: default 32 KiB; shrink for small batches so every SM gets several tiles
+    uint32_t tile = tn.tile_bytes;
+    if (!tile) {
+      tile = 32u << 10;
+      const uint64_t want_tiles = 8ull * pl->num_sms;
+      const uint64_t payload = pl->total_tokens * g.bytes_per_token;
+      while (tile > 4096 && payload / tile < want_tiles) tile >>= 1;
+    }
+    pl->tile_bytes = tile;
+
+    const bool do_transfer = src && dst && !(flags & FLOWKV_PLAN_NO_TRANSFER);
+    const bool do_pack = src && !(flags & FLOWKV_PLAN_NO_PACK);
+    const bool do_unpack = dst && !(flags & FLOWKV_PLAN_NO_UNPACK);
+    // the reported alignment: both sides when both pools are given, else one-sided
+    align_segments(src, dst, reqs, n_reqs, pl->segments);
+    if (do_transfer) {
+      build_schedule(src, dst, g, reqs, pl->segments, tile, 0, pl->transfer.sched);
+      resolve_shape(pl, pl->transfer, src, dst);
+    }
+    if (do_pack) {
+      if (dst) align_segments(src, nullptr, reqs, n_reqs, pl->segs_pack);
+      build_schedule(src, nullptr, g, reqs, dst ? pl->segs_pack : pl->segments, tile, 0, pl->pack.sched);
+      resolve_shape(pl, pl->pack, src, nullptr);
+    }
+    if (do_unpack) {
+      if (src) align_segments(nullptr, dst, reqs, n_reqs, pl->segs_unpack);
+      build_schedule(nullptr, dst, g, reqs, src ? pl->segs_unpack : pl->segments, tile, 0, pl->unpack.sched);
+      resolve_shape(pl, pl->unpack, nullptr, dst);
+    }
+    for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack})
+      if ((uint64_t)op->sched.chunks.size() * 2 * g.L >= (1ull << 31)) {
+        delete pl;
+        return fail(FLOWKV_ERR_UNSUPPORTED, "more than 2^31 tiles in one batch; split the batch");
+      }
+
+    if (device) {
+      // a4: one allocation, one stream-ordered upload for all schedules
+      uint64_t bytes = 0;
+      for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) bytes += op->sched.chunks.size() * sizeof(Chunk);
+      if (bytes) {
+        cudaError_t e = cudaMalloc(&pl->d_buf, bytes);
+        if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaMalloc(plan)"); }
+        pl->d_bytes = bytes;
+        char* p = (char*)pl->d_buf;
+        for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) {
+          const uint64_t n = op->sched.chunks.size() * sizeof(Chunk);
+          if (!n) continue;
+          e = cudaMemcpyAsync(p, op->sched.chunks.data(), n, cudaMemcpyHostToDevice, (cudaStream_t)stream);
+          if (e != cudaSuccess) { cudaFree(pl->d_buf); delete pl; return fail_cuda(e, "cudaMemcpyAsync(plan)"); }
+          op->d_chunks = (const Chunk*)p;
+          p += n;
+        }
+      }
+      pl->on_device = true;
+    }
+  } catch (const std::bad_alloc&) {
+    delete pl;
+    return fail(FLOWKV_ERR_NOMEM, "out of host memory");
+  }
+  *out = pl;
+  return FLOWKV_OK;
+}
+
+Side pool_side(const flowkv_pool& p) {
+  Side s{};
+  s.base = (char*)p.base;
+  s.s_layer = p.stride_bytes[FLOWKV_S_LAYER];
+  s.s_kv = p.stride_bytes[FLOWKV_S_KV];
+  s.s_token = p.stride_bytes[FLOWKV_S_TOKEN];
+  s.s_head = p.stride_bytes[FLOWKV_S_HEAD];
+  s.dense = 0;
+  return s;
+}
+
+Side dense_side(const void* staging, const Geometry& g) {
+  Side s{};
+  s.base = (char*)staging;
+  s.s_layer = 0; s.s_kv = 0;               // plane stride comes from the chunk's req_tokens
+  s.s_token = g.tok_bytes;
+  s.s_head = g.row_bytes;
+  s.dense = 1;
+  return s;
+}
+
+flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Side& d, uint32_t vec_bytes, void* stream) {
+  if (!pl->on_device) return fail(FLOWKV_ERR_UNSUPPORTED, "plan was built by flowkv_plan_host and cannot run");
+  if (op.sched.chunks.empty()) return FLOWKV_OK;       // A11: empty batch, zero launches
+  KernelParams kp{};
+  kp.src = s; kp.dst = d;
+  kp.chunks = op.d_chunks;
+  kp.n_chunks = (uint32_t)op.sched.chunks.size();
+  kp.n_planes = 2 * pl->g.L;
+  kp.n_tiles = kp.n_chunks * kp.n_planes;
+  kp.row_bytes = pl->g.row_bytes;
+  kp.heads = pl->g.Hkv;
+  kp.tok_bytes = pl->g.tok_bytes;
+  kp.tile_order = op.tile_order;
+  LaunchShape ls = op.shape;
+  ls.vec_bytes = vec_bytes;
+  kp.group_log2 = log2u(ls.group_threads);
+  kp.vpr_log2 = log2_or_none(kp.row_bytes / ls.vec_bytes);
+  kp.heads_log2 = log2_or_none(kp.heads);
+  const int e = launch_copy(op.sched.mode, kp, ls, stream);
+  if (e != 0) return fail_cuda((cudaError_t)e, "kernel launch");
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return FLOWKV_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+flowkv_status flowkv_pool_strides(flowkv_pool* p) {
+  if (!p) return fail(FLOWKV_ERR_INVALID_ARG, "pool is NULL");
+  const int64_t row = (int64_t)p->head_dim * p->elem_bytes;
+  if (p->layout == FLOWKV_LAYOUT_LKBTHD) {
+    p->stride_bytes[FLOWKV_S_HEAD] = row;
+    p->stride_bytes[FLOWKV_S_TOKEN] = row * p->num_kv_heads;
+    p->stride_bytes[FLOWKV_S_BLOCK] = p->stride_bytes[FLOWKV_S_TOKEN] * p->block_size;
+    p->stride_bytes[FLOWKV_S_KV] = p->stride_bytes[FLOWKV_S_BLOCK] * p->num_blocks;
+    p->stride_bytes[FLOWKV_S_LAYER] = 2 * p->stride_bytes[FLOWKV_S_KV];
+  } else if (p->layout == FLOWKV_LAYOUT_BLKHTD) {
+    p->stride_bytes[FLOWKV_S_TOKEN] = row;
+    p->stride_bytes[FLOWKV_S_HEAD] = row * p->block_size;
+    p->stride_bytes[FLOWKV_S_KV] = p->stride_bytes[FLOWKV_S_HEAD] * p->num_kv_heads;
+    p->stride_bytes[FLOWKV_S_LAYER] = 2 * p->stride_bytes[FLOWKV_S_KV];
+    p->stride_bytes[FLOWKV_S_BLOCK] = p->stride_bytes[FLOWKV_S_LAYER] * p->num_layers;
+  } else if (p->layout != FLOWKV_LAYOUT_STRIDED) {
+    return fail(FLOWKV_ERR_INVALID_ARG, "unknown layout");
+  }
+  for (int i = 0; i < 5; ++i)
+    if (p->stride_bytes[i] <= 0) return fail(FLOWKV_ERR_INVALID_ARG, "a stride is <= 0");
+  return FLOWKV_OK;
+}
+
+flowkv_status flowkv_plan(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs, uint32_t n_reqs,
+                          uint32_t flags, const flowkv_tuning* tuning, void* stream, flowkv_plan_t** out) {
+  return make_plan(src, dst, reqs, n_reqs, flags, tuning, true, stream, out);
+}
+
+flowkv_status flowkv_plan_host(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
+                               uint32_t n_reqs, uint32_t flags, const flowkv_tuning* tuning, flowkv_plan_t** out) {
+  return make_plan(src, dst, reqs, n_reqs, flags, tuning, false, nullptr, out);
+}
+
+flowkv_status flowkv_plan_info(const flowkv_plan_t* pl, flowkv_plan_stats* st, const flowkv_segment** segments) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (st) {
+    memset(st, 0, sizeof *st);
+    st->n_requests = pl->n_requests;
+    st->n_segments = pl->segments.size();
+    st->total_tokens = pl->total_tokens;
+    st->payload_bytes = pl->total_tokens * pl->g.bytes_per_token;
+    st->staging_bytes = st->payload_bytes;
+    st->n_chunks_transfer = pl->transfer.sched.chunks.size();
+    st->n_chunks_pack = pl->pack.sched.chunks.size();
+    st->n_chunks_unpack = pl->unpack.sched.chunks.size();
+    st->plan_device_bytes = pl->d_bytes;
+    st->n_planes = 2 * pl->g.L;
+    st->mode_transfer = pl->transfer.sched.mode;
+    st->mode_pack = pl->pack.sched.mode;
+    st->mode_unpack = pl->unpack.sched.mode;
+    const Op& op = pl->transfer.sched.mode != MODE_ABSENT ? pl->transfer
+                   : (pl->pack.sched.mode != MODE_ABSENT ? pl->pack : pl->unpack);
+    st->grid = op.shape.grid;
+    st->threads = op.shape.threads;
+    st->group_threads = op.shape.group_threads;
+    st->tile_bytes = pl->tile_bytes;
+    st->variant = op.shape.variant;
+    st->vec_bytes = op.shape.vec_bytes;
+    st->tile_order = op.tile_order + 1;
+    st->cache_hint = op.shape.hint + 1;
+    st->stages = op.shape.n_stages;
+    st->smem_bytes = op.shape.n_stages * op.shape.stage_bytes;
+    st->num_sms = pl->num_sms;
+  }
+  if (segments) *segments = pl->segments.data();
+  return FLOWKV_OK;
+}
+
+flowkv_status flowkv_transfer(const flowkv_plan_t* pl, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (pl->transfer.sched.mode == MODE_ABSENT)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pool-to-pool schedule (needs both pools, no FLOWKV_PLAN_NO_TRANSFER)");
+  return run(pl, pl->transfer, pool_side(pl->src), pool_side(pl->dst), pl->transfer.shape.vec_bytes, stream);
+}
+
+flowkv_status flowkv_pack(const flowkv_plan_t* pl, void* staging, uint64_t bytes, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (pl->pack.sched.mode == MODE_ABSENT)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pack schedule (needs a src pool, no FLOWKV_PLAN_NO_PACK)");
+  if (pl->pack.sched.chunks.empty()) return FLOWKV_OK;
+  if (!staging) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
+  if ((uintptr_t)staging % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
+  if (bytes < pl->total_tokens * pl->g.bytes_per_token) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
+  const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
+  return run(pl, pl->pack, pool_side(pl->src), dense_side(staging, pl->g), vec, stream);
+}
+
+flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (pl->unpack.sched.mode == MODE_ABSENT)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no unpack schedule (needs a dst pool, no FLOWKV_PLAN_NO_UNPACK)");
+  if (pl->unpack.sched.chunks.empty()) return FLOWKV_OK;
+  if (!staging) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
+  if ((uintptr_t)staging % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
+  if (bytes < pl->total_tokens * pl->g.bytes_per_token) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
+  const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
+  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst), vec, stream);
+}
+
+void flowkv_plan_destroy(flowkv_plan_t* pl) {
+  if (!pl) return;
+  if (pl->d_buf) cudaFree(pl->d_buf);
+  delete pl;
+}
+
+const char* flowkv_status_string(flowkv_status s) {
+  switch (s) {
+    case FLOWKV_OK: return "FLOWKV_OK";
+    case FLOWKV_ERR_INVALID_ARG: return "FLOWKV_ERR_INVALID_ARG";
+    case FLOWKV_ERR_BLOCK_OOB: return "FLOWKV_ERR_BLOCK_OOB";
+    case FLOWKV_ERR_TABLE_LEN: return "FLOWKV_ERR_TABLE_LEN";
+    case FLOWKV_ERR_DST_ALIAS: return "FLOWKV_ERR_DST_ALIAS";
+    case FLOWKV_ERR_ALIGN: return "FLOWKV_ERR_ALIGN";
+    case FLOWKV_ERR_SHAPE_MISMATCH: return "FLOWKV_ERR_SHAPE_MISMATCH";
+    case FLOWKV_ERR_UNSUPPORTED: return "FLOWKV_ERR_UNSUPPORTED";
+    case FLOWKV_ERR_STAGING_TOO_SMALL: return "FLOWKV_ERR_STAGING_TOO_SMALL";
+    case FLOWKV_ERR_NOMEM: return "FLOWKV_ERR_NOMEM";
+    case FLOWKV_ERR_CUDA: return "FLOWKV_ERR_CUDA";
+  }
+  return "FLOWKV_ERR_?";
+}
+
+const char* flowkv_last_error(void) { return g_last_error.c_str(); }
+
+uint64_t flowkv_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+// ---- comparison baselines: many cudaMemcpyAsync calls (NOT the product path) --------------------
+flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
+                                        uint32_t n_reqs, void* stream, uint64_t* n_calls) {
+  if (!src || !dst || (n_reqs && !reqs)) return fail(FLOWKV_ERR_INVALID_ARG, "NULL argument");
+  std::string err;
+  flowkv_status st;
+  if ((st = validate_pool(src, "src", err)) != FLOWKV_OK) return fail(st, err);
+  if ((st = validate_pool(dst, "dst", err)) != FLOWKV_OK) return fail(st, err);
+  if ((st = validate_requests(src, dst, reqs, n_reqs, 0, err)) != FLOWKV_OK) return fail(st, err);
+  Geometry g{};
+  g.L = src->num_layers; g.Hkv = src->num_kv_heads; g.Dh = src->head_dim; g.e = src->elem_bytes;
+  g.row_bytes = g.Dh * g.e; g.tok_bytes = g.Hkv * g.row_bytes; g.bytes_per_token = 2ull * g.L * g.tok_bytes;
+  if (src->block_size != dst->block_size || !pool_is_span_capable(*src, g) || !pool_is_span_capable(*dst, g))
+    return fail(FLOWKV_ERR_UNSUPPORTED, "blockwise baseline needs equal block sizes and token-major pools");
+  uint64_t calls = 0;
+  const uint32_t bs = src->block_size;
+  for (uint32_t r = 0; r < n_reqs; ++r)
+    for (uint32_t b = 0; b < reqs[r].n_src_blocks; ++b) {
+      const uint32_t ntok = std::min(bs, reqs[r].num_tokens - b * bs);
+      for (uint32_t l = 0; l < g.L; ++l)
+        for (uint32_t c = 0; c < 2; ++c) {
+          const char* s = (const char*)src->base + l * src->stride_bytes[0] + c * src->stride_bytes[1] +
+                          (int64_t)reqs[r].src_blocks[b] * src->stride_bytes[2];
+          char* d = (char*)dst->base + l * dst->stride_bytes[0] + c * dst->stride_bytes[1] +
+                    (int64_t)reqs[r].dst_blocks[b] * dst->stride_bytes[2];
+          cudaError_t e = cudaMemcpyAsync(d, s, (size_t)ntok * g.tok_bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+          if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
+          ++calls;
+        }
+    }
+  if (n_calls) *n_calls = calls;
+  return FLOWKV_OK;
+}
+
+flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* pl, void* stream, uint64_t* n_calls) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (!pl->has_src || !pl->has_dst || !pool_is_span_capable(pl->src, pl->g) || !pool_is_span_capable(pl->dst, pl->g))
+    return fail(FLOWKV_ERR_UNSUPPORTED, "segmentwise baseline needs two token-major pools");
+  uint64_t calls = 0;
+  const flowkv_pool &S = pl->src, &D = pl->dst;
+  for (const flowkv_segment& sg : pl->segments)
+    for (uint32_t l = 0; l < pl->g.L; ++l)
+      for (uint32_t c = 0; c < 2; ++c) {
+        const char* s = (const char*)S.base + l * S.stride_bytes[0] + c * S.stride_bytes[1] +
+                        (int64_t)sg.src_block * S.stride_bytes[2] + (int64_t)sg.src_tok_off * S.stride_bytes[3];
+        char* d = (char*)D.base + l * D.stride_bytes[0] + c * D.stride_bytes[1] +
+                  (int64_t)sg.dst_block * D.stride_bytes[2] + (int64_t)sg.dst_tok_off * D.stride_bytes[3];
+        cudaError_t e = cudaMemcpyAsync(d, s, (size_t)sg.n_tokens * pl->g.tok_bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+        if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
+        ++calls;
+      }
+  if (n_calls) *n_calls = calls;
+  return FLOWKV_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,99 @@
+// flowkv_internal.h — structures shared by the host planner, the C-ABI layer and the sm_100a
+// kernels of the product path.  Nothing under oracle/ includes this file.
+#pragma once
+
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/flowkv.h"
+
+namespace flowkv {
+
+// ---------------------------------------------------------------------------------------------
+// Device-visible schedule entry ("chunk"): one unit of work of one plane.  The same chunk list
+// serves every plane p = 2*layer + kv; the kernel adds the plane offset of each side:
+//   pool side   : layer*s_layer + kv*s_kv
+//   dense side  : p * req_tokens * tok_bytes            (wire format A12: [req][l][c][t][h][d])
+// span mode: `n` BYTES that are contiguous on both sides.
+// rows mode: `n` TOKENS; token t, head h of the chunk sits at off + t*s_token + h*s_head per side.
+// ---------------------------------------------------------------------------------------------
+struct alignas(32) Chunk {
+  int64_t  src_off;      // bytes from the src side's base, plane offset excluded
+  int64_t  dst_off;      // bytes from the dst side's base, plane offset excluded
+  uint32_t n;            // span: bytes (multiple of the vector width); rows: tokens
+  uint32_t req_tokens;   // T_r of the owning request (dense-side plane stride = T_r * tok_bytes)
+  uint32_t request;      // owning request (reporting only)
+  uint32_t _pad;
+};
+static_assert(sizeof(Chunk) == 32, "Chunk is loaded as one 32-byte vector");
+
+enum Mode : uint32_t { MODE_ABSENT = 0, MODE_SPAN = 1, MODE_ROWS = 2 };
+
+struct Side {            // one end of a copy as the kernel sees it
+  char*    base;         // device (or mapped host) pointer
+  int64_t  s_layer, s_kv, s_token, s_head;   // bytes; s_token/s_head used in rows mode only
+  uint32_t dense;        // 1: dense staging buffer, 0: paged pool
+  uint32_t _pad;
+};
+
+struct KernelParams {
+  Side         src, dst;
+  const Chunk* chunks;       // device
+  uint32_t     n_chunks;     // per plane
+  uint32_t     n_planes;     // 2L
+  uint32_t     n_tiles;      // n_chunks * n_planes
+  uint32_t     row_bytes;    // Dh*e
+  uint32_t     heads;        // Hkv
+  uint32_t     tok_bytes;    // Hkv*Dh*e
+  uint32_t     tile_order;   // 0 plane-major, 1 chunk-major (resolved by the plan)
+  uint32_t     group_log2;   // log2(threads sharing a tile)
+  uint32_t     vpr_log2;     // rows mode: log2(vectors per row) or 0xffffffff if not a power of two
+  uint32_t     heads_log2;   // rows mode: log2(Hkv) or 0xffffffff
+};
+
+struct LaunchShape {
+  uint32_t grid, threads, group_threads, vec_bytes;
+  uint32_t variant;       // FLOWKV_VARIANT_LDST | FLOWKV_VARIANT_BULK
+  uint32_t hint;          // ldst: 0 default caching, 1 L1::no_allocate, 2 + L2::evict_first
+  uint32_t n_stages;      // bulk: ring depth
+  uint32_t stage_bytes;   // bulk: bytes per ring slot (>= largest chunk)
+};
+
+// kernels.cu — launches exactly one kernel; returns cudaError_t as int.
+int launch_copy(Mode mode, const KernelParams& kp, const LaunchShape& ls, void* stream);
+// Largest dynamic shared memory the bulk variant may use on the current device (0 on failure).
+uint32_t bulk_max_smem();
+
+// ---------------------------------------------------------------------------------------------
+// Host planner (planner.cpp) — pure integer host code, no CUDA.
+// ---------------------------------------------------------------------------------------------
+struct Geometry {          // what both sides must agree on
+  uint32_t L, Hkv, Dh, e;
+  uint32_t row_bytes, tok_bytes;
+  uint64_t bytes_per_token;
+};
+
+struct Schedule {
+  Mode mode = MODE_ABSENT;
+  std::vector<Chunk> chunks;
+};
+
+// Is a pool's block interior token-major and dense, with consecutive blocks abutting per plane?
+bool pool_is_span_capable(const flowkv_pool& p, const Geometry& g);
+
+flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string& err);
+flowkv_status validate_requests(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
+                                uint32_t n_reqs, uint32_t flags, std::string& err);
+
+// Bidirectional segment alignment.  `src`/`dst` may be NULL (dense side).
+void align_segments(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
+                    uint32_t n_reqs, std::vector<flowkv_segment>& out);
+
+// Cut aligned segments into chunks no larger than tile_bytes.
+void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geometry& g,
+                    const flowkv_request* reqs, const std::vector<flowkv_segment>& segs,
+                    uint32_t tile_bytes, uint32_t vec_bytes, Schedule& out);
+
+}  // namespace flowkv

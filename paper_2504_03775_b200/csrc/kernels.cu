@@ -1,0 +1,321 @@
+// kernels.cu — the persistent sm_100a copy kernels of the FlowKV transfer path (step a5-a7).
+//
+// One launch moves a whole transfer batch ("from 23,469 [calls] to just 1").  The grid
+// is persistent (a multiple of the SM count); thread groups walk a linear tile space
+//     tile -> (plane, chunk)      plane = 2*layer + kv, chunk = entry of the plan's schedule
+// with a static stride, so there is no per-block / per-layer launch and no atomics.  The path is a
+// pure byte move: no FP, no tensor cores; the bound is HBM bandwidth.
+//
+// Variants
+//   ldst : registers.  256-bit (LDG.E.256 / STG.E.256, sm_100+) or 128-bit vector accesses,
+//          UNROLL independent loads in flight per thread before the first store, streaming cache
+//          hints (L1::no_allocate, L2::evict_first) because nothing is ever re-read.
+//            span mode : a chunk is one byte range contiguous on both sides.
+//            rows mode : a chunk is n tokens x Hkv rows of Dh*e bytes; each side has its own
+//                        token / head stride (layout + block-size conversion, BASELINE configs[3]).
+//   bulk : TMA bulk copies (cp.async.bulk -> UBLKCP) gmem -> smem -> gmem through an mbarrier
+//          ring driven by ONE thread per CTA; span mode only.  Uses no registers or LSU slots
+//          for payload, which is what a copy that co-runs with GEMMs wants.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "flowkv_internal.h"
+
+namespace flowkv {
+
+// ------------------------------------------------------------------------------------------------
+// vector load / store with cache hints
+// ------------------------------------------------------------------------------------------------
+template <int VEC> struct Vec;
+template <> struct alignas(16) Vec<16> { uint32_t x, y, z, w; };
+template <> struct alignas(32) Vec<32> { uint64_t a, b, c, d; };
+
+// HINT 0: default caching.  1: L1::no_allocate.  2: L1::no_allocate + L2::evict_first.
+template <int VEC, int HINT> struct Mem;
+
+template <int HINT> struct Mem<32, HINT> {
+  static __device__ __forceinline__ Vec<32> ld(const char* p, uint64_t) {
+    Vec<32> v;
+    if (HINT == 0)
+      asm volatile("ld.global.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(v.a), "=l"(v.b), "=l"(v.c), "=l"(v.d) : "l"(p));
+    else if (HINT == 1)
+      asm volatile("ld.global.L1::no_allocate.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(v.a), "=l"(v.b), "=l"(v.c), "=l"(v.d) : "l"(p));
+    else
+      asm volatile("ld.global.L1::no_allocate.L2::evict_first.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(v.a), "=l"(v.b), "=l"(v.c), "=l"(v.d) : "l"(p));
+    return v;
+  }
+  static __device__ __forceinline__ void st(char* p, const Vec<32>& v, uint64_t) {
+    if (HINT == 0)
+      asm volatile("st.global.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(v.a), "l"(v.b), "l"(v.c), "l"(v.d) : "memory");
+    else if (HINT == 1)
+      asm volatile("st.global.L1::no_allocate.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(v.a), "l"(v.b), "l"(v.c), "l"(v.d) : "memory");
+    else
+      asm volatile("st.global.L1::no_allocate.L2::evict_first.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(v.a), "l"(v.b), "l"(v.c), "l"(v.d) : "memory");
+  }
+};
+
+template <int HINT> struct Mem<16, HINT> {
+  static __device__ __forceinline__ Vec<16> ld(const char* p, uint64_t pol) {
+    Vec<16> v;
+    if (HINT == 0)
+      asm volatile("ld.global.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    else if (HINT == 1)
+      asm volatile("ld.global.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    else   // 128-bit forms take the L2 priority through a policy operand
+      asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.b32 {%0,%1,%2,%3}, [%4], %5;"
+                   : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol));
+    return v;
+  }
+  static __device__ __forceinline__ void st(char* p, const Vec<16>& v, uint64_t pol) {
+    if (HINT == 0)
+      asm volatile("st.global.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+    else if (HINT == 1)
+      asm volatile("st.global.L1::no_allocate.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+    else
+      asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.b32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y),
+                   "r"(v.z), "r"(v.w), "l"(pol) : "memory");
+  }
+};
+
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+
+__device__ __forceinline__ Chunk load_chunk(const Chunk* p) {
+  // 32-byte read-only load of one schedule entry (every thread of the group reads the same one)
+  Chunk c;
+  uint64_t a, b, d, e;
+  asm volatile("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(d), "=l"(e) : "l"(p));
+  c.src_off = (int64_t)a;
+  c.dst_off = (int64_t)b;
+  c.n = (uint32_t)d;
+  c.req_tokens = (uint32_t)(d >> 32);
+  c.request = (uint32_t)e;
+  c._pad = 0;
+  return c;
+}
+
+__device__ __forceinline__ int64_t plane_offset(const Side& s, uint32_t plane, uint32_t req_tokens, uint32_t tok_bytes) {
+  return s.dense ? (int64_t)plane * ((int64_t)req_tokens * tok_bytes)
+                 : (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv;
+}
+
+__device__ __forceinline__ void decode_tile(const KernelParams& p, uint32_t tile, uint32_t& plane, uint32_t& ci) {
+  if (p.tile_order == 0) { plane = tile / p.n_chunks; ci = tile - plane * p.n_chunks; }
+  else                   { ci = tile / p.n_planes;    plane = tile - ci * p.n_planes; }
+}
+
+// ------------------------------------------------------------------------------------------------
+// ldst / span
+// ------------------------------------------------------------------------------------------------
+template <int VEC, int UNROLL, int HINT>
+__global__ void __launch_bounds__(512, 1) fk_span_ldst(const __grid_constant__ KernelParams p) {
+  const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t G = 1u << p.group_log2;
+  const uint32_t lane = gtid & (G - 1);
+  const uint32_t n_groups = (gridDim.x * blockDim.x) >> p.group_log2;
+  const uint32_t step = G * VEC;
+  const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
+
+  for (uint32_t tile = gtid >> p.group_log2; tile < p.n_tiles; tile += n_groups) {
+    uint32_t plane, ci;
+    decode_tile(p, tile, plane, ci);
+    const Chunk c = load_chunk(p.chunks + ci);
+    const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
+    char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    const uint32_t n = c.n;
+    uint32_t off = lane * VEC;
+    // full rounds: UNROLL independent loads in flight, then UNROLL stores
+    while (off + (UNROLL - 1) * step < n) {
+      Vec<VEC> v[UNROLL];
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) v[j] = Mem<VEC, HINT>::ld(s + off + j * step, pol);
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) Mem<VEC, HINT>::st(d + off + j * step, v[j], pol);
+      off += UNROLL * step;
+    }
+    // ragged tail: at most UNROLL-1 more vectors for this thread
+    if (off < n) {
+      Vec<VEC> v[UNROLL - 1];
+#pragma unroll
+      for (int j = 0; j < UNROLL - 1; ++j)
+        if (off + j * step < n) v[j] = Mem<VEC, HINT>::ld(s + off + j * step, pol);
+#pragma unroll
+      for (int j = 0; j < UNROLL - 1; ++j)
+        if (off + j * step < n) Mem<VEC, HINT>::st(d + off + j * step, v[j], pol);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// ldst / rows: token- and head-strided rows (layout and block-size conversion fused in the move)
+// ------------------------------------------------------------------------------------------------
+template <int VEC, int UNROLL, int HINT>
+__global__ void __launch_bounds__(512, 1) fk_rows_ldst(const __grid_constant__ KernelParams p) {
+  const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t G = 1u << p.group_log2;
+  const uint32_t lane = gtid & (G - 1);
+  const uint32_t n_groups = (gridDim.x * blockDim.x) >> p.group_log2;
+  const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
+  const uint32_t vpr = p.row_bytes / VEC;            // vectors per row
+  const bool pow2 = (p.vpr_log2 != 0xffffffffu) && (p.heads_log2 != 0xffffffffu);
+
+  for (uint32_t tile = gtid >> p.group_log2; tile < p.n_tiles; tile += n_groups) {
+    uint32_t plane, ci;
+    decode_tile(p, tile, plane, ci);
+    const Chunk c = load_chunk(p.chunks + ci);
+    const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
+    char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    const uint32_t pieces = c.n * p.heads * vpr;       // vectors in this chunk, (token, head, vec) order
+    for (uint32_t i0 = lane; i0 < pieces; i0 += G * UNROLL) {
+      Vec<VEC> v[UNROLL];
+      int64_t doff[UNROLL];
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j) {
+        const uint32_t i = i0 + j * G;
+        if (i < pieces) {
+          uint32_t row, o, tok, h;
+          if (pow2) {
+            row = i >> p.vpr_log2;   o = i & (vpr - 1);
+            tok = row >> p.heads_log2; h = row & (p.heads - 1);
+          } else {
+            row = i / vpr;       o = i - row * vpr;
+            tok = row / p.heads; h = row - tok * p.heads;
+          }
+          const int64_t soff = (int64_t)tok * p.src.s_token + (int64_t)h * p.src.s_head + o * VEC;
+          doff[j] = (int64_t)tok * p.dst.s_token + (int64_t)h * p.dst.s_head + o * VEC;
+          v[j] = Mem<VEC, HINT>::ld(s + soff, pol);
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < UNROLL; ++j)
+        if (i0 + j * G < pieces) Mem<VEC, HINT>::st(d + doff[j], v[j], pol);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// bulk / span: TMA bulk copies through a shared-memory ring, one driving thread per CTA
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, uint32_t bytes, uint64_t pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst),
+               "r"(smem_u32(smem_src)), "r"(bytes), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+constexpr int kBulkMaxStages = 16;
+
+// stage_bytes: size of one ring slot (>= every chunk's n).  n_stages in [2, kBulkMaxStages].
+__global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ KernelParams p, uint32_t stage_bytes,
+                                                      uint32_t n_stages) {
+  extern __shared__ __align__(128) char ring[];
+  __shared__ __align__(8) uint64_t full[kBulkMaxStages];
+  if (threadIdx.x != 0) return;                       // one thread drives the TMA unit
+  for (uint32_t i = 0; i < n_stages; ++i) mbar_init(&full[i], 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  const uint64_t pol = policy_evict_first();
+
+  const uint32_t first = blockIdx.x, stride = gridDim.x;
+  const uint32_t n_my = first < p.n_tiles ? (p.n_tiles - first + stride - 1) / stride : 0;
+  const uint32_t ahead = n_stages - 1;                // loads kept in flight
+
+  __shared__ char* dptr[kBulkMaxStages];              // where each slot's bytes go
+  __shared__ uint32_t nbytes[kBulkMaxStages];
+
+  auto issue_load = [&](uint32_t k) {
+    uint32_t plane, ci;
+    decode_tile(p, first + k * stride, plane, ci);
+    const Chunk c = load_chunk(p.chunks + ci);
+    const char* s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
+    const uint32_t slot = k % n_stages;
+    dptr[slot] = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    nbytes[slot] = c.n;
+    mbar_expect_tx(&full[slot], c.n);
+    bulk_g2s(ring + (size_t)slot * stage_bytes, s, c.n, &full[slot], pol);
+  };
+
+  for (uint32_t k = 0; k < ahead && k < n_my; ++k) issue_load(k);
+  for (uint32_t k = 0; k < n_my; ++k) {
+    const uint32_t slot = k % n_stages;
+    mbar_wait(&full[slot], (k / n_stages) & 1);       // tile k has landed in its slot
+    bulk_s2g(dptr[slot], ring + (size_t)slot * stage_bytes, nbytes[slot], pol);
+    bulk_commit();
+    if (k + ahead < n_my) {
+      // slot of tile k+ahead == slot of tile k-1: its store must have finished READING smem
+      bulk_wait_read<1>();
+      issue_load(k + ahead);
+    }
+  }
+  bulk_wait_all();
+}
+
+// ------------------------------------------------------------------------------------------------
+// launcher
+// ------------------------------------------------------------------------------------------------
+template <int VEC, int UNROLL>
+static cudaError_t launch_ldst(Mode mode, const KernelParams& kp, const LaunchShape& ls, int hint, cudaStream_t st) {
+  const dim3 grid(ls.grid), block(ls.threads);
+#define FK_LAUNCH(KERNEL)                                                              \
+  switch (hint) {                                                                      \
+    case 0: KERNEL<VEC, UNROLL, 0><<<grid, block, 0, st>>>(kp); break;                 \
+    case 1: KERNEL<VEC, UNROLL, 1><<<grid, block, 0, st>>>(kp); break;                 \
+    default: KERNEL<VEC, UNROLL, 2><<<grid, block, 0, st>>>(kp); break;                \
+  }
+  if (mode == MODE_SPAN) { FK_LAUNCH(fk_span_ldst) } else { FK_LAUNCH(fk_rows_ldst) }
+#undef FK_LAUNCH
+  return cudaGetLastError();
+}
+
+uint32_t bulk_max_smem() {
+  int dev = 0, v = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return 0;
+  return (uint32_t)v;
+}
+
+int launch_copy(Mode mode, const KernelParams& kp, const LaunchShape& ls, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_SPAN) {
+    const uint32_t smem = ls.n_stages * ls.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(fk_span_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    fk_span_bulk<<<dim3(ls.grid), dim3(32), smem, st>>>(kp, ls.stage_bytes, ls.n_stages);
+    return (int)cudaGetLastError();
+  }
+  if (ls.vec_bytes == 32) return (int)launch_ldst<32, 4>(mode, kp, ls, (int)ls.hint, st);
+  return (int)launch_ldst<16, 8>(mode, kp, ls, (int)ls.hint, st);
+}
+
+}  // namespace flowkv

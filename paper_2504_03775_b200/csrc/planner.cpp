@@ -1,0 +1,219 @@
+// planner.cpp — host side of the FlowKV transfer path: validation (a1), bidirectional segment
+// alignment (a2; §3.3, Fig. 5) and the tile schedule (a3).  Pure integer code.
+//
+// Alignment rule (readings A6-A10): a request is walked left to right in pieces that
+// never cross a block boundary on either side.  A piece extends the open segment iff its first
+// token SLOT (block_id*block_size + offset_in_block) directly follows the segment's last slot on
+// the src side AND on the dst side; otherwise it opens a new segment.  Segments never span two
+// requests.  The partition is the unique coarsest one whose parts are memory-contiguous on both
+// sides in token-slot space, i.e. "N contiguous block IDs present on both sides".
+#include <algorithm>
+#include <cstdio>
+
+#include "flowkv_internal.h"
+
+namespace flowkv {
+
+static bool is_pow2(uint32_t x) { return x && !(x & (x - 1)); }
+
+bool pool_is_span_capable(const flowkv_pool& p, const Geometry& g) {
+  return p.stride_bytes[FLOWKV_S_HEAD] == (int64_t)g.row_bytes &&
+         p.stride_bytes[FLOWKV_S_TOKEN] == (int64_t)g.tok_bytes &&
+         p.stride_bytes[FLOWKV_S_BLOCK] == (int64_t)p.block_size * g.tok_bytes;
+}
+
+flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string& err) {
+  char buf[256];
+  auto fail = [&](flowkv_status s, const char* msg) {
+    snprintf(buf, sizeof buf, "%s pool: %s", which, msg);
+    err = buf;
+    return s;
+  };
+  if (!p->base) return fail(FLOWKV_ERR_INVALID_ARG, "base is NULL");
+  if (!p->num_layers || !p->num_kv_heads || !p->head_dim || !p->elem_bytes || !p->num_blocks)
+    return fail(FLOWKV_ERR_INVALID_ARG, "a shape field is zero");
+  if (!is_pow2(p->block_size)) return fail(FLOWKV_ERR_UNSUPPORTED, "block_size must be a power of two");
+  if (p->layout > FLOWKV_LAYOUT_STRIDED) return fail(FLOWKV_ERR_INVALID_ARG, "unknown layout");
+  const uint64_t row = (uint64_t)p->head_dim * p->elem_bytes;
+  if (row % 16) return fail(FLOWKV_ERR_ALIGN, "head_dim*elem_bytes is not a multiple of 16 bytes");
+  if (row > (1u << 20)) return fail(FLOWKV_ERR_UNSUPPORTED, "row larger than 1 MiB");
+  if ((uintptr_t)p->base % 16) return fail(FLOWKV_ERR_ALIGN, "base is not 16-byte aligned");
+  for (int i = 0; i < 5; ++i) {
+    if (p->stride_bytes[i] <= 0) return fail(FLOWKV_ERR_INVALID_ARG, "a stride is <= 0 (call flowkv_pool_strides)");
+    if (p->stride_bytes[i] % 16) return fail(FLOWKV_ERR_ALIGN, "a stride is not a multiple of 16 bytes");
+  }
+  return FLOWKV_OK;
+}
+
+static uint32_t ceil_div(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a + b - 1) / b); }
+
+flowkv_status validate_requests(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
+                                uint32_t n_reqs, uint32_t flags, std::string& err) {
+  char buf[256];
+  std::vector<uint8_t> seen;
+  if (dst && (flags & FLOWKV_CHECK_DST_ALIAS)) seen.assign(dst->num_blocks, 0);
+  for (uint32_t r = 0; r < n_reqs; ++r) {
+    const flowkv_request& q = reqs[r];
+    if (src) {
+      const uint32_t need = ceil_div(q.num_tokens, src->block_size);
+      if (q.n_src_blocks != need) {
+        snprintf(buf, sizeof buf, "request %u: n_src_blocks=%u but ceil(%u/%u)=%u", r, q.n_src_blocks,
+                 q.num_tokens, src->block_size, need);
+        err = buf;
+        return FLOWKV_ERR_TABLE_LEN;
+      }
+      if (need && !q.src_blocks) { err = "src_blocks is NULL"; return FLOWKV_ERR_INVALID_ARG; }
+      for (uint32_t i = 0; i < need; ++i)
+        if (q.src_blocks[i] < 0 || (uint32_t)q.src_blocks[i] >= src->num_blocks) {
+          snprintf(buf, sizeof buf, "request %u: src block id %d at %u outside [0,%u)", r, q.src_blocks[i], i,
+                   src->num_blocks);
+          err = buf;
+          return FLOWKV_ERR_BLOCK_OOB;
+        }
+    }
+    if (dst) {
+      const uint32_t need = ceil_div(q.num_tokens, dst->block_size);
+      if (q.n_dst_blocks != need) {
+        snprintf(buf, sizeof buf, "request %u: n_dst_blocks=%u but ceil(%u/%u)=%u", r, q.n_dst_blocks,
+                 q.num_tokens, dst->block_size, need);
+        err = buf;
+        return FLOWKV_ERR_TABLE_LEN;
+      }
+      if (need && !q.dst_blocks) { err = "dst_blocks is NULL"; return FLOWKV_ERR_INVALID_ARG; }
+      for (uint32_t i = 0; i < need; ++i) {
+        const int32_t b = q.dst_blocks[i];
+        if (b < 0 || (uint32_t)b >= dst->num_blocks) {
+          snprintf(buf, sizeof buf, "request %u: dst block id %d at %u outside [0,%u)", r, b, i, dst->num_blocks);
+          err = buf;
+          return FLOWKV_ERR_BLOCK_OOB;
+        }
+        if (!seen.empty()) {
+          if (seen[b]) {
+            snprintf(buf, sizeof buf, "request %u: dst block id %d is named twice in the batch", r, b);
+            err = buf;
+            return FLOWKV_ERR_DST_ALIAS;
+          }
+          seen[b] = 1;
+        }
+      }
+    }
+  }
+  return FLOWKV_OK;
+}
+
+void align_segments(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
+                    uint32_t n_reqs, std::vector<flowkv_segment>& out) {
+  out.clear();
+  const uint32_t bs_s = src ? src->block_size : 0, bs_d = dst ? dst->block_size : 0;
+  uint64_t tok_base = 0;   // staging_tok_off of the current request
+  for (uint32_t r = 0; r < n_reqs; ++r) {
+    const uint32_t T = reqs[r].num_tokens;
+    const int32_t* S = reqs[r].src_blocks;
+    const int32_t* D = reqs[r].dst_blocks;
+    bool open = false;
+    int64_t next_s = 0, next_d = 0;          // slot that would continue the open segment
+    uint32_t t = 0;
+    while (t < T) {
+      uint32_t piece = T - t;
+      int64_t slot_s = 0, slot_d = 0;
+      uint32_t sb = 0, so = 0, db = 0, dof = 0;
+      if (src) {
+        so = t & (bs_s - 1);
+        sb = (uint32_t)S[t / bs_s];
+        slot_s = (int64_t)sb * bs_s + so;
+        piece = std::min(piece, bs_s - so);
+      }
+      if (dst) {
+        dof = t & (bs_d - 1);
+        db = (uint32_t)D[t / bs_d];
+        slot_d = (int64_t)db * bs_d + dof;
+        piece = std::min(piece, bs_d - dof);
+      }
+      const bool cont = open && (!src || slot_s == next_s) && (!dst || slot_d == next_d);
+      if (cont) {
+        out.back().n_tokens += piece;
+      } else {
+        flowkv_segment sg{};
+        sg.request = r;
+        sg.first_token = t;
+        sg.n_tokens = piece;
+        sg.src_block = sb; sg.src_tok_off = so;
+        sg.dst_block = db; sg.dst_tok_off = dof;
+        sg.staging_tok_off = tok_base;
+        out.push_back(sg);
+        open = true;
+      }
+      next_s = slot_s + piece;
+      next_d = slot_d + piece;
+      t += piece;
+    }
+    tok_base += T;
+  }
+}
+
+// Byte offset of token slot (block, off) of a pool, plane offset excluded.
+static inline int64_t pool_off(const flowkv_pool* p, uint32_t block, uint32_t off) {
+  return (int64_t)block * p->stride_bytes[FLOWKV_S_BLOCK] + (int64_t)off * p->stride_bytes[FLOWKV_S_TOKEN];
+}
+
+void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geometry& g,
+                    const flowkv_request* reqs, const std::vector<flowkv_segment>& segs,
+                    uint32_t tile_bytes, uint32_t /*vec_bytes*/, Schedule& out) {
+  out.chunks.clear();
+  const bool span = (!src || pool_is_span_capable(*src, g)) && (!dst || pool_is_span_capable(*dst, g));
+  out.mode = span ? MODE_SPAN : MODE_ROWS;
+  const uint32_t tile_tokens = std::max<uint32_t>(1, tile_bytes / g.tok_bytes);
+  for (const flowkv_segment& sg : segs) {
+    const uint32_t T = reqs[sg.request].num_tokens;
+    // dense side: request base + token offset; the plane term (p*T*tok_bytes) is added by the kernel
+    const int64_t dense0 = (int64_t)(sg.staging_tok_off * g.bytes_per_token);
+    if (span) {
+      // the whole segment is one contiguous byte range per plane on both sides
+      const int64_t s0 = src ? pool_off(src, sg.src_block, sg.src_tok_off) : dense0 + (int64_t)sg.first_token * g.tok_bytes;
+      const int64_t d0 = dst ? pool_off(dst, sg.dst_block, sg.dst_tok_off) : dense0 + (int64_t)sg.first_token * g.tok_bytes;
+      uint32_t done = 0;
+      while (done < sg.n_tokens) {
+        const uint32_t n = std::min(tile_tokens, sg.n_tokens - done);
+        Chunk c{};
+        c.src_off = s0 + (int64_t)done * g.tok_bytes;
+        c.dst_off = d0 + (int64_t)done * g.tok_bytes;
+        c.n = n * g.tok_bytes;
+        c.req_tokens = T;
+        c.request = sg.request;
+        out.chunks.push_back(c);
+        done += n;
+      }
+    } else {
+      // rows mode: a chunk stays inside one block on each paged side
+      const int32_t* S = reqs[sg.request].src_blocks;
+      const int32_t* D = reqs[sg.request].dst_blocks;
+      uint32_t t = sg.first_token;
+      const uint32_t end = sg.first_token + sg.n_tokens;
+      while (t < end) {
+        uint32_t n = std::min(tile_tokens, end - t);
+        Chunk c{};
+        if (src) {
+          const uint32_t so = t & (src->block_size - 1);
+          n = std::min(n, src->block_size - so);
+          c.src_off = pool_off(src, (uint32_t)S[t / src->block_size], so);
+        } else {
+          c.src_off = dense0 + (int64_t)t * g.tok_bytes;
+        }
+        if (dst) {
+          const uint32_t dof = t & (dst->block_size - 1);
+          n = std::min(n, dst->block_size - dof);
+          c.dst_off = pool_off(dst, (uint32_t)D[t / dst->block_size], dof);
+        } else {
+          c.dst_off = dense0 + (int64_t)t * g.tok_bytes;
+        }
+        c.n = n;
+        c.req_tokens = T;
+        c.request = sg.request;
+        out.chunks.push_back(c);
+        t += n;
+      }
+    }
+  }
+}
+
+}  // namespace flowkv

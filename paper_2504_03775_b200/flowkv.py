@@ -1,0 +1,301 @@
+"""ctypes binding of ``libflowkv.so`` — same names as include/flowkv.h, argument marshalling only.
+
+Every step of the path (planning, scheduling, the copy) runs inside the C/CUDA library; this module
+turns Python objects into the structs of the header and raises :class:`FlowKVError` on a non-zero
+status.  There is no fallback of any kind: if the library is missing, importing this module fails.
+
+Pointers are plain integers (``tensor.data_ptr()``, ``stream.cuda_stream``); torch is not imported
+here.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libflowkv.so")
+
+# ---- enums / flags of the header -------------------------------------------------------------
+FLOWKV_OK = 0
+(FLOWKV_ERR_INVALID_ARG, FLOWKV_ERR_BLOCK_OOB, FLOWKV_ERR_TABLE_LEN, FLOWKV_ERR_DST_ALIAS, FLOWKV_ERR_ALIGN,
+ FLOWKV_ERR_SHAPE_MISMATCH, FLOWKV_ERR_UNSUPPORTED, FLOWKV_ERR_STAGING_TOO_SMALL, FLOWKV_ERR_NOMEM,
+ FLOWKV_ERR_CUDA) = range(1, 11)
+FLOWKV_LAYOUT_LKBTHD, FLOWKV_LAYOUT_BLKHTD, FLOWKV_LAYOUT_STRIDED = 0, 1, 2
+FLOWKV_CHECK_DST_ALIAS, FLOWKV_PLAN_NO_TRANSFER, FLOWKV_PLAN_NO_PACK, FLOWKV_PLAN_NO_UNPACK = 1, 2, 4, 8
+FLOWKV_VARIANT_AUTO, FLOWKV_VARIANT_LDST, FLOWKV_VARIANT_BULK = 0, 1, 2
+LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "strided": FLOWKV_LAYOUT_STRIDED}
+
+EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
+           "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
+           "flowkv_launch_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise"]
+
+
+class flowkv_pool(C.Structure):
+    _fields_ = [("base", C.c_void_p), ("num_layers", C.c_uint32), ("num_kv_heads", C.c_uint32),
+                ("head_dim", C.c_uint32), ("elem_bytes", C.c_uint32), ("num_blocks", C.c_uint32),
+                ("block_size", C.c_uint32), ("layout", C.c_uint32), ("_reserved", C.c_uint32),
+                ("stride_bytes", C.c_int64 * 5)]
+
+
+class flowkv_request(C.Structure):
+    _fields_ = [("num_tokens", C.c_uint32), ("n_src_blocks", C.c_uint32), ("src_blocks", C.c_void_p),
+                ("dst_blocks", C.c_void_p), ("n_dst_blocks", C.c_uint32), ("_reserved", C.c_uint32)]
+
+
+class flowkv_segment(C.Structure):
+    _fields_ = [("request", C.c_uint32), ("first_token", C.c_uint32), ("n_tokens", C.c_uint32),
+                ("src_block", C.c_uint32), ("src_tok_off", C.c_uint32), ("dst_block", C.c_uint32),
+                ("dst_tok_off", C.c_uint32), ("_reserved", C.c_uint32), ("staging_tok_off", C.c_uint64)]
+
+
+class flowkv_tuning(C.Structure):
+    _fields_ = [("tile_bytes", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("max_sms", C.c_uint32),
+                ("threads", C.c_uint32), ("group_threads", C.c_uint32), ("variant", C.c_uint32),
+                ("tile_order", C.c_uint32), ("cache_hint", C.c_uint32), ("stages", C.c_uint32),
+                ("_reserved", C.c_uint32 * 3)]
+
+
+class flowkv_plan_stats(C.Structure):
+    _fields_ = [("n_requests", C.c_uint64), ("n_segments", C.c_uint64), ("total_tokens", C.c_uint64),
+                ("payload_bytes", C.c_uint64), ("staging_bytes", C.c_uint64), ("n_chunks_transfer", C.c_uint64),
+                ("n_chunks_pack", C.c_uint64), ("n_chunks_unpack", C.c_uint64), ("plan_device_bytes", C.c_uint64),
+                ("n_planes", C.c_uint32), ("mode_transfer", C.c_uint32), ("mode_pack", C.c_uint32),
+                ("mode_unpack", C.c_uint32), ("grid", C.c_uint32), ("threads", C.c_uint32),
+                ("group_threads", C.c_uint32), ("tile_bytes", C.c_uint32), ("variant", C.c_uint32),
+                ("vec_bytes", C.c_uint32), ("tile_order", C.c_uint32), ("cache_hint", C.c_uint32),
+                ("stages", C.c_uint32), ("smem_bytes", C.c_uint32), ("num_sms", C.c_uint32), ("_reserved", C.c_uint32)]
+
+    def as_dict(self) -> dict:
+        return {n: int(getattr(self, n)) for n, _ in self._fields_ if not n.startswith("_")}
+
+
+class FlowKVError(RuntimeError):
+    def __init__(self, status: int, name: str, text: str):
+        super().__init__(f"{name}: {text}")
+        self.status = status
+        self.name = name
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2504_03775_b200.build` "
+                          "(there is no fallback implementation)")
+    lib = C.CDLL(LIB_PATH)
+    P = C.POINTER
+    lib.flowkv_pool_strides.argtypes = [P(flowkv_pool)]
+    lib.flowkv_plan.argtypes = [P(flowkv_pool), P(flowkv_pool), P(flowkv_request), C.c_uint32, C.c_uint32,
+                                P(flowkv_tuning), C.c_void_p, P(C.c_void_p)]
+    lib.flowkv_plan_host.argtypes = [P(flowkv_pool), P(flowkv_pool), P(flowkv_request), C.c_uint32, C.c_uint32,
+                                     P(flowkv_tuning), P(C.c_void_p)]
+    lib.flowkv_plan_info.argtypes = [C.c_void_p, P(flowkv_plan_stats), P(P(flowkv_segment))]
+    lib.flowkv_transfer.argtypes = [C.c_void_p, C.c_void_p]
+    lib.flowkv_pack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+    lib.flowkv_unpack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+    lib.flowkv_plan_destroy.argtypes = [C.c_void_p]
+    lib.flowkv_plan_destroy.restype = None
+    lib.flowkv_status_string.argtypes = [C.c_int]
+    lib.flowkv_status_string.restype = C.c_char_p
+    lib.flowkv_last_error.argtypes = []
+    lib.flowkv_last_error.restype = C.c_char_p
+    lib.flowkv_launch_count.argtypes = []
+    lib.flowkv_launch_count.restype = C.c_uint64
+    lib.flowkv_baseline_blockwise.argtypes = [P(flowkv_pool), P(flowkv_pool), P(flowkv_request), C.c_uint32,
+                                              C.c_void_p, P(C.c_uint64)]
+    lib.flowkv_baseline_segmentwise.argtypes = [C.c_void_p, C.c_void_p, P(C.c_uint64)]
+    for n in EXPORTS:
+        if n not in ("flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error", "flowkv_launch_count"):
+            getattr(lib, n).restype = C.c_int
+    return lib
+
+
+_lib = _load()
+
+
+def _check(status: int) -> None:
+    if status != FLOWKV_OK:
+        raise FlowKVError(status, _lib.flowkv_status_string(status).decode(), _lib.flowkv_last_error().decode())
+
+
+def flowkv_status_string(status: int) -> str:
+    return _lib.flowkv_status_string(status).decode()
+
+
+def flowkv_last_error() -> str:
+    return _lib.flowkv_last_error().decode()
+
+
+def flowkv_launch_count() -> int:
+    return int(_lib.flowkv_launch_count())
+
+
+# ---- marshalling helpers ----------------------------------------------------------------------
+def make_pool(base: int, num_layers: int, num_kv_heads: int, head_dim: int, elem_bytes: int, num_blocks: int,
+              block_size: int, layout="lkbthd", strides: Optional[Sequence[int]] = None) -> flowkv_pool:
+    """Describe a pool.  ``strides`` (layer, kv, block, token, head; bytes) only for layout 'strided'."""
+    p = flowkv_pool()
+    p.base = base
+    p.num_layers, p.num_kv_heads, p.head_dim, p.elem_bytes = num_layers, num_kv_heads, head_dim, elem_bytes
+    p.num_blocks, p.block_size = num_blocks, block_size
+    p.layout = LAYOUTS[layout] if isinstance(layout, str) else int(layout)
+    if strides is not None:
+        for i, s in enumerate(strides):
+            p.stride_bytes[i] = int(s)
+    flowkv_pool_strides(p)
+    return p
+
+
+def flowkv_pool_strides(pool: flowkv_pool) -> flowkv_pool:
+    _check(_lib.flowkv_pool_strides(C.byref(pool)))
+    return pool
+
+
+def pool_bytes(pool: flowkv_pool) -> int:
+    """Bytes from the base to one past the last addressable element."""
+    s = pool.stride_bytes
+    return ((pool.num_layers - 1) * s[0] + s[1] + (pool.num_blocks - 1) * s[2] + (pool.block_size - 1) * s[3]
+            + (pool.num_kv_heads - 1) * s[4] + pool.head_dim * pool.elem_bytes)
+
+
+@dataclass
+class Request:
+    num_tokens: int
+    src_blocks: Optional[np.ndarray] = None
+    dst_blocks: Optional[np.ndarray] = None
+
+
+def _marshal_requests(requests: Sequence) -> tuple:
+    n = len(requests)
+    arr = (flowkv_request * max(n, 1))()
+    keep: List[np.ndarray] = []
+    for i, r in enumerate(requests):
+        arr[i].num_tokens = int(r.num_tokens)
+        for side in ("src", "dst"):
+            tab = getattr(r, side + "_blocks", None)
+            if tab is None:
+                setattr(arr[i], side + "_blocks", None)
+                setattr(arr[i], f"n_{side}_blocks", 0)
+            else:
+                a = np.ascontiguousarray(np.asarray(tab, dtype=np.int32))
+                keep.append(a)
+                setattr(arr[i], side + "_blocks", a.ctypes.data if a.size else None)
+                setattr(arr[i], f"n_{side}_blocks", a.size)
+    return arr, n, keep
+
+
+class Plan:
+    """Owner of a ``flowkv_plan_t*``; destroyed with the object (or by :meth:`destroy`)."""
+
+    def __init__(self, handle: int):
+        self._h = C.c_void_p(handle)
+
+    @property
+    def handle(self) -> C.c_void_p:
+        if not self._h:
+            raise ValueError("plan was destroyed")
+        return self._h
+
+    def info(self):
+        st = flowkv_plan_stats()
+        segp = C.POINTER(flowkv_segment)()
+        _check(_lib.flowkv_plan_info(self.handle, C.byref(st), C.byref(segp)))
+        return st, segp
+
+    @property
+    def stats(self) -> dict:
+        return self.info()[0].as_dict()
+
+    @property
+    def segments(self) -> List[dict]:
+        st, segp = self.info()
+        names = [n for n, _ in flowkv_segment._fields_ if not n.startswith("_")]
+        return [{k: int(getattr(segp[i], k)) for k in names} for i in range(st.n_segments)]
+
+    def transfer(self, stream: int = 0) -> None:
+        flowkv_transfer(self, stream)
+
+    def pack(self, staging: int, nbytes: int, stream: int = 0) -> None:
+        flowkv_pack(self, staging, nbytes, stream)
+
+    def unpack(self, staging: int, nbytes: int, stream: int = 0) -> None:
+        flowkv_unpack(self, staging, nbytes, stream)
+
+    def destroy(self) -> None:
+        if self._h:
+            _lib.flowkv_plan_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def _tuning(tuning) -> Optional[flowkv_tuning]:
+    if tuning is None:
+        return None
+    if isinstance(tuning, flowkv_tuning):
+        return tuning
+    t = flowkv_tuning()
+    for k, v in dict(tuning).items():
+        if isinstance(v, str):
+            v = {"ldst": FLOWKV_VARIANT_LDST, "bulk": FLOWKV_VARIANT_BULK, "auto": 0}[v]
+        setattr(t, k, int(v))
+    return t
+
+
+def flowkv_plan(src: Optional[flowkv_pool], dst: Optional[flowkv_pool], requests: Sequence, flags: int = 0,
+                tuning=None, stream: int = 0) -> Plan:
+    arr, n, keep = _marshal_requests(requests)
+    out = C.c_void_p()
+    t = _tuning(tuning)
+    _check(_lib.flowkv_plan(C.byref(src) if src is not None else None, C.byref(dst) if dst is not None else None,
+                            arr, n, flags, C.byref(t) if t is not None else None, C.c_void_p(stream), C.byref(out)))
+    del keep
+    return Plan(out.value)
+
+
+def flowkv_plan_host(src: Optional[flowkv_pool], dst: Optional[flowkv_pool], requests: Sequence, flags: int = 0,
+                     tuning=None) -> Plan:
+    arr, n, keep = _marshal_requests(requests)
+    out = C.c_void_p()
+    t = _tuning(tuning)
+    _check(_lib.flowkv_plan_host(C.byref(src) if src is not None else None,
+                                 C.byref(dst) if dst is not None else None, arr, n, flags,
+                                 C.byref(t) if t is not None else None, C.byref(out)))
+    del keep
+    return Plan(out.value)
+
+
+def flowkv_transfer(plan: Plan, stream: int = 0) -> None:
+    _check(_lib.flowkv_transfer(plan.handle, C.c_void_p(stream)))
+
+
+def flowkv_pack(plan: Plan, staging: int, nbytes: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_pack(plan.handle, C.c_void_p(staging), nbytes, C.c_void_p(stream)))
+
+
+def flowkv_unpack(plan: Plan, staging: int, nbytes: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_unpack(plan.handle, C.c_void_p(staging), nbytes, C.c_void_p(stream)))
+
+
+def flowkv_plan_destroy(plan: Plan) -> None:
+    plan.destroy()
+
+
+def flowkv_baseline_blockwise(src: flowkv_pool, dst: flowkv_pool, requests: Sequence, stream: int = 0) -> int:
+    arr, n, keep = _marshal_requests(requests)
+    calls = C.c_uint64()
+    _check(_lib.flowkv_baseline_blockwise(C.byref(src), C.byref(dst), arr, n, C.c_void_p(stream), C.byref(calls)))
+    del keep
+    return int(calls.value)
+
+
+def flowkv_baseline_segmentwise(plan: Plan, stream: int = 0) -> int:
+    calls = C.c_uint64()
+    _check(_lib.flowkv_baseline_segmentwise(plan.handle, C.c_void_p(stream), C.byref(calls)))
+    return int(calls.value)

@@ -1,0 +1,81 @@
+"""Device memory for synthetic pools: torch is used ONLY to allocate, fill and read back buffers.
+
+Nothing here copies KV data between pools — that is the C/CUDA library's job (flowkv.py).
+Shared by the GPU tests and bench.py.  Imports neither ``oracle`` nor any oracle output.
+"""
+from __future__ import annotations
+
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import flowkv as F
+from . import synth
+
+SENTINEL_BYTE = 0xA5
+
+
+def pool_numel_bytes(spec: synth.PoolSpec, shape: synth.Shape) -> int:
+    return spec.bytes(shape)
+
+
+def describe(spec: synth.PoolSpec, shape: synth.Shape, base_ptr: int) -> F.flowkv_pool:
+    return F.make_pool(base_ptr, shape.num_layers, shape.num_kv_heads, shape.head_dim, shape.elem_bytes,
+                       spec.num_blocks, spec.block_size, spec.layout)
+
+
+def alloc_bytes(nbytes: int, device="cuda:0") -> torch.Tensor:
+    """Flat uint8 buffer (torch's allocator returns >= 256-byte aligned pointers)."""
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
+
+
+def fill_values(buf: torch.Tensor, dist: str, dtype: str, seed: int, chunk_bytes: int = 1 << 30) -> None:
+    """Seeded values with the distribution BASELINE.json names (irrelevant to a copy, kept anyway):
+    'normal' N(0,1), 'uniform' U[-1,1], 'bits' uniformly random 16-bit patterns (NaNs, Infs, -0,
+    denormals included).  Filled in place, chunk by chunk, so no pool-sized temporary exists."""
+    gen = torch.Generator(device=buf.device)
+    gen.manual_seed(seed)
+    tdt = {"bf16": torch.bfloat16, "fp16": torch.float16}[dtype]
+    n = buf.numel()
+    for off in range(0, n, chunk_bytes):
+        part = buf[off:min(off + chunk_bytes, n)]
+        if dist == "bits":
+            part.view(torch.int16).random_(-32768, 32768, generator=gen)
+        elif dist == "normal":
+            part.view(tdt).normal_(0.0, 1.0, generator=gen)
+        elif dist == "uniform":
+            part.view(tdt).uniform_(-1.0, 1.0, generator=gen)
+        else:
+            raise ValueError(dist)
+
+
+def fill_sentinel(buf: torch.Tensor) -> None:
+    buf.fill_(SENTINEL_BYTE)
+
+
+def requests_of(w: synth.Workload, src: bool = True, dst: bool = True) -> Sequence[F.Request]:
+    return [F.Request(r.num_tokens, r.src_blocks if src else None, r.dst_blocks if dst else None) for r in w.requests]
+
+
+class DevicePools:
+    """src + dst pools of a workload on one device, described for the library."""
+
+    def __init__(self, w: synth.Workload, device="cuda:0", fill: Optional[str] = None, sentinel_dst: bool = True):
+        self.w = w
+        self.device = torch.device(device)
+        self.src_buf = alloc_bytes(w.src.bytes(w.shape), device)
+        self.dst_buf = alloc_bytes(w.dst.bytes(w.shape), device)
+        fill_values(self.src_buf, fill or w.value_dist, w.shape.dtype, w.seed)
+        if sentinel_dst:
+            fill_sentinel(self.dst_buf)
+        self.src = describe(w.src, w.shape, self.src_buf.data_ptr())
+        self.dst = describe(w.dst, w.shape, self.dst_buf.data_ptr())
+        self.requests = requests_of(w)
+
+    def plan(self, flags: int = 0, tuning=None, stream: int = 0) -> F.Plan:
+        return F.flowkv_plan(self.src, self.dst, self.requests, flags, tuning, stream)
+
+
+def to_numpy(buf: torch.Tensor) -> np.ndarray:
+    return buf.cpu().numpy()

@@ -10,6 +10,9 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a real B200 (run with -m gpu on the GPU box)")
+    # the C-ABI library is built in-tree (the .so is git-ignored); nvcc cross-compiles without a GPU
+    from paper_2504_03775_b200 import build as _build
+    _build.build()
 
 
 def pytest_collection_modifyitems(config, items):

@@ -1,0 +1,288 @@
+"""`-m gpu` parity: the CUDA path (through the C-ABI) against the CPU oracle, bit for bit.
+
+Sizes: small enough for the token-by-token oracle to finish in seconds, yet spanning many tiles and
+ragged tails.  Full-size configs are in test_gpu_fullsize.py."""
+import itertools
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2504_03775_b200 import flowkv as F
+from paper_2504_03775_b200 import pools as P
+from paper_2504_03775_b200 import synth
+from tests import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+TUNINGS = [
+    None,
+    {"variant": "ldst", "cache_hint": 1, "group_threads": 32, "threads": 128, "tile_bytes": 4096},
+    {"variant": "ldst", "cache_hint": 2, "group_threads": 64, "threads": 256, "tile_bytes": 8192, "tile_order": 2},
+    {"variant": "ldst", "cache_hint": 3, "threads": 512, "tile_bytes": 65536, "ctas_per_sm": 2},
+    {"variant": "bulk", "tile_bytes": 16384, "stages": 4},
+    {"variant": "bulk", "tile_bytes": 4096, "stages": 16, "ctas_per_sm": 2, "tile_order": 2},
+    {"variant": "ldst", "max_sms": 3, "ctas_per_sm": 1},
+]
+
+
+@pytest.mark.parametrize("tuning", TUNINGS)
+def test_cfg1_tiny_every_variant(tuning):
+    """BASELINE.json configs[0]: 1000 tokens, permutation src table (63 segments), ragged last block."""
+    w = synth.config1_tiny()
+    dp, plan, _ = G.run_transfer_and_check(w, tuning)
+    assert plan.stats["n_segments"] == 63
+
+
+@pytest.mark.parametrize("tuning", [None, {"variant": "bulk"}])
+def test_cfg2_shape_two_layers(tuning):
+    """configs[1] with L=2: same tables (832 blocks, ~208 runs over a 16,384-block pool => 64-bit offsets
+    inside one plane up to 512 MiB), 2 GiB src pool."""
+    w = synth.config2_llama8b_13k(num_layers=2)
+    G.run_transfer_and_check(w, tuning)
+
+
+@pytest.mark.parametrize("tuning", [None, {"variant": "bulk", "tile_bytes": 32768}])
+def test_cfg3_batched_small(tuning):
+    """configs[2] scaled: 6 requests, L=2, src runs of mean 2, dst runs of mean 16, one batch, one launch."""
+    w = synth.config3_batched(n_requests=6, num_layers=2)
+    G.run_transfer_and_check(w, tuning)
+
+
+@pytest.mark.parametrize("tuning", [None, {"cache_hint": 1, "group_threads": 32, "tile_bytes": 8192},
+                                    {"tile_bytes": 131072, "threads": 512}])
+def test_cfg4_hetero_layout_and_block_size(tuning):
+    """configs[3] scaled: src BS16 LKBTHD -> dst BS64 BLKHTD, 3 requests, L=2; partial 64-token dst blocks."""
+    w = synth.config4_hetero(n_requests=3, num_layers=2)
+    assert any(r.num_tokens % 64 for r in w.requests)
+    G.run_transfer_and_check(w, tuning)
+
+
+@pytest.mark.parametrize("src_layout,dst_layout,bs_s,bs_d", [
+    ("blkhtd", "lkbthd", 64, 16), ("blkhtd", "blkhtd", 16, 16), ("blkhtd", "blkhtd", 8, 32),
+    ("lkbthd", "lkbthd", 32, 8), ("lkbthd", "blkhtd", 16, 16),
+])
+def test_other_layout_pairs(src_layout, dst_layout, bs_s, bs_d):
+    lengths = [777, 64, 1, 300]
+    w = synth.make_workload("pairs", 11, synth.Shape(3, 4, 64, "bf16"), lengths,
+                            src_layout, bs_s, ("geometric", 3.0), None, dst_layout, bs_d, ("geometric", 2.0), None)
+    G.run_transfer_and_check(w, None, fill="bits")
+
+
+@pytest.mark.parametrize("heads,dim", [(3, 40), (5, 8), (1, 72), (7, 24)])
+def test_non_power_of_two_heads_and_16_byte_rows(heads, dim):
+    """Rows of 16/48/80/144 bytes and odd head counts: the 128-bit path and the generic div/mod path."""
+    w = synth.make_workload("odd", 12, synth.Shape(2, heads, dim, "fp16"), [333, 17],
+                            "lkbthd", 4, ("geometric", 2.0), None, "blkhtd", 8, ("contiguous",), None)
+    G.run_transfer_and_check(w, None, fill="bits")
+    w2 = synth.make_workload("odd2", 13, synth.Shape(2, heads, dim, "fp16"), [333, 17],
+                             "lkbthd", 4, ("geometric", 2.0), None, "lkbthd", 4, ("geometric", 5.0), None)
+    G.run_transfer_and_check(w2, None, fill="bits")
+    G.run_transfer_and_check(w2, {"variant": "bulk"}, fill="bits")
+
+
+def test_all_65536_bit_patterns_survive():
+    """NaN payloads, +-Inf, -0, denormals: elements move as raw 16-bit words."""
+    w = synth.make_workload("bits", 14, synth.Shape(1, 2, 64, "fp16"), [512], "lkbthd", 16, ("fixed", 1), 64,
+                            "blkhtd", 32, ("contiguous",), None)
+    dp = P.DevicePools(w)
+    pat = torch.arange(65536, dtype=torch.int32, device="cuda").to(torch.int16)   # 65,536 distinct patterns
+    nrep = dp.src_buf.numel() // 2 // 65536
+    assert nrep >= 1
+    dp.src_buf.view(torch.int16)[: nrep * 65536] = pat.repeat(nrep)
+    src_np = P.to_numpy(dp.src_buf)
+    plan = dp.plan()
+    plan.transfer()
+    torch.cuda.synchronize()
+    exp = G.oracle_transfer(w, src_np)
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "bit patterns")
+
+
+def test_brute_force_tiny_pools():
+    """Every injective src table x a set of dst tables x every T in the last block, BS in {2,4}, incl.
+    BS_s != BS_d and both layouts (SURVEY §8c 'everything, exhaustively')."""
+    L, H, D = 2, 2, 8          # 16-byte rows
+    shape = synth.Shape(L, H, D, "fp16")
+    rng = np.random.default_rng(5)
+    cases = 0
+    for (bs_s, bs_d, lay_s, lay_d) in [(2, 2, "lkbthd", "lkbthd"), (4, 2, "lkbthd", "blkhtd"), (2, 4, "blkhtd", "lkbthd")]:
+        NBs, NBd = 4, 4
+        ssp, dsp = synth.PoolSpec(lay_s, bs_s, NBs), synth.PoolSpec(lay_d, bs_d, NBd)
+        src_buf = P.alloc_bytes(ssp.bytes(shape))
+        dst_buf = P.alloc_bytes(dsp.bytes(shape))
+        P.fill_values(src_buf, "bits", "fp16", 99)
+        src_np = P.to_numpy(src_buf)
+        sdesc, ddesc = P.describe(ssp, shape, src_buf.data_ptr()), P.describe(dsp, shape, dst_buf.data_ptr())
+        gs, gd = G.geom(ssp, shape), G.geom(dsp, shape)
+        maxT = min(NBs * bs_s, NBd * bs_d, 8)
+        for T in range(1, maxT + 1):
+            ns, nd = -(-T // bs_s), -(-T // bs_d)
+            dtabs = list(itertools.permutations(range(NBd), nd))
+            for S in itertools.permutations(range(NBs), ns):
+                for Dt in [dtabs[i] for i in rng.choice(len(dtabs), size=min(3, len(dtabs)), replace=False)]:
+                    P.fill_sentinel(dst_buf)
+                    plan = F.flowkv_plan(sdesc, ddesc, [F.Request(T, np.asarray(S, np.int32), np.asarray(Dt, np.int32))])
+                    plan.transfer()
+                    torch.cuda.synchronize()
+                    exp = np.full(dsp.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+                    O.transfer(src_np, gs, exp, gd, S, Dt, T)
+                    G.assert_same(P.to_numpy(dst_buf), exp, f"brute {lay_s}{bs_s}->{lay_d}{bs_d} T={T} S={S} D={Dt}")
+                    assert plan.stats["n_segments"] == O.count_segments(np.asarray(S, np.int32), bs_s, np.asarray(Dt, np.int32), bs_d, T)
+                    plan.destroy()
+                    cases += 1
+    assert cases > 500
+
+
+@pytest.mark.parametrize("w_fn", [
+    lambda: synth.config1_tiny(),
+    lambda: synth.config4_hetero(n_requests=2, num_layers=2),
+    lambda: synth.config3_batched(n_requests=4, num_layers=1),
+])
+@pytest.mark.parametrize("tuning", [None, {"variant": "bulk"}])
+def test_pack_unpack_against_oracle_and_identity(w_fn, tuning):
+    """pack == oracle pack (wire format A12); unpack == oracle unpack; unpack(pack(src)) == transfer(src)."""
+    w = w_fn()
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    plan = dp.plan(0, tuning)
+    nbytes = plan.stats["staging_bytes"]
+    assert nbytes == w.payload_bytes
+    staging = P.alloc_bytes(nbytes + 64)
+    P.fill_sentinel(staging)
+    n0 = F.flowkv_launch_count()
+    plan.pack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1
+    got = P.to_numpy(staging)
+    G.assert_same(got[:nbytes], G.oracle_pack(w, src_np), "pack")
+    assert np.all(got[nbytes:] == P.SENTINEL_BYTE), "pack wrote past the wire size"
+    plan.unpack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    via_staging = P.to_numpy(dp.dst_buf)
+    G.assert_same(via_staging, G.oracle_unpack(w, got[:nbytes]), "unpack")
+    G.assert_same(via_staging, G.oracle_transfer(w, src_np), "unpack(pack(src)) == transfer(src)")
+    # one-sided plans reach the same bytes
+    P.fill_sentinel(staging)
+    p_only = F.flowkv_plan(dp.src, None, P.requests_of(w, dst=False), 0, tuning)
+    p_only.pack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(staging)[:nbytes], got[:nbytes], "pack-only plan")
+    with pytest.raises(F.FlowKVError):
+        p_only.transfer()
+    with pytest.raises(F.FlowKVError) as ei:
+        plan.pack(staging.data_ptr(), nbytes - 1)
+    assert ei.value.status == F.FLOWKV_ERR_STAGING_TOO_SMALL
+
+
+def test_pack_to_unaligned_by_16_staging_and_mapped_pinned_host():
+    """Staging at a 16-byte (not 32-byte) aligned address forces the 128-bit path; pinned host memory
+    (the stand-in for the network endpoint) is written by the same kernel through UVA."""
+    w = synth.config1_tiny()
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    plan = dp.plan()
+    nbytes = plan.stats["staging_bytes"]
+    exp = G.oracle_pack(w, src_np)
+    big = P.alloc_bytes(nbytes + 64)
+    off = 16 if big.data_ptr() % 32 == 0 else 0
+    plan.pack(big.data_ptr() + off, nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(big)[off:off + nbytes], exp, "pack to 16-byte aligned staging")
+    host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    host.fill_(P.SENTINEL_BYTE)
+    plan.pack(host.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(host.numpy(), exp, "pack to pinned host")
+    P.fill_sentinel(dp.dst_buf)
+    plan.unpack(host.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "unpack from pinned host")
+
+
+def test_round_trip_restores_source():
+    """transfer(S->D) then transfer(D->S') with the tables swapped restores every named slot."""
+    w = synth.config4_hetero(n_requests=2, num_layers=1)
+    dp = P.DevicePools(w, fill="bits")
+    dp.plan().transfer()
+    back = P.alloc_bytes(w.src.bytes(w.shape))
+    P.fill_sentinel(back)
+    bdesc = P.describe(w.src, w.shape, back.data_ptr())
+    reqs = [F.Request(r.num_tokens, r.dst_blocks, r.src_blocks) for r in w.requests]
+    F.flowkv_plan(dp.dst, bdesc, reqs).transfer()
+    torch.cuda.synchronize()
+    src_np, back_np = P.to_numpy(dp.src_buf), P.to_numpy(back)
+    # expected: sentinel everywhere except the request's token slots, which equal src (by the oracle, identity tables)
+    exp = np.full(back_np.size, P.SENTINEL_BYTE, np.uint8)
+    gs = G.geom(w.src, w.shape)
+    for r in w.requests:
+        O.transfer(src_np, gs, exp, gs, r.src_blocks, r.src_blocks, r.num_tokens)
+    G.assert_same(back_np, exp, "round trip")
+
+
+def test_empty_batches_launch_nothing():
+    w = synth.config1_tiny()
+    dp = P.DevicePools(w)
+    n0 = F.flowkv_launch_count()
+    for reqs in ([], [F.Request(0, np.zeros(0, np.int32), np.zeros(0, np.int32))]):
+        plan = F.flowkv_plan(dp.src, dp.dst, reqs)
+        plan.transfer()
+        plan.pack(0, 0)
+        plan.unpack(0, 0)
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() == n0
+    assert np.all(P.to_numpy(dp.dst_buf) == P.SENTINEL_BYTE)
+
+
+def test_shared_source_blocks_between_requests():
+    """Prefix sharing (reading A9): two requests may name the same src blocks."""
+    shape = synth.Shape(2, 2, 64, "fp16")
+    ssp, dsp = synth.PoolSpec("lkbthd", 16, 32), synth.PoolSpec("lkbthd", 16, 32)
+    r0 = synth.Request(40, np.asarray([3, 4, 9], np.int32), np.asarray([0, 1, 2], np.int32))
+    r1 = synth.Request(60, np.asarray([3, 4, 20, 21], np.int32), np.asarray([10, 11, 12, 13], np.int32))
+    w = synth.Workload("shared", 15, shape, ssp, dsp, [r0, r1], "uniform")
+    G.run_transfer_and_check(w)
+
+
+def test_non_default_stream_and_strided_pool():
+    """A caller stream other than the current one, and a STRIDED pool (separate K and V tensors with padding)."""
+    L, H, D, NB, BS = 2, 2, 64, 16, 8
+    row, tok = D * 2, H * D * 2
+    blk = BS * tok + 256          # padded blocks => not span-capable => rows mode
+    kv = NB * blk + 4096
+    lay = 2 * kv
+    nbytes = L * lay
+    src_buf, dst_buf = P.alloc_bytes(nbytes), P.alloc_bytes(nbytes)
+    P.fill_values(src_buf, "bits", "fp16", 5)
+    P.fill_sentinel(dst_buf)
+    strides = [lay, kv, blk, tok, row]
+    s = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NB, BS, "strided", strides)
+    d = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NB, BS, "strided", strides)
+    S, Dt, T = np.asarray([5, 6, 1, 9], np.int32), np.asarray([2, 3, 4, 0], np.int32), 29
+    stream = torch.cuda.Stream()
+    plan = F.flowkv_plan(s, d, [F.Request(T, S, Dt)], 0, None, stream.cuda_stream)
+    assert plan.stats["mode_transfer"] == 2
+    plan.transfer(stream.cuda_stream)
+    stream.synchronize()
+    g = O.PoolGeom(L, H, D, 2, NB, BS, lay, kv, blk, tok, row)
+    exp = np.full(nbytes, P.SENTINEL_BYTE, np.uint8)
+    O.transfer(P.to_numpy(src_buf), g, exp, g, S, Dt, T)
+    G.assert_same(P.to_numpy(dst_buf), exp, "strided pool")
+
+
+def test_baselines_reach_the_same_bytes_and_count_calls():
+    """Naive per-(block,layer,K|V) copies: calls == blocks*L*2; per-segment copies: segments*L*2."""
+    w = synth.config1_tiny()
+    dp = P.DevicePools(w)
+    src_np = P.to_numpy(dp.src_buf)
+    exp = G.oracle_transfer(w, src_np)
+    calls = F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests)
+    torch.cuda.synchronize()
+    assert calls == O.blockwise_calls(63, 2) == 252
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "blockwise baseline")
+    P.fill_sentinel(dp.dst_buf)
+    plan = dp.plan()
+    calls = F.flowkv_baseline_segmentwise(plan)
+    torch.cuda.synchronize()
+    assert calls == plan.stats["n_segments"] * 4
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "segmentwise baseline")

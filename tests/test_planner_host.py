@@ -1,0 +1,217 @@
+"""Host logic of the product library (CPU, no device): exports, validation, alignment, schedule.
+
+The library's segment list is compared with (i) the oracle's plan function, (ii) the test-side
+definition in tests/helpers.py, (iii) the hand-worked fixtures in tests/golden/."""
+import ctypes as C
+import json
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2504_03775_b200 import flowkv as F
+from paper_2504_03775_b200 import synth
+from tests import helpers as Hh
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+FAKE = 0x7F0000000000  # never dereferenced by flowkv_plan_host
+
+
+def _pool(layout, L=2, H=2, D=8, NB=16, BS=4, base=FAKE, e=2):
+    return F.make_pool(base, L, H, D, e, NB, BS, layout)
+
+
+def _segs(plan):
+    return [(s["request"], s["first_token"], s["n_tokens"]) for s in plan.segments]
+
+
+def test_library_exports_every_symbol_the_header_declares():
+    hdr = open(os.path.join(ROOT, "include", "flowkv.h")).read()
+    declared = set(re.findall(r"FLOWKV_API\s+[\w\s\*]+?\b(flowkv_\w+)\s*\(", hdr))
+    assert declared == set(F.EXPORTS), declared ^ set(F.EXPORTS)
+    lib = C.CDLL(F.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_struct_sizes_match_header_layout():
+    assert C.sizeof(F.flowkv_pool) == 8 + 8 * 4 + 5 * 8
+    assert C.sizeof(F.flowkv_request) == 32
+    assert C.sizeof(F.flowkv_segment) == 40
+    assert C.sizeof(F.flowkv_tuning) == 48
+    assert C.sizeof(F.flowkv_plan_stats) == 9 * 8 + 16 * 4
+
+
+def test_named_layout_strides():
+    p = _pool("lkbthd", L=32, H=8, D=128, NB=16384, BS=16)
+    assert list(p.stride_bytes) == [2 * 16384 * 32768, 16384 * 32768, 32768, 2048, 256]
+    q = _pool("blkhtd", L=80, H=8, D=128, NB=10, BS=64)
+    assert list(q.stride_bytes) == [262144, 131072, 20971520, 256, 16384]
+    # the oracle's geometry helper must agree (two independent statements of Eq. 5's two orders)
+    g = O.PoolGeom.blkhtd(80, 8, 128, 2, 10, 64)
+    assert [g.s_layer, g.s_kv, g.s_block, g.s_token, g.s_head] == list(q.stride_bytes)
+    assert F.pool_bytes(q) == g.span_bytes()
+
+
+@pytest.mark.parametrize("case", json.load(open(os.path.join(ROOT, "tests", "golden", "align_examples.json")))["cases"])
+def test_alignment_matches_hand_worked_fixtures(case):
+    def tab(x):
+        return np.arange(*x["arange"], dtype=np.int32) if isinstance(x, dict) else np.asarray(x, np.int32)
+    s, d = tab(case["src"]), tab(case["dst"])
+    src = _pool("lkbthd", NB=int(s.max()) + 1, BS=case["bs_src"])
+    dst = _pool("lkbthd", NB=int(d.max()) + 1, BS=case["bs_dst"])
+    plan = F.flowkv_plan_host(src, dst, [F.Request(case["tokens"], s, d)])
+    assert [[a, n] for _, a, n in _segs(plan)] == case["expect"], case["cite"]
+
+
+def test_alignment_equals_oracle_and_definition_on_random_tables():
+    rng = np.random.default_rng(7)
+    for it in range(300):
+        bs_s, bs_d = int(2 ** rng.integers(0, 4)), int(2 ** rng.integers(0, 4))
+        T = int(rng.integers(1, 60))
+        ns, nd = -(-T // bs_s), -(-T // bs_d)
+        NBs, NBd = ns + int(rng.integers(0, 4)), nd + int(rng.integers(0, 4))
+        # tables with runs: random walk that continues +1 with probability 0.6
+        def table(n, NB):
+            perm = []
+            free = set(range(NB))
+            cur = None
+            while len(perm) < n:
+                if cur is not None and cur + 1 in free and rng.random() < 0.6:
+                    cur = cur + 1
+                else:
+                    cur = int(rng.choice(sorted(free)))
+                free.discard(cur)
+                perm.append(cur)
+            return np.asarray(perm, np.int32)
+        S, D = table(ns, NBs), table(nd, NBd)
+        plan = F.flowkv_plan_host(_pool("lkbthd", NB=NBs, BS=bs_s), _pool("blkhtd", NB=NBd, BS=bs_d),
+                                  [F.Request(T, S, D)], F.FLOWKV_CHECK_DST_ALIAS)
+        got = [(a, n) for _, a, n in _segs(plan)]
+        assert got == O.align(S, bs_s, D, bs_d, T)
+        assert got == Hh.segments_from_cuts(Hh.cuts_by_definition(S, bs_s, D, bs_d, T), T)
+        Hh.check_segment_invariants(got, S, bs_s, D, bs_d, T)
+        st = plan.stats
+        assert st["n_segments"] == len(got) and st["total_tokens"] == T
+
+
+def test_segment_fields_point_at_the_right_slots():
+    S = np.asarray([5, 6, 7, 20, 21, 9, 3, 4], np.int32)
+    D = np.asarray([0, 1], np.int32)
+    plan = F.flowkv_plan_host(_pool("lkbthd", NB=32, BS=16), _pool("blkhtd", NB=2, BS=64), [F.Request(120, S, D)])
+    segs = plan.segments
+    assert [(s["src_block"], s["src_tok_off"], s["dst_block"], s["dst_tok_off"], s["n_tokens"]) for s in segs] == \
+        [(5, 0, 0, 0, 48), (20, 0, 0, 48, 32), (9, 0, 1, 16, 16), (3, 0, 1, 32, 24)]
+
+
+def test_batch_segments_never_cross_requests_and_staging_offsets():
+    # request 1 continues request 0's ids on both sides: still two segments (reading A10)
+    r0 = F.Request(32, np.asarray([4, 5], np.int32), np.asarray([0, 1], np.int32))
+    r1 = F.Request(20, np.asarray([6, 7], np.int32), np.asarray([2, 3], np.int32))
+    r2 = F.Request(0, np.zeros(0, np.int32), np.zeros(0, np.int32))
+    plan = F.flowkv_plan_host(_pool("lkbthd", BS=16), _pool("lkbthd", BS=16), [r0, r2, r1])
+    assert _segs(plan) == [(0, 0, 32), (2, 0, 20)]
+    assert [s["staging_tok_off"] for s in plan.segments] == [0, 32]
+    st = plan.stats
+    assert st["n_requests"] == 3 and st["total_tokens"] == 52
+    assert st["payload_bytes"] == 52 * 2 * 2 * 2 * 8 * 2 == st["staging_bytes"]
+
+
+def test_config_segment_counts():
+    """cfg1: permutation table => one segment per block (63); cfg2: ~208; contiguous both sides => 1."""
+    w = synth.config1_tiny()
+    sp = F.make_pool(FAKE, 2, 2, 64, 2, 128, 16, "lkbthd")
+    plan = F.flowkv_plan_host(sp, sp, [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks) for r in w.requests])
+    assert plan.stats["n_segments"] == 63
+    assert plan.stats["mode_transfer"] == 1 and plan.stats["mode_pack"] == 1 and plan.stats["mode_unpack"] == 1
+    w = synth.config2_llama8b_13k()
+    r = w.requests[0]
+    s8 = F.make_pool(FAKE, 32, 8, 128, 2, 16384, 16, "lkbthd")
+    d8 = F.make_pool(FAKE, 32, 8, 128, 2, 1024, 16, "lkbthd")
+    plan = F.flowkv_plan_host(s8, d8, [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks)])
+    assert plan.stats["n_segments"] == synth.n_runs(r.src_blocks) == O.count_segments(r.src_blocks, 16, r.dst_blocks, 16, 13312)
+    assert plan.stats["payload_bytes"] == 1_744_830_464
+    w = synth.config5_point(131072, 0)
+    r = w.requests[0]
+    plan = F.flowkv_plan_host(F.make_pool(FAKE, 32, 8, 128, 2, w.src.num_blocks, 16), F.make_pool(FAKE, 32, 8, 128, 2, w.dst.num_blocks, 16),
+                              [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks)])
+    assert plan.stats["n_segments"] == 1
+
+
+def test_hetero_layout_uses_rows_mode_and_chunks_cover_every_token_once():
+    w = synth.config4_hetero(n_requests=3, num_layers=2)
+    sp = F.make_pool(FAKE, 2, 8, 128, 2, w.src.num_blocks, 16, "lkbthd")
+    dp = F.make_pool(FAKE, 2, 8, 128, 2, w.dst.num_blocks, 64, "blkhtd")
+    plan = F.flowkv_plan_host(sp, dp, [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks) for r in w.requests])
+    st = plan.stats
+    assert st["mode_transfer"] == 2          # rows
+    assert st["mode_pack"] == 1              # lkbthd -> dense is contiguous
+    assert st["mode_unpack"] == 2            # dense -> blkhtd is a head/token transposition
+    exp = sum(O.count_segments(r.src_blocks, 16, r.dst_blocks, 64, r.num_tokens) for r in w.requests)
+    assert st["n_segments"] == exp
+
+
+@pytest.mark.parametrize("mutate,status", [
+    (lambda s, d, r: setattr(r, "src_blocks", np.asarray([0, 1, 99], np.int32)), F.FLOWKV_ERR_BLOCK_OOB),
+    (lambda s, d, r: setattr(r, "dst_blocks", np.asarray([0, -1, 2], np.int32)), F.FLOWKV_ERR_BLOCK_OOB),
+    (lambda s, d, r: setattr(r, "src_blocks", np.asarray([0, 1], np.int32)), F.FLOWKV_ERR_TABLE_LEN),
+    (lambda s, d, r: setattr(r, "dst_blocks", np.asarray([0, 1, 2, 3], np.int32)), F.FLOWKV_ERR_TABLE_LEN),
+    (lambda s, d, r: setattr(r, "dst_blocks", np.asarray([3, 1, 3], np.int32)), F.FLOWKV_ERR_DST_ALIAS),
+    (lambda s, d, r: setattr(d, "head_dim", 16), F.FLOWKV_ERR_SHAPE_MISMATCH),
+    (lambda s, d, r: setattr(s, "base", FAKE + 8), F.FLOWKV_ERR_ALIGN),
+    (lambda s, d, r: setattr(s, "block_size", 3), F.FLOWKV_ERR_UNSUPPORTED),
+    (lambda s, d, r: setattr(s, "base", None), F.FLOWKV_ERR_INVALID_ARG),
+])
+def test_validation_errors(mutate, status):
+    s, d = _pool("lkbthd", NB=8, BS=4), _pool("lkbthd", NB=8, BS=4)
+    r = F.Request(10, np.asarray([0, 1, 2], np.int32), np.asarray([4, 5, 6], np.int32))
+    mutate(s, d, r)
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_plan_host(s, d, [r], F.FLOWKV_CHECK_DST_ALIAS)
+    assert ei.value.status == status, str(ei.value)
+    assert F.flowkv_status_string(status) == ei.value.name
+
+
+def test_row_not_multiple_of_16_bytes_is_rejected():
+    with pytest.raises(F.FlowKVError) as ei:
+        p = _pool("lkbthd", D=4)      # 8-byte rows
+        F.flowkv_plan_host(p, p, [])
+    assert ei.value.status == F.FLOWKV_ERR_ALIGN
+
+
+def test_host_plan_cannot_run_and_empty_batch_is_ok():
+    p = _pool("lkbthd")
+    plan = F.flowkv_plan_host(p, p, [])
+    assert plan.stats["n_segments"] == 0 and plan.stats["payload_bytes"] == 0
+    with pytest.raises(F.FlowKVError) as ei:
+        plan.transfer()
+    assert ei.value.status == F.FLOWKV_ERR_UNSUPPORTED
+    plan.destroy()
+    plan.destroy()   # idempotent
+
+
+def test_no_device_means_loud_failure_not_fallback():
+    """On a machine without a GPU flowkv_plan (device variant) must fail with FLOWKV_ERR_CUDA."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("has a GPU")
+    p = _pool("lkbthd")
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_plan(p, p, [F.Request(4, np.asarray([0], np.int32), np.asarray([1], np.int32))])
+    assert ei.value.status == F.FLOWKV_ERR_CUDA
+
+
+def test_tile_schedule_respects_tile_bytes():
+    s8 = F.make_pool(FAKE, 32, 8, 128, 2, 16384, 16, "lkbthd")
+    d8 = F.make_pool(FAKE, 32, 8, 128, 2, 1024, 16, "lkbthd")
+    w = synth.config2_llama8b_13k()
+    r = w.requests[0]
+    for tile in (8192, 32768, 65536):
+        plan = F.flowkv_plan_host(s8, d8, [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks)], 0, {"tile_bytes": tile})
+        st = plan.stats
+        # every segment of n blocks (32 KiB per block-plane) needs ceil(n*32768/tile) chunks
+        runs = np.diff(np.concatenate([[0], np.nonzero(np.diff(r.src_blocks) != 1)[0] + 1, [len(r.src_blocks)]]))
+        assert st["n_chunks_transfer"] == int(sum(-(-int(n) * 32768 // tile) for n in runs))
+        assert st["tile_bytes"] == tile and st["n_planes"] == 64
