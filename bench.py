@@ -1,0 +1,431 @@
+#!/usr/bin/env python
+"""bench.py — FlowKV KV-cache transfer on B200: device-timed GB/s, % of HBM peak, launches/request.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg2|cfg1|cfg3|cfg4]
+    python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
+    python bench.py --sweep                   # BASELINE.json configs[4]: length x run-length sweep
+
+One "step" is one pass of the whole hot path over one transfer batch: validate + bidirectional
+segment alignment + tile schedule + plan upload (flowkv_plan), ONE persistent kernel (flowkv_transfer),
+plan release.  Pools are resident in HBM before the timed region.  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "kv_transfer_payload_GBps"      # BASELINE.json metric: KV transfer GB/s (payload bytes moved / device time)
+UNIT = "GB/s"
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and clock-event (throttle) reasons through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, device_index: int, period_s: float = 0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self.period = period_s
+        self.h = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                if not uuid.startswith("GPU-"):
+                    uuid = "GPU-" + uuid
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+            self.h = None
+
+    def _reasons_now(self) -> int:
+        for fn in ("nvmlDeviceGetCurrentClocksEventReasons", "nvmlDeviceGetCurrentClocksThrottleReasons"):
+            if hasattr(self.nv, fn):
+                try:
+                    return int(getattr(self.nv, fn)(self.h))
+                except Exception:
+                    pass
+        return 0
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                bits = self._reasons_now()
+                for b, name in self.REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.h is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# workloads
+# ---------------------------------------------------------------------------------------------------
+def build_workload(name: str, free_bytes: int):
+    from paper_2504_03775_b200 import synth
+    budget = int(0.85 * free_bytes)
+    if name == "cfg1":
+        return synth.config1_tiny(), "configs[0] Tiny: 2 layers, 2 KV heads, head_dim 64, fp16, 1 x 1000 tokens"
+    if name == "cfg2":
+        return (synth.config2_llama8b_13k(),
+                "configs[1] Llama-3-8B KV: 32 layers, 8 KV heads, head_dim 128, bf16, block 16, 1 x 13,312 tokens, "
+                "src 16,384-block pool (32 GiB) runs~Geom(mean 4), dst contiguous")
+    if name == "cfg3":
+        w = synth.config3_batched(budget_bytes=budget)
+        return w, (f"configs[2] batched Llama-3-8B KV: first {w.notes['n_requests']} of 64 requests (fit rule), "
+                   "lognormal lengths, src runs mean 2, dst runs mean 16, one batch")
+    if name == "cfg4":
+        w = synth.config4_hetero(budget_bytes=budget)
+        return w, (f"configs[3] hetero Llama-3-70B KV: first {w.notes['n_requests']} of 16 requests (fit rule), "
+                   "src block 16 LKBTHD -> dst block 64 BLKHTD")
+    raise SystemExit(f"unknown --config {name}")
+
+
+def load_peaks() -> tuple:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        j = json.load(open(p))
+        return float(j["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, plain torch copy, read+write bytes)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def load_traffic(workload_key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        return json.load(open(p)).get(workload_key)
+    except Exception:
+        return None
+
+
+# ---------------------------------------------------------------------------------------------------
+# the CPU oracle as a baseline (bounded sample)
+# ---------------------------------------------------------------------------------------------------
+def oracle_geoms(w, num_layers=None):
+    from oracle import oracle as O
+    L = w.shape.num_layers if num_layers is None else num_layers
+    mk = lambda spec: getattr(O.PoolGeom, spec.layout)(L, w.shape.num_kv_heads, w.shape.head_dim, w.shape.elem_bytes,
+                                                       spec.num_blocks, spec.block_size)
+    return mk(w.src), mk(w.dst)
+
+
+def oracle_sample_setup(w, n_layers: int, src_dev=None):
+    """Host copies of the first n_layers of the pools, laid out as n_layers-deep pools of the same kind.
+    For LKBTHD the first layers are a prefix of the buffer; for BLKHTD each block keeps its first layers."""
+    import dataclasses
+    from oracle import oracle as O
+    gs_full, gd_full = oracle_geoms(w)
+    gs, gd = oracle_geoms(w, n_layers)
+    rng = np.random.default_rng(1)
+
+    def host_pool(g, full, dev, layout):
+        nbytes = g.span_bytes()
+        if dev is not None and layout == "lkbthd":
+            return dev[:nbytes].cpu().numpy()
+        return rng.integers(0, 256, size=nbytes, dtype=np.uint8)     # values are irrelevant to a copy's speed
+    src = host_pool(gs, gs_full, src_dev, w.src.layout)
+    dst = np.zeros(gd.span_bytes(), np.uint8)
+    dst[:] = 0xA5                                                    # touch every page before timing
+    return O, gs, gd, src, dst
+
+
+def oracle_run(O, gs, gd, src, dst, w, n_tokens_cap=None) -> int:
+    """Token-by-token oracle transfer over every request (optionally only the first tokens of each).
+    Returns payload bytes moved."""
+    moved = 0
+    for r in w.requests:
+        T = r.num_tokens if n_tokens_cap is None else min(r.num_tokens, n_tokens_cap)
+        O.transfer(src, gs, dst, gd, r.src_blocks[: -(-T // w.src.block_size)], r.dst_blocks[: -(-T // w.dst.block_size)], T)
+        moved += T * 2 * gs.num_layers * gs.num_kv_heads * gs.head_dim * gs.elem_bytes
+    return moved
+
+
+def cpu_baseline(w, src_dev, target_s: float = 12.0) -> dict:
+    n_layers = 1
+    O, gs, gd, src, dst = oracle_sample_setup(w, n_layers, src_dev)
+    t0 = time.perf_counter()
+    moved = oracle_run(O, gs, gd, src, dst, w)
+    dt = time.perf_counter() - t0
+    reps = 1
+    while dt < target_s and reps < 64:                               # repeat the same sample until ~target_s of CPU work
+        t1 = time.perf_counter()
+        moved += oracle_run(O, gs, gd, src, dst, w)
+        dt += time.perf_counter() - t1
+        reps += 1
+    return {"value": moved / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"layer 0 of {w.shape.num_layers} (all requests, all tokens, both K and V) of the same workload, "
+                      f"{reps} passes, {dt:.1f} s of single-threaded oracle/flowkv_oracle.c (gcc -O2)",
+            "seconds": dt, "host_cores_available": os.cpu_count()}
+
+
+# ---------------------------------------------------------------------------------------------------
+# reference arm: the oracle, as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------------
+def run_reference(args) -> None:
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w, desc = build_workload(args.config, 170 * 2 ** 30)
+    O, gs, gd, src, dst = oracle_sample_setup(w, 1, None)
+    # calibrate: how many tokens per request keep the whole run within ~2 minutes
+    t0 = time.perf_counter()
+    moved = oracle_run(O, gs, gd, src, dst, w, n_tokens_cap=512)
+    rate = moved / max(time.perf_counter() - t0, 1e-6)               # bytes/s
+    budget_per_step = 100.0 / max(args.steps + args.warmup, 1)
+    per_tok = 2 * gs.num_kv_heads * gs.head_dim * gs.elem_bytes * len(w.requests)
+    cap = int(max(64, min(max(r.num_tokens for r in w.requests), budget_per_step * rate / per_tok)))
+    for _ in range(args.warmup):
+        oracle_run(O, gs, gd, src, dst, w, cap)
+    t0 = time.perf_counter()
+    moved = 0
+    for _ in range(args.steps):
+        moved += oracle_run(O, gs, gd, src, dst, w, cap)
+    dt = time.perf_counter() - t0
+    val = moved / dt / 1e9
+    sample = (f"layer 0 of {w.shape.num_layers}, first {cap} tokens of each request, per step; "
+              f"single-threaded oracle/flowkv_oracle.c (gcc -O2), host-resident pools")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u16", "data": "synthetic",
+            "config": {"workload": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------------
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+    from paper_2504_03775_b200 import build as B
+    B.build()
+    from paper_2504_03775_b200 import flowkv as F
+    from paper_2504_03775_b200 import pools as P
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    free_b, _total = torch.cuda.mem_get_info()
+    w, desc = build_workload(args.config, free_b)
+    tuning = json.loads(args.tuning) if args.tuning else None
+    dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False)
+    payload = w.payload_bytes
+    stream = torch.cuda.current_stream()
+    s = stream.cuda_stream
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(ev_a=None, ev_b=None):
+        plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)     # a1-a4 (upload is stream-ordered)
+        if ev_a is not None:
+            ev_a.record(stream)
+        F.flowkv_transfer(plan, s)                                           # a5: ONE launch
+        if ev_b is not None:
+            ev_b.record(stream)
+        plan.destroy()                                                       # stream-ordered free
+
+    for _ in range(max(W, 3)):
+        step()
+    plan0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)
+    stats = plan0.stats
+    plan0.destroy()
+    ka = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    kb = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    clocks = ClockSampler(local)
+    barrier()
+    clocks.start()
+    n0 = F.flowkv_launch_count()
+    e0.record(stream)
+    for k in range(K):
+        step(ka[k], kb[k])
+    e1.record(stream)
+    barrier()
+    launches = F.flowkv_launch_count() - n0
+    clk = clocks.stop()
+    t_ms = e0.elapsed_time(e1)
+    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ka, kb)]))
+    kern_min_ms = float(np.min([a.elapsed_time(b) for a, b in zip(ka, kb)]))
+    if world > 1:
+        t = torch.tensor([t_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_ms = float(t.item())
+    value = world * K * payload / (t_ms * 1e-3) / 1e9
+
+    line = None
+    if rank == 0:
+        peak, peak_src = load_peaks()
+        achieved = 2 * payload / (kern_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
+            "ms_per_step": t_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u16", "data": "synthetic",
+            "config": {"workload": desc, "name": w.name, "requests": len(w.requests), "tokens": w.total_tokens,
+                       "payload_bytes": payload, "segments": stats["n_segments"],
+                       "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
+                       if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
+                       "step": "flowkv_plan + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM",
+                       "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
+                                                        "vec_bytes", "cache_hint", "tile_order", "stages")}},
+            "clocks": clk,
+            "gpu_launches": int(launches),
+            "launches_per_batch": launches / K, "launches_per_request": launches / K / max(len(w.requests), 1),
+            "latency_ms_per_request": t_ms / K / max(len(w.requests), 1),
+            "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": load_traffic(w.name), "peak_source": peak_src,
+                         "kernel": "fk_span_ldst" if stats["mode_transfer"] == 1 else "fk_rows_ldst",
+                         "kernel_ms_avg": kern_ms, "kernel_ms_min": kern_min_ms,
+                         "algorithmic_bytes_per_launch": 2 * payload,
+                         "kernel_share_of_step": kern_ms / (t_ms / K)},
+        }
+
+    # ---- end to end through host memory: pool -> pinned host (flowkv_pack) -> pool (flowkv_unpack) -------------
+    if not args.no_e2e:
+        nbytes = payload
+        host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+        Ke = max(2, min(args.e2e_steps, K))
+
+        def e2e_step():
+            plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+            F.flowkv_pack(plan, host.data_ptr(), nbytes, s)          # device -> pinned host, one kernel
+            F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)        # pinned host -> device, one kernel
+            plan.destroy()
+        e2e_step()
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(Ke):
+            e2e_step()
+        b.record(stream)
+        barrier()
+        te = a.elapsed_time(b)
+        if world > 1:
+            t = torch.tensor([te], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            te = float(t.item())
+        # link reference: one contiguous copy-engine D2H and H2D of the same bytes
+        dev_flat = dp.dst_buf[:nbytes] if dp.dst_buf.numel() >= nbytes else P.alloc_bytes(nbytes)
+        a.record(stream); host.copy_(dev_flat, non_blocking=True); b.record(stream); torch.cuda.synchronize()
+        d2h = nbytes / (a.elapsed_time(b) * 1e-3) / 1e9
+        a.record(stream); dev_flat.copy_(host, non_blocking=True); b.record(stream); torch.cuda.synchronize()
+        h2d = nbytes / (a.elapsed_time(b) * 1e-3) / 1e9
+        if rank == 0:
+            line["e2e"] = {"value": world * Ke * payload / (te * 1e-3) / 1e9, "unit": UNIT,
+                           "h2d_bytes_per_step": nbytes + stats["plan_device_bytes"], "d2h_bytes_per_step": nbytes,
+                           "steps": Ke, "ms_per_step": te / Ke,
+                           "path": "flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host",
+                           "link_memcpy_d2h_GBps": d2h, "link_memcpy_h2d_GBps": h2d}
+        del host
+
+    # ---- comparison baselines on the same pools (outside the timed region) ---------------------------------
+    if rank == 0 and not args.no_baselines:
+        extra = {}
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if stats["mode_transfer"] == 1 and w.src.block_size == w.dst.block_size:
+            for name, fn in (("blockwise_memcpy", lambda: F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests, s)),):
+                fn(); torch.cuda.synchronize()
+                t0 = time.perf_counter(); a.record(stream); calls = fn(); b.record(stream); torch.cuda.synchronize()
+                extra[name] = {"calls": calls, "device_ms": a.elapsed_time(b), "wall_ms": (time.perf_counter() - t0) * 1e3,
+                               "GBps": payload / (a.elapsed_time(b) * 1e-3) / 1e9}
+            plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)
+            F.flowkv_baseline_segmentwise(plan, s); torch.cuda.synchronize()
+            t0 = time.perf_counter(); a.record(stream); calls = F.flowkv_baseline_segmentwise(plan, s); b.record(stream)
+            torch.cuda.synchronize()
+            extra["segmentwise_memcpy"] = {"calls": calls, "device_ms": a.elapsed_time(b),
+                                           "wall_ms": (time.perf_counter() - t0) * 1e3,
+                                           "GBps": payload / (a.elapsed_time(b) * 1e-3) / 1e9}
+            plan.destroy()
+        flat_a = dp.src_buf[:payload]
+        flat_b = dp.dst_buf[:payload] if dp.dst_buf.numel() >= payload else P.alloc_bytes(payload)
+        ts = []
+        for _ in range(5):
+            a.record(stream); flat_b.copy_(flat_a); b.record(stream); torch.cuda.synchronize(); ts.append(a.elapsed_time(b))
+        extra["contiguous_copy"] = {"calls": 1, "device_ms": min(ts), "GBps": payload / (min(ts) * 1e-3) / 1e9}
+        line["baselines"] = extra
+
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w, dp.src_buf)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-baselines", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="run the configs[4] sweep instead (see bench_sweep.py)")
+    args = ap.parse_args()
+    if args.sweep:
+        import bench_sweep
+        bench_sweep.main([])
+        return
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

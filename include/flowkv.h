@@ -159,7 +159,8 @@ typedef struct {
 FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
 
 /* Build a plan: validate (a1), bidirectional segment alignment (a2), tile schedule (a3),
- * upload (a4; one cudaMalloc + one cudaMemcpyAsync on `stream`).
+ * upload (a4; one cudaMallocAsync + one cudaMemcpyAsync from cached pinned memory, both on `stream`;
+ * no host synchronisation, so planning batch k+1 overlaps the move of batch k).
  *   src, dst : HOST pointers to pool descriptors; either may be NULL (pack-only / unpack-only).
  *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
  *   tuning   : HOST pointer or NULL.
@@ -190,6 +191,9 @@ FLOWKV_API flowkv_status flowkv_transfer(const flowkv_plan_t* plan, void* stream
 FLOWKV_API flowkv_status flowkv_pack(const flowkv_plan_t* plan, void* staging, uint64_t bytes, void* stream);
 FLOWKV_API flowkv_status flowkv_unpack(const flowkv_plan_t* plan, const void* staging, uint64_t bytes, void* stream);
 
+FLOWKV_API /* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
+ * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,
+ * synchronise that stream first.  NULL is ignored. */
 FLOWKV_API void flowkv_plan_destroy(flowkv_plan_t* plan);
 
 FLOWKV_API const char* flowkv_status_string(flowkv_status s);

@@ -5,6 +5,7 @@
 #include <atomic>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "flowkv_internal.h"
@@ -29,6 +30,53 @@ bool is_pow2(uint32_t x) { return x && !(x & (x - 1)); }
 uint32_t log2u(uint32_t x) { uint32_t l = 0; while ((1u << l) < x) ++l; return l; }
 uint32_t log2_or_none(uint32_t x) { return is_pow2(x) ? log2u(x) : 0xffffffffu; }
 
+// Pinned host staging for plan uploads.  A pageable cudaMemcpyAsync larger than the driver's inline
+// limit waits for earlier work on the stream, which would serialise "plan batch k+1" behind "move
+// batch k"; a pinned source keeps the upload a plain stream-ordered DMA.  Buffers are cached for the
+// life of the process (grow-only); an event marks when the last upload that read a buffer is done.
+struct PinnedBuf {
+  void* p = nullptr;
+  size_t cap = 0;
+  cudaEvent_t ev = nullptr;
+  bool pending = false;
+};
+
+class PinnedCache {
+ public:
+  cudaError_t acquire(size_t bytes, PinnedBuf& out) {
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      for (size_t i = 0; i < free_.size(); ++i)
+        if (free_[i].cap >= bytes) {
+          out = free_[i];
+          free_.erase(free_.begin() + i);
+          if (out.pending) { cudaEventSynchronize(out.ev); out.pending = false; }
+          return cudaSuccess;
+        }
+    }
+    size_t cap = 64 << 10;
+    while (cap < bytes) cap <<= 1;
+    PinnedBuf b;
+    cudaError_t e = cudaHostAlloc(&b.p, cap, cudaHostAllocDefault);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreateWithFlags(&b.ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) { cudaFreeHost(b.p); return e; }
+    b.cap = cap;
+    out = b;
+    return cudaSuccess;
+  }
+  void release(const PinnedBuf& b) {
+    if (!b.p) return;
+    std::lock_guard<std::mutex> lk(mu_);
+    free_.push_back(b);
+  }
+
+ private:
+  std::mutex mu_;
+  std::vector<PinnedBuf> free_;
+};
+PinnedCache g_pinned;
+
 struct Op {                  // one runnable operation of a plan
   Schedule sched;
   const Chunk* d_chunks = nullptr;
@@ -49,8 +97,10 @@ struct flowkv_plan_s {
   std::vector<flowkv_segment> segs_pack, segs_unpack;
   Op transfer, pack, unpack;
   uint64_t n_requests = 0, total_tokens = 0;
-  void* d_buf = nullptr;
+  void* d_buf = nullptr;     // stream-ordered allocation on `stream`
   uint64_t d_bytes = 0;
+  cudaStream_t stream = nullptr;   // the stream flowkv_plan() was given: upload and free are ordered on it
+  PinnedBuf staging{};
   int device = -1;
   uint32_t num_sms = 0, max_smem_optin = 0;
 };
@@ -97,12 +147,15 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
     ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(n_tiles, 1));
     return;
   }
-  ls.threads = t.threads ? t.threads : 256;
-  ls.group_threads = t.group_threads ? t.group_threads : ls.threads;
+  // defaults from the cfg2 sweep on B200 (profiles/r01_tuning_sweep.md): one CTA-wide round of
+  // 512 threads x 4 x 32 B covers a 64 KiB tile; the grid is oversubscribed 8x so that the hardware
+  // CTA scheduler evens out SM-to-SM speed differences.
+  ls.threads = t.threads ? t.threads : std::min<uint32_t>(512, std::max<uint32_t>(128, pl->tile_bytes / 128));
+  ls.group_threads = t.group_threads ? std::min(t.group_threads, ls.threads) : ls.threads;
   ls.hint = t.cache_hint ? t.cache_hint - 1 : 2;
   ls.n_stages = 0;
   ls.stage_bytes = 0;
-  const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 4;
+  const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 8;
   const uint32_t groups_per_cta = ls.threads / ls.group_threads;
   const uint64_t ctas_needed = (n_tiles + groups_per_cta - 1) / groups_per_cta;
   ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(ctas_needed, 1));
@@ -179,10 +232,10 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       pl->num_sms = 148;
     }
 
-    // tile size: default 32 KiB; shrink for small batches so every SM gets several tiles
+    // tile size: default 64 KiB; shrink for small batches so every SM gets several tiles
     uint32_t tile = tn.tile_bytes;
     if (!tile) {
-      tile = 32u << 10;
+      tile = 64u << 10;
       const uint64_t want_tiles = 8ull * pl->num_sms;
       const uint64_t payload = pl->total_tokens * g.bytes_per_token;
       while (tile > 4096 && payload / tile < want_tiles) tile >>= 1;
@@ -215,22 +268,33 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       }
 
     if (device) {
-      // a4: one allocation, one stream-ordered upload for all schedules
+      // a4: one stream-ordered allocation and ONE upload (from cached pinned memory) for all schedules
       uint64_t bytes = 0;
       for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) bytes += op->sched.chunks.size() * sizeof(Chunk);
+      pl->stream = (cudaStream_t)stream;
       if (bytes) {
-        cudaError_t e = cudaMalloc(&pl->d_buf, bytes);
-        if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaMalloc(plan)"); }
+        cudaError_t e = g_pinned.acquire(bytes, pl->staging);
+        if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaHostAlloc(plan staging)"); }
+        e = cudaMallocAsync(&pl->d_buf, bytes, pl->stream);
+        if (e != cudaSuccess) { g_pinned.release(pl->staging); delete pl; return fail_cuda(e, "cudaMallocAsync(plan)"); }
         pl->d_bytes = bytes;
-        char* p = (char*)pl->d_buf;
+        uint64_t off = 0;
         for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) {
           const uint64_t n = op->sched.chunks.size() * sizeof(Chunk);
           if (!n) continue;
-          e = cudaMemcpyAsync(p, op->sched.chunks.data(), n, cudaMemcpyHostToDevice, (cudaStream_t)stream);
-          if (e != cudaSuccess) { cudaFree(pl->d_buf); delete pl; return fail_cuda(e, "cudaMemcpyAsync(plan)"); }
-          op->d_chunks = (const Chunk*)p;
-          p += n;
+          memcpy((char*)pl->staging.p + off, op->sched.chunks.data(), n);
+          op->d_chunks = (const Chunk*)((char*)pl->d_buf + off);
+          off += n;
         }
+        e = cudaMemcpyAsync(pl->d_buf, pl->staging.p, bytes, cudaMemcpyHostToDevice, pl->stream);
+        if (e == cudaSuccess) e = cudaEventRecord(pl->staging.ev, pl->stream);
+        if (e != cudaSuccess) {
+          cudaFreeAsync(pl->d_buf, pl->stream);
+          g_pinned.release(pl->staging);
+          delete pl;
+          return fail_cuda(e, "cudaMemcpyAsync(plan)");
+        }
+        pl->staging.pending = true;
       }
       pl->on_device = true;
     }
@@ -392,7 +456,8 @@ flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64
 
 void flowkv_plan_destroy(flowkv_plan_t* pl) {
   if (!pl) return;
-  if (pl->d_buf) cudaFree(pl->d_buf);
+  if (pl->d_buf) cudaFreeAsync(pl->d_buf, pl->stream);   // ordered after everything queued on the plan's stream
+  g_pinned.release(pl->staging);
   delete pl;
 }
 
