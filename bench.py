@@ -242,6 +242,7 @@ def run_ours(args) -> None:
     B.build()
     from paper_2504_03775_b200 import flowkv as F
     from paper_2504_03775_b200 import pools as P
+    from paper_2504_03775_b200 import shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -296,10 +297,7 @@ def run_ours(args) -> None:
     t_ms = e0.elapsed_time(e1)
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ka, kb)]))
     kern_min_ms = float(np.min([a.elapsed_time(b) for a, b in zip(ka, kb)]))
-    if world > 1:
-        t = torch.tensor([t_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_ms = float(t.item())
+    t_ms = shard.max_over_ranks(t_ms, device="cuda")                        # max over ranks, device-timed
     value = world * K * payload / (t_ms * 1e-3) / 1e9
 
     line = None
@@ -350,10 +348,7 @@ def run_ours(args) -> None:
         b.record(stream)
         barrier()
         te = a.elapsed_time(b)
-        if world > 1:
-            t = torch.tensor([te], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
+        te = shard.max_over_ranks(te, device="cuda")
         # link reference: one contiguous copy-engine D2H and H2D of the same bytes
         dev_flat = dp.dst_buf[:nbytes] if dp.dst_buf.numel() >= nbytes else P.alloc_bytes(nbytes)
         a.record(stream); host.copy_(dev_flat, non_blocking=True); b.record(stream); torch.cuda.synchronize()

@@ -111,7 +111,7 @@ __device__ __forceinline__ void decode_tile(const KernelParams& p, uint32_t tile
 // ldst / span
 // ------------------------------------------------------------------------------------------------
 template <int VEC, int UNROLL, int HINT>
-__global__ void __launch_bounds__(512, 1) fk_span_ldst(const __grid_constant__ KernelParams p) {
+__global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ KernelParams p) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
   const uint32_t lane = gtid & (G - 1);
@@ -119,33 +119,35 @@ __global__ void __launch_bounds__(512, 1) fk_span_ldst(const __grid_constant__ K
   const uint32_t step = G * VEC;
   const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
 
-  for (uint32_t tile = gtid >> p.group_log2; tile < p.n_tiles; tile += n_groups) {
-    uint32_t plane, ci;
-    decode_tile(p, tile, plane, ci);
-    const Chunk c = load_chunk(p.chunks + ci);
+  uint32_t tile = gtid >> p.group_log2;
+  if (tile >= p.n_tiles) return;
+  uint32_t plane, ci;
+  decode_tile(p, tile, plane, ci);
+  Chunk c = load_chunk(p.chunks + ci);
+  for (; tile < p.n_tiles; tile += n_groups) {
+    // fetch the NEXT tile's schedule entry now, so its latency hides behind this tile's copy
+    const uint32_t next = tile + n_groups;
+    uint32_t nplane = 0, nci = 0;
+    Chunk cn = c;
+    if (next < p.n_tiles) {
+      decode_tile(p, next, nplane, nci);
+      cn = load_chunk(p.chunks + nci);
+    }
     const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
     char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
     const uint32_t n = c.n;
-    uint32_t off = lane * VEC;
-    // full rounds: UNROLL independent loads in flight, then UNROLL stores
-    while (off + (UNROLL - 1) * step < n) {
+    // UNROLL independent loads in flight per thread, then UNROLL stores; the last round is ragged
+    for (uint32_t off = lane * VEC; off < n; off += UNROLL * step) {
       Vec<VEC> v[UNROLL];
 #pragma unroll
-      for (int j = 0; j < UNROLL; ++j) v[j] = Mem<VEC, HINT>::ld(s + off + j * step, pol);
-#pragma unroll
-      for (int j = 0; j < UNROLL; ++j) Mem<VEC, HINT>::st(d + off + j * step, v[j], pol);
-      off += UNROLL * step;
-    }
-    // ragged tail: at most UNROLL-1 more vectors for this thread
-    if (off < n) {
-      Vec<VEC> v[UNROLL - 1];
-#pragma unroll
-      for (int j = 0; j < UNROLL - 1; ++j)
+      for (int j = 0; j < UNROLL; ++j)
         if (off + j * step < n) v[j] = Mem<VEC, HINT>::ld(s + off + j * step, pol);
 #pragma unroll
-      for (int j = 0; j < UNROLL - 1; ++j)
+      for (int j = 0; j < UNROLL; ++j)
         if (off + j * step < n) Mem<VEC, HINT>::st(d + off + j * step, v[j], pol);
     }
+    c = cn;
+    plane = nplane;
   }
 }
 
@@ -153,7 +155,7 @@ __global__ void __launch_bounds__(512, 1) fk_span_ldst(const __grid_constant__ K
 // ldst / rows: token- and head-strided rows (layout and block-size conversion fused in the move)
 // ------------------------------------------------------------------------------------------------
 template <int VEC, int UNROLL, int HINT>
-__global__ void __launch_bounds__(512, 1) fk_rows_ldst(const __grid_constant__ KernelParams p) {
+__global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ KernelParams p) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
   const uint32_t lane = gtid & (G - 1);
@@ -162,16 +164,25 @@ __global__ void __launch_bounds__(512, 1) fk_rows_ldst(const __grid_constant__ K
   const uint32_t vpr = p.row_bytes / VEC;            // vectors per row
   const bool pow2 = (p.vpr_log2 != 0xffffffffu) && (p.heads_log2 != 0xffffffffu);
 
-  for (uint32_t tile = gtid >> p.group_log2; tile < p.n_tiles; tile += n_groups) {
-    uint32_t plane, ci;
-    decode_tile(p, tile, plane, ci);
-    const Chunk c = load_chunk(p.chunks + ci);
+  uint32_t tile = gtid >> p.group_log2;
+  if (tile >= p.n_tiles) return;
+  uint32_t plane, ci;
+  decode_tile(p, tile, plane, ci);
+  Chunk c = load_chunk(p.chunks + ci);
+  for (; tile < p.n_tiles; tile += n_groups) {
+    const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see fk_span_ldst)
+    uint32_t nplane = 0, nci = 0;
+    Chunk cn = c;
+    if (next < p.n_tiles) {
+      decode_tile(p, next, nplane, nci);
+      cn = load_chunk(p.chunks + nci);
+    }
     const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
     char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
     const uint32_t pieces = c.n * p.heads * vpr;       // vectors in this chunk, (token, head, vec) order
     for (uint32_t i0 = lane; i0 < pieces; i0 += G * UNROLL) {
       Vec<VEC> v[UNROLL];
-      int64_t doff[UNROLL];
+      uint32_t doff[UNROLL];          // offsets inside one block fit 32 bits (checked by the planner)
 #pragma unroll
       for (int j = 0; j < UNROLL; ++j) {
         const uint32_t i = i0 + j * G;
@@ -184,8 +195,8 @@ __global__ void __launch_bounds__(512, 1) fk_rows_ldst(const __grid_constant__ K
             row = i / vpr;       o = i - row * vpr;
             tok = row / p.heads; h = row - tok * p.heads;
           }
-          const int64_t soff = (int64_t)tok * p.src.s_token + (int64_t)h * p.src.s_head + o * VEC;
-          doff[j] = (int64_t)tok * p.dst.s_token + (int64_t)h * p.dst.s_head + o * VEC;
+          const uint32_t soff = tok * (uint32_t)p.src.s_token + h * (uint32_t)p.src.s_head + o * VEC;
+          doff[j] = tok * (uint32_t)p.dst.s_token + h * (uint32_t)p.dst.s_head + o * VEC;
           v[j] = Mem<VEC, HINT>::ld(s + soff, pol);
         }
       }
@@ -193,6 +204,8 @@ __global__ void __launch_bounds__(512, 1) fk_rows_ldst(const __grid_constant__ K
       for (int j = 0; j < UNROLL; ++j)
         if (i0 + j * G < pieces) Mem<VEC, HINT>::st(d + doff[j], v[j], pol);
     }
+    c = cn;
+    plane = nplane;
   }
 }
 

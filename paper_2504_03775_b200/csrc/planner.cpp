@@ -38,6 +38,10 @@ flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string
   if (row % 16) return fail(FLOWKV_ERR_ALIGN, "head_dim*elem_bytes is not a multiple of 16 bytes");
   if (row > (1u << 20)) return fail(FLOWKV_ERR_UNSUPPORTED, "row larger than 1 MiB");
   if ((uintptr_t)p->base % 16) return fail(FLOWKV_ERR_ALIGN, "base is not 16-byte aligned");
+  // rows mode addresses a chunk (<= one block) with 32-bit offsets
+  if ((uint64_t)p->stride_bytes[FLOWKV_S_TOKEN] * p->block_size + (uint64_t)p->stride_bytes[FLOWKV_S_HEAD] * p->num_kv_heads >=
+      (1ull << 32))
+    return fail(FLOWKV_ERR_UNSUPPORTED, "one block spans 4 GiB or more");
   for (int i = 0; i < 5; ++i) {
     if (p->stride_bytes[i] <= 0) return fail(FLOWKV_ERR_INVALID_ARG, "a stride is <= 0 (call flowkv_pool_strides)");
     if (p->stride_bytes[i] % 16) return fail(FLOWKV_ERR_ALIGN, "a stride is not a multiple of 16 bytes");
