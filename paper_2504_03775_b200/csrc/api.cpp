@@ -147,15 +147,20 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
     ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(n_tiles, 1));
     return;
   }
-  // defaults from the cfg2 sweep on B200 (profiles/r01_tuning_sweep.md): one CTA-wide round of
-  // 512 threads x 4 x 32 B covers a 64 KiB tile; the grid is oversubscribed 8x so that the hardware
-  // CTA scheduler evens out SM-to-SM speed differences.
+  // Defaults from the tuning sweeps on B200 (profiles/r01_tuning.md):
+  //  * one CTA-wide round of 512 threads x 4 x 32 B covers a 64 KiB tile;
+  //  * the grid is a grid-stride loop capped at 256 CTAs per SM.  Up to that cap every tile gets its
+  //    own CTA and the hardware CTA scheduler hands tiles to whichever SM frees up first, which
+  //    measured 3-6 % faster than an exactly-resident persistent grid with a static tile stride
+  //    (SMs do not all drain HBM at the same rate); beyond the cap each CTA strides over tiles;
+  //  * rows mode (strided rows) prefers 128-thread groups: four tiles in flight per CTA.
   ls.threads = t.threads ? t.threads : std::min<uint32_t>(512, std::max<uint32_t>(128, pl->tile_bytes / 128));
-  ls.group_threads = t.group_threads ? std::min(t.group_threads, ls.threads) : ls.threads;
+  const uint32_t group_auto = op.sched.mode == MODE_ROWS ? std::min<uint32_t>(128, ls.threads) : ls.threads;
+  ls.group_threads = t.group_threads ? std::min(t.group_threads, ls.threads) : group_auto;
   ls.hint = t.cache_hint ? t.cache_hint - 1 : 2;
   ls.n_stages = 0;
   ls.stage_bytes = 0;
-  const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 8;
+  const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 256;
   const uint32_t groups_per_cta = ls.threads / ls.group_threads;
   const uint64_t ctas_needed = (n_tiles + groups_per_cta - 1) / groups_per_cta;
   ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(ctas_needed, 1));
@@ -166,14 +171,14 @@ flowkv_status check_tuning(const flowkv_tuning& t) {
     return fail(FLOWKV_ERR_INVALID_ARG, "tuning.tile_bytes must be a power of two in [1 KiB, 1 MiB]");
   if (t.threads && (t.threads % 32 || t.threads > 512 || !is_pow2(t.threads)))
     return fail(FLOWKV_ERR_INVALID_ARG, "tuning.threads must be a power of two in [32, 512]");
-  const uint32_t thr = t.threads ? t.threads : 256;
+  const uint32_t thr = t.threads ? t.threads : 512;      // with threads on auto the group is clamped to it later
   if (t.group_threads && (!is_pow2(t.group_threads) || t.group_threads < 32 || t.group_threads > thr))
     return fail(FLOWKV_ERR_INVALID_ARG, "tuning.group_threads must be a power of two in [32, threads]");
   if (t.variant > FLOWKV_VARIANT_BULK) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.variant unknown");
   if (t.tile_order > 2) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.tile_order unknown");
   if (t.cache_hint > 3) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.cache_hint unknown");
   if (t.stages && (t.stages < 2 || t.stages > 16)) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.stages must be in [2,16]");
-  if (t.ctas_per_sm > 32) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.ctas_per_sm must be <= 32");
+  if (t.ctas_per_sm > 1024) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.ctas_per_sm must be <= 1024");
   if (t.variant == FLOWKV_VARIANT_BULK && t.tile_bytes > (64u << 10))
     return fail(FLOWKV_ERR_INVALID_ARG, "bulk variant: tile_bytes must be <= 64 KiB (two ring slots must fit in shared memory)");
   return FLOWKV_OK;
