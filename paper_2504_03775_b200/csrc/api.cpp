@@ -136,10 +136,13 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
     ls.group_threads = 32;
     ls.stage_bytes = std::max<uint32_t>(op.max_chunk_bytes, 1024);
     ls.stage_bytes = (ls.stage_bytes + 127) & ~127u;
-    const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 1;
+    // like the ldst path the grid is oversubscribed (<= 256 CTAs per SM) and each CTA's ring is short:
+    // several small CTAs per SM, scheduled by hardware, beat one long-lived CTA with a deep ring
+    const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 256;
     const uint32_t smem_cap = (pl->max_smem_optin ? pl->max_smem_optin : 232448) - 1024;
-    const uint32_t budget = std::min<uint32_t>(smem_cap, (228u * 1024 - 2048) / ctas - 1024);
-    uint32_t stages = t.stages ? t.stages : 16;
+    const uint32_t resident = std::min<uint32_t>(ctas, 3);
+    const uint32_t budget = std::min<uint32_t>(smem_cap, (228u * 1024 - 2048) / resident - 1024);
+    uint32_t stages = t.stages ? t.stages : 2;
     stages = std::min<uint32_t>(stages, 16);
     while (stages > 2 && (uint64_t)stages * ls.stage_bytes > budget) --stages;
     ls.n_stages = stages;
@@ -147,7 +150,7 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
     ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(n_tiles, 1));
     return;
   }
-  // Defaults from the tuning sweeps on B200 (profiles/r01_tuning.md):
+  // Defaults from the tuning sweeps on B200 (profiles/r01_ncu.md §4):
   //  * one CTA-wide round of 512 threads x 4 x 32 B covers a 64 KiB tile;
   //  * the grid is a grid-stride loop capped at 256 CTAs per SM.  Up to that cap every tile gets its
   //    own CTA and the hardware CTA scheduler hands tiles to whichever SM frees up first, which
