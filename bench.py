@@ -336,8 +336,11 @@ def run_ours(args) -> None:
 
         def e2e_step():
             plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
-            F.flowkv_pack(plan, host.data_ptr(), nbytes, s)          # device -> pinned host, one kernel
-            F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)        # pinned host -> device, one kernel
+            if args.e2e_serial:
+                F.flowkv_pack(plan, host.data_ptr(), nbytes, s)      # device -> pinned host, one kernel
+                F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)    # pinned host -> device, one kernel
+            else:                                                    # same result, both PCIe directions overlapped
+                F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, args.e2e_chunks, args.e2e_ctas, s)
             plan.destroy()
         e2e_step()
         barrier()
@@ -359,7 +362,10 @@ def run_ours(args) -> None:
             line["e2e"] = {"value": world * Ke * payload / (te * 1e-3) / 1e9, "unit": UNIT,
                            "h2d_bytes_per_step": nbytes + stats["plan_device_bytes"], "d2h_bytes_per_step": nbytes,
                            "steps": Ke, "ms_per_step": te / Ke,
-                           "path": "flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host",
+                           "path": ("flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host"
+                                    if args.e2e_serial else
+                                    "flowkv_plan (host tables) + flowkv_transfer_via_host: pack to pinned host and unpack "
+                                    "from it, pipelined over layer chunks on two streams"),
                            "link_memcpy_d2h_GBps": d2h, "link_memcpy_h2d_GBps": h2d}
         del host
 
@@ -408,6 +414,9 @@ def main() -> None:
     ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-serial", action="store_true", help="pack then unpack on one stream instead of the pipeline")
+    ap.add_argument("--e2e-chunks", type=int, default=0)
+    ap.add_argument("--e2e-ctas", type=int, default=0)
     ap.add_argument("--no-baselines", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run the configs[4] sweep instead (see bench_sweep.py)")

@@ -159,8 +159,9 @@ typedef struct {
 FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
 
 /* Build a plan: validate (a1), bidirectional segment alignment (a2), tile schedule (a3),
- * upload (a4; one cudaMallocAsync + one cudaMemcpyAsync from cached pinned memory, both on `stream`;
- * no host synchronisation, so planning batch k+1 overlaps the move of batch k).
+ * upload (a4; one cudaMallocAsync + one cudaMemcpyAsync from cached pinned memory on a library-owned
+ * upload stream; `stream` only waits on the upload's event.  No host synchronisation, so planning and
+ * uploading batch k+1 overlap the move of batch k).
  *   src, dst : HOST pointers to pool descriptors; either may be NULL (pack-only / unpack-only).
  *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
  *   tuning   : HOST pointer or NULL.
@@ -191,7 +192,28 @@ FLOWKV_API flowkv_status flowkv_transfer(const flowkv_plan_t* plan, void* stream
 FLOWKV_API flowkv_status flowkv_pack(const flowkv_plan_t* plan, void* staging, uint64_t bytes, void* stream);
 FLOWKV_API flowkv_status flowkv_unpack(const flowkv_plan_t* plan, const void* staging, uint64_t bytes, void* stream);
 
-FLOWKV_API /* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
+FLOWKV_API /* Layer-range variants (S§8f NEXT-2; the paper's "layerwise" ablation P:L222-224 and the overlap of transfer
+ * with prefill of later layers): only layers [layer_begin, layer_end) move; everything else —
+ * including the wire-format slabs of other layers in `staging` — is untouched.  One launch each
+ * (zero when the range is empty).  FLOWKV_ERR_INVALID_ARG if the range is not inside [0, num_layers]. */
+FLOWKV_API flowkv_status flowkv_transfer_layers(const flowkv_plan_t* plan, uint32_t layer_begin, uint32_t layer_end, void* stream);
+FLOWKV_API flowkv_status flowkv_pack_layers(const flowkv_plan_t* plan, void* staging, uint64_t bytes,
+                                            uint32_t layer_begin, uint32_t layer_end, void* stream);
+FLOWKV_API flowkv_status flowkv_unpack_layers(const flowkv_plan_t* plan, const void* staging, uint64_t bytes,
+                                              uint32_t layer_begin, uint32_t layer_end, void* stream);
+
+/* Pool -> pinned host -> pool with both PCIe directions busy at once (S§8f NEXT-3: chunked pinned-host
+ * pipeline; the host buffer stands in for the network endpoint, BASELINE.json north_star).  Result ==
+ * flowkv_pack(host_staging) followed by flowkv_unpack(host_staging).  The layers are cut into `n_chunks`
+ * groups (0 = min(L,16)); chunk c is packed on `stream`, and unpacked on a plan-owned second stream as soon as
+ * its pack has finished, so the D2H of chunk c+1 overlaps the H2D of chunk c.  `stream` is made to wait for
+ * the last unpack, so callers see ordinary stream order.  `ctas_per_kernel` caps each kernel's grid
+ * (0 = 64; a PCIe-bound kernel needs few CTAs and both kernels must be co-resident).
+ * Launches: 2 * n_chunks.  host_staging: mapped pinned HOST (or device) pointer, 16-B aligned. */
+FLOWKV_API flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* plan, void* host_staging, uint64_t bytes,
+                                                  uint32_t n_chunks, uint32_t ctas_per_kernel, void* stream);
+
+/* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
  * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,
  * synchronise that stream first.  NULL is ignored. */
 FLOWKV_API void flowkv_plan_destroy(flowkv_plan_t* plan);

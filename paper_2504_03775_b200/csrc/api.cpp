@@ -77,6 +77,22 @@ class PinnedCache {
 };
 PinnedCache g_pinned;
 
+// Plan uploads go through a library-owned non-blocking stream, so the upload for batch k+1 does not
+// queue behind the kernel that is moving batch k on the caller's stream; the caller's stream only
+// waits on the upload's event.  One stream per device, created on first use, never destroyed.
+std::mutex g_upload_mu;
+cudaStream_t g_upload_stream[64] = {};
+cudaError_t upload_stream(int device, cudaStream_t* out) {
+  if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(g_upload_mu);
+  if (!g_upload_stream[device]) {
+    cudaError_t e = cudaStreamCreateWithFlags(&g_upload_stream[device], cudaStreamNonBlocking);
+    if (e != cudaSuccess) return e;
+  }
+  *out = g_upload_stream[device];
+  return cudaSuccess;
+}
+
 struct Op {                  // one runnable operation of a plan
   Schedule sched;
   const Chunk* d_chunks = nullptr;
@@ -99,8 +115,11 @@ struct flowkv_plan_s {
   uint64_t n_requests = 0, total_tokens = 0;
   void* d_buf = nullptr;     // stream-ordered allocation on `stream`
   uint64_t d_bytes = 0;
-  cudaStream_t stream = nullptr;   // the stream flowkv_plan() was given: upload and free are ordered on it
-  PinnedBuf staging{};
+  cudaStream_t stream = nullptr;   // the stream flowkv_plan() was given: it waits on the upload; the free is ordered on it
+  PinnedBuf staging{};             // staging.ev = "upload done" event
+  // flowkv_transfer_via_host: second stream + events, created on first use (plans are logically const)
+  mutable cudaStream_t aux = nullptr;
+  mutable std::vector<cudaEvent_t> events;
   int device = -1;
   uint32_t num_sms = 0, max_smem_optin = 0;
 };
@@ -276,14 +295,18 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       }
 
     if (device) {
-      // a4: one stream-ordered allocation and ONE upload (from cached pinned memory) for all schedules
+      // a4: one stream-ordered allocation and ONE upload (from cached pinned memory) for all schedules,
+      // issued on the library's upload stream; the caller's stream waits on the upload event
       uint64_t bytes = 0;
       for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) bytes += op->sched.chunks.size() * sizeof(Chunk);
       pl->stream = (cudaStream_t)stream;
       if (bytes) {
-        cudaError_t e = g_pinned.acquire(bytes, pl->staging);
+        cudaStream_t up = nullptr;
+        cudaError_t e = upload_stream(pl->device, &up);
+        if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaStreamCreate(upload)"); }
+        e = g_pinned.acquire(bytes, pl->staging);
         if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaHostAlloc(plan staging)"); }
-        e = cudaMallocAsync(&pl->d_buf, bytes, pl->stream);
+        e = cudaMallocAsync(&pl->d_buf, bytes, up);
         if (e != cudaSuccess) { g_pinned.release(pl->staging); delete pl; return fail_cuda(e, "cudaMallocAsync(plan)"); }
         pl->d_bytes = bytes;
         uint64_t off = 0;
@@ -294,10 +317,11 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
           op->d_chunks = (const Chunk*)((char*)pl->d_buf + off);
           off += n;
         }
-        e = cudaMemcpyAsync(pl->d_buf, pl->staging.p, bytes, cudaMemcpyHostToDevice, pl->stream);
-        if (e == cudaSuccess) e = cudaEventRecord(pl->staging.ev, pl->stream);
+        e = cudaMemcpyAsync(pl->d_buf, pl->staging.p, bytes, cudaMemcpyHostToDevice, up);
+        if (e == cudaSuccess) e = cudaEventRecord(pl->staging.ev, up);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(pl->stream, pl->staging.ev, 0);
         if (e != cudaSuccess) {
-          cudaFreeAsync(pl->d_buf, pl->stream);
+          cudaFreeAsync(pl->d_buf, up);
           g_pinned.release(pl->staging);
           delete pl;
           return fail_cuda(e, "cudaMemcpyAsync(plan)");
@@ -335,14 +359,29 @@ Side dense_side(const void* staging, const Geometry& g) {
   return s;
 }
 
-flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Side& d, uint32_t vec_bytes, void* stream) {
+struct RunOpts {
+  bool ranged = false;                       // false: all layers
+  uint32_t layer_begin = 0, layer_end = 0;   // [begin, end) when ranged
+  uint32_t max_grid = 0;                     // 0 = the plan's launch shape
+};
+
+flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Side& d, uint32_t vec_bytes, void* stream,
+                  const RunOpts& ro = RunOpts()) {
   if (!pl->on_device) return fail(FLOWKV_ERR_UNSUPPORTED, "plan was built by flowkv_plan_host and cannot run");
-  if (op.sched.chunks.empty()) return FLOWKV_OK;       // A11: empty batch, zero launches
+  const uint32_t l0 = ro.ranged ? ro.layer_begin : 0, l1 = ro.ranged ? ro.layer_end : pl->g.L;
+  if (l0 > l1 || l1 > pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
+  if (op.sched.chunks.empty() || l0 == l1) return FLOWKV_OK;       // A11: nothing to move, zero launches
+  if ((cudaStream_t)stream != pl->stream && pl->staging.ev) {
+    // a stream other than the plan's own has not been ordered after the plan upload yet
+    cudaError_t e = cudaStreamWaitEvent((cudaStream_t)stream, pl->staging.ev, 0);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent(plan upload)");
+  }
   KernelParams kp{};
   kp.src = s; kp.dst = d;
   kp.chunks = op.d_chunks;
   kp.n_chunks = (uint32_t)op.sched.chunks.size();
-  kp.n_planes = 2 * pl->g.L;
+  kp.n_planes = 2 * (l1 - l0);
+  kp.plane0 = 2 * l0;
   kp.n_tiles = kp.n_chunks * kp.n_planes;
   kp.row_bytes = pl->g.row_bytes;
   kp.heads = pl->g.Hkv;
@@ -350,12 +389,25 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   kp.tile_order = op.tile_order;
   LaunchShape ls = op.shape;
   ls.vec_bytes = vec_bytes;
+  const uint32_t groups_per_cta = ls.variant == FLOWKV_VARIANT_BULK ? 1 : ls.threads / ls.group_threads;
+  ls.grid = std::min<uint32_t>(ls.grid, (kp.n_tiles + groups_per_cta - 1) / groups_per_cta);
+  if (ro.max_grid) ls.grid = std::min(ls.grid, ro.max_grid);
   kp.group_log2 = log2u(ls.group_threads);
   kp.vpr_log2 = log2_or_none(kp.row_bytes / ls.vec_bytes);
   kp.heads_log2 = log2_or_none(kp.heads);
   const int e = launch_copy(op.sched.mode, kp, ls, stream);
   if (e != 0) return fail_cuda((cudaError_t)e, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
+  return FLOWKV_OK;
+}
+
+flowkv_status check_staging(const flowkv_plan_t* pl, const Op& op, const void* staging, uint64_t bytes, const char* what) {
+  if (op.sched.mode == MODE_ABSENT)
+    return fail(FLOWKV_ERR_UNSUPPORTED, std::string("plan has no ") + what + " schedule");
+  if (op.sched.chunks.empty()) return FLOWKV_OK;
+  if (!staging) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
+  if ((uintptr_t)staging % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
+  if (bytes < pl->total_tokens * pl->g.bytes_per_token) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
   return FLOWKV_OK;
 }
 
@@ -431,39 +483,109 @@ flowkv_status flowkv_plan_info(const flowkv_plan_t* pl, flowkv_plan_stats* st, c
   return FLOWKV_OK;
 }
 
-flowkv_status flowkv_transfer(const flowkv_plan_t* pl, void* stream) {
+flowkv_status flowkv_transfer_layers(const flowkv_plan_t* pl, uint32_t layer_begin, uint32_t layer_end, void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
   if (pl->transfer.sched.mode == MODE_ABSENT)
     return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pool-to-pool schedule (needs both pools, no FLOWKV_PLAN_NO_TRANSFER)");
-  return run(pl, pl->transfer, pool_side(pl->src), pool_side(pl->dst), pl->transfer.shape.vec_bytes, stream);
+  RunOpts ro;
+  ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
+  return run(pl, pl->transfer, pool_side(pl->src), pool_side(pl->dst), pl->transfer.shape.vec_bytes, stream, ro);
+}
+
+flowkv_status flowkv_transfer(const flowkv_plan_t* pl, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  return flowkv_transfer_layers(pl, 0, pl->g.L, stream);
+}
+
+flowkv_status flowkv_pack_layers(const flowkv_plan_t* pl, void* staging, uint64_t bytes, uint32_t layer_begin,
+                                 uint32_t layer_end, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  flowkv_status st = check_staging(pl, pl->pack, staging, bytes, "pack");
+  if (st != FLOWKV_OK || pl->pack.sched.chunks.empty()) return st;
+  const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
+  RunOpts ro;
+  ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
+  return run(pl, pl->pack, pool_side(pl->src), dense_side(staging, pl->g), vec, stream, ro);
 }
 
 flowkv_status flowkv_pack(const flowkv_plan_t* pl, void* staging, uint64_t bytes, void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
-  if (pl->pack.sched.mode == MODE_ABSENT)
-    return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pack schedule (needs a src pool, no FLOWKV_PLAN_NO_PACK)");
-  if (pl->pack.sched.chunks.empty()) return FLOWKV_OK;
-  if (!staging) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
-  if ((uintptr_t)staging % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
-  if (bytes < pl->total_tokens * pl->g.bytes_per_token) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
-  const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
-  return run(pl, pl->pack, pool_side(pl->src), dense_side(staging, pl->g), vec, stream);
+  return flowkv_pack_layers(pl, staging, bytes, 0, pl->g.L, stream);
+}
+
+flowkv_status flowkv_unpack_layers(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, uint32_t layer_begin,
+                                   uint32_t layer_end, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  flowkv_status st = check_staging(pl, pl->unpack, staging, bytes, "unpack");
+  if (st != FLOWKV_OK || pl->unpack.sched.chunks.empty()) return st;
+  const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
+  RunOpts ro;
+  ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
+  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst), vec, stream, ro);
 }
 
 flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
-  if (pl->unpack.sched.mode == MODE_ABSENT)
-    return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no unpack schedule (needs a dst pool, no FLOWKV_PLAN_NO_UNPACK)");
-  if (pl->unpack.sched.chunks.empty()) return FLOWKV_OK;
-  if (!staging) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
-  if ((uintptr_t)staging % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
-  if (bytes < pl->total_tokens * pl->g.bytes_per_token) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
-  const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
-  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst), vec, stream);
+  return flowkv_unpack_layers(pl, staging, bytes, 0, pl->g.L, stream);
+}
+
+flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_staging, uint64_t bytes, uint32_t n_chunks,
+                                       uint32_t ctas_per_kernel, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  flowkv_status st = check_staging(pl, pl->pack, host_staging, bytes, "pack");
+  if (st != FLOWKV_OK) return st;
+  st = check_staging(pl, pl->unpack, host_staging, bytes, "unpack");
+  if (st != FLOWKV_OK) return st;
+  if (pl->pack.sched.chunks.empty()) return FLOWKV_OK;
+  if (!pl->on_device) return fail(FLOWKV_ERR_UNSUPPORTED, "plan was built by flowkv_plan_host and cannot run");
+  const uint32_t L = pl->g.L;
+  if (n_chunks == 0) n_chunks = std::min<uint32_t>(L, 16);   // measured on B200: 16 chunks x 64 CTAs (profiles/r01_sweep.md)
+  n_chunks = std::min(n_chunks, L);
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaError_t e;
+  if (!pl->aux) {
+    e = cudaStreamCreateWithFlags(&pl->aux, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaStreamCreate(aux)");
+  }
+  while (pl->events.size() < (size_t)n_chunks + 2) {
+    cudaEvent_t ev;
+    e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+    if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
+    pl->events.push_back(ev);
+  }
+  // the unpack side (aux) starts after everything already queued on the caller's stream
+  cudaEvent_t e_start = pl->events[n_chunks], e_done = pl->events[n_chunks + 1];
+  if ((e = cudaEventRecord(e_start, s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+  if ((e = cudaStreamWaitEvent(pl->aux, e_start, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+  const uint32_t vec = ((uintptr_t)host_staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
+  const uint32_t vecu = ((uintptr_t)host_staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
+  RunOpts ro;
+  ro.ranged = true;
+  ro.max_grid = ctas_per_kernel ? ctas_per_kernel : 64;   // a PCIe-bound kernel needs few CTAs; both must be co-resident
+  for (uint32_t c = 0; c < n_chunks; ++c) {
+    ro.layer_begin = (uint32_t)((uint64_t)L * c / n_chunks);
+    ro.layer_end = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
+    if (ro.layer_begin == ro.layer_end) continue;
+    st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);      // D2H on `stream`
+    if (st != FLOWKV_OK) return st;
+    if ((e = cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+    if ((e = cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+    st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, pl->aux, ro);   // H2D on aux
+    if (st != FLOWKV_OK) return st;
+  }
+  if ((e = cudaEventRecord(e_done, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+  if ((e = cudaStreamWaitEvent(s, e_done, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+  return FLOWKV_OK;
 }
 
 void flowkv_plan_destroy(flowkv_plan_t* pl) {
   if (!pl) return;
+  if (pl->aux) {
+    // via-host work on the aux stream was joined back into the caller's stream by an event, so the
+    // stream-ordered free below is already behind it; destroying a busy stream only defers its release
+    cudaStreamDestroy(pl->aux);
+  }
+  for (cudaEvent_t ev : pl->events) cudaEventDestroy(ev);
   if (pl->d_buf) cudaFreeAsync(pl->d_buf, pl->stream);   // ordered after everything queued on the plan's stream
   g_pinned.release(pl->staging);
   delete pl;

@@ -42,7 +42,8 @@ struct KernelParams {
   Side         src, dst;
   const Chunk* chunks;       // device
   uint32_t     n_chunks;     // per plane
-  uint32_t     n_planes;     // 2L
+  uint32_t     n_planes;     // planes this launch covers: 2*(layer_end - layer_begin)
+  uint32_t     plane0;       // first plane: 2*layer_begin
   uint32_t     n_tiles;      // n_chunks * n_planes
   uint32_t     row_bytes;    // Dh*e
   uint32_t     heads;        // Hkv

@@ -105,6 +105,7 @@ __device__ __forceinline__ int64_t plane_offset(const Side& s, uint32_t plane, u
 __device__ __forceinline__ void decode_tile(const KernelParams& p, uint32_t tile, uint32_t& plane, uint32_t& ci) {
   if (p.tile_order == 0) { plane = tile / p.n_chunks; ci = tile - plane * p.n_chunks; }
   else                   { ci = tile / p.n_planes;    plane = tile - ci * p.n_planes; }
+  plane += p.plane0;       // layer-range launches start at plane 2*layer_begin
 }
 
 // ------------------------------------------------------------------------------------------------

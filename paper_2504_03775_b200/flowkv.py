@@ -31,7 +31,8 @@ LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "stri
 
 EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
-           "flowkv_launch_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise"]
+           "flowkv_launch_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
+           "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host"]
 
 
 class flowkv_pool(C.Structure):
@@ -95,6 +96,10 @@ def _load() -> C.CDLL:
     lib.flowkv_transfer.argtypes = [C.c_void_p, C.c_void_p]
     lib.flowkv_pack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     lib.flowkv_unpack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+    lib.flowkv_transfer_layers.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.flowkv_pack_layers.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.flowkv_unpack_layers.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.flowkv_transfer_via_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
     lib.flowkv_plan_destroy.argtypes = [C.c_void_p]
     lib.flowkv_plan_destroy.restype = None
     lib.flowkv_status_string.argtypes = [C.c_int]
@@ -281,6 +286,24 @@ def flowkv_pack(plan: Plan, staging: int, nbytes: int, stream: int = 0) -> None:
 
 def flowkv_unpack(plan: Plan, staging: int, nbytes: int, stream: int = 0) -> None:
     _check(_lib.flowkv_unpack(plan.handle, C.c_void_p(staging), nbytes, C.c_void_p(stream)))
+
+
+def flowkv_transfer_layers(plan: Plan, layer_begin: int, layer_end: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_transfer_layers(plan.handle, layer_begin, layer_end, C.c_void_p(stream)))
+
+
+def flowkv_pack_layers(plan: Plan, staging: int, nbytes: int, layer_begin: int, layer_end: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_pack_layers(plan.handle, C.c_void_p(staging), nbytes, layer_begin, layer_end, C.c_void_p(stream)))
+
+
+def flowkv_unpack_layers(plan: Plan, staging: int, nbytes: int, layer_begin: int, layer_end: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_unpack_layers(plan.handle, C.c_void_p(staging), nbytes, layer_begin, layer_end, C.c_void_p(stream)))
+
+
+def flowkv_transfer_via_host(plan: Plan, host_staging: int, nbytes: int, n_chunks: int = 0, ctas_per_kernel: int = 0,
+                             stream: int = 0) -> None:
+    _check(_lib.flowkv_transfer_via_host(plan.handle, C.c_void_p(host_staging), nbytes, n_chunks, ctas_per_kernel,
+                                         C.c_void_p(stream)))
 
 
 def flowkv_plan_destroy(plan: Plan) -> None:

@@ -286,3 +286,77 @@ def test_baselines_reach_the_same_bytes_and_count_calls():
     torch.cuda.synchronize()
     assert calls == plan.stats["n_segments"] * 4
     G.assert_same(P.to_numpy(dp.dst_buf), exp, "segmentwise baseline")
+
+
+def test_layer_range_operations():
+    """flowkv_*_layers move exactly layers [l0,l1) (oracle: same loops restricted to those layers); an empty range
+    launches nothing; a range outside [0,L] is rejected; the union of ranges equals the full operation."""
+    w = synth.config4_hetero(n_requests=2, num_layers=5)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    gs, gd = G.geom(w.src, w.shape), G.geom(w.dst, w.shape)
+    plan = dp.plan()
+    nbytes = plan.stats["staging_bytes"]
+    staging = P.alloc_bytes(nbytes)
+    for l0, l1 in [(0, 0), (1, 3), (4, 5), (3, 3), (0, 5), (5, 5)]:
+        P.fill_sentinel(dp.dst_buf)
+        P.fill_sentinel(staging)
+        n0 = F.flowkv_launch_count()
+        F.flowkv_transfer_layers(plan, l0, l1)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if l1 > l0 else 0)
+        exp = np.full(dp.dst_buf.numel(), P.SENTINEL_BYTE, np.uint8)
+        for r in w.requests:
+            O.transfer(src_np, gs, exp, gd, r.src_blocks, r.dst_blocks, r.num_tokens, l0, l1)
+        G.assert_same(P.to_numpy(dp.dst_buf), exp, f"transfer_layers [{l0},{l1})")
+        # pack / unpack of the same range through the wire format
+        F.flowkv_pack_layers(plan, staging.data_ptr(), nbytes, l0, l1)
+        torch.cuda.synchronize()
+        exps = np.full(nbytes, P.SENTINEL_BYTE, np.uint8)
+        off = 0
+        for r in w.requests:
+            O.pack(src_np, gs, r.src_blocks, r.num_tokens, exps, off, l0, l1)
+            off += r.num_tokens
+        got_s = P.to_numpy(staging)
+        G.assert_same(got_s, exps, f"pack_layers [{l0},{l1})")
+        P.fill_sentinel(dp.dst_buf)
+        F.flowkv_unpack_layers(plan, staging.data_ptr(), nbytes, l0, l1)
+        torch.cuda.synchronize()
+        expu = np.full(dp.dst_buf.numel(), P.SENTINEL_BYTE, np.uint8)
+        off = 0
+        for r in w.requests:
+            O.unpack(got_s, off, expu, gd, r.dst_blocks, r.num_tokens, l0, l1)
+            off += r.num_tokens
+        G.assert_same(P.to_numpy(dp.dst_buf), expu, f"unpack_layers [{l0},{l1})")
+    for bad in [(2, 6), (3, 2), (6, 6)]:
+        with pytest.raises(F.FlowKVError) as ei:
+            F.flowkv_transfer_layers(plan, *bad)
+        assert ei.value.status == F.FLOWKV_ERR_INVALID_ARG
+    # union of disjoint ranges == the full transfer
+    P.fill_sentinel(dp.dst_buf)
+    for l0, l1 in [(3, 5), (0, 1), (1, 3)]:
+        F.flowkv_transfer_layers(plan, l0, l1)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "union of layer ranges")
+
+
+@pytest.mark.parametrize("n_chunks,ctas", [(0, 0), (1, 4), (3, 1), (100, 64)])
+def test_transfer_via_pinned_host_pipeline(n_chunks, ctas):
+    """pool -> pinned host -> pool with the two directions pipelined over layer chunks on two streams:
+    dst == oracle transfer, host buffer == oracle pack, caller's stream order is enough to see both."""
+    w = synth.config3_batched(n_requests=3, num_layers=6)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    stream = torch.cuda.Stream()
+    plan = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER, None, stream.cuda_stream)
+    nbytes = plan.stats["staging_bytes"]
+    host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    host.fill_(P.SENTINEL_BYTE)
+    n0 = F.flowkv_launch_count()
+    F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, n_chunks, ctas, stream.cuda_stream)
+    stream.synchronize()
+    chunks = min(n_chunks, 6) if n_chunks else 6          # auto = min(L, 16)
+    assert F.flowkv_launch_count() - n0 == 2 * chunks
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host: dst")
+    G.assert_same(host.numpy(), G.oracle_pack(w, src_np), "via host: wire bytes")
+    plan.destroy()
