@@ -236,6 +236,26 @@ FLOWKV_API flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const
                                         void* stream, uint64_t* n_calls);
 FLOWKV_API flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* plan, void* stream, uint64_t* n_calls);
 
+/* ---- segment-based block allocator (S§8f NEXT-1; §3.3) ----------------------------------
+ * "FlowKV manages free memory blocks with segment-based minimum heaps.  It chooses the right segments
+ *  during allocation to minimize waste and merges adjacent free segments during deallocation."
+ * Host-only (no CUDA).  A segment is a maximal run of consecutive free block ids.  Policy (A19):
+ *   allocate(n): if some free segment holds >= n blocks, take the first n blocks of the SMALLEST such
+ *   segment (ties: lowest start) — best fit, minimum waste, one segment.  Otherwise take whole free
+ *   segments, largest first (ties: lowest start), until the rest fits one segment, then best-fit the
+ *   rest — the fewest segments any choice can reach.  Ids are written in allocation order.
+ *   free(ids): blocks return to the free set; adjacent free segments merge.
+ * Errors: FLOWKV_ERR_NOMEM when fewer than n blocks are free (nothing is taken);
+ *         FLOWKV_ERR_BLOCK_OOB / FLOWKV_ERR_INVALID_ARG for ids out of range / not currently allocated
+ *         (nothing is freed).  All pointers are HOST pointers. */
+typedef struct flowkv_allocator_s flowkv_allocator_t;
+FLOWKV_API flowkv_status flowkv_alloc_create(uint32_t num_blocks, flowkv_allocator_t** out);
+FLOWKV_API flowkv_status flowkv_alloc_allocate(flowkv_allocator_t* a, uint32_t n, int32_t* out_ids, uint32_t* n_segments);
+FLOWKV_API flowkv_status flowkv_alloc_free(flowkv_allocator_t* a, const int32_t* ids, uint32_t n);
+FLOWKV_API flowkv_status flowkv_alloc_stats(const flowkv_allocator_t* a, uint32_t* free_blocks, uint32_t* free_segments,
+                                            uint32_t* largest_segment);
+FLOWKV_API void flowkv_alloc_destroy(flowkv_allocator_t* a);
+
 #ifdef __cplusplus
 }
 #endif

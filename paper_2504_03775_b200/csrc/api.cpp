@@ -21,6 +21,11 @@ flowkv_status fail(flowkv_status s, const std::string& msg) {
   g_last_error = msg;
   return s;
 }
+}  // namespace
+namespace flowkv {
+void set_last_error(const std::string& msg) { g_last_error = msg; }   // for the other translation units
+}
+namespace {
 flowkv_status fail_cuda(cudaError_t e, const char* what) {
   g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
   return FLOWKV_ERR_CUDA;

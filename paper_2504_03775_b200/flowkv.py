@@ -32,7 +32,9 @@ LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "stri
 EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
            "flowkv_launch_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
-           "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host"]
+           "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host",
+           "flowkv_alloc_create", "flowkv_alloc_allocate", "flowkv_alloc_free", "flowkv_alloc_stats",
+           "flowkv_alloc_destroy"]
 
 
 class flowkv_pool(C.Structure):
@@ -111,8 +113,15 @@ def _load() -> C.CDLL:
     lib.flowkv_baseline_blockwise.argtypes = [P(flowkv_pool), P(flowkv_pool), P(flowkv_request), C.c_uint32,
                                               C.c_void_p, P(C.c_uint64)]
     lib.flowkv_baseline_segmentwise.argtypes = [C.c_void_p, C.c_void_p, P(C.c_uint64)]
+    lib.flowkv_alloc_create.argtypes = [C.c_uint32, P(C.c_void_p)]
+    lib.flowkv_alloc_allocate.argtypes = [C.c_void_p, C.c_uint32, C.c_void_p, P(C.c_uint32)]
+    lib.flowkv_alloc_free.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32]
+    lib.flowkv_alloc_stats.argtypes = [C.c_void_p, P(C.c_uint32), P(C.c_uint32), P(C.c_uint32)]
+    lib.flowkv_alloc_destroy.argtypes = [C.c_void_p]
+    lib.flowkv_alloc_destroy.restype = None
     for n in EXPORTS:
-        if n not in ("flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error", "flowkv_launch_count"):
+        if n not in ("flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error", "flowkv_launch_count",
+                     "flowkv_alloc_destroy"):
             getattr(lib, n).restype = C.c_int
     return lib
 
@@ -322,3 +331,39 @@ def flowkv_baseline_segmentwise(plan: Plan, stream: int = 0) -> int:
     calls = C.c_uint64()
     _check(_lib.flowkv_baseline_segmentwise(plan.handle, C.c_void_p(stream), C.byref(calls)))
     return int(calls.value)
+
+
+class Allocator:
+    """Owner of a ``flowkv_allocator_t*`` (segment-based block allocator)."""
+
+    def __init__(self, num_blocks: int):
+        h = C.c_void_p()
+        _check(_lib.flowkv_alloc_create(num_blocks, C.byref(h)))
+        self._h = h
+
+    def allocate(self, n: int):
+        """-> (int32 ids in allocation order, number of segments used)"""
+        ids = np.empty(max(n, 1), dtype=np.int32)
+        segs = C.c_uint32()
+        _check(_lib.flowkv_alloc_allocate(self._h, n, ids.ctypes.data, C.byref(segs)))
+        return ids[:n].copy(), int(segs.value)
+
+    def free(self, ids) -> None:
+        a = np.ascontiguousarray(np.asarray(ids, dtype=np.int32))
+        _check(_lib.flowkv_alloc_free(self._h, a.ctypes.data if a.size else None, a.size))
+
+    def stats(self) -> dict:
+        fb, fs, lg = C.c_uint32(), C.c_uint32(), C.c_uint32()
+        _check(_lib.flowkv_alloc_stats(self._h, C.byref(fb), C.byref(fs), C.byref(lg)))
+        return {"free_blocks": fb.value, "free_segments": fs.value, "largest_segment": lg.value}
+
+    def destroy(self) -> None:
+        if self._h:
+            _lib.flowkv_alloc_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
