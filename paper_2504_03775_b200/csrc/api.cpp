@@ -267,7 +267,8 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
     // tile size: default 64 KiB; shrink for small batches so every SM gets several tiles
     uint32_t tile = tn.tile_bytes;
     if (!tile) {
-      tile = 64u << 10;
+      // ldst: one CTA-wide round of 512 threads; bulk: 2 ring slots x 32 KiB keep 3 CTAs resident per SM
+      tile = tn.variant == FLOWKV_VARIANT_BULK ? (32u << 10) : (64u << 10);
       const uint64_t want_tiles = 8ull * pl->num_sms;
       const uint64_t payload = pl->total_tokens * g.bytes_per_token;
       while (tile > 4096 && payload / tile < want_tiles) tile >>= 1;
