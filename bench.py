@@ -107,6 +107,10 @@ def build_workload(name: str, free_bytes: int):
         return (synth.config2_llama8b_13k(),
                 "configs[1] Llama-3-8B KV: 32 layers, 8 KV heads, head_dim 128, bf16, block 16, 1 x 13,312 tokens, "
                 "src 16,384-block pool (32 GiB) runs~Geom(mean 4), dst contiguous")
+    if name in ("cfg2bm", "cfg2bm_ragged"):
+        w = synth.config2_blockmajor("blkthd", tokens=13312 if name == "cfg2bm" else 13307)
+        return w, ("configs[1] request and tables, both pools in the paper's (B,L,2,H) order (Eq. 5; BLKTHD): "
+                   f"1 x {w.total_tokens} tokens, whole-block runs move as flat 2 MiB-per-block spans")
     if name == "cfg3":
         w = synth.config3_batched(budget_bytes=budget)
         return w, (f"configs[2] batched Llama-3-8B KV: first {w.notes['n_requests']} of 64 requests (fit rule), "
@@ -266,8 +270,10 @@ def run_ours(args) -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
+    XFER_ONLY = F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK      # the step moves pool -> pool only
+
     def step(ev_a=None, ev_b=None):
-        plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)     # a1-a4 (upload is stream-ordered)
+        plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, XFER_ONLY, tuning, s)   # a1-a4 (upload is stream-ordered)
         if ev_a is not None:
             ev_a.record(stream)
         F.flowkv_transfer(plan, s)                                           # a5: ONE launch
@@ -277,7 +283,7 @@ def run_ours(args) -> None:
 
     for _ in range(max(W, 3)):
         step()
-    plan0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)
+    plan0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, XFER_ONLY, tuning, s)
     stats = plan0.stats
     plan0.destroy()
     ka = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
@@ -312,7 +318,7 @@ def run_ours(args) -> None:
                        "payload_bytes": payload, "segments": stats["n_segments"],
                        "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
                        if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
-                       "step": "flowkv_plan + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM",
+                       "step": "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM",
                        "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
                                                         "vec_bytes", "cache_hint", "tile_order", "stages")}},
             "clocks": clk,
@@ -322,7 +328,7 @@ def run_ours(args) -> None:
             "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": load_traffic(w.name), "peak_source": peak_src,
-                         "kernel": "fk_span_ldst" if stats["mode_transfer"] == 1 else "fk_rows_ldst",
+                         "kernel": {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]],
                          "kernel_ms_avg": kern_ms, "kernel_ms_min": kern_min_ms,
                          "algorithmic_bytes_per_launch": 2 * payload,
                          "kernel_share_of_step": kern_ms / (t_ms / K)},
@@ -373,7 +379,7 @@ def run_ours(args) -> None:
     if rank == 0 and not args.no_baselines:
         extra = {}
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        if stats["mode_transfer"] == 1 and w.src.block_size == w.dst.block_size:
+        if stats["mode_transfer"] in (1, 3) and w.src.block_size == w.dst.block_size:
             for name, fn in (("blockwise_memcpy", lambda: F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests, s)),):
                 fn(); torch.cuda.synchronize()
                 t0 = time.perf_counter(); a.record(stream); calls = fn(); b.record(stream); torch.cuda.synchronize()
@@ -410,7 +416,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg2bm", "cfg2bm_ragged", "cfg3", "cfg4"])
     ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")

@@ -80,7 +80,7 @@ def main(argv=None) -> None:
             reqs = [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks)]
             payload = w.payload_bytes
             do_flush = 2 * payload < (256 << 20)
-            plan = F.flowkv_plan(src, dst, reqs, 0, tuning, s)
+            plan = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, tuning, s)
             st = plan.stats
             for _ in range(3):
                 plan.transfer(s)
@@ -95,7 +95,7 @@ def main(argv=None) -> None:
                     flush.zero_()
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
-                p2 = F.flowkv_plan(src, dst, reqs, 0, tuning, s)
+                p2 = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, tuning, s)
                 p2.transfer(s)
                 torch.cuda.synchronize()
                 lat.append((time.perf_counter() - t0) * 1e3)

@@ -66,11 +66,14 @@ typedef enum {
 /* Pool layouts.  `dim` (head_dim elements of elem_bytes) is always innermost and contiguous.
  *   LKBTHD  [layer][K|V][block][token][head][dim]  — Eq. 5 left side  (L,2,B,H), H=[token][head][dim]
  *   BLKHTD  [block][layer][K|V][head][token][dim]  — Eq. 5 right side (B,L,2,H), H=[head][token][dim]
- *   STRIDED caller fills stride_bytes[] itself (separate K and V tensors, padded blocks, ...).    */
+ *   STRIDED caller fills stride_bytes[] itself (separate K and V tensors, padded blocks, ...).
+ *   BLKTHD  [block][layer][K|V][token][head][dim]  — Eq. 5 right side (B,L,2,H) with H exactly as on the
+ *           left side: the paper's own re-order, which only moves the block axis outwards.          */
 typedef enum {
   FLOWKV_LAYOUT_LKBTHD = 0,
   FLOWKV_LAYOUT_BLKHTD = 1,
-  FLOWKV_LAYOUT_STRIDED = 2
+  FLOWKV_LAYOUT_STRIDED = 2,
+  FLOWKV_LAYOUT_BLKTHD = 3
 } flowkv_layout;
 
 enum { FLOWKV_S_LAYER = 0, FLOWKV_S_KV = 1, FLOWKV_S_BLOCK = 2, FLOWKV_S_TOKEN = 3, FLOWKV_S_HEAD = 4 };
@@ -129,7 +132,10 @@ typedef struct {
   uint32_t tile_order;      /* 0 = auto, 1 = plane-major (all tiles of plane 0, then plane 1, ...), 2 = chunk-major */
   uint32_t cache_hint;      /* ldst: 0 = auto, 1 = default caching, 2 = L1::no_allocate, 3 = + L2::evict_first */
   uint32_t stages;          /* bulk: ring depth (0 = auto; 2..16)                                   */
-  uint32_t _reserved[3];
+  uint32_t plan_in_params;  /* 0 = auto: a plan whose schedules have <= 96 entries each is passed in the kernel
+                             *     parameters (no device allocation, no upload; plan_device_bytes == 0);
+                             * 1 = always upload                                                    */
+  uint32_t _reserved[2];
 } flowkv_tuning;
 
 typedef enum {
@@ -147,21 +153,24 @@ typedef struct {
   uint64_t n_chunks_transfer, n_chunks_pack, n_chunks_unpack;  /* schedule entries per plane         */
   uint64_t plan_device_bytes;               /* descriptor bytes resident on the device              */
   uint32_t n_planes;                        /* 2*L                                                  */
-  uint32_t mode_transfer, mode_pack, mode_unpack;   /* 0 = absent, 1 = span (contiguous), 2 = rows  */
+  uint32_t mode_transfer, mode_pack, mode_unpack;   /* 0 = absent, 1 = span (contiguous per plane), 2 = rows,
+                                                     * 3 = flat (block-major both sides, same interior: a run of
+                                                     *     whole blocks is one byte range over all layers, Eq. 5) */
   uint32_t grid, threads, group_threads, tile_bytes, variant, vec_bytes;   /* launch shape in use   */
   uint32_t tile_order, cache_hint, stages, smem_bytes;                     /* (resolved, not 0)     */
   uint32_t num_sms;
-  uint32_t _reserved;
+  uint32_t n_flat_chunks;                   /* mode 3: whole-block byte ranges (no plane term; <= 32 tiles each) among n_chunks_transfer */
 } flowkv_plan_stats;
 
-/* Fill stride_bytes[] of a LKBTHD / BLKHTD pool from its shape.  STRIDED: validates only.
+/* Fill stride_bytes[] of a LKBTHD / BLKHTD / BLKTHD pool from its shape.  STRIDED: validates only.
  * pool: HOST pointer, read-write. */
 FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
 
 /* Build a plan: validate (a1), bidirectional segment alignment (a2), tile schedule (a3),
  * upload (a4; one cudaMallocAsync + one cudaMemcpyAsync from cached pinned memory on a library-owned
  * upload stream; `stream` only waits on the upload's event.  No host synchronisation, so planning and
- * uploading batch k+1 overlap the move of batch k).
+ * uploading batch k+1 overlap the move of batch k.  Small plans are not uploaded at all: their schedule
+ * travels in the kernel parameters, see flowkv_tuning.plan_in_params).
  *   src, dst : HOST pointers to pool descriptors; either may be NULL (pack-only / unpack-only).
  *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
  *   tuning   : HOST pointer or NULL.
@@ -192,7 +201,7 @@ FLOWKV_API flowkv_status flowkv_transfer(const flowkv_plan_t* plan, void* stream
 FLOWKV_API flowkv_status flowkv_pack(const flowkv_plan_t* plan, void* staging, uint64_t bytes, void* stream);
 FLOWKV_API flowkv_status flowkv_unpack(const flowkv_plan_t* plan, const void* staging, uint64_t bytes, void* stream);
 
-FLOWKV_API /* Layer-range variants (S§8f NEXT-2; the paper's "layerwise" ablation P:L222-224 and the overlap of transfer
+/* Layer-range variants (S§8f NEXT-2; the paper's "layerwise" ablation P:L222-224 and the overlap of transfer
  * with prefill of later layers): only layers [layer_begin, layer_end) move; everything else —
  * including the wire-format slabs of other layers in `staging` — is untouched.  One launch each
  * (zero when the range is empty).  FLOWKV_ERR_INVALID_ARG if the range is not inside [0, num_layers]. */
@@ -226,11 +235,13 @@ FLOWKV_API uint64_t flowkv_launch_count(void);
 
 /* ---- comparison baselines (BASELINE.json north_star; they are NOT the product path) ----------
  * Each issues cudaMemcpyAsync D2D copies on `stream` and writes the number issued to *n_calls.
- * They require same-layout, token-major pools (LKBTHD or equivalent strides) and equal block sizes.
- *   blockwise : one copy per (block, layer, K|V) — the pre-optimisation scheme of P:L92/L103;
- *               a partial last block copies only its valid tokens.
- *   segmentwise: one copy per (aligned segment, layer, K|V) — the paper's coalescing
- *               with cudaMemcpyAsync in place of ncclSend/ncclRecv.                              */
+ * They require equal block sizes and either two token-major pools (LKBTHD or equivalent strides) or two
+ * block-major pools with the same interior (BLKHTD/BLKTHD; FLOWKV_ERR_UNSUPPORTED otherwise).
+ *   blockwise : the pre-optimisation scheme of P:L92/L103 — one copy per (block, layer, K|V) for token-major
+ *               pools; for (B,L,2,H) pools one copy per whole block (Eq. 5 makes a block one range).  A partial
+ *               last block copies only its valid tokens (per plane; per plane and head when head-major).
+ *   segmentwise: the paper's coalescing with cudaMemcpyAsync in place of ncclSend/ncclRecv — one copy
+ *               per (aligned segment, layer, K|V); for (B,L,2,H) pools ONE copy per segment (Fig. 5).    */
 FLOWKV_API flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_pool* dst,
                                         const flowkv_request* reqs, uint32_t n_reqs,
                                         void* stream, uint64_t* n_calls);

@@ -73,6 +73,7 @@ class PoolGeom:
     The two named orders of Eq. 5:
       ``lkbthd``  [layer][K|V][block][token][head][dim]   — (L,2,B,H), H=[token][head][dim]
       ``blkhtd``  [block][layer][K|V][head][token][dim]   — (B,L,2,H), H=[head][token][dim]
+      ``blkthd``  [block][layer][K|V][token][head][dim]   — (B,L,2,H), H=[token][head][dim]
     """
     num_layers: int
     num_kv_heads: int
@@ -100,6 +101,16 @@ class PoolGeom:
         s_token = Dh * e
         s_head = BS * s_token
         s_kv = Hkv * s_head
+        s_layer = 2 * s_kv
+        s_block = L * s_layer
+        return PoolGeom(L, Hkv, Dh, e, NB, BS, s_layer, s_kv, s_block, s_token, s_head)
+
+    @staticmethod
+    def blkthd(L, Hkv, Dh, e, NB, BS) -> "PoolGeom":
+        """(B,L,2,H) with H=[token][head][dim]: Eq. 5's right side with H untouched."""
+        s_head = Dh * e
+        s_token = Hkv * s_head
+        s_kv = BS * s_token
         s_layer = 2 * s_kv
         s_block = L * s_layer
         return PoolGeom(L, Hkv, Dh, e, NB, BS, s_layer, s_kv, s_block, s_token, s_head)

@@ -104,6 +104,7 @@ struct Op {                  // one runnable operation of a plan
   LaunchShape shape{};
   uint32_t tile_order = 0;   // resolved: 0 plane-major, 1 chunk-major
   uint32_t max_chunk_bytes = 0;
+  bool in_params = false;    // schedule small enough to ride in the kernel parameters (no upload)
 };
 
 }  // namespace
@@ -151,10 +152,13 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
   ls.variant = t.variant ? t.variant : FLOWKV_VARIANT_LDST;
   if (op.sched.mode != MODE_SPAN) ls.variant = FLOWKV_VARIANT_LDST;   // bulk handles contiguous chunks only
   op.max_chunk_bytes = 0;
-  for (const Chunk& c : op.sched.chunks)
+  for (size_t i = 0; i < op.sched.chunks.size(); ++i) {
+    const Chunk& c = op.sched.chunks[i];
+    if (op.sched.mode == MODE_FLAT && i < op.sched.n_flat) continue;     // cut into flat_tile pieces by the kernel
     op.max_chunk_bytes = std::max(op.max_chunk_bytes, op.sched.mode == MODE_SPAN ? c.n : c.n * pl->g.tok_bytes);
+  }
   op.tile_order = t.tile_order == 2 ? 1 : 0;
-  const uint64_t n_tiles = (uint64_t)op.sched.chunks.size() * 2 * pl->g.L;
+  const uint64_t n_tiles = ((uint64_t)op.sched.n_flat << op.sched.flat_shift) + (uint64_t)op.sched.n_per_plane() * 2 * pl->g.L;
   if (ls.variant == FLOWKV_VARIANT_BULK) {
     ls.threads = 32;
     ls.group_threads = 32;
@@ -206,6 +210,7 @@ flowkv_status check_tuning(const flowkv_tuning& t) {
   if (t.cache_hint > 3) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.cache_hint unknown");
   if (t.stages && (t.stages < 2 || t.stages > 16)) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.stages must be in [2,16]");
   if (t.ctas_per_sm > 1024) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.ctas_per_sm must be <= 1024");
+  if (t.plan_in_params > 1) return fail(FLOWKV_ERR_INVALID_ARG, "tuning.plan_in_params unknown");
   if (t.variant == FLOWKV_VARIANT_BULK && t.tile_bytes > (64u << 10))
     return fail(FLOWKV_ERR_INVALID_ARG, "bulk variant: tile_bytes must be <= 64 KiB (two ring slots must fit in shared memory)");
   return FLOWKV_OK;
@@ -295,7 +300,7 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       resolve_shape(pl, pl->unpack, nullptr, dst);
     }
     for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack})
-      if ((uint64_t)op->sched.chunks.size() * 2 * g.L >= (1ull << 31)) {
+      if ((uint64_t)op->sched.chunks.size() * 2 * g.L + ((uint64_t)op->sched.n_flat << op->sched.flat_shift) >= (1ull << 31)) {
         delete pl;
         return fail(FLOWKV_ERR_UNSUPPORTED, "more than 2^31 tiles in one batch; split the batch");
       }
@@ -303,10 +308,18 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
     if (device) {
       // a4: one stream-ordered allocation and ONE upload (from cached pinned memory) for all schedules,
       // issued on the library's upload stream; the caller's stream waits on the upload event
+      // Small plans (every schedule <= kInlineChunks entries) skip all of that: their entries are passed by
+      // value in the kernel parameters at launch, so nothing stands between planning and the launch.
       uint64_t bytes = 0;
-      for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) bytes += op->sched.chunks.size() * sizeof(Chunk);
+      bool small = tn.plan_in_params != 1;
+      for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) {
+        bytes += op->sched.chunks.size() * sizeof(Chunk);
+        small = small && op->sched.chunks.size() <= kInlineChunks;
+      }
       pl->stream = (cudaStream_t)stream;
-      if (bytes) {
+      if (small) {
+        for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) op->in_params = true;
+      } else if (bytes) {
         cudaStream_t up = nullptr;
         cudaError_t e = upload_stream(pl->device, &up);
         if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaStreamCreate(upload)"); }
@@ -384,11 +397,23 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   }
   KernelParams kp{};
   kp.src = s; kp.dst = d;
-  kp.chunks = op.d_chunks;
-  kp.n_chunks = (uint32_t)op.sched.chunks.size();
+  Mode mode = op.sched.mode;
+  uint32_t first = 0;                      // first schedule entry this launch uses
+  kp.n_chunks = op.sched.n_per_plane();
+  kp.n_flat = op.sched.n_flat;
+  kp.flat_shift = op.sched.flat_shift;
+  kp.flat_tile = op.sched.flat_tile;
+  if (mode == MODE_FLAT && (l0 != 0 || l1 != pl->g.L)) {
+    // a layer range of a block-major pool is not one byte range per block run: use the plan's
+    // complete rows-mode schedule (third part of the chunk list)
+    mode = MODE_ROWS;
+    first = op.sched.n_flat + op.sched.n_ragged;
+    kp.n_chunks = (uint32_t)op.sched.chunks.size() - first;
+    kp.n_flat = 0;
+  }
   kp.n_planes = 2 * (l1 - l0);
   kp.plane0 = 2 * l0;
-  kp.n_tiles = kp.n_chunks * kp.n_planes;
+  kp.n_tiles = (kp.n_flat << kp.flat_shift) + kp.n_chunks * kp.n_planes;
   kp.row_bytes = pl->g.row_bytes;
   kp.heads = pl->g.Hkv;
   kp.tok_bytes = pl->g.tok_bytes;
@@ -401,7 +426,9 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   kp.group_log2 = log2u(ls.group_threads);
   kp.vpr_log2 = log2_or_none(kp.row_bytes / ls.vec_bytes);
   kp.heads_log2 = log2_or_none(kp.heads);
-  const int e = launch_copy(op.sched.mode, kp, ls, stream);
+  const int e = op.in_params
+                    ? launch_copy(mode, kp, nullptr, op.sched.chunks.data() + first, (uint32_t)op.sched.chunks.size() - first, ls, stream)
+                    : launch_copy(mode, kp, op.d_chunks + first, nullptr, 0, ls, stream);
   if (e != 0) return fail_cuda((cudaError_t)e, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return FLOWKV_OK;
@@ -436,6 +463,12 @@ flowkv_status flowkv_pool_strides(flowkv_pool* p) {
     p->stride_bytes[FLOWKV_S_KV] = p->stride_bytes[FLOWKV_S_HEAD] * p->num_kv_heads;
     p->stride_bytes[FLOWKV_S_LAYER] = 2 * p->stride_bytes[FLOWKV_S_KV];
     p->stride_bytes[FLOWKV_S_BLOCK] = p->stride_bytes[FLOWKV_S_LAYER] * p->num_layers;
+  } else if (p->layout == FLOWKV_LAYOUT_BLKTHD) {
+    p->stride_bytes[FLOWKV_S_HEAD] = row;
+    p->stride_bytes[FLOWKV_S_TOKEN] = row * p->num_kv_heads;
+    p->stride_bytes[FLOWKV_S_KV] = p->stride_bytes[FLOWKV_S_TOKEN] * p->block_size;
+    p->stride_bytes[FLOWKV_S_LAYER] = 2 * p->stride_bytes[FLOWKV_S_KV];
+    p->stride_bytes[FLOWKV_S_BLOCK] = p->stride_bytes[FLOWKV_S_LAYER] * p->num_layers;
   } else if (p->layout != FLOWKV_LAYOUT_STRIDED) {
     return fail(FLOWKV_ERR_INVALID_ARG, "unknown layout");
   }
@@ -463,7 +496,10 @@ flowkv_status flowkv_plan_info(const flowkv_plan_t* pl, flowkv_plan_stats* st, c
     st->total_tokens = pl->total_tokens;
     st->payload_bytes = pl->total_tokens * pl->g.bytes_per_token;
     st->staging_bytes = st->payload_bytes;
-    st->n_chunks_transfer = pl->transfer.sched.chunks.size();
+    st->n_chunks_transfer = pl->transfer.sched.mode == MODE_FLAT
+                                ? pl->transfer.sched.n_flat + pl->transfer.sched.n_ragged
+                                : pl->transfer.sched.chunks.size();
+    st->n_flat_chunks = pl->transfer.sched.n_flat;
     st->n_chunks_pack = pl->pack.sched.chunks.size();
     st->n_chunks_unpack = pl->unpack.sched.chunks.size();
     st->plan_device_bytes = pl->d_bytes;
@@ -619,6 +655,32 @@ const char* flowkv_last_error(void) { return g_last_error.c_str(); }
 uint64_t flowkv_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 // ---- comparison baselines: many cudaMemcpyAsync calls (NOT the product path) --------------------
+namespace {
+// n tokens starting at token slot (block, off) on each side, every plane: the fewest contiguous copies the
+// interior order allows (token-major: one per plane; head-major: one per plane and head).
+flowkv_status memcpy_tokens(const flowkv_pool& S, const flowkv_pool& D, const Geometry& g, uint32_t sb, uint32_t so,
+                            uint32_t db, uint32_t dof, uint32_t n, cudaStream_t st, uint64_t& calls) {
+  auto token_major = [&](const flowkv_pool& p) {
+    return p.stride_bytes[FLOWKV_S_HEAD] == (int64_t)g.row_bytes && p.stride_bytes[FLOWKV_S_TOKEN] == (int64_t)g.tok_bytes;
+  };
+  auto head_major = [&](const flowkv_pool& p) { return p.stride_bytes[FLOWKV_S_TOKEN] == (int64_t)g.row_bytes; };
+  const bool tm = token_major(S) && token_major(D), hm = head_major(S) && head_major(D);
+  if (!tm && !hm) return fail(FLOWKV_ERR_UNSUPPORTED, "memcpy baseline: block interiors are neither both token-major nor both head-major");
+  for (uint32_t l = 0; l < g.L; ++l)
+    for (uint32_t c = 0; c < 2; ++c)
+      for (uint32_t h = 0; h < (tm ? 1u : g.Hkv); ++h) {
+        const char* s = (const char*)S.base + l * S.stride_bytes[0] + c * S.stride_bytes[1] + (int64_t)sb * S.stride_bytes[2] +
+                        (int64_t)so * S.stride_bytes[3] + (int64_t)h * S.stride_bytes[4];
+        char* d = (char*)D.base + l * D.stride_bytes[0] + c * D.stride_bytes[1] + (int64_t)db * D.stride_bytes[2] +
+                  (int64_t)dof * D.stride_bytes[3] + (int64_t)h * D.stride_bytes[4];
+        cudaError_t e = cudaMemcpyAsync(d, s, (size_t)n * (tm ? g.tok_bytes : g.row_bytes), cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
+        ++calls;
+      }
+  return FLOWKV_OK;
+}
+}  // namespace
+
 flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,
                                         uint32_t n_reqs, void* stream, uint64_t* n_calls) {
   if (!src || !dst || (n_reqs && !reqs)) return fail(FLOWKV_ERR_INVALID_ARG, "NULL argument");
@@ -630,23 +692,27 @@ flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_poo
   Geometry g{};
   g.L = src->num_layers; g.Hkv = src->num_kv_heads; g.Dh = src->head_dim; g.e = src->elem_bytes;
   g.row_bytes = g.Dh * g.e; g.tok_bytes = g.Hkv * g.row_bytes; g.bytes_per_token = 2ull * g.L * g.tok_bytes;
-  if (src->block_size != dst->block_size || !pool_is_span_capable(*src, g) || !pool_is_span_capable(*dst, g))
-    return fail(FLOWKV_ERR_UNSUPPORTED, "blockwise baseline needs equal block sizes and token-major pools");
+  const bool span = pool_is_span_capable(*src, g) && pool_is_span_capable(*dst, g);
+  const bool flat = !span && pools_are_flat_congruent(*src, *dst, g);
+  if (src->block_size != dst->block_size || (!span && !flat))
+    return fail(FLOWKV_ERR_UNSUPPORTED, "blockwise baseline needs equal block sizes and two token-major pools, or two "
+                                        "block-major pools with the same interior");
   uint64_t calls = 0;
   const uint32_t bs = src->block_size;
   for (uint32_t r = 0; r < n_reqs; ++r)
     for (uint32_t b = 0; b < reqs[r].n_src_blocks; ++b) {
       const uint32_t ntok = std::min(bs, reqs[r].num_tokens - b * bs);
-      for (uint32_t l = 0; l < g.L; ++l)
-        for (uint32_t c = 0; c < 2; ++c) {
-          const char* s = (const char*)src->base + l * src->stride_bytes[0] + c * src->stride_bytes[1] +
-                          (int64_t)reqs[r].src_blocks[b] * src->stride_bytes[2];
-          char* d = (char*)dst->base + l * dst->stride_bytes[0] + c * dst->stride_bytes[1] +
-                    (int64_t)reqs[r].dst_blocks[b] * dst->stride_bytes[2];
-          cudaError_t e = cudaMemcpyAsync(d, s, (size_t)ntok * g.tok_bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
-          if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
-          ++calls;
-        }
+      const uint32_t sb = (uint32_t)reqs[r].src_blocks[b], db = (uint32_t)reqs[r].dst_blocks[b];
+      if (flat && ntok == bs) {
+        // (B,L,2,H): the whole block, every layer and K|V, is one range (Eq. 5)
+        cudaError_t e = cudaMemcpyAsync((char*)dst->base + (int64_t)db * dst->stride_bytes[2],
+                                        (const char*)src->base + (int64_t)sb * src->stride_bytes[2],
+                                        (size_t)src->stride_bytes[2], cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+        if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
+        ++calls;
+      } else if ((st = memcpy_tokens(*src, *dst, g, sb, 0, db, 0, ntok, (cudaStream_t)stream, calls)) != FLOWKV_OK) {
+        return st;
+      }
     }
   if (n_calls) *n_calls = calls;
   return FLOWKV_OK;
@@ -654,21 +720,33 @@ flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_poo
 
 flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* pl, void* stream, uint64_t* n_calls) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
-  if (!pl->has_src || !pl->has_dst || !pool_is_span_capable(pl->src, pl->g) || !pool_is_span_capable(pl->dst, pl->g))
-    return fail(FLOWKV_ERR_UNSUPPORTED, "segmentwise baseline needs two token-major pools");
+  const bool span = pl->has_src && pl->has_dst && pool_is_span_capable(pl->src, pl->g) && pool_is_span_capable(pl->dst, pl->g);
+  const bool flat = pl->has_src && pl->has_dst && !span && pools_are_flat_congruent(pl->src, pl->dst, pl->g);
+  if (!span && !flat)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "segmentwise baseline needs two token-major pools, or two block-major pools "
+                                        "with the same interior and block size");
   uint64_t calls = 0;
   const flowkv_pool &S = pl->src, &D = pl->dst;
-  for (const flowkv_segment& sg : pl->segments)
-    for (uint32_t l = 0; l < pl->g.L; ++l)
-      for (uint32_t c = 0; c < 2; ++c) {
-        const char* s = (const char*)S.base + l * S.stride_bytes[0] + c * S.stride_bytes[1] +
-                        (int64_t)sg.src_block * S.stride_bytes[2] + (int64_t)sg.src_tok_off * S.stride_bytes[3];
-        char* d = (char*)D.base + l * D.stride_bytes[0] + c * D.stride_bytes[1] +
-                  (int64_t)sg.dst_block * D.stride_bytes[2] + (int64_t)sg.dst_tok_off * D.stride_bytes[3];
-        cudaError_t e = cudaMemcpyAsync(d, s, (size_t)sg.n_tokens * pl->g.tok_bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+  flowkv_status st;
+  for (const flowkv_segment& sg : pl->segments) {
+    if (flat) {
+      // whole blocks of the segment: ONE copy over all layers (Fig. 5); then the partial last block
+      const uint32_t bs = S.block_size, nfull = sg.n_tokens / bs, rem = sg.n_tokens % bs;
+      if (nfull) {
+        cudaError_t e = cudaMemcpyAsync((char*)D.base + (int64_t)sg.dst_block * D.stride_bytes[2],
+                                        (const char*)S.base + (int64_t)sg.src_block * S.stride_bytes[2],
+                                        (size_t)nfull * S.stride_bytes[2], cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
         if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
         ++calls;
       }
+      if (rem && (st = memcpy_tokens(S, D, pl->g, sg.src_block + nfull, 0, sg.dst_block + nfull, 0, rem,
+                                     (cudaStream_t)stream, calls)) != FLOWKV_OK)
+        return st;
+    } else if ((st = memcpy_tokens(S, D, pl->g, sg.src_block, sg.src_tok_off, sg.dst_block, sg.dst_tok_off, sg.n_tokens,
+                                   (cudaStream_t)stream, calls)) != FLOWKV_OK) {
+      return st;
+    }
+  }
   if (n_calls) *n_calls = calls;
   return FLOWKV_OK;
 }

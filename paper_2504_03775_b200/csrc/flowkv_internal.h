@@ -29,7 +29,9 @@ struct alignas(32) Chunk {
 };
 static_assert(sizeof(Chunk) == 32, "Chunk is loaded as one 32-byte vector");
 
-enum Mode : uint32_t { MODE_ABSENT = 0, MODE_SPAN = 1, MODE_ROWS = 2 };
+// MODE_FLAT: chunks[0, n_flat) are plane-free byte ranges (whole-block runs of two congruent block-major
+// pools); chunks[n_flat, n_flat + n_chunks) are rows-mode chunks (partial last blocks) served per plane.
+enum Mode : uint32_t { MODE_ABSENT = 0, MODE_SPAN = 1, MODE_ROWS = 2, MODE_FLAT = 3 };
 
 struct Side {            // one end of a copy as the kernel sees it
   char*    base;         // device (or mapped host) pointer
@@ -38,13 +40,19 @@ struct Side {            // one end of a copy as the kernel sees it
   uint32_t _pad;
 };
 
+// Plans whose every schedule has at most this many entries pass them in the kernel parameters
+// (3 KiB of the 4 KiB parameter space) instead of uploading them.
+constexpr uint32_t kInlineChunks = 96;
+
 struct KernelParams {
   Side         src, dst;
-  const Chunk* chunks;       // device
   uint32_t     n_chunks;     // per plane
   uint32_t     n_planes;     // planes this launch covers: 2*(layer_end - layer_begin)
   uint32_t     plane0;       // first plane: 2*layer_begin
-  uint32_t     n_tiles;      // n_chunks * n_planes
+  uint32_t     n_tiles;      // (n_flat << flat_shift) + n_chunks * n_planes
+  uint32_t     n_flat;       // MODE_FLAT: plane-free entries at the front of chunks[] (0 otherwise)
+  uint32_t     flat_shift;   // MODE_FLAT: each of them owns 2^flat_shift tile slots ...
+  uint32_t     flat_tile;    //            ... of this many bytes
   uint32_t     row_bytes;    // Dh*e
   uint32_t     heads;        // Hkv
   uint32_t     tok_bytes;    // Hkv*Dh*e
@@ -62,8 +70,11 @@ struct LaunchShape {
   uint32_t stage_bytes;   // bulk: bytes per ring slot (>= largest chunk)
 };
 
-// kernels.cu — launches exactly one kernel; returns cudaError_t as int.
-int launch_copy(Mode mode, const KernelParams& kp, const LaunchShape& ls, void* stream);
+// kernels.cu — launches exactly one kernel; returns cudaError_t as int.  The schedule entries come from
+// `device_chunks`, or, when `host_chunks` is not NULL (n_host_chunks <= kInlineChunks), travel by value in
+// the kernel parameters.
+int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
+                uint32_t n_host_chunks, const LaunchShape& ls, void* stream);
 // Largest dynamic shared memory the bulk variant may use on the current device (0 on failure).
 uint32_t bulk_max_smem();
 
@@ -78,11 +89,21 @@ struct Geometry {          // what both sides must agree on
 
 struct Schedule {
   Mode mode = MODE_ABSENT;
-  std::vector<Chunk> chunks;
+  std::vector<Chunk> chunks;     // MODE_FLAT: [flat spans][ragged rows chunks][rows chunks of everything]
+  uint32_t n_flat = 0;           // MODE_FLAT: entries of the first part
+  uint32_t flat_shift = 0;       // MODE_FLAT: log2(tile slots per entry); an entry covers <= tile_bytes << flat_shift
+  uint32_t flat_tile = 0;        // MODE_FLAT: bytes per tile slot
+  uint32_t n_ragged = 0;         // MODE_FLAT: entries of the second part
+  // MODE_FLAT keeps a complete rows-mode schedule as its third part: layer-range launches use it,
+  // because a layer range of a block-major pool is not one byte range per block run.
+  uint32_t n_per_plane() const { return mode == MODE_FLAT ? n_ragged : (uint32_t)chunks.size(); }
 };
 
 // Is a pool's block interior token-major and dense, with consecutive blocks abutting per plane?
 bool pool_is_span_capable(const flowkv_pool& p, const Geometry& g);
+// Are both pools block-major (a block = one dense byte range holding all its planes, blocks abutting)
+// with the same block size and the same interior strides?  Then whole-block runs are flat byte ranges.
+bool pools_are_flat_congruent(const flowkv_pool& a, const flowkv_pool& b, const Geometry& g);
 
 flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string& err);
 flowkv_status validate_requests(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,

@@ -18,6 +18,7 @@
 //          for payload, which is what a copy that co-runs with GEMMs wants.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "flowkv_internal.h"
 
@@ -97,6 +98,18 @@ __device__ __forceinline__ Chunk load_chunk(const Chunk* p) {
   return c;
 }
 
+// Where a kernel finds its schedule: in global memory (uploaded by flowkv_plan), or — for small plans —
+// inside the kernel parameters themselves, so that planning a small batch needs no allocation, no
+// upload and no cross-stream dependency before the launch (step a4 "kernel params when tiny").
+struct GlobalChunks {
+  const Chunk* p;
+  __device__ __forceinline__ Chunk get(uint32_t i) const { return load_chunk(p + i); }
+};
+struct ParamChunks {
+  Chunk c[kInlineChunks];
+  __device__ __forceinline__ Chunk get(uint32_t i) const { return c[i]; }    // constant-bank load
+};
+
 __device__ __forceinline__ int64_t plane_offset(const Side& s, uint32_t plane, uint32_t req_tokens, uint32_t tok_bytes) {
   return s.dense ? (int64_t)plane * ((int64_t)req_tokens * tok_bytes)
                  : (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv;
@@ -108,11 +121,60 @@ __device__ __forceinline__ void decode_tile(const KernelParams& p, uint32_t tile
   plane += p.plane0;       // layer-range launches start at plane 2*layer_begin
 }
 
+// One contiguous byte range: UNROLL independent loads in flight per thread, then UNROLL stores; the
+// last round is ragged.  `step` = bytes one round of the whole thread group covers.
+template <int VEC, int UNROLL, int HINT>
+__device__ __forceinline__ void copy_span(const char* __restrict__ s, char* __restrict__ d, uint32_t n, uint32_t lane,
+                                          uint32_t step, uint64_t pol) {
+  for (uint32_t off = lane * VEC; off < n; off += UNROLL * step) {
+    Vec<VEC> v[UNROLL];
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j)
+      if (off + j * step < n) v[j] = Mem<VEC, HINT>::ld(s + off + j * step, pol);
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j)
+      if (off + j * step < n) Mem<VEC, HINT>::st(d + off + j * step, v[j], pol);
+  }
+}
+
+// `ntok` tokens x Hkv rows of row_bytes, each side with its own token / head stride; vectors are
+// indexed (token, head, vec) so consecutive lanes move consecutive bytes of a row.
+template <int VEC, int UNROLL, int HINT>
+__device__ __forceinline__ void copy_rows(const KernelParams& p, const char* __restrict__ s, char* __restrict__ d,
+                                          uint32_t ntok, uint32_t lane, uint32_t G, uint32_t vpr, bool pow2,
+                                          uint64_t pol) {
+  const uint32_t pieces = ntok * p.heads * vpr;       // vectors in this chunk, (token, head, vec) order
+  for (uint32_t i0 = lane; i0 < pieces; i0 += G * UNROLL) {
+    Vec<VEC> v[UNROLL];
+    uint32_t doff[UNROLL];          // offsets inside one block fit 32 bits (checked by the planner)
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j) {
+      const uint32_t i = i0 + j * G;
+      if (i < pieces) {
+        uint32_t row, o, tok, h;
+        if (pow2) {
+          row = i >> p.vpr_log2;   o = i & (vpr - 1);
+          tok = row >> p.heads_log2; h = row & (p.heads - 1);
+        } else {
+          row = i / vpr;       o = i - row * vpr;
+          tok = row / p.heads; h = row - tok * p.heads;
+        }
+        const uint32_t soff = tok * (uint32_t)p.src.s_token + h * (uint32_t)p.src.s_head + o * VEC;
+        doff[j] = tok * (uint32_t)p.dst.s_token + h * (uint32_t)p.dst.s_head + o * VEC;
+        v[j] = Mem<VEC, HINT>::ld(s + soff, pol);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < UNROLL; ++j)
+      if (i0 + j * G < pieces) Mem<VEC, HINT>::st(d + doff[j], v[j], pol);
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // ldst / span
 // ------------------------------------------------------------------------------------------------
-template <int VEC, int UNROLL, int HINT>
-__global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ KernelParams p) {
+template <int VEC, int UNROLL, int HINT, class CS>
+__global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
   const uint32_t lane = gtid & (G - 1);
@@ -124,7 +186,7 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
   if (tile >= p.n_tiles) return;
   uint32_t plane, ci;
   decode_tile(p, tile, plane, ci);
-  Chunk c = load_chunk(p.chunks + ci);
+  Chunk c = cs.get(ci);
   for (; tile < p.n_tiles; tile += n_groups) {
     // fetch the NEXT tile's schedule entry now, so its latency hides behind this tile's copy
     const uint32_t next = tile + n_groups;
@@ -132,21 +194,11 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
     Chunk cn = c;
     if (next < p.n_tiles) {
       decode_tile(p, next, nplane, nci);
-      cn = load_chunk(p.chunks + nci);
+      cn = cs.get(nci);
     }
     const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
     char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
-    const uint32_t n = c.n;
-    // UNROLL independent loads in flight per thread, then UNROLL stores; the last round is ragged
-    for (uint32_t off = lane * VEC; off < n; off += UNROLL * step) {
-      Vec<VEC> v[UNROLL];
-#pragma unroll
-      for (int j = 0; j < UNROLL; ++j)
-        if (off + j * step < n) v[j] = Mem<VEC, HINT>::ld(s + off + j * step, pol);
-#pragma unroll
-      for (int j = 0; j < UNROLL; ++j)
-        if (off + j * step < n) Mem<VEC, HINT>::st(d + off + j * step, v[j], pol);
-    }
+    copy_span<VEC, UNROLL, HINT>(s, d, c.n, lane, step, pol);
     c = cn;
     plane = nplane;
   }
@@ -155,8 +207,8 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
 // ------------------------------------------------------------------------------------------------
 // ldst / rows: token- and head-strided rows (layout and block-size conversion fused in the move)
 // ------------------------------------------------------------------------------------------------
-template <int VEC, int UNROLL, int HINT>
-__global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ KernelParams p) {
+template <int VEC, int UNROLL, int HINT, class CS>
+__global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
   const uint32_t lane = gtid & (G - 1);
@@ -169,44 +221,62 @@ __global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ K
   if (tile >= p.n_tiles) return;
   uint32_t plane, ci;
   decode_tile(p, tile, plane, ci);
-  Chunk c = load_chunk(p.chunks + ci);
+  Chunk c = cs.get(ci);
   for (; tile < p.n_tiles; tile += n_groups) {
     const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see fk_span_ldst)
     uint32_t nplane = 0, nci = 0;
     Chunk cn = c;
     if (next < p.n_tiles) {
       decode_tile(p, next, nplane, nci);
-      cn = load_chunk(p.chunks + nci);
+      cn = cs.get(nci);
     }
     const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
     char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
-    const uint32_t pieces = c.n * p.heads * vpr;       // vectors in this chunk, (token, head, vec) order
-    for (uint32_t i0 = lane; i0 < pieces; i0 += G * UNROLL) {
-      Vec<VEC> v[UNROLL];
-      uint32_t doff[UNROLL];          // offsets inside one block fit 32 bits (checked by the planner)
-#pragma unroll
-      for (int j = 0; j < UNROLL; ++j) {
-        const uint32_t i = i0 + j * G;
-        if (i < pieces) {
-          uint32_t row, o, tok, h;
-          if (pow2) {
-            row = i >> p.vpr_log2;   o = i & (vpr - 1);
-            tok = row >> p.heads_log2; h = row & (p.heads - 1);
-          } else {
-            row = i / vpr;       o = i - row * vpr;
-            tok = row / p.heads; h = row - tok * p.heads;
-          }
-          const uint32_t soff = tok * (uint32_t)p.src.s_token + h * (uint32_t)p.src.s_head + o * VEC;
-          doff[j] = tok * (uint32_t)p.dst.s_token + h * (uint32_t)p.dst.s_head + o * VEC;
-          v[j] = Mem<VEC, HINT>::ld(s + soff, pol);
-        }
-      }
-#pragma unroll
-      for (int j = 0; j < UNROLL; ++j)
-        if (i0 + j * G < pieces) Mem<VEC, HINT>::st(d + doff[j], v[j], pol);
-    }
+    copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
     c = cn;
     plane = nplane;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// ldst / flat: both pools block-major with the same block interior, (B,L,2,H) on both sides — the
+// paper's own scenario (Eq. 5, Fig. 5): a run of whole blocks whose ids are
+// consecutive on both sides is ONE byte range covering every layer and K|V.  chunks[0, n_flat) are
+// pieces of such ranges (no plane term), each owning 2^flat_shift tile slots of flat_tile bytes, so the
+// schedule stays one entry per <= 2 MiB instead of one per tile; the tokens of a partial last block
+// (reading A4: token-granular) follow as rows-mode tiles over (plane, chunk), chunks[n_flat ...].
+// Still one launch.
+// ------------------------------------------------------------------------------------------------
+template <int VEC, int UNROLL, int HINT, class CS>
+__global__ void __launch_bounds__(512, 2) fk_flat_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
+  const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t G = 1u << p.group_log2;
+  const uint32_t lane = gtid & (G - 1);
+  const uint32_t group = gtid >> p.group_log2;
+  const uint32_t n_groups = (gridDim.x * blockDim.x) >> p.group_log2;
+  const uint32_t step = G * VEC;
+  const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
+
+  const uint32_t n_flat_tiles = p.n_flat << p.flat_shift;
+  for (uint32_t tile = group; tile < n_flat_tiles; tile += n_groups) {
+    const Chunk c = cs.get(tile >> p.flat_shift);
+    const uint32_t off = (tile & ((1u << p.flat_shift) - 1)) * p.flat_tile;
+    if (off < c.n)      // the last piece of a range may leave slots empty
+      copy_span<VEC, UNROLL, HINT>(p.src.base + c.src_off + off, p.dst.base + c.dst_off + off,
+                                   min(p.flat_tile, c.n - off), lane, step, pol);
+  }
+  const uint32_t n_ragged = p.n_tiles - n_flat_tiles;  // = n_chunks * n_planes
+  if (n_ragged == 0) return;
+  const uint32_t vpr = p.row_bytes / VEC;
+  const bool pow2 = (p.vpr_log2 != 0xffffffffu) && (p.heads_log2 != 0xffffffffu);
+  // start the ragged tiles where the flat ones stopped so the last wave of groups shares them
+  for (uint32_t tile = (group + n_groups - n_flat_tiles % n_groups) % n_groups; tile < n_ragged; tile += n_groups) {
+    uint32_t plane, ci;
+    decode_tile(p, tile, plane, ci);
+    const Chunk c = cs.get(p.n_flat + ci);
+    const char* s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
+    char* d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
   }
 }
 
@@ -251,8 +321,9 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 constexpr int kBulkMaxStages = 16;
 
 // stage_bytes: size of one ring slot (>= every chunk's n).  n_stages in [2, kBulkMaxStages].
-__global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ KernelParams p, uint32_t stage_bytes,
-                                                      uint32_t n_stages) {
+template <class CS>
+__global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                      uint32_t stage_bytes, uint32_t n_stages) {
   extern __shared__ __align__(128) char ring[];
   __shared__ __align__(8) uint64_t full[kBulkMaxStages];
   if (threadIdx.x != 0) return;                       // one thread drives the TMA unit
@@ -271,7 +342,7 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
   auto issue_load = [&](uint32_t k) {
     uint32_t plane, ci;
     decode_tile(p, first + k * stride, plane, ci);
-    const Chunk c = load_chunk(p.chunks + ci);
+    const Chunk c = cs.get(ci);
     const char* s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
     const uint32_t slot = k % n_stages;
     dptr[slot] = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
@@ -298,16 +369,19 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
 // ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
-template <int VEC, int UNROLL>
-static cudaError_t launch_ldst(Mode mode, const KernelParams& kp, const LaunchShape& ls, int hint, cudaStream_t st) {
+template <int VEC, int UNROLL, class CS>
+static cudaError_t launch_ldst(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, int hint,
+                               cudaStream_t st) {
   const dim3 grid(ls.grid), block(ls.threads);
-#define FK_LAUNCH(KERNEL)                                                              \
-  switch (hint) {                                                                      \
-    case 0: KERNEL<VEC, UNROLL, 0><<<grid, block, 0, st>>>(kp); break;                 \
-    case 1: KERNEL<VEC, UNROLL, 1><<<grid, block, 0, st>>>(kp); break;                 \
-    default: KERNEL<VEC, UNROLL, 2><<<grid, block, 0, st>>>(kp); break;                \
+#define FK_LAUNCH(KERNEL)                                                                  \
+  switch (hint) {                                                                          \
+    case 0: KERNEL<VEC, UNROLL, 0, CS><<<grid, block, 0, st>>>(kp, cs); break;             \
+    case 1: KERNEL<VEC, UNROLL, 1, CS><<<grid, block, 0, st>>>(kp, cs); break;             \
+    default: KERNEL<VEC, UNROLL, 2, CS><<<grid, block, 0, st>>>(kp, cs); break;            \
   }
-  if (mode == MODE_SPAN) { FK_LAUNCH(fk_span_ldst) } else { FK_LAUNCH(fk_rows_ldst) }
+  if (mode == MODE_SPAN) { FK_LAUNCH(fk_span_ldst) }
+  else if (mode == MODE_FLAT) { FK_LAUNCH(fk_flat_ldst) }
+  else { FK_LAUNCH(fk_rows_ldst) }
 #undef FK_LAUNCH
   return cudaGetLastError();
 }
@@ -319,17 +393,30 @@ uint32_t bulk_max_smem() {
   return (uint32_t)v;
 }
 
-int launch_copy(Mode mode, const KernelParams& kp, const LaunchShape& ls, void* stream) {
-  cudaStream_t st = (cudaStream_t)stream;
+template <class CS>
+static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, cudaStream_t st) {
   if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_SPAN) {
     const uint32_t smem = ls.n_stages * ls.stage_bytes;
-    cudaError_t e = cudaFuncSetAttribute(fk_span_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(fk_span_bulk<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    fk_span_bulk<<<dim3(ls.grid), dim3(32), smem, st>>>(kp, ls.stage_bytes, ls.n_stages);
+    fk_span_bulk<CS><<<dim3(ls.grid), dim3(32), smem, st>>>(kp, cs, ls.stage_bytes, ls.n_stages);
     return (int)cudaGetLastError();
   }
-  if (ls.vec_bytes == 32) return (int)launch_ldst<32, 4>(mode, kp, ls, (int)ls.hint, st);
-  return (int)launch_ldst<16, 8>(mode, kp, ls, (int)ls.hint, st);
+  if (ls.vec_bytes == 32) return (int)launch_ldst<32, 4, CS>(mode, kp, cs, ls, (int)ls.hint, st);
+  return (int)launch_ldst<16, 8, CS>(mode, kp, cs, ls, (int)ls.hint, st);
+}
+
+int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
+                uint32_t n_host_chunks, const LaunchShape& ls, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (host_chunks) {                       // small plan: the schedule rides in the kernel parameters
+    if (n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
+    ParamChunks pc;
+    memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
+    return launch_with(mode, kp, pc, ls, st);
+  }
+  GlobalChunks gc{device_chunks};
+  return launch_with(mode, kp, gc, ls, st);
 }
 
 }  // namespace flowkv

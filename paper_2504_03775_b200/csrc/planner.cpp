@@ -33,7 +33,7 @@ flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string
   if (!p->num_layers || !p->num_kv_heads || !p->head_dim || !p->elem_bytes || !p->num_blocks)
     return fail(FLOWKV_ERR_INVALID_ARG, "a shape field is zero");
   if (!is_pow2(p->block_size)) return fail(FLOWKV_ERR_UNSUPPORTED, "block_size must be a power of two");
-  if (p->layout > FLOWKV_LAYOUT_STRIDED) return fail(FLOWKV_ERR_INVALID_ARG, "unknown layout");
+  if (p->layout > FLOWKV_LAYOUT_BLKTHD) return fail(FLOWKV_ERR_INVALID_ARG, "unknown layout");
   const uint64_t row = (uint64_t)p->head_dim * p->elem_bytes;
   if (row % 16) return fail(FLOWKV_ERR_ALIGN, "head_dim*elem_bytes is not a multiple of 16 bytes");
   if (row > (1u << 20)) return fail(FLOWKV_ERR_UNSUPPORTED, "row larger than 1 MiB");
@@ -160,13 +160,106 @@ static inline int64_t pool_off(const flowkv_pool* p, uint32_t block, uint32_t of
   return (int64_t)block * p->stride_bytes[FLOWKV_S_BLOCK] + (int64_t)off * p->stride_bytes[FLOWKV_S_TOKEN];
 }
 
+// One rows-mode chunk list for tokens [t, end) of a request: a chunk stays inside one block on each paged side.
+static void rows_chunks(const flowkv_pool* src, const flowkv_pool* dst, const Geometry& g, const flowkv_request& rq,
+                        uint32_t request, int64_t dense0, uint32_t t, uint32_t end, uint32_t tile_tokens,
+                        std::vector<Chunk>& out) {
+  const int32_t* S = rq.src_blocks;
+  const int32_t* D = rq.dst_blocks;
+  while (t < end) {
+    uint32_t n = std::min(tile_tokens, end - t);
+    Chunk c{};
+    if (src) {
+      const uint32_t so = t & (src->block_size - 1);
+      n = std::min(n, src->block_size - so);
+      c.src_off = pool_off(src, (uint32_t)S[t / src->block_size], so);
+    } else {
+      c.src_off = dense0 + (int64_t)t * g.tok_bytes;
+    }
+    if (dst) {
+      const uint32_t dof = t & (dst->block_size - 1);
+      n = std::min(n, dst->block_size - dof);
+      c.dst_off = pool_off(dst, (uint32_t)D[t / dst->block_size], dof);
+    } else {
+      c.dst_off = dense0 + (int64_t)t * g.tok_bytes;
+    }
+    c.n = n;
+    c.req_tokens = rq.num_tokens;
+    c.request = request;
+    out.push_back(c);
+    t += n;
+  }
+}
+
+bool pools_are_flat_congruent(const flowkv_pool& a, const flowkv_pool& b, const Geometry& g) {
+  if (a.block_size != b.block_size) return false;
+  for (int i : {FLOWKV_S_LAYER, FLOWKV_S_KV, FLOWKV_S_BLOCK, FLOWKV_S_TOKEN, FLOWKV_S_HEAD})
+    if (a.stride_bytes[i] != b.stride_bytes[i]) return false;
+  // the interior of a block must be a dense bijection onto [0, s_block): sorted by stride, every axis
+  // starts where the one below it ends, the smallest is one row, and the block stride closes the product
+  struct Axis { int64_t stride; uint64_t extent; };
+  Axis ax[4] = {{a.stride_bytes[FLOWKV_S_LAYER], g.L}, {a.stride_bytes[FLOWKV_S_KV], 2},
+                {a.stride_bytes[FLOWKV_S_TOKEN], a.block_size}, {a.stride_bytes[FLOWKV_S_HEAD], g.Hkv}};
+  std::sort(ax, ax + 4, [](const Axis& x, const Axis& y) { return x.stride < y.stride; });
+  int64_t expect = g.row_bytes;
+  for (const Axis& x : ax) {
+    if (x.extent == 1) continue;            // a length-1 axis never contributes an offset
+    if (x.stride != expect) return false;
+    expect *= (int64_t)x.extent;
+  }
+  return a.stride_bytes[FLOWKV_S_BLOCK] == expect && (uint64_t)expect < (1ull << 32);
+}
+
 void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geometry& g,
                     const flowkv_request* reqs, const std::vector<flowkv_segment>& segs,
                     uint32_t tile_bytes, uint32_t /*vec_bytes*/, Schedule& out) {
   out.chunks.clear();
+  out.n_flat = out.n_ragged = 0;
   const bool span = (!src || pool_is_span_capable(*src, g)) && (!dst || pool_is_span_capable(*dst, g));
-  out.mode = span ? MODE_SPAN : MODE_ROWS;
+  const bool flat = !span && src && dst && pools_are_flat_congruent(*src, *dst, g);
+  out.mode = span ? MODE_SPAN : (flat ? MODE_FLAT : MODE_ROWS);
   const uint32_t tile_tokens = std::max<uint32_t>(1, tile_bytes / g.tok_bytes);
+  if (flat) {
+    // Equal block sizes: every segment starts on a block boundary on both sides (breaks only happen
+    // between blocks), so it is  whole blocks  +  at most one partial block at the end of its request.
+    const uint32_t bs = src->block_size;
+    const int64_t blk = src->stride_bytes[FLOWKV_S_BLOCK];
+    std::vector<Chunk> ragged;
+    // One entry per piece of 2^shift tiles: the largest power of two <= 32 that divides the tiles of one
+    // block, so whole-block ranges fill every slot of every piece (no idle tile slots).
+    uint32_t shift = 0;
+    if (blk % tile_bytes == 0)
+      while (shift < 5 && (blk / tile_bytes) % (2u << shift) == 0) ++shift;
+    out.flat_shift = shift;
+    out.flat_tile = tile_bytes;
+    const uint64_t piece = (uint64_t)tile_bytes << shift;
+    for (const flowkv_segment& sg : segs) {
+      const uint32_t T = reqs[sg.request].num_tokens;
+      const uint64_t bytes = (uint64_t)(sg.n_tokens / bs) * (uint64_t)blk;
+      const int64_t s0 = (int64_t)sg.src_block * blk, d0 = (int64_t)sg.dst_block * blk;
+      for (uint64_t done = 0; done < bytes; done += piece) {
+        Chunk c{};
+        c.src_off = s0 + (int64_t)done;
+        c.dst_off = d0 + (int64_t)done;
+        c.n = (uint32_t)std::min<uint64_t>(piece, bytes - done);
+        c.req_tokens = T;
+        c.request = sg.request;
+        out.chunks.push_back(c);
+      }
+      const uint32_t rem = sg.n_tokens % bs;
+      if (rem) {
+        const uint32_t end = sg.first_token + sg.n_tokens;
+        rows_chunks(src, dst, g, reqs[sg.request], sg.request, 0, end - rem, end, tile_tokens, ragged);
+      }
+    }
+    out.n_flat = (uint32_t)out.chunks.size();
+    out.n_ragged = (uint32_t)ragged.size();
+    out.chunks.insert(out.chunks.end(), ragged.begin(), ragged.end());
+    for (const flowkv_segment& sg : segs)     // third part: everything in rows mode, for layer-range launches
+      rows_chunks(src, dst, g, reqs[sg.request], sg.request, 0, sg.first_token, sg.first_token + sg.n_tokens,
+                  tile_tokens, out.chunks);
+    return;
+  }
   for (const flowkv_segment& sg : segs) {
     const uint32_t T = reqs[sg.request].num_tokens;
     // dense side: request base + token offset; the plane term (p*T*tok_bytes) is added by the kernel
@@ -188,34 +281,8 @@ void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geomet
         done += n;
       }
     } else {
-      // rows mode: a chunk stays inside one block on each paged side
-      const int32_t* S = reqs[sg.request].src_blocks;
-      const int32_t* D = reqs[sg.request].dst_blocks;
-      uint32_t t = sg.first_token;
-      const uint32_t end = sg.first_token + sg.n_tokens;
-      while (t < end) {
-        uint32_t n = std::min(tile_tokens, end - t);
-        Chunk c{};
-        if (src) {
-          const uint32_t so = t & (src->block_size - 1);
-          n = std::min(n, src->block_size - so);
-          c.src_off = pool_off(src, (uint32_t)S[t / src->block_size], so);
-        } else {
-          c.src_off = dense0 + (int64_t)t * g.tok_bytes;
-        }
-        if (dst) {
-          const uint32_t dof = t & (dst->block_size - 1);
-          n = std::min(n, dst->block_size - dof);
-          c.dst_off = pool_off(dst, (uint32_t)D[t / dst->block_size], dof);
-        } else {
-          c.dst_off = dense0 + (int64_t)t * g.tok_bytes;
-        }
-        c.n = n;
-        c.req_tokens = T;
-        c.request = sg.request;
-        out.chunks.push_back(c);
-        t += n;
-      }
+      rows_chunks(src, dst, g, reqs[sg.request], sg.request, dense0, sg.first_token, sg.first_token + sg.n_tokens,
+                  tile_tokens, out.chunks);
     }
   }
 }

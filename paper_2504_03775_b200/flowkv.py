@@ -24,10 +24,11 @@ FLOWKV_OK = 0
 (FLOWKV_ERR_INVALID_ARG, FLOWKV_ERR_BLOCK_OOB, FLOWKV_ERR_TABLE_LEN, FLOWKV_ERR_DST_ALIAS, FLOWKV_ERR_ALIGN,
  FLOWKV_ERR_SHAPE_MISMATCH, FLOWKV_ERR_UNSUPPORTED, FLOWKV_ERR_STAGING_TOO_SMALL, FLOWKV_ERR_NOMEM,
  FLOWKV_ERR_CUDA) = range(1, 11)
-FLOWKV_LAYOUT_LKBTHD, FLOWKV_LAYOUT_BLKHTD, FLOWKV_LAYOUT_STRIDED = 0, 1, 2
+FLOWKV_LAYOUT_LKBTHD, FLOWKV_LAYOUT_BLKHTD, FLOWKV_LAYOUT_STRIDED, FLOWKV_LAYOUT_BLKTHD = 0, 1, 2, 3
 FLOWKV_CHECK_DST_ALIAS, FLOWKV_PLAN_NO_TRANSFER, FLOWKV_PLAN_NO_PACK, FLOWKV_PLAN_NO_UNPACK = 1, 2, 4, 8
 FLOWKV_VARIANT_AUTO, FLOWKV_VARIANT_LDST, FLOWKV_VARIANT_BULK = 0, 1, 2
-LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "strided": FLOWKV_LAYOUT_STRIDED}
+LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "strided": FLOWKV_LAYOUT_STRIDED,
+           "blkthd": FLOWKV_LAYOUT_BLKTHD}
 
 EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
@@ -59,7 +60,7 @@ class flowkv_tuning(C.Structure):
     _fields_ = [("tile_bytes", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("max_sms", C.c_uint32),
                 ("threads", C.c_uint32), ("group_threads", C.c_uint32), ("variant", C.c_uint32),
                 ("tile_order", C.c_uint32), ("cache_hint", C.c_uint32), ("stages", C.c_uint32),
-                ("_reserved", C.c_uint32 * 3)]
+                ("plan_in_params", C.c_uint32), ("_reserved", C.c_uint32 * 2)]
 
 
 class flowkv_plan_stats(C.Structure):
@@ -70,7 +71,7 @@ class flowkv_plan_stats(C.Structure):
                 ("mode_unpack", C.c_uint32), ("grid", C.c_uint32), ("threads", C.c_uint32),
                 ("group_threads", C.c_uint32), ("tile_bytes", C.c_uint32), ("variant", C.c_uint32),
                 ("vec_bytes", C.c_uint32), ("tile_order", C.c_uint32), ("cache_hint", C.c_uint32),
-                ("stages", C.c_uint32), ("smem_bytes", C.c_uint32), ("num_sms", C.c_uint32), ("_reserved", C.c_uint32)]
+                ("stages", C.c_uint32), ("smem_bytes", C.c_uint32), ("num_sms", C.c_uint32), ("n_flat_chunks", C.c_uint32)]
 
     def as_dict(self) -> dict:
         return {n: int(getattr(self, n)) for n, _ in self._fields_ if not n.startswith("_")}

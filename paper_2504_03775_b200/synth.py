@@ -43,7 +43,7 @@ LLAMA3_70B = Shape(80, 8, 128, "bf16")
 
 @dataclass(frozen=True)
 class PoolSpec:
-    layout: str        # "lkbthd" | "blkhtd"
+    layout: str        # "lkbthd" | "blkhtd" | "blkthd"
     block_size: int    # tokens per block
     num_blocks: int
 
@@ -221,6 +221,16 @@ def config2_llama8b_13k(num_layers: Optional[int] = None) -> Workload:
     return make_workload("cfg2_llama8b_13k", SEED_BASE + 2000, shape, [13312],
                          "lkbthd", 16, ("geometric", 4.0), 16384,
                          "lkbthd", 16, ("contiguous",), 1024)
+
+
+def config2_blockmajor(layout: str = "blkthd", num_layers: Optional[int] = None, tokens: int = 13312) -> Workload:
+    """configs[1]'s request and block tables with BOTH pools in the paper's (B,L,2,H) order (Eq. 5,
+    P:L98-103): a block is one 2 MiB range, a run of blocks one span over all layers."""
+    shape = LLAMA3_8B if num_layers is None else Shape(num_layers, 8, 128, "bf16")
+    w = make_workload(f"cfg2_{layout}_13k", SEED_BASE + 2000, shape, [tokens],
+                      layout, 16, ("geometric", 4.0), 16384,
+                      layout, 16, ("contiguous",), 1024)
+    return w
 
 
 def config3_lengths(n: int = 64) -> List[int]:

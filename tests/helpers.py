@@ -15,12 +15,15 @@ def logical_view(buf_u8: np.ndarray, layout: str, L: int, NB: int, BS: int, H: i
 
     lkbthd = Eq. 5 left side  (L,2,B,H) with H=[token][head][dim]
     blkhtd = Eq. 5 right side (B,L,2,H) with H=[head][token][dim]
+    blkthd = Eq. 5 right side (B,L,2,H) with H=[token][head][dim] (H as on the left side)
     """
     w = buf_u8.view(np.uint16)
     if layout == "lkbthd":
         return w.reshape(L, 2, NB, BS, H, D)
     if layout == "blkhtd":
         return w.reshape(NB, L, 2, H, BS, D).transpose(1, 2, 0, 4, 3, 5)
+    if layout == "blkthd":
+        return w.reshape(NB, L, 2, BS, H, D).transpose(1, 2, 0, 3, 4, 5)
     raise ValueError(layout)
 
 

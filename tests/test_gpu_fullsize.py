@@ -98,6 +98,37 @@ def test_cfg2_full_size():
     _lkbthd_all_planes_property(w, dp)
 
 
+@pytest.mark.parametrize("tokens", [13312, 13307])
+def test_cfg2_block_major_full_size(tokens):
+    """configs[1]'s request with both pools in the paper's (B,L,2,H) order (S§8f NEXT-2), 32 GiB src pool: flat
+    whole-block spans (+ a token-granular partial last block at 13,307 tokens), one launch.  Every block: src
+    block bytes == dst block bytes (identical interiors, torch indexing, test-only); sampled blocks and the
+    partial block: element by element against the oracle run on that block as a one-block pool."""
+    w = synth.config2_blockmajor("blkthd", tokens=tokens)
+    _need(w.src.bytes(w.shape) + w.dst.bytes(w.shape))
+    dp = P.DevicePools(w)
+    n0 = F.flowkv_launch_count()
+    plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS)
+    plan.transfer()
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1 and plan.stats["mode_transfer"] == 3
+    r = w.requests[0]
+    blk = 16 * w.shape.bytes_per_token
+    sv, dv = dp.src_buf.view(w.src.num_blocks, blk), dp.dst_buf.view(w.dst.num_blocks, blk)
+    nfull = tokens // 16
+    S, Dt = torch.from_numpy(r.src_blocks.astype(np.int64)).cuda(), torch.from_numpy(r.dst_blocks.astype(np.int64)).cuda()
+    assert torch.equal(sv[S[:nfull]], dv[Dt[:nfull]])
+    rest = torch.ones(w.dst.num_blocks, dtype=torch.bool, device="cuda")
+    rest[Dt] = False
+    assert bool((dv[rest] == P.SENTINEL_BYTE).all()), "an unnamed dst block changed"
+    g1 = O.PoolGeom.blkthd(w.shape.num_layers, 8, 128, 2, 1, 16)
+    for i in sorted({0, nfull // 2, len(r.src_blocks) - 1}):
+        ntok = min(16, tokens - 16 * i)
+        exp = np.full(blk, P.SENTINEL_BYTE, np.uint8)
+        O.transfer(sv[int(r.src_blocks[i])].cpu().numpy(), g1, exp, g1, [0], [0], ntok)
+        G.assert_same(dv[int(r.dst_blocks[i])].cpu().numpy(), exp, f"block {i} ({ntok} tokens)")
+
+
 def test_cfg3_full_size_fit_rule():
     """configs[2] scaled to fit HBM by the seeded-prefix rule, one batch, one launch."""
     free_b, _ = torch.cuda.mem_get_info()

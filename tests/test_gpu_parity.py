@@ -20,8 +20,8 @@ TUNINGS = [
     None,
     {"variant": "ldst", "cache_hint": 1, "group_threads": 32, "threads": 128, "tile_bytes": 4096},
     {"variant": "ldst", "cache_hint": 2, "group_threads": 64, "threads": 256, "tile_bytes": 8192, "tile_order": 2},
-    {"variant": "ldst", "cache_hint": 3, "threads": 512, "tile_bytes": 65536, "ctas_per_sm": 2},
-    {"variant": "bulk", "tile_bytes": 16384, "stages": 4},
+    {"variant": "ldst", "cache_hint": 3, "threads": 512, "tile_bytes": 65536, "ctas_per_sm": 2, "plan_in_params": 1},
+    {"variant": "bulk", "tile_bytes": 16384, "stages": 4, "plan_in_params": 1},
     {"variant": "bulk", "tile_bytes": 4096, "stages": 16, "ctas_per_sm": 2, "tile_order": 2},
     {"variant": "ldst", "max_sms": 3, "ctas_per_sm": 1},
 ]
@@ -360,3 +360,116 @@ def test_transfer_via_pinned_host_pipeline(n_chunks, ctas):
     G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host: dst")
     G.assert_same(host.numpy(), G.oracle_pack(w, src_np), "via host: wire bytes")
     plan.destroy()
+
+
+@pytest.mark.parametrize("layout", ["blkhtd", "blkthd"])
+@pytest.mark.parametrize("tuning", [None, {"tile_bytes": 4096, "threads": 128, "group_threads": 32},
+                                    {"tile_bytes": 16384, "ctas_per_sm": 1, "max_sms": 2, "cache_hint": 1},
+                                    {"tile_order": 2, "group_threads": 64, "threads": 256}])
+def test_flat_mode_block_major_both_sides(layout, tuning):
+    """S§8f NEXT-2 / Eq. 5 / Fig. 5: both pools (B,L,2,H) with the same interior.  Whole-block runs move as
+    plane-free byte ranges, partial last blocks token-granular (A4) — all in ONE launch, bit-exact incl.
+    the sentinel bytes of every untouched slot."""
+    lengths = [777, 64, 1, 300, 16, 15, 0, 17]
+    w = synth.make_workload("flat", 31, synth.Shape(3, 4, 64, "bf16"), lengths,
+                            layout, 16, ("geometric", 3.0), None, layout, 16, ("geometric", 2.0), None)
+    dp, plan, _ = G.run_transfer_and_check(w, tuning, fill="bits")
+    st = plan.stats
+    assert st["mode_transfer"] == 3 and st["n_flat_chunks"] > 0
+    assert st["n_chunks_transfer"] - st["n_flat_chunks"] >= sum(1 for t in lengths if t % 16)
+
+
+@pytest.mark.parametrize("upload", [0, 1])
+def test_flat_mode_layer_ranges_and_pack_unpack(upload):
+    """Layer-range launches of a flat plan fall back to its rows schedule; pack/unpack of block-major pools go
+    through the dense wire format as before."""
+    w = synth.make_workload("flatL", 32, synth.Shape(5, 2, 64, "fp16"), [100, 33, 48],
+                            "blkthd", 16, ("geometric", 2.0), None, "blkthd", 16, ("contiguous",), None)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    gs, gd = G.geom(w.src, w.shape), G.geom(w.dst, w.shape)
+    plan = dp.plan(0, {"plan_in_params": upload})
+    assert plan.stats["mode_transfer"] == 3 and (plan.stats["plan_device_bytes"] > 0) == bool(upload)
+    for l0, l1 in [(1, 3), (0, 5), (4, 5), (2, 2)]:
+        P.fill_sentinel(dp.dst_buf)
+        n0 = F.flowkv_launch_count()
+        F.flowkv_transfer_layers(plan, l0, l1)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if l1 > l0 else 0)
+        exp = np.full(dp.dst_buf.numel(), P.SENTINEL_BYTE, np.uint8)
+        for r in w.requests:
+            O.transfer(src_np, gs, exp, gd, r.src_blocks, r.dst_blocks, r.num_tokens, l0, l1)
+        G.assert_same(P.to_numpy(dp.dst_buf), exp, f"flat plan, layers [{l0},{l1})")
+    nbytes = plan.stats["staging_bytes"]
+    staging = P.alloc_bytes(nbytes)
+    plan.pack(staging.data_ptr(), nbytes)
+    P.fill_sentinel(dp.dst_buf)
+    plan.unpack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(staging), G.oracle_pack(w, src_np), "pack from blkthd")
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "unpack into blkthd")
+
+
+@pytest.mark.parametrize("src_layout,dst_layout", [("lkbthd", "blkthd"), ("blkthd", "lkbthd"), ("blkthd", "blkhtd")])
+def test_eq5_whole_pool_reorder(src_layout, dst_layout):
+    """Eq. 5 as an operation: the whole pool re-ordered (L,2,B,H) <-> (B,L,2,H) with identity
+    tables, one launch."""
+    NB, BS = 24, 16
+    ident = np.arange(NB, dtype=np.int32)
+    shape = synth.Shape(4, 4, 64, "bf16")
+    w = synth.Workload("eq5", 33, shape, synth.PoolSpec(src_layout, BS, NB), synth.PoolSpec(dst_layout, BS, NB),
+                       [synth.Request(NB * BS, ident, ident)])
+    G.run_transfer_and_check(w, None, fill="bits")
+
+
+def test_baselines_on_block_major_pools_count_calls():
+    """(B,L,2,H) pools: blockwise = one copy per whole block, segmentwise = one per segment (Fig. 5),
+    plus per-plane copies for the partial last block; both reach the oracle's bytes."""
+    L = 3
+    w = synth.make_workload("bm_base", 34, synth.Shape(L, 2, 64, "fp16"), [16 * 9 + 5, 32],
+                            "blkthd", 16, ("geometric", 3.0), None, "blkthd", 16, ("contiguous",), None)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    exp = G.oracle_transfer(w, src_np)
+    calls = F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests)
+    torch.cuda.synchronize()
+    assert calls == (9 + 2) + 2 * L
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "blockwise baseline, block-major")
+    P.fill_sentinel(dp.dst_buf)
+    plan = dp.plan()
+    calls = F.flowkv_baseline_segmentwise(plan)
+    torch.cuda.synchronize()
+    segs = plan.segments
+    assert calls == sum(1 for sg in segs if sg["n_tokens"] >= 16) + 2 * L
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "segmentwise baseline, block-major")
+
+
+@pytest.mark.parametrize("n_blocks", [95, 96, 97])
+@pytest.mark.parametrize("variant", ["ldst", "bulk"])
+def test_small_plans_travel_in_kernel_params(n_blocks, variant):
+    """Step a4 'kernel params when tiny': a plan whose schedules have <= 96 entries is never uploaded
+    (plan_device_bytes == 0) — transfer, pack and unpack read their entries from the parameter space;
+    one entry more and the plan is uploaded as usual.  Same bytes either way."""
+    T = n_blocks * 16 - 3
+    w = synth.make_workload("inparams", 35, synth.Shape(2, 2, 64, "fp16"), [T],
+                            "lkbthd", 16, ("permutation",), 256, "lkbthd", 16, ("contiguous",), 128, "uniform")
+    tuning = {"variant": variant, "tile_bytes": 4096}
+    dp, plan, exp = G.run_transfer_and_check(w, tuning, fill="bits")
+    st = plan.stats
+    if st["n_chunks_transfer"] == n_blocks:          # the seeded permutation had no accidental +1 neighbours
+        assert (st["plan_device_bytes"] == 0) == (n_blocks <= 96)
+    src_np = P.to_numpy(dp.src_buf)
+    nbytes = st["staging_bytes"]
+    staging = P.alloc_bytes(nbytes)
+    plan.pack(staging.data_ptr(), nbytes)
+    P.fill_sentinel(dp.dst_buf)
+    plan.unpack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(staging), G.oracle_pack(w, src_np), "pack")
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "unpack")
+    forced = dp.plan(0, dict(tuning, plan_in_params=1))
+    assert forced.stats["plan_device_bytes"] > 0
+    P.fill_sentinel(dp.dst_buf)
+    forced.transfer()
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "uploaded plan")

@@ -26,7 +26,7 @@ def _geom(layout, L, H, D, NB, BS):
 # ---------------------------------------------------------------------------------------
 # element placement
 # ---------------------------------------------------------------------------------------
-@pytest.mark.parametrize("layout", ["lkbthd", "blkhtd"])
+@pytest.mark.parametrize("layout", ["lkbthd", "blkhtd", "blkthd"])
 def test_same_layout_full_blocks_equals_numpy_fancy_indexing(layout):
     """Catches: wrong stride order, swapped src/dst table, K|V or layer axis mix-up."""
     rng = np.random.default_rng(1)
@@ -46,6 +46,7 @@ def test_same_layout_full_blocks_equals_numpy_fancy_indexing(layout):
 
 @pytest.mark.parametrize("bs_s,bs_d,src_layout,dst_layout", [
     (4, 4, "lkbthd", "blkhtd"), (2, 8, "lkbthd", "blkhtd"), (8, 2, "blkhtd", "lkbthd"), (4, 16, "lkbthd", "lkbthd"),
+    (4, 4, "lkbthd", "blkthd"), (8, 2, "blkthd", "blkhtd"), (2, 4, "blkhtd", "blkthd"),
 ])
 def test_layout_and_block_size_conversion_equals_numpy_reshape(bs_s, bs_d, src_layout, dst_layout):
     """Full blocks on both sides: gather -> flatten tokens -> regroup into dst blocks.
@@ -66,6 +67,24 @@ def test_layout_and_block_size_conversion_equals_numpy_reshape(bs_s, bs_d, src_l
     ev = Hh.logical_view(exp, dst_layout, L, NBd, bs_d, H, D)
     ev[:, :, Dst] = toks.reshape(L, 2, nd, bs_d, H, D)
     assert np.array_equal(dst, exp)
+
+
+def test_eq5_reorder_is_a_pure_axis_permutation():
+    """Eq. 5: (L,2,B,H) -> (B,L,2,H) with identity tables and full blocks is numpy's
+    transpose(2,0,1,3) of the same bytes.  Catches: a blkthd stride that is not the (B,L,2,H) order."""
+    rng = np.random.default_rng(21)
+    L, H, D, NB, BS = 3, 2, 8, 5, 4
+    gs, gd = _geom("lkbthd", L, H, D, NB, BS), _geom("blkthd", L, H, D, NB, BS)
+    src = _rand_pool(rng, gs.span_bytes())
+    dst = np.full(gd.span_bytes(), SENT, np.uint8)
+    ident = np.arange(NB)
+    O.transfer(src, gs, dst, gd, ident, ident, NB * BS)
+    Hbytes = BS * H * D * 2
+    exp = src.reshape(L, 2, NB, Hbytes).transpose(2, 0, 1, 3).reshape(-1)
+    assert np.array_equal(dst, exp)
+    back = np.full(gs.span_bytes(), SENT, np.uint8)
+    O.transfer(dst, gd, back, gs, ident, ident, NB * BS)
+    assert np.array_equal(back, src)
 
 
 def test_self_describing_pool_lands_where_definition_says():

@@ -42,6 +42,7 @@ def test_struct_sizes_match_header_layout():
     assert C.sizeof(F.flowkv_segment) == 40
     assert C.sizeof(F.flowkv_tuning) == 48
     assert C.sizeof(F.flowkv_plan_stats) == 9 * 8 + 16 * 4
+    assert F.flowkv_plan_stats.n_flat_chunks.offset == 9 * 8 + 15 * 4
 
 
 def test_named_layout_strides():
@@ -53,6 +54,11 @@ def test_named_layout_strides():
     g = O.PoolGeom.blkhtd(80, 8, 128, 2, 10, 64)
     assert [g.s_layer, g.s_kv, g.s_block, g.s_token, g.s_head] == list(q.stride_bytes)
     assert F.pool_bytes(q) == g.span_bytes()
+    # blkthd = (B,L,2,H) with H untouched: a block is 2*L*BS*Hkv*Dh*e = 2 MiB at the 8B shape
+    t = _pool("blkthd", L=32, H=8, D=128, NB=7, BS=16)
+    assert list(t.stride_bytes) == [65536, 32768, 2 * 1024 * 1024, 2048, 256]
+    gt = O.PoolGeom.blkthd(32, 8, 128, 2, 7, 16)
+    assert [gt.s_layer, gt.s_kv, gt.s_block, gt.s_token, gt.s_head] == list(t.stride_bytes)
 
 
 @pytest.mark.parametrize("case", json.load(open(os.path.join(ROOT, "tests", "golden", "align_examples.json")))["cases"])
@@ -215,3 +221,42 @@ def test_tile_schedule_respects_tile_bytes():
         runs = np.diff(np.concatenate([[0], np.nonzero(np.diff(r.src_blocks) != 1)[0] + 1, [len(r.src_blocks)]]))
         assert st["n_chunks_transfer"] == int(sum(-(-int(n) * 32768 // tile) for n in runs))
         assert st["tile_bytes"] == tile and st["n_planes"] == 64
+
+
+@pytest.mark.parametrize("layout", ["blkhtd", "blkthd"])
+def test_block_major_pairs_use_flat_whole_block_spans(layout):
+    """Both pools (B,L,2,H) with the same interior (Eq. 5): a run of n whole blocks that is
+    consecutive on both sides is ONE byte range of n * 2*L*BS*Hkv*Dh*e bytes (Fig. 5); only a
+    partial last block needs per-plane work.  Chunk counts follow in closed form."""
+    L, H, D, BS = 4, 2, 64, 16
+    blk = 2 * L * BS * H * D * 2                      # 32 KiB
+    sp, dp = _pool(layout, L, H, D, 64, BS), _pool(layout, L, H, D, 64, BS)
+    S = np.asarray([5, 6, 7, 8, 20, 21, 40], np.int32)
+    Dt = np.asarray([0, 1, 2, 3, 4, 5, 6], np.int32)
+    for T, tile in [(7 * BS, 65536), (7 * BS - 5, 65536), (7 * BS - 5, 16384), (3, 65536)]:
+        nb = -(-T // BS)
+        plan = F.flowkv_plan_host(sp, dp, [F.Request(T, S[:nb], Dt[:nb])], 0, {"tile_bytes": tile})
+        st = plan.stats
+        assert st["mode_transfer"] == 3
+        segs = [(a, n) for _, a, n in _segs(plan)]
+        assert segs == O.align(S[:nb], BS, Dt[:nb], BS, T)
+        slots = 1                                      # an entry owns up to 32 tile slots of one range:
+        while blk % tile == 0 and slots < 32 and (blk // tile) % (2 * slots) == 0:
+            slots *= 2                                 # the largest power of two dividing the tiles of a block
+        piece = tile * slots
+        flat = sum(-(-(n // BS) * blk // piece) for _, n in segs)
+        ragged = sum(1 for _, n in segs if n % BS)
+        assert st["n_flat_chunks"] == flat and st["n_chunks_transfer"] == flat + ragged
+    # fully contiguous on both sides, whole blocks: one segment, and 7 blocks * 32 KiB / 64 KiB tiles = 4 spans
+    plan = F.flowkv_plan_host(sp, dp, [F.Request(7 * BS, np.arange(10, 17, dtype=np.int32), Dt)])
+    assert plan.stats["n_segments"] == 1 and plan.stats["n_flat_chunks"] == plan.stats["n_chunks_transfer"]
+    # differing interiors or block sizes are NOT flat
+    other = "blkthd" if layout == "blkhtd" else "blkhtd"
+    assert F.flowkv_plan_host(sp, _pool(other, L, H, D, 64, BS), [F.Request(16, S[:1], Dt[:1])]).stats["mode_transfer"] == 2
+    d32 = _pool(layout, L, H, D, 64, 32)
+    assert F.flowkv_plan_host(sp, d32, [F.Request(16, S[:1], Dt[:1])]).stats["mode_transfer"] == 2
+    # a padded block-major pool (blocks do not abut) is not flat either
+    strides = list(sp.stride_bytes)
+    strides[F.LAYOUTS["strided"]] += 256            # index 2 == FLOWKV_S_BLOCK
+    pad = F.make_pool(FAKE, L, H, D, 2, 64, BS, "strided", strides)
+    assert F.flowkv_plan_host(pad, pad, [F.Request(16, S[:1], Dt[:1])]).stats["mode_transfer"] == 2
