@@ -339,6 +339,12 @@ def run_ours(args) -> None:
         nbytes = payload
         host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
         Ke = max(2, min(args.e2e_steps, K))
+        scratch, scratch_bytes = None, 0
+        if not (args.e2e_serial or args.e2e_direct):
+            p0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+            scratch_bytes = F.flowkv_via_host_scratch_bytes(p0, args.e2e_chunks)
+            p0.destroy()
+            scratch = P.alloc_bytes(scratch_bytes, device=f"cuda:{local}")
 
         def e2e_step():
             plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
@@ -346,7 +352,8 @@ def run_ours(args) -> None:
                 F.flowkv_pack(plan, host.data_ptr(), nbytes, s)      # device -> pinned host, one kernel
                 F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)    # pinned host -> device, one kernel
             else:                                                    # same result, both PCIe directions overlapped
-                F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, args.e2e_chunks, args.e2e_ctas, s)
+                F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, args.e2e_chunks, args.e2e_ctas, s,
+                                           scratch.data_ptr() if scratch is not None else 0, scratch_bytes)
             plan.destroy()
         e2e_step()
         barrier()
@@ -370,8 +377,13 @@ def run_ours(args) -> None:
                            "steps": Ke, "ms_per_step": te / Ke,
                            "path": ("flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host"
                                     if args.e2e_serial else
-                                    "flowkv_plan (host tables) + flowkv_transfer_via_host: pack to pinned host and unpack "
-                                    "from it, pipelined over layer chunks on two streams"),
+                                    "flowkv_plan (host tables) + flowkv_transfer_via_host, direct mode: pack kernels store to "
+                                    "pinned host and unpack kernels load from it, pipelined over layer chunks on two streams"
+                                    if args.e2e_direct else
+                                    "flowkv_plan (host tables) + flowkv_transfer_via_host, copy-engine mode: per layer chunk "
+                                    "flowkv_pack_window into device scratch, D2H to pinned host, H2D back, flowkv_unpack_window; "
+                                    "both PCIe directions overlapped on two streams"),
+                           "device_scratch_bytes": scratch_bytes,
                            "link_memcpy_d2h_GBps": d2h, "link_memcpy_h2d_GBps": h2d}
         del host
 
@@ -421,6 +433,8 @@ def main() -> None:
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-serial", action="store_true", help="pack then unpack on one stream instead of the pipeline")
+    ap.add_argument("--e2e-direct", action="store_true",
+                    help="pipeline with SM loads/stores over PCIe (no device scratch) instead of the copy engines")
     ap.add_argument("--e2e-chunks", type=int, default=0)
     ap.add_argument("--e2e-ctas", type=int, default=0)
     ap.add_argument("--no-baselines", action="store_true")

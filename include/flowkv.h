@@ -211,16 +211,41 @@ FLOWKV_API flowkv_status flowkv_pack_layers(const flowkv_plan_t* plan, void* sta
 FLOWKV_API flowkv_status flowkv_unpack_layers(const flowkv_plan_t* plan, const void* staging, uint64_t bytes,
                                               uint32_t layer_begin, uint32_t layer_end, void* stream);
 
+/* Layer-window variants: `window` is a dense buffer that holds ONLY layers [layer_begin, layer_end), in the wire
+ * order of a model with that many layers: [request][layer - layer_begin][K|V][token][head][dim], requests
+ * concatenated; request r starts at byte staging_tok_off(r) * 2*(layer_end-layer_begin)*Hkv*Dh*e.  Each window is a
+ * self-contained contiguous message of flowkv_window_bytes() bytes — what a layer-wise / pipelined sender puts
+ * on the wire — so a transfer can be cut into layer chunks that need no full-size staging
+ * buffer.  The window [0, num_layers) is the wire format of flowkv_pack.  One launch each (zero if empty).
+ * `window`: DEVICE or mapped pinned HOST pointer, 16-B aligned, `bytes` >= flowkv_window_bytes(). */
+FLOWKV_API flowkv_status flowkv_window_bytes(const flowkv_plan_t* plan, uint32_t layer_begin, uint32_t layer_end, uint64_t* bytes);
+FLOWKV_API flowkv_status flowkv_pack_window(const flowkv_plan_t* plan, void* window, uint64_t bytes,
+                                            uint32_t layer_begin, uint32_t layer_end, void* stream);
+FLOWKV_API flowkv_status flowkv_unpack_window(const flowkv_plan_t* plan, const void* window, uint64_t bytes,
+                                              uint32_t layer_begin, uint32_t layer_end, void* stream);
+
 /* Pool -> pinned host -> pool with both PCIe directions busy at once (S§8f NEXT-3: chunked pinned-host
- * pipeline; the host buffer stands in for the network endpoint, BASELINE.json north_star).  Result ==
- * flowkv_pack(host_staging) followed by flowkv_unpack(host_staging).  The layers are cut into `n_chunks`
- * groups (0 = min(L,16)); chunk c is packed on `stream`, and unpacked on a plan-owned second stream as soon as
- * its pack has finished, so the D2H of chunk c+1 overlaps the H2D of chunk c.  `stream` is made to wait for
- * the last unpack, so callers see ordinary stream order.  `ctas_per_kernel` caps each kernel's grid
- * (0 = 64; a PCIe-bound kernel needs few CTAs and both kernels must be co-resident).
- * Launches: 2 * n_chunks.  host_staging: mapped pinned HOST (or device) pointer, 16-B aligned. */
+ * pipeline; the host buffer stands in for the network endpoint, BASELINE.json north_star).  dst ends up exactly
+ * as after flowkv_transfer.  The layers are cut into `n_chunks` groups (0 = 16; clamped to [1, L]); chunk c goes
+ * out on `stream` and comes back on a plan-owned second stream as soon as it has landed on the host, so the D2H
+ * of chunk c+1 overlaps the H2D of chunk c.  `stream` is made to wait for the last inbound chunk, so callers see
+ * ordinary stream order.  Two modes:
+ *   device_scratch == NULL — direct: the pack / unpack kernels store to / load from host memory themselves (UVA);
+ *     no extra device memory.  host_staging holds the wire format of flowkv_pack.  `ctas_per_kernel` caps each
+ *     kernel's grid (0 = 64: a PCIe-bound kernel needs few CTAs and both kernels must be co-resident).
+ *   device_scratch != NULL — copy engines: chunk c is packed into a scratch slot in HBM (flowkv_pack_window), moved
+ *     D2H and H2D by cudaMemcpyAsync, and unpacked from a second slot (flowkv_unpack_window).  On B200 the copy
+ *     engines sustain ~50 GB/s in both directions at once where SM loads over PCIe drop to ~38 GB/s.  host_staging
+ *     then holds the chunks back to back, chunk c = the layer window [L*c/n, L*(c+1)/n) at byte offset
+ *     flowkv_window_bytes(0, L*c/n) (== the wire format when n_chunks == 1).  device_scratch: DEVICE pointer,
+ *     256-B aligned, scratch_bytes >= flowkv_via_host_scratch_bytes(plan, n_chunks) (4 slots of the largest
+ *     chunk); caller-owned, reusable once `stream` has passed this call.  `ctas_per_kernel`: 0 = the plan's grid.
+ * Launches: 2 * (non-empty chunks).  host_staging: pinned HOST pointer (mapped / UVA for the direct mode; a device
+ * pointer also works in direct mode), 16-B aligned, bytes >= staging_bytes. */
+FLOWKV_API flowkv_status flowkv_via_host_scratch_bytes(const flowkv_plan_t* plan, uint32_t n_chunks, uint64_t* bytes);
 FLOWKV_API flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* plan, void* host_staging, uint64_t bytes,
-                                                  uint32_t n_chunks, uint32_t ctas_per_kernel, void* stream);
+                                                  uint32_t n_chunks, uint32_t ctas_per_kernel,
+                                                  void* device_scratch, uint64_t scratch_bytes, void* stream);
 
 /* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
  * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,

@@ -368,15 +368,20 @@ Side pool_side(const flowkv_pool& p) {
   return s;
 }
 
-Side dense_side(const void* staging, const Geometry& g) {
+// A dense staging buffer that holds the layer window [w0, w1) in wire order (A12).  The whole wire format
+// is the window [0, L).
+Side dense_side(const void* staging, const Geometry& g, uint32_t w0, uint32_t w1) {
   Side s{};
   s.base = (char*)staging;
-  s.s_layer = 0; s.s_kv = 0;               // plane stride comes from the chunk's req_tokens
+  s.s_layer = 2ll * (w1 - w0) * g.tok_bytes;   // bytes per token of the window
+  s.s_kv = 0;                                  // plane stride comes from the chunk's req_tokens
   s.s_token = g.tok_bytes;
   s.s_head = g.row_bytes;
   s.dense = 1;
+  s.plane0 = 2 * w0;
   return s;
 }
+Side dense_side(const void* staging, const Geometry& g) { return dense_side(staging, g, 0, g.L); }
 
 struct RunOpts {
   bool ranged = false;                       // false: all layers
@@ -434,14 +439,20 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   return FLOWKV_OK;
 }
 
-flowkv_status check_staging(const flowkv_plan_t* pl, const Op& op, const void* staging, uint64_t bytes, const char* what) {
+flowkv_status check_staging(const flowkv_plan_t* pl, const Op& op, const void* staging, uint64_t bytes, const char* what,
+                            uint64_t need = ~0ull) {
   if (op.sched.mode == MODE_ABSENT)
     return fail(FLOWKV_ERR_UNSUPPORTED, std::string("plan has no ") + what + " schedule");
   if (op.sched.chunks.empty()) return FLOWKV_OK;
   if (!staging) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
   if ((uintptr_t)staging % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
-  if (bytes < pl->total_tokens * pl->g.bytes_per_token) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
+  if (need == ~0ull) need = pl->total_tokens * pl->g.bytes_per_token;
+  if (bytes < need) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "staging buffer too small");
   return FLOWKV_OK;
+}
+
+uint64_t window_bytes(const flowkv_plan_t* pl, uint32_t l0, uint32_t l1) {
+  return pl->total_tokens * 2ull * (l1 - l0) * pl->g.tok_bytes;
 }
 
 }  // namespace
@@ -571,8 +582,60 @@ flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64
   return flowkv_unpack_layers(pl, staging, bytes, 0, pl->g.L, stream);
 }
 
+flowkv_status flowkv_window_bytes(const flowkv_plan_t* pl, uint32_t layer_begin, uint32_t layer_end, uint64_t* bytes) {
+  if (!pl || !bytes) return fail(FLOWKV_ERR_INVALID_ARG, "NULL argument");
+  if (layer_begin > layer_end || layer_end > pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
+  *bytes = window_bytes(pl, layer_begin, layer_end);
+  return FLOWKV_OK;
+}
+
+flowkv_status flowkv_pack_window(const flowkv_plan_t* pl, void* window, uint64_t bytes, uint32_t layer_begin,
+                                 uint32_t layer_end, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (layer_begin > layer_end || layer_end > pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
+  flowkv_status st = check_staging(pl, pl->pack, window, bytes, "pack", window_bytes(pl, layer_begin, layer_end));
+  if (st != FLOWKV_OK || pl->pack.sched.chunks.empty()) return st;
+  const uint32_t vec = ((uintptr_t)window % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
+  RunOpts ro;
+  ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
+  return run(pl, pl->pack, pool_side(pl->src), dense_side(window, pl->g, layer_begin, layer_end), vec, stream, ro);
+}
+
+flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, uint64_t bytes, uint32_t layer_begin,
+                                   uint32_t layer_end, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  if (layer_begin > layer_end || layer_end > pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
+  flowkv_status st = check_staging(pl, pl->unpack, window, bytes, "unpack", window_bytes(pl, layer_begin, layer_end));
+  if (st != FLOWKV_OK || pl->unpack.sched.chunks.empty()) return st;
+  const uint32_t vec = ((uintptr_t)window % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
+  RunOpts ro;
+  ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
+  return run(pl, pl->unpack, dense_side(window, pl->g, layer_begin, layer_end), pool_side(pl->dst), vec, stream, ro);
+}
+
+namespace {
+uint32_t via_host_chunks(const flowkv_plan_t* pl, uint32_t n_chunks) {
+  if (n_chunks == 0) n_chunks = 16;      // measured on B200 (profiles/r01_sweep.md)
+  return std::max<uint32_t>(1, std::min(n_chunks, pl->g.L));
+}
+uint64_t via_host_slot_bytes(const flowkv_plan_t* pl, uint32_t n_chunks) {
+  const uint32_t L = pl->g.L;
+  uint32_t most = 0;                     // layers of the largest chunk
+  for (uint32_t c = 0; c < n_chunks; ++c)
+    most = std::max<uint32_t>(most, (uint32_t)((uint64_t)L * (c + 1) / n_chunks - (uint64_t)L * c / n_chunks));
+  return (window_bytes(pl, 0, most) + 255) & ~255ull;
+}
+}  // namespace
+
+flowkv_status flowkv_via_host_scratch_bytes(const flowkv_plan_t* pl, uint32_t n_chunks, uint64_t* bytes) {
+  if (!pl || !bytes) return fail(FLOWKV_ERR_INVALID_ARG, "NULL argument");
+  *bytes = 4 * via_host_slot_bytes(pl, via_host_chunks(pl, n_chunks));
+  return FLOWKV_OK;
+}
+
 flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_staging, uint64_t bytes, uint32_t n_chunks,
-                                       uint32_t ctas_per_kernel, void* stream) {
+                                       uint32_t ctas_per_kernel, void* device_scratch, uint64_t scratch_bytes,
+                                       void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
   flowkv_status st = check_staging(pl, pl->pack, host_staging, bytes, "pack");
   if (st != FLOWKV_OK) return st;
@@ -581,8 +644,13 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   if (pl->pack.sched.chunks.empty()) return FLOWKV_OK;
   if (!pl->on_device) return fail(FLOWKV_ERR_UNSUPPORTED, "plan was built by flowkv_plan_host and cannot run");
   const uint32_t L = pl->g.L;
-  if (n_chunks == 0) n_chunks = std::min<uint32_t>(L, 16);   // measured on B200: 16 chunks x 64 CTAs (profiles/r01_sweep.md)
-  n_chunks = std::min(n_chunks, L);
+  n_chunks = via_host_chunks(pl, n_chunks);
+  const bool engines = device_scratch != nullptr;          // copy engines drive the link, kernels stay in HBM
+  const uint64_t slot = via_host_slot_bytes(pl, n_chunks);
+  if (engines) {
+    if ((uintptr_t)device_scratch % 256) return fail(FLOWKV_ERR_ALIGN, "device_scratch is not 256-byte aligned");
+    if (scratch_bytes < 4 * slot) return fail(FLOWKV_ERR_STAGING_TOO_SMALL, "device_scratch smaller than flowkv_via_host_scratch_bytes()");
+  }
   cudaStream_t s = (cudaStream_t)stream;
   cudaError_t e;
   if (!pl->aux) {
@@ -595,7 +663,7 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
     pl->events.push_back(ev);
   }
-  // the unpack side (aux) starts after everything already queued on the caller's stream
+  // the inbound side (aux) starts after everything already queued on the caller's stream
   cudaEvent_t e_start = pl->events[n_chunks], e_done = pl->events[n_chunks + 1];
   if ((e = cudaEventRecord(e_start, s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
   if ((e = cudaStreamWaitEvent(pl->aux, e_start, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
@@ -603,17 +671,38 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   const uint32_t vecu = ((uintptr_t)host_staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true;
-  ro.max_grid = ctas_per_kernel ? ctas_per_kernel : 64;   // a PCIe-bound kernel needs few CTAs; both must be co-resident
+  // direct mode: a PCIe-bound kernel needs few CTAs and both directions' kernels must be co-resident
+  ro.max_grid = engines ? ctas_per_kernel : (ctas_per_kernel ? ctas_per_kernel : 64);
+  char* scratch = (char*)device_scratch;
+  uint32_t k = 0;                                          // non-empty chunks so far (scratch slot parity)
   for (uint32_t c = 0; c < n_chunks; ++c) {
-    ro.layer_begin = (uint32_t)((uint64_t)L * c / n_chunks);
-    ro.layer_end = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
-    if (ro.layer_begin == ro.layer_end) continue;
-    st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);      // D2H on `stream`
+    const uint32_t l0 = (uint32_t)((uint64_t)L * c / n_chunks), l1 = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
+    ro.layer_begin = l0;
+    ro.layer_end = l1;
+    if (l0 == l1) continue;
+    if (!engines) {
+      st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);      // D2H on `stream`
+      if (st != FLOWKV_OK) return st;
+      if ((e = cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+      if ((e = cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, pl->aux, ro);   // H2D on aux
+      if (st != FLOWKV_OK) return st;
+      continue;
+    }
+    // copy-engine mode: chunk c is its own dense message (layer window [l0,l1)) at host offset window_bytes(0,l0)
+    const uint64_t wb = window_bytes(pl, l0, l1);
+    char* out_slot = scratch + (k & 1) * slot;             // outbound slots 0,1 live on `stream`
+    char* in_slot = scratch + (2 + (k & 1)) * slot;        // inbound slots 2,3 live on aux
+    char* host = (char*)host_staging + window_bytes(pl, 0, l0);
+    st = run(pl, pl->pack, pool_side(pl->src), dense_side(out_slot, pl->g, l0, l1), pl->pack.shape.vec_bytes, s, ro);
     if (st != FLOWKV_OK) return st;
+    if ((e = cudaMemcpyAsync(host, out_slot, wb, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(D2H)");
     if ((e = cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
     if ((e = cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
-    st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, pl->aux, ro);   // H2D on aux
+    if ((e = cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(H2D)");
+    st = run(pl, pl->unpack, dense_side(in_slot, pl->g, l0, l1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, pl->aux, ro);
     if (st != FLOWKV_OK) return st;
+    ++k;
   }
   if ((e = cudaEventRecord(e_done, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
   if ((e = cudaStreamWaitEvent(s, e_done, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");

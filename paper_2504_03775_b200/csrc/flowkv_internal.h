@@ -15,13 +15,13 @@ namespace flowkv {
 // Device-visible schedule entry ("chunk"): one unit of work of one plane.  The same chunk list
 // serves every plane p = 2*layer + kv; the kernel adds the plane offset of each side:
 //   pool side   : layer*s_layer + kv*s_kv
-//   dense side  : p * req_tokens * tok_bytes            (wire format A12: [req][l][c][t][h][d])
+//   dense side  : (p - plane0) * req_tokens * tok_bytes (wire format A12: [req][l][c][t][h][d])
 // span mode: `n` BYTES that are contiguous on both sides.
 // rows mode: `n` TOKENS; token t, head h of the chunk sits at off + t*s_token + h*s_head per side.
 // ---------------------------------------------------------------------------------------------
 struct alignas(32) Chunk {
-  int64_t  src_off;      // bytes from the src side's base, plane offset excluded
-  int64_t  dst_off;      // bytes from the dst side's base, plane offset excluded
+  int64_t  src_off;      // pool side: bytes from the base, plane offset excluded;
+  int64_t  dst_off;      // dense side: (staging_tok_off << 32) | token_in_request (see side_offset())
   uint32_t n;            // span: bytes (multiple of the vector width); rows: tokens
   uint32_t req_tokens;   // T_r of the owning request (dense-side plane stride = T_r * tok_bytes)
   uint32_t request;      // owning request (reporting only)
@@ -35,9 +35,10 @@ enum Mode : uint32_t { MODE_ABSENT = 0, MODE_SPAN = 1, MODE_ROWS = 2, MODE_FLAT 
 
 struct Side {            // one end of a copy as the kernel sees it
   char*    base;         // device (or mapped host) pointer
-  int64_t  s_layer, s_kv, s_token, s_head;   // bytes; s_token/s_head used in rows mode only
+  int64_t  s_layer, s_kv, s_token, s_head;   // bytes; s_token/s_head used in rows mode only.  Dense side:
+                         // s_layer = bytes per token of the layer window the buffer holds, s_kv unused
   uint32_t dense;        // 1: dense staging buffer, 0: paged pool
-  uint32_t _pad;
+  uint32_t plane0;       // dense side: first plane of the layer window the buffer holds (0 = whole wire format)
 };
 
 // Plans whose every schedule has at most this many entries pass them in the kernel parameters

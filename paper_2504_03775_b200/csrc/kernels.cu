@@ -110,9 +110,20 @@ struct ParamChunks {
   __device__ __forceinline__ Chunk get(uint32_t i) const { return c[i]; }    // constant-bank load
 };
 
-__device__ __forceinline__ int64_t plane_offset(const Side& s, uint32_t plane, uint32_t req_tokens, uint32_t tok_bytes) {
-  return s.dense ? (int64_t)plane * ((int64_t)req_tokens * tok_bytes)
-                 : (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv;
+// Byte offset of a chunk inside one plane of one side.
+//   pool side  : layer*s_layer + kv*s_kv + off                                    (off in bytes)
+//   dense side : off = (staging_tok_off << 32) | token_in_request.  The buffer holds the layer window
+//                [plane0/2, ...) in wire order [request][layer][K|V][token][head][dim] (A12), so the
+//                chunk sits at  staging_tok_off * window_bytes_per_token            (request base)
+//                             + (plane - plane0) * T_r * tok_bytes                  (plane slab)
+//                             + token_in_request * tok_bytes.
+__device__ __forceinline__ int64_t side_offset(const Side& s, int64_t off, uint32_t plane, uint32_t req_tokens,
+                                               uint32_t tok_bytes) {
+  if (s.dense) {
+    const uint32_t tok0 = (uint32_t)((uint64_t)off >> 32), t = (uint32_t)off;
+    return (int64_t)tok0 * s.s_layer + ((int64_t)(plane - s.plane0) * req_tokens + t) * (int64_t)tok_bytes;
+  }
+  return (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv + off;
 }
 
 __device__ __forceinline__ void decode_tile(const KernelParams& p, uint32_t tile, uint32_t& plane, uint32_t& ci) {
@@ -196,8 +207,8 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
       decode_tile(p, next, nplane, nci);
       cn = cs.get(nci);
     }
-    const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
-    char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    const char* __restrict__ s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* __restrict__ d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     copy_span<VEC, UNROLL, HINT>(s, d, c.n, lane, step, pol);
     c = cn;
     plane = nplane;
@@ -230,8 +241,8 @@ __global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ K
       decode_tile(p, next, nplane, nci);
       cn = cs.get(nci);
     }
-    const char* __restrict__ s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
-    char* __restrict__ d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    const char* __restrict__ s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* __restrict__ d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
     c = cn;
     plane = nplane;
@@ -274,8 +285,8 @@ __global__ void __launch_bounds__(512, 2) fk_flat_ldst(const __grid_constant__ K
     uint32_t plane, ci;
     decode_tile(p, tile, plane, ci);
     const Chunk c = cs.get(p.n_flat + ci);
-    const char* s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
-    char* d = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    const char* s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
   }
 }
@@ -343,9 +354,9 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
     uint32_t plane, ci;
     decode_tile(p, first + k * stride, plane, ci);
     const Chunk c = cs.get(ci);
-    const char* s = p.src.base + plane_offset(p.src, plane, c.req_tokens, p.tok_bytes) + c.src_off;
+    const char* s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
     const uint32_t slot = k % n_stages;
-    dptr[slot] = p.dst.base + plane_offset(p.dst, plane, c.req_tokens, p.tok_bytes) + c.dst_off;
+    dptr[slot] = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     nbytes[slot] = c.n;
     mbar_expect_tx(&full[slot], c.n);
     bulk_g2s(ring + (size_t)slot * stage_bytes, s, c.n, &full[slot], pol);

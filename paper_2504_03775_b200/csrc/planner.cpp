@@ -174,14 +174,14 @@ static void rows_chunks(const flowkv_pool* src, const flowkv_pool* dst, const Ge
       n = std::min(n, src->block_size - so);
       c.src_off = pool_off(src, (uint32_t)S[t / src->block_size], so);
     } else {
-      c.src_off = dense0 + (int64_t)t * g.tok_bytes;
+      c.src_off = dense0 | (int64_t)t;
     }
     if (dst) {
       const uint32_t dof = t & (dst->block_size - 1);
       n = std::min(n, dst->block_size - dof);
       c.dst_off = pool_off(dst, (uint32_t)D[t / dst->block_size], dof);
     } else {
-      c.dst_off = dense0 + (int64_t)t * g.tok_bytes;
+      c.dst_off = dense0 | (int64_t)t;
     }
     c.n = n;
     c.req_tokens = rq.num_tokens;
@@ -262,18 +262,19 @@ void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geomet
   }
   for (const flowkv_segment& sg : segs) {
     const uint32_t T = reqs[sg.request].num_tokens;
-    // dense side: request base + token offset; the plane term (p*T*tok_bytes) is added by the kernel
-    const int64_t dense0 = (int64_t)(sg.staging_tok_off * g.bytes_per_token);
+    // dense side: (staging_tok_off << 32) | token_in_request; the kernel turns it into bytes for the layer
+    // window the staging buffer holds (side_offset() in kernels.cu)
+    const int64_t dense0 = (int64_t)(sg.staging_tok_off << 32);
     if (span) {
       // the whole segment is one contiguous byte range per plane on both sides
-      const int64_t s0 = src ? pool_off(src, sg.src_block, sg.src_tok_off) : dense0 + (int64_t)sg.first_token * g.tok_bytes;
-      const int64_t d0 = dst ? pool_off(dst, sg.dst_block, sg.dst_tok_off) : dense0 + (int64_t)sg.first_token * g.tok_bytes;
+      const int64_t s0 = src ? pool_off(src, sg.src_block, sg.src_tok_off) : dense0 | (int64_t)sg.first_token;
+      const int64_t d0 = dst ? pool_off(dst, sg.dst_block, sg.dst_tok_off) : dense0 | (int64_t)sg.first_token;
       uint32_t done = 0;
       while (done < sg.n_tokens) {
         const uint32_t n = std::min(tile_tokens, sg.n_tokens - done);
         Chunk c{};
-        c.src_off = s0 + (int64_t)done * g.tok_bytes;
-        c.dst_off = d0 + (int64_t)done * g.tok_bytes;
+        c.src_off = s0 + (int64_t)done * (src ? (int64_t)g.tok_bytes : 1);    // dense side counts tokens
+        c.dst_off = d0 + (int64_t)done * (dst ? (int64_t)g.tok_bytes : 1);
         c.n = n * g.tok_bytes;
         c.req_tokens = T;
         c.request = sg.request;

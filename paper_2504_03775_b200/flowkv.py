@@ -34,6 +34,7 @@ EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_pla
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
            "flowkv_launch_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
            "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host",
+           "flowkv_window_bytes", "flowkv_pack_window", "flowkv_unpack_window", "flowkv_via_host_scratch_bytes",
            "flowkv_alloc_create", "flowkv_alloc_allocate", "flowkv_alloc_free", "flowkv_alloc_stats",
            "flowkv_alloc_destroy"]
 
@@ -102,7 +103,12 @@ def _load() -> C.CDLL:
     lib.flowkv_transfer_layers.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
     lib.flowkv_pack_layers.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
     lib.flowkv_unpack_layers.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
-    lib.flowkv_transfer_via_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.flowkv_transfer_via_host.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p,
+                                             C.c_uint64, C.c_void_p]
+    lib.flowkv_window_bytes.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, P(C.c_uint64)]
+    lib.flowkv_pack_window.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.flowkv_unpack_window.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.flowkv_via_host_scratch_bytes.argtypes = [C.c_void_p, C.c_uint32, P(C.c_uint64)]
     lib.flowkv_plan_destroy.argtypes = [C.c_void_p]
     lib.flowkv_plan_destroy.restype = None
     lib.flowkv_status_string.argtypes = [C.c_int]
@@ -311,9 +317,30 @@ def flowkv_unpack_layers(plan: Plan, staging: int, nbytes: int, layer_begin: int
 
 
 def flowkv_transfer_via_host(plan: Plan, host_staging: int, nbytes: int, n_chunks: int = 0, ctas_per_kernel: int = 0,
-                             stream: int = 0) -> None:
+                             stream: int = 0, device_scratch: int = 0, scratch_bytes: int = 0) -> None:
     _check(_lib.flowkv_transfer_via_host(plan.handle, C.c_void_p(host_staging), nbytes, n_chunks, ctas_per_kernel,
+                                         C.c_void_p(device_scratch) if device_scratch else None, scratch_bytes,
                                          C.c_void_p(stream)))
+
+
+def flowkv_via_host_scratch_bytes(plan: Plan, n_chunks: int = 0) -> int:
+    out = C.c_uint64()
+    _check(_lib.flowkv_via_host_scratch_bytes(plan.handle, n_chunks, C.byref(out)))
+    return int(out.value)
+
+
+def flowkv_window_bytes(plan: Plan, layer_begin: int, layer_end: int) -> int:
+    out = C.c_uint64()
+    _check(_lib.flowkv_window_bytes(plan.handle, layer_begin, layer_end, C.byref(out)))
+    return int(out.value)
+
+
+def flowkv_pack_window(plan: Plan, window: int, nbytes: int, layer_begin: int, layer_end: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_pack_window(plan.handle, C.c_void_p(window), nbytes, layer_begin, layer_end, C.c_void_p(stream)))
+
+
+def flowkv_unpack_window(plan: Plan, window: int, nbytes: int, layer_begin: int, layer_end: int, stream: int = 0) -> None:
+    _check(_lib.flowkv_unpack_window(plan.handle, C.c_void_p(window), nbytes, layer_begin, layer_end, C.c_void_p(stream)))
 
 
 def flowkv_plan_destroy(plan: Plan) -> None:

@@ -69,3 +69,16 @@ def run_transfer_and_check(w: synth.Workload, tuning=None, fill=None, flags=0):
     assert_same(got, exp, f"{w.name} transfer {tuning}")
     assert_same(P.to_numpy(dp.src_buf), src_before, "src pool must not change")
     return dp, plan, exp
+
+
+def window_of(full_wire: np.ndarray, w: synth.Workload, l0: int, l1: int) -> np.ndarray:
+    """Layer window [l0,l1) of the wire format, by its definition: per request, the slab of planes
+    [2*l0, 2*l1) of that request's region ([request][layer][K|V][token][head][dim]), requests concatenated."""
+    tokb = w.shape.num_kv_heads * w.shape.head_dim * w.shape.elem_bytes
+    bpt = w.shape.bytes_per_token
+    parts, off = [], 0
+    for r in w.requests:
+        base = off * bpt
+        parts.append(full_wire[base + 2 * l0 * r.num_tokens * tokb: base + 2 * l1 * r.num_tokens * tokb])
+        off += r.num_tokens
+    return np.concatenate(parts) if parts else np.zeros(0, np.uint8)

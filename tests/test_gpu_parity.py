@@ -473,3 +473,73 @@ def test_small_plans_travel_in_kernel_params(n_blocks, variant):
     forced.transfer()
     torch.cuda.synchronize()
     G.assert_same(P.to_numpy(dp.dst_buf), exp, "uploaded plan")
+
+
+@pytest.mark.parametrize("w_fn", [
+    lambda: synth.config3_batched(n_requests=3, num_layers=5),
+    lambda: synth.config4_hetero(n_requests=2, num_layers=5),
+])
+def test_layer_window_pack_unpack(w_fn):
+    """flowkv_pack_window / flowkv_unpack_window: a window holds only layers [l0,l1) as a self-contained dense
+    message == those planes cut out of the oracle's wire format; unpacking the windows one by one rebuilds the
+    oracle's transfer; bytes past the window are untouched; a short buffer is rejected."""
+    w = w_fn()
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    full = G.oracle_pack(w, src_np)
+    plan = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER)
+    L = w.shape.num_layers
+    assert F.flowkv_window_bytes(plan, 0, L) == plan.stats["staging_bytes"]
+    P.fill_sentinel(dp.dst_buf)
+    for l0, l1 in [(0, 2), (2, 3), (3, 5), (4, 4)]:
+        nb = F.flowkv_window_bytes(plan, l0, l1)
+        assert nb == w.total_tokens * 2 * (l1 - l0) * w.shape.num_kv_heads * w.shape.head_dim * 2
+        win = P.alloc_bytes(nb + 64)
+        P.fill_sentinel(win)
+        n0 = F.flowkv_launch_count()
+        F.flowkv_pack_window(plan, win.data_ptr(), nb, l0, l1)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if l1 > l0 else 0)
+        got = P.to_numpy(win)
+        G.assert_same(got[:nb], G.window_of(full, w, l0, l1), f"pack_window [{l0},{l1})")
+        assert np.all(got[nb:] == P.SENTINEL_BYTE)
+        F.flowkv_unpack_window(plan, win.data_ptr(), nb, l0, l1)
+        if nb:
+            with pytest.raises(F.FlowKVError) as ei:
+                F.flowkv_pack_window(plan, win.data_ptr(), nb - 1, l0, l1)
+            assert ei.value.status == F.FLOWKV_ERR_STAGING_TOO_SMALL
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "windows [0,2)+[2,3)+[3,5) unpacked == transfer")
+    with pytest.raises(F.FlowKVError):
+        F.flowkv_window_bytes(plan, 3, 6)
+
+
+@pytest.mark.parametrize("n_chunks,ctas", [(0, 0), (1, 0), (4, 8), (100, 0)])
+def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas):
+    """Copy-engine mode of flowkv_transfer_via_host: pack_window -> D2H memcpy -> H2D memcpy -> unpack_window per
+    layer chunk through caller-provided device scratch.  dst == oracle transfer; the host buffer holds the chunks
+    back to back, each == its layer window of the oracle's wire format."""
+    L = 6
+    w = synth.config3_batched(n_requests=3, num_layers=L)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    stream = torch.cuda.Stream()
+    plan = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER, None, stream.cuda_stream)
+    nbytes = plan.stats["staging_bytes"]
+    host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    host.fill_(P.SENTINEL_BYTE)
+    sb = F.flowkv_via_host_scratch_bytes(plan, n_chunks)
+    scratch = P.alloc_bytes(sb)
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, n_chunks, ctas, stream.cuda_stream, scratch.data_ptr(), sb - 1)
+    assert ei.value.status == F.FLOWKV_ERR_STAGING_TOO_SMALL
+    n0 = F.flowkv_launch_count()
+    F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, n_chunks, ctas, stream.cuda_stream, scratch.data_ptr(), sb)
+    stream.synchronize()
+    chunks = min(n_chunks, L) if n_chunks else L          # auto = min(L, 16)
+    assert F.flowkv_launch_count() - n0 == 2 * chunks
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host (copy engines): dst")
+    full = G.oracle_pack(w, src_np)
+    exp_host = np.concatenate([G.window_of(full, w, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
+    G.assert_same(host.numpy(), exp_host, "via host (copy engines): chunked wire bytes")
+    plan.destroy()
