@@ -1,0 +1,33 @@
+"""Peer pools over CUDA IPC — the paper's single-machine "IPC" mode.
+
+A decode-side process owns its KV pool and exports it; the prefill-side process maps it and runs the SAME
+``flowkv_transfer`` kernel with the mapped pointer as the dst pool: a one-sided put, no collective, no
+staging buffer, no receiver-side kernel.  On a multi-GPU node the mapping crosses NVLink; with one GPU both
+processes share the device and the stores land in the same HBM.
+
+torch is used for what it is here for — device memory and its IPC plumbing (``cudaIpcGetMemHandle`` /
+``cudaIpcOpenMemHandle`` behind ``torch.multiprocessing.reductions``); no KV byte is moved by torch.
+"""
+from __future__ import annotations
+
+import pickle
+
+import torch
+from torch.multiprocessing import reductions
+
+
+def export_pool(buf: torch.Tensor) -> bytes:
+    """Serialise an IPC handle of a CUDA uint8 buffer.  The exporting process must keep ``buf`` alive (and stay
+    alive itself) for as long as any importer uses the mapping."""
+    assert buf.is_cuda and buf.dtype == torch.uint8 and buf.is_contiguous()
+    fn, args = reductions.reduce_tensor(buf)
+    return pickle.dumps((fn, args))
+
+
+def import_pool(handle: bytes) -> torch.Tensor:
+    """Map an exported buffer into this process; ``.data_ptr()`` is what ``flowkv.make_pool`` takes.
+    The mapping lives as long as the returned tensor."""
+    fn, args = pickle.loads(handle)
+    t = fn(*args)
+    assert t.is_cuda and t.dtype == torch.uint8
+    return t

@@ -543,3 +543,53 @@ def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas):
     exp_host = np.concatenate([G.window_of(full, w, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
     G.assert_same(host.numpy(), exp_host, "via host (copy engines): chunked wire bytes")
     plan.destroy()
+
+
+def test_peer_pool_over_cuda_ipc():
+    """NEXT-3 / P:L90 'IPC' mode: the dst pool belongs to ANOTHER process (the decode side); this process maps it
+    through CUDA IPC and flowkv_transfer stores straight into it — a one-sided put, one launch.  The owner then
+    reads its own pool back and it must equal the oracle over every byte."""
+    import queue
+    import torch.multiprocessing as mp
+    from paper_2504_03775_b200 import peer
+    from tests import peer_child
+
+    w = synth.config4_hetero(n_requests=2, num_layers=2)
+    nbytes = w.dst.bytes(w.shape)
+    ctx = mp.get_context("spawn")
+    to_parent, to_child = ctx.Queue(), ctx.Queue()
+    child = ctx.Process(target=peer_child.decode_side, args=(nbytes, P.SENTINEL_BYTE, to_parent, to_child), daemon=True)
+    child.start()
+    try:
+        try:
+            kind, handle = to_parent.get(timeout=180)
+        except queue.Empty:
+            pytest.skip("decode-side process did not come up")
+        if kind == "error":
+            pytest.skip(f"CUDA IPC export unavailable here: {handle}")
+        try:
+            remote = peer.import_pool(handle)
+        except RuntimeError as e:
+            pytest.skip(f"CUDA IPC import unavailable here: {e}")
+        assert remote.numel() == nbytes
+        src_buf = P.alloc_bytes(w.src.bytes(w.shape))
+        P.fill_values(src_buf, "bits", w.shape.dtype, w.seed)
+        src = P.describe(w.src, w.shape, src_buf.data_ptr())
+        dst = P.describe(w.dst, w.shape, remote.data_ptr())           # the peer's memory
+        n0 = F.flowkv_launch_count()
+        plan = F.flowkv_plan(src, dst, P.requests_of(w), F.FLOWKV_CHECK_DST_ALIAS)
+        plan.transfer()
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == 1
+        to_child.put("written")
+        kind, blob = to_parent.get(timeout=180)
+        assert kind == "bytes", blob
+        got = np.frombuffer(blob, dtype=np.uint8)
+        G.assert_same(got, G.oracle_transfer(w, P.to_numpy(src_buf)), "peer pool over CUDA IPC")
+        plan.destroy()
+        del remote
+        to_child.put("done")
+        child.join(timeout=60)
+    finally:
+        if child.is_alive():
+            child.kill()
