@@ -189,7 +189,7 @@ def cpu_baseline(w, src_dev, target_s: float = 12.0) -> dict:
     moved = oracle_run(O, gs, gd, src, dst, w)
     dt = time.perf_counter() - t0
     reps = 1
-    while dt < target_s and reps < 64:                               # repeat the same sample until ~target_s of CPU work
+    while dt < target_s and reps < 1024:                               # repeat the same sample until ~target_s of CPU work
         t1 = time.perf_counter()
         moved += oracle_run(O, gs, gd, src, dst, w)
         dt += time.perf_counter() - t1

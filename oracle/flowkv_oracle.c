@@ -24,7 +24,8 @@
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): numpy fancy-indexing
  * special cases, a self-describing pool decoded from the definition, identity
  * tables == memcmp, untouched-byte sentinels, all 65,536 16-bit patterns,
- * pack∘unpack identity, brute-force minimal partition count on tiny tables,
+ * pack∘unpack identity, layer windows == planes cut out of the wire format,
+ * brute-force minimal partition count on tiny tables,
  * the paper's "fully contiguous => 1 transfer" and
  * "calls per block = L x 2", hand-worked fixtures in tests/golden/.
  * Unpinned by the paper: its printed latencies and the 23,469-call average
@@ -124,6 +125,51 @@ int okv_unpack(const uint8_t* staging, uint64_t req_tok_off, uint8_t* dst, const
           for (uint32_t d = 0; d < dp->head_dim; ++d)
             okv_copy_elem(dst + okv_addr(dp, l, c, db, dof, h, d),
                           staging + okv_staging_addr(dp, req_tok_off, T, l, c, t, h, d), e);
+  }
+  return 0;
+}
+
+/* Layer-window wire format (reading A20): a message that carries only layers [w0,w1) — what a
+ * layer-wise / pipelined sender puts on the wire ("layer by layer", P:L222-224 the layerwise ablation) —
+ * is the wire format of a model that has just those w1-w0 layers:
+ *   window[request][layer - w0][K|V][token][head][dim], requests concatenated,
+ *   request r starting at byte req_tok_off * 2*(w1-w0)*Hkv*Dh*e.
+ * The window [0,L) is the format of okv_pack. */
+static inline int64_t okv_window_addr(const okv_pool* p, uint32_t w0, uint32_t w1, uint64_t req_tok_off, uint32_t T,
+                                      uint32_t l, uint32_t c, uint32_t t, uint32_t h, uint32_t d) {
+  int64_t bpt = (int64_t)2 * (w1 - w0) * p->num_kv_heads * p->head_dim * p->elem_bytes;
+  int64_t idx = ((((int64_t)((l - w0) * 2 + c) * T + t) * p->num_kv_heads + h) * p->head_dim + d);
+  return (int64_t)req_tok_off * bpt + idx * p->elem_bytes;
+}
+
+int okv_pack_window(const uint8_t* src, const okv_pool* sp, const int32_t* src_tab, uint32_t T,
+                    uint8_t* window, uint64_t req_tok_off, uint32_t w0, uint32_t w1) {
+  const uint32_t e = sp->elem_bytes;
+  for (uint32_t t = 0; t < T; ++t) {
+    int64_t sb = src_tab[t / sp->block_size]; uint32_t so = t % sp->block_size;
+    if (sb < 0 || sb >= (int64_t)sp->num_blocks) return -1;
+    for (uint32_t l = w0; l < w1; ++l)
+      for (uint32_t c = 0; c < 2; ++c)
+        for (uint32_t h = 0; h < sp->num_kv_heads; ++h)
+          for (uint32_t d = 0; d < sp->head_dim; ++d)
+            okv_copy_elem(window + okv_window_addr(sp, w0, w1, req_tok_off, T, l, c, t, h, d),
+                          src + okv_addr(sp, l, c, sb, so, h, d), e);
+  }
+  return 0;
+}
+
+int okv_unpack_window(const uint8_t* window, uint64_t req_tok_off, uint8_t* dst, const okv_pool* dp,
+                      const int32_t* dst_tab, uint32_t T, uint32_t w0, uint32_t w1) {
+  const uint32_t e = dp->elem_bytes;
+  for (uint32_t t = 0; t < T; ++t) {
+    int64_t db = dst_tab[t / dp->block_size]; uint32_t dof = t % dp->block_size;
+    if (db < 0 || db >= (int64_t)dp->num_blocks) return -1;
+    for (uint32_t l = w0; l < w1; ++l)
+      for (uint32_t c = 0; c < 2; ++c)
+        for (uint32_t h = 0; h < dp->num_kv_heads; ++h)
+          for (uint32_t d = 0; d < dp->head_dim; ++d)
+            okv_copy_elem(dst + okv_addr(dp, l, c, db, dof, h, d),
+                          window + okv_window_addr(dp, w0, w1, req_tok_off, T, l, c, t, h, d), e);
   }
   return 0;
 }

@@ -58,6 +58,12 @@ def _load():
         lib.okv_unpack.restype = C.c_int
         lib.okv_unpack.argtypes = [u8p, C.c_uint64, u8p, C.POINTER(_Pool), i32p, C.c_uint32,
                                    C.c_uint32, C.c_uint32]
+        lib.okv_pack_window.restype = C.c_int
+        lib.okv_pack_window.argtypes = [u8p, C.POINTER(_Pool), i32p, C.c_uint32, u8p, C.c_uint64,
+                                        C.c_uint32, C.c_uint32]
+        lib.okv_unpack_window.restype = C.c_int
+        lib.okv_unpack_window.argtypes = [u8p, C.c_uint64, u8p, C.POINTER(_Pool), i32p, C.c_uint32,
+                                          C.c_uint32, C.c_uint32]
         lib.okv_align.restype = C.c_uint64
         lib.okv_align.argtypes = [i32p, C.c_uint32, i32p, C.c_uint32, C.c_uint32, u32p, u32p, C.c_uint64]
         lib.okv_blockwise_calls.restype = C.c_uint64
@@ -175,6 +181,27 @@ def unpack(staging: np.ndarray, req_tok_off: int, dst: np.ndarray, dp: PoolGeom,
     assert len(dt) * dp.block_size >= T
     rc = _load().okv_unpack(_u8(staging, False), req_tok_off, _u8(dst, True), C.byref(dp._c()),
                             dt.ctypes.data, T, l0, l1)
+    if rc != 0:
+        raise ValueError("oracle: block id out of range")
+
+
+def pack_window(src: np.ndarray, sp: PoolGeom, src_tab, T: int, window: np.ndarray, req_tok_off: int,
+                w0: int, w1: int) -> None:
+    """Layers [w0,w1) of one request into a buffer that holds only those layers (reading A20)."""
+    st = _tab(src_tab)
+    assert len(st) * sp.block_size >= T
+    rc = _load().okv_pack_window(_u8(src, False), C.byref(sp._c()), st.ctypes.data, T, _u8(window, True),
+                                 req_tok_off, w0, w1)
+    if rc != 0:
+        raise ValueError("oracle: block id out of range")
+
+
+def unpack_window(window: np.ndarray, req_tok_off: int, dst: np.ndarray, dp: PoolGeom, dst_tab, T: int,
+                  w0: int, w1: int) -> None:
+    dt = _tab(dst_tab)
+    assert len(dt) * dp.block_size >= T
+    rc = _load().okv_unpack_window(_u8(window, False), req_tok_off, _u8(dst, True), C.byref(dp._c()),
+                                   dt.ctypes.data, T, w0, w1)
     if rc != 0:
         raise ValueError("oracle: block id out of range")
 

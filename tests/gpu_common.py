@@ -82,3 +82,15 @@ def window_of(full_wire: np.ndarray, w: synth.Workload, l0: int, l1: int) -> np.
         parts.append(full_wire[base + 2 * l0 * r.num_tokens * tokb: base + 2 * l1 * r.num_tokens * tokb])
         off += r.num_tokens
     return np.concatenate(parts) if parts else np.zeros(0, np.uint8)
+
+
+def oracle_pack_window(w: synth.Workload, src_np: np.ndarray, l0: int, l1: int) -> np.ndarray:
+    """The oracle's layer window [l0,l1) of the whole batch (oracle/flowkv_oracle.c okv_pack_window)."""
+    gs = geom(w.src, w.shape)
+    tokb = w.shape.num_kv_heads * w.shape.head_dim * w.shape.elem_bytes
+    out = np.full(w.total_tokens * 2 * (l1 - l0) * tokb, P.SENTINEL_BYTE, np.uint8)
+    off = 0
+    for r in w.requests:
+        O.pack_window(src_np, gs, r.src_blocks, r.num_tokens, out, off, l0, l1)
+        off += r.num_tokens
+    return out

@@ -501,7 +501,8 @@ def test_layer_window_pack_unpack(w_fn):
         torch.cuda.synchronize()
         assert F.flowkv_launch_count() - n0 == (1 if l1 > l0 else 0)
         got = P.to_numpy(win)
-        G.assert_same(got[:nb], G.window_of(full, w, l0, l1), f"pack_window [{l0},{l1})")
+        G.assert_same(got[:nb], G.oracle_pack_window(w, src_np, l0, l1), f"pack_window [{l0},{l1})")
+        assert np.array_equal(got[:nb], G.window_of(full, w, l0, l1))
         assert np.all(got[nb:] == P.SENTINEL_BYTE)
         F.flowkv_unpack_window(plan, win.data_ptr(), nb, l0, l1)
         if nb:
@@ -539,8 +540,7 @@ def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas):
     chunks = min(n_chunks, L) if n_chunks else L          # auto = min(L, 16)
     assert F.flowkv_launch_count() - n0 == 2 * chunks
     G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host (copy engines): dst")
-    full = G.oracle_pack(w, src_np)
-    exp_host = np.concatenate([G.window_of(full, w, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
+    exp_host = np.concatenate([G.oracle_pack_window(w, src_np, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
     G.assert_same(host.numpy(), exp_host, "via host (copy engines): chunked wire bytes")
     plan.destroy()
 

@@ -235,6 +235,69 @@ def test_pack_equals_numpy_gather_and_unpack_inverts(layout):
     assert np.array_equal(d1, d2)
 
 
+@pytest.mark.parametrize("layout", ["lkbthd", "blkthd"])
+def test_layer_window_equals_planes_cut_out_of_the_wire_format(layout):
+    """Reading A20: a window [w0,w1) is numpy's gather restricted to those layers, i.e. the slab of planes
+    [2*w0, 2*w1) of each request's region of the (already pinned) full wire format; the window [0,L) IS the
+    wire format; unpacking disjoint windows rebuilds unpack of the whole.  Catches: a window base that still
+    uses 2*L planes per token, a plane index not rebased to w0, K|V order inside a layer."""
+    rng = np.random.default_rng(18)
+    L, H, D, NB, BS = 4, 2, 8, 12, 4
+    g = _geom(layout, L, H, D, NB, BS)
+    src = _rand_pool(rng, g.span_bytes())
+    Ts = [7, 12, 0, 5]
+    perm = rng.permutation(NB)
+    tabs, off = [], 0
+    for T in Ts:
+        nb = -(-T // BS)
+        tabs.append(perm[off:off + nb]); off += nb
+    tokb = H * D * 2
+    sv = Hh.logical_view(src, layout, L, NB, BS, H, D)
+    full = np.zeros(sum(Ts) * g.bytes_per_token, np.uint8)
+    tok_off = 0
+    for T, tab in zip(Ts, tabs):
+        O.pack(src, g, tab, T, full, tok_off)
+        tok_off += T
+    for w0, w1 in [(0, 4), (1, 3), (3, 4), (2, 2)]:
+        win = np.full(sum(Ts) * 2 * (w1 - w0) * tokb + 16, SENT, np.uint8)
+        exp_parts, cut_parts, tok_off = [], [], 0
+        for T, tab in zip(Ts, tabs):
+            O.pack_window(src, g, tab, T, win, tok_off, w0, w1)
+            exp_parts.append(sv[w0:w1, :, tab].reshape(w1 - w0, 2, len(tab) * BS, H, D)[:, :, :T].reshape(-1))
+            base = tok_off * g.bytes_per_token
+            cut_parts.append(full[base + 2 * w0 * T * tokb: base + 2 * w1 * T * tokb])
+            tok_off += T
+        body = win[:-16]
+        assert np.array_equal(body.view(np.uint16), np.concatenate(exp_parts))
+        assert np.array_equal(body, np.concatenate(cut_parts))
+        assert np.all(win[-16:] == SENT)
+        if (w0, w1) == (0, 4):
+            assert np.array_equal(body, full)
+    # unpack of windows [0,1) + [1,4) == unpack of the whole wire format
+    gd = _geom("blkhtd", L, H, D, NB, BS * 2)
+    dperm = rng.permutation(NB)
+    d1 = np.full(gd.span_bytes(), SENT, np.uint8)
+    d2 = np.full(gd.span_bytes(), SENT, np.uint8)
+    for w0, w1 in [(0, 1), (1, 4)]:
+        win = np.zeros(sum(Ts) * 2 * (w1 - w0) * tokb, np.uint8)
+        tok_off = doff = 0
+        for T, tab in zip(Ts, tabs):
+            nb = -(-T // (BS * 2))
+            O.pack_window(src, g, tab, T, win, tok_off, w0, w1)
+            tok_off += T
+        tok_off = doff = 0
+        for T, tab in zip(Ts, tabs):
+            nb = -(-T // (BS * 2))
+            O.unpack_window(win, tok_off, d1, gd, dperm[doff:doff + nb], T, w0, w1)
+            tok_off += T; doff += nb
+    tok_off = doff = 0
+    for T, tab in zip(Ts, tabs):
+        nb = -(-T // (BS * 2))
+        O.unpack(full, tok_off, d2, gd, dperm[doff:doff + nb], T)
+        tok_off += T; doff += nb
+    assert np.array_equal(d1, d2)
+
+
 def test_pack_unpack_identity_and_round_trip():
     """unpack(pack(pool,T),T) restores every named slot; transfer S->D then D->S restores src slots."""
     rng = np.random.default_rng(9)
