@@ -593,3 +593,69 @@ def test_peer_pool_over_cuda_ipc():
     finally:
         if child.is_alive():
             child.kill()
+
+
+@pytest.mark.parametrize("upload", [0, 1])
+def test_transfer_is_cuda_graph_capturable(upload):
+    """A built plan's transfer is one kernel launch and nothing else, so it can be captured into a CUDA graph and
+    replayed (launch-bound small transfers: replay costs one graph launch).  Replays reach the oracle's bytes."""
+    w = synth.config1_tiny()
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    stream = torch.cuda.Stream()
+    plan = dp.plan(F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, {"plan_in_params": upload}, stream.cuda_stream)
+    stream.synchronize()                      # the plan upload (if any) is done before capture begins
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=stream):
+        plan.transfer(torch.cuda.current_stream().cuda_stream)
+    exp = G.oracle_transfer(w, src_np)
+    for _ in range(3):
+        P.fill_sentinel(dp.dst_buf)
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        G.assert_same(P.to_numpy(dp.dst_buf), exp, "graph replay")
+    del g
+    plan.destroy()
+
+
+@pytest.mark.parametrize("layouts", [("lkbthd", "lkbthd"), ("lkbthd", "blkhtd"), ("blkthd", "blkthd")])
+@pytest.mark.parametrize("tuning", [None, {"variant": "bulk"}, {"plan_in_params": 1, "tile_bytes": 4096}])
+def test_guard_bands_around_both_pools_stay_intact(layouts, tuning):
+    """Own bounds check (compute-sanitizer is not available on the pool): each pool sits between two 64 KiB guard
+    bands inside one allocation, the request names the FIRST and the LAST block of both pools and ends in a partial
+    block; after transfer, pack and unpack every guard byte still holds its sentinel and dst == oracle."""
+    GUARD = 64 << 10
+    shape = synth.Shape(3, 2, 64, "fp16")
+    NB, BS, T = 12, 16, 5 * 16 + 7
+    stab = np.asarray([NB - 1, 0, 1, 5, 6, NB - 2], np.int32)
+    dtab = np.asarray([0, NB - 2, NB - 1, 3, 4, 7], np.int32)
+    ssp, dsp = synth.PoolSpec(layouts[0], BS, NB), synth.PoolSpec(layouts[1], BS, NB)
+    w = synth.Workload("guard", 36, shape, ssp, dsp, [synth.Request(T, stab, dtab)])
+    sbytes, dbytes = ssp.bytes(shape), dsp.bytes(shape)
+    sbig, dbig = P.alloc_bytes(sbytes + 2 * GUARD), P.alloc_bytes(dbytes + 2 * GUARD)
+    P.fill_sentinel(sbig)
+    P.fill_sentinel(dbig)
+    src_buf, dst_buf = sbig[GUARD:GUARD + sbytes], dbig[GUARD:GUARD + dbytes]
+    P.fill_values(src_buf, "bits", "fp16", 36)
+    src_np = P.to_numpy(src_buf)
+    src = P.describe(ssp, shape, src_buf.data_ptr())
+    dst = P.describe(dsp, shape, dst_buf.data_ptr())
+    plan = F.flowkv_plan(src, dst, P.requests_of(w), F.FLOWKV_CHECK_DST_ALIAS, tuning)
+    nbytes = plan.stats["staging_bytes"]
+    stg_big = P.alloc_bytes(nbytes + 2 * GUARD)
+    P.fill_sentinel(stg_big)
+    plan.transfer()
+    torch.cuda.synchronize()
+    exp = G.oracle_transfer(w, src_np)
+    G.assert_same(P.to_numpy(dst_buf), exp, "guarded transfer")
+    plan.pack(stg_big.data_ptr() + GUARD, nbytes)
+    P.fill_sentinel(dst_buf)
+    plan.unpack(stg_big.data_ptr() + GUARD, nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dst_buf), exp, "guarded unpack(pack)")
+    for name, big, n in (("src", sbig, sbytes), ("dst", dbig, dbytes), ("staging", stg_big, nbytes)):
+        b = P.to_numpy(big)
+        assert np.all(b[:GUARD] == P.SENTINEL_BYTE), f"{name}: bytes below the buffer were written"
+        assert np.all(b[GUARD + n:] == P.SENTINEL_BYTE), f"{name}: bytes above the buffer were written"
+    G.assert_same(P.to_numpy(src_buf), src_np, "src unchanged")
