@@ -183,3 +183,50 @@ def test_cfg4_full_size_fit_rule():
             a = s[2 * layer + c].index_select(0, ss)                    # [tok, H, D]
             b = d6[db, layer, c, :, dt, :]                              # [tok, H, D]
             assert torch.equal(a, b), f"layer {layer} kv {c}"
+
+
+def test_cfg5_largest_sweep_point_full_size():
+    """configs[4]'s largest and most fragmented point as bench_sweep.py runs it: 131,072 tokens (16 GiB payload),
+    src run length 1 (8,192 segments) over a 32 GiB pool; one launch."""
+    w = synth.config5_point(131072, 1)
+    _need(w.src.bytes(w.shape) + w.dst.bytes(w.shape))
+    dp = P.DevicePools(w)
+    n0 = F.flowkv_launch_count()
+    plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS | F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK)
+    plan.transfer()
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1
+    assert plan.stats["n_segments"] == 8192 and plan.stats["payload_bytes"] == 16 * 2 ** 30
+    for layer in (0, 31):
+        _lkbthd_layer_check(w, dp, layer)
+    _lkbthd_all_planes_property(w, dp)
+
+
+def test_cfg5_pack_to_pinned_host_32k_tokens_full_size():
+    """configs[4]'s device -> pinned-host point: 32,768 tokens = 4 GiB of wire format written by one kernel over
+    PCIe, and read back by one kernel into a sentinel pool.  Sampled layers of the wire bytes against the oracle's
+    pack (layer-range form, over a host copy of that src layer); every plane of the round trip through the
+    token-slot gather property."""
+    w = synth.config5_point(32768, 2)
+    _need(w.src.bytes(w.shape) + w.dst.bytes(w.shape))
+    dp = P.DevicePools(w)
+    plan = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER)
+    nbytes = plan.stats["staging_bytes"]
+    assert nbytes == 4 * 2 ** 30
+    host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    n0 = F.flowkv_launch_count()
+    plan.pack(host.data_ptr(), nbytes)
+    plan.unpack(host.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 2
+    gs = G.geom(w.src, w.shape)
+    r = w.requests[0]
+    T, tokb = r.num_tokens, 8 * 128 * 2
+    wire = host.numpy()
+    for layer in (0, 17, 31):
+        src_slab = dp.src_buf[layer * gs.s_layer:(layer + 1) * gs.s_layer].cpu().numpy()
+        g1 = O.PoolGeom.lkbthd(1, 8, 128, 2, w.src.num_blocks, 16)          # that layer as a one-layer pool
+        exp = np.zeros(2 * T * tokb, np.uint8)
+        O.pack(src_slab, g1, r.src_blocks, T, exp, 0)
+        G.assert_same(wire[2 * layer * T * tokb: 2 * (layer + 1) * T * tokb], exp, f"wire bytes of layer {layer}")
+    _lkbthd_all_planes_property(w, dp)

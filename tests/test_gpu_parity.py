@@ -515,17 +515,23 @@ def test_layer_window_pack_unpack(w_fn):
         F.flowkv_window_bytes(plan, 3, 6)
 
 
+@pytest.mark.parametrize("small", [False, True])
 @pytest.mark.parametrize("n_chunks,ctas", [(0, 0), (1, 0), (4, 8), (100, 0)])
-def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas):
+def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas, small):
     """Copy-engine mode of flowkv_transfer_via_host: pack_window -> D2H memcpy -> H2D memcpy -> unpack_window per
     layer chunk through caller-provided device scratch.  dst == oracle transfer; the host buffer holds the chunks
     back to back, each == its layer window of the oracle's wire format."""
     L = 6
-    w = synth.config3_batched(n_requests=3, num_layers=L)
+    if small:      # a plan small enough to ride in the kernel parameters (no upload)
+        w = synth.make_workload("via_small", 37, synth.Shape(L, 2, 64, "fp16"), [200, 90],
+                                "lkbthd", 16, ("geometric", 2.0), None, "blkhtd", 32, ("contiguous",), None)
+    else:
+        w = synth.config3_batched(n_requests=3, num_layers=L)
     dp = P.DevicePools(w, fill="bits")
     src_np = P.to_numpy(dp.src_buf)
     stream = torch.cuda.Stream()
     plan = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER, None, stream.cuda_stream)
+    assert (plan.stats["plan_device_bytes"] == 0) == small
     nbytes = plan.stats["staging_bytes"]
     host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
     host.fill_(P.SENTINEL_BYTE)
