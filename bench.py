@@ -293,12 +293,14 @@ def run_ours(args) -> None:
     barrier()
     clocks.start()
     n0 = F.flowkv_launch_count()
+    c0 = F.flowkv_api_call_count()
     e0.record(stream)
     for k in range(K):
         step(ka[k], kb[k])
     e1.record(stream)
     barrier()
     launches = F.flowkv_launch_count() - n0
+    api_calls = F.flowkv_api_call_count() - c0
     clk = clocks.stop()
     t_ms = e0.elapsed_time(e1)
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ka, kb)]))
@@ -323,7 +325,7 @@ def run_ours(args) -> None:
                                                         "vec_bytes", "cache_hint", "tile_order", "stages")}},
             "clocks": clk,
             "gpu_launches": int(launches),
-            "launches_per_batch": launches / K, "launches_per_request": launches / K / max(len(w.requests), 1),
+            "launches_per_batch": launches / K, "cuda_api_calls_per_batch": api_calls / K, "launches_per_request": launches / K / max(len(w.requests), 1),
             "latency_ms_per_request": t_ms / K / max(len(w.requests), 1),
             "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

@@ -257,6 +257,10 @@ FLOWKV_API const char* flowkv_last_error(void);          /* thread-local text of
 
 /* Number of kernels this library has launched in this process (monotonic; for launch accounting). */
 FLOWKV_API uint64_t flowkv_launch_count(void);
+/* Number of CUDA runtime calls this library has made that put work on a stream or (de)allocate stream-ordered
+ * memory — kernel launches, cudaMemcpyAsync, cudaMallocAsync / cudaFreeAsync, event records and waits
+ * (monotonic).  A small plan's whole step (plan + transfer + destroy) is 1 such call; an uploaded plan's is 6. */
+FLOWKV_API uint64_t flowkv_api_call_count(void);
 
 /* ---- comparison baselines (BASELINE.json north_star; they are NOT the product path) ----------
  * Each issues cudaMemcpyAsync D2D copies on `stream` and writes the number issued to *n_calls.

@@ -16,6 +16,15 @@ namespace {
 
 thread_local std::string g_last_error;
 std::atomic<uint64_t> g_launches{0};
+// CUDA runtime calls that put work on a stream or (de)allocate stream-ordered memory, kernel launches
+// included — the "total API calls per batch" of SURVEY §8d, next to the launch count.
+std::atomic<uint64_t> g_api_calls{0};
+struct EnqTag {};
+inline cudaError_t operator<<(EnqTag, cudaError_t e) {
+  g_api_calls.fetch_add(1, std::memory_order_relaxed);
+  return e;
+}
+#define FK_ENQ EnqTag{} <<      /* prefix of a counted runtime call:  e = FK_ENQ cudaMemcpyAsync(...) */
 
 flowkv_status fail(flowkv_status s, const std::string& msg) {
   g_last_error = msg;
@@ -260,11 +269,18 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
     if (device) {
       cudaError_t e = cudaGetDevice(&pl->device);
       if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaGetDevice"); }
-      int v = 0;
-      e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, pl->device);
-      if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaDeviceGetAttribute"); }
-      pl->num_sms = (uint32_t)v;
-      pl->max_smem_optin = bulk_max_smem();
+      // device attributes never change: query once per device, not once per plan
+      static std::atomic<uint32_t> sms_of[64], smem_of[64];
+      const int di = pl->device & 63;
+      if (!sms_of[di].load(std::memory_order_acquire)) {
+        int v = 0;
+        e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, pl->device);
+        if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaDeviceGetAttribute"); }
+        smem_of[di].store(bulk_max_smem(), std::memory_order_relaxed);
+        sms_of[di].store((uint32_t)v, std::memory_order_release);
+      }
+      pl->num_sms = sms_of[di].load(std::memory_order_relaxed);
+      pl->max_smem_optin = smem_of[di].load(std::memory_order_relaxed);
     } else {
       pl->num_sms = 148;
     }
@@ -325,7 +341,7 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
         if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaStreamCreate(upload)"); }
         e = g_pinned.acquire(bytes, pl->staging);
         if (e != cudaSuccess) { delete pl; return fail_cuda(e, "cudaHostAlloc(plan staging)"); }
-        e = cudaMallocAsync(&pl->d_buf, bytes, up);
+        e = FK_ENQ cudaMallocAsync(&pl->d_buf, bytes, up);
         if (e != cudaSuccess) { g_pinned.release(pl->staging); delete pl; return fail_cuda(e, "cudaMallocAsync(plan)"); }
         pl->d_bytes = bytes;
         uint64_t off = 0;
@@ -336,11 +352,11 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
           op->d_chunks = (const Chunk*)((char*)pl->d_buf + off);
           off += n;
         }
-        e = cudaMemcpyAsync(pl->d_buf, pl->staging.p, bytes, cudaMemcpyHostToDevice, up);
-        if (e == cudaSuccess) e = cudaEventRecord(pl->staging.ev, up);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(pl->stream, pl->staging.ev, 0);
+        e = FK_ENQ cudaMemcpyAsync(pl->d_buf, pl->staging.p, bytes, cudaMemcpyHostToDevice, up);
+        if (e == cudaSuccess) e = FK_ENQ cudaEventRecord(pl->staging.ev, up);
+        if (e == cudaSuccess) e = FK_ENQ cudaStreamWaitEvent(pl->stream, pl->staging.ev, 0);
         if (e != cudaSuccess) {
-          cudaFreeAsync(pl->d_buf, up);
+          FK_ENQ cudaFreeAsync(pl->d_buf, up);
           g_pinned.release(pl->staging);
           delete pl;
           return fail_cuda(e, "cudaMemcpyAsync(plan)");
@@ -397,7 +413,7 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   if (op.sched.chunks.empty() || l0 == l1) return FLOWKV_OK;       // A11: nothing to move, zero launches
   if ((cudaStream_t)stream != pl->stream && pl->staging.ev) {
     // a stream other than the plan's own has not been ordered after the plan upload yet
-    cudaError_t e = cudaStreamWaitEvent((cudaStream_t)stream, pl->staging.ev, 0);
+    cudaError_t e = FK_ENQ cudaStreamWaitEvent((cudaStream_t)stream, pl->staging.ev, 0);
     if (e != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent(plan upload)");
   }
   KernelParams kp{};
@@ -436,6 +452,7 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
                     : launch_copy(mode, kp, op.d_chunks + first, nullptr, 0, ls, stream);
   if (e != 0) return fail_cuda((cudaError_t)e, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
+  g_api_calls.fetch_add(1, std::memory_order_relaxed);
   return FLOWKV_OK;
 }
 
@@ -665,8 +682,8 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   }
   // the inbound side (aux) starts after everything already queued on the caller's stream
   cudaEvent_t e_start = pl->events[n_chunks], e_done = pl->events[n_chunks + 1];
-  if ((e = cudaEventRecord(e_start, s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-  if ((e = cudaStreamWaitEvent(pl->aux, e_start, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+  if ((e = FK_ENQ cudaEventRecord(e_start, s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+  if ((e = FK_ENQ cudaStreamWaitEvent(pl->aux, e_start, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
   const uint32_t vec = ((uintptr_t)host_staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
   const uint32_t vecu = ((uintptr_t)host_staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
   RunOpts ro;
@@ -683,8 +700,8 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     if (!engines) {
       st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);      // D2H on `stream`
       if (st != FLOWKV_OK) return st;
-      if ((e = cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-      if ((e = cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+      if ((e = FK_ENQ cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+      if ((e = FK_ENQ cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
       st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, pl->aux, ro);   // H2D on aux
       if (st != FLOWKV_OK) return st;
       continue;
@@ -696,16 +713,16 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     char* host = (char*)host_staging + window_bytes(pl, 0, l0);
     st = run(pl, pl->pack, pool_side(pl->src), dense_side(out_slot, pl->g, l0, l1), pl->pack.shape.vec_bytes, s, ro);
     if (st != FLOWKV_OK) return st;
-    if ((e = cudaMemcpyAsync(host, out_slot, wb, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(D2H)");
-    if ((e = cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-    if ((e = cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
-    if ((e = cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(H2D)");
+    if ((e = FK_ENQ cudaMemcpyAsync(host, out_slot, wb, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(D2H)");
+    if ((e = FK_ENQ cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+    if ((e = FK_ENQ cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+    if ((e = FK_ENQ cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(H2D)");
     st = run(pl, pl->unpack, dense_side(in_slot, pl->g, l0, l1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, pl->aux, ro);
     if (st != FLOWKV_OK) return st;
     ++k;
   }
-  if ((e = cudaEventRecord(e_done, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-  if ((e = cudaStreamWaitEvent(s, e_done, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+  if ((e = FK_ENQ cudaEventRecord(e_done, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
+  if ((e = FK_ENQ cudaStreamWaitEvent(s, e_done, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
   return FLOWKV_OK;
 }
 
@@ -717,7 +734,7 @@ void flowkv_plan_destroy(flowkv_plan_t* pl) {
     cudaStreamDestroy(pl->aux);
   }
   for (cudaEvent_t ev : pl->events) cudaEventDestroy(ev);
-  if (pl->d_buf) cudaFreeAsync(pl->d_buf, pl->stream);   // ordered after everything queued on the plan's stream
+  if (pl->d_buf) FK_ENQ cudaFreeAsync(pl->d_buf, pl->stream);   // ordered after everything queued on the plan's stream
   g_pinned.release(pl->staging);
   delete pl;
 }
@@ -743,6 +760,8 @@ const char* flowkv_last_error(void) { return g_last_error.c_str(); }
 
 uint64_t flowkv_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
+uint64_t flowkv_api_call_count(void) { return g_api_calls.load(std::memory_order_relaxed); }
+
 // ---- comparison baselines: many cudaMemcpyAsync calls (NOT the product path) --------------------
 namespace {
 // n tokens starting at token slot (block, off) on each side, every plane: the fewest contiguous copies the
@@ -762,7 +781,7 @@ flowkv_status memcpy_tokens(const flowkv_pool& S, const flowkv_pool& D, const Ge
                         (int64_t)so * S.stride_bytes[3] + (int64_t)h * S.stride_bytes[4];
         char* d = (char*)D.base + l * D.stride_bytes[0] + c * D.stride_bytes[1] + (int64_t)db * D.stride_bytes[2] +
                   (int64_t)dof * D.stride_bytes[3] + (int64_t)h * D.stride_bytes[4];
-        cudaError_t e = cudaMemcpyAsync(d, s, (size_t)n * (tm ? g.tok_bytes : g.row_bytes), cudaMemcpyDeviceToDevice, st);
+        cudaError_t e = FK_ENQ cudaMemcpyAsync(d, s, (size_t)n * (tm ? g.tok_bytes : g.row_bytes), cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
         ++calls;
       }
@@ -794,7 +813,7 @@ flowkv_status flowkv_baseline_blockwise(const flowkv_pool* src, const flowkv_poo
       const uint32_t sb = (uint32_t)reqs[r].src_blocks[b], db = (uint32_t)reqs[r].dst_blocks[b];
       if (flat && ntok == bs) {
         // (B,L,2,H): the whole block, every layer and K|V, is one range (Eq. 5)
-        cudaError_t e = cudaMemcpyAsync((char*)dst->base + (int64_t)db * dst->stride_bytes[2],
+        cudaError_t e = FK_ENQ cudaMemcpyAsync((char*)dst->base + (int64_t)db * dst->stride_bytes[2],
                                         (const char*)src->base + (int64_t)sb * src->stride_bytes[2],
                                         (size_t)src->stride_bytes[2], cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
         if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");
@@ -822,7 +841,7 @@ flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* pl, void* stream,
       // whole blocks of the segment: ONE copy over all layers (Fig. 5); then the partial last block
       const uint32_t bs = S.block_size, nfull = sg.n_tokens / bs, rem = sg.n_tokens % bs;
       if (nfull) {
-        cudaError_t e = cudaMemcpyAsync((char*)D.base + (int64_t)sg.dst_block * D.stride_bytes[2],
+        cudaError_t e = FK_ENQ cudaMemcpyAsync((char*)D.base + (int64_t)sg.dst_block * D.stride_bytes[2],
                                         (const char*)S.base + (int64_t)sg.src_block * S.stride_bytes[2],
                                         (size_t)nfull * S.stride_bytes[2], cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
         if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");

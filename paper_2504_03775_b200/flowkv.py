@@ -32,7 +32,7 @@ LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "stri
 
 EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
-           "flowkv_launch_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
+           "flowkv_launch_count", "flowkv_api_call_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
            "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host",
            "flowkv_window_bytes", "flowkv_pack_window", "flowkv_unpack_window", "flowkv_via_host_scratch_bytes",
            "flowkv_alloc_create", "flowkv_alloc_allocate", "flowkv_alloc_free", "flowkv_alloc_stats",
@@ -117,6 +117,8 @@ def _load() -> C.CDLL:
     lib.flowkv_last_error.restype = C.c_char_p
     lib.flowkv_launch_count.argtypes = []
     lib.flowkv_launch_count.restype = C.c_uint64
+    lib.flowkv_api_call_count.argtypes = []
+    lib.flowkv_api_call_count.restype = C.c_uint64
     lib.flowkv_baseline_blockwise.argtypes = [P(flowkv_pool), P(flowkv_pool), P(flowkv_request), C.c_uint32,
                                               C.c_void_p, P(C.c_uint64)]
     lib.flowkv_baseline_segmentwise.argtypes = [C.c_void_p, C.c_void_p, P(C.c_uint64)]
@@ -128,6 +130,7 @@ def _load() -> C.CDLL:
     lib.flowkv_alloc_destroy.restype = None
     for n in EXPORTS:
         if n not in ("flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error", "flowkv_launch_count",
+                     "flowkv_api_call_count",
                      "flowkv_alloc_destroy"):
             getattr(lib, n).restype = C.c_int
     return lib
@@ -151,6 +154,10 @@ def flowkv_last_error() -> str:
 
 def flowkv_launch_count() -> int:
     return int(_lib.flowkv_launch_count())
+
+
+def flowkv_api_call_count() -> int:
+    return int(_lib.flowkv_api_call_count())
 
 
 # ---- marshalling helpers ----------------------------------------------------------------------

@@ -665,3 +665,24 @@ def test_guard_bands_around_both_pools_stay_intact(layouts, tuning):
         assert np.all(b[:GUARD] == P.SENTINEL_BYTE), f"{name}: bytes below the buffer were written"
         assert np.all(b[GUARD + n:] == P.SENTINEL_BYTE), f"{name}: bytes above the buffer were written"
     G.assert_same(P.to_numpy(src_buf), src_np, "src unchanged")
+
+
+def test_launch_and_api_call_accounting():
+    """SURVEY §8d 'launch accounting': a whole step (plan + transfer + destroy) of a small plan is ONE stream
+    call — the launch; an uploaded plan adds allocation, upload, event record + wait and the stream-ordered free."""
+    w = synth.config1_tiny()
+    dp = P.DevicePools(w)
+    xfer_only = F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK
+    for upload, expect in ((0, 1), (1, 6)):
+        c0, n0 = F.flowkv_api_call_count(), F.flowkv_launch_count()
+        plan = dp.plan(xfer_only, {"plan_in_params": upload})
+        plan.transfer()
+        plan.destroy()
+        assert F.flowkv_launch_count() - n0 == 1
+        assert F.flowkv_api_call_count() - c0 == expect
+    torch.cuda.synchronize()
+    # the naive scheme: one call per block per layer per K|V (P:L103)
+    c0 = F.flowkv_api_call_count()
+    calls = F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests)
+    torch.cuda.synchronize()
+    assert F.flowkv_api_call_count() - c0 == calls == 252
