@@ -25,12 +25,16 @@
  *     the caller's; the library never allocates, frees or reallocs them.  A plan owns only
  *     its own small descriptor buffers (host + device).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
- *   - All validation happens in flowkv_plan(); running a plan enqueues EXACTLY ONE kernel on
- *     the caller's stream (zero for an empty plan) and returns without synchronising.
+ *   - All validation happens in flowkv_plan(); flowkv_transfer / pack / unpack and their layer
+ *     forms enqueue EXACTLY ONE kernel on the caller's stream (zero for an empty plan or range)
+ *     and return without synchronising.  flowkv_transfer_via_host is the one composite call
+ *     (2 kernels per layer chunk); it does not synchronise either.
+ *   - A built plan's flowkv_transfer is capturable into a CUDA graph (it is one launch).
  *   - There is no CPU fallback and no other backend: without a CUDA device every call that
  *     needs one returns FLOWKV_ERR_CUDA.
- *   - Thread safety: distinct plans may be used from distinct threads; flowkv_last_error()
- *     is thread-local.
+ *   - Thread safety: distinct plans may be used from distinct threads; one plan is run from one
+ *     thread at a time (flowkv_transfer_via_host keeps its helper streams and events in the
+ *     plan); flowkv_last_error() is thread-local.
  */
 #ifndef FLOWKV_H_
 #define FLOWKV_H_
