@@ -260,3 +260,24 @@ def test_block_major_pairs_use_flat_whole_block_spans(layout):
     strides[F.LAYOUTS["strided"]] += 256            # index 2 == FLOWKV_S_BLOCK
     pad = F.make_pool(FAKE, L, H, D, 2, 64, BS, "strided", strides)
     assert F.flowkv_plan_host(pad, pad, [F.Request(16, S[:1], Dt[:1])]).stats["mode_transfer"] == 2
+
+
+def test_descending_runs_never_merge_and_tile_space_limit():
+    """Reading A8: ids that step by -1 are not one transfer (memory order would be reversed), so a table in
+    descending order gives one segment per block.  And the documented limit: a batch whose tile space
+    (schedule entries x planes) reaches 2^31 is refused with FLOWKV_ERR_UNSUPPORTED instead of overflowing the
+    32-bit tile index of the kernels."""
+    n = 1 << 20
+    desc = np.arange(n - 1, -1, -1, dtype=np.int32)
+    small = F.make_pool(FAKE, 2, 1, 8, 2, n, 1, "lkbthd")
+    plan = F.flowkv_plan_host(small, small, [F.Request(4096, desc[:4096], desc[:4096])],
+                              F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK)
+    assert plan.stats["n_segments"] == 4096 == O.count_segments(desc[:4096], 1, desc[:4096], 1, 4096)
+    plan.destroy()
+    deep = F.make_pool(FAKE, 1024, 1, 8, 2, n, 1, "lkbthd")           # 2048 planes x 2^20 entries = 2^31 tiles
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_plan_host(deep, deep, [F.Request(n, desc, desc)], F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK)
+    assert ei.value.status == F.FLOWKV_ERR_UNSUPPORTED
+    ok = F.flowkv_plan_host(deep, deep, [F.Request(n - 1, desc[:n - 1], desc[:n - 1])],
+                            F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK)
+    assert ok.stats["n_chunks_transfer"] == n - 1
