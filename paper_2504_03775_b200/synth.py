@@ -137,6 +137,40 @@ def place_runs(rng: np.random.Generator, runs: Sequence[int], num_blocks: int,
     return ids
 
 
+def _tables_from_trace(rng, req_blocks: Sequence[int], num_blocks: int, mean: float) -> List[np.ndarray]:
+    """Block tables left behind by a seeded alloc/free trace on a FIFO free list (the plain block manager of a
+    paged-attention server: allocate = pop ids from the head, free = append ids at the tail; no coalescing):
+      1. earlier tenants fill the fresh pool one after another, each taking Geometric(mean) consecutive blocks;
+      2. a seeded subset of them finishes, in seeded order — their blocks join the free list hole by hole
+         (just enough tenants finish to hold this batch plus 10 %, the rest keep their blocks);
+      3. the batch's requests are allocated in order from the head of the free list.
+    A request's table is then a chain of the holes earlier tenants left: runs of mean ~`mean` blocks at
+    scattered addresses (BASELINE.json configs[2]: "50% fragmentation (runs of mean 2) from a seeded alloc/free
+    trace").  Input bookkeeping only — none of FlowKV's own allocator or alignment is involved."""
+    used = int(sum(req_blocks))
+    tenants, pos = [], 0
+    while pos < num_blocks:
+        n = min(int(rng.geometric(1.0 / mean)), num_blocks - pos)
+        tenants.append((pos, n))
+        pos += n
+    order = rng.permutation(len(tenants))
+    free_list, have, want = [], 0, min(num_blocks, int(np.ceil(1.1 * used)))
+    for ti in order:
+        if have >= want:
+            break
+        start, n = tenants[ti]
+        free_list.append(np.arange(start, start + n, dtype=np.int32))
+        have += n
+    if have < used:
+        raise ValueError(f"pool of {num_blocks} blocks cannot hold {used} blocks")
+    flat = np.concatenate(free_list) if free_list else np.zeros(0, dtype=np.int32)
+    out, off = [], 0
+    for nb in req_blocks:
+        out.append(flat[off:off + nb].copy())
+        off += nb
+    return out
+
+
 def _tables_from_runs(rng, req_blocks: Sequence[int], num_blocks: int, kind: Tuple) -> List[np.ndarray]:
     """Per-request block tables with the requested run structure, all sharing one pool."""
     if kind[0] == "contiguous":          # request r's blocks follow request r-1's
@@ -153,6 +187,8 @@ def _tables_from_runs(rng, req_blocks: Sequence[int], num_blocks: int, kind: Tup
             t = rng.permutation(num_blocks)[:nb].astype(np.int32)
             if nb < 2 or not np.any(np.diff(t) == 1):
                 return [t]
+    if kind[0] == "trace":
+        return _tables_from_trace(rng, req_blocks, num_blocks, kind[1])
     all_runs, owner = [], []
     for r, nb in enumerate(req_blocks):
         runs = runs_geometric(rng, nb, kind[1]) if kind[0] == "geometric" else runs_fixed(nb, kind[1])
@@ -177,7 +213,7 @@ def make_workload(name: str, seed: int, shape: Shape, lengths: Sequence[int],
                   value_dist: str = "normal", src_slack: float = 1.25, dst_slack: float = 1.0625,
                   notes: Optional[dict] = None) -> Workload:
     """Generic builder.  ``*_kind``: ("contiguous",) | ("permutation",) | ("geometric", mean) |
-    ("fixed", run).  ``*_blocks`` None => pool sized ``ceil(slack * used)`` (never less than
+    ("fixed", run) | ("trace", mean) (seeded alloc/free trace on a FIFO free list).  ``*_blocks`` None => pool sized ``ceil(slack * used)`` (never less than
     what separated runs need)."""
     rng = np.random.default_rng(np.random.PCG64(seed))
     lengths = [int(t) for t in lengths]
@@ -191,6 +227,8 @@ def make_workload(name: str, seed: int, shape: Shape, lengths: Sequence[int],
         if kind[0] == "contiguous":
             return max(used, 1)
         # enough for `used` blocks in separated runs: worst case one gap per run
+        if kind[0] == "trace":
+            return max(int(np.ceil(slack * used)), 1)
         worst_runs = used if kind[0] != "fixed" else sum(_nblk(n, kind[1]) for n in nb_req)
         return max(int(np.ceil(slack * used)), used + worst_runs, 1)
 
@@ -270,8 +308,8 @@ def _cfg3_dst_blocks(n: int, used: int) -> int:
 
 def config3_batched(budget_bytes: Optional[int] = None, n_requests: Optional[int] = None,
                     num_layers: Optional[int] = None) -> Workload:
-    """BASELINE.json configs[2]: 64 requests, lognormal lengths (median 8k, clip 1k-32k), src runs of
-    mean 2 (break probability 1/2), dst runs of mean 16, one batch.  The literal config needs
+    """BASELINE.json configs[2]: 64 requests, lognormal lengths (median 8k, clip 1k-32k), src tables from a
+    seeded alloc/free trace that leaves runs of mean 2 (break probability 1/2), dst runs of mean 16, one batch.  The literal config needs
     ~201 GiB; ``budget_bytes`` keeps the largest seeded prefix of requests that fits (fit rule)."""
     shape = LLAMA3_8B if num_layers is None else Shape(num_layers, 8, 128, "bf16")
     lengths = config3_lengths()
@@ -282,7 +320,7 @@ def config3_batched(budget_bytes: Optional[int] = None, n_requests: Optional[int
     su = sum(_nblk(t, 16) for t in lengths)
     for attempt in range(8):   # accept iff the generated mean src run is in [1.9, 2.1]
         w = make_workload("cfg3_batched_8b", SEED_BASE + 3000 + attempt, shape, lengths,
-                          "lkbthd", 16, ("geometric", 2.0), _cfg3_src_blocks(n, su),
+                          "lkbthd", 16, ("trace", 2.0), _cfg3_src_blocks(n, su),
                           "lkbthd", 16, ("geometric", 16.0), _cfg3_dst_blocks(n, su))
         runs = sum(n_runs(r.src_blocks) for r in w.requests)
         mean_run = su / max(runs, 1)
