@@ -1,0 +1,160 @@
+"""`-m gpu` seeded differential fuzz: random shapes, layouts (named and padded STRIDED), block-size pairs, block
+tables, batch compositions, operations and tunings — the CUDA path against the CPU oracle, bit for bit over
+whole buffers (sentinel-filled).  Every case is reproducible from its index."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2504_03775_b200 import flowkv as F
+from paper_2504_03775_b200 import pools as P
+from tests import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+LAYOUTS = ["lkbthd", "blkhtd", "blkthd", "padded"]
+
+
+def _geom(rng, layout, L, H, D, NB, BS):
+    """-> (oracle geometry, strides or None).  'padded' = token-major interior with padding after every block,
+    K|V slab and layer (a STRIDED pool: separate allocations / alignment padding)."""
+    if layout != "padded":
+        return getattr(O.PoolGeom, layout)(L, H, D, 2, NB, BS), None
+    row, tok = D * 2, H * D * 2
+    blk = BS * tok + 32 * int(rng.integers(0, 5))
+    kv = NB * blk + 32 * int(rng.integers(0, 9))
+    lay = 2 * kv + 32 * int(rng.integers(0, 3))
+    return O.PoolGeom(L, H, D, 2, NB, BS, lay, kv, blk, tok, row), [lay, kv, blk, tok, row]
+
+
+def _table(rng, n, NB, p_cont):
+    """n distinct block ids; continues +1 with probability p_cont when that id is still free."""
+    free = np.ones(NB, bool)
+    out, cur = [], -2
+    for _ in range(n):
+        if cur + 1 < NB and cur >= 0 and free[cur + 1] and rng.random() < p_cont:
+            cur += 1
+        else:
+            cur = int(rng.choice(np.nonzero(free)[0]))
+        free[cur] = False
+        out.append(cur)
+    return np.asarray(out, np.int32)
+
+
+def _case(idx):
+    rng = np.random.default_rng(9000 + idx)
+    L = int(rng.integers(1, 5))
+    H = int(rng.choice([1, 2, 3, 4, 8]))
+    D = int(rng.choice([8, 16, 24, 64, 128]))
+    bs_s, bs_d = int(2 ** rng.integers(0, 6)), int(2 ** rng.integers(0, 6))
+    lay_s, lay_d = str(rng.choice(LAYOUTS)), str(rng.choice(LAYOUTS))
+    if rng.random() < 0.35:                       # favour the congruent pairs that take the flat path
+        lay_d, bs_d = lay_s, bs_s
+    n_req = int(rng.integers(1, 5))
+    Ts = [int(rng.integers(0, 200)) if rng.random() < 0.9 else 0 for _ in range(n_req)]
+    ns = [-(-t // bs_s) for t in Ts]
+    nd = [-(-t // bs_d) for t in Ts]
+    NBs, NBd = sum(ns) + int(rng.integers(1, 6)), sum(nd) + int(rng.integers(1, 6))
+    stab = _table(rng, sum(ns), NBs, float(rng.choice([0.0, 0.5, 0.9])))
+    dtab = _table(rng, sum(nd), NBd, float(rng.choice([0.0, 0.5, 0.9, 1.0])))
+    if rng.random() < 0.2 and n_req > 1 and ns[0] and ns[1]:      # prefix sharing on the src side (A9)
+        k = min(ns[0], ns[1])
+        stab[ns[0]:ns[0] + k] = stab[:k]
+    reqs, so, do = [], 0, 0
+    for t, a, b in zip(Ts, ns, nd):
+        reqs.append((t, stab[so:so + a].copy(), dtab[do:do + b].copy()))
+        so += a
+        do += b
+    tuning = {}
+    if rng.random() < 0.3:
+        tuning["variant"] = "bulk"
+    if rng.random() < 0.5:
+        tuning["tile_bytes"] = int(2 ** rng.integers(10, 17))
+        if tuning.get("variant") == "bulk":
+            tuning["tile_bytes"] = min(tuning["tile_bytes"], 65536)
+    if rng.random() < 0.4:
+        thr = int(2 ** rng.integers(5, 10))
+        tuning["threads"] = thr
+        tuning["group_threads"] = int(2 ** rng.integers(5, int(np.log2(thr)) + 1))
+    if rng.random() < 0.3:
+        tuning["tile_order"] = int(rng.integers(1, 3))
+    if rng.random() < 0.3:
+        tuning["cache_hint"] = int(rng.integers(1, 4))
+    if rng.random() < 0.3:
+        tuning["max_sms"], tuning["ctas_per_sm"] = int(rng.integers(1, 9)), int(rng.integers(1, 4))
+    if rng.random() < 0.5:
+        tuning["plan_in_params"] = 1
+    op = str(rng.choice(["transfer", "layers", "pack_unpack", "windows"]))
+    return rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op
+
+
+@pytest.mark.parametrize("idx", range(400))
+def test_fuzz_against_oracle(idx):
+    rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op = _case(idx)
+    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
+    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d)
+    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
+    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
+    P.fill_sentinel(dst_buf)
+    src_np = P.to_numpy(src_buf)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs_s, "strided" if ss else lay_s, ss)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs_d, "strided" if sd else lay_d, sd)
+    freqs = [F.Request(t, a, b) for t, a, b in reqs]
+    total = sum(t for t, _, _ in reqs)
+    tokb = H * D * 2
+    what = f"case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} T={[t for t, _, _ in reqs]} {tuning} {op}"
+    plan = F.flowkv_plan(src, dst, freqs, F.FLOWKV_CHECK_DST_ALIAS, tuning or None)
+
+    def expect_transfer(l0=0, l1=L):
+        exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)
+        for t, a, b in reqs:
+            O.transfer(src_np, gs, exp, gd, a, b, t, l0, l1)
+        return exp
+
+    assert plan.stats["n_segments"] == sum(O.count_segments(a, bs_s, b, bs_d, t) for t, a, b in reqs), what
+    n0 = F.flowkv_launch_count()
+    if op == "transfer":
+        plan.transfer()
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if total else 0), what
+        G.assert_same(P.to_numpy(dst_buf), expect_transfer(), what)
+    elif op == "layers":
+        l0 = int(rng.integers(0, L + 1))
+        l1 = int(rng.integers(l0, L + 1))
+        F.flowkv_transfer_layers(plan, l0, l1)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if total and l1 > l0 else 0), what
+        G.assert_same(P.to_numpy(dst_buf), expect_transfer(l0, l1), what)
+    elif op == "pack_unpack":
+        nbytes = plan.stats["staging_bytes"]
+        staging = P.alloc_bytes(nbytes + 32)
+        P.fill_sentinel(staging)
+        plan.pack(staging.data_ptr(), nbytes)
+        plan.unpack(staging.data_ptr(), nbytes)
+        torch.cuda.synchronize()
+        exp = np.full(nbytes + 32, P.SENTINEL_BYTE, np.uint8)
+        off = 0
+        for t, a, _ in reqs:
+            O.pack(src_np, gs, a, t, exp, off)
+            off += t
+        G.assert_same(P.to_numpy(staging), exp, what + " (wire bytes)")
+        G.assert_same(P.to_numpy(dst_buf), expect_transfer(), what + " (unpack)")
+    else:
+        cut = int(rng.integers(0, L + 1))
+        for w0, w1 in ((0, cut), (cut, L)):
+            nb = F.flowkv_window_bytes(plan, w0, w1)
+            assert nb == total * 2 * (w1 - w0) * tokb
+            win = P.alloc_bytes(nb + 32)
+            P.fill_sentinel(win)
+            F.flowkv_pack_window(plan, win.data_ptr(), nb, w0, w1)
+            F.flowkv_unpack_window(plan, win.data_ptr(), nb, w0, w1)
+            torch.cuda.synchronize()
+            exp = np.full(nb + 32, P.SENTINEL_BYTE, np.uint8)
+            off = 0
+            for t, a, _ in reqs:
+                O.pack_window(src_np, gs, a, t, exp, off, w0, w1)
+                off += t
+            G.assert_same(P.to_numpy(win), exp, what + f" (window [{w0},{w1}))")
+        G.assert_same(P.to_numpy(dst_buf), expect_transfer(), what + " (windows unpacked)")
+    G.assert_same(P.to_numpy(src_buf), src_np, what + " (src unchanged)")
+    plan.destroy()
