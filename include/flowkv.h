@@ -137,7 +137,8 @@ typedef struct {
   uint32_t cache_hint;      /* ldst: 0 = auto, 1 = default caching, 2 = L1::no_allocate, 3 = + L2::evict_first */
   uint32_t stages;          /* bulk: ring depth (0 = auto; 2..16)                                   */
   uint32_t plan_in_params;  /* 0 = auto: a plan whose schedules have <= 96 entries each is passed in the kernel
-                             *     parameters (no device allocation, no upload; plan_device_bytes == 0);
+                             *     parameters (no device allocation, no upload; plan_device_bytes == 0; a 512-byte
+                             *     form serves schedules of <= 16 entries, a 3 KiB form the rest);
                              * 1 = always upload                                                    */
   uint32_t _reserved[2];
 } flowkv_tuning;

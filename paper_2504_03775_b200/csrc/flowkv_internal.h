@@ -42,8 +42,10 @@ struct Side {            // one end of a copy as the kernel sees it
 };
 
 // Plans whose every schedule has at most this many entries pass them in the kernel parameters
-// (3 KiB of the 4 KiB parameter space) instead of uploading them.
+// (3 KiB of the 4 KiB parameter space) instead of uploading them.  Parameter bytes cost launch time
+// (measured: ~1 us for 3 KiB), so schedules of <= kInlineChunksSmall entries use a 512-byte form.
 constexpr uint32_t kInlineChunks = 96;
+constexpr uint32_t kInlineChunksSmall = 16;
 
 struct KernelParams {
   Side         src, dst;

@@ -105,8 +105,8 @@ struct GlobalChunks {
   const Chunk* p;
   __device__ __forceinline__ Chunk get(uint32_t i) const { return load_chunk(p + i); }
 };
-struct ParamChunks {
-  Chunk c[kInlineChunks];
+template <uint32_t N> struct ParamChunks {
+  Chunk c[N];
   __device__ __forceinline__ Chunk get(uint32_t i) const { return c[i]; }    // constant-bank load
 };
 
@@ -422,7 +422,12 @@ int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, c
   cudaStream_t st = (cudaStream_t)stream;
   if (host_chunks) {                       // small plan: the schedule rides in the kernel parameters
     if (n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
-    ParamChunks pc;
+    if (n_host_chunks <= kInlineChunksSmall) {
+      ParamChunks<kInlineChunksSmall> pc;
+      memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
+      return launch_with(mode, kp, pc, ls, st);
+    }
+    ParamChunks<kInlineChunks> pc;
     memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
     return launch_with(mode, kp, pc, ls, st);
   }

@@ -444,7 +444,7 @@ def test_baselines_on_block_major_pools_count_calls():
     G.assert_same(P.to_numpy(dp.dst_buf), exp, "segmentwise baseline, block-major")
 
 
-@pytest.mark.parametrize("n_blocks", [95, 96, 97])
+@pytest.mark.parametrize("n_blocks", [15, 16, 17, 95, 96, 97])
 @pytest.mark.parametrize("variant", ["ldst", "bulk"])
 def test_small_plans_travel_in_kernel_params(n_blocks, variant):
     """Step a4 'kernel params when tiny': a plan whose schedules have <= 96 entries is never uploaded
