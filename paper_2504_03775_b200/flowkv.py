@@ -195,22 +195,43 @@ class Request:
     dst_blocks: Optional[np.ndarray] = None
 
 
+def _table(tab) -> np.ndarray:
+    """int32 C-contiguous view/copy of a block table (no copy when it already is one)."""
+    if type(tab) is np.ndarray and tab.dtype == np.int32 and tab.flags.c_contiguous:
+        return tab
+    return np.ascontiguousarray(np.asarray(tab, dtype=np.int32))
+
+
+def _addr(a: np.ndarray) -> int:
+    """Address of an array's first element (the ctypes buffer route is ~3x faster than ``a.ctypes.data``)."""
+    try:
+        return C.addressof(C.c_char.from_buffer(a))
+    except (TypeError, ValueError):          # read-only arrays cannot export a writable buffer
+        return a.ctypes.data
+
+
 def _marshal_requests(requests: Sequence) -> tuple:
+    """-> (flowkv_request array, n, arrays kept alive for the duration of the call)."""
     n = len(requests)
     arr = (flowkv_request * max(n, 1))()
     keep: List[np.ndarray] = []
     for i, r in enumerate(requests):
-        arr[i].num_tokens = int(r.num_tokens)
-        for side in ("src", "dst"):
-            tab = getattr(r, side + "_blocks", None)
-            if tab is None:
-                setattr(arr[i], side + "_blocks", None)
-                setattr(arr[i], f"n_{side}_blocks", 0)
-            else:
-                a = np.ascontiguousarray(np.asarray(tab, dtype=np.int32))
-                keep.append(a)
-                setattr(arr[i], side + "_blocks", a.ctypes.data if a.size else None)
-                setattr(arr[i], f"n_{side}_blocks", a.size)
+        q = arr[i]
+        q.num_tokens = int(r.num_tokens)
+        tab = getattr(r, "src_blocks", None)
+        if tab is not None:
+            a = _table(tab)
+            keep.append(a)
+            q.n_src_blocks = a.size
+            if a.size:
+                q.src_blocks = _addr(a)
+        tab = getattr(r, "dst_blocks", None)
+        if tab is not None:
+            a = _table(tab)
+            keep.append(a)
+            q.n_dst_blocks = a.size
+            if a.size:
+                q.dst_blocks = _addr(a)
     return arr, n, keep
 
 
