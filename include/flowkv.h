@@ -180,7 +180,16 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
  *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
  *   tuning   : HOST pointer or NULL.
  *   out      : HOST pointer; receives the plan (caller destroys it).  Untouched on error.
- * The plan stays valid until destroyed; pools must stay alive while it is run. */
+ * The plan stays valid until destroyed; pools must stay alive while it is run.
+ * Errors (nothing is allocated or enqueued when one is returned):
+ *   INVALID_ARG  out NULL, both pools NULL, reqs NULL with n_reqs > 0, a table pointer NULL, unknown flag /
+ *                layout / tuning value, a zero shape field or a stride <= 0
+ *   ALIGN        a base, a stride or head_dim*elem_bytes is not a multiple of 16 bytes
+ *   SHAPE_MISMATCH  src and dst differ in L, Hkv, Dh or elem_bytes
+ *   TABLE_LEN    n_*_blocks != ceil(num_tokens / block_size);  BLOCK_OOB  an id outside [0, num_blocks)
+ *   DST_ALIAS    (only with FLOWKV_CHECK_DST_ALIAS) a dst block id named twice in the batch
+ *   UNSUPPORTED  block_size not a power of two, a block spanning >= 4 GiB, a row > 1 MiB, >= 2^31 tiles
+ *   NOMEM        host allocation failed;  CUDA  a runtime call failed (no device, allocation, upload) */
 FLOWKV_API flowkv_status flowkv_plan(const flowkv_pool* src, const flowkv_pool* dst,
                           const flowkv_request* reqs, uint32_t n_reqs, uint32_t flags,
                           const flowkv_tuning* tuning, void* stream, flowkv_plan_t** out);
@@ -196,13 +205,19 @@ FLOWKV_API flowkv_status flowkv_plan_host(const flowkv_pool* src, const flowkv_p
 FLOWKV_API flowkv_status flowkv_plan_info(const flowkv_plan_t* plan, flowkv_plan_stats* stats,
                                const flowkv_segment** segments);
 
-/* Pool -> pool (a5).  One kernel launch on `stream`; no host synchronisation. */
+/* Pool -> pool (a5; "transfers the KV Cache K and V from node P_p to node D_d", through both block tables
+ * P:L107).  One kernel launch on `stream`; no host synchronisation.  dst may be device memory of this GPU or a
+ * peer's pool mapped into this process (CUDA IPC / peer access).
+ * Errors: INVALID_ARG plan NULL; UNSUPPORTED the plan has no pool->pool schedule (one pool NULL or
+ * FLOWKV_PLAN_NO_TRANSFER) or was built by flowkv_plan_host; CUDA the launch failed. */
 FLOWKV_API flowkv_status flowkv_transfer(const flowkv_plan_t* plan, void* stream);
 
 /* Pool -> dense staging (a6) / dense staging -> pool (a7).  Wire format (A12):
  * [request][layer][K|V][token][head][dim], requests concatenated; request r starts at byte
  * staging_tok_off(r) * bytes_per_token.  `staging`: DEVICE pointer, or a mapped pinned HOST
- * pointer reachable from the device (UVA); 16-B aligned; `bytes` >= staging_bytes. */
+ * pointer reachable from the device (UVA); 16-B aligned; `bytes` >= staging_bytes.
+ * Errors: INVALID_ARG plan or staging NULL; ALIGN staging not 16-B aligned; STAGING_TOO_SMALL; UNSUPPORTED the plan
+ * lacks that schedule (pool NULL / FLOWKV_PLAN_NO_PACK / _NO_UNPACK / host plan); CUDA the launch failed. */
 FLOWKV_API flowkv_status flowkv_pack(const flowkv_plan_t* plan, void* staging, uint64_t bytes, void* stream);
 FLOWKV_API flowkv_status flowkv_unpack(const flowkv_plan_t* plan, const void* staging, uint64_t bytes, void* stream);
 
