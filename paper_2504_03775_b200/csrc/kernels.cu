@@ -1,21 +1,27 @@
-// kernels.cu — the persistent sm_100a copy kernels of the FlowKV transfer path (step a5-a7).
+// kernels.cu — the sm_100a copy kernels of the FlowKV transfer path (steps a5-a7).
 //
-// One launch moves a whole transfer batch ("from 23,469 [calls] to just 1").  The grid
-// is persistent (a multiple of the SM count); thread groups walk a linear tile space
+// One launch moves a whole transfer batch ("from 23,469 [calls] to just 1").  Thread groups walk
+// a linear tile space with a grid-stride loop
 //     tile -> (plane, chunk)      plane = 2*layer + kv, chunk = entry of the plan's schedule
-// with a static stride, so there is no per-block / per-layer launch and no atomics.  The path is a
-// pure byte move: no FP, no tensor cores; the bound is HBM bandwidth.
+// and the grid is capped at 256 CTAs per SM: up to the cap every tile has its own CTA and the hardware CTA
+// scheduler hands tiles to whichever SM frees up first (measured 3-6 % faster than an exactly-resident grid
+// with a static stride); beyond the cap each CTA strides.  No per-block / per-layer launch, no
+// atomics, no inter-CTA dependence.  The path is a pure byte move: no FP, no tensor cores; the bound is HBM
+// bandwidth.
 //
 // Variants
 //   ldst : registers.  256-bit (LDG.E.256 / STG.E.256, sm_100+) or 128-bit vector accesses,
 //          UNROLL independent loads in flight per thread before the first store, streaming cache
 //          hints (L1::no_allocate, L2::evict_first) because nothing is ever re-read.
-//            span mode : a chunk is one byte range contiguous on both sides.
+//            span mode : a chunk is one byte range contiguous on both sides (per plane).
 //            rows mode : a chunk is n tokens x Hkv rows of Dh*e bytes; each side has its own
 //                        token / head stride (layout + block-size conversion, BASELINE configs[3]).
+//            flat mode : both pools block-major with the same interior (Eq. 5's (B,L,2,H)): whole-block
+//                        runs are plane-free byte ranges; partial last blocks ride along as rows tiles.
 //   bulk : TMA bulk copies (cp.async.bulk -> UBLKCP) gmem -> smem -> gmem through an mbarrier
 //          ring driven by ONE thread per CTA; span mode only.  Uses no registers or LSU slots
 //          for payload, which is what a copy that co-runs with GEMMs wants.
+// Every kernel exists for a schedule in global memory and for one passed by value in the kernel parameters.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>

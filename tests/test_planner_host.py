@@ -281,3 +281,41 @@ def test_descending_runs_never_merge_and_tile_space_limit():
     ok = F.flowkv_plan_host(deep, deep, [F.Request(n - 1, desc[:n - 1], desc[:n - 1])],
                             F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK)
     assert ok.stats["n_chunks_transfer"] == n - 1
+
+
+def test_planning_from_several_threads_at_once():
+    """Header: 'distinct plans may be used from distinct threads; flowkv_last_error() is thread-local'.  ctypes
+    releases the GIL during the call, so these planners really run concurrently."""
+    import threading
+    w = synth.config3_batched(n_requests=6, num_layers=2)
+    sp = F.make_pool(FAKE, 2, 8, 128, 2, w.src.num_blocks, 16, "lkbthd")
+    dp = F.make_pool(FAKE, 2, 8, 128, 2, w.dst.num_blocks, 16, "lkbthd")
+    reqs = [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks) for r in w.requests]
+    ref = _segs(F.flowkv_plan_host(sp, dp, reqs))
+    bad = F.Request(16, np.asarray([w.src.num_blocks], np.int32), np.asarray([0], np.int32))   # BLOCK_OOB
+    errors = []
+
+    def worker(k):
+        try:
+            for i in range(40):
+                if (i + k) % 4 == 0:
+                    try:
+                        F.flowkv_plan_host(sp, dp, [bad])
+                        errors.append("bad request accepted")
+                    except F.FlowKVError as e:
+                        if e.status != F.FLOWKV_ERR_BLOCK_OOB or "src block id" not in str(e):
+                            errors.append(f"wrong error text in thread {k}: {e}")
+                else:
+                    p = F.flowkv_plan_host(sp, dp, reqs)
+                    if _segs(p) != ref:
+                        errors.append(f"thread {k}: segments differ")
+                    p.destroy()
+        except Exception as e:  # pragma: no cover
+            errors.append(repr(e))
+
+    threads = [threading.Thread(target=worker, args=(k,)) for k in range(6)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors[:3]
