@@ -686,3 +686,22 @@ def test_launch_and_api_call_accounting():
     calls = F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests)
     torch.cuda.synchronize()
     assert F.flowkv_api_call_count() - c0 == calls == 252
+
+
+def test_product_path_from_plain_c_without_torch(tmp_path):
+    """tests/c_abi/transfer_gpu.c: cudaMalloc'd pools, flowkv_plan + flowkv_transfer from C on its own stream, the
+    whole dst pool against the oracle's C function — no Python, no torch in that process.  One launch."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe = tmp_path / "transfer_gpu"
+    libdir, odir = os.path.dirname(F.LIB_PATH), os.path.join(root, "oracle")
+    O.build()
+    cuda = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(root, "include"), "-I", f"{cuda}/include",
+                           os.path.join(root, "tests", "c_abi", "transfer_gpu.c"), "-o", str(exe),
+                           "-L", libdir, "-lflowkv", "-L", odir, "-lflowkv_oracle", "-L", f"{cuda}/lib64", "-lcudart",
+                           f"-Wl,-rpath,{libdir}", f"-Wl,-rpath,{odir}", f"-Wl,-rpath,{cuda}/lib64"])
+    out = subprocess.run([str(exe)], capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0, out.stderr + out.stdout
+    assert out.stdout.strip() == "ok 1"

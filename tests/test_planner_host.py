@@ -319,3 +319,18 @@ def test_planning_from_several_threads_at_once():
     for t in threads:
         t.join()
     assert not errors, errors[:3]
+
+
+def test_header_is_plain_c_and_the_library_links_from_c(tmp_path):
+    """include/flowkv.h compiles as C99 (-pedantic) and a C program reaches the planner through the ABI: the
+    hand-worked example of SURVEY §8c gives (0,48,5,0) (48,32,20,3) (80,16,9,5) (96,24,3,6)."""
+    import subprocess
+    exe = tmp_path / "plan_host"
+    src = os.path.join(ROOT, "tests", "c_abi", "plan_host.c")
+    libdir = os.path.dirname(F.LIB_PATH)
+    subprocess.check_call(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), src,
+                           "-o", str(exe), "-L", libdir, "-lflowkv", f"-Wl,-rpath,{libdir}"])
+    out = subprocess.run([str(exe)], capture_output=True, text=True, timeout=60)
+    assert out.returncode == 0, out.stderr
+    got = [tuple(int(x) for x in line.split()) for line in out.stdout.strip().splitlines()]
+    assert got == [(0, 48, 5, 0), (48, 32, 20, 3), (80, 16, 9, 5), (96, 24, 3, 6)]
