@@ -114,6 +114,26 @@ void align_segments(const flowkv_pool* src, const flowkv_pool* dst, const flowkv
     const uint32_t T = reqs[r].num_tokens;
     const int32_t* S = reqs[r].src_blocks;
     const int32_t* D = reqs[r].dst_blocks;
+    if (src && dst && bs_s == bs_d && T) {
+      // Equal block sizes (the common case): pieces are whole blocks, so walk the two id lists directly —
+      // a segment continues while both ids step by +1 (same rule, ~10x fewer instructions per block).
+      const uint32_t nb = (uint32_t)(((uint64_t)T + bs_s - 1) / bs_s);
+      uint32_t start = 0;
+      for (uint32_t b = 1; b <= nb; ++b) {
+        if (b < nb && S[b] == S[b - 1] + 1 && D[b] == D[b - 1] + 1) continue;
+        flowkv_segment sg{};
+        sg.request = r;
+        sg.first_token = start * bs_s;
+        sg.n_tokens = (b < nb ? b * bs_s : T) - sg.first_token;
+        sg.src_block = (uint32_t)S[start];
+        sg.dst_block = (uint32_t)D[start];
+        sg.staging_tok_off = tok_base;
+        out.push_back(sg);
+        start = b;
+      }
+      tok_base += T;
+      continue;
+    }
     bool open = false;
     int64_t next_s = 0, next_d = 0;          // slot that would continue the open segment
     uint32_t t = 0;
