@@ -131,11 +131,33 @@ def load_peaks() -> tuple:
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+NCU_CAPTURES = {      # workload name -> committed summary of its `ncu --set full` capture (profiles/r01_ncu.md)
+    "cfg2_llama8b_13k": "r01_ncu_full_cfg2_fk_span_ldst.csv",
+    "cfg2_blkthd_13k": "r01_ncu_full_cfg2bm_fk_flat_ldst.csv",
+    "cfg3_batched_8b": "r01_ncu_full_cfg3_fk_span_ldst.csv",
+    "cfg4_hetero_70b": "r01_ncu_full_cfg4_fk_rows_ldst.csv",
+}
+
+
 def load_traffic(workload_key: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes; mean over the captured launches) from the
+    committed summary of the ncu --set full capture of this workload's kernel, or None."""
+    import csv
+    name = NCU_CAPTURES.get(workload_key)
+    if not name:
+        return None
     try:
-        return json.load(open(p)).get(workload_key)
+        rows = list(csv.reader(open(os.path.join(ROOT, "profiles", name))))
+        head, units = rows[0], rows[1]
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+        tot = []
+        for r in rows[2:]:
+            v = 0.0
+            for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                i = head.index(col)
+                v += float(r[i]) * scale[units[i]]
+            tot.append(v)
+        return sum(tot) / len(tot) if tot else None
     except Exception:
         return None
 
