@@ -172,7 +172,7 @@ typedef struct {
 FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
 
 /* Build a plan: validate (a1), bidirectional segment alignment (a2), tile schedule (a3),
- * upload (a4; one cudaMallocAsync + one cudaMemcpyAsync from cached pinned memory on a library-owned
+ * upload (a4; one stream-ordered allocation from a library-owned memory pool + one cudaMemcpyAsync from cached pinned memory on a library-owned
  * upload stream; `stream` only waits on the upload's event.  No host synchronisation, so planning and
  * uploading batch k+1 overlap the move of batch k.  Small plans are not uploaded at all: their schedule
  * travels in the kernel parameters, see flowkv_tuning.plan_in_params).

@@ -94,16 +94,37 @@ PinnedCache g_pinned;
 // Plan uploads go through a library-owned non-blocking stream, so the upload for batch k+1 does not
 // queue behind the kernel that is moving batch k on the caller's stream; the caller's stream only
 // waits on the upload's event.  One stream per device, created on first use, never destroyed.
+// Plan buffers come from a library-owned memory pool per device whose release threshold is "never": the default
+// pool hands freed memory back to the OS at the next synchronisation, after which every cudaMallocAsync is a
+// fresh driver allocation (slow, and ordered against running work).  A few hundred KiB per plan in flight stay
+// cached for the life of the process.
 std::mutex g_upload_mu;
 cudaStream_t g_upload_stream[64] = {};
-cudaError_t upload_stream(int device, cudaStream_t* out) {
+cudaMemPool_t g_plan_pool[64] = {};
+cudaError_t upload_stream(int device, cudaStream_t* out, cudaMemPool_t* pool) {
   if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
   std::lock_guard<std::mutex> lk(g_upload_mu);
   if (!g_upload_stream[device]) {
-    cudaError_t e = cudaStreamCreateWithFlags(&g_upload_stream[device], cudaStreamNonBlocking);
+    cudaStream_t st = nullptr;
+    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
     if (e != cudaSuccess) return e;
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = device;
+    cudaMemPool_t mp = nullptr;
+    e = cudaMemPoolCreate(&mp, &props);
+    if (e == cudaSuccess) {
+      uint64_t never = ~0ull;
+      e = cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &never);
+    }
+    if (e != cudaSuccess) { cudaStreamDestroy(st); return e; }
+    g_plan_pool[device] = mp;
+    g_upload_stream[device] = st;
   }
   *out = g_upload_stream[device];
+  *pool = g_plan_pool[device];
   return cudaSuccess;
 }
 
@@ -379,11 +400,12 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
         for (Op* op : {&pl->transfer, &pl->pack, &pl->unpack}) op->in_params = true;
       } else if (bytes) {
         cudaStream_t up = nullptr;
-        cudaError_t e = upload_stream(pl->device, &up);
+        cudaMemPool_t mp = nullptr;
+        cudaError_t e = upload_stream(pl->device, &up, &mp);
         if (e != cudaSuccess) { drop_plan(pl); return fail_cuda(e, "cudaStreamCreate(upload)"); }
         e = g_pinned.acquire(bytes, pl->staging);
         if (e != cudaSuccess) { drop_plan(pl); return fail_cuda(e, "cudaHostAlloc(plan staging)"); }
-        e = FK_ENQ cudaMallocAsync(&pl->d_buf, bytes, up);
+        e = FK_ENQ cudaMallocFromPoolAsync(&pl->d_buf, bytes, mp, up);
         if (e != cudaSuccess) { g_pinned.release(pl->staging); drop_plan(pl); return fail_cuda(e, "cudaMallocAsync(plan)"); }
         pl->d_bytes = bytes;
         uint64_t off = 0;
