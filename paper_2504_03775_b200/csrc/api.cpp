@@ -221,7 +221,7 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
   const uint32_t use_sms = t.max_sms ? std::min(t.max_sms, sms) : sms;
   ls.vec_bytes = pick_vec(a, b, pl->g);
   ls.variant = t.variant ? t.variant : FLOWKV_VARIANT_LDST;
-  if (op.sched.mode != MODE_SPAN) ls.variant = FLOWKV_VARIANT_LDST;   // bulk handles contiguous chunks only
+  if (op.sched.mode != MODE_SPAN && op.sched.mode != MODE_FLAT) ls.variant = FLOWKV_VARIANT_LDST;   // bulk moves byte ranges only
   op.max_chunk_bytes = 0;
   for (size_t i = 0; i < op.sched.chunks.size(); ++i) {
     const Chunk& c = op.sched.chunks[i];
@@ -233,7 +233,7 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
   if (ls.variant == FLOWKV_VARIANT_BULK) {
     ls.threads = 32;
     ls.group_threads = 32;
-    ls.stage_bytes = std::max<uint32_t>(op.max_chunk_bytes, 1024);
+    ls.stage_bytes = std::max<uint32_t>(op.sched.mode == MODE_FLAT ? op.sched.flat_tile : op.max_chunk_bytes, 1024);
     ls.stage_bytes = (ls.stage_bytes + 127) & ~127u;
     // like the ldst path the grid is oversubscribed (<= 256 CTAs per SM) and each CTA's ring is short:
     // several small CTAs per SM, scheduled by hardware, beat one long-lived CTA with a deep ring

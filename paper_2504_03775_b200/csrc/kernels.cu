@@ -19,7 +19,7 @@
 //            flat mode : both pools block-major with the same interior (Eq. 5's (B,L,2,H)): whole-block
 //                        runs are plane-free byte ranges; partial last blocks ride along as rows tiles.
 //   bulk : TMA bulk copies (cp.async.bulk -> UBLKCP) gmem -> smem -> gmem through an mbarrier
-//          ring driven by ONE thread per CTA; span mode only.  Uses no registers or LSU slots
+//          ring driven by ONE thread per CTA; span and flat modes (byte ranges).  Uses no registers or LSU slots
 //          for payload, which is what a copy that co-runs with GEMMs wants.
 // Every kernel exists for a schedule in global memory and for one passed by value in the kernel parameters.
 #include <cuda_runtime.h>
@@ -383,6 +383,67 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
   bulk_wait_all();
 }
 
+// bulk / flat: the same TMA ring over the plane-free tiles of two congruent block-major pools (the paper's
+// (B,L,2,H) layout next to the paper's SM-contention concern): thread 0 drives the ring; the few tiles
+// of partial last blocks are then moved by the whole warp with 128-bit loads/stores.
+template <class CS>
+__global__ void __launch_bounds__(32, 1) fk_flat_bulk(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                      uint32_t stage_bytes, uint32_t n_stages) {
+  extern __shared__ __align__(128) char ring[];
+  __shared__ __align__(8) uint64_t full[kBulkMaxStages];
+  __shared__ char* dptr[kBulkMaxStages];
+  __shared__ uint32_t nbytes[kBulkMaxStages];
+  const uint32_t n_flat_tiles = p.n_flat << p.flat_shift;
+  if (threadIdx.x == 0) {
+    for (uint32_t i = 0; i < n_stages; ++i) mbar_init(&full[i], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    const uint64_t pol = policy_evict_first();
+    uint32_t cursor = blockIdx.x;                     // next tile of this CTA to look at
+    uint32_t loaded = 0, stored = 0;                  // non-empty tiles whose load / store has been issued
+    auto issue_next = [&]() -> bool {                 // skips the empty slots at the end of a range
+      for (; cursor < n_flat_tiles; cursor += gridDim.x) {
+        const Chunk c = cs.get(cursor >> p.flat_shift);
+        const uint32_t off = (cursor & ((1u << p.flat_shift) - 1)) * p.flat_tile;
+        if (off >= c.n) continue;
+        const uint32_t n = min(p.flat_tile, c.n - off), slot = loaded % n_stages;
+        dptr[slot] = p.dst.base + c.dst_off + off;
+        nbytes[slot] = n;
+        mbar_expect_tx(&full[slot], n);
+        bulk_g2s(ring + (size_t)slot * stage_bytes, p.src.base + c.src_off + off, n, &full[slot], pol);
+        ++loaded;
+        cursor += gridDim.x;
+        return true;
+      }
+      return false;
+    };
+    for (uint32_t k = 0; k + 1 < n_stages; ++k)
+      if (!issue_next()) break;
+    while (stored < loaded) {
+      const uint32_t slot = stored % n_stages;
+      mbar_wait(&full[slot], (stored / n_stages) & 1);
+      bulk_s2g(dptr[slot], ring + (size_t)slot * stage_bytes, nbytes[slot], pol);
+      bulk_commit();
+      ++stored;
+      // the next load reuses the slot of store `stored-2`: all but the latest store have finished reading smem
+      bulk_wait_read<1>();
+      issue_next();
+    }
+    bulk_wait_all();
+  }
+  __syncwarp();
+  const uint32_t n_ragged = p.n_tiles - n_flat_tiles;   // partial last blocks: rows tiles, 128-bit vectors
+  const uint32_t vpr = p.row_bytes / 16;
+  for (uint32_t tile = blockIdx.x; tile < n_ragged; tile += gridDim.x) {
+    uint32_t plane, ci;
+    decode_tile(p, tile, plane, ci);
+    const Chunk c = cs.get(p.n_flat + ci);
+    const char* s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    copy_rows<16, 8, 0>(p, s, d, c.n, threadIdx.x, 32, vpr, false, 0);
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
@@ -417,6 +478,13 @@ static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const La
     cudaError_t e = cudaFuncSetAttribute(fk_span_bulk<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
     fk_span_bulk<CS><<<dim3(ls.grid), dim3(32), smem, st>>>(kp, cs, ls.stage_bytes, ls.n_stages);
+    return (int)cudaGetLastError();
+  }
+  if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_FLAT) {
+    const uint32_t smem = ls.n_stages * ls.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(fk_flat_bulk<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    fk_flat_bulk<CS><<<dim3(ls.grid), dim3(32), smem, st>>>(kp, cs, ls.stage_bytes, ls.n_stages);
     return (int)cudaGetLastError();
   }
   if (ls.vec_bytes == 32) return (int)launch_ldst<32, 4, CS>(mode, kp, cs, ls, (int)ls.hint, st);

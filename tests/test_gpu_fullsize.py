@@ -112,6 +112,17 @@ def test_cfg2_block_major_full_size(tokens):
     plan.transfer()
     torch.cuda.synchronize()
     assert F.flowkv_launch_count() - n0 == 1 and plan.stats["mode_transfer"] == 3
+    _check_block_major(w, dp, tokens)
+    # the TMA variant under an SM budget (co-run shape), same bytes
+    P.fill_sentinel(dp.dst_buf)
+    bulk = dp.plan(0, {"variant": "bulk", "max_sms": 32, "ctas_per_sm": 1, "stages": 6, "tile_bytes": 32768})
+    assert bulk.stats["variant"] == F.FLOWKV_VARIANT_BULK and bulk.stats["grid"] == 32
+    bulk.transfer()
+    torch.cuda.synchronize()
+    _check_block_major(w, dp, tokens)
+
+
+def _check_block_major(w, dp, tokens):
     r = w.requests[0]
     blk = 16 * w.shape.bytes_per_token
     sv, dv = dp.src_buf.view(w.src.num_blocks, blk), dp.dst_buf.view(w.dst.num_blocks, blk)

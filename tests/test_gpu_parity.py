@@ -365,7 +365,9 @@ def test_transfer_via_pinned_host_pipeline(n_chunks, ctas):
 @pytest.mark.parametrize("layout", ["blkhtd", "blkthd"])
 @pytest.mark.parametrize("tuning", [None, {"tile_bytes": 4096, "threads": 128, "group_threads": 32},
                                     {"tile_bytes": 16384, "ctas_per_sm": 1, "max_sms": 2, "cache_hint": 1},
-                                    {"tile_order": 2, "group_threads": 64, "threads": 256}])
+                                    {"tile_order": 2, "group_threads": 64, "threads": 256},
+                                    {"variant": "bulk"}, {"variant": "bulk", "tile_bytes": 4096, "stages": 3, "max_sms": 2,
+                                                          "ctas_per_sm": 1, "plan_in_params": 1}])
 def test_flat_mode_block_major_both_sides(layout, tuning):
     """S§8f NEXT-2 / Eq. 5 / Fig. 5: both pools (B,L,2,H) with the same interior.  Whole-block runs move as
     plane-free byte ranges, partial last blocks token-granular (A4) — all in ONE launch, bit-exact incl.
@@ -377,6 +379,7 @@ def test_flat_mode_block_major_both_sides(layout, tuning):
     st = plan.stats
     assert st["mode_transfer"] == 3 and st["n_flat_chunks"] > 0
     assert st["n_chunks_transfer"] - st["n_flat_chunks"] >= sum(1 for t in lengths if t % 16)
+    assert st["variant"] == (F.FLOWKV_VARIANT_BULK if tuning and tuning.get("variant") == "bulk" else F.FLOWKV_VARIANT_LDST)
 
 
 @pytest.mark.parametrize("upload", [0, 1])
