@@ -293,8 +293,28 @@ def run_ours(args) -> None:
         torch.cuda.synchronize()
 
     XFER_ONLY = F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK      # the step moves pool -> pool only
+    dev_tables = None
+    if args.device_tables:           # block tables resident in HBM, read by the kernel: no plan at all
+        n_rq = len(w.requests)
+        max_t = max((r.num_tokens for r in w.requests), default=0)
+        ws_, wd_ = max(1, -(-max_t // w.src.block_size)), max(1, -(-max_t // w.dst.block_size))
+        hs_, hd_ = np.full((n_rq, ws_), -1, np.int32), np.full((n_rq, wd_), -1, np.int32)
+        for i, r in enumerate(w.requests):
+            hs_[i, :len(r.src_blocks)], hd_[i, :len(r.dst_blocks)] = r.src_blocks, r.dst_blocks
+        dev_tables = (torch.from_numpy(hs_).to(dp.device), torch.from_numpy(hd_).to(dp.device),
+                      torch.tensor([r.num_tokens for r in w.requests], dtype=torch.int32, device=dp.device),
+                      torch.zeros(1, dtype=torch.int32, device=dp.device), n_rq, ws_, wd_, max_t)
 
     def step(ev_a=None, ev_b=None):
+        if dev_tables is not None:
+            st_, dt_, ln_, fl_, n_rq, ws_, wd_, max_t = dev_tables
+            if ev_a is not None:
+                ev_a.record(stream)
+            F.flowkv_transfer_tables(dp.src, dp.dst, st_.data_ptr(), dt_.data_ptr(), ln_.data_ptr(), n_rq, ws_, wd_, max_t,
+                                     fl_.data_ptr(), tuning, s)             # ONE launch, nothing else
+            if ev_b is not None:
+                ev_b.record(stream)
+            return
         plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, XFER_ONLY, tuning, s)   # a1-a4 (upload is stream-ordered)
         if ev_a is not None:
             ev_a.record(stream)
@@ -342,7 +362,9 @@ def run_ours(args) -> None:
                        "payload_bytes": payload, "segments": stats["n_segments"],
                        "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
                        if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
-                       "step": "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM",
+                       "step": ("flowkv_transfer_tables per step (device-resident block tables, no plan); pools resident in HBM"
+                                if args.device_tables else
+                                "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM"),
                        "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
                                                         "vec_bytes", "cache_hint", "tile_order", "stages")}},
             "clocks": clk,
@@ -351,8 +373,9 @@ def run_ours(args) -> None:
             "latency_ms_per_request": t_ms / K / max(len(w.requests), 1),
             "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": load_traffic(w.name), "peak_source": peak_src,
-                         "kernel": {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]],
+                         "traffic": None if args.device_tables else load_traffic(w.name), "peak_source": peak_src,
+                         "kernel": "fk_tables_ldst" if args.device_tables else
+                         {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]],
                          "kernel_ms_avg": kern_ms, "kernel_ms_min": kern_min_ms,
                          "algorithmic_bytes_per_launch": 2 * payload,
                          "kernel_share_of_step": kern_ms / (t_ms / K)},
@@ -454,6 +477,8 @@ def main() -> None:
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg2bm", "cfg2bm_ragged", "cfg3", "cfg4"])
     ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
+    ap.add_argument("--device-tables", action="store_true",
+                    help="time flowkv_transfer_tables (block tables resident on the device, no plan) instead of plan+transfer")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-serial", action="store_true", help="pack then unpack on one stream instead of the pipeline")

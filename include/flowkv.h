@@ -267,6 +267,27 @@ FLOWKV_API flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* plan, voi
                                                   uint32_t n_chunks, uint32_t ctas_per_kernel,
                                                   void* device_scratch, uint64_t scratch_bytes, void* stream);
 
+/* Table-driven transfer: no plan.  The block tables and lengths are DEVICE-resident (as in servers that keep
+ * their block tables in HBM) and are read by the kernel itself; the host never sees them, so nothing is planned,
+ * allocated or uploaded, and the call can be captured in a CUDA graph and replayed while the tables' CONTENTS change.
+ * Same result as flowkv_plan + flowkv_transfer on the same tables (the definition at the top of this file); segments
+ * play no role because one kernel moves everything (a tile = min(BS_s, BS_d) tokens of one plane).  One launch.
+ *   src_tables  DEVICE int32 [n_reqs][max_src_blocks], row r = request r's src block ids (padding ignored)
+ *   dst_tables  DEVICE int32 [n_reqs][max_dst_blocks]
+ *   num_tokens  DEVICE uint32 [n_reqs]; request r moves tokens [0, num_tokens[r]); must be <= max_tokens
+ *   max_tokens  upper bound of num_tokens[] known to the host (sizes the grid; tiles past a request's end exit)
+ *   error_flag  DEVICE uint32 or NULL: OR-ed with 1 if a block id in use is outside its pool (that tile is
+ *               skipped, nothing out of bounds is touched); the host cannot validate what it never sees.
+ *               A dst block named twice is NOT detected (undefined result, as without FLOWKV_CHECK_DST_ALIAS).
+ *   tuning      threads, group_threads, max_sms, ctas_per_sm are honoured; may be NULL.
+ * Errors: INVALID_ARG, ALIGN, SHAPE_MISMATCH, UNSUPPORTED as for flowkv_plan; TABLE_LEN if max_*_blocks cannot
+ * hold max_tokens; CUDA.  n_reqs == 0 or max_tokens == 0: FLOWKV_OK, zero launches. */
+FLOWKV_API flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* dst,
+                                                const int32_t* src_tables, const int32_t* dst_tables,
+                                                const uint32_t* num_tokens, uint32_t n_reqs,
+                                                uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
+                                                uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
+
 /* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
  * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,
  * synchronise that stream first.  NULL is ignored. */

@@ -790,6 +790,70 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   return FLOWKV_OK;
 }
 
+flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables,
+                                     const int32_t* dst_tables, const uint32_t* num_tokens, uint32_t n_reqs,
+                                     uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
+                                     uint32_t* error_flag, const flowkv_tuning* tuning, void* stream) {
+  if (!src || !dst) return fail(FLOWKV_ERR_INVALID_ARG, "a pool is NULL");
+  std::string err;
+  flowkv_status st;
+  if ((st = validate_pool(src, "src", err)) != FLOWKV_OK) return fail(st, err);
+  if ((st = validate_pool(dst, "dst", err)) != FLOWKV_OK) return fail(st, err);
+  if (src->num_layers != dst->num_layers || src->num_kv_heads != dst->num_kv_heads || src->head_dim != dst->head_dim ||
+      src->elem_bytes != dst->elem_bytes)
+    return fail(FLOWKV_ERR_SHAPE_MISMATCH, "src and dst pools differ in num_layers, num_kv_heads, head_dim or elem_bytes");
+  flowkv_tuning tn{};
+  if (tuning) tn = *tuning;
+  if ((st = check_tuning(tn)) != FLOWKV_OK) return st;
+  if (n_reqs == 0 || max_tokens == 0) return FLOWKV_OK;               // A11: nothing to move, zero launches
+  if (!src_tables || !dst_tables || !num_tokens) return fail(FLOWKV_ERR_INVALID_ARG, "a table pointer is NULL");
+  if ((uint64_t)max_src_blocks * src->block_size < max_tokens || (uint64_t)max_dst_blocks * dst->block_size < max_tokens)
+    return fail(FLOWKV_ERR_TABLE_LEN, "max_*_blocks * block_size < max_tokens");
+  Geometry g{};
+  g.L = src->num_layers; g.Hkv = src->num_kv_heads; g.Dh = src->head_dim; g.e = src->elem_bytes;
+  g.row_bytes = g.Dh * g.e; g.tok_bytes = g.Hkv * g.row_bytes; g.bytes_per_token = 2ull * g.L * g.tok_bytes;
+  TablesParams tp{};
+  tp.kp.src = pool_side(*src);
+  tp.kp.dst = pool_side(*dst);
+  tp.kp.n_planes = 2 * g.L;
+  tp.kp.row_bytes = g.row_bytes;
+  tp.kp.heads = g.Hkv;
+  tp.kp.tok_bytes = g.tok_bytes;
+  tp.src_tables = src_tables; tp.dst_tables = dst_tables; tp.num_tokens = num_tokens; tp.error = error_flag;
+  tp.src_s_block = src->stride_bytes[FLOWKV_S_BLOCK]; tp.dst_s_block = dst->stride_bytes[FLOWKV_S_BLOCK];
+  tp.n_reqs = n_reqs; tp.max_src_blocks = max_src_blocks; tp.max_dst_blocks = max_dst_blocks;
+  tp.src_bs_log2 = log2u(src->block_size); tp.dst_bs_log2 = log2u(dst->block_size);
+  tp.granule_log2 = std::min(tp.src_bs_log2, tp.dst_bs_log2);
+  tp.q_per_req = (uint32_t)(((uint64_t)max_tokens + (1u << tp.granule_log2) - 1) >> tp.granule_log2);
+  tp.src_num_blocks = src->num_blocks; tp.dst_num_blocks = dst->num_blocks;
+  const uint64_t n_tiles = (uint64_t)tp.kp.n_planes * n_reqs * tp.q_per_req;
+  if (n_tiles >= (1ull << 31)) return fail(FLOWKV_ERR_UNSUPPORTED, "more than 2^31 tiles in one batch; split the batch");
+  tp.n_tiles = (uint32_t)n_tiles;
+  int dev = 0, sms = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
+  LaunchShape ls{};
+  ls.vec_bytes = pick_vec(src, dst, g);
+  const uint32_t tile_bytes = (1u << tp.granule_log2) * g.tok_bytes;
+  ls.threads = tn.threads ? tn.threads : 512;
+  uint32_t grp = tn.group_threads ? std::min(tn.group_threads, ls.threads) : 128;
+  while (grp > 32 && grp * ls.vec_bytes > tile_bytes) grp >>= 1;       // no more threads than vectors in a tile
+  ls.group_threads = grp;
+  const uint32_t use_sms = tn.max_sms ? std::min<uint32_t>(tn.max_sms, (uint32_t)sms) : (uint32_t)sms;
+  const uint32_t per_cta = ls.threads / ls.group_threads;
+  ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * (tn.ctas_per_sm ? tn.ctas_per_sm : 256),
+                                         (n_tiles + per_cta - 1) / per_cta);
+  tp.kp.group_log2 = log2u(ls.group_threads);
+  tp.kp.vpr_log2 = log2_or_none(g.row_bytes / ls.vec_bytes);
+  tp.kp.heads_log2 = log2_or_none(g.Hkv);
+  const int rc = launch_tables(tp, ls, stream);
+  if (rc != 0) return fail_cuda((cudaError_t)rc, "kernel launch");
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  g_api_calls.fetch_add(1, std::memory_order_relaxed);
+  return FLOWKV_OK;
+}
+
 void flowkv_plan_destroy(flowkv_plan_t* pl) {
   if (!pl) return;
   if (pl->aux) {

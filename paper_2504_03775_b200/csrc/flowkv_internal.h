@@ -78,6 +78,23 @@ struct LaunchShape {
 // the kernel parameters.
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
                 uint32_t n_host_chunks, const LaunchShape& ls, void* stream);
+// Table-driven transfer (flowkv_transfer_tables): no host plan; the kernel walks device-resident block tables.
+struct TablesParams {
+  KernelParams    kp;          // src/dst sides, row_bytes, heads, tok_bytes, group_log2, vpr_log2, heads_log2, n_planes
+  const int32_t*  src_tables;  // device [n_reqs][max_src_blocks]
+  const int32_t*  dst_tables;  // device [n_reqs][max_dst_blocks]
+  const uint32_t* num_tokens;  // device [n_reqs]
+  uint32_t*       error;       // device flag or NULL: set to 1 when a block id is out of range (that tile is skipped)
+  int64_t         src_s_block, dst_s_block;
+  uint32_t        n_reqs, max_src_blocks, max_dst_blocks;
+  uint32_t        granule_log2;           // tokens per tile = min(BS_s, BS_d)
+  uint32_t        src_bs_log2, dst_bs_log2;
+  uint32_t        q_per_req;              // tiles per (request, plane) = ceil(max_tokens / granule)
+  uint32_t        src_num_blocks, dst_num_blocks;
+  uint32_t        n_tiles;                // n_planes * n_reqs * q_per_req
+};
+int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream);
+
 // Largest dynamic shared memory the bulk variant may use on the current device (0 on failure).
 uint32_t bulk_max_smem();
 

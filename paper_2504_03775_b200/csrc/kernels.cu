@@ -21,7 +21,8 @@
 //   bulk : TMA bulk copies (cp.async.bulk -> UBLKCP) gmem -> smem -> gmem through an mbarrier
 //          ring driven by ONE thread per CTA; span and flat modes (byte ranges).  Uses no registers or LSU slots
 //          for payload, which is what a copy that co-runs with GEMMs wants.
-// Every kernel exists for a schedule in global memory and for one passed by value in the kernel parameters.
+//   tables : no schedule at all — the kernel reads device-resident block tables (flowkv_transfer_tables).
+// Every scheduled kernel exists for a schedule in global memory and for one passed by value in the kernel parameters.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>
@@ -507,6 +508,54 @@ int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, c
   }
   GlobalChunks gc{device_chunks};
   return launch_with(mode, kp, gc, ls, st);
+}
+
+// ------------------------------------------------------------------------------------------------
+// ldst / tables: no host plan at all.  tile -> (plane, request, granule); the group reads its two block ids
+// from device-resident tables and moves one granule (min(BS_s, BS_d) tokens) of one plane in rows form.
+// Segments are irrelevant to this kernel (a granule of a plane is >= one block-plane of contiguous bytes on
+// the token-major side), so nothing has to be coalesced, uploaded or even known on the host — the tables may
+// change between replays of a captured graph.
+// ------------------------------------------------------------------------------------------------
+template <int VEC, int UNROLL, int HINT>
+__global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__ TablesParams tp) {
+  const KernelParams& p = tp.kp;
+  const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint32_t G = 1u << p.group_log2;
+  const uint32_t lane = gtid & (G - 1);
+  const uint32_t n_groups = (gridDim.x * blockDim.x) >> p.group_log2;
+  const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
+  const uint32_t vpr = p.row_bytes / VEC;
+  const bool pow2 = (p.vpr_log2 != 0xffffffffu) && (p.heads_log2 != 0xffffffffu);
+  const uint32_t g = 1u << tp.granule_log2;
+  const uint32_t per_plane = tp.n_reqs * tp.q_per_req;
+  for (uint32_t tile = gtid >> p.group_log2; tile < tp.n_tiles; tile += n_groups) {
+    const uint32_t plane = tile / per_plane, rq = tile - plane * per_plane;
+    const uint32_t r = rq / tp.q_per_req, q = rq - r * tp.q_per_req;
+    const uint32_t T = __ldg(tp.num_tokens + r), t0 = q << tp.granule_log2;
+    if (t0 >= T) continue;
+    const uint32_t n = min(g, T - t0);
+    const int32_t sb = __ldg(tp.src_tables + (size_t)r * tp.max_src_blocks + (t0 >> tp.src_bs_log2));
+    const int32_t db = __ldg(tp.dst_tables + (size_t)r * tp.max_dst_blocks + (t0 >> tp.dst_bs_log2));
+    if ((uint32_t)sb >= tp.src_num_blocks || (uint32_t)db >= tp.dst_num_blocks) {
+      if (tp.error && lane == 0) atomicOr(tp.error, 1u);
+      continue;
+    }
+    const uint32_t so = t0 & ((1u << tp.src_bs_log2) - 1), dof = t0 & ((1u << tp.dst_bs_log2) - 1);
+    const char* s = p.src.base + (int64_t)(plane >> 1) * p.src.s_layer + (int64_t)(plane & 1) * p.src.s_kv +
+                    (int64_t)sb * tp.src_s_block + (int64_t)so * p.src.s_token;
+    char* d = p.dst.base + (int64_t)(plane >> 1) * p.dst.s_layer + (int64_t)(plane & 1) * p.dst.s_kv +
+              (int64_t)db * tp.dst_s_block + (int64_t)dof * p.dst.s_token;
+    copy_rows<VEC, UNROLL, HINT>(p, s, d, n, lane, G, vpr, pow2, pol);
+  }
+}
+
+int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  const dim3 grid(ls.grid), block(ls.threads);
+  if (ls.vec_bytes == 32) fk_tables_ldst<32, 4, 2><<<grid, block, 0, st>>>(tp);
+  else                    fk_tables_ldst<16, 8, 2><<<grid, block, 0, st>>>(tp);
+  return (int)cudaGetLastError();
 }
 
 }  // namespace flowkv

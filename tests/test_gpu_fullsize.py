@@ -140,6 +140,27 @@ def _check_block_major(w, dp, tokens):
         G.assert_same(dv[int(r.dst_blocks[i])].cpu().numpy(), exp, f"block {i} ({ntok} tokens)")
 
 
+def test_cfg2_full_size_table_driven():
+    """configs[1] through flowkv_transfer_tables: block tables and length resident on the device, no plan, one launch;
+    same checks as the planned transfer (sampled layers against the oracle, every plane through the gather property)."""
+    w = synth.config2_llama8b_13k()
+    _need(w.src.bytes(w.shape) + w.dst.bytes(w.shape))
+    dp = P.DevicePools(w)
+    r = w.requests[0]
+    st = torch.from_numpy(np.concatenate([r.src_blocks, np.full(5, -1, np.int32)])[None, :].copy()).cuda()
+    dt = torch.from_numpy(np.concatenate([r.dst_blocks, np.full(1, -1, np.int32)])[None, :].copy()).cuda()
+    lens = torch.tensor([r.num_tokens], dtype=torch.int32).cuda()
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    n0 = F.flowkv_launch_count()
+    F.flowkv_transfer_tables(dp.src, dp.dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), 1, st.shape[1], dt.shape[1],
+                             r.num_tokens + 3, flag.data_ptr())
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1 and int(flag.item()) == 0
+    for layer in (0, 31):
+        _lkbthd_layer_check(w, dp, layer)
+    _lkbthd_all_planes_property(w, dp)
+
+
 def test_cfg3_full_size_fit_rule():
     """configs[2] scaled to fit HBM by the seeded-prefix rule, one batch, one launch."""
     free_b, _ = torch.cuda.mem_get_info()

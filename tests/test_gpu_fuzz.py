@@ -158,3 +158,48 @@ def test_fuzz_against_oracle(idx):
         G.assert_same(P.to_numpy(dst_buf), expect_transfer(), what + " (windows unpacked)")
     G.assert_same(P.to_numpy(src_buf), src_np, what + " (src unchanged)")
     plan.destroy()
+
+
+def _device_tables(reqs, width_s, width_d):
+    """Padded 2-D tables (pad value -7: must never be read as a block id in use) and lengths, on the device."""
+    n = len(reqs)
+    st = np.full((n, width_s), -7, np.int32)
+    dt = np.full((n, width_d), -7, np.int32)
+    for i, (_, a, b) in enumerate(reqs):
+        st[i, :len(a)] = a
+        dt[i, :len(b)] = b
+    lens = np.asarray([t for t, _, _ in reqs], np.uint32)
+    to = lambda x: torch.from_numpy(x.view(np.int32) if x.dtype == np.uint32 else x).cuda()
+    return to(st), to(dt), to(lens)
+
+
+@pytest.mark.parametrize("idx", range(120))
+def test_fuzz_table_driven_transfer(idx):
+    """flowkv_transfer_tables: the kernel walks device-resident padded block tables itself (no plan) — same seeded
+    cases as above, whole dst pool against the oracle, one launch, error flag stays clear."""
+    rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
+    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
+    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d)
+    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
+    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
+    P.fill_sentinel(dst_buf)
+    src_np = P.to_numpy(src_buf)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs_s, "strided" if ss else lay_s, ss)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs_d, "strided" if sd else lay_d, sd)
+    max_t = max(t for t, _, _ in reqs) + int(rng.integers(0, 40))
+    ws, wd = -(-max_t // bs_s) + int(rng.integers(0, 3)), -(-max_t // bs_d) + int(rng.integers(0, 3))
+    st, dt, lens = _device_tables(reqs, max(ws, 1), max(wd, 1))
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    tn = {k: v for k, v in tuning.items() if k in ("threads", "group_threads", "max_sms", "ctas_per_sm")}
+    n0 = F.flowkv_launch_count()
+    F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), len(reqs), st.shape[1], dt.shape[1],
+                             max_t, flag.data_ptr(), tn or None)
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == (1 if max_t else 0)
+    exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)
+    for t, a, b in reqs:
+        O.transfer(src_np, gs, exp, gd, a, b, t)
+    what = f"tables case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} T={[t for t, _, _ in reqs]} {tn}"
+    G.assert_same(P.to_numpy(dst_buf), exp, what)
+    assert int(flag.item()) == 0, what
+    G.assert_same(P.to_numpy(src_buf), src_np, what + " (src unchanged)")

@@ -708,3 +708,72 @@ def test_product_path_from_plain_c_without_torch(tmp_path):
     out = subprocess.run([str(exe)], capture_output=True, text=True, timeout=120)
     assert out.returncode == 0, out.stderr + out.stdout
     assert out.stdout.strip() == "ok 1"
+
+
+def test_table_driven_transfer_graph_replay_and_error_flag():
+    """flowkv_transfer_tables captured ONCE in a CUDA graph; between replays only the CONTENTS of the device tables
+    and lengths change (new requests, new block ids) and every replay lands where the oracle says.  A block id
+    outside the pool raises the device error flag, skips that tile and touches nothing else."""
+    shape = synth.Shape(3, 2, 64, "fp16")
+    NBs, NBd, n_req, max_t = 64, 40, 3, 150
+    ssp, dsp = synth.PoolSpec("lkbthd", 16, NBs), synth.PoolSpec("blkhtd", 32, NBd)
+    src_buf, dst_buf = P.alloc_bytes(ssp.bytes(shape)), P.alloc_bytes(dsp.bytes(shape))
+    P.fill_values(src_buf, "bits", "fp16", 41)
+    src_np = P.to_numpy(src_buf)
+    src, dst = P.describe(ssp, shape, src_buf.data_ptr()), P.describe(dsp, shape, dst_buf.data_ptr())
+    gs, gd = G.geom(ssp, shape), G.geom(dsp, shape)
+    ws, wd = -(-max_t // 16), -(-max_t // 32)
+    st = torch.full((n_req, ws), -1, dtype=torch.int32, device="cuda")
+    dt = torch.full((n_req, wd), -1, dtype=torch.int32, device="cuda")
+    lens = torch.zeros(n_req, dtype=torch.int32, device="cuda")
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    stream = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=stream):
+        F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), n_req, ws, wd, max_t,
+                                 flag.data_ptr(), None, torch.cuda.current_stream().cuda_stream)
+    rng = np.random.default_rng(42)
+    for it in range(4):
+        Ts = [int(rng.integers(0, max_t + 1)) for _ in range(n_req)]
+        sperm, dperm = rng.permutation(NBs).astype(np.int32), rng.permutation(NBd).astype(np.int32)
+        reqs, so, do = [], 0, 0
+        hs, hd = np.full((n_req, ws), -1, np.int32), np.full((n_req, wd), -1, np.int32)
+        for i, t in enumerate(Ts):
+            a, b = sperm[so:so + -(-t // 16)], dperm[do:do + -(-t // 32)]
+            so, do = so + len(a), do + len(b)
+            hs[i, :len(a)], hd[i, :len(b)] = a, b
+            reqs.append((t, a, b))
+        st.copy_(torch.from_numpy(hs)); dt.copy_(torch.from_numpy(hd)); lens.copy_(torch.tensor(Ts, dtype=torch.int32))
+        P.fill_sentinel(dst_buf)
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        exp = np.full(dsp.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+        for t, a, b in reqs:
+            O.transfer(src_np, gs, exp, gd, a, b, t)
+        G.assert_same(P.to_numpy(dst_buf), exp, f"graph replay {it} with new tables {Ts}")
+        assert int(flag.item()) == 0
+    # an id outside the pool: flagged, its tiles skipped, the rest of the batch still lands
+    bad = hs.copy()
+    victim = next(i for i, t in enumerate(Ts) if t > 0)
+    bad[victim, 0] = NBs + 5
+    st.copy_(torch.from_numpy(bad))
+    P.fill_sentinel(dst_buf)
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    assert int(flag.item()) == 1
+    exp = np.full(dsp.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+    for i, (t, a, b) in enumerate(reqs):
+        if i != victim:
+            O.transfer(src_np, gs, exp, gd, a, b, t)
+    got = P.to_numpy(dst_buf)
+    # every byte outside the victim's dst blocks is exactly the oracle's; inside them only tokens >= 16 may be written
+    blk = 32 * shape.bytes_per_token
+    mask = np.ones(got.size, bool)
+    for b in reqs[victim][2]:
+        mask[int(b) * blk:(int(b) + 1) * blk] = False
+    assert np.array_equal(got[mask], exp[mask])
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), n_req, ws - 1, wd, max_t)
+    assert ei.value.status == F.FLOWKV_ERR_TABLE_LEN
