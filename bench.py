@@ -134,6 +134,7 @@ def load_peaks() -> tuple:
 NCU_CAPTURES = {      # workload name -> committed summary of its `ncu --set full` capture (profiles/r01_ncu.md)
     "cfg2_llama8b_13k": "r01_ncu_full_cfg2_fk_span_ldst.csv",
     "cfg2_blkthd_13k": "r01_ncu_full_cfg2bm_fk_flat_ldst.csv",
+    "cfg2_llama8b_13k+tables": "r01_ncu_full_cfg2_fk_tables_ldst.csv",
     "cfg3_batched_8b": "r01_ncu_full_cfg3_fk_span_ldst.csv",
     "cfg4_hetero_70b": "r01_ncu_full_cfg4_fk_rows_ldst.csv",
 }
@@ -373,7 +374,7 @@ def run_ours(args) -> None:
             "latency_ms_per_request": t_ms / K / max(len(w.requests), 1),
             "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None if args.device_tables else load_traffic(w.name), "peak_source": peak_src,
+                         "traffic": load_traffic(w.name + ("+tables" if args.device_tables else "")), "peak_source": peak_src,
                          "kernel": "fk_tables_ldst" if args.device_tables else
                          {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]],
                          "kernel_ms_avg": kern_ms, "kernel_ms_min": kern_min_ms,
