@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define FLOWKV_VERSION 1
+#define FLOWKV_VERSION 2
 
 #if defined(__GNUC__)
 #define FLOWKV_API __attribute__((visibility("default")))
