@@ -12,7 +12,12 @@ from tests import gpu_common as G
 
 pytestmark = pytest.mark.gpu
 
+import os
+
 LAYOUTS = ["lkbthd", "blkhtd", "blkthd", "padded"]
+# FLOWKV_FUZZ_OFFSET shifts the case indices (a soak run: FLOWKV_FUZZ_OFFSET=400 FLOWKV_FUZZ_CASES=4000 pytest ...)
+FUZZ_OFFSET = int(os.environ.get("FLOWKV_FUZZ_OFFSET", "0"))
+FUZZ_CASES = int(os.environ.get("FLOWKV_FUZZ_CASES", "400"))
 
 
 def _geom(rng, layout, L, H, D, NB, BS):
@@ -88,7 +93,7 @@ def _case(idx):
     return rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op
 
 
-@pytest.mark.parametrize("idx", range(400))
+@pytest.mark.parametrize("idx", range(FUZZ_OFFSET, FUZZ_OFFSET + FUZZ_CASES))
 def test_fuzz_against_oracle(idx):
     rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op = _case(idx)
     gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
@@ -173,7 +178,7 @@ def _device_tables(reqs, width_s, width_d):
     return to(st), to(dt), to(lens)
 
 
-@pytest.mark.parametrize("idx", range(120))
+@pytest.mark.parametrize("idx", range(FUZZ_OFFSET, FUZZ_OFFSET + max(1, FUZZ_CASES * 3 // 10)))
 def test_fuzz_table_driven_transfer(idx):
     """flowkv_transfer_tables: the kernel walks device-resident padded block tables itself (no plan) — same seeded
     cases as above, whole dst pool against the oracle, one launch, error flag stays clear."""
