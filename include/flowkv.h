@@ -288,6 +288,25 @@ FLOWKV_API flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const fl
                                                 uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
                                                 uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
 
+/* Table-driven pack / unpack of the layer window [layer_begin, layer_end) (the window [0, num_layers) is the wire
+ * format of flowkv_pack): the same kernel with one side dense.  Tables as for flowkv_transfer_tables; lengths come as
+ *   cu_tokens   DEVICE uint64 [n_reqs + 1], exclusive prefix sums of the request lengths (cu_tokens[0] == 0): request r
+ *               has cu_tokens[r+1] - cu_tokens[r] tokens (<= max_tokens) and starts at wire token offset cu_tokens[r]
+ *               — the "cumulative sequence lengths" array servers already keep on the device.
+ *   window      DEVICE or mapped pinned HOST pointer, 16-B aligned; `bytes` = its capacity.  The host cannot see the
+ *               total length, so the bound is enforced on the device: a request that would reach past `bytes` is
+ *               skipped whole and error_flag is OR-ed with 2 (1 = a block id out of range, as above).
+ * One launch (zero if n_reqs, max_tokens or the layer range is empty).  Errors as flowkv_transfer_tables, plus
+ * INVALID_ARG for a layer range outside [0, num_layers] or a NULL window / cu_tokens, ALIGN for the window. */
+FLOWKV_API flowkv_status flowkv_pack_tables(const flowkv_pool* src, const int32_t* src_tables, const uint64_t* cu_tokens,
+                                            uint32_t n_reqs, uint32_t max_src_blocks, uint32_t max_tokens,
+                                            void* window, uint64_t bytes, uint32_t layer_begin, uint32_t layer_end,
+                                            uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
+FLOWKV_API flowkv_status flowkv_unpack_tables(const flowkv_pool* dst, const int32_t* dst_tables, const uint64_t* cu_tokens,
+                                              uint32_t n_reqs, uint32_t max_dst_blocks, uint32_t max_tokens,
+                                              const void* window, uint64_t bytes, uint32_t layer_begin, uint32_t layer_end,
+                                              uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
+
 /* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
  * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,
  * synchronise that stream first.  NULL is ignored. */

@@ -790,42 +790,57 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   return FLOWKV_OK;
 }
 
-flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables,
-                                     const int32_t* dst_tables, const uint32_t* num_tokens, uint32_t n_reqs,
-                                     uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
-                                     uint32_t* error_flag, const flowkv_tuning* tuning, void* stream) {
-  if (!src || !dst) return fail(FLOWKV_ERR_INVALID_ARG, "a pool is NULL");
+namespace {
+// Common body of the table-driven calls.  Exactly one of src / dst may be NULL: that side is then the dense
+// buffer `dense` holding the layer window [l0, l1) (wire format A12 / A20) and `cu_tokens` gives each request's base.
+flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables, const int32_t* dst_tables,
+                            const uint32_t* num_tokens, const uint64_t* cu_tokens, uint32_t n_reqs, uint32_t max_src_blocks,
+                            uint32_t max_dst_blocks, uint32_t max_tokens, const void* dense, uint64_t dense_bytes,
+                            uint32_t l0, uint32_t l1, uint32_t* error_flag, const flowkv_tuning* tuning, void* stream) {
+  const flowkv_pool* any = src ? src : dst;
+  if (!any) return fail(FLOWKV_ERR_INVALID_ARG, "a pool is NULL");
   std::string err;
   flowkv_status st;
-  if ((st = validate_pool(src, "src", err)) != FLOWKV_OK) return fail(st, err);
-  if ((st = validate_pool(dst, "dst", err)) != FLOWKV_OK) return fail(st, err);
-  if (src->num_layers != dst->num_layers || src->num_kv_heads != dst->num_kv_heads || src->head_dim != dst->head_dim ||
-      src->elem_bytes != dst->elem_bytes)
+  if (src && (st = validate_pool(src, "src", err)) != FLOWKV_OK) return fail(st, err);
+  if (dst && (st = validate_pool(dst, "dst", err)) != FLOWKV_OK) return fail(st, err);
+  if (src && dst &&
+      (src->num_layers != dst->num_layers || src->num_kv_heads != dst->num_kv_heads || src->head_dim != dst->head_dim ||
+       src->elem_bytes != dst->elem_bytes))
     return fail(FLOWKV_ERR_SHAPE_MISMATCH, "src and dst pools differ in num_layers, num_kv_heads, head_dim or elem_bytes");
+  if (l0 > l1 || l1 > any->num_layers) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
   flowkv_tuning tn{};
   if (tuning) tn = *tuning;
   if ((st = check_tuning(tn)) != FLOWKV_OK) return st;
-  if (n_reqs == 0 || max_tokens == 0) return FLOWKV_OK;               // A11: nothing to move, zero launches
-  if (!src_tables || !dst_tables || !num_tokens) return fail(FLOWKV_ERR_INVALID_ARG, "a table pointer is NULL");
-  if ((uint64_t)max_src_blocks * src->block_size < max_tokens || (uint64_t)max_dst_blocks * dst->block_size < max_tokens)
+  if (n_reqs == 0 || max_tokens == 0 || l0 == l1) return FLOWKV_OK;    // A11: nothing to move, zero launches
+  if ((src && !src_tables) || (dst && !dst_tables) || (!num_tokens && !cu_tokens))
+    return fail(FLOWKV_ERR_INVALID_ARG, "a table pointer is NULL");
+  if ((src && (uint64_t)max_src_blocks * src->block_size < max_tokens) ||
+      (dst && (uint64_t)max_dst_blocks * dst->block_size < max_tokens))
     return fail(FLOWKV_ERR_TABLE_LEN, "max_*_blocks * block_size < max_tokens");
+  if (!(src && dst)) {
+    if (!dense) return fail(FLOWKV_ERR_INVALID_ARG, "staging is NULL");
+    if ((uintptr_t)dense % 16) return fail(FLOWKV_ERR_ALIGN, "staging is not 16-byte aligned");
+    if (!cu_tokens) return fail(FLOWKV_ERR_INVALID_ARG, "cu_tokens is NULL");
+  }
   Geometry g{};
-  g.L = src->num_layers; g.Hkv = src->num_kv_heads; g.Dh = src->head_dim; g.e = src->elem_bytes;
+  g.L = any->num_layers; g.Hkv = any->num_kv_heads; g.Dh = any->head_dim; g.e = any->elem_bytes;
   g.row_bytes = g.Dh * g.e; g.tok_bytes = g.Hkv * g.row_bytes; g.bytes_per_token = 2ull * g.L * g.tok_bytes;
   TablesParams tp{};
-  tp.kp.src = pool_side(*src);
-  tp.kp.dst = pool_side(*dst);
-  tp.kp.n_planes = 2 * g.L;
+  tp.kp.src = src ? pool_side(*src) : dense_side(dense, g, l0, l1);
+  tp.kp.dst = dst ? pool_side(*dst) : dense_side(dense, g, l0, l1);
+  tp.kp.n_planes = 2 * (l1 - l0);
+  tp.kp.plane0 = 2 * l0;
   tp.kp.row_bytes = g.row_bytes;
   tp.kp.heads = g.Hkv;
   tp.kp.tok_bytes = g.tok_bytes;
-  tp.src_tables = src_tables; tp.dst_tables = dst_tables; tp.num_tokens = num_tokens; tp.error = error_flag;
-  tp.src_s_block = src->stride_bytes[FLOWKV_S_BLOCK]; tp.dst_s_block = dst->stride_bytes[FLOWKV_S_BLOCK];
+  tp.src_tables = src_tables; tp.dst_tables = dst_tables; tp.num_tokens = num_tokens; tp.cu_tokens = cu_tokens;
+  tp.dense_bytes = dense_bytes;
+  tp.error = error_flag;
   tp.n_reqs = n_reqs; tp.max_src_blocks = max_src_blocks; tp.max_dst_blocks = max_dst_blocks;
-  tp.src_bs_log2 = log2u(src->block_size); tp.dst_bs_log2 = log2u(dst->block_size);
-  tp.granule_log2 = std::min(tp.src_bs_log2, tp.dst_bs_log2);
+  if (src) { tp.src_s_block = src->stride_bytes[FLOWKV_S_BLOCK]; tp.src_bs_log2 = log2u(src->block_size); tp.src_num_blocks = src->num_blocks; }
+  if (dst) { tp.dst_s_block = dst->stride_bytes[FLOWKV_S_BLOCK]; tp.dst_bs_log2 = log2u(dst->block_size); tp.dst_num_blocks = dst->num_blocks; }
+  tp.granule_log2 = src && dst ? std::min(tp.src_bs_log2, tp.dst_bs_log2) : (src ? tp.src_bs_log2 : tp.dst_bs_log2);
   tp.q_per_req = (uint32_t)(((uint64_t)max_tokens + (1u << tp.granule_log2) - 1) >> tp.granule_log2);
-  tp.src_num_blocks = src->num_blocks; tp.dst_num_blocks = dst->num_blocks;
   const uint64_t n_tiles = (uint64_t)tp.kp.n_planes * n_reqs * tp.q_per_req;
   if (n_tiles >= (1ull << 31)) return fail(FLOWKV_ERR_UNSUPPORTED, "more than 2^31 tiles in one batch; split the batch");
   tp.n_tiles = (uint32_t)n_tiles;
@@ -835,6 +850,7 @@ flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* 
   if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
   LaunchShape ls{};
   ls.vec_bytes = pick_vec(src, dst, g);
+  if (!(src && dst) && (uintptr_t)dense % 32) ls.vec_bytes = 16;
   const uint32_t tile_bytes = (1u << tp.granule_log2) * g.tok_bytes;
   ls.threads = tn.threads ? tn.threads : 512;
   uint32_t grp = tn.group_threads ? std::min(tn.group_threads, ls.threads) : 128;
@@ -852,6 +868,34 @@ flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* 
   g_launches.fetch_add(1, std::memory_order_relaxed);
   g_api_calls.fetch_add(1, std::memory_order_relaxed);
   return FLOWKV_OK;
+}
+}  // namespace
+
+flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables,
+                                     const int32_t* dst_tables, const uint32_t* num_tokens, uint32_t n_reqs,
+                                     uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
+                                     uint32_t* error_flag, const flowkv_tuning* tuning, void* stream) {
+  if (!src || !dst) return fail(FLOWKV_ERR_INVALID_ARG, "a pool is NULL");
+  return tables_common(src, dst, src_tables, dst_tables, num_tokens, nullptr, n_reqs, max_src_blocks, max_dst_blocks,
+                       max_tokens, nullptr, 0, 0, src->num_layers, error_flag, tuning, stream);
+}
+
+flowkv_status flowkv_pack_tables(const flowkv_pool* src, const int32_t* src_tables, const uint64_t* cu_tokens, uint32_t n_reqs,
+                                 uint32_t max_src_blocks, uint32_t max_tokens, void* window, uint64_t bytes,
+                                 uint32_t layer_begin, uint32_t layer_end, uint32_t* error_flag,
+                                 const flowkv_tuning* tuning, void* stream) {
+  if (!src) return fail(FLOWKV_ERR_INVALID_ARG, "pool is NULL");
+  return tables_common(src, nullptr, src_tables, nullptr, nullptr, cu_tokens, n_reqs, max_src_blocks, 0, max_tokens, window,
+                       bytes, layer_begin, layer_end, error_flag, tuning, stream);
+}
+
+flowkv_status flowkv_unpack_tables(const flowkv_pool* dst, const int32_t* dst_tables, const uint64_t* cu_tokens, uint32_t n_reqs,
+                                   uint32_t max_dst_blocks, uint32_t max_tokens, const void* window, uint64_t bytes,
+                                   uint32_t layer_begin, uint32_t layer_end, uint32_t* error_flag,
+                                   const flowkv_tuning* tuning, void* stream) {
+  if (!dst) return fail(FLOWKV_ERR_INVALID_ARG, "pool is NULL");
+  return tables_common(nullptr, dst, nullptr, dst_tables, nullptr, cu_tokens, n_reqs, 0, max_dst_blocks, max_tokens, window,
+                       bytes, layer_begin, layer_end, error_flag, tuning, stream);
 }
 
 void flowkv_plan_destroy(flowkv_plan_t* pl) {

@@ -83,7 +83,9 @@ struct TablesParams {
   KernelParams    kp;          // src/dst sides, row_bytes, heads, tok_bytes, group_log2, vpr_log2, heads_log2, n_planes
   const int32_t*  src_tables;  // device [n_reqs][max_src_blocks]
   const int32_t*  dst_tables;  // device [n_reqs][max_dst_blocks]
-  const uint32_t* num_tokens;  // device [n_reqs]
+  const uint32_t* num_tokens;  // device [n_reqs]               (pool -> pool)
+  const uint64_t* cu_tokens;   // device [n_reqs + 1], exclusive prefix sums of the lengths (pack / unpack; else NULL)
+  uint64_t        dense_bytes; // capacity of the dense side (pack / unpack)
   uint32_t*       error;       // device flag or NULL: set to 1 when a block id is out of range (that tile is skipped)
   int64_t         src_s_block, dst_s_block;
   uint32_t        n_reqs, max_src_blocks, max_dst_blocks;

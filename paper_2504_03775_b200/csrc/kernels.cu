@@ -517,6 +517,18 @@ int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, c
 // the token-major side), so nothing has to be coalesced, uploaded or even known on the host — the tables may
 // change between replays of a captured graph.
 // ------------------------------------------------------------------------------------------------
+// Address of token t0 of request r in plane `plane` on one side; `ok` is cleared when a block id is out of range.
+__device__ __forceinline__ int64_t tables_side(const Side& sd, const int32_t* tab, uint32_t max_blocks, uint32_t bs_log2,
+                                               int64_t s_block, uint32_t num_blocks, uint32_t r, uint32_t t0, uint32_t plane,
+                                               uint32_t T, uint64_t tok0, uint32_t tok_bytes, bool& ok) {
+  if (sd.dense)       // layer window in wire order (A12/A20): request base + plane slab + token
+    return (int64_t)tok0 * sd.s_layer + ((int64_t)(plane - sd.plane0) * T + t0) * (int64_t)tok_bytes;
+  const int32_t b = __ldg(tab + (size_t)r * max_blocks + (t0 >> bs_log2));
+  if ((uint32_t)b >= num_blocks) ok = false;
+  return (int64_t)(plane >> 1) * sd.s_layer + (int64_t)(plane & 1) * sd.s_kv + (int64_t)b * s_block +
+         (int64_t)(t0 & ((1u << bs_log2) - 1)) * sd.s_token;
+}
+
 template <int VEC, int UNROLL, int HINT>
 __global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__ TablesParams tp) {
   const KernelParams& p = tp.kp;
@@ -530,23 +542,28 @@ __global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__
   const uint32_t g = 1u << tp.granule_log2;
   const uint32_t per_plane = tp.n_reqs * tp.q_per_req;
   for (uint32_t tile = gtid >> p.group_log2; tile < tp.n_tiles; tile += n_groups) {
-    const uint32_t plane = tile / per_plane, rq = tile - plane * per_plane;
+    const uint32_t pl = tile / per_plane, rq = tile - pl * per_plane;
+    const uint32_t plane = pl + p.plane0;
     const uint32_t r = rq / tp.q_per_req, q = rq - r * tp.q_per_req;
-    const uint32_t T = __ldg(tp.num_tokens + r), t0 = q << tp.granule_log2;
+    uint32_t T;
+    uint64_t tok0 = 0;                                 // tokens of the requests before r (dense side only)
+    if (tp.cu_tokens) { tok0 = __ldg(tp.cu_tokens + r); T = (uint32_t)(__ldg(tp.cu_tokens + r + 1) - tok0); }
+    else              { T = __ldg(tp.num_tokens + r); }
+    const uint32_t t0 = q << tp.granule_log2;
     if (t0 >= T) continue;
     const uint32_t n = min(g, T - t0);
-    const int32_t sb = __ldg(tp.src_tables + (size_t)r * tp.max_src_blocks + (t0 >> tp.src_bs_log2));
-    const int32_t db = __ldg(tp.dst_tables + (size_t)r * tp.max_dst_blocks + (t0 >> tp.dst_bs_log2));
-    if ((uint32_t)sb >= tp.src_num_blocks || (uint32_t)db >= tp.dst_num_blocks) {
-      if (tp.error && lane == 0) atomicOr(tp.error, 1u);
+    bool ok = true;
+    const int64_t so = tables_side(p.src, tp.src_tables, tp.max_src_blocks, tp.src_bs_log2, tp.src_s_block, tp.src_num_blocks,
+                                   r, t0, plane, T, tok0, p.tok_bytes, ok);
+    const int64_t dof = tables_side(p.dst, tp.dst_tables, tp.max_dst_blocks, tp.dst_bs_log2, tp.dst_s_block, tp.dst_num_blocks,
+                                    r, t0, plane, T, tok0, p.tok_bytes, ok);
+    uint32_t bad = ok ? 0u : 1u;
+    if (tp.cu_tokens && (tok0 + T) * (uint64_t)(p.src.dense ? p.src.s_layer : p.dst.s_layer) > tp.dense_bytes) bad |= 2u;
+    if (bad) {                                         // nothing out of bounds is touched; the caller reads the flag
+      if (tp.error && lane == 0) atomicOr(tp.error, bad);
       continue;
     }
-    const uint32_t so = t0 & ((1u << tp.src_bs_log2) - 1), dof = t0 & ((1u << tp.dst_bs_log2) - 1);
-    const char* s = p.src.base + (int64_t)(plane >> 1) * p.src.s_layer + (int64_t)(plane & 1) * p.src.s_kv +
-                    (int64_t)sb * tp.src_s_block + (int64_t)so * p.src.s_token;
-    char* d = p.dst.base + (int64_t)(plane >> 1) * p.dst.s_layer + (int64_t)(plane & 1) * p.dst.s_kv +
-              (int64_t)db * tp.dst_s_block + (int64_t)dof * p.dst.s_token;
-    copy_rows<VEC, UNROLL, HINT>(p, s, d, n, lane, G, vpr, pow2, pol);
+    copy_rows<VEC, UNROLL, HINT>(p, p.src.base + so, p.dst.base + dof, n, lane, G, vpr, pow2, pol);
   }
 }
 

@@ -208,3 +208,61 @@ def test_fuzz_table_driven_transfer(idx):
     G.assert_same(P.to_numpy(dst_buf), exp, what)
     assert int(flag.item()) == 0, what
     G.assert_same(P.to_numpy(src_buf), src_np, what + " (src unchanged)")
+
+
+@pytest.mark.parametrize("idx", range(FUZZ_OFFSET, FUZZ_OFFSET + max(1, FUZZ_CASES * 3 // 10)))
+def test_fuzz_table_driven_pack_unpack_windows(idx):
+    """flowkv_pack_tables / flowkv_unpack_tables: device-resident tables and cumulative lengths, layer windows split
+    at a random layer; each window == the oracle's okv_pack_window, unpacking them rebuilds the oracle's transfer;
+    a window buffer that is too small raises flag bit 2 and is left untouched."""
+    rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
+    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
+    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d)
+    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
+    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
+    P.fill_sentinel(dst_buf)
+    src_np = P.to_numpy(src_buf)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs_s, "strided" if ss else lay_s, ss)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs_d, "strided" if sd else lay_d, sd)
+    Ts = [t for t, _, _ in reqs]
+    total, max_t = sum(Ts), max(Ts) + int(rng.integers(0, 9))
+    st, dt, _ = _device_tables(reqs, max(1, -(-max_t // bs_s)), max(1, -(-max_t // bs_d)))
+    cu = torch.from_numpy(np.concatenate([[0], np.cumsum(Ts)]).astype(np.int64)).cuda()
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    tn = {k: v for k, v in tuning.items() if k in ("threads", "group_threads", "max_sms", "ctas_per_sm")} or None
+    tokb = H * D * 2
+    cut = int(rng.integers(0, L + 1))
+    what = f"tables windows case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} T={Ts} cut={cut} {tn}"
+    for w0, w1 in ((0, cut), (cut, L)):
+        nb = total * 2 * (w1 - w0) * tokb
+        win = P.alloc_bytes(nb + 32)
+        P.fill_sentinel(win)
+        n0 = F.flowkv_launch_count()
+        F.flowkv_pack_tables(src, st.data_ptr(), cu.data_ptr(), len(reqs), st.shape[1], max_t, win.data_ptr(), nb, w0, w1,
+                             flag.data_ptr(), tn)
+        F.flowkv_unpack_tables(dst, dt.data_ptr(), cu.data_ptr(), len(reqs), dt.shape[1], max_t, win.data_ptr(), nb, w0, w1,
+                               flag.data_ptr(), tn)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (2 if max_t and w1 > w0 else 0), what
+        exp = np.full(nb + 32, P.SENTINEL_BYTE, np.uint8)
+        off = 0
+        for t, a, _ in reqs:
+            O.pack_window(src_np, gs, a, t, exp, off, w0, w1)
+            off += t
+        G.assert_same(P.to_numpy(win), exp, what + f" window [{w0},{w1})")
+    exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)
+    for t, a, b in reqs:
+        O.transfer(src_np, gs, exp, gd, a, b, t)
+    G.assert_same(P.to_numpy(dst_buf), exp, what + " (windows unpacked)")
+    assert int(flag.item()) == 0, what
+    if total and L:
+        nb = total * 2 * L * tokb
+        small = P.alloc_bytes(nb)
+        P.fill_sentinel(small)
+        F.flowkv_pack_tables(src, st.data_ptr(), cu.data_ptr(), len(reqs), st.shape[1], max_t, small.data_ptr(), nb - 16, 0, L,
+                             flag.data_ptr(), tn)
+        torch.cuda.synchronize()
+        assert int(flag.item()) & 2, what + " (capacity flag)"
+        last = max(i for i, t in enumerate(Ts) if t)           # the request that would cross the end is skipped whole
+        lo = int(np.cumsum([0] + Ts)[last]) * 2 * L * tokb
+        assert np.all(P.to_numpy(small)[lo:] == P.SENTINEL_BYTE), what + " (bytes of the skipped request)"
