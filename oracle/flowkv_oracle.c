@@ -24,6 +24,8 @@
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): numpy fancy-indexing
  * special cases, a self-describing pool decoded from the definition, identity
  * tables == memcmp, untouched-byte sentinels, all 65,536 16-bit patterns,
+ * 1-, 4- and 8-byte elements against numpy item views (the generic branch of
+ * okv_copy_elem), all 256 byte codes and fp32 NaN payloads,
  * pack∘unpack identity, layer windows == planes cut out of the wire format,
  * brute-force minimal partition count on tiny tables,
  * the paper's "fully contiguous => 1 transfer" and

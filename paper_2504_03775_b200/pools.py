@@ -16,10 +16,6 @@ from . import synth
 SENTINEL_BYTE = 0xA5
 
 
-def pool_numel_bytes(spec: synth.PoolSpec, shape: synth.Shape) -> int:
-    return spec.bytes(shape)
-
-
 def describe(spec: synth.PoolSpec, shape: synth.Shape, base_ptr: int) -> F.flowkv_pool:
     return F.make_pool(base_ptr, shape.num_layers, shape.num_kv_heads, shape.head_dim, shape.elem_bytes,
                        spec.num_blocks, spec.block_size, spec.layout)
@@ -36,7 +32,9 @@ def fill_values(buf: torch.Tensor, dist: str, dtype: str, seed: int, chunk_bytes
     denormals included).  Filled in place, chunk by chunk, so no pool-sized temporary exists."""
     gen = torch.Generator(device=buf.device)
     gen.manual_seed(seed)
-    tdt = {"bf16": torch.bfloat16, "fp16": torch.float16}[dtype]
+    tdt = {"bf16": torch.bfloat16, "fp16": torch.float16, "fp32": torch.float32, "fp8": None}[dtype]
+    if tdt is None:                   # fp8: every byte is a valid code; values are irrelevant to a copy
+        dist = "bits"
     n = buf.numel()
     for off in range(0, n, chunk_bytes):
         part = buf[off:min(off + chunk_bytes, n)]

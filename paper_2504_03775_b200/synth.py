@@ -20,16 +20,19 @@ import numpy as np
 SEED_BASE = 250403775  # + 1000*config + point
 
 
+ELEM_BYTES = {"fp8": 1, "fp16": 2, "bf16": 2, "fp32": 4}
+
+
 @dataclass(frozen=True)
 class Shape:
     num_layers: int
     num_kv_heads: int
     head_dim: int
-    dtype: str  # "fp16" | "bf16" — 2-byte elements either way
+    dtype: str  # "fp16" | "bf16" (2-byte elements), "fp8" (1 byte), "fp32" (4 bytes)
 
     @property
     def elem_bytes(self) -> int:
-        return 2
+        return ELEM_BYTES[self.dtype]
 
     @property
     def bytes_per_token(self) -> int:
@@ -39,6 +42,7 @@ class Shape:
 TINY = Shape(2, 2, 64, "fp16")
 LLAMA3_8B = Shape(32, 8, 128, "bf16")
 LLAMA3_70B = Shape(80, 8, 128, "bf16")
+LLAMA3_8B_FP8 = Shape(32, 8, 128, "fp8")      # fp8 KV cache: rows of 128 B
 
 
 @dataclass(frozen=True)

@@ -10,14 +10,18 @@ import itertools
 import numpy as np
 
 
-def logical_view(buf_u8: np.ndarray, layout: str, L: int, NB: int, BS: int, H: int, D: int) -> np.ndarray:
-    """uint16 view of a flat pool buffer, indexed [l, c, block, token, head, dim] (2-byte elements).
+ELEM_DTYPE = {1: np.uint8, 2: np.uint16, 4: np.uint32, 8: np.uint64}
+
+
+def logical_view(buf_u8: np.ndarray, layout: str, L: int, NB: int, BS: int, H: int, D: int, e: int = 2) -> np.ndarray:
+    """Unsigned-integer view (one item per `e`-byte element) of a flat pool buffer, indexed
+    [l, c, block, token, head, dim].
 
     lkbthd = Eq. 5 left side  (L,2,B,H) with H=[token][head][dim]
     blkhtd = Eq. 5 right side (B,L,2,H) with H=[head][token][dim]
     blkthd = Eq. 5 right side (B,L,2,H) with H=[token][head][dim] (H as on the left side)
     """
-    w = buf_u8.view(np.uint16)
+    w = buf_u8.view(ELEM_DTYPE[e])
     if layout == "lkbthd":
         return w.reshape(L, 2, NB, BS, H, D)
     if layout == "blkhtd":

@@ -408,3 +408,148 @@ def test_expected_break_rate_independent_sides():
         return out
     segs = O.count_segments(tab(0.5), 16, tab(1 / 16), 16, n * 16)
     assert abs(segs / n - (1 - 0.5 * 15 / 16)) < 0.01
+
+
+# ---------------------------------------------------------------------------------------
+# element sizes other than 2 bytes (reading A14: elements move as `elem_bytes` raw bytes; fp8 = 1, fp32 = 4)
+# These reach okv_copy_elem's generic branch, which no 2-byte test touches.
+# ---------------------------------------------------------------------------------------
+ELEM_SIZES = [1, 4, 8]
+
+
+def _geom_e(layout, L, H, D, e, NB, BS):
+    return getattr(O.PoolGeom, layout)(L, H, D, e, NB, BS)
+
+
+@pytest.mark.parametrize("e", ELEM_SIZES)
+@pytest.mark.parametrize("layout", ["lkbthd", "blkhtd", "blkthd"])
+def test_elem_sizes_same_layout_equals_numpy_fancy_indexing(e, layout):
+    """numpy indexes whole `e`-byte items (uint8 / uint32 / uint64 views).  Catches: a dim stride that is not
+    elem_bytes, a generic-branch copy that drops, repeats or reorders bytes of an element."""
+    rng = np.random.default_rng(30 + e)
+    L, H, D, NB, BS, n = 2, 3, 8, 9, 4, 5
+    g = _geom_e(layout, L, H, D, e, NB, BS)
+    assert g.span_bytes() == L * 2 * NB * BS * H * D * e
+    src = _rand_pool(rng, g.span_bytes())
+    dst = np.full(g.span_bytes(), SENT, np.uint8)
+    Src, Dst = rng.permutation(NB)[:n], rng.permutation(NB)[:n]
+    O.transfer(src, g, dst, g, Src, Dst, n * BS)
+    exp = np.full(g.span_bytes(), SENT, np.uint8)
+    ev, sv = Hh.logical_view(exp, layout, L, NB, BS, H, D, e), Hh.logical_view(src, layout, L, NB, BS, H, D, e)
+    ev[:, :, Dst] = sv[:, :, Src]
+    assert np.array_equal(dst, exp)
+
+
+@pytest.mark.parametrize("e", ELEM_SIZES)
+@pytest.mark.parametrize("bs_s,bs_d,src_layout,dst_layout,T", [
+    (4, 4, "lkbthd", "blkhtd", 13), (2, 8, "lkbthd", "blkhtd", 16), (8, 2, "blkhtd", "lkbthd", 11), (4, 8, "blkthd", "blkhtd", 9)])
+def test_elem_sizes_conversion_partial_block_and_untouched_bytes(e, bs_s, bs_d, src_layout, dst_layout, T):
+    """Layout + block-size conversion with a partial last block, token by token in numpy item views; every other
+    dst byte keeps the sentinel.  Catches: head/token transposition or tail spill that only shows at e != 2."""
+    rng = np.random.default_rng(40 + e)
+    L, H, D = 2, 2, 4
+    ns, nd = -(-T // bs_s), -(-T // bs_d)
+    NBs, NBd = ns + 2, nd + 2
+    gs, gd = _geom_e(src_layout, L, H, D, e, NBs, bs_s), _geom_e(dst_layout, L, H, D, e, NBd, bs_d)
+    src = _rand_pool(rng, gs.span_bytes())
+    src0 = src.copy()
+    dst = np.full(gd.span_bytes(), SENT, np.uint8)
+    Src, Dst = rng.permutation(NBs)[:ns], rng.permutation(NBd)[:nd]
+    O.transfer(src, gs, dst, gd, Src, Dst, T)
+    exp = np.full(gd.span_bytes(), SENT, np.uint8)
+    ev, sv = Hh.logical_view(exp, dst_layout, L, NBd, bs_d, H, D, e), Hh.logical_view(src, src_layout, L, NBs, bs_s, H, D, e)
+    for t in range(T):
+        ev[:, :, Dst[t // bs_d], t % bs_d] = sv[:, :, Src[t // bs_s], t % bs_s]
+    assert np.array_equal(dst, exp)
+    assert np.array_equal(src, src0)
+
+
+@pytest.mark.parametrize("e", ELEM_SIZES)
+def test_elem_sizes_wire_format_windows_and_unpack(e):
+    """Wire format A12 and layer windows A20 in `e`-byte items: pack == numpy gather, a window == the planes cut out
+    of the wire format, unpack(pack) == transfer.  Catches: a bytes-per-token that assumes 2-byte elements."""
+    rng = np.random.default_rng(50 + e)
+    L, H, D, NB, BS = 3, 2, 4, 10, 4
+    g = _geom_e("blkhtd", L, H, D, e, NB, BS)
+    assert g.bytes_per_token == 2 * L * H * D * e
+    src = _rand_pool(rng, g.span_bytes())
+    Ts = [6, 0, 9]
+    perm = rng.permutation(NB)
+    tabs, off = [], 0
+    for T in Ts:
+        tabs.append(perm[off:off + -(-T // BS)]); off += -(-T // BS)
+    sv = Hh.logical_view(src, "blkhtd", L, NB, BS, H, D, e)
+    staging = np.full(sum(Ts) * g.bytes_per_token, SENT, np.uint8)
+    parts, tok_off = [], 0
+    for T, tab in zip(Ts, tabs):
+        O.pack(src, g, tab, T, staging, tok_off)
+        tok_off += T
+        parts.append(sv[:, :, tab].reshape(L, 2, len(tab) * BS, H, D)[:, :, :T].reshape(-1))
+    assert np.array_equal(staging.view(Hh.ELEM_DTYPE[e]), np.concatenate(parts))
+    tokb = H * D * e
+    w0, w1 = 1, 3
+    win = np.full(sum(Ts) * 2 * (w1 - w0) * tokb, SENT, np.uint8)
+    cut, tok_off = [], 0
+    for T, tab in zip(Ts, tabs):
+        O.pack_window(src, g, tab, T, win, tok_off, w0, w1)
+        base = tok_off * g.bytes_per_token
+        cut.append(staging[base + 2 * w0 * T * tokb: base + 2 * w1 * T * tokb])
+        tok_off += T
+    assert np.array_equal(win, np.concatenate(cut))
+    gd = _geom_e("lkbthd", L, H, D, e, NB, BS * 2)
+    dperm = rng.permutation(NB)
+    d1, d2 = np.full(gd.span_bytes(), SENT, np.uint8), np.full(gd.span_bytes(), SENT, np.uint8)
+    d3 = np.full(gd.span_bytes(), SENT, np.uint8)
+    tok_off = doff = 0
+    for T, tab in zip(Ts, tabs):
+        nb = -(-T // (BS * 2))
+        dtab = dperm[doff:doff + nb]; doff += nb
+        O.unpack(staging, tok_off, d1, gd, dtab, T)
+        O.transfer(src, g, d2, gd, tab, dtab, T)
+        O.unpack_window(win, tok_off, d3, gd, dtab, T, w0, w1)
+        tok_off += T
+    assert np.array_equal(d1, d2)
+    lay = gd.s_layer
+    assert np.array_equal(d3[w0 * lay:w1 * lay], d2[w0 * lay:w1 * lay])
+    assert np.all(d3[:w0 * lay] == SENT) and np.all(d3[w1 * lay:] == SENT)
+
+
+def test_elem_size_is_only_how_a_row_is_cut_into_items():
+    """The same bytes described as (Dh=16,e=1), (8,2), (4,4), (2,8) are the same rows, so every description must
+    move the same bytes.  Catches: any place where elem_bytes enters other than through Dh*e."""
+    rng = np.random.default_rng(60)
+    L, H, NB, BS, T = 2, 3, 7, 4, 18
+    outs = []
+    for D, e in [(16, 1), (8, 2), (4, 4), (2, 8)]:
+        gs, gd = _geom_e("lkbthd", L, H, D, e, NB, BS), _geom_e("blkhtd", L, H, D, e, NB, BS * 2)
+        r = np.random.default_rng(61)
+        src = _rand_pool(r, gs.span_bytes())
+        Src, Dst = r.permutation(NB)[:5], r.permutation(NB)[:3]
+        dst = np.full(gd.span_bytes(), SENT, np.uint8)
+        O.transfer(src, gs, dst, gd, Src, Dst, T)
+        outs.append(dst)
+    for o in outs[1:]:
+        assert np.array_equal(o, outs[0])
+
+
+def test_all_256_byte_patterns_and_fp32_specials_survive():
+    """Raw-bit fidelity at e = 1 (every fp8 code) and e = 4 (NaN payloads, -0, Inf, denormals as uint32)."""
+    L, H, D, BS, NB = 1, 1, 16, 4, 4
+    g = _geom_e("lkbthd", L, H, D, 1, NB, BS)                 # 2*4*4*16 = 512 one-byte elements
+    src = np.tile(np.arange(256, dtype=np.uint8), 2)
+    assert src.size == g.span_bytes()
+    dst = np.zeros_like(src)
+    perm = np.asarray([2, 0, 3, 1])
+    O.transfer(src, g, dst, g, perm, np.arange(NB), NB * BS)
+    sv, dv = Hh.logical_view(src, "lkbthd", L, NB, BS, H, D, 1), Hh.logical_view(dst, "lkbthd", L, NB, BS, H, D, 1)
+    assert np.array_equal(dv, sv[:, :, perm])
+    assert np.array_equal(np.sort(dst), np.sort(src))
+    g4 = _geom_e("lkbthd", L, H, 4, 4, NB, BS)
+    special = np.asarray([0x7FC00001, 0xFFC12345, 0x7F800000, 0xFF800000, 0x80000000, 0x00000001, 0x807FFFFF, 0x7FFFFFFF],
+                         np.uint32)
+    src4 = np.resize(special, g4.span_bytes() // 4).copy()
+    src4[::3] ^= np.arange(src4[::3].size, dtype=np.uint32) << 8      # make rows distinguishable
+    dst4 = np.zeros(g4.span_bytes(), np.uint8)
+    O.transfer(src4.view(np.uint8), g4, dst4, g4, perm, np.arange(NB), NB * BS)
+    s4, d4 = Hh.logical_view(src4.view(np.uint8), "lkbthd", L, NB, BS, H, 4, 4), Hh.logical_view(dst4, "lkbthd", L, NB, BS, H, 4, 4)
+    assert np.array_equal(d4, s4[:, :, perm])
