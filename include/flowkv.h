@@ -173,9 +173,12 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
 
 /* Build a plan: validate (a1), bidirectional segment alignment (a2), tile schedule (a3),
  * upload (a4; one stream-ordered allocation from a library-owned memory pool + one cudaMemcpyAsync from cached pinned memory on a library-owned
- * upload stream; `stream` only waits on the upload's event.  No host synchronisation, so planning and
- * uploading batch k+1 overlap the move of batch k.  Small plans are not uploaded at all: their schedule
- * travels in the kernel parameters, see flowkv_tuning.plan_in_params).
+ * upload stream; `stream` only waits on the upload's event.  The call does not synchronise with `stream` or with
+ * any caller kernel, so planning and uploading batch k+1 overlap the move of batch k: pinned staging buffers
+ * whose previous upload is still in flight are skipped (cudaEventQuery) and a fresh one is taken; only with 256
+ * uploads in flight at once does the call wait for the oldest — a few-KiB DMA on the library's own stream.  Small
+ * plans are not uploaded at all: their schedule travels in the kernel parameters, see
+ * flowkv_tuning.plan_in_params).
  *   src, dst : HOST pointers to pool descriptors; either may be NULL (pack-only / unpack-only).
  *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
  *   tuning   : HOST pointer or NULL.
@@ -278,6 +281,9 @@ FLOWKV_API flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* plan, voi
  *   max_tokens  upper bound of num_tokens[] known to the host (sizes the grid; tiles past a request's end exit)
  *   error_flag  DEVICE uint32 or NULL: OR-ed with 1 if a block id in use is outside its pool (that tile is
  *               skipped, nothing out of bounds is touched); the host cannot validate what it never sees.
+ *               The library only ever ORs bits into the flag and never clears or reads it: the CALLER zeroes it
+ *               (cudaMemsetAsync on `stream` before the call, or once if it reads "any error since then") and
+ *               reads it back after synchronising `stream`.
  *               A dst block named twice is NOT detected (undefined result, as without FLOWKV_CHECK_DST_ALIAS).
  *   tuning      threads, group_threads, max_sms, ctas_per_sm are honoured; may be NULL.
  * Errors: INVALID_ARG, ALIGN, SHAPE_MISMATCH, UNSUPPORTED as for flowkv_plan; TABLE_LEN if max_*_blocks cannot
@@ -287,6 +293,18 @@ FLOWKV_API flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const fl
                                                 const uint32_t* num_tokens, uint32_t n_reqs,
                                                 uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
                                                 uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
+
+/* Layer-range form of flowkv_transfer_tables (S§8f NEXT-2): only layers [layer_begin, layer_end)
+ * move, everything else in dst is untouched.  One launch per call (zero when the range is empty), so a layer-wise
+ * sender that overlaps the transfer with the prefill of later layers needs no host plan and can live inside a
+ * captured CUDA graph whose tables change between replays.  flowkv_transfer_tables == the range [0, num_layers).
+ * Errors as flowkv_transfer_tables, plus INVALID_ARG for a range outside [0, num_layers]. */
+FLOWKV_API flowkv_status flowkv_transfer_tables_layers(const flowkv_pool* src, const flowkv_pool* dst,
+                                                       const int32_t* src_tables, const int32_t* dst_tables,
+                                                       const uint32_t* num_tokens, uint32_t n_reqs,
+                                                       uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
+                                                       uint32_t layer_begin, uint32_t layer_end,
+                                                       uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
 
 /* Table-driven pack / unpack of the layer window [layer_begin, layer_end) (the window [0, num_layers) is the wire
  * format of flowkv_pack): the same kernel with one side dense.  Tables as for flowkv_transfer_tables; lengths come as

@@ -10,7 +10,7 @@
 #include <utility>
 #include <vector>
 
-#include "../../include/flowkv.h"
+#include "flowkv_internal.h"
 
 struct flowkv_allocator_s {
   uint32_t num_blocks = 0, free_blocks = 0;
@@ -50,13 +50,12 @@ struct flowkv_allocator_s {
 
 // set by api.cpp's error channel
 extern "C" const char* flowkv_last_error(void);
-namespace flowkv { void set_last_error(const std::string& msg); }
 static flowkv_status fail(flowkv_status s, const char* msg) {
   flowkv::set_last_error(msg);
   return s;
 }
 
-extern "C" {
+namespace impl {
 
 flowkv_status flowkv_alloc_create(uint32_t num_blocks, flowkv_allocator_t** out) {
   if (!out || !num_blocks) return fail(FLOWKV_ERR_INVALID_ARG, "allocator: out is NULL or num_blocks is 0");
@@ -134,4 +133,26 @@ flowkv_status flowkv_alloc_stats(const flowkv_allocator_t* a, uint32_t* free_blo
 
 void flowkv_alloc_destroy(flowkv_allocator_t* a) { delete a; }
 
+}  // namespace impl
+
+// exported C ABI (exceptions never cross it; see api.cpp).  A std::bad_alloc inside allocate / free returns
+// FLOWKV_ERR_NOMEM; the allocator must then be destroyed (its indexes may be half-updated).
+extern "C" {
+flowkv_status flowkv_alloc_create(uint32_t num_blocks, flowkv_allocator_t** out) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_alloc_create(num_blocks, out); });
+}
+flowkv_status flowkv_alloc_allocate(flowkv_allocator_t* a, uint32_t n, int32_t* out_ids, uint32_t* n_segments) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_alloc_allocate(a, n, out_ids, n_segments); });
+}
+flowkv_status flowkv_alloc_free(flowkv_allocator_t* a, const int32_t* ids, uint32_t n) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_alloc_free(a, ids, n); });
+}
+flowkv_status flowkv_alloc_stats(
+    const flowkv_allocator_t* a, uint32_t* free_blocks, uint32_t* free_segments,
+    uint32_t* largest_segment) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_alloc_stats(a, free_blocks, free_segments, largest_segment); });
+}
+void flowkv_alloc_destroy(flowkv_allocator_t* a) {
+  try { impl::flowkv_alloc_destroy(a); } catch (...) {}
+}
 }  // extern "C"

@@ -57,24 +57,49 @@ struct PinnedBuf {
 
 class PinnedCache {
  public:
+  // Never blocks on the common path: a cached buffer whose last upload is still in flight (cudaEventQuery) is
+  // skipped and a fresh one is allocated instead.  Only when kMaxBuffers buffers exist and all of them are
+  // pending does the call wait — outside the mutex — for the oldest upload (a few-KiB DMA on the library's own
+  // upload stream, never a caller kernel: the plan pool does not reuse memory through cross-stream dependencies).
   cudaError_t acquire(size_t bytes, PinnedBuf& out) {
+    PinnedBuf oldest{};
     {
       std::lock_guard<std::mutex> lk(mu_);
-      for (size_t i = 0; i < free_.size(); ++i)
-        if (free_[i].cap >= bytes) {
-          out = free_[i];
-          free_.erase(free_.begin() + i);
-          if (out.pending) { cudaEventSynchronize(out.ev); out.pending = false; }
-          return cudaSuccess;
+      for (size_t i = 0; i < free_.size(); ++i) {
+        if (free_[i].cap < bytes) continue;
+        if (free_[i].pending) {
+          if (cudaEventQuery(free_[i].ev) != cudaSuccess) continue;     // upload still reading this buffer
+          free_[i].pending = false;
         }
+        out = free_[i];
+        free_.erase(free_.begin() + i);
+        return cudaSuccess;
+      }
+      if (n_alive_ >= kMaxBuffers)
+        for (size_t i = 0; i < free_.size(); ++i)
+          if (free_[i].cap >= bytes) { oldest = free_[i]; free_.erase(free_.begin() + i); break; }
+      if (!oldest.p) ++n_alive_;
+    }
+    if (oldest.p) {
+      cudaError_t e = cudaEventSynchronize(oldest.ev);
+      if (e != cudaSuccess) { release(oldest); return e; }
+      oldest.pending = false;
+      out = oldest;
+      return cudaSuccess;
     }
     size_t cap = 64 << 10;
     while (cap < bytes) cap <<= 1;
     PinnedBuf b;
     cudaError_t e = cudaHostAlloc(&b.p, cap, cudaHostAllocDefault);
-    if (e != cudaSuccess) return e;
-    e = cudaEventCreateWithFlags(&b.ev, cudaEventDisableTiming);
-    if (e != cudaSuccess) { cudaFreeHost(b.p); return e; }
+    if (e == cudaSuccess) {
+      e = cudaEventCreateWithFlags(&b.ev, cudaEventDisableTiming);
+      if (e != cudaSuccess) cudaFreeHost(b.p);
+    }
+    if (e != cudaSuccess) {
+      std::lock_guard<std::mutex> lk(mu_);
+      --n_alive_;
+      return e;
+    }
     b.cap = cap;
     out = b;
     return cudaSuccess;
@@ -86,8 +111,10 @@ class PinnedCache {
   }
 
  private:
+  static constexpr size_t kMaxBuffers = 256;
   std::mutex mu_;
   std::vector<PinnedBuf> free_;
+  size_t n_alive_ = 0;
 };
 PinnedCache g_pinned;
 
@@ -118,6 +145,13 @@ cudaError_t upload_stream(int device, cudaStream_t* out, cudaMemPool_t* pool) {
     if (e == cudaSuccess) {
       uint64_t never = ~0ull;
       e = cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &never);
+    }
+    if (e == cudaSuccess) {
+      // Plan buffers are freed on caller streams and allocated on the upload stream.  Reuse "through an internal
+      // dependency" would make the upload of batch k+1 wait for the kernel of batch k to finish; only memory whose
+      // free has already completed may be reused (otherwise the pool grows by one small buffer).
+      int off = 0;
+      e = cudaMemPoolSetAttribute(mp, cudaMemPoolReuseAllowInternalDependencies, &off);
     }
     if (e != cudaSuccess) { cudaStreamDestroy(st); return e; }
     g_plan_pool[device] = mp;
@@ -231,6 +265,13 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
   op.tile_order = t.tile_order == 2 ? 1 : 0;
   const uint64_t n_tiles = ((uint64_t)op.sched.n_flat << op.sched.flat_shift) + (uint64_t)op.sched.n_per_plane() * 2 * pl->g.L;
   if (ls.variant == FLOWKV_VARIANT_BULK) {
+    // a ring slot holds the largest chunk (span mode: at least one token's plane bytes); two slots must fit in
+    // shared memory, else the plan runs the register path (reported in flowkv_plan_stats.variant)
+    const uint32_t stage = ((std::max<uint32_t>(op.sched.mode == MODE_FLAT ? op.sched.flat_tile : op.max_chunk_bytes, 1024)) + 127) & ~127u;
+    const uint32_t cap = (pl->max_smem_optin ? pl->max_smem_optin : 232448) - 1024;
+    if (2ull * stage > cap) ls.variant = FLOWKV_VARIANT_LDST;
+  }
+  if (ls.variant == FLOWKV_VARIANT_BULK) {
     ls.threads = 32;
     ls.group_threads = 32;
     ls.stage_bytes = std::max<uint32_t>(op.sched.mode == MODE_FLAT ? op.sched.flat_tile : op.max_chunk_bytes, 1024);
@@ -305,7 +346,7 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
   flowkv_tuning tn{};
   if (tuning) tn = *tuning;
   if ((st = check_tuning(tn)) != FLOWKV_OK) return st;
-  if ((st = validate_requests(src, dst, reqs, n_reqs, flags, err)) != FLOWKV_OK) return fail(st, err);
+  if ((st = validate_requests(src, dst, reqs, n_reqs, flags, err)) != FLOWKV_OK) return fail(st, err);   // (guarded by the C-ABI wrapper)
 
   flowkv_plan_t* pl = new (std::nothrow) flowkv_plan_s();
   if (!pl) return fail(FLOWKV_ERR_NOMEM, "out of host memory");
@@ -538,7 +579,7 @@ uint64_t window_bytes(const flowkv_plan_t* pl, uint32_t l0, uint32_t l1) {
 
 }  // namespace
 
-extern "C" {
+namespace impl {
 
 flowkv_status flowkv_pool_strides(flowkv_pool* p) {
   if (!p) return fail(FLOWKV_ERR_INVALID_ARG, "pool is NULL");
@@ -628,7 +669,7 @@ flowkv_status flowkv_transfer_layers(const flowkv_plan_t* pl, uint32_t layer_beg
 
 flowkv_status flowkv_transfer(const flowkv_plan_t* pl, void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
-  return flowkv_transfer_layers(pl, 0, pl->g.L, stream);
+  return impl::flowkv_transfer_layers(pl, 0, pl->g.L, stream);
 }
 
 flowkv_status flowkv_pack_layers(const flowkv_plan_t* pl, void* staging, uint64_t bytes, uint32_t layer_begin,
@@ -644,7 +685,7 @@ flowkv_status flowkv_pack_layers(const flowkv_plan_t* pl, void* staging, uint64_
 
 flowkv_status flowkv_pack(const flowkv_plan_t* pl, void* staging, uint64_t bytes, void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
-  return flowkv_pack_layers(pl, staging, bytes, 0, pl->g.L, stream);
+  return impl::flowkv_pack_layers(pl, staging, bytes, 0, pl->g.L, stream);
 }
 
 flowkv_status flowkv_unpack_layers(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, uint32_t layer_begin,
@@ -660,7 +701,7 @@ flowkv_status flowkv_unpack_layers(const flowkv_plan_t* pl, const void* staging,
 
 flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, void* stream) {
   if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
-  return flowkv_unpack_layers(pl, staging, bytes, 0, pl->g.L, stream);
+  return impl::flowkv_unpack_layers(pl, staging, bytes, 0, pl->g.L, stream);
 }
 
 flowkv_status flowkv_window_bytes(const flowkv_plan_t* pl, uint32_t layer_begin, uint32_t layer_end, uint64_t* bytes) {
@@ -853,7 +894,7 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   if (!(src && dst) && (uintptr_t)dense % 32) ls.vec_bytes = 16;
   const uint32_t tile_bytes = (1u << tp.granule_log2) * g.tok_bytes;
   ls.threads = tn.threads ? tn.threads : 512;
-  uint32_t grp = tn.group_threads ? std::min(tn.group_threads, ls.threads) : 128;
+  uint32_t grp = tn.group_threads ? std::min(tn.group_threads, ls.threads) : std::min<uint32_t>(128u, ls.threads);
   while (grp > 32 && grp * ls.vec_bytes > tile_bytes) grp >>= 1;       // no more threads than vectors in a tile
   ls.group_threads = grp;
   const uint32_t use_sms = tn.max_sms ? std::min<uint32_t>(tn.max_sms, (uint32_t)sms) : (uint32_t)sms;
@@ -878,6 +919,16 @@ flowkv_status flowkv_transfer_tables(const flowkv_pool* src, const flowkv_pool* 
   if (!src || !dst) return fail(FLOWKV_ERR_INVALID_ARG, "a pool is NULL");
   return tables_common(src, dst, src_tables, dst_tables, num_tokens, nullptr, n_reqs, max_src_blocks, max_dst_blocks,
                        max_tokens, nullptr, 0, 0, src->num_layers, error_flag, tuning, stream);
+}
+
+flowkv_status flowkv_transfer_tables_layers(const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables,
+                                            const int32_t* dst_tables, const uint32_t* num_tokens, uint32_t n_reqs,
+                                            uint32_t max_src_blocks, uint32_t max_dst_blocks, uint32_t max_tokens,
+                                            uint32_t layer_begin, uint32_t layer_end, uint32_t* error_flag,
+                                            const flowkv_tuning* tuning, void* stream) {
+  if (!src || !dst) return fail(FLOWKV_ERR_INVALID_ARG, "a pool is NULL");
+  return tables_common(src, dst, src_tables, dst_tables, num_tokens, nullptr, n_reqs, max_src_blocks, max_dst_blocks,
+                       max_tokens, nullptr, 0, layer_begin, layer_end, error_flag, tuning, stream);
 }
 
 flowkv_status flowkv_pack_tables(const flowkv_pool* src, const int32_t* src_tables, const uint64_t* cu_tokens, uint32_t n_reqs,
@@ -1031,4 +1082,121 @@ flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* pl, void* stream,
   return FLOWKV_OK;
 }
 
+}  // namespace impl
+
+// ---- the exported C ABI: every entry point runs its implementation under flowkv::guarded(), so that no C++
+// exception (std::bad_alloc from a vector, a set insert, a string) ever crosses into a C caller: the header
+// promises a status code, never a throw or an abort.
+extern "C" {
+flowkv_status flowkv_pool_strides(flowkv_pool* pool) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_pool_strides(pool); });
+}
+flowkv_status flowkv_plan(
+    const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs, uint32_t n_reqs,
+    uint32_t flags, const flowkv_tuning* tuning, void* stream, flowkv_plan_t** out) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_plan(src, dst, reqs, n_reqs, flags, tuning, stream, out); });
+}
+flowkv_status flowkv_plan_host(
+    const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs, uint32_t n_reqs,
+    uint32_t flags, const flowkv_tuning* tuning, flowkv_plan_t** out) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_plan_host(src, dst, reqs, n_reqs, flags, tuning, out); });
+}
+flowkv_status flowkv_plan_info(const flowkv_plan_t* plan, flowkv_plan_stats* stats, const flowkv_segment** segments) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_plan_info(plan, stats, segments); });
+}
+flowkv_status flowkv_transfer(const flowkv_plan_t* plan, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer(plan, stream); });
+}
+flowkv_status flowkv_pack(const flowkv_plan_t* plan, void* staging, uint64_t bytes, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_pack(plan, staging, bytes, stream); });
+}
+flowkv_status flowkv_unpack(const flowkv_plan_t* plan, const void* staging, uint64_t bytes, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_unpack(plan, staging, bytes, stream); });
+}
+flowkv_status flowkv_transfer_layers(
+    const flowkv_plan_t* plan, uint32_t layer_begin, uint32_t layer_end, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer_layers(plan, layer_begin, layer_end, stream); });
+}
+flowkv_status flowkv_pack_layers(
+    const flowkv_plan_t* plan, void* staging, uint64_t bytes, uint32_t layer_begin, uint32_t layer_end,
+    void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_pack_layers(plan, staging, bytes, layer_begin, layer_end, stream); });
+}
+flowkv_status flowkv_unpack_layers(
+    const flowkv_plan_t* plan, const void* staging, uint64_t bytes, uint32_t layer_begin,
+    uint32_t layer_end, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_unpack_layers(plan, staging, bytes, layer_begin, layer_end, stream); });
+}
+flowkv_status flowkv_window_bytes(
+    const flowkv_plan_t* plan, uint32_t layer_begin, uint32_t layer_end, uint64_t* bytes) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_window_bytes(plan, layer_begin, layer_end, bytes); });
+}
+flowkv_status flowkv_pack_window(
+    const flowkv_plan_t* plan, void* window, uint64_t bytes, uint32_t layer_begin, uint32_t layer_end,
+    void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_pack_window(plan, window, bytes, layer_begin, layer_end, stream); });
+}
+flowkv_status flowkv_unpack_window(
+    const flowkv_plan_t* plan, const void* window, uint64_t bytes, uint32_t layer_begin,
+    uint32_t layer_end, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_unpack_window(plan, window, bytes, layer_begin, layer_end, stream); });
+}
+flowkv_status flowkv_via_host_scratch_bytes(const flowkv_plan_t* plan, uint32_t n_chunks, uint64_t* bytes) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_via_host_scratch_bytes(plan, n_chunks, bytes); });
+}
+flowkv_status flowkv_transfer_via_host(
+    const flowkv_plan_t* plan, void* host_staging, uint64_t bytes, uint32_t n_chunks,
+    uint32_t ctas_per_kernel, void* device_scratch, uint64_t scratch_bytes, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer_via_host(plan, host_staging, bytes, n_chunks, ctas_per_kernel, device_scratch, scratch_bytes, stream); });
+}
+flowkv_status flowkv_transfer_tables(
+    const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables,
+    const int32_t* dst_tables, const uint32_t* num_tokens, uint32_t n_reqs, uint32_t max_src_blocks,
+    uint32_t max_dst_blocks, uint32_t max_tokens, uint32_t* error_flag, const flowkv_tuning* tuning,
+    void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer_tables(src, dst, src_tables, dst_tables, num_tokens, n_reqs, max_src_blocks, max_dst_blocks, max_tokens, error_flag, tuning, stream); });
+}
+flowkv_status flowkv_transfer_tables_layers(
+    const flowkv_pool* src, const flowkv_pool* dst, const int32_t* src_tables,
+    const int32_t* dst_tables, const uint32_t* num_tokens, uint32_t n_reqs, uint32_t max_src_blocks,
+    uint32_t max_dst_blocks, uint32_t max_tokens, uint32_t layer_begin, uint32_t layer_end,
+    uint32_t* error_flag, const flowkv_tuning* tuning, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer_tables_layers(src, dst, src_tables, dst_tables, num_tokens, n_reqs, max_src_blocks, max_dst_blocks, max_tokens, layer_begin, layer_end, error_flag, tuning, stream); });
+}
+flowkv_status flowkv_pack_tables(
+    const flowkv_pool* src, const int32_t* src_tables, const uint64_t* cu_tokens, uint32_t n_reqs,
+    uint32_t max_src_blocks, uint32_t max_tokens, void* window, uint64_t bytes, uint32_t layer_begin,
+    uint32_t layer_end, uint32_t* error_flag, const flowkv_tuning* tuning, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_pack_tables(src, src_tables, cu_tokens, n_reqs, max_src_blocks, max_tokens, window, bytes, layer_begin, layer_end, error_flag, tuning, stream); });
+}
+flowkv_status flowkv_unpack_tables(
+    const flowkv_pool* dst, const int32_t* dst_tables, const uint64_t* cu_tokens, uint32_t n_reqs,
+    uint32_t max_dst_blocks, uint32_t max_tokens, const void* window, uint64_t bytes,
+    uint32_t layer_begin, uint32_t layer_end, uint32_t* error_flag, const flowkv_tuning* tuning,
+    void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_unpack_tables(dst, dst_tables, cu_tokens, n_reqs, max_dst_blocks, max_tokens, window, bytes, layer_begin, layer_end, error_flag, tuning, stream); });
+}
+void flowkv_plan_destroy(flowkv_plan_t* plan) {
+  try { impl::flowkv_plan_destroy(plan); } catch (...) {}
+}
+const char* flowkv_status_string(flowkv_status s) {
+  return impl::flowkv_status_string(s);
+}
+const char* flowkv_last_error(void) {
+  return impl::flowkv_last_error();
+}
+uint64_t flowkv_launch_count(void) {
+  return impl::flowkv_launch_count();
+}
+uint64_t flowkv_api_call_count(void) {
+  return impl::flowkv_api_call_count();
+}
+flowkv_status flowkv_baseline_blockwise(
+    const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs, uint32_t n_reqs,
+    void* stream, uint64_t* n_calls) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_baseline_blockwise(src, dst, reqs, n_reqs, stream, n_calls); });
+}
+flowkv_status flowkv_baseline_segmentwise(const flowkv_plan_t* plan, void* stream, uint64_t* n_calls) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_baseline_segmentwise(plan, stream, n_calls); });
+}
 }  // extern "C"

@@ -4,12 +4,29 @@
 
 #include <stdint.h>
 
+#include <new>
 #include <string>
 #include <vector>
 
 #include "../../include/flowkv.h"
 
 namespace flowkv {
+
+void set_last_error(const std::string& msg);     // api.cpp: thread-local text behind flowkv_last_error()
+
+// Runs one C-ABI entry point's body; turns any C++ exception into a status code.
+template <class F>
+flowkv_status guarded(F&& f) noexcept {
+  try {
+    return f();
+  } catch (const std::bad_alloc&) {
+    try { set_last_error("out of host memory"); } catch (...) {}
+    return FLOWKV_ERR_NOMEM;
+  } catch (...) {
+    try { set_last_error("unexpected C++ exception inside the library"); } catch (...) {}
+    return FLOWKV_ERR_INVALID_ARG;
+  }
+}
 
 // ---------------------------------------------------------------------------------------------
 // Device-visible schedule entry ("chunk"): one unit of work of one plane.  The same chunk list

@@ -35,7 +35,7 @@ EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_pla
            "flowkv_launch_count", "flowkv_api_call_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
            "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host",
            "flowkv_window_bytes", "flowkv_pack_window", "flowkv_unpack_window", "flowkv_via_host_scratch_bytes",
-           "flowkv_transfer_tables", "flowkv_pack_tables", "flowkv_unpack_tables",
+           "flowkv_transfer_tables", "flowkv_transfer_tables_layers", "flowkv_pack_tables", "flowkv_unpack_tables",
            "flowkv_alloc_create", "flowkv_alloc_allocate", "flowkv_alloc_free", "flowkv_alloc_stats",
            "flowkv_alloc_destroy"]
 
@@ -112,6 +112,9 @@ def _load() -> C.CDLL:
     lib.flowkv_via_host_scratch_bytes.argtypes = [C.c_void_p, C.c_uint32, P(C.c_uint64)]
     lib.flowkv_transfer_tables.argtypes = [P(flowkv_pool), P(flowkv_pool), C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32,
                                            C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, P(flowkv_tuning), C.c_void_p]
+    lib.flowkv_transfer_tables_layers.argtypes = [P(flowkv_pool), P(flowkv_pool), C.c_void_p, C.c_void_p, C.c_void_p,
+                                                  C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
+                                                  C.c_void_p, P(flowkv_tuning), C.c_void_p]
     for fn in (lib.flowkv_pack_tables, lib.flowkv_unpack_tables):
         fn.argtypes = [P(flowkv_pool), C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_uint64,
                        C.c_uint32, C.c_uint32, C.c_void_p, P(flowkv_tuning), C.c_void_p]
@@ -386,6 +389,17 @@ def flowkv_transfer_tables(src: flowkv_pool, dst: flowkv_pool, src_tables: int, 
                                        C.c_void_p(num_tokens), n_reqs, max_src_blocks, max_dst_blocks, max_tokens,
                                        C.c_void_p(error_flag) if error_flag else None,
                                        C.byref(t) if t is not None else None, C.c_void_p(stream)))
+
+
+def flowkv_transfer_tables_layers(src: flowkv_pool, dst: flowkv_pool, src_tables: int, dst_tables: int, num_tokens: int,
+                                  n_reqs: int, max_src_blocks: int, max_dst_blocks: int, max_tokens: int,
+                                  layer_begin: int, layer_end: int, error_flag: int = 0, tuning=None, stream: int = 0) -> None:
+    """flowkv_transfer_tables restricted to layers [layer_begin, layer_end)."""
+    t = _tuning(tuning)
+    _check(_lib.flowkv_transfer_tables_layers(C.byref(src), C.byref(dst), C.c_void_p(src_tables), C.c_void_p(dst_tables),
+                                              C.c_void_p(num_tokens), n_reqs, max_src_blocks, max_dst_blocks, max_tokens,
+                                              layer_begin, layer_end, C.c_void_p(error_flag) if error_flag else None,
+                                              C.byref(t) if t is not None else None, C.c_void_p(stream)))
 
 
 def _tables_window(fn, pool, tables, cu_tokens, n_reqs, max_blocks, max_tokens, window, nbytes, layer_begin, layer_end,

@@ -24,10 +24,32 @@ def export_pool(buf: torch.Tensor) -> bytes:
     return pickle.dumps((fn, args))
 
 
+class _HandleUnpickler(pickle.Unpickler):
+    """Unpickles an export_pool() handle and nothing else: the only globals a handle may name are torch's CUDA-IPC
+    rebuild function, torch.device / dtype objects and the storage classes its argument tuple carries.  Anything
+    else (``os.system``, ``builtins.eval`` ...) is refused instead of being called."""
+    _ALLOWED = {("torch.multiprocessing.reductions", "rebuild_cuda_tensor"), ("torch", "device"), ("torch", "Size"),
+                ("torch", "uint8"), ("torch", "Tensor"), ("torch", "UntypedStorage"), ("torch.storage", "UntypedStorage"),
+                ("torch", "TypedStorage"), ("torch.storage", "TypedStorage")}
+
+    def find_class(self, module, name):
+        if (module, name) not in self._ALLOWED:
+            raise pickle.UnpicklingError(f"peer handle names {module}.{name}: not a CUDA-IPC pool handle")
+        return super().find_class(module, name)
+
+
 def import_pool(handle: bytes) -> torch.Tensor:
     """Map an exported buffer into this process; ``.data_ptr()`` is what ``flowkv.make_pool`` takes.
-    The mapping lives as long as the returned tensor."""
-    fn, args = pickle.loads(handle)
+    The mapping lives as long as the returned tensor.
+
+    ``handle`` must come from :func:`export_pool` in another process ON THE SAME MACHINE.  It is unpickled with a
+    restricted unpickler (only torch's CUDA-IPC rebuild function and its plain arguments are accepted), so a forged
+    handle is rejected rather than executed; mapping another process's memory still requires trusting that process
+    with the bytes this GPU writes there."""
+    import io
+    fn, args = _HandleUnpickler(io.BytesIO(handle)).load()
+    if fn is not reductions.rebuild_cuda_tensor:
+        raise pickle.UnpicklingError("peer handle does not rebuild a CUDA tensor")
     t = fn(*args)
     assert t.is_cuda and t.dtype == torch.uint8
     return t

@@ -175,6 +175,45 @@ def _tables_from_trace(rng, req_blocks: Sequence[int], num_blocks: int, mean: fl
     return out
 
 
+def alloc_free_trace(rng, req_blocks: Sequence[int], num_blocks: int, mean: float) -> List[tuple]:
+    """The event list of the alloc/free trace behind ``_tables_from_trace`` — WITHOUT deciding which blocks an
+    allocation gets: ("alloc", key, n) for the earlier tenants that fill the pool (Geometric(mean) blocks each),
+    ("free", key) for the seeded subset that finishes (in seeded order, until the batch plus 10 % fits), then
+    ("request", r, n) for the batch.  Which ids each allocation receives is the block allocator's business
+    (P:L105): feed the events to any allocator with ``tables_from_allocator``."""
+    used = int(sum(req_blocks))
+    events, sizes, pos = [], [], 0
+    while pos < num_blocks:
+        n = min(int(rng.geometric(1.0 / mean)), num_blocks - pos)
+        events.append(("alloc", len(sizes), n))
+        sizes.append(n)
+        pos += n
+    have, want = 0, min(num_blocks, int(np.ceil(1.1 * used)))
+    for ti in rng.permutation(len(sizes)):
+        if have >= want:
+            break
+        events.append(("free", int(ti)))
+        have += sizes[int(ti)]
+    if have < used:
+        raise ValueError(f"pool of {num_blocks} blocks cannot hold {used} blocks")
+    events += [("request", r, int(nb)) for r, nb in enumerate(req_blocks)]
+    return events
+
+
+def tables_from_allocator(events: Sequence[tuple], allocator) -> List[np.ndarray]:
+    """Replay a trace on ``allocator`` (any object with ``allocate(n) -> (ids, n_segments)`` and ``free(ids)``)
+    and return the block table each ("request", r, n) event received.  Bookkeeping only."""
+    held, out = {}, {}
+    for ev in events:
+        if ev[0] == "alloc":
+            held[ev[1]] = np.asarray(allocator.allocate(ev[2])[0], np.int32)
+        elif ev[0] == "free":
+            allocator.free(held.pop(ev[1]))
+        else:
+            out[ev[1]] = np.asarray(allocator.allocate(ev[2])[0], np.int32)
+    return [out[r] for r in sorted(out)]
+
+
 def _tables_from_runs(rng, req_blocks: Sequence[int], num_blocks: int, kind: Tuple) -> List[np.ndarray]:
     """Per-request block tables with the requested run structure, all sharing one pool."""
     if kind[0] == "contiguous":          # request r's blocks follow request r-1's
@@ -193,6 +232,8 @@ def _tables_from_runs(rng, req_blocks: Sequence[int], num_blocks: int, kind: Tup
                 return [t]
     if kind[0] == "trace":
         return _tables_from_trace(rng, req_blocks, num_blocks, kind[1])
+    if kind[0] == "allocator":           # the same trace, ids chosen by a caller-supplied block allocator
+        return tables_from_allocator(alloc_free_trace(rng, req_blocks, num_blocks, kind[1]), kind[2](num_blocks))
     all_runs, owner = [], []
     for r, nb in enumerate(req_blocks):
         runs = runs_geometric(rng, nb, kind[1]) if kind[0] == "geometric" else runs_fixed(nb, kind[1])
@@ -217,7 +258,8 @@ def make_workload(name: str, seed: int, shape: Shape, lengths: Sequence[int],
                   value_dist: str = "normal", src_slack: float = 1.25, dst_slack: float = 1.0625,
                   notes: Optional[dict] = None) -> Workload:
     """Generic builder.  ``*_kind``: ("contiguous",) | ("permutation",) | ("geometric", mean) |
-    ("fixed", run) | ("trace", mean) (seeded alloc/free trace on a FIFO free list).  ``*_blocks`` None => pool sized ``ceil(slack * used)`` (never less than
+    ("fixed", run) | ("trace", mean) (seeded alloc/free trace on a FIFO free list) | ("allocator", mean, factory)
+    (the same trace with the ids chosen by ``factory(num_blocks)``, an object with allocate(n) / free(ids)).  ``*_blocks`` None => pool sized ``ceil(slack * used)`` (never less than
     what separated runs need)."""
     rng = np.random.default_rng(np.random.PCG64(seed))
     lengths = [int(t) for t in lengths]
@@ -231,7 +273,7 @@ def make_workload(name: str, seed: int, shape: Shape, lengths: Sequence[int],
         if kind[0] == "contiguous":
             return max(used, 1)
         # enough for `used` blocks in separated runs: worst case one gap per run
-        if kind[0] == "trace":
+        if kind[0] in ("trace", "allocator"):
             return max(int(np.ceil(slack * used)), 1)
         worst_runs = used if kind[0] != "fixed" else sum(_nblk(n, kind[1]) for n in nb_req)
         return max(int(np.ceil(slack * used)), used + worst_runs, 1)
@@ -311,7 +353,7 @@ def _cfg3_dst_blocks(n: int, used: int) -> int:
 
 
 def config3_batched(budget_bytes: Optional[int] = None, n_requests: Optional[int] = None,
-                    num_layers: Optional[int] = None) -> Workload:
+                    num_layers: Optional[int] = None, allocator=None) -> Workload:
     """BASELINE.json configs[2]: 64 requests, lognormal lengths (median 8k, clip 1k-32k), src tables from a
     seeded alloc/free trace that leaves runs of mean 2 (break probability 1/2), dst runs of mean 16, one batch.  The literal config needs
     ~201 GiB; ``budget_bytes`` keeps the largest seeded prefix of requests that fits (fit rule)."""
@@ -322,6 +364,15 @@ def config3_batched(budget_bytes: Optional[int] = None, n_requests: Optional[int
         n = min(n, fit_prefix(lengths, shape, 16, 16, budget_bytes, _cfg3_src_blocks, _cfg3_dst_blocks))
     lengths = lengths[:n]
     su = sum(_nblk(t, 16) for t in lengths)
+    if allocator is not None:
+        # the same seeded alloc/free trace, but a block allocator (``allocator(num_blocks)`` ->
+        # object with allocate / free; the library's segment allocator) chooses the ids on BOTH sides
+        w = make_workload("cfg3_batched_8b_allocator", SEED_BASE + 3000, shape, lengths,
+                          "lkbthd", 16, ("allocator", 2.0, allocator), _cfg3_src_blocks(n, su),
+                          "lkbthd", 16, ("allocator", 16.0, allocator), _cfg3_dst_blocks(n, su))
+        runs = sum(n_runs(r.src_blocks) for r in w.requests)
+        w.notes.update(n_requests=n, of_requests=64, mean_src_run=su / max(runs, 1))
+        return w
     for attempt in range(8):   # accept iff the generated mean src run is in [1.9, 2.1]
         w = make_workload("cfg3_batched_8b", SEED_BASE + 3000 + attempt, shape, lengths,
                           "lkbthd", 16, ("trace", 2.0), _cfg3_src_blocks(n, su),

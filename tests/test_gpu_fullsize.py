@@ -72,8 +72,37 @@ def _lkbthd_all_planes_property(w, dp):
     mask[ds] = False
     rest = torch.nonzero(mask).flatten()
     sent = torch.tensor(P.SENTINEL_BYTE * 257, dtype=torch.int32).to(torch.int16).item()
-    for p in range(0, 2 * L, 7):
+    for p in range(2 * L):
         assert bool((d[p].index_select(0, rest) == sent).all()), f"plane {p}: an untouched slot changed"
+
+
+def _sampled_layers(L, seed):
+    """First, last and two seeded layers in between (>= 4 layers per config against the oracle)."""
+    rng = np.random.default_rng(seed)
+    mid = rng.choice(np.arange(1, L - 1), size=2, replace=False)
+    return sorted({0, L - 1, int(mid[0]), int(mid[1])})
+
+
+def _device_tables(w):
+    """Padded block tables + lengths on the device, as flowkv_transfer_tables takes them."""
+    n = len(w.requests)
+    max_t = max(r.num_tokens for r in w.requests)
+    ws, wd = -(-max_t // w.src.block_size) + 2, -(-max_t // w.dst.block_size) + 1
+    hs, hd = np.full((n, ws), -1, np.int32), np.full((n, wd), -1, np.int32)
+    for i, r in enumerate(w.requests):
+        hs[i, :len(r.src_blocks)], hd[i, :len(r.dst_blocks)] = r.src_blocks, r.dst_blocks
+    lens = torch.tensor([r.num_tokens for r in w.requests], dtype=torch.int32, device="cuda")
+    return torch.from_numpy(hs).cuda(), torch.from_numpy(hd).cuda(), lens, ws, wd, max_t + 5
+
+
+def _run_tables(w, dp):
+    st, dt, lens, ws, wd, max_t = _device_tables(w)
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    n0 = F.flowkv_launch_count()
+    F.flowkv_transfer_tables(dp.src, dp.dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), len(w.requests), ws, wd, max_t,
+                             flag.data_ptr())
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1 and int(flag.item()) == 0
 
 
 def test_cfg2_full_size():
@@ -87,7 +116,7 @@ def test_cfg2_full_size():
     torch.cuda.synchronize()
     assert F.flowkv_launch_count() - n0 == 1
     assert plan.stats["payload_bytes"] == 1_744_830_464
-    for layer in (0, 13, 31):           # 31: byte offsets beyond 31 GiB
+    for layer in _sampled_layers(32, 2):           # layer 31: byte offsets beyond 31 GiB
         _lkbthd_layer_check(w, dp, layer)
     _lkbthd_all_planes_property(w, dp)
     # bulk (TMA) variant at full size, same bytes
@@ -156,46 +185,52 @@ def test_cfg2_full_size_table_driven():
                              r.num_tokens + 3, flag.data_ptr())
     torch.cuda.synchronize()
     assert F.flowkv_launch_count() - n0 == 1 and int(flag.item()) == 0
-    for layer in (0, 31):
+    for layer in _sampled_layers(32, 5):
         _lkbthd_layer_check(w, dp, layer)
     _lkbthd_all_planes_property(w, dp)
 
 
 def test_cfg3_full_size_fit_rule():
-    """configs[2] scaled to fit HBM by the seeded-prefix rule, one batch, one launch."""
+    """configs[2] scaled to fit HBM by the seeded-prefix rule, one batch, one launch — planned
+    (register path), planned with the TMA variant, and table-driven (device-resident tables, the multi-request
+    q_per_req padding: tiles past a request's end exit).  Each: four layers against the oracle over the whole dst
+    layer slab, every plane through the gather property, untouched slots of every plane still sentinel."""
     free_b, _ = torch.cuda.mem_get_info()
     w = synth.config3_batched(budget_bytes=int(0.85 * free_b))
     if w.notes["n_requests"] < 8:
         pytest.skip("not enough HBM")
     dp = P.DevicePools(w)
+    layers = _sampled_layers(w.shape.num_layers, 3)
     n0 = F.flowkv_launch_count()
     plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS)
     plan.transfer()
     torch.cuda.synchronize()
     assert F.flowkv_launch_count() - n0 == 1
-    _lkbthd_layer_check(w, dp, w.shape.num_layers - 1)
+    for layer in layers:
+        _lkbthd_layer_check(w, dp, layer)
+    _lkbthd_all_planes_property(w, dp)
+    plan.destroy()
+    P.fill_sentinel(dp.dst_buf)
+    _run_tables(w, dp)
+    for layer in layers:
+        _lkbthd_layer_check(w, dp, layer)
+    _lkbthd_all_planes_property(w, dp)
+    P.fill_sentinel(dp.dst_buf)
+    bulk = dp.plan(0, {"variant": "bulk"})
+    assert bulk.stats["variant"] == F.FLOWKV_VARIANT_BULK
+    bulk.transfer()
+    torch.cuda.synchronize()
+    _lkbthd_layer_check(w, dp, layers[-1])
     _lkbthd_all_planes_property(w, dp)
 
 
-def test_cfg4_full_size_fit_rule():
-    """configs[3] scaled to fit: 80 layers, src BS16 LKBTHD -> dst BS64 BLKHTD; one sampled layer against the oracle
-    over the whole dst layer (all blocks), every plane through the gather property."""
-    free_b, _ = torch.cuda.mem_get_info()
-    w = synth.config4_hetero(budget_bytes=int(0.85 * free_b))
-    if w.notes["n_requests"] < 2:
-        pytest.skip("not enough HBM")
-    dp = P.DevicePools(w)
-    n0 = F.flowkv_launch_count()
-    plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS)
-    plan.transfer()
-    torch.cuda.synchronize()
-    assert F.flowkv_launch_count() - n0 == 1
+def _cfg4_check(w, dp, layers):
     L, H, D, e = w.shape.num_layers, w.shape.num_kv_heads, w.shape.head_dim, 2
     gs = G.geom(w.src, w.shape)
     NBd, BSd = w.dst.num_blocks, w.dst.block_size
     layer_bytes = 2 * H * BSd * D * e                     # one layer of one BLKHTD block
     dview = dp.dst_buf.view(NBd, L, layer_bytes)
-    for layer in (L - 1,):
+    for layer in layers:
         src_slab = dp.src_buf[layer * gs.s_layer:(layer + 1) * gs.s_layer].cpu().numpy()
         got = dview[:, layer].contiguous().cpu().numpy().reshape(-1)
         # the dst layer slab as a pool of its own: same in-block strides, block stride = one layer
@@ -205,16 +240,46 @@ def test_cfg4_full_size_fit_rule():
         for r in w.requests:
             O.transfer(src_slab, gs, exp, gd, r.src_blocks, r.dst_blocks, r.num_tokens, layer, layer + 1, layer, layer)
         G.assert_same(got, exp, f"cfg4 layer {layer}")
-    # property on every plane: src token rows == dst token rows (dst viewed [block][layer][kv][head][token][dim])
+    # property on every plane: src token rows == dst token rows (dst viewed [block][layer][kv][head][token][dim]);
+    # token slots of dst blocks no request names (tails of partial 64-token blocks) still hold the sentinel
     s = dp.src_buf.view(torch.int16).view(2 * L, w.src.num_blocks * 16, H, D)
     d6 = dp.dst_buf.view(torch.int16).view(NBd, L, 2, H, BSd, D)
     ss, ds = _slots(w, "src"), _slots(w, "dst")
     db, dt = ds // BSd, ds % BSd
-    for layer in range(0, L, 9):
+    mask = torch.ones(NBd * BSd, dtype=torch.bool, device="cuda")
+    mask[ds] = False
+    rest = torch.nonzero(mask).flatten()
+    rb, rt = rest // BSd, rest % BSd
+    sent = torch.tensor(P.SENTINEL_BYTE * 257, dtype=torch.int32).to(torch.int16).item()
+    for layer in range(L):
         for c in range(2):
             a = s[2 * layer + c].index_select(0, ss)                    # [tok, H, D]
             b = d6[db, layer, c, :, dt, :]                              # [tok, H, D]
             assert torch.equal(a, b), f"layer {layer} kv {c}"
+            if rest.numel():
+                assert bool((d6[rb, layer, c, :, rt, :] == sent).all()), f"layer {layer} kv {c}: an untouched slot changed"
+
+
+def test_cfg4_full_size_fit_rule():
+    """configs[3] scaled to fit: 80 layers, src BS16 LKBTHD -> dst BS64 BLKHTD; planned and table-driven.  Each: four
+    layers against the oracle over the whole dst layer (all blocks), every plane of every layer through the gather
+    property and the untouched-slot sentinel check."""
+    free_b, _ = torch.cuda.mem_get_info()
+    w = synth.config4_hetero(budget_bytes=int(0.85 * free_b))
+    if w.notes["n_requests"] < 2:
+        pytest.skip("not enough HBM")
+    dp = P.DevicePools(w)
+    layers = _sampled_layers(w.shape.num_layers, 4)
+    n0 = F.flowkv_launch_count()
+    plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS)
+    plan.transfer()
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1
+    _cfg4_check(w, dp, layers)
+    plan.destroy()
+    P.fill_sentinel(dp.dst_buf)
+    _run_tables(w, dp)
+    _cfg4_check(w, dp, layers)
 
 
 def test_cfg5_largest_sweep_point_full_size():

@@ -15,21 +15,22 @@ pytestmark = pytest.mark.gpu
 import os
 
 LAYOUTS = ["lkbthd", "blkhtd", "blkthd", "padded"]
+ELEM_BYTES = [2, 1, 2, 4]
 # FLOWKV_FUZZ_OFFSET shifts the case indices (a soak run: FLOWKV_FUZZ_OFFSET=400 FLOWKV_FUZZ_CASES=4000 pytest ...)
 FUZZ_OFFSET = int(os.environ.get("FLOWKV_FUZZ_OFFSET", "0"))
 FUZZ_CASES = int(os.environ.get("FLOWKV_FUZZ_CASES", "400"))
 
 
-def _geom(rng, layout, L, H, D, NB, BS):
+def _geom(rng, layout, L, H, D, NB, BS, e=2):
     """-> (oracle geometry, strides or None).  'padded' = token-major interior with padding after every block,
     K|V slab and layer (a STRIDED pool: separate allocations / alignment padding)."""
     if layout != "padded":
-        return getattr(O.PoolGeom, layout)(L, H, D, 2, NB, BS), None
-    row, tok = D * 2, H * D * 2
+        return getattr(O.PoolGeom, layout)(L, H, D, e, NB, BS), None
+    row, tok = D * e, H * D * e
     blk = BS * tok + 32 * int(rng.integers(0, 5))
     kv = NB * blk + 32 * int(rng.integers(0, 9))
     lay = 2 * kv + 32 * int(rng.integers(0, 3))
-    return O.PoolGeom(L, H, D, 2, NB, BS, lay, kv, blk, tok, row), [lay, kv, blk, tok, row]
+    return O.PoolGeom(L, H, D, e, NB, BS, lay, kv, blk, tok, row), [lay, kv, blk, tok, row]
 
 
 def _table(rng, n, NB, p_cont):
@@ -50,7 +51,8 @@ def _case(idx):
     rng = np.random.default_rng(9000 + idx)
     L = int(rng.integers(1, 5))
     H = int(rng.choice([1, 2, 3, 4, 8]))
-    D = int(rng.choice([8, 16, 24, 64, 128]))
+    e = ELEM_BYTES[idx % 4]                        # half the cases 2-byte, a quarter fp8 (1), a quarter fp32 (4)
+    D = int(rng.choice([16, 32, 48, 128, 256])) // e          # rows of 16 .. 256 bytes at every element size
     bs_s, bs_d = int(2 ** rng.integers(0, 6)), int(2 ** rng.integers(0, 6))
     lay_s, lay_d = str(rng.choice(LAYOUTS)), str(rng.choice(LAYOUTS))
     if rng.random() < 0.35:                       # favour the congruent pairs that take the flat path
@@ -90,24 +92,24 @@ def _case(idx):
     if rng.random() < 0.5:
         tuning["plan_in_params"] = 1
     op = str(rng.choice(["transfer", "layers", "pack_unpack", "windows"]))
-    return rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op
+    return rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op
 
 
 @pytest.mark.parametrize("idx", range(FUZZ_OFFSET, FUZZ_OFFSET + FUZZ_CASES))
 def test_fuzz_against_oracle(idx):
-    rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op = _case(idx)
-    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
-    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d)
+    rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op = _case(idx)
+    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s, e)
+    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d, e)
     src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
     P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
     P.fill_sentinel(dst_buf)
     src_np = P.to_numpy(src_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs_s, "strided" if ss else lay_s, ss)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs_d, "strided" if sd else lay_d, sd)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd)
     freqs = [F.Request(t, a, b) for t, a, b in reqs]
     total = sum(t for t, _, _ in reqs)
-    tokb = H * D * 2
-    what = f"case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} T={[t for t, _, _ in reqs]} {tuning} {op}"
+    tokb = H * D * e
+    what = f"case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} e{e} T={[t for t, _, _ in reqs]} {tuning} {op}"
     plan = F.flowkv_plan(src, dst, freqs, F.FLOWKV_CHECK_DST_ALIAS, tuning or None)
 
     def expect_transfer(l0=0, l1=L):
@@ -182,29 +184,38 @@ def _device_tables(reqs, width_s, width_d):
 def test_fuzz_table_driven_transfer(idx):
     """flowkv_transfer_tables: the kernel walks device-resident padded block tables itself (no plan) — same seeded
     cases as above, whole dst pool against the oracle, one launch, error flag stays clear."""
-    rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
-    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
-    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d)
+    rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
+    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s, e)
+    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d, e)
     src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
     P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
     P.fill_sentinel(dst_buf)
     src_np = P.to_numpy(src_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs_s, "strided" if ss else lay_s, ss)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs_d, "strided" if sd else lay_d, sd)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd)
     max_t = max(t for t, _, _ in reqs) + int(rng.integers(0, 40))
     ws, wd = -(-max_t // bs_s) + int(rng.integers(0, 3)), -(-max_t // bs_d) + int(rng.integers(0, 3))
     st, dt, lens = _device_tables(reqs, max(ws, 1), max(wd, 1))
     flag = torch.zeros(1, dtype=torch.int32, device="cuda")
     tn = {k: v for k, v in tuning.items() if k in ("threads", "group_threads", "max_sms", "ctas_per_sm")}
+    if idx % 5 == 0:                        # narrow CTAs with the group left on auto (must clamp, not divide by zero)
+        tn = {"threads": 32 if idx % 10 == 0 else 64}
     n0 = F.flowkv_launch_count()
-    F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), len(reqs), st.shape[1], dt.shape[1],
-                             max_t, flag.data_ptr(), tn or None)
+    l0, l1 = 0, L
+    if idx % 3 == 1:                        # layer-range form: one launch per range, the other layers stay untouched
+        l0 = int(rng.integers(0, L + 1))
+        l1 = int(rng.integers(l0, L + 1))
+        F.flowkv_transfer_tables_layers(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), len(reqs), st.shape[1],
+                                        dt.shape[1], max_t, l0, l1, flag.data_ptr(), tn or None)
+    else:
+        F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), len(reqs), st.shape[1], dt.shape[1],
+                                 max_t, flag.data_ptr(), tn or None)
     torch.cuda.synchronize()
-    assert F.flowkv_launch_count() - n0 == (1 if max_t else 0)
+    assert F.flowkv_launch_count() - n0 == (1 if max_t and l1 > l0 else 0)
     exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)
     for t, a, b in reqs:
-        O.transfer(src_np, gs, exp, gd, a, b, t)
-    what = f"tables case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} T={[t for t, _, _ in reqs]} {tn}"
+        O.transfer(src_np, gs, exp, gd, a, b, t, l0, l1)
+    what = f"tables case {idx} layers [{l0},{l1}): {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} e{e} T={[t for t, _, _ in reqs]} {tn}"
     G.assert_same(P.to_numpy(dst_buf), exp, what)
     assert int(flag.item()) == 0, what
     G.assert_same(P.to_numpy(src_buf), src_np, what + " (src unchanged)")
@@ -215,24 +226,26 @@ def test_fuzz_table_driven_pack_unpack_windows(idx):
     """flowkv_pack_tables / flowkv_unpack_tables: device-resident tables and cumulative lengths, layer windows split
     at a random layer; each window == the oracle's okv_pack_window, unpacking them rebuilds the oracle's transfer;
     a window buffer that is too small raises flag bit 2 and is left untouched."""
-    rng, (L, H, D), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
-    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s)
-    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d)
+    rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
+    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s, e)
+    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d, e)
     src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
     P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
     P.fill_sentinel(dst_buf)
     src_np = P.to_numpy(src_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs_s, "strided" if ss else lay_s, ss)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs_d, "strided" if sd else lay_d, sd)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd)
     Ts = [t for t, _, _ in reqs]
     total, max_t = sum(Ts), max(Ts) + int(rng.integers(0, 9))
     st, dt, _ = _device_tables(reqs, max(1, -(-max_t // bs_s)), max(1, -(-max_t // bs_d)))
     cu = torch.from_numpy(np.concatenate([[0], np.cumsum(Ts)]).astype(np.int64)).cuda()
     flag = torch.zeros(1, dtype=torch.int32, device="cuda")
     tn = {k: v for k, v in tuning.items() if k in ("threads", "group_threads", "max_sms", "ctas_per_sm")} or None
-    tokb = H * D * 2
+    if idx % 5 == 0:
+        tn = {"threads": 32 if idx % 10 == 0 else 64}
+    tokb = H * D * e
     cut = int(rng.integers(0, L + 1))
-    what = f"tables windows case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} T={Ts} cut={cut} {tn}"
+    what = f"tables windows case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} e{e} T={Ts} cut={cut} {tn}"
     for w0, w1 in ((0, cut), (cut, L)):
         nb = total * 2 * (w1 - w0) * tokb
         win = P.alloc_bytes(nb + 32)

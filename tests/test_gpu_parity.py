@@ -777,3 +777,144 @@ def test_table_driven_transfer_graph_replay_and_error_flag():
     with pytest.raises(F.FlowKVError) as ei:
         F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), n_req, ws - 1, wd, max_t)
     assert ei.value.status == F.FLOWKV_ERR_TABLE_LEN
+
+
+# ---------------------------------------------------------------------------------------------------------
+# round 2: element sizes other than 2 bytes, table-driven layer ranges, the allocator wired through to bytes
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,dim", [("fp8", 128), ("fp32", 64), ("fp8", 16), ("fp32", 12)])
+@pytest.mark.parametrize("pair", [("lkbthd", 16, "lkbthd", 16), ("lkbthd", 16, "blkhtd", 64), ("blkthd", 16, "blkthd", 16)])
+def test_one_and_four_byte_elements_every_operation(dtype, dim, pair):
+    """fp8 KV (Llama-3-8B heads: rows of 128 B, the 256-bit path at 4 vectors per row; and 16-B rows) and fp32:
+    planned transfer, pack / unpack, layer windows and the table-driven kernel against the oracle run with the
+    same elem_bytes (its generic element copy, pinned in tests/test_oracle_pins.py)."""
+    sl, sbs, dl, dbs = pair
+    shape = synth.Shape(3, 8, dim, dtype)
+    assert shape.elem_bytes in (1, 4)
+    w = synth.make_workload(f"{dtype}_{sl}{sbs}_{dl}{dbs}", 777, shape, [333, 0, 1000, 17],
+                            sl, sbs, ("geometric", 3.0), None, dl, dbs, ("geometric", 8.0), None)
+    dp, plan, exp = G.run_transfer_and_check(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    nbytes = plan.stats["staging_bytes"]
+    assert nbytes == w.total_tokens * 2 * 3 * 8 * dim * shape.elem_bytes
+    staging = P.alloc_bytes(nbytes)
+    P.fill_sentinel(dp.dst_buf)
+    plan.pack(staging.data_ptr(), nbytes)
+    plan.unpack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(staging), G.oracle_pack(w, src_np), "wire bytes")
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "unpack")
+    wb = F.flowkv_window_bytes(plan, 1, 3)
+    win = P.alloc_bytes(wb)
+    F.flowkv_pack_window(plan, win.data_ptr(), wb, 1, 3)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(win), G.oracle_pack_window(w, src_np, 1, 3), "window [1,3)")
+    # table-driven, same bytes
+    P.fill_sentinel(dp.dst_buf)
+    st, dt, lens, ws, wd, max_t = _padded_tables(w)
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    F.flowkv_transfer_tables(dp.src, dp.dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), len(w.requests), ws, wd, max_t,
+                             flag.data_ptr())
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "table-driven")
+    assert int(flag.item()) == 0
+
+
+def _padded_tables(w):
+    n = len(w.requests)
+    max_t = max(r.num_tokens for r in w.requests)
+    ws, wd = max(1, -(-max_t // w.src.block_size)), max(1, -(-max_t // w.dst.block_size))
+    hs, hd = np.full((n, ws), -3, np.int32), np.full((n, wd), -3, np.int32)
+    for i, r in enumerate(w.requests):
+        hs[i, :len(r.src_blocks)], hd[i, :len(r.dst_blocks)] = r.src_blocks, r.dst_blocks
+    lens = torch.tensor([r.num_tokens for r in w.requests], dtype=torch.int32, device="cuda")
+    return torch.from_numpy(hs).cuda(), torch.from_numpy(hd).cuda(), lens, ws, wd, max_t
+
+
+def test_table_driven_layer_ranges_parity_and_one_graph_of_layerwise_launches():
+    """flowkv_transfer_tables_layers: (i) each range alone == the oracle's layer-range loop, other layers keep the
+    sentinel, one launch per range, zero for an empty one; (ii) a layer-wise sender — one launch per layer — captured
+    ONCE in a CUDA graph and replayed while the device tables change, whole pool against the oracle each time."""
+    shape = synth.Shape(5, 2, 64, "fp16")
+    L = shape.num_layers
+    w = synth.make_workload("tables_layers", 4242, shape, [150, 31, 0, 64], "lkbthd", 16, ("geometric", 2.0), None,
+                            "blkhtd", 32, ("geometric", 4.0), None)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    gs, gd = G.geom(w.src, shape), G.geom(w.dst, shape)
+    st, dt, lens, ws, wd, max_t = _padded_tables(w)
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    n = len(w.requests)
+    for l0, l1 in [(0, 1), (1, 4), (4, 5), (0, 5), (2, 2)]:
+        P.fill_sentinel(dp.dst_buf)
+        n0 = F.flowkv_launch_count()
+        F.flowkv_transfer_tables_layers(dp.src, dp.dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), n, ws, wd, max_t, l0, l1,
+                                        flag.data_ptr())
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if l1 > l0 else 0)
+        exp = np.full(w.dst.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+        for r in w.requests:
+            O.transfer(src_np, gs, exp, gd, r.src_blocks, r.dst_blocks, r.num_tokens, l0, l1)
+        G.assert_same(P.to_numpy(dp.dst_buf), exp, f"table-driven layers [{l0},{l1})")
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_transfer_tables_layers(dp.src, dp.dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), n, ws, wd, max_t, 3, L + 1)
+    assert ei.value.status == F.FLOWKV_ERR_INVALID_ARG
+    # (ii) layer-wise sender inside one captured graph
+    stream = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=stream):
+        for layer in range(L):
+            F.flowkv_transfer_tables_layers(dp.src, dp.dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), n, ws, wd, max_t,
+                                            layer, layer + 1, flag.data_ptr(), None, torch.cuda.current_stream().cuda_stream)
+    rng = np.random.default_rng(7)
+    for it in range(3):
+        Ts = [int(rng.integers(0, max_t + 1)) for _ in range(n)]
+        sperm = rng.permutation(w.src.num_blocks).astype(np.int32)
+        dperm = rng.permutation(w.dst.num_blocks).astype(np.int32)
+        hs, hd = np.full((n, ws), -1, np.int32), np.full((n, wd), -1, np.int32)
+        reqs, so, do = [], 0, 0
+        for i, t in enumerate(Ts):
+            a, b = sperm[so:so + -(-t // 16)], dperm[do:do + -(-t // 32)]
+            so, do = so + len(a), do + len(b)
+            hs[i, :len(a)], hd[i, :len(b)] = a, b
+            reqs.append((t, a, b))
+        st.copy_(torch.from_numpy(hs)); dt.copy_(torch.from_numpy(hd)); lens.copy_(torch.tensor(Ts, dtype=torch.int32))
+        P.fill_sentinel(dp.dst_buf)
+        torch.cuda.synchronize()
+        n0 = F.flowkv_launch_count()
+        g.replay()
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() == n0          # replays launch from the graph, not through the library
+        exp = np.full(w.dst.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+        for t, a, b in reqs:
+            O.transfer(src_np, gs, exp, gd, a, b, t)
+        G.assert_same(P.to_numpy(dp.dst_buf), exp, f"layer-wise graph replay {it}")
+        assert int(flag.item()) == 0
+
+
+def test_segment_allocator_tables_through_plan_and_transfer():
+    """S§8f NEXT-1 end to end (P:L105 -> P:L107 -> the copy): a seeded alloc/free churn runs through flowkv_alloc_* for
+    BOTH pools, the tables it hands out go into flowkv_plan + flowkv_transfer, the bytes are the oracle's, the segment
+    count is okv_align's, and the product allocator handed out exactly what the oracle allocator does."""
+    from oracle.allocator_oracle import OracleAllocator
+
+    class OA:
+        def __init__(self, nb):
+            self.a = OracleAllocator(nb)
+
+        def allocate(self, k):
+            return self.a.allocate(k)
+
+        def free(self, ids):
+            self.a.release([int(i) for i in ids])
+
+    w = synth.config3_batched(n_requests=5, num_layers=2, allocator=F.Allocator)
+    wo = synth.config3_batched(n_requests=5, num_layers=2, allocator=OA)
+    for a, b in zip(w.requests, wo.requests):
+        assert np.array_equal(a.src_blocks, b.src_blocks) and np.array_equal(a.dst_blocks, b.dst_blocks)
+    fifo = synth.config3_batched(n_requests=5, num_layers=2)
+    dp, plan, _ = G.run_transfer_and_check(w)
+    n_seg = sum(O.count_segments(r.src_blocks, 16, r.dst_blocks, 16, r.num_tokens) for r in w.requests)
+    assert plan.stats["n_segments"] == n_seg
+    fifo_seg = sum(O.count_segments(r.src_blocks, 16, r.dst_blocks, 16, r.num_tokens) for r in fifo.requests)
+    assert n_seg * 3 < fifo_seg, (n_seg, fifo_seg)        # the allocator's point: far fewer, longer segments

@@ -334,3 +334,17 @@ def test_header_is_plain_c_and_the_library_links_from_c(tmp_path):
     assert out.returncode == 0, out.stderr
     got = [tuple(int(x) for x in line.split()) for line in out.stdout.strip().splitlines()]
     assert got == [(0, 48, 5, 0), (48, 32, 20, 3), (80, 16, 9, 5), (96, 24, 3, 6)]
+
+
+def test_bulk_variant_falls_back_when_two_ring_slots_cannot_fit_shared_memory():
+    """in span mode a chunk is at least one token's plane bytes; a token of 128 KiB needs ring slots that
+    do not fit 227 KB twice.  The plan must not promise a TMA launch it cannot make: it runs the register path and
+    says so in stats.variant (all validation happens in flowkv_plan)."""
+    big = F.make_pool(FAKE, 1, 64, 1024, 2, 8, 1, "lkbthd")          # tok_bytes = 64*1024*2 = 128 KiB
+    p = F.flowkv_plan_host(big, big, [F.Request(2, np.array([0, 1], np.int32), np.array([2, 3], np.int32))], 0,
+                           {"variant": "bulk"})
+    assert p.stats["variant"] == F.FLOWKV_VARIANT_LDST
+    small = F.make_pool(FAKE, 1, 8, 128, 2, 8, 16, "lkbthd")
+    q = F.flowkv_plan_host(small, small, [F.Request(16, np.array([0], np.int32), np.array([1], np.int32))], 0,
+                           {"variant": "bulk"})
+    assert q.stats["variant"] == F.FLOWKV_VARIANT_BULK and q.stats["smem_bytes"] <= 227 * 1024
