@@ -36,7 +36,7 @@ class ClockSampler:
     REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
                0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
 
-    def __init__(self, device_index: int, period_s: float = 0.01):
+    def __init__(self, device_index: int, period_s: float = 0.001):
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()
         self._thr = None
@@ -68,24 +68,33 @@ class ClockSampler:
                     pass
         return 0
 
+    def sample(self):
+        if self.h is None:
+            return
+        try:
+            self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+            bits = self._reasons_now()
+            for b, name in self.REASONS.items():
+                if bits & b:
+                    self.reasons.add(name)
+        except Exception:
+            pass
+
     def _run(self):
         while not self._stop.is_set():
-            try:
-                self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
-                bits = self._reasons_now()
-                for b, name in self.REASONS.items():
-                    if bits & b:
-                        self.reasons.add(name)
-            except Exception:
-                pass
+            self.sample()
             self._stop.wait(self.period)
 
     def start(self):
+        """One sample now (the GPU is already under load: call after the warm-up steps have been queued), then one
+        per millisecond until stop(); stop() takes a last one, so even a 10 ms timed region is covered."""
+        self.sample()
         if self.h is not None:
             self._thr = threading.Thread(target=self._run, daemon=True)
             self._thr.start()
 
     def stop(self) -> dict:
+        self.sample()
         self._stop.set()
         if self._thr:
             self._thr.join()
@@ -262,61 +271,65 @@ def run_reference(args) -> None:
 # ---------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------
-def run_ours(args) -> None:
+def host_info(device_index: int) -> dict:
+    """What SURVEY §8d asks to state beside the numbers: the host CPU model behind `cpu_baseline.cores` and the PCIe
+    link the pinned-host route runs over (generation and width as NVML reports them, current / maximum)."""
+    info = {"cpu_model": None, "host_cores": os.cpu_count()}
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                info["cpu_model"] = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    try:
+        import pynvml
+        import torch
+        pynvml.nvmlInit()
+        uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+        h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid if not uuid.startswith("GPU-") else uuid).encode())
+        info["pcie"] = {"gen_current": int(pynvml.nvmlDeviceGetCurrPcieLinkGeneration(h)),
+                        "gen_max": int(pynvml.nvmlDeviceGetMaxPcieLinkGeneration(h)),
+                        "width_current": int(pynvml.nvmlDeviceGetCurrPcieLinkWidth(h)),
+                        "width_max": int(pynvml.nvmlDeviceGetMaxPcieLinkWidth(h))}
+    except Exception as e:  # pragma: no cover
+        info["pcie"] = {"error": repr(e)}
+    return info
+
+
+def device_tables_of(w, device):
+    """Padded block tables + lengths resident on the device, as flowkv_transfer_tables takes them."""
     import torch
-    import torch.distributed as dist
-    from paper_2504_03775_b200 import build as B
-    B.build()
-    from paper_2504_03775_b200 import flowkv as F
-    from paper_2504_03775_b200 import pools as P
-    from paper_2504_03775_b200 import shard
+    n_rq = len(w.requests)
+    max_t = max((r.num_tokens for r in w.requests), default=0)
+    ws_, wd_ = max(1, -(-max_t // w.src.block_size)), max(1, -(-max_t // w.dst.block_size))
+    hs_, hd_ = np.full((n_rq, ws_), -1, np.int32), np.full((n_rq, wd_), -1, np.int32)
+    for i, r in enumerate(w.requests):
+        hs_[i, :len(r.src_blocks)], hd_[i, :len(r.dst_blocks)] = r.src_blocks, r.dst_blocks
+    return (torch.from_numpy(hs_).to(device), torch.from_numpy(hd_).to(device),
+            torch.tensor([r.num_tokens for r in w.requests], dtype=torch.int32, device=device),
+            torch.zeros(1, dtype=torch.int32, device=device), n_rq, ws_, wd_, max_t)
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    free_b, _total = torch.cuda.mem_get_info()
-    w, desc = build_workload(args.config, free_b)
-    tuning = json.loads(args.tuning) if args.tuning else None
-    dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False)
-    payload = w.payload_bytes
-    stream = torch.cuda.current_stream()
+
+def time_steps(F, w, src, dst, requests, K, W, tuning, stream, barrier, local, dev_tables=None, latency_reps=0):
+    """W warm-up steps, then EXACTLY K timed steps of the whole hot path (plan + one kernel + release, or the
+    table-driven launch) bracketed by barrier + synchronize; one CUDA-event pair around every kernel launch, on
+    the launching stream.  Returns a dict of raw measurements (this rank's)."""
+    import torch
     s = stream.cuda_stream
-    K, W = args.steps, args.warmup
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     XFER_ONLY = F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK      # the step moves pool -> pool only
-    dev_tables = None
-    if args.device_tables:           # block tables resident in HBM, read by the kernel: no plan at all
-        n_rq = len(w.requests)
-        max_t = max((r.num_tokens for r in w.requests), default=0)
-        ws_, wd_ = max(1, -(-max_t // w.src.block_size)), max(1, -(-max_t // w.dst.block_size))
-        hs_, hd_ = np.full((n_rq, ws_), -1, np.int32), np.full((n_rq, wd_), -1, np.int32)
-        for i, r in enumerate(w.requests):
-            hs_[i, :len(r.src_blocks)], hd_[i, :len(r.dst_blocks)] = r.src_blocks, r.dst_blocks
-        dev_tables = (torch.from_numpy(hs_).to(dp.device), torch.from_numpy(hd_).to(dp.device),
-                      torch.tensor([r.num_tokens for r in w.requests], dtype=torch.int32, device=dp.device),
-                      torch.zeros(1, dtype=torch.int32, device=dp.device), n_rq, ws_, wd_, max_t)
 
     def step(ev_a=None, ev_b=None):
         if dev_tables is not None:
             st_, dt_, ln_, fl_, n_rq, ws_, wd_, max_t = dev_tables
             if ev_a is not None:
                 ev_a.record(stream)
-            F.flowkv_transfer_tables(dp.src, dp.dst, st_.data_ptr(), dt_.data_ptr(), ln_.data_ptr(), n_rq, ws_, wd_, max_t,
+            F.flowkv_transfer_tables(src, dst, st_.data_ptr(), dt_.data_ptr(), ln_.data_ptr(), n_rq, ws_, wd_, max_t,
                                      fl_.data_ptr(), tuning, s)             # ONE launch, nothing else
             if ev_b is not None:
                 ev_b.record(stream)
             return
-        plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, XFER_ONLY, tuning, s)   # a1-a4 (upload is stream-ordered)
+        plan = F.flowkv_plan(src, dst, requests, XFER_ONLY, tuning, s)   # a1-a4 (upload is stream-ordered)
         if ev_a is not None:
             ev_a.record(stream)
         F.flowkv_transfer(plan, s)                                           # a5: ONE launch
@@ -326,7 +339,7 @@ def run_ours(args) -> None:
 
     for _ in range(max(W, 3)):
         step()
-    plan0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, XFER_ONLY, tuning, s)
+    plan0 = F.flowkv_plan(src, dst, requests, XFER_ONLY, tuning, s)
     stats = plan0.stats
     plan0.destroy()
     ka = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
@@ -334,6 +347,8 @@ def run_ours(args) -> None:
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     clocks = ClockSampler(local)
     barrier()
+    for _ in range(3):                       # the sampler's first sample must see the GPU under this load
+        step()
     clocks.start()
     n0 = F.flowkv_launch_count()
     c0 = F.flowkv_api_call_count()
@@ -345,129 +360,291 @@ def run_ours(args) -> None:
     launches = F.flowkv_launch_count() - n0
     api_calls = F.flowkv_api_call_count() - c0
     clk = clocks.stop()
-    t_ms = e0.elapsed_time(e1)
-    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ka, kb)]))
-    kern_min_ms = float(np.min([a.elapsed_time(b) for a, b in zip(ka, kb)]))
-    t_ms = shard.max_over_ranks(t_ms, device="cuda")                        # max over ranks, device-timed
-    value = world * K * payload / (t_ms * 1e-3) / 1e9
-
-    line = None
-    if rank == 0:
-        peak, peak_src = load_peaks()
-        achieved = 2 * payload / (kern_ms * 1e-3) / 1e9
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
-            "ms_per_step": t_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "u16", "data": "synthetic",
-            "config": {"workload": desc, "name": w.name, "requests": len(w.requests), "tokens": w.total_tokens,
-                       "payload_bytes": payload, "segments": stats["n_segments"],
-                       "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
-                       if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
-                       "step": ("flowkv_transfer_tables per step (device-resident block tables, no plan); pools resident in HBM"
-                                if args.device_tables else
-                                "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM"),
-                       "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
-                                                        "vec_bytes", "cache_hint", "tile_order", "stages")}},
-            "clocks": clk,
-            "gpu_launches": int(launches),
-            "launches_per_batch": launches / K, "cuda_api_calls_per_batch": api_calls / K, "launches_per_request": launches / K / max(len(w.requests), 1),
-            "latency_ms_per_request": t_ms / K / max(len(w.requests), 1),
-            "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": load_traffic(w.name + ("+tables" if args.device_tables else "")), "peak_source": peak_src,
-                         "kernel": "fk_tables_ldst" if args.device_tables else
-                         {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]],
-                         "kernel_ms_avg": kern_ms, "kernel_ms_min": kern_min_ms,
-                         "algorithmic_bytes_per_launch": 2 * payload,
-                         "kernel_share_of_step": kern_ms / (t_ms / K)},
-        }
-
-    # ---- end to end through host memory: pool -> pinned host (flowkv_pack) -> pool (flowkv_unpack) -------------
-    if not args.no_e2e:
-        nbytes = payload
-        host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
-        Ke = max(2, min(args.e2e_steps, K))
-        scratch, scratch_bytes = None, 0
-        if not (args.e2e_serial or args.e2e_direct):
-            p0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
-            scratch_bytes = F.flowkv_via_host_scratch_bytes(p0, args.e2e_chunks)
-            p0.destroy()
-            scratch = P.alloc_bytes(scratch_bytes, device=f"cuda:{local}")
-
-        def e2e_step():
-            plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
-            if args.e2e_serial:
-                F.flowkv_pack(plan, host.data_ptr(), nbytes, s)      # device -> pinned host, one kernel
-                F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)    # pinned host -> device, one kernel
-            else:                                                    # same result, both PCIe directions overlapped
-                F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, args.e2e_chunks, args.e2e_ctas, s,
-                                           scratch.data_ptr() if scratch is not None else 0, scratch_bytes)
-            plan.destroy()
-        e2e_step()
-        barrier()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        for _ in range(Ke):
-            e2e_step()
-        b.record(stream)
-        barrier()
-        te = a.elapsed_time(b)
-        te = shard.max_over_ranks(te, device="cuda")
-        # link reference: one contiguous copy-engine D2H and H2D of the same bytes
-        dev_flat = dp.dst_buf[:nbytes] if dp.dst_buf.numel() >= nbytes else P.alloc_bytes(nbytes)
-        a.record(stream); host.copy_(dev_flat, non_blocking=True); b.record(stream); torch.cuda.synchronize()
-        d2h = nbytes / (a.elapsed_time(b) * 1e-3) / 1e9
-        a.record(stream); dev_flat.copy_(host, non_blocking=True); b.record(stream); torch.cuda.synchronize()
-        h2d = nbytes / (a.elapsed_time(b) * 1e-3) / 1e9
-        if rank == 0:
-            line["e2e"] = {"value": world * Ke * payload / (te * 1e-3) / 1e9, "unit": UNIT,
-                           "h2d_bytes_per_step": nbytes + stats["plan_device_bytes"], "d2h_bytes_per_step": nbytes,
-                           "steps": Ke, "ms_per_step": te / Ke,
-                           "path": ("flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host"
-                                    if args.e2e_serial else
-                                    "flowkv_plan (host tables) + flowkv_transfer_via_host, direct mode: pack kernels store to "
-                                    "pinned host and unpack kernels load from it, pipelined over layer chunks on two streams"
-                                    if args.e2e_direct else
-                                    "flowkv_plan (host tables) + flowkv_transfer_via_host, copy-engine mode: per layer chunk "
-                                    "flowkv_pack_window into device scratch, D2H to pinned host, H2D back, flowkv_unpack_window; "
-                                    "both PCIe directions overlapped on two streams"),
-                           "device_scratch_bytes": scratch_bytes,
-                           "link_memcpy_d2h_GBps": d2h, "link_memcpy_h2d_GBps": h2d}
-        del host
-
-    # ---- comparison baselines on the same pools (outside the timed region) ---------------------------------
-    if rank == 0 and not args.no_baselines:
-        extra = {}
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        if stats["mode_transfer"] in (1, 3) and w.src.block_size == w.dst.block_size:
-            for name, fn in (("blockwise_memcpy", lambda: F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests, s)),):
-                fn(); torch.cuda.synchronize()
-                t0 = time.perf_counter(); a.record(stream); calls = fn(); b.record(stream); torch.cuda.synchronize()
-                extra[name] = {"calls": calls, "device_ms": a.elapsed_time(b), "wall_ms": (time.perf_counter() - t0) * 1e3,
-                               "GBps": payload / (a.elapsed_time(b) * 1e-3) / 1e9}
-            plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)
-            F.flowkv_baseline_segmentwise(plan, s); torch.cuda.synchronize()
-            t0 = time.perf_counter(); a.record(stream); calls = F.flowkv_baseline_segmentwise(plan, s); b.record(stream)
+    per_kernel = [a.elapsed_time(b) for a, b in zip(ka, kb)]
+    out = {"t_ms": e0.elapsed_time(e1), "kern_ms": float(np.mean(per_kernel)), "kern_min_ms": float(np.min(per_kernel)),
+           "launches": int(launches), "api_calls": int(api_calls), "clocks": clk, "stats": stats}
+    if latency_reps:
+        # true request latency: host wall clock from the flowkv_plan call until the stream has drained, one
+        # synchronous request at a time (nothing pipelined, nothing queued behind another batch)
+        lat = []
+        for _ in range(latency_reps):
             torch.cuda.synchronize()
-            extra["segmentwise_memcpy"] = {"calls": calls, "device_ms": a.elapsed_time(b),
-                                           "wall_ms": (time.perf_counter() - t0) * 1e3,
-                                           "GBps": payload / (a.elapsed_time(b) * 1e-3) / 1e9}
-            plan.destroy()
-        flat_a = dp.src_buf[:payload]
-        flat_b = dp.dst_buf[:payload] if dp.dst_buf.numel() >= payload else P.alloc_bytes(payload)
-        ts = []
-        for _ in range(5):
-            a.record(stream); flat_b.copy_(flat_a); b.record(stream); torch.cuda.synchronize(); ts.append(a.elapsed_time(b))
-        extra["contiguous_copy"] = {"calls": 1, "device_ms": min(ts), "GBps": payload / (min(ts) * 1e-3) / 1e9}
-        line["baselines"] = extra
+            t0 = time.perf_counter()
+            if dev_tables is not None:
+                step()
+                plan = None
+            else:
+                plan = F.flowkv_plan(src, dst, requests, XFER_ONLY, tuning, s)
+                F.flowkv_transfer(plan, s)
+            stream.synchronize()
+            lat.append((time.perf_counter() - t0) * 1e3)
+            if plan is not None:
+                plan.destroy()
+        out["latency_ms_call_to_done"] = float(np.median(lat))
+        out["latency_ms_call_to_done_min"] = float(np.min(lat))
+    return out
+
+
+def kernel_name(stats, device_tables: bool) -> str:
+    return "fk_tables_ldst" if device_tables else {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]]
+
+
+def roofline_of(m, payload, w_key, stats, K, device_tables):
+    peak, peak_src = load_peaks()
+    achieved = 2 * payload / (m["kern_ms"] * 1e-3) / 1e9
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": load_traffic(w_key), "peak_source": peak_src, "kernel": kernel_name(stats, device_tables),
+            "kernel_ms_avg": m["kern_ms"], "kernel_ms_min": m["kern_min_ms"], "algorithmic_bytes_per_launch": 2 * payload,
+            "kernel_share_of_step": m["kern_ms"] / (m["t_ms"] / K)}
+
+
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+    from paper_2504_03775_b200 import build as B
+    B.build()
+    from paper_2504_03775_b200 import flowkv as F
+    from paper_2504_03775_b200 import pools as P
+    from paper_2504_03775_b200 import shard
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = 0 if args.same_device else int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    assert local < torch.cuda.device_count(), f"rank {rank}: no cuda:{local} on this node (--gpus {args.gpus})"
+    torch.cuda.set_device(local)
+    backend = "gloo" if args.same_device else "nccl"     # ranks sharing one GPU (tests) cannot form an NCCL group
+    reduce_dev = "cpu" if args.same_device else "cuda"
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    tuning = json.loads(args.tuning) if args.tuning else None
+    stream = torch.cuda.current_stream()
+    K, W = args.steps, args.warmup
+
+    def primary():
+        """Everything measured on --config's workload; its pools die with this frame (the batched config that follows
+        sizes its own pools from the free HBM)."""
+        s = stream.cuda_stream
+        free_b, _total = torch.cuda.mem_get_info()
+        if args.same_device:
+            free_b //= world
+        w, desc = build_workload(args.config, free_b)
+        dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False)
+        payload = w.payload_bytes
+        # --peer: rank r's kernel stores into the dst pool that rank (r+1) % N owns, mapped through CUDA IPC — the paper's
+        # single-machine "IPC" mode (P:L90) as a one-sided put; over NVLink when the ranks sit on different GPUs
+        dst_desc, peer_keep = dp.dst, None
+        if args.peer:
+            assert world > 1, "--peer needs at least 2 ranks (torchrun, or bench.py --gpus N)"
+            from paper_2504_03775_b200 import peer
+            handles = [None] * world
+            dist.all_gather_object(handles, peer.export_pool(dp.dst_buf))
+            peer_keep = peer.import_pool(handles[(rank + 1) % world])
+            dst_desc = P.describe(w.dst, w.shape, peer_keep.data_ptr())
+            barrier()
+
+        dev_tables = device_tables_of(w, dp.device) if args.device_tables else None
+        m = time_steps(F, w, dp.src, dst_desc, dp.requests, K, W, tuning, stream, barrier, local, dev_tables,
+                       latency_reps=max(20, args.latency_reps))
+        stats = m["stats"]
+        t_ms = shard.max_over_ranks(m["t_ms"], device=reduce_dev)                   # max over ranks, device-timed
+        value = world * K * payload / (t_ms * 1e-3) / 1e9
+
+        line = None
+        if rank == 0:
+            m["t_ms"] = t_ms
+            wkey = w.name + ("+tables" if args.device_tables else "")
+            line = {
+                "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
+                "ms_per_step": t_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "u16", "data": "synthetic",
+                "config": {"workload": desc, "name": w.name, "requests": len(w.requests), "tokens": w.total_tokens,
+                           "payload_bytes": payload, "segments": stats["n_segments"],
+                           "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
+                           if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
+                           "step": ("flowkv_transfer_tables per step (device-resident block tables, no plan); pools resident in HBM"
+                                    if args.device_tables else
+                                    "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM"),
+                           "dst": ("the NEXT rank's dst pool, mapped through CUDA IPC (one-sided peer put)" if args.peer
+                                   else "this rank's own dst pool"),
+                           "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
+                                                            "vec_bytes", "cache_hint", "tile_order", "stages")}},
+                "clocks": m["clocks"],
+                "gpu_launches": m["launches"],
+                "launches_per_batch": m["launches"] / K, "cuda_api_calls_per_batch": m["api_calls"] / K,
+                "launches_per_request": m["launches"] / K / max(len(w.requests), 1),
+                # throughput view: steps are pipelined (planning batch k+1 overlaps the kernel of batch k)
+                "pipelined_step_ms_per_request": t_ms / K / max(len(w.requests), 1),
+                # latency view: one synchronous request at a time, host wall clock, flowkv_plan call -> stream drained
+                "latency_ms_call_to_done": m["latency_ms_call_to_done"],
+                "latency_ms_call_to_done_min": m["latency_ms_call_to_done_min"],
+                "latency_ms_call_to_done_per_request": m["latency_ms_call_to_done"] / max(len(w.requests), 1),
+                "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
+                "roofline": roofline_of(m, payload, wkey, stats, K, args.device_tables),
+                "host": host_info(local),
+            }
+
+        # ---- end to end through host memory: pool -> pinned host (flowkv_pack) -> pool (flowkv_unpack) -------------
+        if not args.no_e2e:
+            nbytes = payload
+            host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+            Ke = max(2, min(args.e2e_steps, K))
+            scratch, scratch_bytes = None, 0
+            if not (args.e2e_serial or args.e2e_direct):
+                p0 = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                scratch_bytes = F.flowkv_via_host_scratch_bytes(p0, args.e2e_chunks)
+                p0.destroy()
+                scratch = P.alloc_bytes(scratch_bytes, device=f"cuda:{local}")
+
+            def e2e_step():
+                plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                if args.e2e_serial:
+                    F.flowkv_pack(plan, host.data_ptr(), nbytes, s)      # device -> pinned host, one kernel
+                    F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)    # pinned host -> device, one kernel
+                else:                                                    # same result, both PCIe directions overlapped
+                    F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, args.e2e_chunks, args.e2e_ctas, s,
+                                               scratch.data_ptr() if scratch is not None else 0, scratch_bytes)
+                plan.destroy()
+            e2e_step()
+            barrier()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(Ke):
+                e2e_step()
+            b.record(stream)
+            barrier()
+            te = a.elapsed_time(b)
+            te = shard.max_over_ranks(te, device=reduce_dev)
+            # link references: one contiguous copy-engine D2H / H2D of the same bytes, alone and both at once
+            dev_flat = dp.dst_buf[:nbytes] if dp.dst_buf.numel() >= nbytes else P.alloc_bytes(nbytes)
+            dev_flat2 = dp.src_buf[:nbytes]                       # read-only leg of the duplex probe
+            host2 = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+            a.record(stream); host.copy_(dev_flat, non_blocking=True); b.record(stream); torch.cuda.synchronize()
+            d2h = nbytes / (a.elapsed_time(b) * 1e-3) / 1e9
+            a.record(stream); dev_flat.copy_(host, non_blocking=True); b.record(stream); torch.cuda.synchronize()
+            h2d = nbytes / (a.elapsed_time(b) * 1e-3) / 1e9
+            side = torch.cuda.Stream()
+            best = None
+            for _ in range(3):                                    # D2H on the side stream + H2D on this one, together
+                torch.cuda.synchronize()
+                a.record(stream)
+                side.wait_stream(stream)
+                with torch.cuda.stream(side):
+                    host2.copy_(dev_flat2, non_blocking=True)
+                dev_flat.copy_(host, non_blocking=True)
+                stream.wait_stream(side)
+                b.record(stream)
+                torch.cuda.synchronize()
+                best = a.elapsed_time(b) if best is None else min(best, a.elapsed_time(b))
+            duplex = nbytes / (best * 1e-3) / 1e9
+            if rank == 0:
+                e2e_val = world * Ke * payload / (te * 1e-3) / 1e9
+                line["e2e"] = {"value": e2e_val, "unit": UNIT,
+                               "h2d_bytes_per_step": nbytes + stats["plan_device_bytes"], "d2h_bytes_per_step": nbytes,
+                               "steps": Ke, "ms_per_step": te / Ke,
+                               "path": ("flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host"
+                                        if args.e2e_serial else
+                                        "flowkv_plan (host tables) + flowkv_transfer_via_host, direct mode: pack kernels store to "
+                                        "pinned host and unpack kernels load from it, pipelined over layer chunks on two streams"
+                                        if args.e2e_direct else
+                                        "flowkv_plan (host tables) + flowkv_transfer_via_host, copy-engine mode: per layer chunk "
+                                        "flowkv_pack_window into device scratch, D2H to pinned host, H2D back, flowkv_unpack_window; "
+                                        "four queues (pack kernels, D2H engine, H2D engine, unpack kernels), both PCIe directions busy"),
+                               "device_scratch_bytes": scratch_bytes,
+                               "link_memcpy_d2h_GBps": d2h, "link_memcpy_h2d_GBps": h2d,
+                               "link_memcpy_duplex_GBps_each_way": duplex,
+                               "frac_of_one_way_link": e2e_val / world / min(d2h, h2d),
+                               "frac_of_duplex_bound": e2e_val / world / duplex}
+            del host, host2
+
+        # ---- comparison baselines on the same pools (outside the timed region) ---------------------------------
+        if rank == 0 and not args.no_baselines and not args.peer:
+            extra = {}
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            if stats["mode_transfer"] in (1, 3) and w.src.block_size == w.dst.block_size:
+                for name, fn in (("blockwise_memcpy", lambda: F.flowkv_baseline_blockwise(dp.src, dp.dst, dp.requests, s)),):
+                    fn(); torch.cuda.synchronize()
+                    t0 = time.perf_counter(); a.record(stream); calls = fn(); b.record(stream); torch.cuda.synchronize()
+                    extra[name] = {"calls": calls, "device_ms": a.elapsed_time(b), "wall_ms": (time.perf_counter() - t0) * 1e3,
+                                   "GBps": payload / (a.elapsed_time(b) * 1e-3) / 1e9}
+                plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, tuning, s)
+                F.flowkv_baseline_segmentwise(plan, s); torch.cuda.synchronize()
+                t0 = time.perf_counter(); a.record(stream); calls = F.flowkv_baseline_segmentwise(plan, s); b.record(stream)
+                torch.cuda.synchronize()
+                extra["segmentwise_memcpy"] = {"calls": calls, "device_ms": a.elapsed_time(b),
+                                               "wall_ms": (time.perf_counter() - t0) * 1e3,
+                                               "GBps": payload / (a.elapsed_time(b) * 1e-3) / 1e9}
+                plan.destroy()
+            flat_a = dp.src_buf[:payload]
+            flat_b = dp.dst_buf[:payload] if dp.dst_buf.numel() >= payload else P.alloc_bytes(payload)
+            ts = []
+            for _ in range(5):
+                a.record(stream); flat_b.copy_(flat_a); b.record(stream); torch.cuda.synchronize(); ts.append(a.elapsed_time(b))
+            extra["contiguous_copy"] = {"calls": 1, "device_ms": min(ts), "GBps": payload / (min(ts) * 1e-3) / 1e9}
+            line["baselines"] = extra
+
+        if rank == 0 and world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w, dp.src_buf)
+        return line
+
+    line = primary()
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+
+    # ---- the batched config (BASELINE.json configs[2]) in the same line: north_star asks for >= 80 % of HBM peak on
+    # "the Llama-3-8B 13k-token AND batched configs".  Same step, same timing rules, its own clock record.
+    if args.config == "cfg2" and not args.no_secondary and not args.peer and not args.same_device:
+        free_b, _ = torch.cuda.mem_get_info()
+        w3, desc3 = build_workload("cfg3", free_b)
+        dp3 = P.DevicePools(w3, device=f"cuda:{local}", sentinel_dst=False)
+        K3 = max(20, min(K, args.secondary_steps))
+        m3 = time_steps(F, w3, dp3.src, dp3.dst, dp3.requests, K3, 3, tuning, stream, barrier, local,
+                        device_tables_of(w3, dp3.device) if args.device_tables else None, latency_reps=5)
+        t3 = shard.max_over_ranks(m3["t_ms"], device=reduce_dev)
+        if rank == 0:
+            m3["t_ms"] = t3
+            p3 = w3.payload_bytes
+            line["secondary"] = {
+                "workload": desc3, "name": w3.name, "requests": len(w3.requests), "tokens": w3.total_tokens,
+                "payload_bytes": p3, "segments": m3["stats"]["n_segments"], "steps": K3,
+                "value": world * K3 * p3 / (t3 * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": t3 / K3,
+                "kernel_ms_avg": m3["kern_ms"], "kernel_ms_min": m3["kern_min_ms"],
+                "pct_of_8TBps_nominal": 100 * 2 * K3 * p3 / (t3 * 1e-3) / 8e12,
+                "pct_of_8TBps_nominal_kernel_only": 100 * 2 * p3 / (m3["kern_ms"] * 1e-3) / 8e12,
+                "roofline": roofline_of(m3, p3, w3.name + ("+tables" if args.device_tables else ""), m3["stats"], K3,
+                                        args.device_tables),
+                "clocks": m3["clocks"], "gpu_launches": m3["launches"], "launches_per_batch": m3["launches"] / K3,
+                "latency_ms_call_to_done": m3["latency_ms_call_to_done"],
+                "latency_ms_call_to_done_per_request": m3["latency_ms_call_to_done"] / max(len(w3.requests), 1)}
+        del dp3
 
     if rank == 0:
-        if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(w, dp.src_buf)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def spawn_ranks(args) -> None:
+    """`python bench.py --gpus N` with N > 1 and no launcher: start the N ranks here, one process per GPU, exactly as
+    the driver does (`python -m torch.distributed.run --nnodes=1 --nproc-per-node N ...`), and become that launcher."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
 
 
 def main() -> None:
@@ -490,7 +667,17 @@ def main() -> None:
     ap.add_argument("--no-baselines", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run the configs[4] sweep instead (see bench_sweep.py)")
+    ap.add_argument("--latency-reps", type=int, default=20, help="synchronous requests behind latency_ms_call_to_done")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the configs[2] (batched) measurement that the "
+                    "default cfg2 run appends under `secondary`")
+    ap.add_argument("--secondary-steps", type=int, default=20)
+    ap.add_argument("--peer", action="store_true", help="rank r stores into rank (r+1)%%N's dst pool through CUDA IPC "
+                    "(one-sided peer put; needs >= 2 ranks)")
+    ap.add_argument("--same-device", action="store_true", help="all ranks on cuda:0 with a gloo control plane (a "
+                    "functional check of the multi-rank path on a one-GPU box; not a scaling number)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)          # does not return
     if args.sweep:
         import bench_sweep
         bench_sweep.main([])

@@ -2,11 +2,17 @@
 """bench_sweep.py — BASELINE.json configs[4]: Llama-3-8B shape, request length 128..131,072 tokens x src run
 length {1, 2, 8, 64, contiguous}, plus the device -> pinned-host pack path at 32,768 tokens.
 
-    python bench_sweep.py [--out gpurun_out/sweep.json] [--reps 20] [--quick]
+    python bench_sweep.py [--out gpurun_out/sweep.json] [--reps 20] [--quick] [--tokens 1024,4096] [--runs 1,0]
+    python bench_sweep.py --tuning-grid [--tokens 128,512,1024,4096]     # A/B grid of launch shapes on the small points
 
-Per point: payload, kernel time (CUDA events, median and min over reps, L2 flushed between reps when
-the payload could stay L2-resident), GB/s, request latency (host call of flowkv_plan -> stream drained),
+Per point: payload, kernel time (CUDA events, mean and min over reps, L2 flushed between reps when
+the payload could stay L2-resident), GB/s, the SAME-SIZE PLAIN COPY under the same conditions (one contiguous
+cudaMemcpyAsync D2D of payload bytes: the honest ceiling at L2-scale sizes) and kernel time as a fraction of it,
+the CUDA-graph replay time of flowkv_transfer, request latency (host call of flowkv_plan -> stream drained),
 kernel launches, segments, and the cudaMemcpyAsync baselines (per block/layer/K|V and per segment/layer/K|V).
+
+L2 flush = a READ pass over a 512 MiB buffer (leaves clean lines; a write pass would leave ~100 MB of dirty lines
+whose write-back the timed kernel then pays for).
 """
 from __future__ import annotations
 
@@ -30,6 +36,10 @@ def main(argv=None) -> None:
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--tuning", default=None)
     ap.add_argument("--no-baselines", action="store_true")
+    ap.add_argument("--tokens", default=None, help="comma-separated request lengths (default: the whole sweep)")
+    ap.add_argument("--runs", default=None, help="comma-separated src run lengths, 0 = contiguous")
+    ap.add_argument("--tuning-grid", action="store_true",
+                    help="time a grid of tile sizes / CTA shapes per point instead of the baselines (launch-shape A/B)")
     args = ap.parse_args(argv)
 
     import torch
@@ -46,12 +56,19 @@ def main(argv=None) -> None:
     tuning = json.loads(args.tuning) if args.tuning else None
     tokens = synth.SWEEP_TOKENS if not args.quick else [128, 4096, 32768]
     runs = synth.SWEEP_RUNS if not args.quick else [1, 0]
+    if args.tokens:
+        tokens = [int(x) for x in args.tokens.split(",")]
+    if args.runs:
+        runs = [int(x) for x in args.runs.split(",")]
+    if args.tuning_grid:
+        args.no_baselines = True
     max_nb = max(tokens) // 16
     src_spec_max = synth.PoolSpec("lkbthd", 16, max(16384, 2 * max_nb))
     src_buf = P.alloc_bytes(src_spec_max.bytes(shape))
     dst_buf = P.alloc_bytes(synth.PoolSpec("lkbthd", 16, max_nb).bytes(shape))
     P.fill_values(src_buf, "normal", "bf16", synth.SEED_BASE + 5000)
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")       # > L2 (126 MB)
+    flush = torch.zeros(512 << 20, dtype=torch.uint8, device="cuda").view(torch.int64)       # > L2 (126 MB)
+    flush_out = torch.zeros(1, dtype=torch.int64, device="cuda")
     ev = lambda: torch.cuda.Event(enable_timing=True)
     rows = []
 
@@ -59,12 +76,13 @@ def main(argv=None) -> None:
         ts = []
         for _ in range(reps):
             if do_flush:
-                flush.zero_()
+                flush.sum()               # read pass: evicts everything, leaves clean lines
             a, b = ev(), ev()
             a.record(stream); fn(); b.record(stream)
             torch.cuda.synchronize()
             ts.append(a.elapsed_time(b))
-        return float(np.median(ts)), float(np.min(ts))
+        # CUDA event timestamps tick every ~1 us; the MEAN over reps dithers below one tick (min is kept beside it)
+        return float(np.mean(ts)), float(np.min(ts))
 
     seen = set()
     for T in tokens:
@@ -92,7 +110,7 @@ def main(argv=None) -> None:
             lat = []
             for _ in range(min(args.reps, 10)):
                 if do_flush:
-                    flush.zero_()
+                    flush.sum()
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
                 p2 = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, tuning, s)
@@ -100,7 +118,45 @@ def main(argv=None) -> None:
                 torch.cuda.synchronize()
                 lat.append((time.perf_counter() - t0) * 1e3)
                 p2.destroy()
+            # the same bytes as ONE contiguous cudaMemcpyAsync D2D, timed the same way (same flush, same events)
+            flat_s, flat_d = src_buf[:payload], dst_buf[:payload]
+            def plain():
+                flat_d.copy_(flat_s, non_blocking=True)       # torch issues one cudaMemcpyAsync D2D for this
+            plain(); torch.cuda.synchronize()
+            pmed, pmn = timed(plain, args.reps, do_flush)
+            # CUDA-graph replay of the same flowkv_transfer launch
+            gstream = torch.cuda.Stream()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=gstream):
+                plan.transfer(torch.cuda.current_stream().cuda_stream)
+            graph.replay(); torch.cuda.synchronize()
+            gmed, gmn = timed(graph.replay, args.reps, do_flush)
+            # back to back: 8 launches of the same transfer in a row, per launch (launch ramps can overlap)
+            def eight():
+                for _ in range(8):
+                    plan.transfer(s)
+            b2b = timed(eight, max(3, args.reps // 4), do_flush)[0] / 8
+            if args.tuning_grid:
+                grid_rows = []
+                for tb in (8192, 16384, 32768, 65536, 131072):
+                    for thr, grp in ((128, 64), (128, 128), (256, 64), (256, 128), (256, 256), (512, 64), (512, 128),
+                                     (512, 256), (512, 512)):
+                        if grp * 32 > tb:               # more threads than 32-byte vectors in a tile: idle lanes
+                            continue
+                        tn = dict(tuning or {}, tile_bytes=tb, threads=thr, group_threads=grp)
+                        p3 = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, tn, s)
+                        p3.transfer(s); torch.cuda.synchronize()
+                        m3, n3 = timed(lambda: p3.transfer(s), args.reps, do_flush)
+                        grid_rows.append({"tile_bytes": tb, "threads": thr, "group_threads": grp, "grid": p3.stats["grid"],
+                                          "kernel_us_med": m3 * 1e3, "kernel_us_min": n3 * 1e3})
+                        p3.destroy()
+                best = min(grid_rows, key=lambda r: r["kernel_us_med"])
+                print(json.dumps({"tokens": T, "run": run or "contig", "default_us": med * 1e3, "plain_copy_us": pmed * 1e3,
+                                  "default_shape": {k: st[k] for k in ("tile_bytes", "threads", "group_threads", "grid")},
+                                  "best": best, "grid": grid_rows}), flush=True)
             row = {"tokens": T, "run": run or "contig", "segments": st["n_segments"], "payload_bytes": payload,
+                   "plain_copy_ms_med": pmed, "plain_copy_ms_min": pmn, "frac_of_plain_copy": pmed / med,
+                   "graph_replay_ms_med": gmed, "back_to_back_ms_per_launch": b2b,
                    "kernel_ms_med": med, "kernel_ms_min": mn, "payload_GBps": payload / (med * 1e-3) / 1e9,
                    "hbm_GBps": 2 * payload / (med * 1e-3) / 1e9, "hbm_GBps_best": 2 * payload / (mn * 1e-3) / 1e9,
                    "latency_ms_plan_to_done": float(np.median(lat)), "launches_per_request": launches,

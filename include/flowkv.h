@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define FLOWKV_VERSION 2
+#define FLOWKV_VERSION 3
 
 #if defined(__GNUC__)
 #define FLOWKV_API __attribute__((visibility("default")))
@@ -249,20 +249,24 @@ FLOWKV_API flowkv_status flowkv_unpack_window(const flowkv_plan_t* plan, const v
 
 /* Pool -> pinned host -> pool with both PCIe directions busy at once (S§8f NEXT-3: chunked pinned-host
  * pipeline; the host buffer stands in for the network endpoint, BASELINE.json north_star).  dst ends up exactly
- * as after flowkv_transfer.  The layers are cut into `n_chunks` groups (0 = 16; clamped to [1, L]); chunk c goes
- * out on `stream` and comes back on a plan-owned second stream as soon as it has landed on the host, so the D2H
- * of chunk c+1 overlaps the H2D of chunk c.  `stream` is made to wait for the last inbound chunk, so callers see
- * ordinary stream order.  Two modes:
+ * as after flowkv_transfer.  The layers are cut into `n_chunks` groups (0 = default; clamped to [1, L]); a chunk
+ * comes back as soon as it has landed on the host, so the outbound leg of chunk c+1 overlaps the inbound leg of
+ * chunk c.  The helper streams and events are library-owned (cached between plans); `stream` is made to wait for
+ * the last inbound chunk, so callers see ordinary stream order.  Two modes:
  *   device_scratch == NULL — direct: the pack / unpack kernels store to / load from host memory themselves (UVA);
- *     no extra device memory.  host_staging holds the wire format of flowkv_pack.  `ctas_per_kernel` caps each
- *     kernel's grid (0 = 64: a PCIe-bound kernel needs few CTAs and both kernels must be co-resident).
- *   device_scratch != NULL — copy engines: chunk c is packed into a scratch slot in HBM (flowkv_pack_window), moved
- *     D2H and H2D by cudaMemcpyAsync, and unpacked from a second slot (flowkv_unpack_window).  On B200 the copy
- *     engines sustain ~50 GB/s in both directions at once where SM loads over PCIe drop to ~38 GB/s.  host_staging
- *     then holds the chunks back to back, chunk c = the layer window [L*c/n, L*(c+1)/n) at byte offset
- *     flowkv_window_bytes(0, L*c/n) (== the wire format when n_chunks == 1).  device_scratch: DEVICE pointer,
- *     256-B aligned, scratch_bytes >= flowkv_via_host_scratch_bytes(plan, n_chunks) (4 slots of the largest
- *     chunk); caller-owned, reusable once `stream` has passed this call.  `ctas_per_kernel`: 0 = the plan's grid.
+ *     no extra device memory.  host_staging holds the wire format of flowkv_pack.  Default 16 chunks.
+ *     `ctas_per_kernel` caps each kernel's grid (0 = 64: a PCIe-bound kernel needs few CTAs and both kernels must
+ *     be co-resident).
+ *   device_scratch != NULL — copy engines, four queues: chunk c is packed into a scratch slot in HBM
+ *     (flowkv_pack_window, on `stream`), moved D2H and H2D by cudaMemcpyAsync on two copy queues of their own, and
+ *     unpacked from a second slot (flowkv_unpack_window, on a fourth queue), so neither engine ever waits behind a
+ *     kernel.  On B200 the copy engines sustain ~50 GB/s in both directions at once where SM loads over PCIe drop
+ *     to ~38 GB/s.  Default 32 chunks (the first outbound and the last inbound chunk cross the link alone).
+ *     host_staging then holds the chunks back to back, chunk c = the layer window [L*c/n, L*(c+1)/n) at byte
+ *     offset flowkv_window_bytes(0, L*c/n) (== the wire format when n_chunks == 1).  device_scratch: DEVICE
+ *     pointer, 256-B aligned, scratch_bytes >= flowkv_via_host_scratch_bytes(plan, n_chunks) (4 slots of the
+ *     largest chunk); caller-owned, reusable once `stream` has passed this call.  `ctas_per_kernel`: 0 = the
+ *     plan's grid.
  * Launches: 2 * (non-empty chunks).  host_staging: pinned HOST pointer (mapped / UVA for the direct mode; a device
  * pointer also works in direct mode), 16-B aligned, bytes >= staging_bytes. */
 FLOWKV_API flowkv_status flowkv_via_host_scratch_bytes(const flowkv_plan_t* plan, uint32_t n_chunks, uint64_t* bytes);

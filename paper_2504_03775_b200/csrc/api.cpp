@@ -162,6 +162,56 @@ cudaError_t upload_stream(int device, cudaStream_t* out, cudaMemPool_t* pool) {
   return cudaSuccess;
 }
 
+// Helper streams and events of flowkv_transfer_via_host.  Created once and recycled between plans (a plan per
+// batch would otherwise pay three cudaStreamCreate and ~100 cudaEventCreate per step).
+struct ViaHostCtx {
+  cudaStream_t q_d2h = nullptr, q_h2d = nullptr, q_unpack = nullptr;
+  std::vector<cudaEvent_t> ev;
+  int device = -1;
+};
+class ViaHostCache {
+ public:
+  ViaHostCtx* acquire(int device) {
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      for (size_t i = 0; i < free_.size(); ++i)
+        if (free_[i]->device == device) {
+          ViaHostCtx* c = free_[i];
+          free_.erase(free_.begin() + i);
+          return c;
+        }
+    }
+    ViaHostCtx* c = new (std::nothrow) ViaHostCtx();
+    if (!c) return nullptr;
+    c->device = device;
+    if (cudaStreamCreateWithFlags(&c->q_d2h, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->q_h2d, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->q_unpack, cudaStreamNonBlocking) != cudaSuccess) {
+      destroy(c);
+      return nullptr;
+    }
+    return c;
+  }
+  void release(ViaHostCtx* c) {
+    if (!c) return;
+    std::lock_guard<std::mutex> lk(mu_);
+    if (free_.size() < 8) { free_.push_back(c); return; }
+    destroy(c);
+  }
+  static void destroy(ViaHostCtx* c) {
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    if (c->q_d2h) cudaStreamDestroy(c->q_d2h);
+    if (c->q_h2d) cudaStreamDestroy(c->q_h2d);
+    if (c->q_unpack) cudaStreamDestroy(c->q_unpack);
+    delete c;
+  }
+
+ private:
+  std::mutex mu_;
+  std::vector<ViaHostCtx*> free_;
+};
+ViaHostCache g_via_host;
+
 struct Op {                  // one runnable operation of a plan
   Schedule sched;
   const Chunk* d_chunks = nullptr;
@@ -187,9 +237,9 @@ struct flowkv_plan_s {
   uint64_t d_bytes = 0;
   cudaStream_t stream = nullptr;   // the stream flowkv_plan() was given: it waits on the upload; the free is ordered on it
   PinnedBuf staging{};             // staging.ev = "upload done" event
-  // flowkv_transfer_via_host: second stream + events, created on first use (plans are logically const)
-  mutable cudaStream_t aux = nullptr;
-  mutable std::vector<cudaEvent_t> events;
+  mutable std::atomic<bool> upload_seen_done{false};   // run(): the upload event has been observed complete
+  // flowkv_transfer_via_host: helper streams + events, taken from a library cache on first use (plans are logically const)
+  mutable ViaHostCtx* via = nullptr;
   int device = -1;
   uint32_t num_sms = 0, max_smem_optin = 0;
 };
@@ -298,6 +348,8 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
   //    (SMs do not all drain HBM at the same rate); beyond the cap each CTA strides over tiles;
   //  * rows mode (strided rows) prefers 128-thread groups: four tiles in flight per CTA.
   ls.threads = t.threads ? t.threads : std::min<uint32_t>(512, std::max<uint32_t>(128, pl->tile_bytes / 128));
+  //  * span / flat mode: the whole CTA shares one tile (round 2 re-checked 256- and 128-thread groups on configs[1]:
+  //    0.5242 / 0.5285 ms against 0.5182 ms — fewer, fatter CTAs lose the fine-grained hardware scheduling).
   const uint32_t group_auto = op.sched.mode == MODE_ROWS ? std::min<uint32_t>(128, ls.threads) : ls.threads;
   ls.group_threads = t.group_threads ? std::min(t.group_threads, ls.threads) : group_auto;
   ls.hint = t.cache_hint ? t.cache_hint - 1 : 2;
@@ -394,9 +446,12 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
     if (!tile) {
       // ldst: one CTA-wide round of 512 threads; bulk: 2 ring slots x 32 KiB keep 3 CTAs resident per SM
       tile = tn.variant == FLOWKV_VARIANT_BULK ? (32u << 10) : (64u << 10);
-      const uint64_t want_tiles = 8ull * pl->num_sms;
+      // small batches: at least two tiles per SM, but no smaller than 16 KiB — a launch-bound copy wants few, fat
+      // CTAs and a schedule short enough for the 512-byte parameter form (profiles/r02_sweep.md, tuning grid:
+      // 128 tokens 11.2 us with 8 KiB tiles, 10.3 us with >= 16 KiB; the same-size cudaMemcpyAsync takes 10.2 us)
+      const uint64_t want_tiles = 2ull * pl->num_sms;
       const uint64_t payload = pl->total_tokens * g.bytes_per_token;
-      while (tile > 4096 && payload / tile < want_tiles) tile >>= 1;
+      while (tile > 16384 && payload / tile < want_tiles) tile >>= 1;
     }
     pl->tile_bytes = tile;
 
@@ -516,10 +571,29 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   const uint32_t l0 = ro.ranged ? ro.layer_begin : 0, l1 = ro.ranged ? ro.layer_end : pl->g.L;
   if (l0 > l1 || l1 > pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
   if (op.sched.chunks.empty() || l0 == l1) return FLOWKV_OK;       // A11: nothing to move, zero launches
-  if ((cudaStream_t)stream != pl->stream && pl->staging.ev) {
-    // a stream other than the plan's own has not been ordered after the plan upload yet
-    cudaError_t e = FK_ENQ cudaStreamWaitEvent((cudaStream_t)stream, pl->staging.ev, 0);
-    if (e != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent(plan upload)");
+  if ((cudaStream_t)stream != pl->stream && pl->staging.ev && !pl->upload_seen_done.load(std::memory_order_acquire)) {
+    // A stream other than the plan's own has not been ordered after the plan upload yet.  Once the upload is known
+    // to have finished no edge is needed — which also lets a long-lived plan be captured into a CUDA graph on any
+    // stream (an edge to an event recorded outside the capture would invalidate it).  The query is made in relaxed
+    // capture mode: it is a host-side read of an event that belongs to no capture.
+    cudaStreamCaptureMode mode = cudaStreamCaptureModeRelaxed;
+    cudaThreadExchangeStreamCaptureMode(&mode);
+    cudaError_t q = cudaEventQuery(pl->staging.ev);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (q != cudaSuccess) {
+      (void)cudaGetLastError();
+      cudaStreamIsCapturing((cudaStream_t)stream, &cap);
+      // capturing and the few-KiB upload is still in flight: the only correct order is to let it finish first
+      if (cap == cudaStreamCaptureStatusActive) q = cudaEventSynchronize(pl->staging.ev);
+    }
+    cudaThreadExchangeStreamCaptureMode(&mode);
+    if (q == cudaSuccess) {
+      pl->upload_seen_done.store(true, std::memory_order_release);
+    } else {
+      (void)cudaGetLastError();
+      cudaError_t e = FK_ENQ cudaStreamWaitEvent((cudaStream_t)stream, pl->staging.ev, 0);
+      if (e != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent(plan upload)");
+    }
   }
   KernelParams kp{};
   kp.src = s; kp.dst = d;
@@ -736,8 +810,10 @@ flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, 
 }
 
 namespace {
-uint32_t via_host_chunks(const flowkv_plan_t* pl, uint32_t n_chunks) {
-  if (n_chunks == 0) n_chunks = 16;      // measured on B200 (profiles/r01_sweep.md)
+uint32_t via_host_chunks(const flowkv_plan_t* pl, uint32_t n_chunks, bool engines) {
+  // defaults measured on B200 (profiles/r02_host_route.md): the first outbound and the last inbound chunk cross the
+  // link alone, so the copy-engine pipeline wants many small chunks; the direct mode pays a kernel pair per chunk
+  if (n_chunks == 0) n_chunks = engines ? 32 : 16;
   return std::max<uint32_t>(1, std::min(n_chunks, pl->g.L));
 }
 uint64_t via_host_slot_bytes(const flowkv_plan_t* pl, uint32_t n_chunks) {
@@ -751,7 +827,7 @@ uint64_t via_host_slot_bytes(const flowkv_plan_t* pl, uint32_t n_chunks) {
 
 flowkv_status flowkv_via_host_scratch_bytes(const flowkv_plan_t* pl, uint32_t n_chunks, uint64_t* bytes) {
   if (!pl || !bytes) return fail(FLOWKV_ERR_INVALID_ARG, "NULL argument");
-  *bytes = 4 * via_host_slot_bytes(pl, via_host_chunks(pl, n_chunks));
+  *bytes = 4 * via_host_slot_bytes(pl, via_host_chunks(pl, n_chunks, true));
   return FLOWKV_OK;
 }
 
@@ -766,8 +842,8 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   if (pl->pack.sched.chunks.empty()) return FLOWKV_OK;
   if (!pl->on_device) return fail(FLOWKV_ERR_UNSUPPORTED, "plan was built by flowkv_plan_host and cannot run");
   const uint32_t L = pl->g.L;
-  n_chunks = via_host_chunks(pl, n_chunks);
   const bool engines = device_scratch != nullptr;          // copy engines drive the link, kernels stay in HBM
+  n_chunks = via_host_chunks(pl, n_chunks, engines);
   const uint64_t slot = via_host_slot_bytes(pl, n_chunks);
   if (engines) {
     if ((uintptr_t)device_scratch % 256) return fail(FLOWKV_ERR_ALIGN, "device_scratch is not 256-byte aligned");
@@ -775,59 +851,92 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   }
   cudaStream_t s = (cudaStream_t)stream;
   cudaError_t e;
-  if (!pl->aux) {
-    e = cudaStreamCreateWithFlags(&pl->aux, cudaStreamNonBlocking);
-    if (e != cudaSuccess) return fail_cuda(e, "cudaStreamCreate(aux)");
+  if (!pl->via) {
+    pl->via = g_via_host.acquire(pl->device);
+    if (!pl->via) return fail(FLOWKV_ERR_CUDA, "cudaStreamCreate(via-host helper streams)");
   }
-  while (pl->events.size() < (size_t)n_chunks + 2) {
+  ViaHostCtx& vc = *pl->via;
+  const size_t n_events = 4 * (size_t)n_chunks + 2;
+  while (vc.ev.size() < n_events) {
     cudaEvent_t ev;
     e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
     if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
-    pl->events.push_back(ev);
+    vc.ev.push_back(ev);
   }
-  // the inbound side (aux) starts after everything already queued on the caller's stream
-  cudaEvent_t e_start = pl->events[n_chunks], e_done = pl->events[n_chunks + 1];
-  if ((e = FK_ENQ cudaEventRecord(e_start, s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-  if ((e = FK_ENQ cudaStreamWaitEvent(pl->aux, e_start, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
-  const uint32_t vec = ((uintptr_t)host_staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
-  const uint32_t vecu = ((uintptr_t)host_staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
+#define FK_TRY(call, what) do { if ((e = FK_ENQ call) != cudaSuccess) return fail_cuda(e, what); } while (0)
   RunOpts ro;
   ro.ranged = true;
-  // direct mode: a PCIe-bound kernel needs few CTAs and both directions' kernels must be co-resident
-  ro.max_grid = engines ? ctas_per_kernel : (ctas_per_kernel ? ctas_per_kernel : 64);
+  if (!engines) {
+    // direct mode: the kernels touch host memory themselves; pack on `stream`, unpack on a helper stream.
+    // A PCIe-bound kernel needs few CTAs and both directions' kernels must be co-resident.
+    cudaStream_t aux = vc.q_unpack;
+    cudaEvent_t e_start = vc.ev[4 * (size_t)n_chunks], e_done = vc.ev[4 * (size_t)n_chunks + 1];
+    FK_TRY(cudaEventRecord(e_start, s), "cudaEventRecord");
+    FK_TRY(cudaStreamWaitEvent(aux, e_start, 0), "cudaStreamWaitEvent");
+    const uint32_t vec = ((uintptr_t)host_staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
+    const uint32_t vecu = ((uintptr_t)host_staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
+    ro.max_grid = ctas_per_kernel ? ctas_per_kernel : 64;
+    for (uint32_t c = 0; c < n_chunks; ++c) {
+      ro.layer_begin = (uint32_t)((uint64_t)L * c / n_chunks);
+      ro.layer_end = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
+      if (ro.layer_begin == ro.layer_end) continue;
+      st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);          // D2H on `stream`
+      if (st != FLOWKV_OK) return st;
+      FK_TRY(cudaEventRecord(vc.ev[c], s), "cudaEventRecord");
+      FK_TRY(cudaStreamWaitEvent(aux, vc.ev[c], 0), "cudaStreamWaitEvent");
+      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, aux, ro);     // H2D on the helper
+      if (st != FLOWKV_OK) return st;
+    }
+    FK_TRY(cudaEventRecord(e_done, aux), "cudaEventRecord");
+    FK_TRY(cudaStreamWaitEvent(s, e_done, 0), "cudaStreamWaitEvent");
+    return FLOWKV_OK;
+  }
+  // Copy-engine mode, four queues so that neither engine ever waits behind a kernel:
+  //   `stream`  pack kernels      pool -> out slot (k & 1)           waits: D2H of chunk k-2 has drained that slot
+  //   q_d2h     cudaMemcpyAsync   out slot -> host chunk             waits: pack k
+  //   q_h2d     cudaMemcpyAsync   host chunk -> in slot 2 + (k & 1)  waits: D2H k; unpack k-2 has drained that slot
+  //   q_unpack  unpack kernels    in slot -> pool                    waits: H2D k
+  // Chunk k is its own dense message (layer window [l0,l1), A20) at host offset window_bytes(0,l0).  While chunk k
+  // crosses the link outbound, chunk k-1 crosses it inbound and chunks k+1 / k-2 are packed / unpacked in HBM.
+  ro.max_grid = ctas_per_kernel;
   char* scratch = (char*)device_scratch;
-  uint32_t k = 0;                                          // non-empty chunks so far (scratch slot parity)
+  cudaEvent_t* packed = vc.ev.data();                       // [n_chunks] each
+  cudaEvent_t* landed = packed + n_chunks;
+  cudaEvent_t* arrived = landed + n_chunks;
+  cudaEvent_t* unpacked = arrived + n_chunks;
+  uint32_t k = 0;                                           // non-empty chunks so far
+  int64_t prev1 = -1, prev2 = -1;                           // chunk indices of the two previous non-empty chunks
   for (uint32_t c = 0; c < n_chunks; ++c) {
     const uint32_t l0 = (uint32_t)((uint64_t)L * c / n_chunks), l1 = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
+    if (l0 == l1) continue;
     ro.layer_begin = l0;
     ro.layer_end = l1;
-    if (l0 == l1) continue;
-    if (!engines) {
-      st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);      // D2H on `stream`
-      if (st != FLOWKV_OK) return st;
-      if ((e = FK_ENQ cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-      if ((e = FK_ENQ cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
-      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, pl->aux, ro);   // H2D on aux
-      if (st != FLOWKV_OK) return st;
-      continue;
-    }
-    // copy-engine mode: chunk c is its own dense message (layer window [l0,l1)) at host offset window_bytes(0,l0)
     const uint64_t wb = window_bytes(pl, l0, l1);
-    char* out_slot = scratch + (k & 1) * slot;             // outbound slots 0,1 live on `stream`
-    char* in_slot = scratch + (2 + (k & 1)) * slot;        // inbound slots 2,3 live on aux
+    char* out_slot = scratch + (k & 1) * slot;
+    char* in_slot = scratch + (2 + (k & 1)) * slot;
     char* host = (char*)host_staging + window_bytes(pl, 0, l0);
+    if (prev2 >= 0) FK_TRY(cudaStreamWaitEvent(s, landed[prev2], 0), "cudaStreamWaitEvent");          // out slot free again
     st = run(pl, pl->pack, pool_side(pl->src), dense_side(out_slot, pl->g, l0, l1), pl->pack.shape.vec_bytes, s, ro);
     if (st != FLOWKV_OK) return st;
-    if ((e = FK_ENQ cudaMemcpyAsync(host, out_slot, wb, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(D2H)");
-    if ((e = FK_ENQ cudaEventRecord(pl->events[c], s)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-    if ((e = FK_ENQ cudaStreamWaitEvent(pl->aux, pl->events[c], 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
-    if ((e = FK_ENQ cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync(H2D)");
-    st = run(pl, pl->unpack, dense_side(in_slot, pl->g, l0, l1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, pl->aux, ro);
+    FK_TRY(cudaEventRecord(packed[c], s), "cudaEventRecord");
+    FK_TRY(cudaStreamWaitEvent(vc.q_d2h, packed[c], 0), "cudaStreamWaitEvent");
+    FK_TRY(cudaMemcpyAsync(host, out_slot, wb, cudaMemcpyDeviceToHost, vc.q_d2h), "cudaMemcpyAsync(D2H)");
+    FK_TRY(cudaEventRecord(landed[c], vc.q_d2h), "cudaEventRecord");
+    FK_TRY(cudaStreamWaitEvent(vc.q_h2d, landed[c], 0), "cudaStreamWaitEvent");
+    if (prev2 >= 0) FK_TRY(cudaStreamWaitEvent(vc.q_h2d, unpacked[prev2], 0), "cudaStreamWaitEvent"); // in slot free again
+    FK_TRY(cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, vc.q_h2d), "cudaMemcpyAsync(H2D)");
+    FK_TRY(cudaEventRecord(arrived[c], vc.q_h2d), "cudaEventRecord");
+    FK_TRY(cudaStreamWaitEvent(vc.q_unpack, arrived[c], 0), "cudaStreamWaitEvent");
+    st = run(pl, pl->unpack, dense_side(in_slot, pl->g, l0, l1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
     if (st != FLOWKV_OK) return st;
+    FK_TRY(cudaEventRecord(unpacked[c], vc.q_unpack), "cudaEventRecord");
+    prev2 = prev1;
+    prev1 = c;
     ++k;
   }
-  if ((e = FK_ENQ cudaEventRecord(e_done, pl->aux)) != cudaSuccess) return fail_cuda(e, "cudaEventRecord");
-  if ((e = FK_ENQ cudaStreamWaitEvent(s, e_done, 0)) != cudaSuccess) return fail_cuda(e, "cudaStreamWaitEvent");
+  // `stream` continues only after the last chunk has been unpacked (q_unpack is in order, so that covers all)
+  if (prev1 >= 0) FK_TRY(cudaStreamWaitEvent(s, unpacked[prev1], 0), "cudaStreamWaitEvent");
+#undef FK_TRY
   return FLOWKV_OK;
 }
 
@@ -951,12 +1060,9 @@ flowkv_status flowkv_unpack_tables(const flowkv_pool* dst, const int32_t* dst_ta
 
 void flowkv_plan_destroy(flowkv_plan_t* pl) {
   if (!pl) return;
-  if (pl->aux) {
-    // via-host work on the aux stream was joined back into the caller's stream by an event, so the
-    // stream-ordered free below is already behind it; destroying a busy stream only defers its release
-    cudaStreamDestroy(pl->aux);
-  }
-  for (cudaEvent_t ev : pl->events) cudaEventDestroy(ev);
+  // via-host work on the helper streams was joined back into the caller's stream by an event, so the
+  // stream-ordered free below is already behind it; the helper streams and events go back to the cache
+  g_via_host.release(pl->via);
   if (pl->d_buf) FK_ENQ cudaFreeAsync(pl->d_buf, pl->stream);   // ordered after everything queued on the plan's stream
   g_pinned.release(pl->staging);
   drop_plan(pl);

@@ -25,7 +25,10 @@
 // Every scheduled kernel exists for a schedule in global memory and for one passed by value in the kernel parameters.
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
+
+#include <utility>
 
 #include "flowkv_internal.h"
 
@@ -84,6 +87,13 @@ template <int HINT> struct Mem<16, HINT> {
                    "r"(v.z), "r"(v.w), "l"(pol) : "memory");
   }
 };
+
+// Programmatic dependent launch (sm_90+): every copy kernel lets the NEXT kernel in the stream start its CTAs and
+// prologue while this one drains (launch_dependents, issued at entry), and waits for the PREVIOUS kernel's memory
+// to be complete and visible (wait) before it touches global memory.  Back-to-back small batches thereby overlap
+// their launch ramps with each other's tails.  Without the launch attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait_prior_grid() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 __device__ __forceinline__ uint64_t policy_evict_first() {
   uint64_t pol;
@@ -200,10 +210,12 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
   const uint32_t step = G * VEC;
   const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
 
+  pdl_launch_dependents();
   uint32_t tile = gtid >> p.group_log2;
   if (tile >= p.n_tiles) return;
   uint32_t plane, ci;
   decode_tile(p, tile, plane, ci);
+  pdl_wait_prior_grid();
   Chunk c = cs.get(ci);
   for (; tile < p.n_tiles; tile += n_groups) {
     // fetch the NEXT tile's schedule entry now, so its latency hides behind this tile's copy
@@ -235,10 +247,12 @@ __global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ K
   const uint32_t vpr = p.row_bytes / VEC;            // vectors per row
   const bool pow2 = (p.vpr_log2 != 0xffffffffu) && (p.heads_log2 != 0xffffffffu);
 
+  pdl_launch_dependents();
   uint32_t tile = gtid >> p.group_log2;
   if (tile >= p.n_tiles) return;
   uint32_t plane, ci;
   decode_tile(p, tile, plane, ci);
+  pdl_wait_prior_grid();
   Chunk c = cs.get(ci);
   for (; tile < p.n_tiles; tile += n_groups) {
     const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see fk_span_ldst)
@@ -275,6 +289,8 @@ __global__ void __launch_bounds__(512, 2) fk_flat_ldst(const __grid_constant__ K
   const uint32_t step = G * VEC;
   const uint64_t pol = (HINT == 2 && VEC == 16) ? policy_evict_first() : 0;
 
+  pdl_launch_dependents();
+  pdl_wait_prior_grid();
   const uint32_t n_flat_tiles = p.n_flat << p.flat_shift;
   for (uint32_t tile = group; tile < n_flat_tiles; tile += n_groups) {
     const Chunk c = cs.get(tile >> p.flat_shift);
@@ -344,11 +360,13 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
                                                       uint32_t stage_bytes, uint32_t n_stages) {
   extern __shared__ __align__(128) char ring[];
   __shared__ __align__(8) uint64_t full[kBulkMaxStages];
+  pdl_launch_dependents();
   if (threadIdx.x != 0) return;                       // one thread drives the TMA unit
   for (uint32_t i = 0; i < n_stages; ++i) mbar_init(&full[i], 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   const uint64_t pol = policy_evict_first();
+  pdl_wait_prior_grid();
 
   const uint32_t first = blockIdx.x, stride = gridDim.x;
   const uint32_t n_my = first < p.n_tiles ? (p.n_tiles - first + stride - 1) / stride : 0;
@@ -395,6 +413,8 @@ __global__ void __launch_bounds__(32, 1) fk_flat_bulk(const __grid_constant__ Ke
   __shared__ char* dptr[kBulkMaxStages];
   __shared__ uint32_t nbytes[kBulkMaxStages];
   const uint32_t n_flat_tiles = p.n_flat << p.flat_shift;
+  pdl_launch_dependents();
+  pdl_wait_prior_grid();
   if (threadIdx.x == 0) {
     for (uint32_t i = 0; i < n_stages; ++i) mbar_init(&full[i], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -448,21 +468,41 @@ __global__ void __launch_bounds__(32, 1) fk_flat_bulk(const __grid_constant__ Ke
 // ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
+// One launch with the programmatic-stream-serialization attribute (see pdl_launch_dependents()).  FLOWKV_PDL=0 in
+// the environment turns the attribute off (A/B measurements); results never depend on it.
+static bool pdl_enabled() {
+  static const bool on = [] { const char* e = getenv("FLOWKV_PDL"); return !(e && e[0] == '0'); }();
+  return on;
+}
+template <class... KArgs, class... Args>
+static cudaError_t launch_kernel(void (*kernel)(KArgs...), uint32_t grid, uint32_t block, size_t smem, cudaStream_t st,
+                                 Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 template <int VEC, int UNROLL, class CS>
 static cudaError_t launch_ldst(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, int hint,
                                cudaStream_t st) {
-  const dim3 grid(ls.grid), block(ls.threads);
-#define FK_LAUNCH(KERNEL)                                                                  \
-  switch (hint) {                                                                          \
-    case 0: KERNEL<VEC, UNROLL, 0, CS><<<grid, block, 0, st>>>(kp, cs); break;             \
-    case 1: KERNEL<VEC, UNROLL, 1, CS><<<grid, block, 0, st>>>(kp, cs); break;             \
-    default: KERNEL<VEC, UNROLL, 2, CS><<<grid, block, 0, st>>>(kp, cs); break;            \
+#define FK_LAUNCH(KERNEL)                                                                                  \
+  switch (hint) {                                                                                          \
+    case 0: return launch_kernel(KERNEL<VEC, UNROLL, 0, CS>, ls.grid, ls.threads, 0, st, kp, cs);          \
+    case 1: return launch_kernel(KERNEL<VEC, UNROLL, 1, CS>, ls.grid, ls.threads, 0, st, kp, cs);          \
+    default: return launch_kernel(KERNEL<VEC, UNROLL, 2, CS>, ls.grid, ls.threads, 0, st, kp, cs);         \
   }
   if (mode == MODE_SPAN) { FK_LAUNCH(fk_span_ldst) }
   else if (mode == MODE_FLAT) { FK_LAUNCH(fk_flat_ldst) }
   else { FK_LAUNCH(fk_rows_ldst) }
 #undef FK_LAUNCH
-  return cudaGetLastError();
 }
 
 uint32_t bulk_max_smem() {
@@ -478,15 +518,13 @@ static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const La
     const uint32_t smem = ls.n_stages * ls.stage_bytes;
     cudaError_t e = cudaFuncSetAttribute(fk_span_bulk<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    fk_span_bulk<CS><<<dim3(ls.grid), dim3(32), smem, st>>>(kp, cs, ls.stage_bytes, ls.n_stages);
-    return (int)cudaGetLastError();
+    return (int)launch_kernel(fk_span_bulk<CS>, ls.grid, 32, smem, st, kp, cs, ls.stage_bytes, ls.n_stages);
   }
   if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_FLAT) {
     const uint32_t smem = ls.n_stages * ls.stage_bytes;
     cudaError_t e = cudaFuncSetAttribute(fk_flat_bulk<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
-    fk_flat_bulk<CS><<<dim3(ls.grid), dim3(32), smem, st>>>(kp, cs, ls.stage_bytes, ls.n_stages);
-    return (int)cudaGetLastError();
+    return (int)launch_kernel(fk_flat_bulk<CS>, ls.grid, 32, smem, st, kp, cs, ls.stage_bytes, ls.n_stages);
   }
   if (ls.vec_bytes == 32) return (int)launch_ldst<32, 4, CS>(mode, kp, cs, ls, (int)ls.hint, st);
   return (int)launch_ldst<16, 8, CS>(mode, kp, cs, ls, (int)ls.hint, st);
@@ -541,6 +579,8 @@ __global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__
   const bool pow2 = (p.vpr_log2 != 0xffffffffu) && (p.heads_log2 != 0xffffffffu);
   const uint32_t g = 1u << tp.granule_log2;
   const uint32_t per_plane = tp.n_reqs * tp.q_per_req;
+  pdl_launch_dependents();
+  pdl_wait_prior_grid();               // the tables themselves may have been written by the previous kernel
   for (uint32_t tile = gtid >> p.group_log2; tile < tp.n_tiles; tile += n_groups) {
     const uint32_t pl = tile / per_plane, rq = tile - pl * per_plane;
     const uint32_t plane = pl + p.plane0;
@@ -569,10 +609,8 @@ __global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__
 
 int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
-  const dim3 grid(ls.grid), block(ls.threads);
-  if (ls.vec_bytes == 32) fk_tables_ldst<32, 4, 2><<<grid, block, 0, st>>>(tp);
-  else                    fk_tables_ldst<16, 8, 2><<<grid, block, 0, st>>>(tp);
-  return (int)cudaGetLastError();
+  if (ls.vec_bytes == 32) return (int)launch_kernel(fk_tables_ldst<32, 4, 2>, ls.grid, ls.threads, 0, st, tp);
+  return (int)launch_kernel(fk_tables_ldst<16, 8, 2>, ls.grid, ls.threads, 0, st, tp);
 }
 
 }  // namespace flowkv

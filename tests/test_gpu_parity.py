@@ -837,8 +837,8 @@ def test_table_driven_layer_ranges_parity_and_one_graph_of_layerwise_launches():
     ONCE in a CUDA graph and replayed while the device tables change, whole pool against the oracle each time."""
     shape = synth.Shape(5, 2, 64, "fp16")
     L = shape.num_layers
-    w = synth.make_workload("tables_layers", 4242, shape, [150, 31, 0, 64], "lkbthd", 16, ("geometric", 2.0), None,
-                            "blkhtd", 32, ("geometric", 4.0), None)
+    w = synth.make_workload("tables_layers", 4242, shape, [150, 31, 0, 64], "lkbthd", 16, ("geometric", 2.0), 64,
+                            "blkhtd", 32, ("geometric", 4.0), 32)
     dp = P.DevicePools(w, fill="bits")
     src_np = P.to_numpy(dp.src_buf)
     gs, gd = G.geom(w.src, shape), G.geom(w.dst, shape)
