@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libflowkv.so")
-SOURCES = ["kernels.cu", "api.cpp", "planner.cpp", "allocator.cpp"]
+SOURCES = ["kernels.cu", "api.cpp", "planner.cpp", "allocator.cpp", "tma.cpp"]
 HEADERS = [os.path.join(CSRC, "flowkv_internal.h"), os.path.join(INCLUDE, "flowkv.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-Wall,-fvisibility=hidden", "-cudart", "static"]

@@ -219,6 +219,7 @@ struct Op {                  // one runnable operation of a plan
   uint32_t tile_order = 0;   // resolved: 0 plane-major, 1 chunk-major
   uint32_t max_chunk_bytes = 0;
   bool in_params = false;    // schedule small enough to ride in the kernel parameters (no upload)
+  RowsTma tma;               // rows mode + bulk variant: the tensor maps of both pools (ok == false: register path)
 };
 
 }  // namespace
@@ -305,27 +306,37 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
   const uint32_t use_sms = t.max_sms ? std::min(t.max_sms, sms) : sms;
   ls.vec_bytes = pick_vec(a, b, pl->g);
   ls.variant = t.variant ? t.variant : FLOWKV_VARIANT_LDST;
-  if (op.sched.mode != MODE_SPAN && op.sched.mode != MODE_FLAT) ls.variant = FLOWKV_VARIANT_LDST;   // bulk moves byte ranges only
   op.max_chunk_bytes = 0;
   for (size_t i = 0; i < op.sched.chunks.size(); ++i) {
     const Chunk& c = op.sched.chunks[i];
     if (op.sched.mode == MODE_FLAT && i < op.sched.n_flat) continue;     // cut into flat_tile pieces by the kernel
     op.max_chunk_bytes = std::max(op.max_chunk_bytes, op.sched.mode == MODE_SPAN ? c.n : c.n * pl->g.tok_bytes);
   }
+  op.tma.ok = false;
+  if (op.sched.mode == MODE_ROWS && ls.variant == FLOWKV_VARIANT_BULK) {
+    // rows mode rides the TMA TENSOR path when both sides are pools a 5-D tensor map can describe (tma.cpp); a dense
+    // side (pack / unpack: its plane stride is T_r, per request) and host-only plans run the register path
+    std::string why;
+    const uint32_t box_tok = op.max_chunk_bytes / pl->g.tok_bytes;
+    if (!(a && b && pl->device >= 0 && box_tok && build_rows_tma(*a, *b, pl->g, box_tok, op.tma, why)))
+      ls.variant = FLOWKV_VARIANT_LDST;
+  }
   op.tile_order = t.tile_order == 2 ? 1 : 0;
   const uint64_t n_tiles = ((uint64_t)op.sched.n_flat << op.sched.flat_shift) + (uint64_t)op.sched.n_per_plane() * 2 * pl->g.L;
   if (ls.variant == FLOWKV_VARIANT_BULK) {
     // a ring slot holds the largest chunk (span mode: at least one token's plane bytes); two slots must fit in
     // shared memory, else the plan runs the register path (reported in flowkv_plan_stats.variant)
-    const uint32_t stage = ((std::max<uint32_t>(op.sched.mode == MODE_FLAT ? op.sched.flat_tile : op.max_chunk_bytes, 1024)) + 127) & ~127u;
+    uint32_t stage_need = op.sched.mode == MODE_FLAT ? op.sched.flat_tile : op.max_chunk_bytes;
+    if (op.sched.mode == MODE_ROWS)          // a ragged chunk parks each token at a 128-byte aligned offset
+      stage_need = std::max<uint32_t>(stage_need, (op.tma.box_tok ? op.tma.box_tok - 1 : 0) * op.tma.tok_slot);
+    const uint32_t stage = ((std::max<uint32_t>(stage_need, 1024)) + 127) & ~127u;
     const uint32_t cap = (pl->max_smem_optin ? pl->max_smem_optin : 232448) - 1024;
     if (2ull * stage > cap) ls.variant = FLOWKV_VARIANT_LDST;
+    ls.stage_bytes = stage;
   }
   if (ls.variant == FLOWKV_VARIANT_BULK) {
     ls.threads = 32;
     ls.group_threads = 32;
-    ls.stage_bytes = std::max<uint32_t>(op.sched.mode == MODE_FLAT ? op.sched.flat_tile : op.max_chunk_bytes, 1024);
-    ls.stage_bytes = (ls.stage_bytes + 127) & ~127u;
     // like the ldst path the grid is oversubscribed (<= 256 CTAs per SM) and each CTA's ring is short:
     // several small CTAs per SM, scheduled by hardware, beat one long-lived CTA with a deep ring
     const uint32_t ctas = t.ctas_per_sm ? t.ctas_per_sm : 256;
@@ -620,6 +631,15 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   kp.tile_order = op.tile_order;
   LaunchShape ls = op.shape;
   ls.vec_bytes = vec_bytes;
+  if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_ROWS && !op.tma.ok) {
+    // a layer range of a flat (block-major) bulk plan runs its rows schedule: no tensor maps for it, register path
+    ls.variant = FLOWKV_VARIANT_LDST;
+    ls.threads = 512;
+    ls.group_threads = 128;
+    ls.hint = 2;
+    ls.grid = (pl->tuning.max_sms ? std::min(pl->tuning.max_sms, pl->num_sms) : pl->num_sms) *
+              (pl->tuning.ctas_per_sm ? pl->tuning.ctas_per_sm : 256);
+  }
   const uint32_t groups_per_cta = ls.variant == FLOWKV_VARIANT_BULK ? 1 : ls.threads / ls.group_threads;
   ls.grid = std::min<uint32_t>(ls.grid, (kp.n_tiles + groups_per_cta - 1) / groups_per_cta);
   if (ro.max_grid) ls.grid = std::min(ls.grid, ro.max_grid);
@@ -627,8 +647,8 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   kp.vpr_log2 = log2_or_none(kp.row_bytes / ls.vec_bytes);
   kp.heads_log2 = log2_or_none(kp.heads);
   const int e = op.in_params
-                    ? launch_copy(mode, kp, nullptr, op.sched.chunks.data() + first, (uint32_t)op.sched.chunks.size() - first, ls, stream)
-                    : launch_copy(mode, kp, op.d_chunks + first, nullptr, 0, ls, stream);
+                    ? launch_copy(mode, kp, nullptr, op.sched.chunks.data() + first, (uint32_t)op.sched.chunks.size() - first, ls, stream, &op.tma)
+                    : launch_copy(mode, kp, op.d_chunks + first, nullptr, 0, ls, stream, &op.tma);
   if (e != 0) return fail_cuda((cudaError_t)e, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
   g_api_calls.fetch_add(1, std::memory_order_relaxed);

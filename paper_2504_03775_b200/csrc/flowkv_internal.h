@@ -2,6 +2,7 @@
 // kernels of the product path.  Nothing under oracle/ includes this file.
 #pragma once
 
+#include <cuda.h>          // CUtensorMap (types only; the driver is reached through cudaGetDriverEntryPoint)
 #include <stdint.h>
 
 #include <new>
@@ -90,11 +91,29 @@ struct LaunchShape {
   uint32_t stage_bytes;   // bulk: bytes per ring slot (>= largest chunk)
 };
 
+// Rows mode through the TMA tensor path (cp.async.bulk.tensor): one 5-D tensor map per pool over
+//   (row element, token in block, head, block, plane = 2*layer + kv)
+// in that order on BOTH sides, whatever the pool's strides are.  A box of (row, box_tok tokens, Hkv heads, 1, 1)
+// therefore lands in shared memory as dense [head][token][row] bytes and is stored through the other pool's map
+// with the other pool's strides: the layout / block-size conversion is done by the TMA unit's address generation,
+// one elected thread, no payload registers.  `one` = the same maps with a 1-token box for ragged chunks (A4).
+struct RowsTma {
+  CUtensorMap src_full, dst_full, src_one, dst_one;
+  uint32_t box_tok = 0;        // tokens per full box (= largest chunk of the schedule)
+  uint32_t tok_slot = 0;       // shared-memory bytes one token occupies in a ragged slot (tok_bytes rounded to 128)
+  int64_t  src_s_block = 0, dst_s_block = 0, src_s_token = 0, dst_s_token = 0;
+  bool     ok = false;
+};
+// tma.cpp — builds (and caches per pool pair) the maps; false + `why` when the shape cannot ride the tensor path
+// (then the plan runs the register path and says so in flowkv_plan_stats.variant).
+bool build_rows_tma(const flowkv_pool& src, const flowkv_pool& dst, const struct Geometry& g, uint32_t box_tok,
+                    RowsTma& out, std::string& why);
+
 // kernels.cu — launches exactly one kernel; returns cudaError_t as int.  The schedule entries come from
 // `device_chunks`, or, when `host_chunks` is not NULL (n_host_chunks <= kInlineChunks), travel by value in
 // the kernel parameters.
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
-                uint32_t n_host_chunks, const LaunchShape& ls, void* stream);
+                uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma = nullptr);
 // Table-driven transfer (flowkv_transfer_tables): no host plan; the kernel walks device-resident block tables.
 struct TablesParams {
   KernelParams    kp;          // src/dst sides, row_bytes, heads, tok_bytes, group_log2, vpr_log2, heads_log2, n_planes

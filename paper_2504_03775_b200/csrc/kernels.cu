@@ -466,6 +466,93 @@ __global__ void __launch_bounds__(32, 1) fk_flat_bulk(const __grid_constant__ Ke
 }
 
 // ------------------------------------------------------------------------------------------------
+// bulk / rows: the TMA TENSOR path (cp.async.bulk.tensor -> UTMALDG / UTMASTG).  Both pools are 5-D tensors over
+// (row element, token in block, head, block, plane) — same dimension order, different strides (tma.cpp).  One
+// thread per CTA loads a box of (row, box_tok tokens, Hkv heads) through the src map into a ring slot, where it
+// sits as dense [head][token][row] bytes, and stores the slot through the dst map: the token-major -> head-major
+// conversion and the block-size change (BASELINE configs[3]) happen in the TMA unit's address generation.  No payload
+// registers, no LSU slots — the shape that co-runs with GEMMs.  Chunks shorter than a box (the
+// ragged end of a request, reading A4) move token by token through 1-token boxes, so nothing past T_r is touched.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* map, uint32_t c1, uint32_t c3, uint32_t c4,
+                                            uint64_t* bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4, %5, %6}], [%7], %8;" ::"r"(smem_u32(smem_dst)),
+      "l"(map), "r"(0), "r"(c1), "r"(0), "r"(c3), "r"(c4), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* map, uint32_t c1, uint32_t c3, uint32_t c4, const void* smem_src,
+                                             uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group.L2::cache_hint"
+      " [%0, {%1, %2, %3, %4, %5}], [%6], %7;" ::"l"(map),
+      "r"(0), "r"(c1), "r"(0), "r"(c3), "r"(c4), "r"(smem_u32(smem_src)), "l"(pol) : "memory");
+}
+
+struct RowsTmaParams {              // by value in the kernel parameters; the maps must be __grid_constant__
+  CUtensorMap src_full, dst_full, src_one, dst_one;
+  int64_t  src_s_block, dst_s_block, src_s_token, dst_s_token;
+  uint32_t box_tok, tok_slot, stage_bytes, n_stages;
+};
+
+template <class CS>
+__global__ void __launch_bounds__(32, 1) fk_rows_tma(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                     const __grid_constant__ RowsTmaParams tp) {
+  extern __shared__ __align__(128) char ring[];
+  __shared__ __align__(8) uint64_t full[kBulkMaxStages];
+  __shared__ uint32_t s_db[kBulkMaxStages], s_dt[kBulkMaxStages], s_n[kBulkMaxStages], s_plane[kBulkMaxStages];
+  pdl_launch_dependents();
+  if (threadIdx.x != 0) return;                       // one thread drives the TMA unit
+  for (uint32_t i = 0; i < tp.n_stages; ++i) mbar_init(&full[i], 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  const uint64_t pol = policy_evict_first();
+  pdl_wait_prior_grid();
+
+  const uint32_t first = blockIdx.x, stride = gridDim.x;
+  const uint32_t n_my = first < p.n_tiles ? (p.n_tiles - first + stride - 1) / stride : 0;
+  const uint32_t ahead = tp.n_stages - 1;
+
+  auto issue_load = [&](uint32_t k) {
+    uint32_t plane, ci;
+    decode_tile(p, first + k * stride, plane, ci);
+    const Chunk c = cs.get(ci);
+    // chunk offsets are bytes inside one plane: block * s_block + token * s_token (planner.cpp pool_off)
+    const uint32_t sb = (uint32_t)(c.src_off / tp.src_s_block), st = (uint32_t)((c.src_off - sb * tp.src_s_block) / tp.src_s_token);
+    const uint32_t db = (uint32_t)(c.dst_off / tp.dst_s_block), dt = (uint32_t)((c.dst_off - db * tp.dst_s_block) / tp.dst_s_token);
+    const uint32_t slot = k % tp.n_stages;
+    s_db[slot] = db; s_dt[slot] = dt; s_n[slot] = c.n; s_plane[slot] = plane;
+    char* buf = ring + (size_t)slot * tp.stage_bytes;
+    if (c.n == tp.box_tok) {
+      mbar_expect_tx(&full[slot], c.n * p.tok_bytes);
+      tma_load_5d(buf, &tp.src_full, st, sb, plane, &full[slot], pol);
+    } else {                                          // ragged chunk: token by token (A4: nothing past T_r moves)
+      mbar_expect_tx(&full[slot], c.n * p.tok_bytes);
+      for (uint32_t t = 0; t < c.n; ++t) tma_load_5d(buf + (size_t)t * tp.tok_slot, &tp.src_one, st + t, sb, plane, &full[slot], pol);
+    }
+  };
+
+  for (uint32_t k = 0; k < ahead && k < n_my; ++k) issue_load(k);
+  for (uint32_t k = 0; k < n_my; ++k) {
+    const uint32_t slot = k % tp.n_stages;
+    mbar_wait(&full[slot], (k / tp.n_stages) & 1);    // the box has landed in its slot
+    const char* buf = ring + (size_t)slot * tp.stage_bytes;
+    const uint32_t n = s_n[slot], db = s_db[slot], dt = s_dt[slot], plane = s_plane[slot];
+    if (n == tp.box_tok) {
+      tma_store_5d(&tp.dst_full, dt, db, plane, buf, pol);
+    } else {
+      for (uint32_t t = 0; t < n; ++t) tma_store_5d(&tp.dst_one, dt + t, db, plane, buf + (size_t)t * tp.tok_slot, pol);
+    }
+    bulk_commit();
+    if (k + ahead < n_my) {
+      bulk_wait_read<1>();                            // slot of tile k-1 has been read out by its store
+      issue_load(k + ahead);
+    }
+  }
+  bulk_wait_all();
+}
+
+// ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
 // One launch with the programmatic-stream-serialization attribute (see pdl_launch_dependents()).  FLOWKV_PDL=0 in
@@ -513,7 +600,19 @@ uint32_t bulk_max_smem() {
 }
 
 template <class CS>
-static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, cudaStream_t st) {
+static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, cudaStream_t st,
+                       const RowsTma* tma) {
+  if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_ROWS && tma && tma->ok) {
+    RowsTmaParams tp;
+    tp.src_full = tma->src_full; tp.dst_full = tma->dst_full; tp.src_one = tma->src_one; tp.dst_one = tma->dst_one;
+    tp.src_s_block = tma->src_s_block; tp.dst_s_block = tma->dst_s_block;
+    tp.src_s_token = tma->src_s_token; tp.dst_s_token = tma->dst_s_token;
+    tp.box_tok = tma->box_tok; tp.tok_slot = tma->tok_slot; tp.stage_bytes = ls.stage_bytes; tp.n_stages = ls.n_stages;
+    const uint32_t smem = ls.n_stages * ls.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(fk_rows_tma<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    return (int)launch_kernel(fk_rows_tma<CS>, ls.grid, 32, smem, st, kp, cs, tp);
+  }
   if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_SPAN) {
     const uint32_t smem = ls.n_stages * ls.stage_bytes;
     cudaError_t e = cudaFuncSetAttribute(fk_span_bulk<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -531,21 +630,21 @@ static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const La
 }
 
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
-                uint32_t n_host_chunks, const LaunchShape& ls, void* stream) {
+                uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma) {
   cudaStream_t st = (cudaStream_t)stream;
   if (host_chunks) {                       // small plan: the schedule rides in the kernel parameters
     if (n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
     if (n_host_chunks <= kInlineChunksSmall) {
       ParamChunks<kInlineChunksSmall> pc;
       memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
-      return launch_with(mode, kp, pc, ls, st);
+      return launch_with(mode, kp, pc, ls, st, tma);
     }
     ParamChunks<kInlineChunks> pc;
     memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
-    return launch_with(mode, kp, pc, ls, st);
+    return launch_with(mode, kp, pc, ls, st, tma);
   }
   GlobalChunks gc{device_chunks};
-  return launch_with(mode, kp, gc, ls, st);
+  return launch_with(mode, kp, gc, ls, st, tma);
 }
 
 // ------------------------------------------------------------------------------------------------

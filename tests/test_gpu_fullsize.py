@@ -280,6 +280,15 @@ def test_cfg4_full_size_fit_rule():
     P.fill_sentinel(dp.dst_buf)
     _run_tables(w, dp)
     _cfg4_check(w, dp, layers)
+    # the TMA tensor path (cp.async.bulk.tensor) at full size, under the SM budget it is meant for
+    for tuning in ({"variant": "bulk"}, {"variant": "bulk", "max_sms": 32, "ctas_per_sm": 2, "stages": 4}):
+        P.fill_sentinel(dp.dst_buf)
+        tma = dp.plan(0, tuning)
+        assert tma.stats["variant"] == F.FLOWKV_VARIANT_BULK and tma.stats["mode_transfer"] == 2
+        tma.transfer()
+        torch.cuda.synchronize()
+        _cfg4_check(w, dp, layers[-2:])
+        tma.destroy()
 
 
 def test_cfg5_largest_sweep_point_full_size():

@@ -111,6 +111,9 @@ def test_fuzz_against_oracle(idx):
     tokb = H * D * e
     what = f"case {idx}: {lay_s}{bs_s}->{lay_d}{bs_d} L{L} H{H} D{D} e{e} T={[t for t, _, _ in reqs]} {tuning} {op}"
     plan = F.flowkv_plan(src, dst, freqs, F.FLOWKV_CHECK_DST_ALIAS, tuning or None)
+    if tuning.get("variant") == "bulk" and plan.stats["mode_transfer"] == 2 and not ss and not sd and total:
+        # named layouts in rows mode: the bulk variant is honoured (TMA tensor path), not silently replaced
+        assert plan.stats["variant"] == F.FLOWKV_VARIANT_BULK, what
 
     def expect_transfer(l0=0, l1=L):
         exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)

@@ -918,3 +918,86 @@ def test_segment_allocator_tables_through_plan_and_transfer():
     assert plan.stats["n_segments"] == n_seg
     fifo_seg = sum(O.count_segments(r.src_blocks, 16, r.dst_blocks, 16, r.num_tokens) for r in fifo.requests)
     assert n_seg * 3 < fifo_seg, (n_seg, fifo_seg)        # the allocator's point: far fewer, longer segments
+
+
+# ---------------------------------------------------------------------------------------------------------
+# rows mode through the TMA tensor path (cp.async.bulk.tensor): layout / block-size conversion by the TMA unit
+# ---------------------------------------------------------------------------------------------------------
+ROWS_TMA_TUNINGS = [
+    {"variant": "bulk"},
+    {"variant": "bulk", "stages": 4, "tile_bytes": 16384},
+    {"variant": "bulk", "max_sms": 16, "ctas_per_sm": 2, "stages": 6},
+    {"variant": "bulk", "plan_in_params": 1, "tile_order": 2, "tile_bytes": 8192},
+]
+
+
+@pytest.mark.parametrize("tuning", ROWS_TMA_TUNINGS)
+def test_cfg4_hetero_through_the_tma_tensor_path(tuning):
+    """configs[3] scaled (src BS16 LKBTHD -> dst BS64 BLKHTD, partial 64-token dst blocks, ragged request ends): the
+    bulk variant is honoured in rows mode (stats.variant says so) and the whole dst pool is the oracle's."""
+    w = synth.config4_hetero(n_requests=3, num_layers=2)
+    dp, plan, _ = G.run_transfer_and_check(w, tuning)
+    st = plan.stats
+    assert st["mode_transfer"] == 2 and st["variant"] == F.FLOWKV_VARIANT_BULK and st["threads"] == 32, st
+    assert st["smem_bytes"] <= 227 * 1024
+
+
+@pytest.mark.parametrize("pair", [("lkbthd", 16, "blkhtd", 64), ("blkhtd", 64, "lkbthd", 16), ("blkhtd", 8, "blkhtd", 32),
+                                  ("blkthd", 4, "blkhtd", 4), ("lkbthd", 1, "blkhtd", 2), ("blkhtd", 32, "blkthd", 16)])
+@pytest.mark.parametrize("heads,dim,dtype", [(8, 128, "bf16"), (3, 40, "fp16"), (1, 8, "fp16"), (5, 16, "fp8"), (2, 64, "fp32")])
+def test_rows_tma_layout_pairs_shapes_and_ragged_ends(pair, heads, dim, dtype):
+    """Every rows-mode layout pair, odd head counts, 16-byte rows (tokens of 48 .. 2048 bytes: ragged chunks park
+    tokens at 128-byte aligned shared-memory offsets), 1-, 2- and 4-byte elements; request lengths that end inside a
+    block on both sides, an empty request and a one-token request; layer ranges ride the same maps."""
+    sl, sbs, dl, dbs = pair
+    shape = synth.Shape(3, heads, dim, dtype)
+    w = synth.make_workload(f"rows_tma_{sl}{sbs}_{dl}{dbs}", 31337, shape, [97, 0, 1, 130, 64], sl, sbs, ("geometric", 3.0), None,
+                            dl, dbs, ("geometric", 5.0), None)
+    dp, plan, exp = G.run_transfer_and_check(w, {"variant": "bulk"}, fill="bits")
+    assert plan.stats["variant"] == F.FLOWKV_VARIANT_BULK, plan.stats
+    src_np = P.to_numpy(dp.src_buf)
+    gs, gd = G.geom(w.src, shape), G.geom(w.dst, shape)
+    for l0, l1 in [(0, 1), (1, 3), (2, 2)]:
+        P.fill_sentinel(dp.dst_buf)
+        n0 = F.flowkv_launch_count()
+        F.flowkv_transfer_layers(plan, l0, l1)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == (1 if l1 > l0 else 0)
+        e2 = np.full(w.dst.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+        for r in w.requests:
+            O.transfer(src_np, gs, e2, gd, r.src_blocks, r.dst_blocks, r.num_tokens, l0, l1)
+        G.assert_same(P.to_numpy(dp.dst_buf), e2, f"rows TMA layers [{l0},{l1})")
+    # pack / unpack of a bulk rows plan run the register path (a dense side has no tensor map) and still match
+    nbytes = plan.stats["staging_bytes"]
+    staging = P.alloc_bytes(nbytes)
+    P.fill_sentinel(dp.dst_buf)
+    plan.pack(staging.data_ptr(), nbytes)
+    plan.unpack(staging.data_ptr(), nbytes)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(staging), G.oracle_pack(w, src_np), "wire bytes of a bulk rows plan")
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "unpack of a bulk rows plan")
+
+
+def test_rows_tma_falls_back_where_a_tensor_map_cannot_describe_the_pool():
+    """A STRIDED pool whose layer stride is not twice its K|V stride has no uniform plane axis: the plan says LDST in
+    stats.variant and the bytes are still the oracle's."""
+    shape = synth.Shape(2, 2, 64, "fp16")
+    L, H, D, NBs, NBd, bs = 2, 2, 64, 12, 10, 8
+    row, tok = D * 2, H * D * 2
+    blk, kv = bs * tok, NBs * bs * tok + 64
+    lay = 2 * kv + 96
+    gs = O.PoolGeom(L, H, D, 2, NBs, bs, lay, kv, blk, tok, row)
+    gd = O.PoolGeom.blkhtd(L, H, D, 2, NBd, bs)
+    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
+    P.fill_values(src_buf, "bits", "fp16", 5)
+    P.fill_sentinel(dst_buf)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, 2, NBs, bs, "strided", [lay, kv, blk, tok, row])
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, 2, NBd, bs, "blkhtd")
+    a, b = np.asarray([3, 4, 9, 0], np.int32), np.asarray([7, 1, 2, 5], np.int32)
+    plan = F.flowkv_plan(src, dst, [F.Request(29, a, b)], 0, {"variant": "bulk"})
+    assert plan.stats["mode_transfer"] == 2 and plan.stats["variant"] == F.FLOWKV_VARIANT_LDST
+    plan.transfer()
+    torch.cuda.synchronize()
+    exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)
+    O.transfer(P.to_numpy(src_buf), gs, exp, gd, a, b, 29)
+    G.assert_same(P.to_numpy(dst_buf), exp, "fallback")
