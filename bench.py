@@ -386,7 +386,11 @@ def time_steps(F, w, src, dst, requests, K, W, tuning, stream, barrier, local, d
 
 
 def kernel_name(stats, device_tables: bool) -> str:
-    return "fk_tables_ldst" if device_tables else {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]]
+    if device_tables:
+        return "fk_tables_ldst"
+    if stats["variant"] == 2:       # FLOWKV_VARIANT_BULK: the TMA kernels (rows mode = the tensor path)
+        return {1: "fk_span_bulk", 2: "fk_rows_tma", 3: "fk_flat_bulk"}[stats["mode_transfer"]]
+    return {1: "fk_span_ldst", 2: "fk_rows_ldst", 3: "fk_flat_ldst"}[stats["mode_transfer"]]
 
 
 def roofline_of(m, payload, w_key, stats, K, device_tables):

@@ -5,9 +5,11 @@ processes like GEMM"; S§8f NEXT-4).
     python bench_corun.py [--out gpurun_out/corun.json]
 
 A bf16 8192^3 cuBLAS GEMM loop (the interferer; library code, not part of the product) runs on one stream, the
-configs[1] transfer on another.  Each is timed alone and then together (CUDA events on its own stream, both
-loops sized to ~80 ms so they overlap fully), for several SM budgets of the transfer kernel
-(`flowkv_tuning.max_sms` x `ctas_per_sm`, ldst and bulk/TMA variants)."""
+transfer (configs[1], or with --config cfg4 a rows-mode slice of configs[3]) on another.  Each is timed alone and then
+next to the other: both loops run for ~0.3 s, every iteration stamps its completion with a CUDA event on its own
+stream, and both rates are read over the same window (the middle of the time both streams were busy) — for several
+SM budgets of the transfer kernel (`flowkv_tuning.max_sms` x
+`ctas_per_sm`, ldst and bulk/TMA variants; in rows mode the bulk variant is the TMA tensor path, fk_rows_tma)."""
 from __future__ import annotations
 
 import argparse
@@ -22,13 +24,16 @@ sys.path.insert(0, ROOT)
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "corun.json"))
+    ap.add_argument("--config", default="cfg2", choices=["cfg2", "cfg4"],
+                    help="cfg2: configs[1] (span mode); cfg4: a 4-request slice of configs[3] (rows mode: src BS16 LKBTHD -> "
+                         "dst BS64 BLKHTD; the bulk variant is the TMA tensor path)")
     args = ap.parse_args()
     import torch
     from paper_2504_03775_b200 import build as B
     B.build()
     from paper_2504_03775_b200 import flowkv as F, pools as P, synth
 
-    w = synth.config2_llama8b_13k()
+    w = synth.config2_llama8b_13k() if args.config == "cfg2" else synth.config4_hetero(n_requests=4)
     dp = P.DevicePools(w, sentinel_dst=False)
     N = 8192
     a = torch.randn(N, N, device="cuda", dtype=torch.bfloat16)
@@ -36,52 +41,77 @@ def main():
     c = torch.empty(N, N, device="cuda", dtype=torch.bfloat16)
     sg, sc = torch.cuda.Stream(), torch.cuda.Stream()
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    n_gemm, n_copy = 120, 150
 
-    def gemm_loop():
-        e0, e1 = ev(), ev()
+    def gemm_loop(n, stamps=None):
         with torch.cuda.stream(sg):
-            e0.record(sg)
-            for _ in range(n_gemm):
+            for _ in range(n):
                 torch.matmul(a, b, out=c)
-            e1.record(sg)
-        return e0, e1
+                if stamps is not None:
+                    e = ev(); e.record(sg); stamps.append(e)
 
-    def copy_loop(plan):
-        e0, e1 = ev(), ev()
-        e0.record(sc)
-        for _ in range(n_copy):
+    def copy_loop(plan, n, stamps=None):
+        for _ in range(n):
             plan.transfer(sc.cuda_stream)
-        e1.record(sc)
-        return e0, e1
+            if stamps is not None:
+                e = ev(); e.record(sc); stamps.append(e)
 
-    tf = lambda ms: n_gemm * 2 * N ** 3 / (ms * 1e-3) / 1e12
-    gb = lambda ms: n_copy * 2 * w.payload_bytes / (ms * 1e-3) / 1e9
-    for _ in range(2):
-        e0, e1 = gemm_loop(); torch.cuda.synchronize()
-    gemm_alone = tf(e0.elapsed_time(e1))
+    def rate_in_window(t0, stamps, lo, hi):
+        """Iterations that completed inside [lo, hi] ms (per-iteration completion stamps) per ms."""
+        ts = [t0.elapsed_time(e) for e in stamps]
+        inside = [t for t in ts if lo <= t <= hi]
+        return (len(inside) - 1) / (inside[-1] - inside[0]) if len(inside) > 2 else float("nan")
+
+    tf = lambda per_ms: per_ms * 2 * N ** 3 / 1e-3 / 1e12
+    gb = lambda per_ms: per_ms * 2 * w.payload_bytes / 1e-3 / 1e9
+    gemm_loop(10); torch.cuda.synchronize()
+    t0 = ev(); st_ = []
+    t0.record(sg); gemm_loop(20, st_); torch.cuda.synchronize()
+    gemm_ms = t0.elapsed_time(st_[-1]) / 20
+    # the GEMM alone over the same ~0.3 s and the same window rule (a 1 kW part settles under its power cap: the
+    # burst rate of a short loop is not what a co-run of this length should be compared with)
+    t0 = ev(); st_ = []
+    t0.record(sg); gemm_loop(max(20, int(300.0 / gemm_ms)), st_); torch.cuda.synchronize()
+    end = t0.elapsed_time(st_[-1])
+    gemm_alone = tf(rate_in_window(t0, st_, 0.15 * end, 0.95 * end))
     rows = []
-    settings = [("default (grid <= 256 CTAs/SM)", None),
-                ("max_sms 64 x 2 CTAs", {"max_sms": 64, "ctas_per_sm": 2}),
-                ("max_sms 32 x 2 CTAs", {"max_sms": 32, "ctas_per_sm": 2}),
-                ("max_sms 16 x 2 CTAs", {"max_sms": 16, "ctas_per_sm": 2}),
+    settings = [("ldst, default (grid <= 256 CTAs/SM)", None),
+                ("ldst, max_sms 64 x 2 CTAs", {"max_sms": 64, "ctas_per_sm": 2}),
+                ("ldst, max_sms 32 x 2 CTAs", {"max_sms": 32, "ctas_per_sm": 2}),
+                ("ldst, max_sms 16 x 2 CTAs", {"max_sms": 16, "ctas_per_sm": 2}),
+                ("ldst, max_sms 16 x 1 CTA", {"max_sms": 16, "ctas_per_sm": 1}),
                 ("bulk/TMA, default grid", {"variant": "bulk"}),
-                ("bulk/TMA, max_sms 148 x 1 CTA x 1 thread, 6 stages", {"variant": "bulk", "ctas_per_sm": 1, "stages": 6, "tile_bytes": 32768}),
-                ("bulk/TMA, max_sms 32 x 1 CTA, 6 stages", {"variant": "bulk", "max_sms": 32, "ctas_per_sm": 1, "stages": 6, "tile_bytes": 32768})]
+                ("bulk/TMA, 148 SMs x 1 CTA x 1 thread, 6 stages", {"variant": "bulk", "ctas_per_sm": 1, "stages": 6, "tile_bytes": 32768}),
+                ("bulk/TMA, max_sms 32 x 1 CTA, 6 stages", {"variant": "bulk", "max_sms": 32, "ctas_per_sm": 1, "stages": 6, "tile_bytes": 32768}),
+                ("bulk/TMA, max_sms 32 x 2 CTAs, 3 stages", {"variant": "bulk", "max_sms": 32, "ctas_per_sm": 2, "stages": 3, "tile_bytes": 32768}),
+                ("bulk/TMA, max_sms 16 x 2 CTAs, 3 stages", {"variant": "bulk", "max_sms": 16, "ctas_per_sm": 2, "stages": 3, "tile_bytes": 32768}),
+                ("bulk/TMA, max_sms 16 x 1 CTA, 6 stages", {"variant": "bulk", "max_sms": 16, "ctas_per_sm": 1, "stages": 6, "tile_bytes": 32768})]
     for name, t in settings:
-        plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, t, sc.cuda_stream)
+        plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, t, sc.cuda_stream)
         sc.synchronize()
-        c0, c1 = copy_loop(plan); torch.cuda.synchronize()
-        c0, c1 = copy_loop(plan); torch.cuda.synchronize()
-        copy_alone = gb(c0.elapsed_time(c1))
+        copy_loop(plan, 2); torch.cuda.synchronize()
+        t0 = ev(); cs_ = []
+        t0.record(sc); copy_loop(plan, 3, cs_); torch.cuda.synchronize()
+        copy_ms = t0.elapsed_time(cs_[-1]) / 3
+        n_copy = max(4, int(100.0 / copy_ms))                         # ~100 ms of copying alone
+        t0 = ev(); cs_ = []
+        t0.record(sc); copy_loop(plan, n_copy, cs_); torch.cuda.synchronize()
+        copy_alone = gb(rate_in_window(t0, cs_, 0, 1e9))
+        # both loops ~300 ms of their stand-alone time, started together; every iteration stamps its completion on its
+        # own stream and both rates are read over the SAME window: the middle of the time both streams were busy
+        n_c, n_g = max(6, int(300.0 / copy_ms)), max(20, int(300.0 / gemm_ms))
+        t0 = ev(); gs_, cs_ = [], []
+        t0.record(sg)
+        sc.wait_event(t0)
+        gemm_loop(n_g, gs_)
+        copy_loop(plan, n_c, cs_)
         torch.cuda.synchronize()
-        g0, g1 = gemm_loop()
-        c0, c1 = copy_loop(plan)
-        torch.cuda.synchronize()
-        row = {"setting": name, "tuning": t, "grid": plan.stats["grid"], "copy_alone_GBps": copy_alone,
-               "gemm_alone_TFLOPs": gemm_alone, "copy_corun_GBps": gb(c0.elapsed_time(c1)),
-               "gemm_corun_TFLOPs": tf(g0.elapsed_time(g1)),
-               "copy_loop_ms": c0.elapsed_time(c1), "gemm_loop_ms": g0.elapsed_time(g1)}
+        end = min(t0.elapsed_time(gs_[-1]), t0.elapsed_time(cs_[-1]))
+        lo, hi = 0.15 * end, 0.95 * end
+        st = plan.stats
+        row = {"config": args.config, "setting": name, "tuning": t, "grid": st["grid"], "variant": st["variant"],
+               "mode": st["mode_transfer"], "copy_alone_GBps": copy_alone, "gemm_alone_TFLOPs": gemm_alone,
+               "copy_corun_GBps": gb(rate_in_window(t0, cs_, lo, hi)), "gemm_corun_TFLOPs": tf(rate_in_window(t0, gs_, lo, hi)),
+               "copy_ms_alone": copy_ms, "window_ms": hi - lo}
         rows.append(row)
         print(json.dumps(row), flush=True)
         plan.destroy()
