@@ -140,12 +140,13 @@ def load_peaks() -> tuple:
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-NCU_CAPTURES = {      # workload name -> committed summary of its `ncu --set full` capture (profiles/r01_ncu.md)
-    "cfg2_llama8b_13k": "r01_ncu_full_cfg2_fk_span_ldst.csv",
-    "cfg2_blkthd_13k": "r01_ncu_full_cfg2bm_fk_flat_ldst.csv",
-    "cfg2_llama8b_13k+tables": "r01_ncu_full_cfg2_fk_tables_ldst.csv",
-    "cfg3_batched_8b": "r01_ncu_full_cfg3_fk_span_ldst.csv",
-    "cfg4_hetero_70b": "r01_ncu_full_cfg4_fk_rows_ldst.csv",
+NCU_CAPTURES = {      # workload name -> committed summary of its `ncu --set full` capture (profiles/r02_ncu.md)
+    "cfg2_llama8b_13k": "r02_ncu_full_cfg2_fk_span_ldst.csv",
+    "cfg2_blkthd_13k": "r02_ncu_full_cfg2bm_fk_flat_ldst.csv",
+    "cfg2_llama8b_13k+tables": "r02_ncu_full_cfg2_fk_tables_ldst.csv",
+    "cfg3_batched_8b": "r02_ncu_full_cfg3_fk_span_ldst.csv",
+    "cfg4_hetero_70b": "r02_ncu_full_cfg4_fk_rows_ldst.csv",
+    "cfg4_hetero_70b+bulk": "r02_ncu_full_cfg4_fk_rows_tma.csv",
 }
 
 
@@ -466,7 +467,7 @@ def run_ours(args) -> None:
         line = None
         if rank == 0:
             m["t_ms"] = t_ms
-            wkey = w.name + ("+tables" if args.device_tables else "")
+            wkey = w.name + ("+tables" if args.device_tables else "+bulk" if stats["variant"] == 2 and stats["mode_transfer"] == 2 else "")
             line = {
                 "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
                 "ms_per_step": t_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -40,6 +40,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--requests", type=int, default=24)
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "allocator.json"))
+    ap.add_argument("--cfg3-requests", type=int, default=16, help="requests of configs[2]'s trace moved on the GPU")
     args = ap.parse_args()
     import torch
     from paper_2504_03775_b200 import build as B
@@ -98,6 +99,47 @@ def main():
                        "launches": 1, "segmentwise_memcpy_calls": calls, "segmentwise_memcpy_ms": a.elapsed_time(b)}
         print(policy, json.dumps(out[policy]), flush=True)
         plan.destroy()
+    del src_buf, dst_buf
+    torch.cuda.empty_cache()
+
+    # ---- BASELINE.json configs[2]'s own alloc/free trace, driven by the allocator ----------------
+    # The same seeded trace (earlier tenants fill the pool, a seeded subset finishes, the 64 requests are allocated)
+    # with the block ids chosen (i) by the plain FIFO free list of synth.config3_batched (the config as bench.py runs
+    # it) and (ii) by flowkv_alloc_* on both pools.  All 64 requests are planned on the host (segments per request);
+    # the first `--cfg3-requests` of each are moved on the GPU.
+    out["cfg3_trace"] = {}
+    for policy, alloc in (("fifo_free_list", None), ("segment_allocator", F.Allocator)):
+        w = synth.config3_batched(allocator=alloc)
+        n_src = sum(synth.n_runs(r.src_blocks) for r in w.requests)
+        n_dst = sum(synth.n_runs(r.dst_blocks) for r in w.requests)
+        blocks = sum(len(r.src_blocks) for r in w.requests)
+        fake = 0x7F0000000000
+        hp = F.flowkv_plan_host(P.describe(w.src, w.shape, fake), P.describe(w.dst, w.shape, fake), P.requests_of(w))
+        segs = hp.stats["n_segments"]
+        hp.destroy()
+        w16 = synth.config3_batched(n_requests=args.cfg3_requests, allocator=alloc)
+        dp = P.DevicePools(w16, sentinel_dst=False)
+        plan = dp.plan(F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, None, s)
+        for _ in range(3):
+            plan.transfer(s)
+        ts = []
+        for _ in range(10):
+            a, b = ev(), ev()
+            a.record(); plan.transfer(s); b.record(); torch.cuda.synchronize(); ts.append(a.elapsed_time(b))
+        F.flowkv_baseline_segmentwise(plan, s); torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record(); calls = F.flowkv_baseline_segmentwise(plan, s); b.record(); torch.cuda.synchronize()
+        st16 = plan.stats
+        out["cfg3_trace"][policy] = {
+            "requests": len(w.requests), "blocks": blocks, "mean_src_run_blocks": blocks / n_src,
+            "mean_dst_run_blocks": blocks / n_dst, "aligned_segments": segs, "segments_per_request": segs / len(w.requests),
+            "gpu_requests": len(w16.requests), "gpu_segments": st16["n_segments"], "gpu_payload_bytes": st16["payload_bytes"],
+            "kernel_ms": float(np.median(ts)), "hbm_GBps": 2 * st16["payload_bytes"] / np.median(ts) / 1e6,
+            "segmentwise_memcpy_calls": calls, "segmentwise_memcpy_ms": a.elapsed_time(b)}
+        print("cfg3_trace", policy, json.dumps(out["cfg3_trace"][policy]), flush=True)
+        plan.destroy()
+        del dp
+        torch.cuda.empty_cache()
     os.makedirs(os.path.dirname(args.out), exist_ok=True)
     json.dump(out, open(args.out, "w"), indent=1)
 

@@ -53,8 +53,14 @@ def main():
     in_slots = [P.alloc_bytes(per_layer) for _ in range(2)]
     ev = lambda: torch.cuda.Event(enable_timing=True)
     plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, 0, None, comp.cuda_stream)
-    scratch_bytes = F.flowkv_via_host_scratch_bytes(plan, 16)
+    scratch_bytes = F.flowkv_via_host_scratch_bytes(plan, 0)
     scratch = P.alloc_bytes(scratch_bytes)
+    # device-resident block tables for the plan-free layer-range launches (flowkv_transfer_tables_layers)
+    r0 = w.requests[0]
+    d_st = torch.from_numpy(r0.src_blocks[None, :].copy()).cuda()
+    d_dt = torch.from_numpy(r0.dst_blocks[None, :].copy()).cuda()
+    d_len = torch.tensor([r0.num_tokens], dtype=torch.int32, device="cuda")
+    d_flag = torch.zeros(1, dtype=torch.int32, device="cuda")
     torch.cuda.synchronize()
 
     def prefill_layer():
@@ -90,11 +96,18 @@ def main():
                 done.record(comp)
                 s_out.wait_event(done)
                 F.flowkv_transfer_layers(plan, l, l + 1, s_out.cuda_stream)
+            elif mode == "layerwise_d2d_tables":                         # no host plan: the kernel reads the tables
+                done = torch.cuda.Event()
+                done.record(comp)
+                s_out.wait_event(done)
+                F.flowkv_transfer_tables_layers(dp.src, dp.dst, d_st.data_ptr(), d_dt.data_ptr(), d_len.data_ptr(), 1,
+                                                d_st.shape[1], d_dt.shape[1], r0.num_tokens, l, l + 1, d_flag.data_ptr(),
+                                                None, s_out.cuda_stream)
         e_pre.record(comp)
         if mode == "serial_d2d":
             F.flowkv_transfer(plan, comp.cuda_stream)
         elif mode == "serial_via_host":
-            F.flowkv_transfer_via_host(plan, host.data_ptr(), payload, 16, 0, comp.cuda_stream, scratch.data_ptr(), scratch_bytes)
+            F.flowkv_transfer_via_host(plan, host.data_ptr(), payload, 0, 0, comp.cuda_stream, scratch.data_ptr(), scratch_bytes)
         for st in (s_out, s_in):
             j = torch.cuda.Event()
             j.record(st)
@@ -104,11 +117,11 @@ def main():
         return e0.elapsed_time(e_pre), e0.elapsed_time(e_all)
 
     rows = []
-    for mode in ("prefill_only", "serial_d2d", "layerwise_d2d", "serial_via_host", "layerwise_via_host"):
+    for mode in ("prefill_only", "serial_d2d", "layerwise_d2d", "layerwise_d2d_tables", "serial_via_host", "layerwise_via_host"):
         run(mode)
         best = min((run(mode) for _ in range(args.reps)), key=lambda t: t[1])
         row = {"mode": mode, "prefill_ms": best[0], "total_ms": best[1], "exposed_transfer_ms": best[1] - best[0],
-               "launches_per_request": {"prefill_only": 0, "serial_d2d": 1, "layerwise_d2d": L, "serial_via_host": 32,
+               "launches_per_request": {"prefill_only": 0, "serial_d2d": 1, "layerwise_d2d": L, "layerwise_d2d_tables": L, "serial_via_host": 64,
                                         "layerwise_via_host": 2 * L}[mode]}
         rows.append(row)
         print(json.dumps(row), flush=True)

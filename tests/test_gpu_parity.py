@@ -1001,3 +1001,27 @@ def test_rows_tma_falls_back_where_a_tensor_map_cannot_describe_the_pool():
     exp = np.full(gd.span_bytes(), P.SENTINEL_BYTE, np.uint8)
     O.transfer(P.to_numpy(src_buf), gs, exp, gd, a, b, 29)
     G.assert_same(P.to_numpy(dst_buf), exp, "fallback")
+
+
+def test_bench_starts_its_own_ranks_and_peer_mode_runs_on_one_gpu():
+    """`python bench.py --gpus 2` with no launcher starts 2 ranks itself (one process per rank, torch.distributed
+    rendezvous on 127.0.0.1); --peer makes rank r store into rank (r+1)%2's dst pool through CUDA IPC; --same-device puts
+    both ranks on cuda:0 with a gloo control plane (there is one GPU here).  A functional check of the multi-rank
+    path, not a scaling number: the line must report both ranks and one launch per step per rank 0."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ)
+    for k in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT"):
+        env.pop(k, None)
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--same-device", "--peer", "--config", "cfg1",
+                          "--steps", "10", "--warmup", "3", "--no-e2e", "--no-baselines", "--no-cpu-baseline"],
+                         capture_output=True, text=True, timeout=600, env=env, cwd=root)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, out.stdout
+    j = json.loads(lines[0])
+    assert j["n_gpus"] == 2 and j["gpu_launches"] == 10 and j["launches_per_batch"] == 1.0
+    assert "CUDA IPC" in j["config"]["dst"]
