@@ -26,7 +26,7 @@
  * tables == memcmp, untouched-byte sentinels, all 65,536 16-bit patterns,
  * 1-, 4- and 8-byte elements against numpy item views (the generic branch of
  * okv_copy_elem), all 256 byte codes and fp32 NaN payloads,
- * pack∘unpack identity, layer windows == planes cut out of the wire format,
+ * pack∘unpack identity, layer windows and plane windows == planes cut out of the wire format,
  * brute-force minimal partition count on tiny tables,
  * the paper's "fully contiguous => 1 transfer" and
  * "calls per block = L x 2", hand-worked fixtures in tests/golden/.
@@ -172,6 +172,49 @@ int okv_unpack_window(const uint8_t* window, uint64_t req_tok_off, uint8_t* dst,
           for (uint32_t d = 0; d < dp->head_dim; ++d)
             okv_copy_elem(dst + okv_addr(dp, l, c, db, dof, h, d),
                           window + okv_window_addr(dp, w0, w1, req_tok_off, T, l, c, t, h, d), e);
+  }
+  return 0;
+}
+
+/* Plane-window wire format (reading A21): the same idea one level finer — a message that carries only the
+ * planes [p0,p1), plane = 2*layer + (0 for K, 1 for V), in wire order:
+ *   window[request][plane - p0][token][head][dim], requests concatenated,
+ *   request r starting at byte req_tok_off * (p1-p0)*Hkv*Dh*e.
+ * The planes [2*w0, 2*w1) are the layer window [w0,w1) of okv_pack_window.  (The chunked pinned-host pipeline cuts a
+ * transfer into such messages when it wants more chunks than the model has layers.) */
+static inline int64_t okv_planes_addr(const okv_pool* p, uint32_t p0, uint32_t p1, uint64_t req_tok_off, uint32_t T,
+                                      uint32_t plane, uint32_t t, uint32_t h, uint32_t d) {
+  int64_t bpt = (int64_t)(p1 - p0) * p->num_kv_heads * p->head_dim * p->elem_bytes;
+  int64_t idx = ((((int64_t)(plane - p0) * T + t) * p->num_kv_heads + h) * p->head_dim + d);
+  return (int64_t)req_tok_off * bpt + idx * p->elem_bytes;
+}
+
+int okv_pack_planes(const uint8_t* src, const okv_pool* sp, const int32_t* src_tab, uint32_t T,
+                    uint8_t* window, uint64_t req_tok_off, uint32_t p0, uint32_t p1) {
+  const uint32_t e = sp->elem_bytes;
+  for (uint32_t t = 0; t < T; ++t) {
+    int64_t sb = src_tab[t / sp->block_size]; uint32_t so = t % sp->block_size;
+    if (sb < 0 || sb >= (int64_t)sp->num_blocks) return -1;
+    for (uint32_t plane = p0; plane < p1; ++plane)
+      for (uint32_t h = 0; h < sp->num_kv_heads; ++h)
+        for (uint32_t d = 0; d < sp->head_dim; ++d)
+          okv_copy_elem(window + okv_planes_addr(sp, p0, p1, req_tok_off, T, plane, t, h, d),
+                        src + okv_addr(sp, plane / 2, plane % 2, sb, so, h, d), e);
+  }
+  return 0;
+}
+
+int okv_unpack_planes(const uint8_t* window, uint64_t req_tok_off, uint8_t* dst, const okv_pool* dp,
+                      const int32_t* dst_tab, uint32_t T, uint32_t p0, uint32_t p1) {
+  const uint32_t e = dp->elem_bytes;
+  for (uint32_t t = 0; t < T; ++t) {
+    int64_t db = dst_tab[t / dp->block_size]; uint32_t dof = t % dp->block_size;
+    if (db < 0 || db >= (int64_t)dp->num_blocks) return -1;
+    for (uint32_t plane = p0; plane < p1; ++plane)
+      for (uint32_t h = 0; h < dp->num_kv_heads; ++h)
+        for (uint32_t d = 0; d < dp->head_dim; ++d)
+          okv_copy_elem(dst + okv_addr(dp, plane / 2, plane % 2, db, dof, h, d),
+                        window + okv_planes_addr(dp, p0, p1, req_tok_off, T, plane, t, h, d), e);
   }
   return 0;
 }

@@ -64,6 +64,10 @@ def _load():
         lib.okv_unpack_window.restype = C.c_int
         lib.okv_unpack_window.argtypes = [u8p, C.c_uint64, u8p, C.POINTER(_Pool), i32p, C.c_uint32,
                                           C.c_uint32, C.c_uint32]
+        lib.okv_pack_planes.restype = C.c_int
+        lib.okv_pack_planes.argtypes = lib.okv_pack_window.argtypes
+        lib.okv_unpack_planes.restype = C.c_int
+        lib.okv_unpack_planes.argtypes = lib.okv_unpack_window.argtypes
         lib.okv_align.restype = C.c_uint64
         lib.okv_align.argtypes = [i32p, C.c_uint32, i32p, C.c_uint32, C.c_uint32, u32p, u32p, C.c_uint64]
         lib.okv_blockwise_calls.restype = C.c_uint64
@@ -202,6 +206,27 @@ def unpack_window(window: np.ndarray, req_tok_off: int, dst: np.ndarray, dp: Poo
     assert len(dt) * dp.block_size >= T
     rc = _load().okv_unpack_window(_u8(window, False), req_tok_off, _u8(dst, True), C.byref(dp._c()),
                                    dt.ctypes.data, T, w0, w1)
+    if rc != 0:
+        raise ValueError("oracle: block id out of range")
+
+
+def pack_planes(src: np.ndarray, sp: PoolGeom, src_tab, T: int, window: np.ndarray, req_tok_off: int,
+                p0: int, p1: int) -> None:
+    """Planes [p0,p1) (plane = 2*layer + kv) of one request into a buffer that holds only those planes (A21)."""
+    st = _tab(src_tab)
+    assert len(st) * sp.block_size >= T and 0 <= p0 <= p1 <= 2 * sp.num_layers
+    rc = _load().okv_pack_planes(_u8(src, False), C.byref(sp._c()), st.ctypes.data, T, _u8(window, True),
+                                 req_tok_off, p0, p1)
+    if rc != 0:
+        raise ValueError("oracle: block id out of range")
+
+
+def unpack_planes(window: np.ndarray, req_tok_off: int, dst: np.ndarray, dp: PoolGeom, dst_tab, T: int,
+                  p0: int, p1: int) -> None:
+    dt = _tab(dst_tab)
+    assert len(dt) * dp.block_size >= T and 0 <= p0 <= p1 <= 2 * dp.num_layers
+    rc = _load().okv_unpack_planes(_u8(window, False), req_tok_off, _u8(dst, True), C.byref(dp._c()),
+                                   dt.ctypes.data, T, p0, p1)
     if rc != 0:
         raise ValueError("oracle: block id out of range")
 

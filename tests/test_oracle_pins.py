@@ -553,3 +553,70 @@ def test_all_256_byte_patterns_and_fp32_specials_survive():
     O.transfer(src4.view(np.uint8), g4, dst4, g4, perm, np.arange(NB), NB * BS)
     s4, d4 = Hh.logical_view(src4.view(np.uint8), "lkbthd", L, NB, BS, H, 4, 4), Hh.logical_view(dst4, "lkbthd", L, NB, BS, H, 4, 4)
     assert np.array_equal(d4, s4[:, :, perm])
+
+
+# ---------------------------------------------------------------------------------------
+# plane windows (reading A21): the wire format cut at plane granularity
+# ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("layout", ["lkbthd", "blkhtd"])
+def test_plane_window_equals_planes_cut_out_of_the_wire_format(layout):
+    """A window [p0,p1) of planes (plane = 2*layer + kv) is numpy's gather restricted to those planes == the slab of
+    planes [p0,p1) of each request's region of the (pinned) wire format; even-aligned plane windows ARE layer windows;
+    unpacking disjoint plane windows rebuilds unpack of the whole.  Catches: K|V order inside a layer (plane % 2),
+    a plane index not rebased to p0, a per-token size that still counts whole layers."""
+    rng = np.random.default_rng(28)
+    L, H, D, NB, BS = 3, 2, 8, 12, 4
+    g = _geom(layout, L, H, D, NB, BS)
+    src = _rand_pool(rng, g.span_bytes())
+    Ts = [7, 12, 0, 5]
+    perm = rng.permutation(NB)
+    tabs, off = [], 0
+    for T in Ts:
+        nb = -(-T // BS)
+        tabs.append(perm[off:off + nb]); off += nb
+    tokb = H * D * 2
+    sv = Hh.logical_view(src, layout, L, NB, BS, H, D).reshape(2 * L, NB, BS, H, D)      # [plane, block, token, head, dim]
+    full = np.zeros(sum(Ts) * g.bytes_per_token, np.uint8)
+    tok_off = 0
+    for T, tab in zip(Ts, tabs):
+        O.pack(src, g, tab, T, full, tok_off)
+        tok_off += T
+    for p0, p1 in [(0, 6), (1, 2), (1, 4), (3, 6), (5, 5), (2, 4)]:
+        win = np.full(sum(Ts) * (p1 - p0) * tokb + 16, SENT, np.uint8)
+        exp_parts, cut_parts, tok_off = [], [], 0
+        for T, tab in zip(Ts, tabs):
+            O.pack_planes(src, g, tab, T, win, tok_off, p0, p1)
+            exp_parts.append(sv[p0:p1][:, tab].reshape(p1 - p0, len(tab) * BS, H, D)[:, :T].reshape(-1))
+            base = tok_off * g.bytes_per_token
+            cut_parts.append(full[base + p0 * T * tokb: base + p1 * T * tokb])
+            tok_off += T
+        body = win[:-16]
+        assert np.array_equal(body.view(np.uint16), np.concatenate(exp_parts)) and np.array_equal(body, np.concatenate(cut_parts))
+        assert np.all(win[-16:] == SENT)
+        if p0 % 2 == 0 and p1 % 2 == 0:
+            lw = np.zeros(body.size, np.uint8)
+            tok_off = 0
+            for T, tab in zip(Ts, tabs):
+                O.pack_window(src, g, tab, T, lw, tok_off, p0 // 2, p1 // 2)
+                tok_off += T
+            assert np.array_equal(body, lw)
+    gd = _geom("blkhtd" if layout == "lkbthd" else "lkbthd", L, H, D, NB, BS * 2)
+    dperm = rng.permutation(NB)
+    d1, d2 = np.full(gd.span_bytes(), SENT, np.uint8), np.full(gd.span_bytes(), SENT, np.uint8)
+    for p0, p1 in [(0, 1), (1, 5), (5, 6)]:
+        win = np.zeros(sum(Ts) * (p1 - p0) * tokb, np.uint8)
+        tok_off = 0
+        for T, tab in zip(Ts, tabs):
+            O.pack_planes(src, g, tab, T, win, tok_off, p0, p1)
+            tok_off += T
+        tok_off = doff = 0
+        for T, tab in zip(Ts, tabs):
+            nb = -(-T // (BS * 2))
+            O.unpack_planes(win, tok_off, d1, gd, dperm[doff:doff + nb], T, p0, p1)
+            tok_off += T; doff += nb
+    tok_off = doff = 0
+    for T, tab in zip(Ts, tabs):
+        nb = -(-T // (BS * 2))
+        O.unpack(full, tok_off, d2, gd, dperm[doff:doff + nb], T)
+        tok_off += T; doff += nb
+    assert np.array_equal(d1, d2)
