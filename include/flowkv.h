@@ -261,9 +261,12 @@ FLOWKV_API flowkv_status flowkv_unpack_window(const flowkv_plan_t* plan, const v
  *     (flowkv_pack_window, on `stream`), moved D2H and H2D by cudaMemcpyAsync on two copy queues of their own, and
  *     unpacked from a second slot (flowkv_unpack_window, on a fourth queue), so neither engine ever waits behind a
  *     kernel.  On B200 the copy engines sustain ~50 GB/s in both directions at once where SM loads over PCIe drop
- *     to ~38 GB/s.  Default 32 chunks (the first outbound and the last inbound chunk cross the link alone).
- *     host_staging then holds the chunks back to back, chunk c = the layer window [L*c/n, L*(c+1)/n) at byte
- *     offset flowkv_window_bytes(0, L*c/n) (== the wire format when n_chunks == 1).  device_scratch: DEVICE
+ *     to ~38 GB/s.  n_chunks is clamped to [1, 2L]; default 64 (the first outbound and the last inbound chunk cross
+ *     the link alone, so many small chunks win).  host_staging then holds the chunks back to back: with n <= L
+ *     chunk c = the layer window [L*c/n, L*(c+1)/n) at byte offset flowkv_window_bytes(0, L*c/n) (== the wire
+ *     format when n_chunks == 1); with n > L chunk c = the PLANES [2L*c/n, 2L*(c+1)/n) (plane = 2*layer + K|V) in
+ *     wire order [request][plane - first][token][head][dim] at byte offset total_tokens * first * Hkv*Dh*e — a layer
+ *     window cut once more between K and V.  device_scratch: DEVICE
  *     pointer, 256-B aligned, scratch_bytes >= flowkv_via_host_scratch_bytes(plan, n_chunks) (4 slots of the
  *     largest chunk); caller-owned, reusable once `stream` has passed this call.  `ctas_per_kernel`: 0 = the
  *     plan's grid.

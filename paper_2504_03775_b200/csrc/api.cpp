@@ -557,22 +557,26 @@ Side pool_side(const flowkv_pool& p) {
 
 // A dense staging buffer that holds the layer window [w0, w1) in wire order (A12).  The whole wire format
 // is the window [0, L).
-Side dense_side(const void* staging, const Geometry& g, uint32_t w0, uint32_t w1) {
+// A dense buffer that holds the PLANES [p0, p1) (plane = 2*layer + kv) in wire order (A21).
+Side dense_planes(const void* staging, const Geometry& g, uint32_t p0, uint32_t p1) {
   Side s{};
   s.base = (char*)staging;
-  s.s_layer = 2ll * (w1 - w0) * g.tok_bytes;   // bytes per token of the window
-  s.s_kv = 0;                                  // plane stride comes from the chunk's req_tokens
+  s.s_layer = (int64_t)(p1 - p0) * g.tok_bytes;   // bytes per token of the window
+  s.s_kv = 0;                                     // plane stride comes from the chunk's req_tokens
   s.s_token = g.tok_bytes;
   s.s_head = g.row_bytes;
   s.dense = 1;
-  s.plane0 = 2 * w0;
+  s.plane0 = p0;
   return s;
 }
+Side dense_side(const void* staging, const Geometry& g, uint32_t w0, uint32_t w1) { return dense_planes(staging, g, 2 * w0, 2 * w1); }
 Side dense_side(const void* staging, const Geometry& g) { return dense_side(staging, g, 0, g.L); }
 
 struct RunOpts {
   bool ranged = false;                       // false: all layers
   uint32_t layer_begin = 0, layer_end = 0;   // [begin, end) when ranged
+  bool by_planes = false;                    // ranged by PLANES [plane_begin, plane_end) instead (via-host chunks, A21)
+  uint32_t plane_begin = 0, plane_end = 0;
   uint32_t max_grid = 0;                     // 0 = the plan's launch shape
 };
 
@@ -581,7 +585,9 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   if (!pl->on_device) return fail(FLOWKV_ERR_UNSUPPORTED, "plan was built by flowkv_plan_host and cannot run");
   const uint32_t l0 = ro.ranged ? ro.layer_begin : 0, l1 = ro.ranged ? ro.layer_end : pl->g.L;
   if (l0 > l1 || l1 > pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "layer range outside [0, num_layers]");
-  if (op.sched.chunks.empty() || l0 == l1) return FLOWKV_OK;       // A11: nothing to move, zero launches
+  const uint32_t p0 = ro.by_planes ? ro.plane_begin : 2 * l0, p1 = ro.by_planes ? ro.plane_end : 2 * l1;
+  if (p0 > p1 || p1 > 2 * pl->g.L) return fail(FLOWKV_ERR_INVALID_ARG, "plane range outside [0, 2*num_layers]");
+  if (op.sched.chunks.empty() || p0 == p1) return FLOWKV_OK;       // A11: nothing to move, zero launches
   if ((cudaStream_t)stream != pl->stream && pl->staging.ev && !pl->upload_seen_done.load(std::memory_order_acquire)) {
     // A stream other than the plan's own has not been ordered after the plan upload yet.  Once the upload is known
     // to have finished no edge is needed — which also lets a long-lived plan be captured into a CUDA graph on any
@@ -614,7 +620,7 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   kp.n_flat = op.sched.n_flat;
   kp.flat_shift = op.sched.flat_shift;
   kp.flat_tile = op.sched.flat_tile;
-  if (mode == MODE_FLAT && (l0 != 0 || l1 != pl->g.L)) {
+  if (mode == MODE_FLAT && (p0 != 0 || p1 != 2 * pl->g.L)) {
     // a layer range of a block-major pool is not one byte range per block run: use the plan's
     // complete rows-mode schedule (third part of the chunk list)
     mode = MODE_ROWS;
@@ -622,8 +628,8 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
     kp.n_chunks = (uint32_t)op.sched.chunks.size() - first;
     kp.n_flat = 0;
   }
-  kp.n_planes = 2 * (l1 - l0);
-  kp.plane0 = 2 * l0;
+  kp.n_planes = p1 - p0;
+  kp.plane0 = p0;
   kp.n_tiles = (kp.n_flat << kp.flat_shift) + kp.n_chunks * kp.n_planes;
   kp.row_bytes = pl->g.row_bytes;
   kp.heads = pl->g.Hkv;
@@ -832,16 +838,27 @@ flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, 
 namespace {
 uint32_t via_host_chunks(const flowkv_plan_t* pl, uint32_t n_chunks, bool engines) {
   // defaults measured on B200 (profiles/r02_host_route.md): the first outbound and the last inbound chunk cross the
-  // link alone, so the copy-engine pipeline wants many small chunks; the direct mode pays a kernel pair per chunk
-  if (n_chunks == 0) n_chunks = engines ? 32 : 16;
-  return std::max<uint32_t>(1, std::min(n_chunks, pl->g.L));
+  // link alone, so the copy-engine pipeline wants many small chunks (up to one per plane); the direct mode pays a
+  // kernel pair per chunk and stays at layer granularity
+  if (n_chunks == 0) n_chunks = engines ? 64 : 16;
+  return std::max<uint32_t>(1, std::min(n_chunks, engines ? 2 * pl->g.L : pl->g.L));
 }
+// Chunk c of n covers the planes [first, last): whole layers while n <= L (the layer windows of A20), single planes
+// or small groups of planes beyond that (plane windows, A21).
+void via_host_chunk_planes(const flowkv_plan_t* pl, uint32_t n_chunks, uint32_t c, uint32_t& first, uint32_t& last) {
+  const uint64_t L = pl->g.L;
+  if (n_chunks <= L) { first = 2 * (uint32_t)(L * c / n_chunks); last = 2 * (uint32_t)(L * (c + 1) / n_chunks); }
+  else               { first = (uint32_t)(2 * L * c / n_chunks); last = (uint32_t)(2 * L * (c + 1) / n_chunks); }
+}
+uint64_t planes_bytes(const flowkv_plan_t* pl, uint32_t p0, uint32_t p1) { return pl->total_tokens * (uint64_t)(p1 - p0) * pl->g.tok_bytes; }
 uint64_t via_host_slot_bytes(const flowkv_plan_t* pl, uint32_t n_chunks) {
-  const uint32_t L = pl->g.L;
-  uint32_t most = 0;                     // layers of the largest chunk
-  for (uint32_t c = 0; c < n_chunks; ++c)
-    most = std::max<uint32_t>(most, (uint32_t)((uint64_t)L * (c + 1) / n_chunks - (uint64_t)L * c / n_chunks));
-  return (window_bytes(pl, 0, most) + 255) & ~255ull;
+  uint32_t most = 0;                     // planes of the largest chunk
+  for (uint32_t c = 0; c < n_chunks; ++c) {
+    uint32_t a, b;
+    via_host_chunk_planes(pl, n_chunks, c, a, b);
+    most = std::max(most, b - a);
+  }
+  return (planes_bytes(pl, 0, most) + 255) & ~255ull;
 }
 }  // namespace
 
@@ -916,7 +933,8 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   //   q_d2h     cudaMemcpyAsync   out slot -> host chunk             waits: pack k
   //   q_h2d     cudaMemcpyAsync   host chunk -> in slot 2 + (k & 1)  waits: D2H k; unpack k-2 has drained that slot
   //   q_unpack  unpack kernels    in slot -> pool                    waits: H2D k
-  // Chunk k is its own dense message (layer window [l0,l1), A20) at host offset window_bytes(0,l0).  While chunk k
+  // Chunk k is its own dense message (a layer window, A20, or — with more chunks than layers — a plane window, A21)
+  // at the host offset of its first plane.  While chunk k
   // crosses the link outbound, chunk k-1 crosses it inbound and chunks k+1 / k-2 are packed / unpacked in HBM.
   ro.max_grid = ctas_per_kernel;
   char* scratch = (char*)device_scratch;
@@ -926,17 +944,21 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
   cudaEvent_t* unpacked = arrived + n_chunks;
   uint32_t k = 0;                                           // non-empty chunks so far
   int64_t prev1 = -1, prev2 = -1;                           // chunk indices of the two previous non-empty chunks
+  ro.by_planes = true;
+  ro.layer_begin = 0;
+  ro.layer_end = L;
   for (uint32_t c = 0; c < n_chunks; ++c) {
-    const uint32_t l0 = (uint32_t)((uint64_t)L * c / n_chunks), l1 = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
-    if (l0 == l1) continue;
-    ro.layer_begin = l0;
-    ro.layer_end = l1;
-    const uint64_t wb = window_bytes(pl, l0, l1);
+    uint32_t p0, p1;
+    via_host_chunk_planes(pl, n_chunks, c, p0, p1);
+    if (p0 == p1) continue;
+    ro.plane_begin = p0;
+    ro.plane_end = p1;
+    const uint64_t wb = planes_bytes(pl, p0, p1);
     char* out_slot = scratch + (k & 1) * slot;
     char* in_slot = scratch + (2 + (k & 1)) * slot;
-    char* host = (char*)host_staging + window_bytes(pl, 0, l0);
+    char* host = (char*)host_staging + planes_bytes(pl, 0, p0);
     if (prev2 >= 0) FK_TRY(cudaStreamWaitEvent(s, landed[prev2], 0), "cudaStreamWaitEvent");          // out slot free again
-    st = run(pl, pl->pack, pool_side(pl->src), dense_side(out_slot, pl->g, l0, l1), pl->pack.shape.vec_bytes, s, ro);
+    st = run(pl, pl->pack, pool_side(pl->src), dense_planes(out_slot, pl->g, p0, p1), pl->pack.shape.vec_bytes, s, ro);
     if (st != FLOWKV_OK) return st;
     FK_TRY(cudaEventRecord(packed[c], s), "cudaEventRecord");
     FK_TRY(cudaStreamWaitEvent(vc.q_d2h, packed[c], 0), "cudaStreamWaitEvent");
@@ -947,7 +969,7 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     FK_TRY(cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, vc.q_h2d), "cudaMemcpyAsync(H2D)");
     FK_TRY(cudaEventRecord(arrived[c], vc.q_h2d), "cudaEventRecord");
     FK_TRY(cudaStreamWaitEvent(vc.q_unpack, arrived[c], 0), "cudaStreamWaitEvent");
-    st = run(pl, pl->unpack, dense_side(in_slot, pl->g, l0, l1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
+    st = run(pl, pl->unpack, dense_planes(in_slot, pl->g, p0, p1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
     if (st != FLOWKV_OK) return st;
     FK_TRY(cudaEventRecord(unpacked[c], vc.q_unpack), "cudaEventRecord");
     prev2 = prev1;

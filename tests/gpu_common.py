@@ -94,3 +94,15 @@ def oracle_pack_window(w: synth.Workload, src_np: np.ndarray, l0: int, l1: int) 
         O.pack_window(src_np, gs, r.src_blocks, r.num_tokens, out, off, l0, l1)
         off += r.num_tokens
     return out
+
+
+def oracle_pack_planes(w: synth.Workload, src_np: np.ndarray, p0: int, p1: int) -> np.ndarray:
+    """The oracle's plane window [p0,p1) of the whole batch (oracle/flowkv_oracle.c okv_pack_planes, reading A21)."""
+    gs = geom(w.src, w.shape)
+    tokb = w.shape.num_kv_heads * w.shape.head_dim * w.shape.elem_bytes
+    out = np.full(w.total_tokens * (p1 - p0) * tokb, P.SENTINEL_BYTE, np.uint8)
+    off = 0
+    for r in w.requests:
+        O.pack_planes(src_np, gs, r.src_blocks, r.num_tokens, out, off, p0, p1)
+        off += r.num_tokens
+    return out

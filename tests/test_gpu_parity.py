@@ -519,7 +519,7 @@ def test_layer_window_pack_unpack(w_fn):
 
 
 @pytest.mark.parametrize("small", [False, True])
-@pytest.mark.parametrize("n_chunks,ctas", [(0, 0), (1, 0), (4, 8), (100, 0)])
+@pytest.mark.parametrize("n_chunks,ctas", [(0, 0), (1, 0), (4, 8), (6, 0), (9, 4), (100, 0)])
 def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas, small):
     """Copy-engine mode of flowkv_transfer_via_host: pack_window -> D2H memcpy -> H2D memcpy -> unpack_window per
     layer chunk through caller-provided device scratch.  dst == oracle transfer; the host buffer holds the chunks
@@ -546,10 +546,14 @@ def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas, small):
     n0 = F.flowkv_launch_count()
     F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, n_chunks, ctas, stream.cuda_stream, scratch.data_ptr(), sb)
     stream.synchronize()
-    chunks = min(n_chunks, L) if n_chunks else L          # auto = min(L, 16)
+    chunks = min(n_chunks, 2 * L) if n_chunks else min(64, 2 * L)      # clamped to one chunk per plane
     assert F.flowkv_launch_count() - n0 == 2 * chunks
     G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host (copy engines): dst")
-    exp_host = np.concatenate([G.oracle_pack_window(w, src_np, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
+    if chunks <= L:       # layer windows (A20)
+        exp_host = np.concatenate([G.oracle_pack_window(w, src_np, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
+    else:                 # more chunks than layers: plane windows (A21), the oracle's okv_pack_planes
+        exp_host = np.concatenate([G.oracle_pack_planes(w, src_np, 2 * L * c // chunks, 2 * L * (c + 1) // chunks)
+                                   for c in range(chunks)])
     G.assert_same(host.numpy(), exp_host, "via host (copy engines): chunked wire bytes")
     plan.destroy()
 
