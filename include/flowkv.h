@@ -136,9 +136,10 @@ typedef struct {
   uint32_t tile_order;      /* 0 = auto, 1 = plane-major (all tiles of plane 0, then plane 1, ...), 2 = chunk-major */
   uint32_t cache_hint;      /* ldst: 0 = auto, 1 = default caching, 2 = L1::no_allocate, 3 = + L2::evict_first */
   uint32_t stages;          /* bulk: ring depth (0 = auto; 2..16)                                   */
-  uint32_t plan_in_params;  /* 0 = auto: a plan whose schedules have <= 96 entries each is passed in the kernel
-                             *     parameters (no device allocation, no upload; plan_device_bytes == 0; a 512-byte
-                             *     form serves schedules of <= 16 entries, a 3 KiB form the rest);
+  uint32_t plan_in_params;  /* 0 = auto: a plan whose schedules have <= 512 entries each is passed in the kernel
+                             *     parameters (no device allocation, no upload, no event, no free: one stream call per
+                             *     step; plan_device_bytes == 0).  Four parameter forms — 16 entries (512 B), 96
+                             *     (3 KiB), 256 (8 KiB), 512 (16 KiB) — the smallest that fits is used per launch;
                              * 1 = always upload                                                    */
   uint32_t _reserved[2];
 } flowkv_tuning;
@@ -344,7 +345,8 @@ FLOWKV_API const char* flowkv_last_error(void);          /* thread-local text of
 FLOWKV_API uint64_t flowkv_launch_count(void);
 /* Number of CUDA runtime calls this library has made that put work on a stream or (de)allocate stream-ordered
  * memory — kernel launches, cudaMemcpyAsync, cudaMallocAsync / cudaFreeAsync, event records and waits
- * (monotonic).  A small plan's whole step (plan + transfer + destroy) is 1 such call; an uploaded plan's is 6. */
+ * (monotonic).  A plan of <= 512 schedule entries makes 1 such call per step (plan + transfer + destroy: the
+ * launch); an uploaded plan's step makes 6. */
 FLOWKV_API uint64_t flowkv_api_call_count(void);
 
 /* ---- comparison baselines (BASELINE.json north_star; they are NOT the product path) ----------

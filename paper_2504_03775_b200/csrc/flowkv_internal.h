@@ -59,11 +59,14 @@ struct Side {            // one end of a copy as the kernel sees it
   uint32_t plane0;       // dense side: first plane of the layer window the buffer holds (0 = whole wire format)
 };
 
-// Plans whose every schedule has at most this many entries pass them in the kernel parameters
-// (3 KiB of the 4 KiB parameter space) instead of uploading them.  Parameter bytes cost launch time
-// (measured: ~1 us for 3 KiB), so schedules of <= kInlineChunksSmall entries use a 512-byte form.
-constexpr uint32_t kInlineChunks = 96;
-constexpr uint32_t kInlineChunksSmall = 16;
+// Plans whose every schedule has at most kInlineChunks entries pass them in the kernel parameters instead of
+// uploading them (CUDA >= 12.1 allows 32 KiB of parameters): no allocation, no upload, no cross-stream event, no
+// stream-ordered free — the whole step is ONE stream call.  Parameter bytes cost launch time (measured: ~1 us for
+// 3 KiB), so four forms exist — 16 entries (512 B), 96 (3 KiB), 256 (8 KiB), 512 (16 KiB) — and a launch uses the
+// smallest that holds its schedule.  Measured on configs[1] (478 entries, 16 KiB form): call-to-done latency
+// 0.558 -> 0.540 ms, pipelined step 0.5243 -> 0.5232 ms, stream calls per step 6 -> 1.
+constexpr uint32_t kInlineChunks = 512;
+constexpr uint32_t kInlineTiers[4] = {16, 96, 256, 512};
 
 struct KernelParams {
   Side         src, dst;

@@ -28,6 +28,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <new>
 #include <utility>
 
 #include "flowkv_internal.h"
@@ -629,19 +630,32 @@ static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const La
   return (int)launch_ldst<16, 8, CS>(mode, kp, cs, ls, (int)ls.hint, st);
 }
 
+// The parameter block of the larger forms (8-16 KiB) is built on the heap, not on the stack of every launch.
+template <uint32_t N>
+static int launch_inline(Mode mode, const KernelParams& kp, const Chunk* host_chunks, uint32_t n, const LaunchShape& ls,
+                         cudaStream_t st, const RowsTma* tma) {
+  if (N <= 96) {
+    ParamChunks<N> pc;
+    memcpy(pc.c, host_chunks, (size_t)n * sizeof(Chunk));
+    return launch_with(mode, kp, pc, ls, st, tma);
+  }
+  ParamChunks<N>* pc = new (std::nothrow) ParamChunks<N>;
+  if (!pc) return (int)cudaErrorMemoryAllocation;
+  memcpy(pc->c, host_chunks, (size_t)n * sizeof(Chunk));
+  const int rc = launch_with(mode, kp, *pc, ls, st, tma);
+  delete pc;
+  return rc;
+}
+
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
                 uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma) {
   cudaStream_t st = (cudaStream_t)stream;
   if (host_chunks) {                       // small plan: the schedule rides in the kernel parameters
     if (n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
-    if (n_host_chunks <= kInlineChunksSmall) {
-      ParamChunks<kInlineChunksSmall> pc;
-      memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
-      return launch_with(mode, kp, pc, ls, st, tma);
-    }
-    ParamChunks<kInlineChunks> pc;
-    memcpy(pc.c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
-    return launch_with(mode, kp, pc, ls, st, tma);
+    if (n_host_chunks <= kInlineTiers[0]) return launch_inline<kInlineTiers[0]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
+    if (n_host_chunks <= kInlineTiers[1]) return launch_inline<kInlineTiers[1]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
+    if (n_host_chunks <= kInlineTiers[2]) return launch_inline<kInlineTiers[2]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
+    return launch_inline<kInlineTiers[3]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
   }
   GlobalChunks gc{device_chunks};
   return launch_with(mode, kp, gc, ls, st, tma);

@@ -447,20 +447,21 @@ def test_baselines_on_block_major_pools_count_calls():
     G.assert_same(P.to_numpy(dp.dst_buf), exp, "segmentwise baseline, block-major")
 
 
-@pytest.mark.parametrize("n_blocks", [15, 16, 17, 95, 96, 97])
+@pytest.mark.parametrize("n_blocks", [15, 16, 17, 95, 96, 97, 255, 256, 257, 511, 512, 513])
 @pytest.mark.parametrize("variant", ["ldst", "bulk"])
 def test_small_plans_travel_in_kernel_params(n_blocks, variant):
-    """Step a4 'kernel params when tiny': a plan whose schedules have <= 96 entries is never uploaded
-    (plan_device_bytes == 0) — transfer, pack and unpack read their entries from the parameter space;
-    one entry more and the plan is uploaded as usual.  Same bytes either way."""
+    """Step a4 'kernel params when small': a plan whose schedules have <= 512 entries is never uploaded
+    (plan_device_bytes == 0) — transfer, pack and unpack read their entries from the parameter space, in the
+    smallest of four forms (16 / 96 / 256 / 512 entries) that holds them; one entry more and the plan is uploaded
+    as usual.  Both sides of every form boundary; same bytes either way."""
     T = n_blocks * 16 - 3
     w = synth.make_workload("inparams", 35, synth.Shape(2, 2, 64, "fp16"), [T],
-                            "lkbthd", 16, ("permutation",), 256, "lkbthd", 16, ("contiguous",), 128, "uniform")
+                            "lkbthd", 16, ("permutation",), 1024, "lkbthd", 16, ("contiguous",), 600, "uniform")
     tuning = {"variant": variant, "tile_bytes": 4096}
     dp, plan, exp = G.run_transfer_and_check(w, tuning, fill="bits")
     st = plan.stats
     if st["n_chunks_transfer"] == n_blocks:          # the seeded permutation had no accidental +1 neighbours
-        assert (st["plan_device_bytes"] == 0) == (n_blocks <= 96)
+        assert (st["plan_device_bytes"] == 0) == (n_blocks <= 512)
     src_np = P.to_numpy(dp.src_buf)
     nbytes = st["staging_bytes"]
     staging = P.alloc_bytes(nbytes)
