@@ -207,6 +207,24 @@ def test_no_device_means_loud_failure_not_fallback():
     with pytest.raises(F.FlowKVError) as ei:
         F.flowkv_plan(p, p, [F.Request(4, np.asarray([0], np.int32), np.asarray([1], np.int32))])
     assert ei.value.status == F.FLOWKV_ERR_CUDA
+    # the plan-free calls validate on the host first, then need a device: no silent success, no CPU path
+    for call in (lambda: F.flowkv_transfer_tables(p, p, FAKE, FAKE, FAKE, 1, 1, 1, 4),
+                 lambda: F.flowkv_transfer_tables_layers(p, p, FAKE, FAKE, FAKE, 1, 1, 1, 4, 0, 1),
+                 lambda: F.flowkv_pack_tables(p, FAKE, FAKE, 1, 1, 4, FAKE, 1 << 20, 0, 1),
+                 lambda: F.flowkv_unpack_tables(p, FAKE, FAKE, 1, 1, 4, FAKE, 1 << 20, 0, 1)):
+        with pytest.raises(F.FlowKVError) as ei:
+            call()
+        assert ei.value.status == F.FLOWKV_ERR_CUDA
+    with pytest.raises(F.FlowKVError) as ei:       # argument errors come before any device call
+        F.flowkv_transfer_tables_layers(p, p, FAKE, FAKE, FAKE, 1, 1, 1, 4, 2, 1)
+    assert ei.value.status == F.FLOWKV_ERR_INVALID_ARG
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_transfer_tables(p, p, FAKE, FAKE, FAKE, 1, 1, 1, 400)      # tables too short for max_tokens
+    assert ei.value.status == F.FLOWKV_ERR_TABLE_LEN
+    for thr in (32, 64):       # threads below the default group with the group on auto must not divide by zero
+        with pytest.raises(F.FlowKVError) as ei:
+            F.flowkv_transfer_tables(p, p, FAKE, FAKE, FAKE, 1, 1, 1, 4, 0, {"threads": thr})
+        assert ei.value.status == F.FLOWKV_ERR_CUDA
 
 
 def test_tile_schedule_respects_tile_bytes():
