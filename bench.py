@@ -458,7 +458,7 @@ def run_ours(args) -> None:
             barrier()
 
         dev_tables = device_tables_of(w, dp.device) if args.device_tables else None
-        m = time_steps(F, w, dp.src, dst_desc, dp.requests, K, W, tuning, stream, barrier, local, dev_tables,
+        m = time_steps(F, w, dp.src, dst_desc, dp.batch, K, W, tuning, stream, barrier, local, dev_tables,
                        latency_reps=max(20, args.latency_reps))
         stats = m["stats"]
         t_ms = shard.max_over_ranks(m["t_ms"], device=reduce_dev)                   # max over ranks, device-timed
@@ -515,7 +515,7 @@ def run_ours(args) -> None:
                 scratch = P.alloc_bytes(scratch_bytes, device=f"cuda:{local}")
 
             def e2e_step():
-                plan = F.flowkv_plan(dp.src, dp.dst, dp.requests, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                plan = F.flowkv_plan(dp.src, dp.dst, dp.batch, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
                 if args.e2e_serial:
                     F.flowkv_pack(plan, host.data_ptr(), nbytes, s)      # device -> pinned host, one kernel
                     F.flowkv_unpack(plan, host.data_ptr(), nbytes, s)    # pinned host -> device, one kernel
@@ -645,7 +645,7 @@ def run_ours(args) -> None:
         w3, desc3 = build_workload("cfg3", free_b)
         dp3 = P.DevicePools(w3, device=f"cuda:{local}", sentinel_dst=False)
         K3 = max(20, min(K, args.secondary_steps))
-        m3 = time_steps(F, w3, dp3.src, dp3.dst, dp3.requests, K3, 3, tuning, stream, barrier, local,
+        m3 = time_steps(F, w3, dp3.src, dp3.dst, dp3.batch, K3, 3, tuning, stream, barrier, local,
                         device_tables_of(w3, dp3.device) if args.device_tables else None, latency_reps=5)
         t3 = shard.max_over_ranks(m3["t_ms"], device=reduce_dev)
         if rank == 0:

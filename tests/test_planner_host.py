@@ -366,3 +366,22 @@ def test_bulk_variant_falls_back_when_two_ring_slots_cannot_fit_shared_memory():
     q = F.flowkv_plan_host(small, small, [F.Request(16, np.array([0], np.int32), np.array([1], np.int32))], 0,
                            {"variant": "bulk"})
     assert q.stats["variant"] == F.FLOWKV_VARIANT_BULK and q.stats["smem_bytes"] <= 227 * 1024
+
+
+def test_request_batch_marshalled_once_plans_like_the_list():
+    """flowkv.RequestBatch (the C array built once) gives the same plan as passing the Python requests, can be reused
+    across calls, and an empty batch is fine."""
+    w = synth.config3_batched(n_requests=5, num_layers=2)
+    src = F.make_pool(FAKE, 2, 8, 128, 2, w.src.num_blocks, 16, "lkbthd")
+    dst = F.make_pool(FAKE, 2, 8, 128, 2, w.dst.num_blocks, 16, "lkbthd")
+    reqs = [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks) for r in w.requests]
+    batch = F.RequestBatch(reqs)
+    assert len(batch) == 5
+    a = F.flowkv_plan_host(src, dst, reqs, F.FLOWKV_CHECK_DST_ALIAS)
+    for _ in range(3):
+        b = F.flowkv_plan_host(src, dst, batch, F.FLOWKV_CHECK_DST_ALIAS)
+        assert b.stats == a.stats and b.segments == a.segments
+    assert F.flowkv_plan_host(src, dst, F.RequestBatch([])).stats["n_segments"] == 0
+    # the schedule walks scattered batches in dst-address order, the reported segments stay in request / token order
+    segs = a.segments
+    assert [(s["request"], s["first_token"]) for s in segs] == sorted((s["request"], s["first_token"]) for s in segs)
