@@ -95,7 +95,7 @@ def main(argv=None) -> None:
             seen.add(key)
             src = P.describe(w.src, shape, src_buf.data_ptr())
             dst = P.describe(w.dst, shape, dst_buf.data_ptr())
-            reqs = [F.Request(r.num_tokens, r.src_blocks, r.dst_blocks)]
+            reqs = F.RequestBatch([F.Request(r.num_tokens, r.src_blocks, r.dst_blocks)])    # marshalled once, as a C caller would hold it
             payload = w.payload_bytes
             do_flush = 2 * payload < (256 << 20)
             plan = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, tuning, s)
