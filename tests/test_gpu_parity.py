@@ -1030,3 +1030,42 @@ def test_bench_starts_its_own_ranks_and_peer_mode_runs_on_one_gpu():
     j = json.loads(lines[0])
     assert j["n_gpus"] == 2 and j["gpu_launches"] == 10 and j["launches_per_batch"] == 1.0
     assert "CUDA IPC" in j["config"]["dst"]
+
+
+def test_hand_worked_golden_example_on_the_gpu():
+    """tests/golden/transfer_example.json (5 tokens, block tables [2,0,1] -> [1,0], LKBTHD/2 -> BLKHTD/4): the CUDA path
+    against the hand-worked values directly — register path, TMA tensor path and the table-driven kernel."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "transfer_example.json")) as f:
+        fx = json.load(f)
+    src_h = np.zeros(2 * 3 * 2 * 2 * 8, np.uint16)
+    for c in range(2):
+        for b in range(3):
+            for t in range(2):
+                for h in range(2):
+                    off = ((c * 3 + b) * 2 + t) * 2 * 8 + h * 8
+                    src_h[off:off + 8] = 1000 * c + 100 * b + 10 * t + h
+    exp = np.full(2 * 128, 65535, np.uint16)
+    for blk, c, h, tok, val in fx["expect_dst_rows"]["rows"]:
+        off = blk * 128 + c * 64 + h * 32 + tok * 8
+        exp[off:off + 8] = val
+    src_buf = torch.from_numpy(src_h.view(np.uint8).copy()).cuda()
+    src = F.make_pool(src_buf.data_ptr(), 1, 2, 8, 2, 3, 2, "lkbthd")
+    rq = fx["request"]
+    a, b = np.asarray(rq["src_blocks"], np.int32), np.asarray(rq["dst_blocks"], np.int32)
+    for tuning in (None, {"variant": "bulk"}, "tables"):
+        dst_buf = torch.full((exp.size * 2,), 255, dtype=torch.uint8, device="cuda")
+        dst = F.make_pool(dst_buf.data_ptr(), 1, 2, 8, 2, 2, 4, "blkhtd")
+        if tuning == "tables":
+            st, dt = torch.from_numpy(a[None, :].copy()).cuda(), torch.from_numpy(b[None, :].copy()).cuda()
+            lens = torch.tensor([rq["num_tokens"]], dtype=torch.int32, device="cuda")
+            F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), 1, 3, 2, rq["num_tokens"])
+        else:
+            plan = F.flowkv_plan(src, dst, [F.Request(rq["num_tokens"], a, b)], F.FLOWKV_CHECK_DST_ALIAS, tuning)
+            if tuning:
+                assert plan.stats["variant"] == F.FLOWKV_VARIANT_BULK
+            plan.transfer()
+        torch.cuda.synchronize()
+        got = dst_buf.cpu().numpy().view(np.uint16)
+        assert np.array_equal(got, exp), tuning

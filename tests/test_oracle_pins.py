@@ -620,3 +620,40 @@ def test_plane_window_equals_planes_cut_out_of_the_wire_format(layout):
         O.unpack(full, tok_off, d2, gd, dperm[doff:doff + nb], T)
         tok_off += T; doff += nb
     assert np.array_equal(d1, d2)
+
+
+def test_golden_hand_worked_transfer_and_wire_format():
+    """tests/golden/transfer_example.json: a 5-token request worked by hand (block tables [2,0,1] -> [1,0], src block 2
+    LKBTHD, dst block 4 BLKHTD, partial blocks on both sides).  The offsets are evaluated here from the layout formulas
+    stated in the fixture, not by the oracle or by numpy reshapes.  Catches what the numpy pins share with each other:
+    a consistent misreading of an axis order."""
+    with open(os.path.join(GOLD, "transfer_example.json")) as f:
+        fx = json.load(f)
+    L, H, D = fx["shape"]["L"], fx["shape"]["Hkv"], fx["shape"]["Dh"]
+    gs = _geom("lkbthd", L, H, D, fx["src"]["num_blocks"], fx["src"]["block_size"])
+    gd = _geom("blkhtd", L, H, D, fx["dst"]["num_blocks"], fx["dst"]["block_size"])
+    src = np.zeros(gs.span_bytes() // 2, np.uint16)
+    for c in range(2):
+        for b in range(3):
+            for t in range(2):
+                for h in range(H):
+                    off = ((c * 3 + b) * 2 + t) * 2 * 8 + h * 8
+                    src[off:off + 8] = 1000 * c + 100 * b + 10 * t + h
+    dst = np.full(gd.span_bytes() // 2, fx["dst"]["prefill"], np.uint16)
+    rq = fx["request"]
+    O.transfer(src.view(np.uint8), gs, dst.view(np.uint8), gd, rq["src_blocks"], rq["dst_blocks"], rq["num_tokens"])
+    exp = np.full(dst.size, fx["expect_dst_rows"]["every_other_element"], np.uint16)
+    for blk, c, h, tok, val in fx["expect_dst_rows"]["rows"]:
+        off = blk * 128 + c * 64 + h * 32 + tok * 8
+        exp[off:off + 8] = val
+    assert np.array_equal(dst, exp)
+    wire = np.full(rq["num_tokens"] * gs.bytes_per_token // 2, 65535, np.uint16)
+    O.pack(src.view(np.uint8), gs, rq["src_blocks"], rq["num_tokens"], wire.view(np.uint8), 0)
+    expw = np.full(wire.size, 65535, np.uint16)
+    for c, t, h, val in fx["expect_wire"]["rows"]:
+        off = ((c * 5 + t) * 2 + h) * 8
+        expw[off:off + 8] = val
+    assert np.array_equal(wire, expw)
+    back = np.full(dst.size, 65535, np.uint16)
+    O.unpack(wire.view(np.uint8), 0, back.view(np.uint8), gd, rq["dst_blocks"], rq["num_tokens"])
+    assert np.array_equal(back, exp)
