@@ -386,6 +386,13 @@ def time_steps(F, w, src, dst, requests, K, W, tuning, stream, barrier, local, d
     return out
 
 
+def run_mean(w, side: str) -> float:
+    """Mean length (blocks) of the maximal +1 runs in the generated block tables (input statistics, S§8d)."""
+    from paper_2504_03775_b200 import synth
+    tabs = [r.src_blocks if side == "src" else r.dst_blocks for r in w.requests]
+    return sum(len(t) for t in tabs) / max(1, sum(synth.n_runs(t) for t in tabs))
+
+
 def kernel_name(stats, device_tables: bool) -> str:
     if device_tables:
         return "fk_tables_ldst"
@@ -474,6 +481,7 @@ def run_ours(args) -> None:
                 "dtype": "u16", "data": "synthetic",
                 "config": {"workload": desc, "name": w.name, "requests": len(w.requests), "tokens": w.total_tokens,
                            "payload_bytes": payload, "segments": stats["n_segments"],
+                           "mean_src_run_blocks": run_mean(w, "src"), "mean_dst_run_blocks": run_mean(w, "dst"),
                            "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
                            if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
                            "step": ("flowkv_transfer_tables per step (device-resident block tables, no plan); pools resident in HBM"
@@ -654,6 +662,7 @@ def run_ours(args) -> None:
             line["secondary"] = {
                 "workload": desc3, "name": w3.name, "requests": len(w3.requests), "tokens": w3.total_tokens,
                 "payload_bytes": p3, "segments": m3["stats"]["n_segments"], "steps": K3,
+                "mean_src_run_blocks": run_mean(w3, "src"), "mean_dst_run_blocks": run_mean(w3, "dst"),
                 "value": world * K3 * p3 / (t3 * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": t3 / K3,
                 "kernel_ms_avg": m3["kern_ms"], "kernel_ms_min": m3["kern_min_ms"],
                 "pct_of_8TBps_nominal": 100 * 2 * K3 * p3 / (t3 * 1e-3) / 8e12,
