@@ -131,6 +131,17 @@ def build_workload(name: str, free_bytes: int):
     raise SystemExit(f"unknown --config {name}")
 
 
+def workload_config(w, desc: str, n_segments: int) -> dict:
+    """`config` of the JSON line: names the workload only, so both arms (ours, --impl reference) print the same dict.
+    What an arm DOES with it (step, launch shape, dst placement) goes under the line's `run` key."""
+    payload = w.payload_bytes
+    return {"workload": desc, "name": w.name, "requests": len(w.requests), "tokens": w.total_tokens,
+            "payload_bytes": payload, "segments": int(n_segments),
+            "mean_src_run_blocks": run_mean(w, "src"), "mean_dst_run_blocks": run_mean(w, "dst"),
+            "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
+            if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)"}
+
+
 def load_peaks() -> tuple:
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -262,7 +273,10 @@ def run_reference(args) -> None:
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "u16", "data": "synthetic",
-            "config": {"workload": desc},
+            "config": workload_config(w, desc, sum(O.count_segments(r.src_blocks, w.src.block_size, r.dst_blocks,
+                                                                     w.dst.block_size, r.num_tokens) for r in w.requests)),
+            "run": {"step": "okv_transfer (oracle/flowkv_oracle.c) over a bounded sample of the workload per step; "
+                            "host-resident pools, no device"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -479,18 +493,14 @@ def run_ours(args) -> None:
                 "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
                 "ms_per_step": t_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "u16", "data": "synthetic",
-                "config": {"workload": desc, "name": w.name, "requests": len(w.requests), "tokens": w.total_tokens,
-                           "payload_bytes": payload, "segments": stats["n_segments"],
-                           "mean_src_run_blocks": run_mean(w, "src"), "mean_dst_run_blocks": run_mean(w, "dst"),
-                           "l2": "inputs larger than L2 (payload %.0f MiB >> 126 MB), no flush" % (payload / 2 ** 20)
-                           if payload > 512 * 2 ** 20 else "payload is L2-resident; no flush (latency-bound config)",
-                           "step": ("flowkv_transfer_tables per step (device-resident block tables, no plan); pools resident in HBM"
-                                    if args.device_tables else
-                                    "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM"),
-                           "dst": ("the NEXT rank's dst pool, mapped through CUDA IPC (one-sided peer put)" if args.peer
-                                   else "this rank's own dst pool"),
-                           "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
-                                                            "vec_bytes", "cache_hint", "tile_order", "stages")}},
+                "config": workload_config(w, desc, stats["n_segments"]),
+                "run": {"step": ("flowkv_transfer_tables per step (device-resident block tables, no plan); pools resident in HBM"
+                                 if args.device_tables else
+                                 "flowkv_plan (pool->pool schedule only) + flowkv_transfer + flowkv_plan_destroy per step; pools resident in HBM"),
+                        "dst": ("the NEXT rank's dst pool, mapped through CUDA IPC (one-sided peer put)" if args.peer
+                                else "this rank's own dst pool"),
+                        "launch": {k: stats[k] for k in ("grid", "threads", "group_threads", "tile_bytes", "variant",
+                                                         "vec_bytes", "cache_hint", "tile_order", "stages")}},
                 "clocks": m["clocks"],
                 "gpu_launches": m["launches"],
                 "launches_per_batch": m["launches"] / K, "cuda_api_calls_per_batch": m["api_calls"] / K,

@@ -4,6 +4,7 @@ length {1, 2, 8, 64, contiguous}, plus the device -> pinned-host pack path at 32
 
     python bench_sweep.py [--out gpurun_out/sweep.json] [--reps 20] [--quick] [--tokens 1024,4096] [--runs 1,0]
     python bench_sweep.py --tuning-grid [--tokens 128,512,1024,4096]     # A/B grid of launch shapes on the small points
+    python bench_sweep.py --table3          # the paper's own request sizes (Table 3: 500 .. 12,000 tokens)
 
 Per point: payload, kernel time (CUDA events, mean and min over reps, L2 flushed between reps when
 the payload could stay L2-resident), GB/s, the SAME-SIZE PLAIN COPY under the same conditions (one contiguous
@@ -38,6 +39,9 @@ def main(argv=None) -> None:
     ap.add_argument("--no-baselines", action="store_true")
     ap.add_argument("--tokens", default=None, help="comma-separated request lengths (default: the whole sweep)")
     ap.add_argument("--runs", default=None, help="comma-separated src run lengths, 0 = contiguous")
+    ap.add_argument("--table3", action="store_true",
+                    help="the paper's Table 3 request sizes (500 .. 12,000 tokens, src runs ~ Geometric(mean 4)); adds the "
+                         "latency of the host route (flowkv_plan + flowkv_transfer_via_host: pool -> pinned host -> pool)")
     ap.add_argument("--tuning-grid", action="store_true",
                     help="time a grid of tile sizes / CTA shapes per point instead of the baselines (launch-shape A/B)")
     args = ap.parse_args(argv)
@@ -56,13 +60,15 @@ def main(argv=None) -> None:
     tuning = json.loads(args.tuning) if args.tuning else None
     tokens = synth.SWEEP_TOKENS if not args.quick else [128, 4096, 32768]
     runs = synth.SWEEP_RUNS if not args.quick else [1, 0]
+    if args.table3:
+        tokens, runs = list(synth.TABLE3_TOKENS), [4]            # one point per length: Geometric(mean 4) runs, as configs[1]
     if args.tokens:
         tokens = [int(x) for x in args.tokens.split(",")]
-    if args.runs:
+    if args.runs and not args.table3:
         runs = [int(x) for x in args.runs.split(",")]
     if args.tuning_grid:
         args.no_baselines = True
-    max_nb = max(tokens) // 16
+    max_nb = (max(tokens) + 15) // 16
     src_spec_max = synth.PoolSpec("lkbthd", 16, max(16384, 2 * max_nb))
     src_buf = P.alloc_bytes(src_spec_max.bytes(shape))
     dst_buf = P.alloc_bytes(synth.PoolSpec("lkbthd", 16, max_nb).bytes(shape))
@@ -85,9 +91,10 @@ def main(argv=None) -> None:
         return float(np.mean(ts)), float(np.min(ts))
 
     seen = set()
+    via_host = None
     for T in tokens:
         for run in runs:
-            w = synth.config5_point(T, run)
+            w = synth.table3_point(T) if args.table3 else synth.config5_point(T, run)
             r = w.requests[0]
             key = (T, synth.n_runs(r.src_blocks))
             if key in seen:                                   # run >= request size duplicates "contiguous"
@@ -154,13 +161,35 @@ def main(argv=None) -> None:
                 print(json.dumps({"tokens": T, "run": run or "contig", "default_us": med * 1e3, "plain_copy_us": pmed * 1e3,
                                   "default_shape": {k: st[k] for k in ("tile_bytes", "threads", "group_threads", "grid")},
                                   "best": best, "grid": grid_rows}), flush=True)
-            row = {"tokens": T, "run": run or "contig", "segments": st["n_segments"], "payload_bytes": payload,
+            row = {"tokens": T, "run": ("geometric(4)" if args.table3 else run or "contig"), "segments": st["n_segments"], "payload_bytes": payload,
                    "plain_copy_ms_med": pmed, "plain_copy_ms_min": pmn, "frac_of_plain_copy": pmed / med,
                    "graph_replay_ms_med": gmed, "back_to_back_ms_per_launch": b2b,
                    "kernel_ms_med": med, "kernel_ms_min": mn, "payload_GBps": payload / (med * 1e-3) / 1e9,
                    "hbm_GBps": 2 * payload / (med * 1e-3) / 1e9, "hbm_GBps_best": 2 * payload / (mn * 1e-3) / 1e9,
                    "latency_ms_plan_to_done": float(np.median(lat)), "launches_per_request": launches,
                    "l2_flushed": do_flush, "tile_bytes": st["tile_bytes"], "grid": st["grid"], "threads": st["threads"]}
+            if args.table3:
+                # the host route (the network stand-in): pool -> pinned host -> pool, both PCIe directions inside the
+                # timed region; host wall clock from the flowkv_plan call until the stream has drained
+                if via_host is None:
+                    via_host = torch.empty(max(tokens) * shape.bytes_per_token, dtype=torch.uint8, pin_memory=True)
+                pv = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                sb = F.flowkv_via_host_scratch_bytes(pv, 0)
+                pv.destroy()
+                scratch = P.alloc_bytes(sb)
+                hl = []
+                for i in range(min(args.reps, 10) + 1):
+                    torch.cuda.synchronize()
+                    t0 = time.perf_counter()
+                    pv = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                    F.flowkv_transfer_via_host(pv, via_host.data_ptr(), payload, 0, 0, s, scratch.data_ptr(), sb)
+                    torch.cuda.synchronize()
+                    if i:                                         # the first call creates the helper streams
+                        hl.append((time.perf_counter() - t0) * 1e3)
+                    pv.destroy()
+                del scratch
+                row["via_host_latency_ms_plan_to_done"] = float(np.median(hl))
+                row["via_host_GBps_each_way"] = payload / (float(np.median(hl)) * 1e-3) / 1e9
             if not args.no_baselines:
                 a, b = ev(), ev()
                 F.flowkv_baseline_segmentwise(plan, s); torch.cuda.synchronize()
@@ -177,7 +206,7 @@ def main(argv=None) -> None:
 
     # ---- device -> pinned host pack at the 32k-token point ------------------------------------------------------
     T = 32768
-    if T in tokens:
+    if T in tokens and not args.table3:
         nbytes = T * shape.bytes_per_token
         host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
         dev_flat = dst_buf[:nbytes]

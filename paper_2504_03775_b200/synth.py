@@ -426,3 +426,18 @@ def config5_point(tokens: int, run: int, num_layers: Optional[int] = None) -> Wo
     return make_workload(f"cfg5_sweep_T{tokens}_run{run or 'contig'}", SEED_BASE + 5000 + point, shape,
                          [tokens], "lkbthd", 16, kind, max(16384, 2 * nb),
                          "lkbthd", 16, ("contiguous",), nb)
+
+
+# The paper's own request sizes: Table 3 reports KV transfer latency for simulated requests of
+# 500 .. 12,000 input tokens on Llama-3.1-8B.  Only the lengths come from the paper; the tables are seeded draws.
+TABLE3_TOKENS = [500, 1000, 2000, 4000, 8000, 10000, 12000]
+
+
+def table3_point(tokens: int, num_layers: Optional[int] = None) -> Workload:
+    """One request of a Table 3 input length, src runs ~ Geometric(mean 4) over a 16,384-block pool
+    and dst contiguous, exactly as configs[1] is built; lengths that are no multiple of 16 end in a partial block."""
+    shape = LLAMA3_8B if num_layers is None else Shape(num_layers, 8, 128, "bf16")
+    nb = _nblk(tokens, 16)
+    return make_workload(f"table3_T{tokens}", SEED_BASE + 6000 + TABLE3_TOKENS.index(tokens), shape, [tokens],
+                         "lkbthd", 16, ("geometric", 4.0), 16384,
+                         "lkbthd", 16, ("contiguous",), nb)

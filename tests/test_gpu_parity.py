@@ -1029,7 +1029,7 @@ def test_bench_starts_its_own_ranks_and_peer_mode_runs_on_one_gpu():
     assert len(lines) == 1, out.stdout
     j = json.loads(lines[0])
     assert j["n_gpus"] == 2 and j["gpu_launches"] == 10 and j["launches_per_batch"] == 1.0
-    assert "CUDA IPC" in j["config"]["dst"]
+    assert "CUDA IPC" in j["run"]["dst"]
 
 
 def test_hand_worked_golden_example_on_the_gpu():
@@ -1069,3 +1069,45 @@ def test_hand_worked_golden_example_on_the_gpu():
         torch.cuda.synchronize()
         got = dst_buf.cpu().numpy().view(np.uint16)
         assert np.array_equal(got, exp), tuning
+
+
+@pytest.mark.parametrize("tokens", synth.TABLE3_TOKENS)
+def test_paper_table3_request_lengths(tokens):
+    """The paper's own request sizes (Table 3: 500 .. 12,000 input tokens), L = 2: planned transfer
+    (register and TMA paths), the table-free host route and the table-driven kernel all reach the oracle's dst pool;
+    lengths that are no multiple of the block size leave the tail of the last block untouched (A4)."""
+    w = synth.table3_point(tokens, num_layers=2)
+    dp, plan, exp = G.run_transfer_and_check(w)
+    assert plan.stats["n_segments"] == synth.n_runs(w.requests[0].src_blocks)
+    plan.destroy()
+    s = torch.cuda.current_stream().cuda_stream
+    dp.dst_buf.fill_(P.SENTINEL_BYTE)
+    pb = dp.plan(0, {"variant": "bulk"}, s)
+    assert pb.stats["variant"] == F.FLOWKV_VARIANT_BULK
+    pb.transfer(s)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, f"table 3 T={tokens}: TMA bulk path")
+    pb.destroy()
+    # host route: pool -> pinned host -> pool
+    dp.dst_buf.fill_(P.SENTINEL_BYTE)
+    pv = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER, None, s)
+    nbytes = pv.stats["staging_bytes"]
+    host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    sb = F.flowkv_via_host_scratch_bytes(pv, 0)
+    scratch = P.alloc_bytes(sb)
+    F.flowkv_transfer_via_host(pv, host.data_ptr(), nbytes, 0, 0, s, scratch.data_ptr(), sb)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, f"table 3 T={tokens}: host route")
+    pv.destroy()
+    # table-driven: block tables and the length stay on the device
+    r = w.requests[0]
+    dp.dst_buf.fill_(P.SENTINEL_BYTE)
+    st_ = torch.from_numpy(np.ascontiguousarray(r.src_blocks)).cuda()
+    dt_ = torch.from_numpy(np.ascontiguousarray(r.dst_blocks)).cuda()
+    nt = torch.tensor([tokens], dtype=torch.int32, device="cuda")
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    F.flowkv_transfer_tables(dp.src, dp.dst, st_.data_ptr(), dt_.data_ptr(), nt.data_ptr(), 1, len(r.src_blocks),
+                             len(r.dst_blocks), tokens, flag.data_ptr(), None, s)
+    torch.cuda.synchronize()
+    assert int(flag.item()) == 0
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, f"table 3 T={tokens}: table-driven")

@@ -72,3 +72,15 @@ def test_cfg5_points():
             exp_runs = 1 if (run == 0 or run >= nb) else -(-nb // run)
             assert synth.n_runs(tab) == exp_runs
             assert w.src.num_blocks == max(16384, 2 * nb)
+
+
+def test_table3_points():
+    """The paper's Table 3 request lengths: 131,072 B per token, ragged last blocks, seeded tables."""
+    assert synth.TABLE3_TOKENS == [500, 1000, 2000, 4000, 8000, 10000, 12000]
+    for T in synth.TABLE3_TOKENS:
+        w = synth.table3_point(T)
+        _check_tables(w)
+        r = w.requests[0]
+        assert r.num_tokens == T and w.payload_bytes == T * 131072
+        assert synth.n_runs(r.dst_blocks) == 1 and 1 <= synth.n_runs(r.src_blocks) <= len(r.src_blocks)
+        assert np.array_equal(synth.table3_point(T).requests[0].src_blocks, r.src_blocks)
