@@ -577,7 +577,7 @@ def run_ours(args) -> None:
             duplex = pb / (best * 1e-3) / 1e9
             # ... and what the route must be: a CHUNKED duplex pipeline (chunk c returns once it has landed), copy
             # engines only, same chunk count as the route — the bound e2e.value is read against (bench_hostlink.py)
-            n_ch = args.e2e_chunks or 64
+            n_ch = args.e2e_chunks or int(min(64, max(4, np.floor(np.sqrt(nbytes / 400e3) + 0.5))))   # the library's default rule
             wbp = pb // n_ch
             side2 = torch.cuda.Stream()
             bestp = None

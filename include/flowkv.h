@@ -130,7 +130,7 @@ typedef struct {
   uint32_t tile_bytes;      /* max bytes one thread group copies per tile (0 = auto; pow2, 1 KiB..1 MiB) */
   uint32_t ctas_per_sm;     /* resident CTAs per SM of the persistent grid (0 = auto)               */
   uint32_t max_sms;         /* SM budget: grid = min(#SMs, max_sms) * ctas_per_sm (0 = all SMs; P:L92 co-run) */
-  uint32_t threads;         /* threads per CTA (0 = auto; multiple of 32, <= 1024)                  */
+  uint32_t threads;         /* threads per CTA (0 = auto; power of two in [32, 512])                */
   uint32_t group_threads;   /* threads that share one tile (0 = auto; 32..threads, power of two)    */
   uint32_t variant;         /* flowkv_variant (0 = auto)                                            */
   uint32_t tile_order;      /* 0 = auto, 1 = plane-major (all tiles of plane 0, then plane 1, ...), 2 = chunk-major */
@@ -262,8 +262,10 @@ FLOWKV_API flowkv_status flowkv_unpack_window(const flowkv_plan_t* plan, const v
  *     (flowkv_pack_window, on `stream`), moved D2H and H2D by cudaMemcpyAsync on two copy queues of their own, and
  *     unpacked from a second slot (flowkv_unpack_window, on a fourth queue), so neither engine ever waits behind a
  *     kernel.  On B200 the copy engines sustain ~50 GB/s in both directions at once where SM loads over PCIe drop
- *     to ~38 GB/s.  n_chunks is clamped to [1, 2L]; default 64 (the first outbound and the last inbound chunk cross
- *     the link alone, so many small chunks win).  host_staging then holds the chunks back to back: with n <= L
+ *     to ~38 GB/s.  n_chunks is clamped to [1, 2L]; default (0) = round(sqrt(payload_bytes / 400 KB)) in [4, 64]:
+ *     the first outbound and the last inbound chunk cross the link alone, so many small chunks win until the
+ *     hand-over between the queues (a few microseconds per chunk) outweighs the shorter head — 16 chunks for a
+ *     500-token Llama-3-8B request, 64 from 12,000 tokens up.  host_staging then holds the chunks back to back: with n <= L
  *     chunk c = the layer window [L*c/n, L*(c+1)/n) at byte offset flowkv_window_bytes(0, L*c/n) (== the wire
  *     format when n_chunks == 1); with n > L chunk c = the PLANES [2L*c/n, 2L*(c+1)/n) (plane = 2*layer + K|V) in
  *     wire order [request][plane - first][token][head][dim] at byte offset total_tokens * first * Hkv*Dh*e — a layer

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -838,9 +839,20 @@ flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, 
 namespace {
 uint32_t via_host_chunks(const flowkv_plan_t* pl, uint32_t n_chunks, bool engines) {
   // defaults measured on B200 (profiles/r02_host_route.md): the first outbound and the last inbound chunk cross the
-  // link alone, so the copy-engine pipeline wants many small chunks (up to one per plane); the direct mode pays a
-  // kernel pair per chunk and stays at layer granularity
-  if (n_chunks == 0) n_chunks = engines ? 64 : 16;
+  // link alone, so the copy-engine pipeline wants many small chunks (up to one per plane) — as long as a chunk stays
+  // large against the hand-over between the queues; the direct mode pays a kernel pair per chunk and stays at layer
+  // granularity
+  if (n_chunks == 0) {
+    n_chunks = 16;
+    if (engines) {
+      // time ~ payload/bw * (1 + 1/n) + n * gap: the lonely head and tail shrink with n, every chunk costs a few
+      // microseconds of queue hand-over.  The minimum sits at n = sqrt(payload / (bw * gap)) = sqrt(payload / 400 KB)
+      // at ~50 GB/s and ~8 us; measured optimum on the paper's request sizes (profiles/r02_table3.md): 16 chunks at
+      // 500 tokens (62.5 MiB), 32 at 4,000, 64 from 12,000 tokens up.
+      const double payload = (double)pl->total_tokens * (double)pl->g.bytes_per_token;
+      n_chunks = (uint32_t)std::min(64.0, std::max(4.0, std::floor(std::sqrt(payload / 400e3) + 0.5)));
+    }
+  }
   return std::max<uint32_t>(1, std::min(n_chunks, engines ? 2 * pl->g.L : pl->g.L));
 }
 // Chunk c of n covers the planes [first, last): whole layers while n <= L (the layer windows of A20), single planes

@@ -547,8 +547,12 @@ def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas, small):
     n0 = F.flowkv_launch_count()
     F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, n_chunks, ctas, stream.cuda_stream, scratch.data_ptr(), sb)
     stream.synchronize()
-    chunks = min(n_chunks, 2 * L) if n_chunks else min(64, 2 * L)      # clamped to one chunk per plane
-    assert F.flowkv_launch_count() - n0 == 2 * chunks
+    launched = F.flowkv_launch_count() - n0
+    if n_chunks:
+        chunks = min(n_chunks, 2 * L)                                  # clamped to one chunk per plane
+    else:       # default: round(sqrt(payload / 400 KB)) in [4, 64] (flowkv.h), then the same clamp
+        chunks = min(int(min(64, max(4, np.floor(np.sqrt(nbytes / 400e3) + 0.5)))), 2 * L)
+    assert launched == 2 * chunks
     G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host (copy engines): dst")
     if chunks <= L:       # layer windows (A20)
         exp_host = np.concatenate([G.oracle_pack_window(w, src_np, L * c // chunks, L * (c + 1) // chunks) for c in range(chunks)])
