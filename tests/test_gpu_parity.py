@@ -1115,3 +1115,54 @@ def test_paper_table3_request_lengths(tokens):
     torch.cuda.synchronize()
     assert int(flag.item()) == 0
     G.assert_same(P.to_numpy(dp.dst_buf), exp, f"table 3 T={tokens}: table-driven")
+
+
+def test_distinct_plans_from_distinct_threads_on_distinct_streams():
+    """Header: 'distinct plans may be used from distinct threads'.  Four threads, each with its own stream and pools,
+    loop plan -> transfer (-> host route) -> destroy at once — uploaded plans and plans that ride in the kernel
+    parameters — so the library's shared caches (pinned staging, plan memory pool, upload stream, recycled vectors,
+    via-host helper streams) are hit concurrently; every dst pool must equal the oracle's."""
+    import threading
+    shape = synth.Shape(3, 4, 64, "bf16")
+    works = []
+    for k in range(4):
+        lengths = [700 + 37 * k, 90, 1500 + k] if k % 2 == 0 else [8 + k]       # odd threads: tiny plans (kernel params)
+        run = 2.0
+        works.append(synth.make_workload(f"mt{k}", 9000 + k, shape, lengths, "lkbthd", 16,
+                                         ("fixed", 1) if k % 2 == 0 else ("geometric", run), None,
+                                         "blkhtd" if k == 2 else "lkbthd", 32 if k == 2 else 16, ("geometric", 3.0), None))
+    dps = [P.DevicePools(w, fill="bits") for w in works]
+    srcs = [P.to_numpy(dp.src_buf) for dp in dps]
+    streams = [torch.cuda.Stream() for _ in works]
+    hosts = [torch.empty(max(w.payload_bytes, 16), dtype=torch.uint8, pin_memory=True) for w in works]
+    errors, uploaded = [], [False] * 4
+    torch.cuda.synchronize()
+
+    def worker(k):
+        try:
+            dp, s = dps[k], streams[k].cuda_stream
+            for it in range(25):
+                plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS, {"plan_in_params": 1} if k % 2 == 0 else None, s)   # even threads upload
+                uploaded[k] = plan.stats["plan_device_bytes"] > 0
+                plan.transfer(s)
+                if it % 5 == 4:
+                    sb = F.flowkv_via_host_scratch_bytes(plan, 3)
+                    scratch = P.alloc_bytes(sb)
+                    F.flowkv_transfer_via_host(plan, hosts[k].data_ptr(), hosts[k].numel(), 3, 0, s, scratch.data_ptr(), sb)
+                    streams[k].synchronize()
+                plan.destroy()
+            streams[k].synchronize()
+        except Exception as e:          # noqa: BLE001 — reported by the main thread
+            errors.append(f"thread {k}: {e!r}")
+
+    threads = [threading.Thread(target=worker, args=(k,)) for k in range(4)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    assert uploaded[0] and uploaded[2] and not uploaded[1] and not uploaded[3], uploaded
+    torch.cuda.synchronize()
+    for k, w in enumerate(works):
+        G.assert_same(P.to_numpy(dps[k].dst_buf), G.oracle_transfer(w, srcs[k]), f"thread {k} ({w.name})")
+        G.assert_same(P.to_numpy(dps[k].src_buf), srcs[k], "src pool must not change")
