@@ -38,6 +38,7 @@ class _Pool(C.Structure):
         ("s_layer", C.c_int64), ("s_kv", C.c_int64), ("s_block", C.c_int64),
         ("s_token", C.c_int64), ("s_head", C.c_int64),
         ("layer0", C.c_uint32), ("_pad", C.c_uint32),
+        ("layer_off", C.c_void_p),
     ]
 
 
@@ -96,6 +97,20 @@ class PoolGeom:
     s_block: int
     s_token: int
     s_head: int
+    layer_off: tuple | None = None      # reading A22: byte offset of every layer (separate allocations); s_layer unused
+
+    def with_layer_offsets(self, layer_off) -> "PoolGeom":
+        """The same pool with every layer at its own byte offset from the buffer start (the cache the paper
+        starts from keeps 'separate tensor structures across all layer dimensions')."""
+        off = tuple(int(x) for x in layer_off)
+        assert len(off) == self.num_layers
+        return PoolGeom(self.num_layers, self.num_kv_heads, self.head_dim, self.elem_bytes, self.num_blocks,
+                        self.block_size, self.s_layer, self.s_kv, self.s_block, self.s_token, self.s_head, off)
+
+    def layer_bytes(self) -> int:
+        """Bytes from the first to one past the last addressable element of ONE layer."""
+        return (self.s_kv + (self.num_blocks - 1) * self.s_block + (self.block_size - 1) * self.s_token
+                + (self.num_kv_heads - 1) * self.s_head + self.head_dim * self.elem_bytes)
 
     @staticmethod
     def lkbthd(L, Hkv, Dh, e, NB, BS) -> "PoolGeom":
@@ -131,14 +146,21 @@ class PoolGeom:
 
     def span_bytes(self) -> int:
         """Bytes from the first to one past the last addressable element."""
+        if self.layer_off is not None:
+            return max(self.layer_off) + self.layer_bytes()
         return ((self.num_layers - 1) * self.s_layer + self.s_kv + (self.num_blocks - 1) * self.s_block
                 + (self.block_size - 1) * self.s_token + (self.num_kv_heads - 1) * self.s_head
                 + self.head_dim * self.elem_bytes)
 
     def _c(self, layer0: int = 0) -> _Pool:
-        return _Pool(self.num_layers, self.num_kv_heads, self.head_dim, self.elem_bytes,
-                     self.num_blocks, self.block_size, self.s_layer, self.s_kv, self.s_block,
-                     self.s_token, self.s_head, layer0, 0)
+        p = _Pool(self.num_layers, self.num_kv_heads, self.head_dim, self.elem_bytes,
+                  self.num_blocks, self.block_size, self.s_layer, self.s_kv, self.s_block,
+                  self.s_token, self.s_head, layer0, 0, None)
+        if self.layer_off is not None:
+            assert layer0 == 0, "a pool of separate layers is handed over whole"
+            p._keep = np.asarray(self.layer_off, dtype=np.int64)     # kept alive by the struct object
+            p.layer_off = p._keep.ctypes.data
+        return p
 
 
 def _u8(a: np.ndarray, writable: bool) -> int:

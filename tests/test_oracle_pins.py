@@ -657,3 +657,97 @@ def test_golden_hand_worked_transfer_and_wire_format():
     back = np.full(dst.size, 65535, np.uint16)
     O.unpack(wire.view(np.uint8), 0, back.view(np.uint8), gd, rq["dst_blocks"], rq["num_tokens"])
     assert np.array_equal(back, exp)
+
+
+# ---------------------------------------------------------------------------------------
+# reading A22: pools whose layers are separate allocations ("separate tensor structures across all layer
+# dimensions" — the cache the paper starts from).  Pinned against numpy arrays that really ARE separate.
+# ---------------------------------------------------------------------------------------
+def _scatter_layers(rng, layers, gap=48):
+    """Place separate per-layer arrays (uint8, flat) at shuffled, gapped offsets of one buffer -> (buffer, offsets)."""
+    order = rng.permutation(len(layers))
+    off, pos = [0] * len(layers), 16 * int(rng.integers(0, 4))
+    for l in order:
+        off[l] = pos
+        pos += layers[l].size + 16 * int(rng.integers(1, gap // 16 + 1))
+    buf = rng.integers(0, 256, size=pos, dtype=np.uint8)
+    for l, a in enumerate(layers):
+        buf[off[l]:off[l] + a.size] = a
+    return buf, off
+
+
+@pytest.mark.parametrize("e", [1, 2, 4])
+@pytest.mark.parametrize("dst_separate", [False, True])
+def test_separate_layer_tensors_equal_numpy_fancy_indexing_layer_by_layer(e, dst_separate):
+    """Every src layer is its own [2][NB][BS][H][D] array somewhere in memory (shuffled order, gaps in between);
+    the move must equal `dst_l[:, Dst] = src_l[:, Src]` for every layer separately.  Catches: a layer offset applied
+    to the wrong layer, s_layer still added, K|V stride taken from the stacked pool, gaps overwritten."""
+    rng = np.random.default_rng(2200 + e)
+    L, H, D, NB, BS, n = 4, 2, 16 // e * 2, 7, 4, 5
+    dt = Hh.ELEM_DTYPE[e]
+    src_layers = [rng.integers(0, 256, size=2 * NB * BS * H * D * e, dtype=np.uint8) for _ in range(L)]
+    src, soff = _scatter_layers(rng, src_layers)
+    one = O.PoolGeom.lkbthd(1, H, D, e, NB, BS)                       # geometry of ONE layer tensor
+    gs = O.PoolGeom(L, H, D, e, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head).with_layer_offsets(soff)
+    assert gs.span_bytes() <= src.size
+    Src, Dst = rng.permutation(NB)[:n], rng.permutation(NB)[:n]
+    T = n * BS - 3                                                    # partial last block (A4)
+    if dst_separate:
+        dst_layers = [np.full(2 * NB * BS * H * D * e, SENT, np.uint8) for _ in range(L)]
+        dst, doff = _scatter_layers(rng, dst_layers)
+        gd = O.PoolGeom(L, H, D, e, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head).with_layer_offsets(doff)
+    else:
+        gd = O.PoolGeom.lkbthd(L, H, D, e, NB, BS)
+        dst = np.full(gd.span_bytes(), SENT, np.uint8)
+        doff = [l * gd.s_layer for l in range(L)]
+    exp = dst.copy()
+    O.transfer(src, gs, dst, gd, Src, Dst, T)
+    per_layer = 2 * NB * BS * H * D * e
+    for l in range(L):
+        sv = src_layers[l].view(dt).reshape(2, NB * 0 + NB, BS, H, D)
+        ev = exp[doff[l]:doff[l] + per_layer].view(dt).reshape(2, NB, BS, H, D)
+        full = T // BS
+        ev[:, Dst[:full]] = sv[:, Src[:full]]
+        ev[:, Dst[full], :T % BS] = sv[:, Src[full], :T % BS]
+    assert np.array_equal(dst, exp)
+
+
+def test_separate_layers_at_uniform_offsets_are_the_stacked_pool():
+    """layer_off[l] = l * s_layer must give exactly what the stacked (L,2,B,H) pool gives — wire format included.
+    Catches: layer_off used on one side of pack/unpack only, or ignored by the window functions."""
+    rng = np.random.default_rng(2210)
+    L, H, D, NB, BS, T = 3, 2, 8, 6, 4, 18
+    g = _geom("lkbthd", L, H, D, NB, BS)
+    gl = g.with_layer_offsets([l * g.s_layer for l in range(L)])
+    src = _rand_pool(rng, g.span_bytes())
+    tab = rng.permutation(NB)[:-(-T // BS)]
+    a, b = np.full(T * g.bytes_per_token, SENT, np.uint8), np.full(T * g.bytes_per_token, SENT, np.uint8)
+    O.pack(src, g, tab, T, a, 0)
+    O.pack(src, gl, tab, T, b, 0)
+    assert np.array_equal(a, b)
+    wa, wb = np.full(T * 2 * 2 * H * D * 2, SENT, np.uint8), np.full(T * 2 * 2 * H * D * 2, SENT, np.uint8)
+    O.pack_window(src, g, tab, T, wa, 0, 1, 3)
+    O.pack_window(src, gl, tab, T, wb, 0, 1, 3)
+    assert np.array_equal(wa, wb)
+    da, db = np.full(g.span_bytes(), SENT, np.uint8), np.full(g.span_bytes(), SENT, np.uint8)
+    O.unpack(a, 0, da, g, tab, T)
+    O.unpack(a, 0, db, gl, tab, T)
+    assert np.array_equal(da, db)
+
+
+def test_separate_layers_into_one_block_major_tensor_is_eq5():
+    """The migration Eq. 5 describes: per-layer tensors (L x [2][B][H]) -> ONE (B,L,2,H) tensor, identity
+    tables: equals numpy stack + transpose.  Catches: a layer landing in another layer's slot of the block."""
+    rng = np.random.default_rng(2220)
+    L, H, D, NB, BS = 3, 2, 8, 5, 4
+    Hbytes = BS * H * D * 2
+    layers = [rng.integers(0, 256, size=2 * NB * Hbytes, dtype=np.uint8) for _ in range(L)]
+    src, soff = _scatter_layers(rng, layers)
+    one = O.PoolGeom.lkbthd(1, H, D, 2, NB, BS)
+    gs = O.PoolGeom(L, H, D, 2, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head).with_layer_offsets(soff)
+    gd = _geom("blkthd", L, H, D, NB, BS)
+    dst = np.full(gd.span_bytes(), SENT, np.uint8)
+    ident = np.arange(NB)
+    O.transfer(src, gs, dst, gd, ident, ident, NB * BS)
+    exp = np.stack([a.reshape(2, NB, Hbytes) for a in layers]).transpose(2, 0, 1, 3).reshape(-1)
+    assert np.array_equal(dst, exp)
