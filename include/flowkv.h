@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define FLOWKV_VERSION 3
+#define FLOWKV_VERSION 4
 
 #if defined(__GNUC__)
 #define FLOWKV_API __attribute__((visibility("default")))
@@ -94,6 +94,13 @@ typedef struct {
   uint32_t layout;          /* flowkv_layout                                                        */
   uint32_t _reserved;
   int64_t  stride_bytes[5]; /* layer, kv, block, token, head — see FLOWKV_S_*; multiples of 16      */
+  const int64_t* layer_offsets; /* NULL, or HOST array [num_layers] (borrowed for the call; a plan keeps a copy): layer l
+                             * starts layer_offsets[l] bytes from `base` and stride_bytes[FLOWKV_S_LAYER] is ignored.  For
+                             * a cache whose layers are separate allocations — the state the paper starts from
+                             * "separate tensor structures across all layer dimensions" (reading A22): set
+                             * base to any one of them and the offsets to the signed distances; multiples of 16, any
+                             * order, gaps allowed.  The other four strides describe one layer.  Such pools run the
+                             * register / bulk-copy paths (no flat mode, no TMA tensor path). */
 } flowkv_pool;
 
 /* One request: its length and both sides' block-id lists.
@@ -184,11 +191,13 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
  *   reqs     : HOST array of n_reqs requests (n_reqs may be 0).
  *   tuning   : HOST pointer or NULL.
  *   out      : HOST pointer; receives the plan (caller destroys it).  Untouched on error.
- * The plan stays valid until destroyed; pools must stay alive while it is run.
+ * The plan stays valid until destroyed; pools must stay alive while it is run.  The first plan (or table-driven call)
+ * that names a new layer_offsets[] array copies it to the device once (8*L bytes on the library's own stream, waited
+ * for; cached by content for the life of the process) — the one exception to "does not synchronise".
  * Errors (nothing is allocated or enqueued when one is returned):
  *   INVALID_ARG  out NULL, both pools NULL, reqs NULL with n_reqs > 0, a table pointer NULL, unknown flag /
  *                layout / tuning value, a zero shape field or a stride <= 0
- *   ALIGN        a base, a stride or head_dim*elem_bytes is not a multiple of 16 bytes
+ *   ALIGN        a base, a stride, a layer offset or head_dim*elem_bytes is not a multiple of 16 bytes
  *   SHAPE_MISMATCH  src and dst differ in L, Hkv, Dh or elem_bytes
  *   TABLE_LEN    n_*_blocks != ceil(num_tokens / block_size);  BLOCK_OOB  an id outside [0, num_blocks)
  *   DST_ALIAS    (only with FLOWKV_CHECK_DST_ALIAS) a dst block id named twice in the batch

@@ -57,6 +57,8 @@ struct Side {            // one end of a copy as the kernel sees it
                          // s_layer = bytes per token of the layer window the buffer holds, s_kv unused
   uint32_t dense;        // 1: dense staging buffer, 0: paged pool
   uint32_t plane0;       // dense side: first plane of the layer window the buffer holds (0 = whole wire format)
+  const int64_t* layer_off;   // pool side, DEVICE array [L] or NULL: layer l starts layer_off[l] bytes from base and
+                              // s_layer is unused (layers are separate allocations, reading A22)
 };
 
 // Plans whose every schedule has at most kInlineChunks entries pass them in the kernel parameters instead of
@@ -165,6 +167,11 @@ bool pool_is_span_capable(const flowkv_pool& p, const Geometry& g);
 // Are both pools block-major (a block = one dense byte range holding all its planes, blocks abutting)
 // with the same block size and the same interior strides?  Then whole-block runs are flat byte ranges.
 bool pools_are_flat_congruent(const flowkv_pool& a, const flowkv_pool& b, const Geometry& g);
+
+// Byte offset of layer l from the pool's base (uniform stride, or the caller's per-layer offsets: reading A22).
+inline int64_t pool_layer_off(const flowkv_pool& p, uint32_t l) {
+  return p.layer_offsets ? p.layer_offsets[l] : (int64_t)l * p.stride_bytes[FLOWKV_S_LAYER];
+}
 
 flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string& err);
 flowkv_status validate_requests(const flowkv_pool* src, const flowkv_pool* dst, const flowkv_request* reqs,

@@ -21,16 +21,37 @@ FUZZ_OFFSET = int(os.environ.get("FLOWKV_FUZZ_OFFSET", "0"))
 FUZZ_CASES = int(os.environ.get("FLOWKV_FUZZ_CASES", "400"))
 
 
-def _geom(rng, layout, L, H, D, NB, BS, e=2):
-    """-> (oracle geometry, strides or None).  'padded' = token-major interior with padding after every block,
-    K|V slab and layer (a STRIDED pool: separate allocations / alignment padding)."""
+def _geom(rng, layout, L, H, D, NB, BS, e=2, separate=False):
+    """-> (oracle geometry, strides or None, layer offsets or None).  'padded' = token-major interior with padding
+    after every block, K|V slab and layer (a STRIDED pool: separate allocations / alignment padding); with
+    ``separate`` its layers sit at shuffled, gapped offsets of their own (reading A22: a tensor per layer)."""
     if layout != "padded":
-        return getattr(O.PoolGeom, layout)(L, H, D, e, NB, BS), None
+        return getattr(O.PoolGeom, layout)(L, H, D, e, NB, BS), None, None
     row, tok = D * e, H * D * e
     blk = BS * tok + 32 * int(rng.integers(0, 5))
     kv = NB * blk + 32 * int(rng.integers(0, 9))
     lay = 2 * kv + 32 * int(rng.integers(0, 3))
-    return O.PoolGeom(L, H, D, e, NB, BS, lay, kv, blk, tok, row), [lay, kv, blk, tok, row]
+    g = O.PoolGeom(L, H, D, e, NB, BS, lay, kv, blk, tok, row)
+    if not separate:
+        return g, [lay, kv, blk, tok, row], None
+    unit = 16 if rng.random() < 0.25 else 32               # a quarter of them only 16-byte aligned (128-bit path)
+    off, pos = [0] * L, unit * int(rng.integers(0, 3))
+    for l in rng.permutation(L):
+        off[int(l)] = pos
+        pos += g.layer_bytes() + unit * int(rng.integers(1, 6))
+    return g.with_layer_offsets(off), [lay, kv, blk, tok, row], off
+
+
+def _pools(rng, idx, L, H, D, e, lay_s, bs_s, NBs, lay_d, bs_d, NBd):
+    """Both pools of a case: oracle geometries, device buffers (src random bits, dst sentinel) and descriptors."""
+    gs, ss, los = _geom(rng, lay_s, L, H, D, NBs, bs_s, e, separate=lay_s == "padded" and idx % 2 == 0)
+    gd, sd, lod = _geom(rng, lay_d, L, H, D, NBd, bs_d, e, separate=lay_d == "padded" and idx % 2 == 1)
+    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
+    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
+    P.fill_sentinel(dst_buf)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss, los)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd, lod)
+    return gs, gd, ss, sd, src_buf, dst_buf, src, dst
 
 
 def _table(rng, n, NB, p_cont):
@@ -98,14 +119,8 @@ def _case(idx):
 @pytest.mark.parametrize("idx", range(FUZZ_OFFSET, FUZZ_OFFSET + FUZZ_CASES))
 def test_fuzz_against_oracle(idx):
     rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, op = _case(idx)
-    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s, e)
-    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d, e)
-    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
-    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
-    P.fill_sentinel(dst_buf)
+    gs, gd, ss, sd, src_buf, dst_buf, src, dst = _pools(rng, idx, L, H, D, e, lay_s, bs_s, NBs, lay_d, bs_d, NBd)
     src_np = P.to_numpy(src_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd)
     freqs = [F.Request(t, a, b) for t, a, b in reqs]
     total = sum(t for t, _, _ in reqs)
     tokb = H * D * e
@@ -188,14 +203,8 @@ def test_fuzz_table_driven_transfer(idx):
     """flowkv_transfer_tables: the kernel walks device-resident padded block tables itself (no plan) — same seeded
     cases as above, whole dst pool against the oracle, one launch, error flag stays clear."""
     rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
-    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s, e)
-    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d, e)
-    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
-    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
-    P.fill_sentinel(dst_buf)
+    gs, gd, ss, sd, src_buf, dst_buf, src, dst = _pools(rng, idx, L, H, D, e, lay_s, bs_s, NBs, lay_d, bs_d, NBd)
     src_np = P.to_numpy(src_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd)
     max_t = max(t for t, _, _ in reqs) + int(rng.integers(0, 40))
     ws, wd = -(-max_t // bs_s) + int(rng.integers(0, 3)), -(-max_t // bs_d) + int(rng.integers(0, 3))
     st, dt, lens = _device_tables(reqs, max(ws, 1), max(wd, 1))
@@ -230,14 +239,8 @@ def test_fuzz_table_driven_pack_unpack_windows(idx):
     at a random layer; each window == the oracle's okv_pack_window, unpacking them rebuilds the oracle's transfer;
     a window buffer that is too small raises flag bit 2 and is left untouched."""
     rng, (L, H, D, e), (lay_s, bs_s, NBs), (lay_d, bs_d, NBd), reqs, tuning, _ = _case(idx)
-    gs, ss = _geom(rng, lay_s, L, H, D, NBs, bs_s, e)
-    gd, sd = _geom(rng, lay_d, L, H, D, NBd, bs_d, e)
-    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
-    P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
-    P.fill_sentinel(dst_buf)
+    gs, gd, ss, sd, src_buf, dst_buf, src, dst = _pools(rng, idx, L, H, D, e, lay_s, bs_s, NBs, lay_d, bs_d, NBd)
     src_np = P.to_numpy(src_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd)
     Ts = [t for t, _, _ in reqs]
     total, max_t = sum(Ts), max(Ts) + int(rng.integers(0, 9))
     st, dt, _ = _device_tables(reqs, max(1, -(-max_t // bs_s)), max(1, -(-max_t // bs_d)))

@@ -1166,3 +1166,131 @@ def test_distinct_plans_from_distinct_threads_on_distinct_streams():
     for k, w in enumerate(works):
         G.assert_same(P.to_numpy(dps[k].dst_buf), G.oracle_transfer(w, srcs[k]), f"thread {k} ({w.name})")
         G.assert_same(P.to_numpy(dps[k].src_buf), srcs[k], "src pool must not change")
+
+
+def _separate_layers(rng, L, H, D, e, NB, BS, unit=32):
+    """A cache whose layers are separate allocations (reading A22): every layer a (2,NB,BS,H,D) tensor at a shuffled,
+    gapped offset of one device buffer -> (oracle geometry, offsets, total bytes)."""
+    one = O.PoolGeom.lkbthd(1, H, D, e, NB, BS)
+    off, pos = [0] * L, unit * int(rng.integers(0, 4))
+    for l in rng.permutation(L):
+        off[int(l)] = pos
+        pos += one.layer_bytes() + unit * int(rng.integers(1, 9))
+    g = O.PoolGeom(L, H, D, e, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head).with_layer_offsets(off)
+    return g, off, pos
+
+
+@pytest.mark.parametrize("dst_kind", ["lkbthd", "separate", "blkthd", "blkhtd32"])
+@pytest.mark.parametrize("tuning", [None, {"variant": "bulk"}, {"plan_in_params": 1, "tile_bytes": 4096}])
+def test_pools_whose_layers_are_separate_allocations(dst_kind, tuning):
+    """before Eq. 5 the cache is 'separate tensor structures across all layer dimensions'.  src = L tensors at
+    scattered addresses (flowkv_pool.layer_offsets, base in the MIDDLE so some offsets are negative); dst = a stacked
+    pool, another set of separate tensors, or ONE (B,L,2,H) tensor — the paper's own migration — incl. a block-size
+    change.  Transfer, layer range, pack / unpack, windows, the table-driven kernel and the memcpy baseline against
+    the oracle over whole buffers (the gaps between the tensors stay untouched)."""
+    rng = np.random.default_rng(4100 + len(dst_kind))
+    L, H, D, e, NBs, BS = 5, 4, 64, 2, 40, 16
+    gs, soff, sbytes = _separate_layers(rng, L, H, D, e, NBs, BS)
+    src_buf = P.alloc_bytes(sbytes)
+    P.fill_values(src_buf, "bits", "fp16", 4100)
+    src_np = P.to_numpy(src_buf)
+    mid = soff[2]
+    src = F.make_pool(src_buf.data_ptr() + mid, L, H, D, e, NBs, BS, "lkbthd", layer_offsets=[o - mid for o in soff])
+    if dst_kind == "separate":
+        NBd, bs_d = 24, BS
+        gd, doff, dbytes = _separate_layers(rng, L, H, D, e, NBd, bs_d, unit=16)      # 16-byte aligned only: 128-bit path
+        dst_buf = P.alloc_bytes(dbytes)
+        dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "lkbthd", layer_offsets=doff)
+    else:
+        lay, bs_d = {"lkbthd": ("lkbthd", BS), "blkthd": ("blkthd", BS), "blkhtd32": ("blkhtd", 32)}[dst_kind]
+        NBd = 24 * BS // bs_d
+        gd = getattr(O.PoolGeom, lay)(L, H, D, e, NBd, bs_d)
+        dst_buf = P.alloc_bytes(gd.span_bytes())
+        dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, lay)
+    Ts = [150, 0, 77, 16]
+    stab = rng.permutation(NBs)
+    dtab = rng.permutation(NBd)
+    reqs, so, do = [], 0, 0
+    for t in Ts:
+        a, b = -(-t // BS), -(-t // bs_d)
+        reqs.append((t, stab[so:so + a].astype(np.int32), dtab[do:do + b].astype(np.int32)))
+        so, do = so + a, do + b
+    freqs = [F.Request(t, a, b) for t, a, b in reqs]
+    s = torch.cuda.current_stream().cuda_stream
+
+    def expect(l0=0, l1=L):
+        exp = np.full(dst_buf.numel(), P.SENTINEL_BYTE, np.uint8)
+        for t, a, b in reqs:
+            O.transfer(src_np, gs, exp, gd, a, b, t, l0, l1)
+        return exp
+
+    what = f"separate layers -> {dst_kind} {tuning}"
+    plan = F.flowkv_plan(src, dst, freqs, F.FLOWKV_CHECK_DST_ALIAS, tuning, s)
+    st = plan.stats
+    assert st["mode_transfer"] == (1 if dst_kind in ("lkbthd", "separate") else 2)
+    assert st["vec_bytes"] == (16 if dst_kind == "separate" else 32)
+    if tuning and tuning.get("variant") == "bulk":      # span: the bulk ring; rows: no tensor map for such a pool
+        assert st["variant"] == (F.FLOWKV_VARIANT_BULK if st["mode_transfer"] == 1 else F.FLOWKV_VARIANT_LDST)
+    P.fill_sentinel(dst_buf)
+    n0 = F.flowkv_launch_count()
+    plan.transfer(s)
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1
+    G.assert_same(P.to_numpy(dst_buf), expect(), what + ": transfer")
+    P.fill_sentinel(dst_buf)
+    F.flowkv_transfer_layers(plan, 1, 4, s)
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dst_buf), expect(1, 4), what + ": layers [1,4)")
+    # wire format and a window
+    nbytes = st["staging_bytes"]
+    staging = P.alloc_bytes(nbytes)
+    P.fill_sentinel(staging)
+    P.fill_sentinel(dst_buf)
+    plan.pack(staging.data_ptr(), nbytes, s)
+    plan.unpack(staging.data_ptr(), nbytes, s)
+    torch.cuda.synchronize()
+    wire = np.full(nbytes, P.SENTINEL_BYTE, np.uint8)
+    off = 0
+    for t, a, _ in reqs:
+        O.pack(src_np, gs, a, t, wire, off)
+        off += t
+    G.assert_same(P.to_numpy(staging), wire, what + ": wire bytes")
+    G.assert_same(P.to_numpy(dst_buf), expect(), what + ": unpack")
+    nb = F.flowkv_window_bytes(plan, 2, 5)
+    win = P.alloc_bytes(nb)
+    F.flowkv_pack_window(plan, win.data_ptr(), nb, 2, 5, s)
+    torch.cuda.synchronize()
+    wexp = np.full(nb, P.SENTINEL_BYTE, np.uint8)
+    off = 0
+    for t, a, _ in reqs:
+        O.pack_window(src_np, gs, a, t, wexp, off, 2, 5)
+        off += t
+    G.assert_same(P.to_numpy(win), wexp, what + ": window [2,5)")
+    # memcpy baseline (token-major on both sides only) walks the same per-layer addresses
+    if dst_kind in ("lkbthd", "separate"):
+        P.fill_sentinel(dst_buf)
+        calls = F.flowkv_baseline_segmentwise(plan, s)
+        torch.cuda.synchronize()
+        assert calls == st["n_segments"] * 2 * L
+        G.assert_same(P.to_numpy(dst_buf), expect(), what + ": segmentwise memcpy baseline")
+    plan.destroy()
+    # table-driven: nothing planned, tables on the device
+    if tuning is None:
+        n = len(reqs)
+        ws, wd = max(len(a) for _, a, _ in reqs), max(len(b) for _, _, b in reqs)
+        st_ = np.full((n, ws), -3, np.int32)
+        dt_ = np.full((n, wd), -3, np.int32)
+        for i, (_, a, b) in enumerate(reqs):
+            st_[i, :len(a)], dt_[i, :len(b)] = a, b
+        dst_t, ddt_t = torch.from_numpy(st_).cuda(), torch.from_numpy(dt_).cuda()
+        lens = torch.tensor(Ts, dtype=torch.int32, device="cuda")
+        flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+        P.fill_sentinel(dst_buf)
+        F.flowkv_transfer_tables_layers(src, dst, dst_t.data_ptr(), ddt_t.data_ptr(), lens.data_ptr(), n, ws, wd, max(Ts), 0, 3,
+                                        flag.data_ptr(), None, s)
+        F.flowkv_transfer_tables_layers(src, dst, dst_t.data_ptr(), ddt_t.data_ptr(), lens.data_ptr(), n, ws, wd, max(Ts), 3, L,
+                                        flag.data_ptr(), None, s)
+        torch.cuda.synchronize()
+        assert int(flag.item()) == 0
+        G.assert_same(P.to_numpy(dst_buf), expect(), what + ": table-driven, two layer ranges")
+    G.assert_same(P.to_numpy(src_buf), src_np, what + ": src unchanged")

@@ -37,7 +37,8 @@ def test_library_exports_every_symbol_the_header_declares():
 
 
 def test_struct_sizes_match_header_layout():
-    assert C.sizeof(F.flowkv_pool) == 8 + 8 * 4 + 5 * 8
+    assert C.sizeof(F.flowkv_pool) == 8 + 8 * 4 + 5 * 8 + 8          # + layer_offsets (FLOWKV_VERSION 4)
+    assert F.flowkv_pool.layer_offsets.offset == 80
     assert C.sizeof(F.flowkv_request) == 32
     assert C.sizeof(F.flowkv_segment) == 40
     assert C.sizeof(F.flowkv_tuning) == 48
@@ -385,3 +386,39 @@ def test_request_batch_marshalled_once_plans_like_the_list():
     # the schedule walks scattered batches in dst-address order, the reported segments stay in request / token order
     segs = a.segments
     assert [(s["request"], s["first_token"]) for s in segs] == sorted((s["request"], s["first_token"]) for s in segs)
+
+
+def test_pools_whose_layers_are_separate_allocations_on_the_host_side():
+    """flowkv_pool.layer_offsets (reading A22; P:L98 'separate tensor structures across all layer dimensions'): the
+    alignment is unchanged (layers play no part in it), a token-major pool stays in span mode, two block-major pools
+    are no longer flat (a block is not one byte range), a misaligned offset is refused, the layer stride is ignored."""
+    L, NB, BS = 3, 16, 4
+    stab, dtab = [5, 6, 7, 1, 2], [0, 1, 2, 3, 9]
+    req = [F.Request(18, stab, dtab)]
+    plain = F.flowkv_plan_host(_pool("lkbthd", L=L), _pool("lkbthd", L=L), req)
+    one = O.PoolGeom.lkbthd(1, 2, 8, 2, NB, BS)
+    off = [4096 + one.layer_bytes(), 0, 3 * 4096 + 2 * one.layer_bytes()]            # shuffled, gapped
+    sep = F.make_pool(FAKE + 65536, L, 2, 8, 2, NB, BS, "lkbthd", layer_offsets=[o - 4096 for o in off])   # negative too
+    p = F.flowkv_plan_host(sep, _pool("lkbthd", L=L), req)
+    assert _segs(p) == _segs(plain) and p.stats["n_segments"] == O.count_segments(stab, BS, dtab, BS, 18)
+    assert p.stats["mode_transfer"] == 1 and p.stats["mode_pack"] == 1                # span: strides inside a layer decide
+    assert F.pool_bytes(sep) == max(off) - 4096 + one.layer_bytes()
+    # block-major + block-major would be flat; with separate layers on one side it is not
+    bm = _pool("blkthd", L=L)
+    assert F.flowkv_plan_host(bm, _pool("blkthd", L=L), req).stats["mode_transfer"] == 3
+    bms = F.make_pool(FAKE, L, 2, 8, 2, NB, BS, "blkthd", layer_offsets=[l * bm.stride_bytes[0] for l in range(L)])
+    assert F.flowkv_plan_host(bms, _pool("blkthd", L=L), req).stats["mode_transfer"] == 2
+    # the layer stride is ignored (may be anything, even 0) once offsets are given
+    st = list(sep.stride_bytes)
+    st[0] = 0
+    z = F.make_pool(FAKE, L, 2, 8, 2, NB, BS, "strided", st, layer_offsets=off)
+    assert _segs(F.flowkv_plan_host(z, _pool("lkbthd", L=L), req)) == _segs(plain)
+    with pytest.raises(F.FlowKVError) as ei:
+        F.flowkv_plan_host(F.make_pool(FAKE, L, 2, 8, 2, NB, BS, "lkbthd", layer_offsets=[0, 4104, 8192]), _pool("lkbthd", L=L), req)
+    assert ei.value.status == F.FLOWKV_ERR_ALIGN and "layer offset" in str(ei.value)
+    # 32-byte vectors need 32-byte aligned offsets
+    v32 = F.flowkv_plan_host(F.make_pool(FAKE, L, 2, 16, 2, NB, BS, "lkbthd", layer_offsets=[0, 1 << 20, 2 << 20]),
+                             _pool("lkbthd", L=L, D=16), req)
+    v16 = F.flowkv_plan_host(F.make_pool(FAKE, L, 2, 16, 2, NB, BS, "lkbthd", layer_offsets=[0, (1 << 20) + 16, 2 << 20]),
+                             _pool("lkbthd", L=L, D=16), req)
+    assert v32.stats["vec_bytes"] == 32 and v16.stats["vec_bytes"] == 16
