@@ -116,6 +116,10 @@ def build_workload(name: str, free_bytes: int):
         return (synth.config2_llama8b_13k(),
                 "configs[1] Llama-3-8B KV: 32 layers, 8 KV heads, head_dim 128, bf16, block 16, 1 x 13,312 tokens, "
                 "src 16,384-block pool (32 GiB) runs~Geom(mean 4), dst contiguous")
+    if name == "cfg2sep":
+        return (synth.config2_llama8b_13k(),
+                "configs[1] request and tables, src pool as 32 SEPARATE per-layer tensors of 1 GiB (the cache the paper "
+                "starts from, P:L98; flowkv_pool.layer_offsets), dst one contiguous pool")
     if name in ("cfg2bm", "cfg2bm_ragged"):
         w = synth.config2_blockmajor("blkthd", tokens=13312 if name == "cfg2bm" else 13307)
         return w, ("configs[1] request and tables, both pools in the paper's (B,L,2,H) order (Eq. 5; BLKTHD): "
@@ -464,7 +468,7 @@ def run_ours(args) -> None:
         if args.same_device:
             free_b //= world
         w, desc = build_workload(args.config, free_b)
-        dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False)
+        dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False, separate_src_layers=args.config == "cfg2sep")
         payload = w.payload_bytes
         # --peer: rank r's kernel stores into the dst pool that rank (r+1) % N owns, mapped through CUDA IPC — the paper's
         # single-machine "IPC" mode as a one-sided put; over NVLink when the ranks sit on different GPUs
@@ -709,7 +713,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg2bm", "cfg2bm_ragged", "cfg3", "cfg4"])
+    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg2sep", "cfg2bm", "cfg2bm_ragged", "cfg3", "cfg4"])
     ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
     ap.add_argument("--device-tables", action="store_true",
                     help="time flowkv_transfer_tables (block tables resident on the device, no plan) instead of plan+transfer")
@@ -732,6 +736,8 @@ def main() -> None:
     ap.add_argument("--same-device", action="store_true", help="all ranks on cuda:0 with a gloo control plane (a "
                     "functional check of the multi-rank path on a one-GPU box; not a scaling number)")
     args = ap.parse_args()
+    if args.config == "cfg2sep":     # the src pool is 32 separate tensors: no whole-pool probes, link legs or memcpy baselines
+        args.no_e2e = args.no_baselines = True
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         spawn_ranks(args)          # does not return
     if args.sweep:

@@ -16,7 +16,8 @@
  * Result that every entry point below reaches exactly (pure byte movement):
  *   for every request r, token t in [0,T_r), layer l, c in {K,V}, head h, dim d
  *     dst[l, c, Dst_r[t div BS_d], t mod BS_d, h, d] := src[l, c, Src_r[t div BS_s], t mod BS_s, h, d]
- *   each side addressed as base + l*s_layer + c*s_kv + blk*s_block + tok*s_token + h*s_head + d*e.
+ *   each side addressed as base + l*s_layer + c*s_kv + blk*s_block + tok*s_token + h*s_head + d*e
+ *   (layer_offsets[l] in place of l*s_layer for a pool whose layers are separate allocations).
  *   Every other byte of dst keeps its value; src is never written.
  *
  * Conventions

@@ -59,15 +59,31 @@ def requests_of(w: synth.Workload, src: bool = True, dst: bool = True) -> Sequen
 class DevicePools:
     """src + dst pools of a workload on one device, described for the library."""
 
-    def __init__(self, w: synth.Workload, device="cuda:0", fill: Optional[str] = None, sentinel_dst: bool = True):
+    def __init__(self, w: synth.Workload, device="cuda:0", fill: Optional[str] = None, sentinel_dst: bool = True,
+                 separate_src_layers: bool = False):
+        """``separate_src_layers``: the src pool (LKBTHD) is allocated as one tensor PER LAYER — the cache the paper
+        starts from — and described through ``flowkv_pool.layer_offsets``; ``src_layers`` holds the tensors and
+        ``src_buf`` is layer 0's."""
         self.w = w
         self.device = torch.device(device)
-        self.src_buf = alloc_bytes(w.src.bytes(w.shape), device)
         self.dst_buf = alloc_bytes(w.dst.bytes(w.shape), device)
-        fill_values(self.src_buf, fill or w.value_dist, w.shape.dtype, w.seed)
+        if separate_src_layers:
+            assert w.src.layout == "lkbthd", "separate layer tensors are (2,B,H) each"
+            L = w.shape.num_layers
+            per = w.src.bytes(w.shape) // L
+            self.src_layers = [alloc_bytes(per, device) for _ in range(L)]
+            for l, t in enumerate(self.src_layers):
+                fill_values(t, fill or w.value_dist, w.shape.dtype, w.seed + l)
+            base = min(t.data_ptr() for t in self.src_layers)
+            self.src_buf = self.src_layers[0]
+            self.src = F.make_pool(base, L, w.shape.num_kv_heads, w.shape.head_dim, w.shape.elem_bytes, w.src.num_blocks,
+                                   w.src.block_size, "lkbthd", layer_offsets=[t.data_ptr() - base for t in self.src_layers])
+        else:
+            self.src_buf = alloc_bytes(w.src.bytes(w.shape), device)
+            fill_values(self.src_buf, fill or w.value_dist, w.shape.dtype, w.seed)
+            self.src = describe(w.src, w.shape, self.src_buf.data_ptr())
         if sentinel_dst:
             fill_sentinel(self.dst_buf)
-        self.src = describe(w.src, w.shape, self.src_buf.data_ptr())
         self.dst = describe(w.dst, w.shape, self.dst_buf.data_ptr())
         self.requests = requests_of(w)
         self.batch = F.RequestBatch(self.requests)      # marshalled once; what bench.py's timed step passes

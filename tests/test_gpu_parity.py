@@ -1294,3 +1294,24 @@ def test_pools_whose_layers_are_separate_allocations(dst_kind, tuning):
         assert int(flag.item()) == 0
         G.assert_same(P.to_numpy(dst_buf), expect(), what + ": table-driven, two layer ranges")
     G.assert_same(P.to_numpy(src_buf), src_np, what + ": src unchanged")
+
+
+def test_src_layers_as_really_separate_torch_allocations():
+    """The same through REAL separate allocations: one torch tensor per layer (`DevicePools(separate_src_layers=True)`),
+    offsets = differences of their device pointers (any sign, any size).  dst equals the oracle run layer by layer on
+    each tensor's own bytes."""
+    w = synth.config2_llama8b_13k(num_layers=3)
+    dp = P.DevicePools(w, separate_src_layers=True)
+    assert len({t.data_ptr() for t in dp.src_layers}) == 3 and dp.src.layer_offsets
+    plan, s = dp.plan(F.FLOWKV_CHECK_DST_ALIAS), torch.cuda.current_stream().cuda_stream
+    plan.transfer(s)
+    torch.cuda.synchronize()
+    r = w.requests[0]
+    one_s = G.geom(w.src, w.shape, num_layers=1)
+    gd = G.geom(w.dst, w.shape)
+    exp = np.full(w.dst.bytes(w.shape), P.SENTINEL_BYTE, np.uint8)
+    for l, t in enumerate(dp.src_layers):          # layer l of dst := layer 0 of the 1-layer pool that tensor l is
+        O.transfer(P.to_numpy(t), one_s, exp[l * gd.s_layer:(l + 1) * gd.s_layer], G.geom(w.dst, w.shape, num_layers=1),
+                   r.src_blocks, r.dst_blocks, r.num_tokens)
+    G.assert_same(P.to_numpy(dp.dst_buf), exp, "separate torch tensors per layer")
+    plan.destroy()
