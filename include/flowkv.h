@@ -194,7 +194,8 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
  *   out      : HOST pointer; receives the plan (caller destroys it).  Untouched on error.
  * The plan stays valid until destroyed; pools must stay alive while it is run.  The first plan (or table-driven call)
  * that names a new layer_offsets[] array copies it to the device once (8*L bytes on the library's own stream, waited
- * for; cached by content for the life of the process) — the one exception to "does not synchronise".
+ * for; cached by content for the life of the process) — the one exception to "does not synchronise".  Inside a
+ * stream capture the table must already be cached: make one call (or build any plan) with the same offsets first.
  * Errors (nothing is allocated or enqueued when one is returned):
  *   INVALID_ARG  out NULL, both pools NULL, reqs NULL with n_reqs > 0, a table pointer NULL, unknown flag /
  *                layout / tuning value, a zero shape field or a stride <= 0
