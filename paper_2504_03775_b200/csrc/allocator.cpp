@@ -61,9 +61,14 @@ flowkv_status flowkv_alloc_create(uint32_t num_blocks, flowkv_allocator_t** out)
   if (!out || !num_blocks) return fail(FLOWKV_ERR_INVALID_ARG, "allocator: out is NULL or num_blocks is 0");
   flowkv_allocator_s* a = new (std::nothrow) flowkv_allocator_s();
   if (!a) return fail(FLOWKV_ERR_NOMEM, "out of host memory");
-  a->num_blocks = a->free_blocks = num_blocks;
-  a->used.assign(num_blocks, 0);
-  a->insert(0, num_blocks);
+  try {
+    a->num_blocks = a->free_blocks = num_blocks;
+    a->used.assign(num_blocks, 0);
+    a->insert(0, num_blocks);
+  } catch (...) {                  // the guard of the C ABI turns it into a status; do not leak the object
+    delete a;
+    throw;
+  }
   *out = a;
   return FLOWKV_OK;
 }
