@@ -105,7 +105,10 @@ typedef struct {
 } flowkv_pool;
 
 /* One request: its length and both sides' block-id lists.
- * HOST pointers, borrowed only for the duration of flowkv_plan(). */
+ * HOST pointers, borrowed only for the duration of flowkv_plan().
+ * A request need not start at token 0 of a sequence: to move only tokens [t0, T) — the suffix a prefix-cache match on
+ * the decode side leaves, or the chunk a chunked prefill has just produced — pass the tables from entry
+ * t0 / block_size on and num_tokens = T - t0 (t0 a multiple of both block sizes). */
 typedef struct {
   uint32_t       num_tokens;     /* T_r; 0 is legal (contributes nothing)                          */
   uint32_t       n_src_blocks;   /* must equal ceil(T_r / src.block_size) when src pool is given   */

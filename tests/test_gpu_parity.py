@@ -1273,6 +1273,15 @@ def test_pools_whose_layers_are_separate_allocations(dst_kind, tuning):
         torch.cuda.synchronize()
         assert calls == st["n_segments"] * 2 * L
         G.assert_same(P.to_numpy(dst_buf), expect(), what + ": segmentwise memcpy baseline")
+    # the host route (pack windows -> pinned host -> unpack windows) walks the same per-layer addresses
+    if tuning is None:
+        host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+        sb = F.flowkv_via_host_scratch_bytes(plan, 7)
+        scratch = P.alloc_bytes(sb)
+        P.fill_sentinel(dst_buf)
+        F.flowkv_transfer_via_host(plan, host.data_ptr(), nbytes, 7, 0, s, scratch.data_ptr(), sb)
+        torch.cuda.synchronize()
+        G.assert_same(P.to_numpy(dst_buf), expect(), what + ": host route")
     plan.destroy()
     # table-driven: nothing planned, tables on the device
     if tuning is None:
