@@ -27,7 +27,7 @@
  * 1-, 4- and 8-byte elements against numpy item views (the generic branch of
  * okv_copy_elem), all 256 byte codes and fp32 NaN payloads,
  * pack∘unpack identity, layer windows and plane windows == planes cut out of the wire format,
- * pools whose layers are separate allocations (layer_off, A22) == numpy fancy indexing layer by layer,
+ * pools whose planes are separate allocations (plane_off, A22 / A3) == numpy fancy indexing plane by plane,
  * brute-force minimal partition count on tiny tables,
  * the paper's "fully contiguous => 1 transfer" and
  * "calls per block = L x 2", hand-worked fixtures in tests/golden/.
@@ -41,24 +41,25 @@
 /* Geometry of one paged pool.  Strides are in BYTES; dim stride is elem_bytes.
  * `layer0`: the buffer handed in starts at layer `layer0` of the logical pool
  * (lets a caller hand over one layer slab of a pool too big for host RAM). */
-/* `layer_off` (reading A22): the pool the paper STARTS from keeps every layer in a tensor of its own
- * ("combines the separate tensor structures across all layer dimensions into a continuous tensor"), so
- * the layers are separate allocations with no common stride.  When layer_off != NULL, layer l begins
- * layer_off[l] bytes after the buffer's first byte and s_layer is not used (layer0 must then be 0);
- * inside a layer nothing changes. */
+/* `plane_off` (readings A22 and A3): the pool the paper STARTS from keeps every layer in a tensor of its
+ * own ("combines the separate tensor structures across all layer dimensions into a continuous tensor"), and K
+ * and V may be separate tensors too (A3), so the planes — plane = 2*layer + (0 for K, 1 for V) — are separate
+ * allocations with no common stride.  When plane_off != NULL, plane (l, c) begins plane_off[2*l + c] bytes after the
+ * buffer's first byte and neither s_layer nor s_kv is used (layer0 must then be 0); inside a plane nothing changes. */
 typedef struct {
   uint32_t num_layers, num_kv_heads, head_dim, elem_bytes;
   uint32_t num_blocks, block_size;
   int64_t  s_layer, s_kv, s_block, s_token, s_head;
   uint32_t layer0;
   uint32_t _pad;
-  const int64_t* layer_off;
+  const int64_t* plane_off;
 } okv_pool;
 
 static inline int64_t okv_addr(const okv_pool* p, uint32_t l, uint32_t c, int64_t blk,
                                uint32_t tok, uint32_t h, uint32_t d) {
-  const int64_t layer = p->layer_off ? p->layer_off[l] : (int64_t)(l - p->layer0) * p->s_layer;
-  return layer + (int64_t)c * p->s_kv + blk * p->s_block +
+  const int64_t plane = p->plane_off ? p->plane_off[2 * l + c]
+                                     : (int64_t)(l - p->layer0) * p->s_layer + (int64_t)c * p->s_kv;
+  return plane + blk * p->s_block +
          (int64_t)tok * p->s_token + (int64_t)h * p->s_head + (int64_t)d * p->elem_bytes;
 }
 

@@ -38,7 +38,7 @@ class _Pool(C.Structure):
         ("s_layer", C.c_int64), ("s_kv", C.c_int64), ("s_block", C.c_int64),
         ("s_token", C.c_int64), ("s_head", C.c_int64),
         ("layer0", C.c_uint32), ("_pad", C.c_uint32),
-        ("layer_off", C.c_void_p),
+        ("plane_off", C.c_void_p),
     ]
 
 
@@ -97,20 +97,30 @@ class PoolGeom:
     s_block: int
     s_token: int
     s_head: int
-    layer_off: tuple | None = None      # reading A22: byte offset of every layer (separate allocations); s_layer unused
+    plane_off: tuple | None = None      # readings A22 / A3: byte offset of every plane 2*l + c (separate allocations)
 
-    def with_layer_offsets(self, layer_off) -> "PoolGeom":
-        """The same pool with every layer at its own byte offset from the buffer start (the cache the paper
-        starts from keeps 'separate tensor structures across all layer dimensions')."""
-        off = tuple(int(x) for x in layer_off)
-        assert len(off) == self.num_layers
+    def with_plane_offsets(self, plane_off) -> "PoolGeom":
+        """The same pool with every plane (layer, K|V) at its own byte offset from the buffer start; s_layer and s_kv
+        are then unused (the cache the paper starts from keeps 'separate tensor structures across all layer
+        dimensions'; A3: K and V may be separate tensors as well)."""
+        off = tuple(int(x) for x in plane_off)
+        assert len(off) == 2 * self.num_layers
         return PoolGeom(self.num_layers, self.num_kv_heads, self.head_dim, self.elem_bytes, self.num_blocks,
                         self.block_size, self.s_layer, self.s_kv, self.s_block, self.s_token, self.s_head, off)
 
-    def layer_bytes(self) -> int:
-        """Bytes from the first to one past the last addressable element of ONE layer."""
-        return (self.s_kv + (self.num_blocks - 1) * self.s_block + (self.block_size - 1) * self.s_token
+    def with_layer_offsets(self, layer_off) -> "PoolGeom":
+        """One tensor per layer with K and V stacked inside it: plane (l, c) at layer_off[l] + c * s_kv."""
+        assert len(layer_off) == self.num_layers
+        return self.with_plane_offsets([int(o) + c * self.s_kv for o in layer_off for c in (0, 1)])
+
+    def plane_bytes(self) -> int:
+        """Bytes from the first to one past the last addressable element of ONE plane."""
+        return ((self.num_blocks - 1) * self.s_block + (self.block_size - 1) * self.s_token
                 + (self.num_kv_heads - 1) * self.s_head + self.head_dim * self.elem_bytes)
+
+    def layer_bytes(self) -> int:
+        """The same for ONE layer with K and V stacked (s_kv apart)."""
+        return self.s_kv + self.plane_bytes()
 
     @staticmethod
     def lkbthd(L, Hkv, Dh, e, NB, BS) -> "PoolGeom":
@@ -146,8 +156,8 @@ class PoolGeom:
 
     def span_bytes(self) -> int:
         """Bytes from the first to one past the last addressable element."""
-        if self.layer_off is not None:
-            return max(self.layer_off) + self.layer_bytes()
+        if self.plane_off is not None:
+            return max(self.plane_off) + self.plane_bytes()
         return ((self.num_layers - 1) * self.s_layer + self.s_kv + (self.num_blocks - 1) * self.s_block
                 + (self.block_size - 1) * self.s_token + (self.num_kv_heads - 1) * self.s_head
                 + self.head_dim * self.elem_bytes)
@@ -156,10 +166,10 @@ class PoolGeom:
         p = _Pool(self.num_layers, self.num_kv_heads, self.head_dim, self.elem_bytes,
                   self.num_blocks, self.block_size, self.s_layer, self.s_kv, self.s_block,
                   self.s_token, self.s_head, layer0, 0, None)
-        if self.layer_off is not None:
-            assert layer0 == 0, "a pool of separate layers is handed over whole"
-            p._keep = np.asarray(self.layer_off, dtype=np.int64)     # kept alive by the struct object
-            p.layer_off = p._keep.ctypes.data
+        if self.plane_off is not None:
+            assert layer0 == 0, "a pool of separate planes is handed over whole"
+            p._keep = np.asarray(self.plane_off, dtype=np.int64)     # kept alive by the struct object
+            p.plane_off = p._keep.ctypes.data
         return p
 
 

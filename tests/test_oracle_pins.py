@@ -751,3 +751,45 @@ def test_separate_layers_into_one_block_major_tensor_is_eq5():
     O.transfer(src, gs, dst, gd, ident, ident, NB * BS)
     exp = np.stack([a.reshape(2, NB, Hbytes) for a in layers]).transpose(2, 0, 1, 3).reshape(-1)
     assert np.array_equal(dst, exp)
+
+
+@pytest.mark.parametrize("layout_in_plane", ["token_major", "head_major"])
+def test_separate_k_and_v_tensors_per_layer_equal_numpy_fancy_indexing_plane_by_plane(layout_in_plane):
+    """Readings A22 + A3: K and V of every layer are tensors of their own ([NB][BS][H][D] or [NB][H][BS][D]) at shuffled,
+    gapped offsets; the move must equal `dst_p[Dst] = src_p[Src]` for each of the 2L planes separately.  Catches: K and
+    V offsets swapped (2*l + c vs 2*c + l or l + c*L), s_kv still added on top of a plane offset, a plane offset applied
+    to the neighbouring layer."""
+    rng = np.random.default_rng(2230)
+    L, H, D, NB, BS, n, e = 3, 2, 8, 6, 4, 4, 2
+    per = NB * BS * H * D * e
+    src_planes = [rng.integers(0, 256, size=per, dtype=np.uint8) for _ in range(2 * L)]
+    src, soff = _scatter_layers(rng, src_planes)
+    dst_planes = [np.full(per, SENT, np.uint8) for _ in range(2 * L)]
+    dst, doff = _scatter_layers(rng, dst_planes)
+    row = D * e
+    if layout_in_plane == "token_major":
+        s_head, s_token = row, H * row
+        view = lambda a: a.view(np.uint16).reshape(NB, BS, H, D)
+    else:
+        s_token, s_head = row, BS * row
+        view = lambda a: a.view(np.uint16).reshape(NB, H, BS, D).transpose(0, 2, 1, 3)
+    s_block = BS * H * row
+    bogus_kv, bogus_layer = 5 * per + 16, 11 * per + 32          # must not be used once plane offsets are given
+    gs = O.PoolGeom(L, H, D, e, NB, BS, bogus_layer, bogus_kv, s_block, s_token, s_head).with_plane_offsets(soff)
+    gd = O.PoolGeom(L, H, D, e, NB, BS, bogus_layer, bogus_kv, s_block, s_token, s_head).with_plane_offsets(doff)
+    Src, Dst = rng.permutation(NB)[:n], rng.permutation(NB)[:n]
+    T = n * BS - 1
+    exp = dst.copy()
+    O.transfer(src, gs, dst, gd, Src, Dst, T)
+    full = T // BS
+    for p in range(2 * L):
+        sv = view(src_planes[p])
+        ev = view(exp[doff[p]:doff[p] + per])
+        ev[Dst[:full]] = sv[Src[:full]]
+        ev[Dst[full], :T % BS] = sv[Src[full], :T % BS]
+    assert np.array_equal(dst, exp)
+    # the wire format sees the planes in order 2*l + c whatever their addresses are
+    wire = np.full(T * gs.bytes_per_token, SENT, np.uint8)
+    O.pack(src, gs, Src, T, wire, 0)
+    toks = np.stack([np.concatenate([view(src_planes[p])[b] for b in Src])[:T] for p in range(2 * L)])     # [plane][t][h][d]
+    assert np.array_equal(wire.view(np.uint16), toks.reshape(-1))
