@@ -119,7 +119,7 @@ def build_workload(name: str, free_bytes: int):
     if name == "cfg2sep":
         return (synth.config2_llama8b_13k(),
                 "configs[1] request and tables, src pool as 32 SEPARATE per-layer tensors of 1 GiB (the cache the paper "
-                "starts from, P:L98; flowkv_pool.layer_offsets), dst one contiguous pool")
+                "starts from, P:L98; flowkv_pool.plane_offsets), dst one contiguous pool")
     if name in ("cfg2bm", "cfg2bm_ragged"):
         w = synth.config2_blockmajor("blkthd", tokens=13312 if name == "cfg2bm" else 13307)
         return w, ("configs[1] request and tables, both pools in the paper's (B,L,2,H) order (Eq. 5; BLKTHD): "
@@ -555,6 +555,14 @@ def run_ours(args) -> None:
             barrier()
             te = a.elapsed_time(b)
             te = shard.max_over_ranks(te, device=reduce_dev)
+            # latency view of the same route: one synchronous request at a time, host wall clock, plan call -> drained
+            e2e_lat = []
+            for _ in range(5):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                e2e_step()
+                torch.cuda.synchronize()
+                e2e_lat.append((time.perf_counter() - t0) * 1e3)
             # link references: one contiguous copy-engine D2H / H2D of the same bytes, alone and both at once
             pb = min(nbytes, 2 << 30)                             # link probes: at most 2 GiB each way
             dev_flat = dp.dst_buf[:pb] if dp.dst_buf.numel() >= pb else P.alloc_bytes(pb)
@@ -608,6 +616,7 @@ def run_ours(args) -> None:
                 line["e2e"] = {"value": e2e_val, "unit": UNIT,
                                "h2d_bytes_per_step": nbytes + stats["plan_device_bytes"], "d2h_bytes_per_step": nbytes,
                                "steps": Ke, "ms_per_step": te / Ke,
+                               "latency_ms_call_to_done": float(np.median(e2e_lat)),
                                "path": ("flowkv_plan (host tables) + flowkv_pack to pinned host + flowkv_unpack from pinned host"
                                         if args.e2e_serial else
                                         "flowkv_plan (host tables) + flowkv_transfer_via_host, direct mode: pack kernels store to "

@@ -17,7 +17,7 @@
  *   for every request r, token t in [0,T_r), layer l, c in {K,V}, head h, dim d
  *     dst[l, c, Dst_r[t div BS_d], t mod BS_d, h, d] := src[l, c, Src_r[t div BS_s], t mod BS_s, h, d]
  *   each side addressed as base + l*s_layer + c*s_kv + blk*s_block + tok*s_token + h*s_head + d*e
- *   (layer_offsets[l] in place of l*s_layer for a pool whose layers are separate allocations).
+ *   (plane_offsets[2*l + c] in place of l*s_layer + c*s_kv for a pool whose planes are separate allocations).
  *   Every other byte of dst keeps its value; src is never written.
  *
  * Conventions
@@ -95,13 +95,16 @@ typedef struct {
   uint32_t layout;          /* flowkv_layout                                                        */
   uint32_t _reserved;
   int64_t  stride_bytes[5]; /* layer, kv, block, token, head — see FLOWKV_S_*; multiples of 16      */
-  const int64_t* layer_offsets; /* NULL, or HOST array [num_layers] (borrowed for the call; a plan keeps a copy): layer l
-                             * starts layer_offsets[l] bytes from `base` and stride_bytes[FLOWKV_S_LAYER] is ignored.  For
-                             * a cache whose layers are separate allocations — the state the paper starts from
-                             * "separate tensor structures across all layer dimensions" (reading A22): set
-                             * base to any one of them and the offsets to the signed distances; multiples of 16, any
-                             * order, gaps allowed.  The other four strides describe one layer.  Such pools run the
-                             * register / bulk-copy paths (no flat mode, no TMA tensor path). */
+  const int64_t* plane_offsets; /* NULL, or HOST array [2*num_layers] (borrowed for the call; a plan keeps a copy): plane
+                             * p = 2*layer + (0 for K, 1 for V) starts plane_offsets[p] bytes from `base`, and
+                             * stride_bytes[FLOWKV_S_LAYER] and [FLOWKV_S_KV] are ignored.  For a cache whose layers — and
+                             * possibly K and V inside a layer — are separate allocations: the state the paper starts
+                             * from, "separate tensor structures across all layer dimensions" (DESIGN.md readings
+                             * A22, A3).  Set base to any one of the tensors and the offsets to the signed distances;
+                             * multiples of 16, any order, gaps allowed.  One tensor per layer with K and V stacked inside
+                             * is plane_offsets[2l + c] = layer_offset[l] + c * s_kv.  The block, token and head strides
+                             * describe one plane.  Such pools run the register / bulk-copy paths (no flat mode, no TMA
+                             * tensor path). */
 } flowkv_pool;
 
 /* One request: its length and both sides' block-id lists.
@@ -196,13 +199,13 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
  *   tuning   : HOST pointer or NULL.
  *   out      : HOST pointer; receives the plan (caller destroys it).  Untouched on error.
  * The plan stays valid until destroyed; pools must stay alive while it is run.  The first plan (or table-driven call)
- * that names a new layer_offsets[] array copies it to the device once (8*L bytes on the library's own stream, waited
+ * that names a new plane_offsets[] array copies it to the device once (16*L bytes on the library's own stream, waited
  * for; cached by content for the life of the process) — the one exception to "does not synchronise".  Inside a
  * stream capture the table must already be cached: make one call (or build any plan) with the same offsets first.
  * Errors (nothing is allocated or enqueued when one is returned):
  *   INVALID_ARG  out NULL, both pools NULL, reqs NULL with n_reqs > 0, a table pointer NULL, unknown flag /
  *                layout / tuning value, a zero shape field or a stride <= 0
- *   ALIGN        a base, a stride, a layer offset or head_dim*elem_bytes is not a multiple of 16 bytes
+ *   ALIGN        a base, a stride, a plane offset or head_dim*elem_bytes is not a multiple of 16 bytes
  *   SHAPE_MISMATCH  src and dst differ in L, Hkv, Dh or elem_bytes
  *   TABLE_LEN    n_*_blocks != ceil(num_tokens / block_size);  BLOCK_OOB  an id outside [0, num_blocks)
  *   DST_ALIAS    (only with FLOWKV_CHECK_DST_ALIAS) a dst block id named twice in the batch

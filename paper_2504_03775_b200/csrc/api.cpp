@@ -164,10 +164,10 @@ cudaError_t upload_stream(int device, cudaStream_t* out, cudaMemPool_t* pool) {
   return cudaSuccess;
 }
 
-// Per-layer offset tables (flowkv_pool.layer_offsets, reading A22) as the kernels read them: DEVICE arrays, uploaded
+// Per-plane offset tables (flowkv_pool.plane_offsets, reading A22) as the kernels read them: DEVICE arrays, uploaded
 // once per distinct content and device and kept for the life of the process (a server has a handful of pools).  The
 // upload rides the library's own stream and is waited for here — the first plan that names a new table pays for it.
-class LayerOffsetCache {
+class PlaneOffsetCache {
  public:
   cudaError_t get(int device, const int64_t* host, uint32_t n, const int64_t** out) {
     uint64_t h = 1469598103934665603ull ^ (uint64_t)device;           // FNV-1a over the offsets
@@ -203,7 +203,7 @@ class LayerOffsetCache {
   std::mutex mu_;
   std::unordered_multimap<uint64_t, Entry> entries_;
 };
-LayerOffsetCache g_layer_offsets;
+PlaneOffsetCache g_plane_offsets;
 
 // Helper streams and events of flowkv_transfer_via_host.  Created once and recycled between plans (a plan per
 // batch would otherwise pay three cudaStreamCreate and ~100 cudaEventCreate per step).
@@ -269,9 +269,9 @@ struct Op {                  // one runnable operation of a plan
 
 struct flowkv_plan_s {
   bool has_src = false, has_dst = false, on_device = false;
-  flowkv_pool src{}, dst{};            // layer_offsets (if any) point into the copies below
-  std::vector<int64_t> src_layer_off, dst_layer_off;
-  const int64_t *d_src_layer_off = nullptr, *d_dst_layer_off = nullptr;   // their device copies (library cache)
+  flowkv_pool src{}, dst{};            // plane_offsets (if any) point into the copies below
+  std::vector<int64_t> src_plane_off, dst_plane_off;
+  const int64_t *d_src_plane_off = nullptr, *d_dst_plane_off = nullptr;   // their device copies (library cache)
   Geometry g{};
   flowkv_tuning tuning{};
   uint32_t tile_bytes = 0;
@@ -339,9 +339,9 @@ uint32_t pick_vec(const flowkv_pool* a, const flowkv_pool* b, const Geometry& g)
     if (!p) return true;
     if ((uintptr_t)p->base % 32) return false;
     for (int i = 0; i < 5; ++i)
-      if (!(i == FLOWKV_S_LAYER && p->layer_offsets) && p->stride_bytes[i] % 32) return false;
-    if (p->layer_offsets)
-      for (uint32_t l = 0; l < p->num_layers; ++l) if (p->layer_offsets[l] % 32) return false;
+      if (!((i == FLOWKV_S_LAYER || i == FLOWKV_S_KV) && p->plane_offsets) && p->stride_bytes[i] % 32) return false;
+    if (p->plane_offsets)
+      for (uint32_t q = 0; q < 2 * p->num_layers; ++q) if (p->plane_offsets[q] % 32) return false;
     return true;
   };
   return (g.row_bytes % 32 == 0 && ok32(a) && ok32(b)) ? 32 : 16;
@@ -468,13 +468,13 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
     pl->has_dst = dst != nullptr;
     if (src) pl->src = *src;
     if (dst) pl->dst = *dst;
-    if (src && src->layer_offsets) {       // the caller's array is borrowed for this call only
-      pl->src_layer_off.assign(src->layer_offsets, src->layer_offsets + src->num_layers);
-      pl->src.layer_offsets = pl->src_layer_off.data();
+    if (src && src->plane_offsets) {       // the caller's array is borrowed for this call only
+      pl->src_plane_off.assign(src->plane_offsets, src->plane_offsets + 2 * (size_t)src->num_layers);
+      pl->src.plane_offsets = pl->src_plane_off.data();
     }
-    if (dst && dst->layer_offsets) {
-      pl->dst_layer_off.assign(dst->layer_offsets, dst->layer_offsets + dst->num_layers);
-      pl->dst.layer_offsets = pl->dst_layer_off.data();
+    if (dst && dst->plane_offsets) {
+      pl->dst_plane_off.assign(dst->plane_offsets, dst->plane_offsets + 2 * (size_t)dst->num_layers);
+      pl->dst.plane_offsets = pl->dst_plane_off.data();
     }
     pl->tuning = tn;
     Geometry& g = pl->g;
@@ -504,11 +504,11 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       }
       pl->num_sms = sms_of[di].load(std::memory_order_relaxed);
       pl->max_smem_optin = smem_of[di].load(std::memory_order_relaxed);
-      if (!pl->src_layer_off.empty())
-        e = g_layer_offsets.get(pl->device, pl->src_layer_off.data(), g.L, &pl->d_src_layer_off);
-      if (e == cudaSuccess && !pl->dst_layer_off.empty())
-        e = g_layer_offsets.get(pl->device, pl->dst_layer_off.data(), g.L, &pl->d_dst_layer_off);
-      if (e != cudaSuccess) { drop_plan(pl); return fail_cuda(e, "upload of layer_offsets"); }
+      if (!pl->src_plane_off.empty())
+        e = g_plane_offsets.get(pl->device, pl->src_plane_off.data(), 2 * g.L, &pl->d_src_plane_off);
+      if (e == cudaSuccess && !pl->dst_plane_off.empty())
+        e = g_plane_offsets.get(pl->device, pl->dst_plane_off.data(), 2 * g.L, &pl->d_dst_plane_off);
+      if (e != cudaSuccess) { drop_plan(pl); return fail_cuda(e, "upload of plane_offsets"); }
     } else {
       pl->num_sms = 148;
     }
@@ -605,9 +605,9 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
   return FLOWKV_OK;
 }
 
-Side pool_side(const flowkv_pool& p, const int64_t* device_layer_off) {
+Side pool_side(const flowkv_pool& p, const int64_t* device_plane_off) {
   Side s{};
-  s.layer_off = device_layer_off;
+  s.plane_off = device_plane_off;
   s.base = (char*)p.base;
   s.s_layer = p.stride_bytes[FLOWKV_S_LAYER];
   s.s_kv = p.stride_bytes[FLOWKV_S_KV];
@@ -768,7 +768,7 @@ flowkv_status flowkv_pool_strides(flowkv_pool* p) {
     return fail(FLOWKV_ERR_INVALID_ARG, "unknown layout");
   }
   for (int i = 0; i < 5; ++i)
-    if (!(i == FLOWKV_S_LAYER && p->layer_offsets) && p->stride_bytes[i] <= 0) return fail(FLOWKV_ERR_INVALID_ARG, "a stride is <= 0");
+    if (!((i == FLOWKV_S_LAYER || i == FLOWKV_S_KV) && p->plane_offsets) && p->stride_bytes[i] <= 0) return fail(FLOWKV_ERR_INVALID_ARG, "a stride is <= 0");
   return FLOWKV_OK;
 }
 
@@ -826,7 +826,7 @@ flowkv_status flowkv_transfer_layers(const flowkv_plan_t* pl, uint32_t layer_beg
     return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pool-to-pool schedule (needs both pools, no FLOWKV_PLAN_NO_TRANSFER)");
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->transfer, pool_side(pl->src, pl->d_src_layer_off), pool_side(pl->dst, pl->d_dst_layer_off), pl->transfer.shape.vec_bytes, stream, ro);
+  return run(pl, pl->transfer, pool_side(pl->src, pl->d_src_plane_off), pool_side(pl->dst, pl->d_dst_plane_off), pl->transfer.shape.vec_bytes, stream, ro);
 }
 
 flowkv_status flowkv_transfer(const flowkv_plan_t* pl, void* stream) {
@@ -842,7 +842,7 @@ flowkv_status flowkv_pack_layers(const flowkv_plan_t* pl, void* staging, uint64_
   const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->pack, pool_side(pl->src, pl->d_src_layer_off), dense_side(staging, pl->g), vec, stream, ro);
+  return run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_side(staging, pl->g), vec, stream, ro);
 }
 
 flowkv_status flowkv_pack(const flowkv_plan_t* pl, void* staging, uint64_t bytes, void* stream) {
@@ -858,7 +858,7 @@ flowkv_status flowkv_unpack_layers(const flowkv_plan_t* pl, const void* staging,
   const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst, pl->d_dst_layer_off), vec, stream, ro);
+  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst, pl->d_dst_plane_off), vec, stream, ro);
 }
 
 flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, void* stream) {
@@ -882,7 +882,7 @@ flowkv_status flowkv_pack_window(const flowkv_plan_t* pl, void* window, uint64_t
   const uint32_t vec = ((uintptr_t)window % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->pack, pool_side(pl->src, pl->d_src_layer_off), dense_side(window, pl->g, layer_begin, layer_end), vec, stream, ro);
+  return run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_side(window, pl->g, layer_begin, layer_end), vec, stream, ro);
 }
 
 flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, uint64_t bytes, uint32_t layer_begin,
@@ -894,7 +894,7 @@ flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, 
   const uint32_t vec = ((uintptr_t)window % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->unpack, dense_side(window, pl->g, layer_begin, layer_end), pool_side(pl->dst, pl->d_dst_layer_off), vec, stream, ro);
+  return run(pl, pl->unpack, dense_side(window, pl->g, layer_begin, layer_end), pool_side(pl->dst, pl->d_dst_plane_off), vec, stream, ro);
 }
 
 namespace {
@@ -990,11 +990,11 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
       ro.layer_begin = (uint32_t)((uint64_t)L * c / n_chunks);
       ro.layer_end = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
       if (ro.layer_begin == ro.layer_end) continue;
-      st = run(pl, pl->pack, pool_side(pl->src, pl->d_src_layer_off), dense_side(host_staging, pl->g), vec, s, ro);          // D2H on `stream`
+      st = run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_side(host_staging, pl->g), vec, s, ro);          // D2H on `stream`
       if (st != FLOWKV_OK) return st;
       FK_TRY(cudaEventRecord(vc.ev[c], s), "cudaEventRecord");
       FK_TRY(cudaStreamWaitEvent(aux, vc.ev[c], 0), "cudaStreamWaitEvent");
-      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst, pl->d_dst_layer_off), vecu, aux, ro);     // H2D on the helper
+      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst, pl->d_dst_plane_off), vecu, aux, ro);     // H2D on the helper
       if (st != FLOWKV_OK) return st;
     }
     FK_TRY(cudaEventRecord(e_done, aux), "cudaEventRecord");
@@ -1031,7 +1031,7 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     char* in_slot = scratch + (2 + (k & 1)) * slot;
     char* host = (char*)host_staging + planes_bytes(pl, 0, p0);
     if (prev2 >= 0) FK_TRY(cudaStreamWaitEvent(s, landed[prev2], 0), "cudaStreamWaitEvent");          // out slot free again
-    st = run(pl, pl->pack, pool_side(pl->src, pl->d_src_layer_off), dense_planes(out_slot, pl->g, p0, p1), pl->pack.shape.vec_bytes, s, ro);
+    st = run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_planes(out_slot, pl->g, p0, p1), pl->pack.shape.vec_bytes, s, ro);
     if (st != FLOWKV_OK) return st;
     FK_TRY(cudaEventRecord(packed[c], s), "cudaEventRecord");
     FK_TRY(cudaStreamWaitEvent(vc.q_d2h, packed[c], 0), "cudaStreamWaitEvent");
@@ -1042,7 +1042,7 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     FK_TRY(cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, vc.q_h2d), "cudaMemcpyAsync(H2D)");
     FK_TRY(cudaEventRecord(arrived[c], vc.q_h2d), "cudaEventRecord");
     FK_TRY(cudaStreamWaitEvent(vc.q_unpack, arrived[c], 0), "cudaStreamWaitEvent");
-    st = run(pl, pl->unpack, dense_planes(in_slot, pl->g, p0, p1), pool_side(pl->dst, pl->d_dst_layer_off), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
+    st = run(pl, pl->unpack, dense_planes(in_slot, pl->g, p0, p1), pool_side(pl->dst, pl->d_dst_plane_off), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
     if (st != FLOWKV_OK) return st;
     FK_TRY(cudaEventRecord(unpacked[c], vc.q_unpack), "cudaEventRecord");
     prev2 = prev1;
@@ -1094,10 +1094,10 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (e != cudaSuccess) return fail_cuda(e, "cudaGetDevice");
-  const int64_t *d_slo = nullptr, *d_dlo = nullptr;      // device copies of the per-layer offsets (A22), cached
-  if (src && src->layer_offsets) e = g_layer_offsets.get(dev, src->layer_offsets, src->num_layers, &d_slo);
-  if (e == cudaSuccess && dst && dst->layer_offsets) e = g_layer_offsets.get(dev, dst->layer_offsets, dst->num_layers, &d_dlo);
-  if (e != cudaSuccess) return fail_cuda(e, "upload of layer_offsets");
+  const int64_t *d_slo = nullptr, *d_dlo = nullptr;      // device copies of the per-plane offsets (A22), cached
+  if (src && src->plane_offsets) e = g_plane_offsets.get(dev, src->plane_offsets, 2 * src->num_layers, &d_slo);
+  if (e == cudaSuccess && dst && dst->plane_offsets) e = g_plane_offsets.get(dev, dst->plane_offsets, 2 * dst->num_layers, &d_dlo);
+  if (e != cudaSuccess) return fail_cuda(e, "upload of plane_offsets");
   TablesParams tp{};
   tp.kp.src = src ? pool_side(*src, d_slo) : dense_side(dense, g, l0, l1);
   tp.kp.dst = dst ? pool_side(*dst, d_dlo) : dense_side(dense, g, l0, l1);
@@ -1225,9 +1225,9 @@ flowkv_status memcpy_tokens(const flowkv_pool& S, const flowkv_pool& D, const Ge
   for (uint32_t l = 0; l < g.L; ++l)
     for (uint32_t c = 0; c < 2; ++c)
       for (uint32_t h = 0; h < (tm ? 1u : g.Hkv); ++h) {
-        const char* s = (const char*)S.base + pool_layer_off(S, l) + c * S.stride_bytes[1] + (int64_t)sb * S.stride_bytes[2] +
+        const char* s = (const char*)S.base + pool_plane_off(S, l, c) + (int64_t)sb * S.stride_bytes[2] +
                         (int64_t)so * S.stride_bytes[3] + (int64_t)h * S.stride_bytes[4];
-        char* d = (char*)D.base + pool_layer_off(D, l) + c * D.stride_bytes[1] + (int64_t)db * D.stride_bytes[2] +
+        char* d = (char*)D.base + pool_plane_off(D, l, c) + (int64_t)db * D.stride_bytes[2] +
                   (int64_t)dof * D.stride_bytes[3] + (int64_t)h * D.stride_bytes[4];
         cudaError_t e = FK_ENQ cudaMemcpyAsync(d, s, (size_t)n * (tm ? g.tok_bytes : g.row_bytes), cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) return fail_cuda(e, "cudaMemcpyAsync");

@@ -57,8 +57,8 @@ struct Side {            // one end of a copy as the kernel sees it
                          // s_layer = bytes per token of the layer window the buffer holds, s_kv unused
   uint32_t dense;        // 1: dense staging buffer, 0: paged pool
   uint32_t plane0;       // dense side: first plane of the layer window the buffer holds (0 = whole wire format)
-  const int64_t* layer_off;   // pool side, DEVICE array [L] or NULL: layer l starts layer_off[l] bytes from base and
-                              // s_layer is unused (layers are separate allocations, reading A22)
+  const int64_t* plane_off;   // pool side, DEVICE array [2L] or NULL: plane p starts plane_off[p] bytes from base and
+                              // s_layer / s_kv are unused (planes are separate allocations, readings A22 / A3)
 };
 
 // Plans whose every schedule has at most kInlineChunks entries pass them in the kernel parameters instead of
@@ -168,9 +168,10 @@ bool pool_is_span_capable(const flowkv_pool& p, const Geometry& g);
 // with the same block size and the same interior strides?  Then whole-block runs are flat byte ranges.
 bool pools_are_flat_congruent(const flowkv_pool& a, const flowkv_pool& b, const Geometry& g);
 
-// Byte offset of layer l from the pool's base (uniform stride, or the caller's per-layer offsets: reading A22).
-inline int64_t pool_layer_off(const flowkv_pool& p, uint32_t l) {
-  return p.layer_offsets ? p.layer_offsets[l] : (int64_t)l * p.stride_bytes[FLOWKV_S_LAYER];
+// Byte offset of plane (l, c) from the pool's base (uniform strides, or the caller's per-plane offsets: reading A22).
+inline int64_t pool_plane_off(const flowkv_pool& p, uint32_t l, uint32_t c) {
+  return p.plane_offsets ? p.plane_offsets[2 * l + c]
+                         : (int64_t)l * p.stride_bytes[FLOWKV_S_LAYER] + (int64_t)c * p.stride_bytes[FLOWKV_S_KV];
 }
 
 flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string& err);

@@ -130,7 +130,7 @@ template <uint32_t N> struct ParamChunks {
 
 // Byte offset of a chunk inside one plane of one side.
 //   pool side  : layer*s_layer + kv*s_kv + off                                    (off in bytes);
-//                layer_off[layer] in place of layer*s_layer when the layers are separate allocations (A22)
+//                plane_off[plane] in place of layer*s_layer + kv*s_kv when the planes are separate allocations (A22)
 //   dense side : off = (staging_tok_off << 32) | token_in_request.  The buffer holds the layer window
 //                [plane0/2, ...) in wire order [request][layer][K|V][token][head][dim] (A12), so the
 //                chunk sits at  staging_tok_off * window_bytes_per_token            (request base)
@@ -142,8 +142,8 @@ __device__ __forceinline__ int64_t side_offset(const Side& s, int64_t off, uint3
     const uint32_t tok0 = (uint32_t)((uint64_t)off >> 32), t = (uint32_t)off;
     return (int64_t)tok0 * s.s_layer + ((int64_t)(plane - s.plane0) * req_tokens + t) * (int64_t)tok_bytes;
   }
-  const int64_t layer = s.layer_off ? __ldg(s.layer_off + (plane >> 1)) : (int64_t)(plane >> 1) * s.s_layer;   // A22
-  return layer + (int64_t)(plane & 1) * s.s_kv + off;
+  if (s.plane_off) return __ldg(s.plane_off + plane) + off;          // planes are separate allocations (A22)
+  return (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv + off;
 }
 
 __device__ __forceinline__ void decode_tile(const KernelParams& p, uint32_t tile, uint32_t& plane, uint32_t& ci) {
@@ -678,8 +678,8 @@ __device__ __forceinline__ int64_t tables_side(const Side& sd, const int32_t* ta
     return (int64_t)tok0 * sd.s_layer + ((int64_t)(plane - sd.plane0) * T + t0) * (int64_t)tok_bytes;
   const int32_t b = __ldg(tab + (size_t)r * max_blocks + (t0 >> bs_log2));
   if ((uint32_t)b >= num_blocks) ok = false;
-  const int64_t layer = sd.layer_off ? __ldg(sd.layer_off + (plane >> 1)) : (int64_t)(plane >> 1) * sd.s_layer;
-  return layer + (int64_t)(plane & 1) * sd.s_kv + (int64_t)b * s_block +
+  const int64_t pl = sd.plane_off ? __ldg(sd.plane_off + plane) : (int64_t)(plane >> 1) * sd.s_layer + (int64_t)(plane & 1) * sd.s_kv;
+  return pl + (int64_t)b * s_block +
          (int64_t)(t0 & ((1u << bs_log2) - 1)) * sd.s_token;
 }
 

@@ -43,13 +43,13 @@ flowkv_status validate_pool(const flowkv_pool* p, const char* which, std::string
       (1ull << 32))
     return fail(FLOWKV_ERR_UNSUPPORTED, "one block spans 4 GiB or more");
   for (int i = 0; i < 5; ++i) {
-    if (i == FLOWKV_S_LAYER && p->layer_offsets) continue;      // replaced by the per-layer offsets (A22)
+    if ((i == FLOWKV_S_LAYER || i == FLOWKV_S_KV) && p->plane_offsets) continue;   // replaced by the per-plane offsets (A22)
     if (p->stride_bytes[i] <= 0) return fail(FLOWKV_ERR_INVALID_ARG, "a stride is <= 0 (call flowkv_pool_strides)");
     if (p->stride_bytes[i] % 16) return fail(FLOWKV_ERR_ALIGN, "a stride is not a multiple of 16 bytes");
   }
-  if (p->layer_offsets)
-    for (uint32_t l = 0; l < p->num_layers; ++l)
-      if (p->layer_offsets[l] % 16) return fail(FLOWKV_ERR_ALIGN, "a layer offset is not a multiple of 16 bytes");
+  if (p->plane_offsets)
+    for (uint32_t pl = 0; pl < 2 * p->num_layers; ++pl)
+      if (p->plane_offsets[pl] % 16) return fail(FLOWKV_ERR_ALIGN, "a plane offset is not a multiple of 16 bytes");
   return FLOWKV_OK;
 }
 
@@ -230,7 +230,7 @@ static void rows_chunks(const flowkv_pool* src, const flowkv_pool* dst, const Ge
 
 bool pools_are_flat_congruent(const flowkv_pool& a, const flowkv_pool& b, const Geometry& g) {
   if (a.block_size != b.block_size) return false;
-  if (a.layer_offsets || b.layer_offsets) return false;      // separate layer allocations: a block is not one range
+  if (a.plane_offsets || b.plane_offsets) return false;      // separate plane allocations: a block is not one range
   for (int i : {FLOWKV_S_LAYER, FLOWKV_S_KV, FLOWKV_S_BLOCK, FLOWKV_S_TOKEN, FLOWKV_S_HEAD})
     if (a.stride_bytes[i] != b.stride_bytes[i]) return false;
   // the interior of a block must be a dense bijection onto [0, s_block): sorted by stride, every axis

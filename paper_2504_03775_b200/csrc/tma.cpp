@@ -72,7 +72,7 @@ bool build_rows_tma(const flowkv_pool& src, const flowkv_pool& dst, const Geomet
   out.ok = false;
   // what the tensor path needs (everything else runs the register path)
   for (const flowkv_pool* p : {&src, &dst}) {
-    if (p->layer_offsets) { why = "layers are separate allocations (no uniform plane stride)"; return false; }
+    if (p->plane_offsets) { why = "planes are separate allocations (no uniform plane stride)"; return false; }
     if (p->stride_bytes[FLOWKV_S_LAYER] != 2 * p->stride_bytes[FLOWKV_S_KV]) { why = "s_layer != 2*s_kv (plane axis is not uniform)"; return false; }
     for (int i = 0; i < 5; ++i)
       if ((uint64_t)p->stride_bytes[i] >= (1ull << 40)) { why = "a stride of 2^40 bytes or more"; return false; }

@@ -44,7 +44,7 @@ class flowkv_pool(C.Structure):
     _fields_ = [("base", C.c_void_p), ("num_layers", C.c_uint32), ("num_kv_heads", C.c_uint32),
                 ("head_dim", C.c_uint32), ("elem_bytes", C.c_uint32), ("num_blocks", C.c_uint32),
                 ("block_size", C.c_uint32), ("layout", C.c_uint32), ("_reserved", C.c_uint32),
-                ("stride_bytes", C.c_int64 * 5), ("layer_offsets", C.c_void_p)]
+                ("stride_bytes", C.c_int64 * 5), ("plane_offsets", C.c_void_p)]
 
 
 class flowkv_request(C.Structure):
@@ -172,16 +172,13 @@ def flowkv_api_call_count() -> int:
 # ---- marshalling helpers ----------------------------------------------------------------------
 def make_pool(base: int, num_layers: int, num_kv_heads: int, head_dim: int, elem_bytes: int, num_blocks: int,
               block_size: int, layout="lkbthd", strides: Optional[Sequence[int]] = None,
-              layer_offsets: Optional[Sequence[int]] = None) -> flowkv_pool:
+              layer_offsets: Optional[Sequence[int]] = None, plane_offsets: Optional[Sequence[int]] = None) -> flowkv_pool:
     """Describe a pool.  ``strides`` (layer, kv, block, token, head; bytes) only for layout 'strided'.
-    ``layer_offsets``: byte offset of every layer from ``base`` when the layers are separate allocations (reading
-    A22); the int64 array is kept alive by the returned object."""
+    ``plane_offsets``: byte offset of every plane 2*layer + (0 K | 1 V) from ``base`` when the planes are separate
+    allocations (reading A22); ``layer_offsets``: the special case of one tensor per layer with K and V stacked s_kv
+    apart inside it.  The int64 array is kept alive by the returned object."""
+    assert layer_offsets is None or plane_offsets is None
     p = flowkv_pool()
-    if layer_offsets is not None:
-        lo = np.ascontiguousarray(np.asarray(layer_offsets, dtype=np.int64))
-        assert lo.shape == (num_layers,), "one offset per layer"
-        p._layer_offsets_keep = lo
-        p.layer_offsets = lo.ctypes.data
     p.base = base
     p.num_layers, p.num_kv_heads, p.head_dim, p.elem_bytes = num_layers, num_kv_heads, head_dim, elem_bytes
     p.num_blocks, p.block_size = num_blocks, block_size
@@ -189,6 +186,19 @@ def make_pool(base: int, num_layers: int, num_kv_heads: int, head_dim: int, elem
     if strides is not None:
         for i, s in enumerate(strides):
             p.stride_bytes[i] = int(s)
+    if plane_offsets is not None:           # set before the stride check: layer / K|V strides are then ignored
+        po = np.ascontiguousarray(np.asarray(plane_offsets, dtype=np.int64))
+        assert po.shape == (2 * num_layers,), "one offset per plane"
+        p._plane_offsets_keep = po
+        p.plane_offsets = po.ctypes.data
+    if layer_offsets is not None:
+        assert len(layer_offsets) == num_layers, "one offset per layer"
+        po = np.zeros(2 * num_layers, dtype=np.int64)
+        p._plane_offsets_keep = po
+        p.plane_offsets = po.ctypes.data
+        flowkv_pool_strides(p)              # fills s_kv for the named layouts (the layer stride is already ignored)
+        assert p.stride_bytes[1] > 0, "layer_offsets needs the K|V stride inside a layer"
+        po[:] = [int(o) + c * p.stride_bytes[1] for o in layer_offsets for c in (0, 1)]
     flowkv_pool_strides(p)
     return p
 
@@ -201,9 +211,9 @@ def flowkv_pool_strides(pool: flowkv_pool) -> flowkv_pool:
 def pool_bytes(pool: flowkv_pool) -> int:
     """Bytes from the base to one past the last addressable element."""
     s = pool.stride_bytes
-    if pool.layer_offsets:
-        lo = getattr(pool, "_layer_offsets_keep")
-        return int(lo.max()) + (s[1] + (pool.num_blocks - 1) * s[2] + (pool.block_size - 1) * s[3]
+    if pool.plane_offsets:
+        po = getattr(pool, "_plane_offsets_keep")
+        return int(po.max()) + ((pool.num_blocks - 1) * s[2] + (pool.block_size - 1) * s[3]
                                 + (pool.num_kv_heads - 1) * s[4] + pool.head_dim * pool.elem_bytes)
     return ((pool.num_layers - 1) * s[0] + s[1] + (pool.num_blocks - 1) * s[2] + (pool.block_size - 1) * s[3]
             + (pool.num_kv_heads - 1) * s[4] + pool.head_dim * pool.elem_bytes)

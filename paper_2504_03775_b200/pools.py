@@ -62,7 +62,7 @@ class DevicePools:
     def __init__(self, w: synth.Workload, device="cuda:0", fill: Optional[str] = None, sentinel_dst: bool = True,
                  separate_src_layers: bool = False):
         """``separate_src_layers``: the src pool (LKBTHD) is allocated as one tensor PER LAYER — the cache the paper
-        starts from — and described through ``flowkv_pool.layer_offsets``; ``src_layers`` holds the tensors and
+        starts from — and described through ``flowkv_pool.plane_offsets``; ``src_layers`` holds the tensors and
         ``src_buf`` is layer 0's."""
         self.w = w
         self.device = torch.device(device)

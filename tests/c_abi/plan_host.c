@@ -15,7 +15,7 @@ int main(void) {
   flowkv_status rc;
 
   src.base = (void*)0x1000; src.num_layers = 2; src.num_kv_heads = 2; src.head_dim = 64; src.elem_bytes = 2;
-  src.num_blocks = 32; src.block_size = 16; src.layout = FLOWKV_LAYOUT_LKBTHD; src._reserved = 0; src.layer_offsets = NULL;
+  src.num_blocks = 32; src.block_size = 16; src.layout = FLOWKV_LAYOUT_LKBTHD; src._reserved = 0; src.plane_offsets = NULL;
   dst = src;
   if (flowkv_pool_strides(&src) != FLOWKV_OK || flowkv_pool_strides(&dst) != FLOWKV_OK) return 2;
   req.num_tokens = 120; req.n_src_blocks = 8; req.src_blocks = s; req.dst_blocks = d; req.n_dst_blocks = 8; req._reserved = 0;

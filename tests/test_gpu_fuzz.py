@@ -22,9 +22,10 @@ FUZZ_CASES = int(os.environ.get("FLOWKV_FUZZ_CASES", "400"))
 
 
 def _geom(rng, layout, L, H, D, NB, BS, e=2, separate=False):
-    """-> (oracle geometry, strides or None, layer offsets or None).  'padded' = token-major interior with padding
+    """-> (oracle geometry, strides or None, plane offsets or None).  'padded' = token-major interior with padding
     after every block, K|V slab and layer (a STRIDED pool: separate allocations / alignment padding); with
-    ``separate`` its layers sit at shuffled, gapped offsets of their own (reading A22: a tensor per layer)."""
+    ``separate`` its layers — or every K and every V — sit at shuffled, gapped offsets of their own (reading A22: a
+    tensor per layer, or per plane)."""
     if layout != "padded":
         return getattr(O.PoolGeom, layout)(L, H, D, e, NB, BS), None, None
     row, tok = D * e, H * D * e
@@ -35,11 +36,15 @@ def _geom(rng, layout, L, H, D, NB, BS, e=2, separate=False):
     if not separate:
         return g, [lay, kv, blk, tok, row], None
     unit = 16 if rng.random() < 0.25 else 32               # a quarter of them only 16-byte aligned (128-bit path)
-    off, pos = [0] * L, unit * int(rng.integers(0, 3))
-    for l in rng.permutation(L):
-        off[int(l)] = pos
-        pos += g.layer_bytes() + unit * int(rng.integers(1, 6))
-    return g.with_layer_offsets(off), [lay, kv, blk, tok, row], off
+    planes = rng.random() < 0.5                            # K and V separate tensors too (A3), else stacked per layer
+    n = 2 * L if planes else L
+    size = g.plane_bytes() if planes else g.layer_bytes()
+    off, pos = [0] * n, unit * int(rng.integers(0, 3))
+    for i in rng.permutation(n):
+        off[int(i)] = pos
+        pos += size + unit * int(rng.integers(1, 6))
+    g = g.with_plane_offsets(off) if planes else g.with_layer_offsets(off)
+    return g, [lay, kv, blk, tok, row], list(g.plane_off)
 
 
 def _pools(rng, idx, L, H, D, e, lay_s, bs_s, NBs, lay_d, bs_d, NBd):
@@ -49,8 +54,8 @@ def _pools(rng, idx, L, H, D, e, lay_s, bs_s, NBs, lay_d, bs_d, NBd):
     src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
     P.fill_values(src_buf, "bits", "fp16", 9000 + idx)
     P.fill_sentinel(dst_buf)
-    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss, los)
-    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd, lod)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, NBs, bs_s, "strided" if ss else lay_s, ss, plane_offsets=los)
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "strided" if sd else lay_d, sd, plane_offsets=lod)
     return gs, gd, ss, sd, src_buf, dst_buf, src, dst
 
 

@@ -1168,39 +1168,43 @@ def test_distinct_plans_from_distinct_threads_on_distinct_streams():
         G.assert_same(P.to_numpy(dps[k].src_buf), srcs[k], "src pool must not change")
 
 
-def _separate_layers(rng, L, H, D, e, NB, BS, unit=32):
-    """A cache whose layers are separate allocations (reading A22): every layer a (2,NB,BS,H,D) tensor at a shuffled,
-    gapped offset of one device buffer -> (oracle geometry, offsets, total bytes)."""
+def _separate_layers(rng, L, H, D, e, NB, BS, unit=32, planes=False):
+    """A cache whose layers are separate allocations (reading A22): every layer a (2,NB,BS,H,D) tensor — or, with
+    ``planes``, every K and every V a (NB,BS,H,D) tensor of its own (A3) — at a shuffled, gapped offset of one device
+    buffer -> (oracle geometry, plane offsets, total bytes)."""
     one = O.PoolGeom.lkbthd(1, H, D, e, NB, BS)
-    off, pos = [0] * L, unit * int(rng.integers(0, 4))
-    for l in rng.permutation(L):
-        off[int(l)] = pos
-        pos += one.layer_bytes() + unit * int(rng.integers(1, 9))
-    g = O.PoolGeom(L, H, D, e, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head).with_layer_offsets(off)
-    return g, off, pos
+    n = 2 * L if planes else L
+    size = one.plane_bytes() if planes else one.layer_bytes()
+    off, pos = [0] * n, unit * int(rng.integers(0, 4))
+    for i in rng.permutation(n):
+        off[int(i)] = pos
+        pos += size + unit * int(rng.integers(1, 9))
+    g = O.PoolGeom(L, H, D, e, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head)
+    g = g.with_plane_offsets(off) if planes else g.with_layer_offsets(off)
+    return g, list(g.plane_off), pos
 
 
-@pytest.mark.parametrize("dst_kind", ["lkbthd", "separate", "blkthd", "blkhtd32"])
+@pytest.mark.parametrize("dst_kind", ["lkbthd", "separate", "separate_kv", "blkthd", "blkhtd32"])
 @pytest.mark.parametrize("tuning", [None, {"variant": "bulk"}, {"plan_in_params": 1, "tile_bytes": 4096}])
 def test_pools_whose_layers_are_separate_allocations(dst_kind, tuning):
     """before Eq. 5 the cache is 'separate tensor structures across all layer dimensions'.  src = L tensors at
-    scattered addresses (flowkv_pool.layer_offsets, base in the MIDDLE so some offsets are negative); dst = a stacked
-    pool, another set of separate tensors, or ONE (B,L,2,H) tensor — the paper's own migration — incl. a block-size
+    scattered addresses (flowkv_pool.plane_offsets, base in the MIDDLE so some offsets are negative); dst = a stacked
+    pool, another set of separate tensors (per layer, or per layer AND K|V: 2L tensors on both sides), or ONE (B,L,2,H) tensor — the paper's own migration — incl. a block-size
     change.  Transfer, layer range, pack / unpack, windows, the table-driven kernel and the memcpy baseline against
     the oracle over whole buffers (the gaps between the tensors stay untouched)."""
     rng = np.random.default_rng(4100 + len(dst_kind))
     L, H, D, e, NBs, BS = 5, 4, 64, 2, 40, 16
-    gs, soff, sbytes = _separate_layers(rng, L, H, D, e, NBs, BS)
+    gs, soff, sbytes = _separate_layers(rng, L, H, D, e, NBs, BS, planes=dst_kind == "separate_kv")
     src_buf = P.alloc_bytes(sbytes)
     P.fill_values(src_buf, "bits", "fp16", 4100)
     src_np = P.to_numpy(src_buf)
-    mid = soff[2]
-    src = F.make_pool(src_buf.data_ptr() + mid, L, H, D, e, NBs, BS, "lkbthd", layer_offsets=[o - mid for o in soff])
-    if dst_kind == "separate":
+    mid = soff[4]
+    src = F.make_pool(src_buf.data_ptr() + mid, L, H, D, e, NBs, BS, "lkbthd", plane_offsets=[o - mid for o in soff])
+    if dst_kind in ("separate", "separate_kv"):
         NBd, bs_d = 24, BS
-        gd, doff, dbytes = _separate_layers(rng, L, H, D, e, NBd, bs_d, unit=16)      # 16-byte aligned only: 128-bit path
+        gd, doff, dbytes = _separate_layers(rng, L, H, D, e, NBd, bs_d, unit=16, planes=dst_kind == "separate_kv")   # 16-byte aligned only: 128-bit path
         dst_buf = P.alloc_bytes(dbytes)
-        dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "lkbthd", layer_offsets=doff)
+        dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, NBd, bs_d, "lkbthd", plane_offsets=doff)
     else:
         lay, bs_d = {"lkbthd": ("lkbthd", BS), "blkthd": ("blkthd", BS), "blkhtd32": ("blkhtd", 32)}[dst_kind]
         NBd = 24 * BS // bs_d
@@ -1227,8 +1231,8 @@ def test_pools_whose_layers_are_separate_allocations(dst_kind, tuning):
     what = f"separate layers -> {dst_kind} {tuning}"
     plan = F.flowkv_plan(src, dst, freqs, F.FLOWKV_CHECK_DST_ALIAS, tuning, s)
     st = plan.stats
-    assert st["mode_transfer"] == (1 if dst_kind in ("lkbthd", "separate") else 2)
-    assert st["vec_bytes"] == (16 if dst_kind == "separate" else 32)
+    assert st["mode_transfer"] == (1 if dst_kind in ("lkbthd", "separate", "separate_kv") else 2)
+    assert st["vec_bytes"] == (16 if dst_kind in ("separate", "separate_kv") else 32)
     if tuning and tuning.get("variant") == "bulk":      # span: the bulk ring; rows: no tensor map for such a pool
         assert st["variant"] == (F.FLOWKV_VARIANT_BULK if st["mode_transfer"] == 1 else F.FLOWKV_VARIANT_LDST)
     P.fill_sentinel(dst_buf)
@@ -1267,7 +1271,7 @@ def test_pools_whose_layers_are_separate_allocations(dst_kind, tuning):
         off += t
     G.assert_same(P.to_numpy(win), wexp, what + ": window [2,5)")
     # memcpy baseline (token-major on both sides only) walks the same per-layer addresses
-    if dst_kind in ("lkbthd", "separate"):
+    if dst_kind in ("lkbthd", "separate", "separate_kv"):
         P.fill_sentinel(dst_buf)
         calls = F.flowkv_baseline_segmentwise(plan, s)
         torch.cuda.synchronize()
@@ -1311,7 +1315,7 @@ def test_src_layers_as_really_separate_torch_allocations():
     each tensor's own bytes."""
     w = synth.config2_llama8b_13k(num_layers=3)
     dp = P.DevicePools(w, separate_src_layers=True)
-    assert len({t.data_ptr() for t in dp.src_layers}) == 3 and dp.src.layer_offsets
+    assert len({t.data_ptr() for t in dp.src_layers}) == 3 and dp.src.plane_offsets
     plan, s = dp.plan(F.FLOWKV_CHECK_DST_ALIAS), torch.cuda.current_stream().cuda_stream
     plan.transfer(s)
     torch.cuda.synchronize()

@@ -37,8 +37,8 @@ def test_library_exports_every_symbol_the_header_declares():
 
 
 def test_struct_sizes_match_header_layout():
-    assert C.sizeof(F.flowkv_pool) == 8 + 8 * 4 + 5 * 8 + 8          # + layer_offsets (FLOWKV_VERSION 4)
-    assert F.flowkv_pool.layer_offsets.offset == 80
+    assert C.sizeof(F.flowkv_pool) == 8 + 8 * 4 + 5 * 8 + 8          # + plane_offsets (FLOWKV_VERSION 4)
+    assert F.flowkv_pool.plane_offsets.offset == 80
     assert C.sizeof(F.flowkv_request) == 32
     assert C.sizeof(F.flowkv_segment) == 40
     assert C.sizeof(F.flowkv_tuning) == 48
@@ -389,7 +389,7 @@ def test_request_batch_marshalled_once_plans_like_the_list():
 
 
 def test_pools_whose_layers_are_separate_allocations_on_the_host_side():
-    """flowkv_pool.layer_offsets (reading A22; P:L98 'separate tensor structures across all layer dimensions'): the
+    """flowkv_pool.plane_offsets (reading A22; `layer_offsets=` of the binding is its stacked-K|V special case; P:L98 'separate tensor structures across all layer dimensions'): the
     alignment is unchanged (layers play no part in it), a token-major pool stays in span mode, two block-major pools
     are no longer flat (a block is not one byte range), a misaligned offset is refused, the layer stride is ignored."""
     L, NB, BS = 3, 16, 4
@@ -415,7 +415,17 @@ def test_pools_whose_layers_are_separate_allocations_on_the_host_side():
     assert _segs(F.flowkv_plan_host(z, _pool("lkbthd", L=L), req)) == _segs(plain)
     with pytest.raises(F.FlowKVError) as ei:
         F.flowkv_plan_host(F.make_pool(FAKE, L, 2, 8, 2, NB, BS, "lkbthd", layer_offsets=[0, 4104, 8192]), _pool("lkbthd", L=L), req)
-    assert ei.value.status == F.FLOWKV_ERR_ALIGN and "layer offset" in str(ei.value)
+    assert ei.value.status == F.FLOWKV_ERR_ALIGN and "plane offset" in str(ei.value)
+    # fully separate K and V tensors per layer: 2L plane offsets; both the layer and the K|V stride are ignored
+    po = [4096 * (7 * p_ % 6) + 16 * p_ for p_ in range(2 * L)]
+    zz = list(sep.stride_bytes)
+    zz[0] = zz[1] = 0
+    kvsep = F.make_pool(FAKE, L, 2, 8, 2, NB, BS, "strided", zz, plane_offsets=po)
+    pk = F.flowkv_plan_host(kvsep, _pool("lkbthd", L=L), req)
+    assert _segs(pk) == _segs(plain) and pk.stats["mode_transfer"] == 1 and pk.stats["vec_bytes"] == 16
+    assert F.pool_bytes(kvsep) == max(po) + O.PoolGeom.lkbthd(1, 2, 8, 2, NB, BS).plane_bytes()
+    with pytest.raises(F.FlowKVError):
+        F.make_pool(FAKE, L, 2, 8, 2, NB, BS, "strided", zz)                      # without offsets those strides are required
     # 32-byte vectors need 32-byte aligned offsets
     v32 = F.flowkv_plan_host(F.make_pool(FAKE, L, 2, 16, 2, NB, BS, "lkbthd", layer_offsets=[0, 1 << 20, 2 << 20]),
                              _pool("lkbthd", L=L, D=16), req)
