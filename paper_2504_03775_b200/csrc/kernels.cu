@@ -136,13 +136,16 @@ template <uint32_t N> struct ParamChunks {
 //                chunk sits at  staging_tok_off * window_bytes_per_token            (request base)
 //                             + (plane - plane0) * T_r * tok_bytes                  (plane slab)
 //                             + token_in_request * tok_bytes.
+// PO = false: the caller has already established that neither side carries per-plane offsets (the branch is then
+// compiled out: the rows-type kernels, whose tiles are small, pick their loop body once per launch).
+template <bool PO = true>
 __device__ __forceinline__ int64_t side_offset(const Side& s, int64_t off, uint32_t plane, uint32_t req_tokens,
                                                uint32_t tok_bytes) {
   if (s.dense) {
     const uint32_t tok0 = (uint32_t)((uint64_t)off >> 32), t = (uint32_t)off;
     return (int64_t)tok0 * s.s_layer + ((int64_t)(plane - s.plane0) * req_tokens + t) * (int64_t)tok_bytes;
   }
-  if (s.plane_off) return __ldg(s.plane_off + plane) + off;          // planes are separate allocations (A22)
+  if (PO && s.plane_off) return __ldg(s.plane_off + plane) + off;    // planes are separate allocations (A22)
   return (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv + off;
 }
 
@@ -240,6 +243,26 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
 // ------------------------------------------------------------------------------------------------
 // ldst / rows: token- and head-strided rows (layout and block-size conversion fused in the move)
 // ------------------------------------------------------------------------------------------------
+template <int VEC, int UNROLL, int HINT, class CS, bool PO>
+__device__ __forceinline__ void rows_tiles(const KernelParams& p, const CS& cs, uint32_t tile, uint32_t plane, uint32_t ci,
+                                           uint32_t lane, uint32_t G, uint32_t n_groups, uint32_t vpr, bool pow2, uint64_t pol) {
+  Chunk c = cs.get(ci);
+  for (; tile < p.n_tiles; tile += n_groups) {
+    const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see fk_span_ldst)
+    uint32_t nplane = 0, nci = 0;
+    Chunk cn = c;
+    if (next < p.n_tiles) {
+      decode_tile(p, next, nplane, nci);
+      cn = cs.get(nci);
+    }
+    const char* __restrict__ s = p.src.base + side_offset<PO>(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* __restrict__ d = p.dst.base + side_offset<PO>(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
+    c = cn;
+    plane = nplane;
+  }
+}
+
 template <int VEC, int UNROLL, int HINT, class CS>
 __global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -256,21 +279,12 @@ __global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ K
   uint32_t plane, ci;
   decode_tile(p, tile, plane, ci);
   pdl_wait_prior_grid();
-  Chunk c = cs.get(ci);
-  for (; tile < p.n_tiles; tile += n_groups) {
-    const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see fk_span_ldst)
-    uint32_t nplane = 0, nci = 0;
-    Chunk cn = c;
-    if (next < p.n_tiles) {
-      decode_tile(p, next, nplane, nci);
-      cn = cs.get(nci);
-    }
-    const char* __restrict__ s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
-    char* __restrict__ d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
-    copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
-    c = cn;
-    plane = nplane;
-  }
+  // rows tiles are small (one block's tokens of one plane): the per-plane-offset lookup (A22) is decided once per
+  // launch, not once per tile, so pools without it run exactly the loop they ran before it existed
+  if (p.src.plane_off || p.dst.plane_off)
+    rows_tiles<VEC, UNROLL, HINT, CS, true>(p, cs, tile, plane, ci, lane, G, n_groups, vpr, pow2, pol);
+  else
+    rows_tiles<VEC, UNROLL, HINT, CS, false>(p, cs, tile, plane, ci, lane, G, n_groups, vpr, pow2, pol);
 }
 
 // ------------------------------------------------------------------------------------------------
