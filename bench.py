@@ -726,7 +726,7 @@ def main() -> None:
     ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
     ap.add_argument("--device-tables", action="store_true",
                     help="time flowkv_transfer_tables (block tables resident on the device, no plan) instead of plan+transfer")
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-serial", action="store_true", help="pack then unpack on one stream instead of the pipeline")
     ap.add_argument("--e2e-direct", action="store_true",
