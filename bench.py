@@ -589,7 +589,10 @@ def run_ours(args) -> None:
             duplex = pb / (best * 1e-3) / 1e9
             # ... and what the route must be: a CHUNKED duplex pipeline (chunk c returns once it has landed), copy
             # engines only, same chunk count as the route — the bound e2e.value is read against (bench_hostlink.py)
-            n_ch = args.e2e_chunks or int(min(64, max(4, np.floor(np.sqrt(nbytes / 400e3) + 0.5))))   # the library's default rule
+            planes_ = 2 * w.shape.num_layers                     # the library's default rule: equal chunks, count nearest sqrt(payload / 400 KB)
+            tgt_ = min(64.0, max(4.0, float(np.sqrt(nbytes / 400e3))))
+            n_ch = args.e2e_chunks or min((d for d in range(min(planes_, 4), min(planes_, 64) + 1) if planes_ % d == 0),
+                                          key=lambda d: abs(np.log(d / tgt_)))
             wbp = pb // n_ch
             side2 = torch.cuda.Stream()
             bestp = None

@@ -42,6 +42,9 @@ def main(argv=None) -> None:
     ap.add_argument("--table3", action="store_true",
                     help="the paper's Table 3 request sizes (500 .. 12,000 tokens, src runs ~ Geometric(mean 4)); adds the "
                          "latency of the host route (flowkv_plan + flowkv_transfer_via_host: pool -> pinned host -> pool)")
+    ap.add_argument("--chunk-grid", action="store_true",
+                    help="with --table3: the host route's latency for n_chunks = 1 .. 64 per request size (what the "
+                         "library's default chunk rule was fitted to)")
     ap.add_argument("--tuning-grid", action="store_true",
                     help="time a grid of tile sizes / CTA shapes per point instead of the baselines (launch-shape A/B)")
     args = ap.parse_args(argv)
@@ -188,6 +191,26 @@ def main(argv=None) -> None:
                         hl.append((time.perf_counter() - t0) * 1e3)
                     pv.destroy()
                 del scratch
+                if args.chunk_grid:
+                    grid = {}
+                    for nc in (1, 2, 4, 8, 16, 32, 64):
+                        pv = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                        sbn = F.flowkv_via_host_scratch_bytes(pv, nc)
+                        pv.destroy()
+                        scr = P.alloc_bytes(sbn)
+                        gl = []
+                        for i in range(9):
+                            torch.cuda.synchronize()
+                            t0 = time.perf_counter()
+                            pv = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
+                            F.flowkv_transfer_via_host(pv, via_host.data_ptr(), payload, nc, 0, s, scr.data_ptr(), sbn)
+                            torch.cuda.synchronize()
+                            if i:
+                                gl.append((time.perf_counter() - t0) * 1e3)
+                            pv.destroy()
+                        del scr
+                        grid[nc] = float(np.median(gl))
+                    row["via_host_latency_ms_by_chunks"] = grid
                 row["via_host_latency_ms_plan_to_done"] = float(np.median(hl))
                 row["via_host_GBps_each_way"] = payload / (float(np.median(hl)) * 1e-3) / 1e9
             if not args.no_baselines:

@@ -279,7 +279,8 @@ FLOWKV_API flowkv_status flowkv_unpack_window(const flowkv_plan_t* plan, const v
  *     (flowkv_pack_window, on `stream`), moved D2H and H2D by cudaMemcpyAsync on two copy queues of their own, and
  *     unpacked from a second slot (flowkv_unpack_window, on a fourth queue), so neither engine ever waits behind a
  *     kernel.  On B200 the copy engines sustain ~50 GB/s in both directions at once where SM loads over PCIe drop
- *     to ~38 GB/s.  n_chunks is clamped to [1, 2L]; default (0) = round(sqrt(payload_bytes / 400 KB)) in [4, 64]:
+ *     to ~38 GB/s.  n_chunks is clamped to [1, 2L]; default (0) = the divisor of 2L nearest sqrt(payload_bytes / 400 KB),
+ *     within [4, 64] (equal chunks):
  *     the first outbound and the last inbound chunk cross the link alone, so many small chunks win until the
  *     hand-over between the queues (a few microseconds per chunk) outweighs the shorter head — 16 chunks for a
  *     500-token Llama-3-8B request, 64 from 12,000 tokens up.  host_staging then holds the chunks back to back: with n <= L

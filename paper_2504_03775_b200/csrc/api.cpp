@@ -911,7 +911,18 @@ uint32_t via_host_chunks(const flowkv_plan_t* pl, uint32_t n_chunks, bool engine
       // at ~50 GB/s and ~8 us; measured optimum on the paper's request sizes (profiles/r02_table3.md): 16 chunks at
       // 500 tokens (62.5 MiB), 32 at 4,000, 64 from 12,000 tokens up.
       const double payload = (double)pl->total_tokens * (double)pl->g.bytes_per_token;
-      n_chunks = (uint32_t)std::min(64.0, std::max(4.0, std::floor(std::sqrt(payload / 400e3) + 0.5)));
+      const double target = std::min(64.0, std::max(4.0, std::sqrt(payload / 400e3)));
+      // ... and chunks of EQUAL size: among the counts that divide the 2L planes evenly, the one nearest the target
+      // on a log scale (26 chunks of 2-3 planes measured 6.6 ms where 16 or 32 equal chunks take 6.1-6.2 ms)
+      const uint32_t planes = 2 * pl->g.L;
+      uint32_t best = std::min<uint32_t>(planes, 4);
+      double best_err = 1e30;
+      for (uint32_t d = std::min<uint32_t>(planes, 4); d <= std::min<uint32_t>(planes, 64); ++d) {
+        if (planes % d) continue;
+        const double err = std::fabs(std::log((double)d / target));
+        if (err < best_err) { best_err = err; best = d; }
+      }
+      n_chunks = best;
     }
   }
   return std::max<uint32_t>(1, std::min(n_chunks, engines ? 2 * pl->g.L : pl->g.L));

@@ -550,8 +550,10 @@ def test_transfer_via_pinned_host_with_copy_engines(n_chunks, ctas, small):
     launched = F.flowkv_launch_count() - n0
     if n_chunks:
         chunks = min(n_chunks, 2 * L)                                  # clamped to one chunk per plane
-    else:       # default: round(sqrt(payload / 400 KB)) in [4, 64] (flowkv.h), then the same clamp
-        chunks = min(int(min(64, max(4, np.floor(np.sqrt(nbytes / 400e3) + 0.5)))), 2 * L)
+    else:       # default: the divisor of 2L nearest sqrt(payload / 400 KB) on a log scale, within [4, 64] (flowkv.h)
+        target = min(64.0, max(4.0, np.sqrt(nbytes / 400e3)))
+        cands = [d for d in range(min(2 * L, 4), min(2 * L, 64) + 1) if (2 * L) % d == 0]
+        chunks = min(cands, key=lambda d: abs(np.log(d / target)))
     assert launched == 2 * chunks
     G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "via host (copy engines): dst")
     if chunks <= L:       # layer windows (A20)
