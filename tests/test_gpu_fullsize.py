@@ -338,3 +338,32 @@ def test_cfg5_pack_to_pinned_host_32k_tokens_full_size():
         O.pack(src_slab, g1, r.src_blocks, T, exp, 0)
         G.assert_same(wire[2 * layer * T * tokb: 2 * (layer + 1) * T * tokb], exp, f"wire bytes of layer {layer}")
     _lkbthd_all_planes_property(w, dp)
+
+
+def test_cfg2_full_size_from_separate_layer_tensors():
+    """configs[1]'s request with the src pool as 32 SEPARATELY allocated 1 GiB tensors (the cache the paper starts from,
+    P:L98; reading A22; `bench.py --config cfg2sep`): offsets = differences of real device pointers.  Every dst layer
+    slab against the oracle run on that layer's own tensor; the planned kernel and the table-driven one."""
+    w = synth.config2_llama8b_13k()
+    _need(w.src.bytes(w.shape) + w.dst.bytes(w.shape))
+    dp = P.DevicePools(w, separate_src_layers=True)
+    assert len(dp.src_layers) == 32 and dp.src.plane_offsets
+    one_s, one_d, gd = G.geom(w.src, w.shape, num_layers=1), G.geom(w.dst, w.shape, num_layers=1), G.geom(w.dst, w.shape)
+    r = w.requests[0]
+
+    def check(what):
+        for layer, t in enumerate(dp.src_layers):
+            got = dp.dst_buf[layer * gd.s_layer:(layer + 1) * gd.s_layer].cpu().numpy()
+            exp = np.full(gd.s_layer, P.SENTINEL_BYTE, np.uint8)
+            O.transfer(t.cpu().numpy(), one_s, exp, one_d, r.src_blocks, r.dst_blocks, r.num_tokens)
+            G.assert_same(got, exp, f"{what}: layer {layer}")
+
+    n0 = F.flowkv_launch_count()
+    plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS)
+    plan.transfer()
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1 and plan.stats["mode_transfer"] == 1 and plan.stats["vec_bytes"] == 32
+    check("planned")
+    P.fill_sentinel(dp.dst_buf)
+    _run_tables(w, dp)
+    check("table-driven")
