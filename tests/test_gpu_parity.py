@@ -1330,3 +1330,55 @@ def test_src_layers_as_really_separate_torch_allocations():
                    r.src_blocks, r.dst_blocks, r.num_tokens)
     G.assert_same(P.to_numpy(dp.dst_buf), exp, "separate torch tensors per layer")
     plan.destroy()
+
+
+@pytest.mark.parametrize("reader", ["span_ldst", "rows_ldst", "span_bulk", "rows_tma", "tables", "span_ldst_uploaded"])
+def test_back_to_back_dependent_transfers_see_each_others_writes(reader):
+    """Programmatic dependent launch: every copy kernel lets the next one start early (launch_dependents at entry) and
+    must wait for the previous grid's memory before touching any (griddepcontrol.wait).  Writer: pool0 -> pool1 as 48
+    CTAs of ONE 1 MiB tile each — a grid that leaves most SMs free and runs for tens of microseconds, so the reader's
+    CTAs are resident while it is still storing.  Reader: pool1 -> pool2 launched right behind it on the same stream,
+    one of each kernel family.  pool2 must equal the oracle applied twice; with the wait removed from the kernels
+    every one of these cases reads sentinel bytes (checked once by building the library without it)."""
+    L, H, D, e, T = 24, 4, 64, 2, 2048                      # 512 B per token and plane: 1 MiB per plane
+    lay2, bs2 = ("blkhtd", 32) if reader.startswith("rows") else ("lkbthd", 16)
+    g0 = g1 = O.PoolGeom.lkbthd(L, H, D, e, T // 16, 16)
+    g2 = getattr(O.PoolGeom, lay2)(L, H, D, e, T // bs2 + 3, bs2)
+    b0, b1, b2 = P.alloc_bytes(g0.span_bytes()), P.alloc_bytes(g1.span_bytes()), P.alloc_bytes(g2.span_bytes())
+    P.fill_values(b0, "bits", "fp16", 78)
+    p0 = F.make_pool(b0.data_ptr(), L, H, D, e, T // 16, 16, "lkbthd")
+    p1 = F.make_pool(b1.data_ptr(), L, H, D, e, T // 16, 16, "lkbthd")
+    p2 = F.make_pool(b2.data_ptr(), L, H, D, e, T // bs2 + 3, bs2, lay2)
+    ident = np.arange(T // 16, dtype=np.int32)
+    tab2 = np.random.default_rng(78).permutation(T // bs2 + 3)[:T // bs2].astype(np.int32)
+    s = torch.cuda.current_stream().cuda_stream
+    writer = F.flowkv_plan(p0, p1, [F.Request(T, ident, ident)], 0, {"tile_bytes": 1 << 20, "threads": 512}, s)
+    assert writer.stats["n_chunks_transfer"] == 1 and writer.stats["grid"] == 2 * L
+    tun = {"span_ldst": None, "rows_ldst": None, "span_bulk": {"variant": "bulk"}, "rows_tma": {"variant": "bulk"},
+           "tables": None, "span_ldst_uploaded": {"plan_in_params": 1}}[reader]
+    rd = F.flowkv_plan(p1, p2, [F.Request(T, ident, tab2)], 0, tun, s)
+    if reader in ("span_bulk", "rows_tma"):
+        assert rd.stats["variant"] == F.FLOWKV_VARIANT_BULK
+    st1, dt2 = torch.from_numpy(ident).cuda(), torch.from_numpy(tab2).cuda()
+    lens = torch.tensor([T], dtype=torch.int32, device="cuda")
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    src_np = P.to_numpy(b0)
+    e1 = np.full(g1.span_bytes(), P.SENTINEL_BYTE, np.uint8)
+    O.transfer(src_np, g0, e1, g1, ident, ident, T)
+    e2 = np.full(g2.span_bytes(), P.SENTINEL_BYTE, np.uint8)
+    O.transfer(e1, g1, e2, g2, ident, tab2, T)
+    for rep in range(4):
+        P.fill_sentinel(b1)
+        P.fill_sentinel(b2)
+        torch.cuda.synchronize()
+        writer.transfer(s)                                  # nothing between the two launches
+        if reader == "tables":
+            F.flowkv_transfer_tables(p1, p2, st1.data_ptr(), dt2.data_ptr(), lens.data_ptr(), 1, len(ident), len(tab2), T,
+                                     flag.data_ptr(), None, s)
+        else:
+            rd.transfer(s)
+        torch.cuda.synchronize()
+        G.assert_same(P.to_numpy(b2), e2, f"{reader} behind a long writer, pass {rep}")
+    assert int(flag.item()) == 0
+    writer.destroy()
+    rd.destroy()
