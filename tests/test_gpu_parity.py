@@ -1382,3 +1382,21 @@ def test_back_to_back_dependent_transfers_see_each_others_writes(reader):
     assert int(flag.item()) == 0
     writer.destroy()
     rd.destroy()
+
+
+@pytest.mark.parametrize("stages", [2, 3, 16])
+@pytest.mark.parametrize("kind", ["span", "flat", "rows_tma"])
+def test_tma_rings_over_many_iterations_on_one_cta(kind, stages):
+    """One driving thread on ONE SM walks the whole batch: hundreds of turns of the mbarrier ring per CTA (phase parity
+    flips every `stages` tiles, slots are reused as soon as their store has read them).  Span ring, flat ring and the
+    TMA tensor path, ring depths 2 / 3 / 16, ragged request ends included; whole dst pool against the oracle."""
+    lay_s, lay_d, bs_d = {"span": ("lkbthd", "lkbthd", 16), "flat": ("blkthd", "blkthd", 16), "rows_tma": ("lkbthd", "blkhtd", 64)}[kind]
+    w = synth.make_workload(f"ring_{kind}", 611 + stages, synth.Shape(3, 4, 64, "bf16"), [1234, 777, 5],
+                            lay_s, 16, ("geometric", 3.0), None, lay_d, bs_d, ("geometric", 5.0), None)
+    tuning = {"variant": "bulk", "max_sms": 1, "ctas_per_sm": 1, "stages": stages, "tile_bytes": 4096}
+    dp, plan, _ = G.run_transfer_and_check(w, tuning)
+    st = plan.stats
+    assert st["variant"] == F.FLOWKV_VARIANT_BULK and st["grid"] == 1 and st["stages"] == stages
+    assert st["mode_transfer"] == {"span": 1, "flat": 3, "rows_tma": 2}[kind]
+    assert (st["n_chunks_transfer"] * st["n_planes"] if kind != "flat" else st["n_chunks_transfer"]) >= 300     # turns of the ring
+    plan.destroy()
