@@ -1400,3 +1400,33 @@ def test_tma_rings_over_many_iterations_on_one_cta(kind, stages):
     assert st["mode_transfer"] == {"span": 1, "flat": 3, "rows_tma": 2}[kind]
     assert (st["n_chunks_transfer"] * st["n_planes"] if kind != "flat" else st["n_chunks_transfer"]) >= 300     # turns of the ring
     plan.destroy()
+
+
+@pytest.mark.parametrize("stages", [2, 3])
+def test_tma_ring_slot_reuse_with_slow_stores_to_pinned_host(stages):
+    """The ring may refill a slot only after the store that drained it has READ it (cp.async.bulk.wait_group.read).
+    Make the stores slow and the loads fast — pack from HBM into mapped pinned host memory through the bulk variant,
+    few CTAs with a short ring — the ordering the PTX model requires the wait for.  (On B200 a library built with that
+    wait relaxed by one group still passes: one SM's TMA unit appears to work its queue in order.  The test pins the
+    result, not the hardware's slack.)"""
+    w = synth.make_workload("ring_host", 733, synth.Shape(4, 8, 128, "bf16"), [4096, 1000],
+                            "lkbthd", 16, ("geometric", 4.0), None, "lkbthd", 16, ("contiguous",), None)
+    dp = P.DevicePools(w, fill="bits")
+    src_np = P.to_numpy(dp.src_buf)
+    s = torch.cuda.current_stream().cuda_stream
+    plan = dp.plan(F.FLOWKV_PLAN_NO_TRANSFER, {"variant": "bulk", "stages": stages, "max_sms": 4, "ctas_per_sm": 1,
+                                               "tile_bytes": 32768}, s)
+    assert plan.stats["variant"] == F.FLOWKV_VARIANT_BULK and plan.stats["stages"] == stages and plan.stats["grid"] == 4
+    nbytes = plan.stats["staging_bytes"]
+    host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    exp = G.oracle_pack(w, src_np)
+    for rep in range(2):
+        host.fill_(P.SENTINEL_BYTE)
+        plan.pack(host.data_ptr(), nbytes, s)
+        torch.cuda.synchronize()
+        G.assert_same(host.numpy(), exp, f"bulk pack to pinned host, pass {rep}")
+    P.fill_sentinel(dp.dst_buf)
+    plan.unpack(host.data_ptr(), nbytes, s)              # slow loads, fast stores: the other direction
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "bulk unpack from pinned host")
+    plan.destroy()
