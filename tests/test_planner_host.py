@@ -432,3 +432,62 @@ def test_pools_whose_layers_are_separate_allocations_on_the_host_side():
     v16 = F.flowkv_plan_host(F.make_pool(FAKE, L, 2, 16, 2, NB, BS, "lkbthd", layer_offsets=[0, (1 << 20) + 16, 2 << 20]),
                              _pool("lkbthd", L=L, D=16), req)
     assert v32.stats["vec_bytes"] == 32 and v16.stats["vec_bytes"] == 16
+
+
+def test_alignment_properties_under_hypothesis():
+    """Property test (hypothesis): batches of 1-4 requests, block sizes 1-64 on each side, tables drawn as runs, two-sided
+    and one-sided plans.  The library's segments == the oracle's okv_align == the test-side definition, request by
+    request; segments never cross requests; staging offsets are the prefix sums of the lengths."""
+    from hypothesis import given, settings, strategies as st, HealthCheck
+
+    @st.composite
+    def batches(draw):
+        bs_s, bs_d = 2 ** draw(st.integers(0, 6)), 2 ** draw(st.integers(0, 6))
+        lens = draw(st.lists(st.integers(0, 150), min_size=1, max_size=4))
+        sides = draw(st.sampled_from(["both", "src", "dst"]))
+        seed = draw(st.integers(0, 2 ** 31 - 1))
+        p_cont = draw(st.sampled_from([0.0, 0.3, 0.7, 1.0]))
+        return bs_s, bs_d, lens, sides, seed, p_cont
+
+    def tables(rng, lens, bs, p_cont):
+        need = [-(-t // bs) for t in lens]
+        NB = sum(need) + int(rng.integers(1, 5))
+        free, out, cur = np.ones(NB, bool), [], -2
+        for n in need:
+            tab = []
+            for _ in range(n):
+                if cur >= 0 and cur + 1 < NB and free[cur + 1] and rng.random() < p_cont:
+                    cur += 1
+                else:
+                    cur = int(rng.choice(np.nonzero(free)[0]))
+                free[cur] = False
+                tab.append(cur)
+            out.append(np.asarray(tab, np.int32))
+        return out, NB
+
+    @settings(max_examples=250, deadline=None, suppress_health_check=list(HealthCheck))
+    @given(batches())
+    def check(b):
+        bs_s, bs_d, lens, sides, seed, p_cont = b
+        rng = np.random.default_rng(seed)
+        S, NBs = tables(rng, lens, bs_s, p_cont)
+        D, NBd = tables(rng, lens, bs_d, p_cont)
+        src = _pool("lkbthd", NB=NBs, BS=bs_s) if sides != "dst" else None
+        dst = _pool("blkhtd", NB=NBd, BS=bs_d) if sides != "src" else None
+        reqs = [F.Request(t, S[i] if src is not None else None, D[i] if dst is not None else None) for i, t in enumerate(lens)]
+        plan = F.flowkv_plan_host(src, dst, reqs, F.FLOWKV_CHECK_DST_ALIAS if dst is not None else 0)
+        segs = plan.segments
+        off = 0
+        for i, t in enumerate(lens):
+            mine = [(s["first_token"], s["n_tokens"]) for s in segs if s["request"] == i]
+            s_tab, d_tab = (S[i] if src is not None else None), (D[i] if dst is not None else None)
+            exp = Hh.segments_from_cuts(Hh.cuts_by_definition(s_tab, bs_s, d_tab, bs_d, t), t) if t else []
+            assert mine == exp, (b, i)
+            if src is not None and dst is not None:
+                assert mine == O.align(S[i], bs_s, D[i], bs_d, t)
+            assert all(s["staging_tok_off"] == off for s in segs if s["request"] == i)
+            off += t
+        assert [s["request"] for s in segs] == sorted(s["request"] for s in segs)
+        assert plan.stats["total_tokens"] == sum(lens)
+
+    check()
