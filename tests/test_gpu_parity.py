@@ -1430,3 +1430,39 @@ def test_tma_ring_slot_reuse_with_slow_stores_to_pinned_host(stages):
     torch.cuda.synchronize()
     G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "bulk unpack from pinned host")
     plan.destroy()
+
+
+def test_prefix_cache_hit_moves_only_the_suffix():
+    """the controller 'identifies global cache prefix matches to ... reduce KV Cache transfer latency' — the decode
+    side already holds the first t0 tokens.  The request then carries the tables from block t0 / BS on and
+    num_tokens = T - t0 (flowkv.h): the cached prefix blocks of dst keep their bytes, the suffix lands exactly where the
+    oracle puts tokens [t0, T) of the full request; segments are those of the full alignment clipped at t0."""
+    L, H, D, e, T, t0 = 3, 4, 64, 2, 1000, 320                     # t0 a multiple of both block sizes (16, 32)
+    gs, gd = O.PoolGeom.lkbthd(L, H, D, e, 80, 16), O.PoolGeom.blkhtd(L, H, D, e, 40, 32)
+    rng = np.random.default_rng(86)
+    stab = np.concatenate([np.arange(5, 25), rng.permutation(np.arange(30, 80))[:43]]).astype(np.int32)     # 63 blocks
+    dtab = rng.permutation(40)[:32].astype(np.int32)
+    src_buf, dst_buf = P.alloc_bytes(gs.span_bytes()), P.alloc_bytes(gd.span_bytes())
+    P.fill_values(src_buf, "bits", "fp16", 86)
+    P.fill_values(dst_buf, "bits", "fp16", 87)                      # the decode pool is full of other requests' bytes
+    src_np, dst0 = P.to_numpy(src_buf), P.to_numpy(dst_buf)
+    src = F.make_pool(src_buf.data_ptr(), L, H, D, e, 80, 16, "lkbthd")
+    dst = F.make_pool(dst_buf.data_ptr(), L, H, D, e, 40, 32, "blkhtd")
+    sub_s, sub_d = stab[t0 // 16:], dtab[t0 // 32:]
+    plan = F.flowkv_plan(src, dst, [F.Request(T - t0, sub_s, sub_d)], F.FLOWKV_CHECK_DST_ALIAS)
+    full = O.align(stab, 16, dtab, 32, T)
+    clipped = [(max(a, t0) - t0, a + n - max(a, t0)) for a, n in full if a + n > t0]
+    assert [(s_["first_token"], s_["n_tokens"]) for s_ in plan.segments] == clipped
+    plan.transfer()
+    torch.cuda.synchronize()
+    # oracle: the FULL request into a scratch copy, then keep only what tokens [t0, T) wrote
+    whole = dst0.copy()
+    O.transfer(src_np, gs, whole, gd, stab, dtab, T)
+    prefix_only = dst0.copy()
+    O.transfer(src_np, gs, prefix_only, gd, stab[:t0 // 16], dtab[:t0 // 32], t0)
+    exp = np.where(prefix_only != dst0, dst0, whole)                # undo the prefix tokens' writes
+    exp2 = dst0.copy()
+    O.transfer(src_np, gs, exp2, gd, sub_s, sub_d, T - t0)          # the same through the sub-tables
+    assert np.array_equal(exp, exp2)
+    G.assert_same(P.to_numpy(dst_buf), exp, "suffix after a prefix-cache hit")
+    plan.destroy()
