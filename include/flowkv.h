@@ -209,7 +209,8 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
  *   SHAPE_MISMATCH  src and dst differ in L, Hkv, Dh or elem_bytes
  *   TABLE_LEN    n_*_blocks != ceil(num_tokens / block_size);  BLOCK_OOB  an id outside [0, num_blocks)
  *   DST_ALIAS    (only with FLOWKV_CHECK_DST_ALIAS) a dst block id named twice in the batch
- *   UNSUPPORTED  block_size not a power of two, a block spanning >= 4 GiB, a row > 1 MiB, >= 2^31 tiles
+ *   UNSUPPORTED  block_size not a power of two, a block spanning >= 4 GiB, a row > 1 MiB, a token > 16 MiB per plane,
+ *                >= 2^31 tiles in one batch (split it)
  *   NOMEM        host allocation failed;  CUDA  a runtime call failed (no device, allocation, upload) */
 FLOWKV_API flowkv_status flowkv_plan(const flowkv_pool* src, const flowkv_pool* dst,
                           const flowkv_request* reqs, uint32_t n_reqs, uint32_t flags,
