@@ -605,9 +605,8 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
   return FLOWKV_OK;
 }
 
-Side pool_side(const flowkv_pool& p, const int64_t* device_plane_off) {
+Side pool_side(const flowkv_pool& p) {
   Side s{};
-  s.plane_off = device_plane_off;
   s.base = (char*)p.base;
   s.s_layer = p.stride_bytes[FLOWKV_S_LAYER];
   s.s_kv = p.stride_bytes[FLOWKV_S_KV];
@@ -714,9 +713,11 @@ flowkv_status run(const flowkv_plan_t* pl, const Op& op, const Side& s, const Si
   kp.group_log2 = log2u(ls.group_threads);
   kp.vpr_log2 = log2_or_none(kp.row_bytes / ls.vec_bytes);
   kp.heads_log2 = log2_or_none(kp.heads);
+  // per-plane offset tables (A22) of whichever side is a pool of this launch (a dense side has none)
+  const PlaneOffs po{s.dense ? nullptr : pl->d_src_plane_off, d.dense ? nullptr : pl->d_dst_plane_off};
   const int e = op.in_params
-                    ? launch_copy(mode, kp, nullptr, op.sched.chunks.data() + first, (uint32_t)op.sched.chunks.size() - first, ls, stream, &op.tma)
-                    : launch_copy(mode, kp, op.d_chunks + first, nullptr, 0, ls, stream, &op.tma);
+                    ? launch_copy(mode, kp, nullptr, op.sched.chunks.data() + first, (uint32_t)op.sched.chunks.size() - first, ls, stream, &op.tma, &po)
+                    : launch_copy(mode, kp, op.d_chunks + first, nullptr, 0, ls, stream, &op.tma, &po);
   if (e != 0) return fail_cuda((cudaError_t)e, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
   g_api_calls.fetch_add(1, std::memory_order_relaxed);
@@ -826,7 +827,7 @@ flowkv_status flowkv_transfer_layers(const flowkv_plan_t* pl, uint32_t layer_beg
     return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pool-to-pool schedule (needs both pools, no FLOWKV_PLAN_NO_TRANSFER)");
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->transfer, pool_side(pl->src, pl->d_src_plane_off), pool_side(pl->dst, pl->d_dst_plane_off), pl->transfer.shape.vec_bytes, stream, ro);
+  return run(pl, pl->transfer, pool_side(pl->src), pool_side(pl->dst), pl->transfer.shape.vec_bytes, stream, ro);
 }
 
 flowkv_status flowkv_transfer(const flowkv_plan_t* pl, void* stream) {
@@ -842,7 +843,7 @@ flowkv_status flowkv_pack_layers(const flowkv_plan_t* pl, void* staging, uint64_
   const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_side(staging, pl->g), vec, stream, ro);
+  return run(pl, pl->pack, pool_side(pl->src), dense_side(staging, pl->g), vec, stream, ro);
 }
 
 flowkv_status flowkv_pack(const flowkv_plan_t* pl, void* staging, uint64_t bytes, void* stream) {
@@ -858,7 +859,7 @@ flowkv_status flowkv_unpack_layers(const flowkv_plan_t* pl, const void* staging,
   const uint32_t vec = ((uintptr_t)staging % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst, pl->d_dst_plane_off), vec, stream, ro);
+  return run(pl, pl->unpack, dense_side(staging, pl->g), pool_side(pl->dst), vec, stream, ro);
 }
 
 flowkv_status flowkv_unpack(const flowkv_plan_t* pl, const void* staging, uint64_t bytes, void* stream) {
@@ -882,7 +883,7 @@ flowkv_status flowkv_pack_window(const flowkv_plan_t* pl, void* window, uint64_t
   const uint32_t vec = ((uintptr_t)window % 32 == 0) ? pl->pack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_side(window, pl->g, layer_begin, layer_end), vec, stream, ro);
+  return run(pl, pl->pack, pool_side(pl->src), dense_side(window, pl->g, layer_begin, layer_end), vec, stream, ro);
 }
 
 flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, uint64_t bytes, uint32_t layer_begin,
@@ -894,7 +895,7 @@ flowkv_status flowkv_unpack_window(const flowkv_plan_t* pl, const void* window, 
   const uint32_t vec = ((uintptr_t)window % 32 == 0) ? pl->unpack.shape.vec_bytes : 16;
   RunOpts ro;
   ro.ranged = true; ro.layer_begin = layer_begin; ro.layer_end = layer_end;
-  return run(pl, pl->unpack, dense_side(window, pl->g, layer_begin, layer_end), pool_side(pl->dst, pl->d_dst_plane_off), vec, stream, ro);
+  return run(pl, pl->unpack, dense_side(window, pl->g, layer_begin, layer_end), pool_side(pl->dst), vec, stream, ro);
 }
 
 namespace {
@@ -1001,11 +1002,11 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
       ro.layer_begin = (uint32_t)((uint64_t)L * c / n_chunks);
       ro.layer_end = (uint32_t)((uint64_t)L * (c + 1) / n_chunks);
       if (ro.layer_begin == ro.layer_end) continue;
-      st = run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_side(host_staging, pl->g), vec, s, ro);          // D2H on `stream`
+      st = run(pl, pl->pack, pool_side(pl->src), dense_side(host_staging, pl->g), vec, s, ro);          // D2H on `stream`
       if (st != FLOWKV_OK) return st;
       FK_TRY(cudaEventRecord(vc.ev[c], s), "cudaEventRecord");
       FK_TRY(cudaStreamWaitEvent(aux, vc.ev[c], 0), "cudaStreamWaitEvent");
-      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst, pl->d_dst_plane_off), vecu, aux, ro);     // H2D on the helper
+      st = run(pl, pl->unpack, dense_side(host_staging, pl->g), pool_side(pl->dst), vecu, aux, ro);     // H2D on the helper
       if (st != FLOWKV_OK) return st;
     }
     FK_TRY(cudaEventRecord(e_done, aux), "cudaEventRecord");
@@ -1042,7 +1043,7 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     char* in_slot = scratch + (2 + (k & 1)) * slot;
     char* host = (char*)host_staging + planes_bytes(pl, 0, p0);
     if (prev2 >= 0) FK_TRY(cudaStreamWaitEvent(s, landed[prev2], 0), "cudaStreamWaitEvent");          // out slot free again
-    st = run(pl, pl->pack, pool_side(pl->src, pl->d_src_plane_off), dense_planes(out_slot, pl->g, p0, p1), pl->pack.shape.vec_bytes, s, ro);
+    st = run(pl, pl->pack, pool_side(pl->src), dense_planes(out_slot, pl->g, p0, p1), pl->pack.shape.vec_bytes, s, ro);
     if (st != FLOWKV_OK) return st;
     FK_TRY(cudaEventRecord(packed[c], s), "cudaEventRecord");
     FK_TRY(cudaStreamWaitEvent(vc.q_d2h, packed[c], 0), "cudaStreamWaitEvent");
@@ -1053,7 +1054,7 @@ flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* pl, void* host_stagi
     FK_TRY(cudaMemcpyAsync(in_slot, host, wb, cudaMemcpyHostToDevice, vc.q_h2d), "cudaMemcpyAsync(H2D)");
     FK_TRY(cudaEventRecord(arrived[c], vc.q_h2d), "cudaEventRecord");
     FK_TRY(cudaStreamWaitEvent(vc.q_unpack, arrived[c], 0), "cudaStreamWaitEvent");
-    st = run(pl, pl->unpack, dense_planes(in_slot, pl->g, p0, p1), pool_side(pl->dst, pl->d_dst_plane_off), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
+    st = run(pl, pl->unpack, dense_planes(in_slot, pl->g, p0, p1), pool_side(pl->dst), pl->unpack.shape.vec_bytes, vc.q_unpack, ro);
     if (st != FLOWKV_OK) return st;
     FK_TRY(cudaEventRecord(unpacked[c], vc.q_unpack), "cudaEventRecord");
     prev2 = prev1;
@@ -1110,8 +1111,9 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   if (e == cudaSuccess && dst && dst->plane_offsets) e = g_plane_offsets.get(dev, dst->plane_offsets, 2 * dst->num_layers, &d_dlo);
   if (e != cudaSuccess) return fail_cuda(e, "upload of plane_offsets");
   TablesParams tp{};
-  tp.kp.src = src ? pool_side(*src, d_slo) : dense_side(dense, g, l0, l1);
-  tp.kp.dst = dst ? pool_side(*dst, d_dlo) : dense_side(dense, g, l0, l1);
+  tp.kp.src = src ? pool_side(*src) : dense_side(dense, g, l0, l1);
+  tp.kp.dst = dst ? pool_side(*dst) : dense_side(dense, g, l0, l1);
+  const PlaneOffs po{d_slo, d_dlo};
   tp.kp.n_planes = 2 * (l1 - l0);
   tp.kp.plane0 = 2 * l0;
   tp.kp.row_bytes = g.row_bytes;
@@ -1143,7 +1145,7 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   tp.kp.group_log2 = log2u(ls.group_threads);
   tp.kp.vpr_log2 = log2_or_none(g.row_bytes / ls.vec_bytes);
   tp.kp.heads_log2 = log2_or_none(g.Hkv);
-  const int rc = launch_tables(tp, ls, stream);
+  const int rc = launch_tables(tp, ls, stream, &po);
   if (rc != 0) return fail_cuda((cudaError_t)rc, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
   g_api_calls.fetch_add(1, std::memory_order_relaxed);

@@ -57,8 +57,14 @@ struct Side {            // one end of a copy as the kernel sees it
                          // s_layer = bytes per token of the layer window the buffer holds, s_kv unused
   uint32_t dense;        // 1: dense staging buffer, 0: paged pool
   uint32_t plane0;       // dense side: first plane of the layer window the buffer holds (0 = whole wire format)
-  const int64_t* plane_off;   // pool side, DEVICE array [2L] or NULL: plane p starts plane_off[p] bytes from base and
-                              // s_layer / s_kv are unused (planes are separate allocations, readings A22 / A3)
+};
+
+// Pools whose planes are separate allocations (readings A22 / A3): per side a DEVICE array [2L] of byte offsets from the
+// side's base (plane p starts at [p]; s_layer / s_kv are then unused), or NULL for an ordinary pool.  Handed to the
+// *_po kernels as a parameter of their own, so that the kernels of ordinary pools are untouched by the feature.
+struct PlaneOffs {
+  const int64_t* src;
+  const int64_t* dst;
 };
 
 // Plans whose every schedule has at most kInlineChunks entries pass them in the kernel parameters instead of
@@ -118,7 +124,8 @@ bool build_rows_tma(const flowkv_pool& src, const flowkv_pool& dst, const struct
 // `device_chunks`, or, when `host_chunks` is not NULL (n_host_chunks <= kInlineChunks), travel by value in
 // the kernel parameters.
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
-                uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma = nullptr);
+                uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma = nullptr,
+                const PlaneOffs* po = nullptr);
 // Table-driven transfer (flowkv_transfer_tables): no host plan; the kernel walks device-resident block tables.
 struct TablesParams {
   KernelParams    kp;          // src/dst sides, row_bytes, heads, tok_bytes, group_log2, vpr_log2, heads_log2, n_planes
@@ -136,7 +143,7 @@ struct TablesParams {
   uint32_t        src_num_blocks, dst_num_blocks;
   uint32_t        n_tiles;                // n_planes * n_reqs * q_per_req
 };
-int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream);
+int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream, const PlaneOffs* po = nullptr);
 
 // Largest dynamic shared memory the bulk variant may use on the current device (0 on failure).
 uint32_t bulk_max_smem();

@@ -136,16 +136,17 @@ template <uint32_t N> struct ParamChunks {
 //                chunk sits at  staging_tok_off * window_bytes_per_token            (request base)
 //                             + (plane - plane0) * T_r * tok_bytes                  (plane slab)
 //                             + token_in_request * tok_bytes.
-// PO = false: the caller has already established that neither side carries per-plane offsets (the branch is then
-// compiled out: the rows-type kernels, whose tiles are small, pick their loop body once per launch).
-template <bool PO = true>
-__device__ __forceinline__ int64_t side_offset(const Side& s, int64_t off, uint32_t plane, uint32_t req_tokens,
-                                               uint32_t tok_bytes) {
+// PO = true only in the *_po kernels, which serve pools whose planes are separate allocations (reading A22): `po` is
+// then that side's DEVICE table of per-plane byte offsets (or NULL: that side is an ordinary pool).  Every other
+// kernel passes PO = false and compiles to exactly the code it had before such pools existed.
+template <bool PO>
+__device__ __forceinline__ int64_t side_offset(const Side& s, const int64_t* po, int64_t off, uint32_t plane,
+                                               uint32_t req_tokens, uint32_t tok_bytes) {
   if (s.dense) {
     const uint32_t tok0 = (uint32_t)((uint64_t)off >> 32), t = (uint32_t)off;
     return (int64_t)tok0 * s.s_layer + ((int64_t)(plane - s.plane0) * req_tokens + t) * (int64_t)tok_bytes;
   }
-  if (PO && s.plane_off) return __ldg(s.plane_off + plane) + off;    // planes are separate allocations (A22)
+  if (PO && po) return __ldg(po + plane) + off;
   return (int64_t)(plane >> 1) * s.s_layer + (int64_t)(plane & 1) * s.s_kv + off;
 }
 
@@ -207,8 +208,8 @@ __device__ __forceinline__ void copy_rows(const KernelParams& p, const char* __r
 // ------------------------------------------------------------------------------------------------
 // ldst / span
 // ------------------------------------------------------------------------------------------------
-template <int VEC, int UNROLL, int HINT, class CS>
-__global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
+template <int VEC, int UNROLL, int HINT, class CS, bool PO>
+__device__ __forceinline__ void span_kernel(const KernelParams& p, const CS& cs, const int64_t* po_src, const int64_t* po_dst) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
   const uint32_t lane = gtid & (G - 1);
@@ -232,39 +233,28 @@ __global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ K
       decode_tile(p, next, nplane, nci);
       cn = cs.get(nci);
     }
-    const char* __restrict__ s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
-    char* __restrict__ d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    const char* __restrict__ s = p.src.base + side_offset<PO>(p.src, po_src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* __restrict__ d = p.dst.base + side_offset<PO>(p.dst, po_dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     copy_span<VEC, UNROLL, HINT>(s, d, c.n, lane, step, pol);
     c = cn;
     plane = nplane;
   }
+}
+template <int VEC, int UNROLL, int HINT, class CS>
+__global__ void __launch_bounds__(512, 2) fk_span_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
+  span_kernel<VEC, UNROLL, HINT, CS, false>(p, cs, nullptr, nullptr);
+}
+template <int VEC, int UNROLL, int HINT, class CS>     // planes of a side are separate allocations (A22)
+__global__ void __launch_bounds__(512, 2) fk_span_ldst_po(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                          const __grid_constant__ PlaneOffs po) {
+  span_kernel<VEC, UNROLL, HINT, CS, true>(p, cs, po.src, po.dst);
 }
 
 // ------------------------------------------------------------------------------------------------
 // ldst / rows: token- and head-strided rows (layout and block-size conversion fused in the move)
 // ------------------------------------------------------------------------------------------------
 template <int VEC, int UNROLL, int HINT, class CS, bool PO>
-__device__ __forceinline__ void rows_tiles(const KernelParams& p, const CS& cs, uint32_t tile, uint32_t plane, uint32_t ci,
-                                           uint32_t lane, uint32_t G, uint32_t n_groups, uint32_t vpr, bool pow2, uint64_t pol) {
-  Chunk c = cs.get(ci);
-  for (; tile < p.n_tiles; tile += n_groups) {
-    const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see fk_span_ldst)
-    uint32_t nplane = 0, nci = 0;
-    Chunk cn = c;
-    if (next < p.n_tiles) {
-      decode_tile(p, next, nplane, nci);
-      cn = cs.get(nci);
-    }
-    const char* __restrict__ s = p.src.base + side_offset<PO>(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
-    char* __restrict__ d = p.dst.base + side_offset<PO>(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
-    copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
-    c = cn;
-    plane = nplane;
-  }
-}
-
-template <int VEC, int UNROLL, int HINT, class CS>
-__global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
+__device__ __forceinline__ void rows_kernel(const KernelParams& p, const CS& cs, const int64_t* po_src, const int64_t* po_dst) {
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
   const uint32_t lane = gtid & (G - 1);
@@ -279,12 +269,30 @@ __global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ K
   uint32_t plane, ci;
   decode_tile(p, tile, plane, ci);
   pdl_wait_prior_grid();
-  // rows tiles are small (one block's tokens of one plane): the per-plane-offset lookup (A22) is decided once per
-  // launch, not once per tile, so pools without it run exactly the loop they ran before it existed
-  if (p.src.plane_off || p.dst.plane_off)
-    rows_tiles<VEC, UNROLL, HINT, CS, true>(p, cs, tile, plane, ci, lane, G, n_groups, vpr, pow2, pol);
-  else
-    rows_tiles<VEC, UNROLL, HINT, CS, false>(p, cs, tile, plane, ci, lane, G, n_groups, vpr, pow2, pol);
+  Chunk c = cs.get(ci);
+  for (; tile < p.n_tiles; tile += n_groups) {
+    const uint32_t next = tile + n_groups;           // prefetch the next schedule entry (see span_kernel)
+    uint32_t nplane = 0, nci = 0;
+    Chunk cn = c;
+    if (next < p.n_tiles) {
+      decode_tile(p, next, nplane, nci);
+      cn = cs.get(nci);
+    }
+    const char* __restrict__ s = p.src.base + side_offset<PO>(p.src, po_src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* __restrict__ d = p.dst.base + side_offset<PO>(p.dst, po_dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
+    c = cn;
+    plane = nplane;
+  }
+}
+template <int VEC, int UNROLL, int HINT, class CS>
+__global__ void __launch_bounds__(512, 2) fk_rows_ldst(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs) {
+  rows_kernel<VEC, UNROLL, HINT, CS, false>(p, cs, nullptr, nullptr);
+}
+template <int VEC, int UNROLL, int HINT, class CS>     // planes of a side are separate allocations (A22)
+__global__ void __launch_bounds__(512, 2) fk_rows_ldst_po(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                          const __grid_constant__ PlaneOffs po) {
+  rows_kernel<VEC, UNROLL, HINT, CS, true>(p, cs, po.src, po.dst);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -325,8 +333,8 @@ __global__ void __launch_bounds__(512, 2) fk_flat_ldst(const __grid_constant__ K
     uint32_t plane, ci;
     decode_tile(p, tile, plane, ci);
     const Chunk c = cs.get(p.n_flat + ci);
-    const char* s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
-    char* d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    const char* s = p.src.base + side_offset<false>(p.src, nullptr, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* d = p.dst.base + side_offset<false>(p.dst, nullptr, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     copy_rows<VEC, UNROLL, HINT>(p, s, d, c.n, lane, G, vpr, pow2, pol);
   }
 }
@@ -372,9 +380,9 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 constexpr int kBulkMaxStages = 16;
 
 // stage_bytes: size of one ring slot (>= every chunk's n).  n_stages in [2, kBulkMaxStages].
-template <class CS>
-__global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
-                                                      uint32_t stage_bytes, uint32_t n_stages) {
+template <class CS, bool PO>
+__device__ __forceinline__ void span_bulk_kernel(const KernelParams& p, const CS& cs, uint32_t stage_bytes, uint32_t n_stages,
+                                                 const int64_t* po_src, const int64_t* po_dst) {
   extern __shared__ __align__(128) char ring[];
   __shared__ __align__(8) uint64_t full[kBulkMaxStages];
   pdl_launch_dependents();
@@ -396,9 +404,9 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
     uint32_t plane, ci;
     decode_tile(p, first + k * stride, plane, ci);
     const Chunk c = cs.get(ci);
-    const char* s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    const char* s = p.src.base + side_offset<PO>(p.src, po_src, c.src_off, plane, c.req_tokens, p.tok_bytes);
     const uint32_t slot = k % n_stages;
-    dptr[slot] = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    dptr[slot] = p.dst.base + side_offset<PO>(p.dst, po_dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     nbytes[slot] = c.n;
     mbar_expect_tx(&full[slot], c.n);
     bulk_g2s(ring + (size_t)slot * stage_bytes, s, c.n, &full[slot], pol);
@@ -417,6 +425,16 @@ __global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ Ke
     }
   }
   bulk_wait_all();
+}
+template <class CS>
+__global__ void __launch_bounds__(32, 1) fk_span_bulk(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                      uint32_t stage_bytes, uint32_t n_stages) {
+  span_bulk_kernel<CS, false>(p, cs, stage_bytes, n_stages, nullptr, nullptr);
+}
+template <class CS>                                   // planes of a side are separate allocations (A22)
+__global__ void __launch_bounds__(32, 1) fk_span_bulk_po(const __grid_constant__ KernelParams p, const __grid_constant__ CS cs,
+                                                         uint32_t stage_bytes, uint32_t n_stages, const __grid_constant__ PlaneOffs po) {
+  span_bulk_kernel<CS, true>(p, cs, stage_bytes, n_stages, po.src, po.dst);
 }
 
 // bulk / flat: the same TMA ring over the plane-free tiles of two congruent block-major pools (the paper's
@@ -476,8 +494,8 @@ __global__ void __launch_bounds__(32, 1) fk_flat_bulk(const __grid_constant__ Ke
     uint32_t plane, ci;
     decode_tile(p, tile, plane, ci);
     const Chunk c = cs.get(p.n_flat + ci);
-    const char* s = p.src.base + side_offset(p.src, c.src_off, plane, c.req_tokens, p.tok_bytes);
-    char* d = p.dst.base + side_offset(p.dst, c.dst_off, plane, c.req_tokens, p.tok_bytes);
+    const char* s = p.src.base + side_offset<false>(p.src, nullptr, c.src_off, plane, c.req_tokens, p.tok_bytes);
+    char* d = p.dst.base + side_offset<false>(p.dst, nullptr, c.dst_off, plane, c.req_tokens, p.tok_bytes);
     copy_rows<16, 8, 0>(p, s, d, c.n, threadIdx.x, 32, vpr, false, 0);
   }
 }
@@ -646,6 +664,35 @@ static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const La
   return (int)launch_ldst<16, 8, CS>(mode, kp, cs, ls, (int)ls.hint, st);
 }
 
+// Pools whose planes are separate allocations (reading A22): the *_po kernels take the per-plane offset tables as one
+// more parameter.  They exist for the uploaded schedule and for the largest parameter form only (a plan of <= 512
+// entries rides in the 16 KiB form whatever its size), in span and rows mode — such pools are never flat and never on
+// the TMA tensor path — so the kernels of every other pool stay exactly what they were.
+template <class CS>
+static int launch_with_po(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, cudaStream_t st,
+                          const PlaneOffs& po) {
+  if (mode != MODE_SPAN && mode != MODE_ROWS) return (int)cudaErrorInvalidValue;
+  if (ls.variant == FLOWKV_VARIANT_BULK && mode == MODE_SPAN) {
+    const uint32_t smem = ls.n_stages * ls.stage_bytes;
+    cudaError_t e = cudaFuncSetAttribute(fk_span_bulk_po<CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    return (int)launch_kernel(fk_span_bulk_po<CS>, ls.grid, 32, smem, st, kp, cs, ls.stage_bytes, ls.n_stages, po);
+  }
+#define FK_LAUNCH_PO(KERNEL, VEC, UNROLL)                                                                       \
+  switch ((int)ls.hint) {                                                                                      \
+    case 0: return (int)launch_kernel(KERNEL<VEC, UNROLL, 0, CS>, ls.grid, ls.threads, 0, st, kp, cs, po);     \
+    case 1: return (int)launch_kernel(KERNEL<VEC, UNROLL, 1, CS>, ls.grid, ls.threads, 0, st, kp, cs, po);     \
+    default: return (int)launch_kernel(KERNEL<VEC, UNROLL, 2, CS>, ls.grid, ls.threads, 0, st, kp, cs, po);    \
+  }
+  if (mode == MODE_SPAN) {
+    if (ls.vec_bytes == 32) { FK_LAUNCH_PO(fk_span_ldst_po, 32, 4) }
+    FK_LAUNCH_PO(fk_span_ldst_po, 16, 8)
+  }
+  if (ls.vec_bytes == 32) { FK_LAUNCH_PO(fk_rows_ldst_po, 32, 4) }
+  FK_LAUNCH_PO(fk_rows_ldst_po, 16, 8)
+#undef FK_LAUNCH_PO
+}
+
 // The parameter block of the larger forms (8-16 KiB) is built on the heap, not on the stack of every launch.
 template <uint32_t N>
 static int launch_inline(Mode mode, const KernelParams& kp, const Chunk* host_chunks, uint32_t n, const LaunchShape& ls,
@@ -664,10 +711,19 @@ static int launch_inline(Mode mode, const KernelParams& kp, const Chunk* host_ch
 }
 
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
-                uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma) {
+                uint32_t n_host_chunks, const LaunchShape& ls, void* stream, const RowsTma* tma, const PlaneOffs* po) {
   cudaStream_t st = (cudaStream_t)stream;
+  if (host_chunks && n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
+  if (po && (po->src || po->dst)) {        // planes of a side are separate allocations (A22)
+    if (!host_chunks) return launch_with_po(mode, kp, GlobalChunks{device_chunks}, ls, st, *po);
+    ParamChunks<kInlineChunks>* pc = new (std::nothrow) ParamChunks<kInlineChunks>;
+    if (!pc) return (int)cudaErrorMemoryAllocation;
+    memcpy(pc->c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
+    const int rc = launch_with_po(mode, kp, *pc, ls, st, *po);
+    delete pc;
+    return rc;
+  }
   if (host_chunks) {                       // small plan: the schedule rides in the kernel parameters
-    if (n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
     if (n_host_chunks <= kInlineTiers[0]) return launch_inline<kInlineTiers[0]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
     if (n_host_chunks <= kInlineTiers[1]) return launch_inline<kInlineTiers[1]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
     if (n_host_chunks <= kInlineTiers[2]) return launch_inline<kInlineTiers[2]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
@@ -685,20 +741,20 @@ int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, c
 // change between replays of a captured graph.
 // ------------------------------------------------------------------------------------------------
 // Address of token t0 of request r in plane `plane` on one side; `ok` is cleared when a block id is out of range.
-__device__ __forceinline__ int64_t tables_side(const Side& sd, const int32_t* tab, uint32_t max_blocks, uint32_t bs_log2,
-                                               int64_t s_block, uint32_t num_blocks, uint32_t r, uint32_t t0, uint32_t plane,
-                                               uint32_t T, uint64_t tok0, uint32_t tok_bytes, bool& ok) {
+template <bool PO>
+__device__ __forceinline__ int64_t tables_side(const Side& sd, const int64_t* po, const int32_t* tab, uint32_t max_blocks,
+                                               uint32_t bs_log2, int64_t s_block, uint32_t num_blocks, uint32_t r, uint32_t t0,
+                                               uint32_t plane, uint32_t T, uint64_t tok0, uint32_t tok_bytes, bool& ok) {
   if (sd.dense)       // layer window in wire order (A12/A20): request base + plane slab + token
     return (int64_t)tok0 * sd.s_layer + ((int64_t)(plane - sd.plane0) * T + t0) * (int64_t)tok_bytes;
   const int32_t b = __ldg(tab + (size_t)r * max_blocks + (t0 >> bs_log2));
   if ((uint32_t)b >= num_blocks) ok = false;
-  const int64_t pl = sd.plane_off ? __ldg(sd.plane_off + plane) : (int64_t)(plane >> 1) * sd.s_layer + (int64_t)(plane & 1) * sd.s_kv;
-  return pl + (int64_t)b * s_block +
-         (int64_t)(t0 & ((1u << bs_log2) - 1)) * sd.s_token;
+  const int64_t pl = (PO && po) ? __ldg(po + plane) : (int64_t)(plane >> 1) * sd.s_layer + (int64_t)(plane & 1) * sd.s_kv;
+  return pl + (int64_t)b * s_block + (int64_t)(t0 & ((1u << bs_log2) - 1)) * sd.s_token;
 }
 
-template <int VEC, int UNROLL, int HINT>
-__global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__ TablesParams tp) {
+template <int VEC, int UNROLL, int HINT, bool PO>
+__device__ __forceinline__ void tables_kernel(const TablesParams& tp, const int64_t* po_src, const int64_t* po_dst) {
   const KernelParams& p = tp.kp;
   const uint32_t gtid = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t G = 1u << p.group_log2;
@@ -723,9 +779,9 @@ __global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__
     if (t0 >= T) continue;
     const uint32_t n = min(g, T - t0);
     bool ok = true;
-    const int64_t so = tables_side(p.src, tp.src_tables, tp.max_src_blocks, tp.src_bs_log2, tp.src_s_block, tp.src_num_blocks,
+    const int64_t so = tables_side<PO>(p.src, po_src, tp.src_tables, tp.max_src_blocks, tp.src_bs_log2, tp.src_s_block, tp.src_num_blocks,
                                    r, t0, plane, T, tok0, p.tok_bytes, ok);
-    const int64_t dof = tables_side(p.dst, tp.dst_tables, tp.max_dst_blocks, tp.dst_bs_log2, tp.dst_s_block, tp.dst_num_blocks,
+    const int64_t dof = tables_side<PO>(p.dst, po_dst, tp.dst_tables, tp.max_dst_blocks, tp.dst_bs_log2, tp.dst_s_block, tp.dst_num_blocks,
                                     r, t0, plane, T, tok0, p.tok_bytes, ok);
     uint32_t bad = ok ? 0u : 1u;
     if (tp.cu_tokens && (tok0 + T) * (uint64_t)(p.src.dense ? p.src.s_layer : p.dst.s_layer) > tp.dense_bytes) bad |= 2u;
@@ -736,9 +792,22 @@ __global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__
     copy_rows<VEC, UNROLL, HINT>(p, p.src.base + so, p.dst.base + dof, n, lane, G, vpr, pow2, pol);
   }
 }
+template <int VEC, int UNROLL, int HINT>
+__global__ void __launch_bounds__(512, 2) fk_tables_ldst(const __grid_constant__ TablesParams tp) {
+  tables_kernel<VEC, UNROLL, HINT, false>(tp, nullptr, nullptr);
+}
+template <int VEC, int UNROLL, int HINT>              // planes of a side are separate allocations (A22)
+__global__ void __launch_bounds__(512, 2) fk_tables_ldst_po(const __grid_constant__ TablesParams tp,
+                                                            const __grid_constant__ PlaneOffs po) {
+  tables_kernel<VEC, UNROLL, HINT, true>(tp, po.src, po.dst);
+}
 
-int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream) {
+int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream, const PlaneOffs* po) {
   cudaStream_t st = (cudaStream_t)stream;
+  if (po && (po->src || po->dst)) {
+    if (ls.vec_bytes == 32) return (int)launch_kernel(fk_tables_ldst_po<32, 4, 2>, ls.grid, ls.threads, 0, st, tp, *po);
+    return (int)launch_kernel(fk_tables_ldst_po<16, 8, 2>, ls.grid, ls.threads, 0, st, tp, *po);
+  }
   if (ls.vec_bytes == 32) return (int)launch_kernel(fk_tables_ldst<32, 4, 2>, ls.grid, ls.threads, 0, st, tp);
   return (int)launch_kernel(fk_tables_ldst<16, 8, 2>, ls.grid, ls.threads, 0, st, tp);
 }
