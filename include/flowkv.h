@@ -104,7 +104,8 @@ typedef struct {
                              * multiples of 16, any order, gaps allowed.  One tensor per layer with K and V stacked inside
                              * is plane_offsets[2l + c] = layer_offset[l] + c * s_kv.  The block, token and head strides
                              * describe one plane.  Such pools run the register / bulk-copy paths (no flat mode, no TMA
-                             * tensor path). */
+                             * tensor path) through kernels of their own; a schedule of <= 512 entries then always rides
+                             * in the largest (16 KiB) parameter form. */
 } flowkv_pool;
 
 /* One request: its length and both sides' block-id lists.
