@@ -157,6 +157,7 @@ def load_peaks() -> tuple:
 
 NCU_CAPTURES = {      # workload name -> committed summary of its `ncu --set full` capture (profiles/r02_ncu.md)
     "cfg2_llama8b_13k": "r02_ncu_full_cfg2_fk_span_ldst.csv",
+    "cfg2_llama8b_13k+po": "r02_ncu_full_cfg2sep_fk_span_ldst_po.csv",
     "cfg2_blkthd_13k": "r02_ncu_full_cfg2bm_fk_flat_ldst.csv",
     "cfg2_llama8b_13k+tables": "r02_ncu_full_cfg2_fk_tables_ldst.csv",
     "cfg3_batched_8b": "r02_ncu_full_cfg3_fk_span_ldst.csv",
@@ -423,8 +424,8 @@ def roofline_of(m, payload, w_key, stats, K, device_tables, po=False):
     peak, peak_src = load_peaks()
     achieved = 2 * payload / (m["kern_ms"] * 1e-3) / 1e9
     return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": None if po else load_traffic(w_key), "peak_source": peak_src,
-            # pools with per-plane offsets (cfg2sep) run the *_po instantiation of the same loop body (no ncu capture of it)
+            "traffic": load_traffic(w_key + "+po" if po else w_key), "peak_source": peak_src,
+            # pools with per-plane offsets (cfg2sep) run the *_po instantiation of the same loop body
             "kernel": kernel_name(stats, device_tables) + ("_po" if po else ""),
             "kernel_ms_avg": m["kern_ms"], "kernel_ms_min": m["kern_min_ms"], "algorithmic_bytes_per_launch": 2 * payload,
             "kernel_share_of_step": m["kern_ms"] / (m["t_ms"] / K)}
