@@ -30,5 +30,22 @@ int main(void) {
   /* error path: table too short */
   req.n_src_blocks = 7;
   if (flowkv_plan_host(&src, &dst, &req, 1, 0, NULL, &plan) != FLOWKV_ERR_TABLE_LEN) return 6;
+  req.n_src_blocks = 8;
+  /* a cache whose planes are separate allocations (plane_offsets): same segments, the layer and K|V strides
+   * are ignored; an offset that is no multiple of 16 is refused */
+  {
+    int64_t off[4] = {3 * 65536, 0, 65536 + 4096, 7 * 65536};       /* planes (l0,K) (l0,V) (l1,K) (l1,V) */
+    uint64_t nseg = 0;
+    src.plane_offsets = off;
+    src.stride_bytes[FLOWKV_S_LAYER] = 0;
+    src.stride_bytes[FLOWKV_S_KV] = 0;
+    if (flowkv_plan_host(&src, &dst, &req, 1, 0, NULL, &plan) != FLOWKV_OK) return 7;
+    if (flowkv_plan_info(plan, &st, NULL) != FLOWKV_OK) return 8;
+    nseg = st.n_segments;
+    flowkv_plan_destroy(plan);
+    if (nseg != 4 || st.mode_transfer != 1) return 9;               /* still span mode: strides inside a plane decide */
+    off[2] += 8;
+    if (flowkv_plan_host(&src, &dst, &req, 1, 0, NULL, &plan) != FLOWKV_ERR_ALIGN) return 10;
+  }
   return 0;
 }
