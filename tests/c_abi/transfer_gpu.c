@@ -14,7 +14,7 @@ typedef struct {                       /* mirrors okv_pool of oracle/flowkv_orac
   uint32_t num_layers, num_kv_heads, head_dim, elem_bytes, num_blocks, block_size;
   int64_t s_layer, s_kv, s_block, s_token, s_head;
   uint32_t layer0, _pad;
-  const int64_t* layer_off;            /* NULL here: a stacked pool (reading A22 otherwise) */
+  const int64_t* plane_off;            /* NULL here: a stacked pool (reading A22 otherwise) */
 } okv_pool;
 int okv_transfer(const uint8_t* src, const okv_pool* sp, uint8_t* dst, const okv_pool* dp, const int32_t* src_tab,
                  const int32_t* dst_tab, uint32_t T, uint32_t l0, uint32_t l1);
