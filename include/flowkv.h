@@ -360,6 +360,10 @@ FLOWKV_API flowkv_status flowkv_unpack_tables(const flowkv_pool* dst, const int3
  * synchronise that stream first.  NULL is ignored. */
 FLOWKV_API void flowkv_plan_destroy(flowkv_plan_t* plan);
 
+/* FLOWKV_VERSION the library was built with.  The layout of flowkv_pool changed in version 4 (plane_offsets): a caller
+ * compiled against another header must not pass structs to this library — compare before the first call. */
+FLOWKV_API uint32_t flowkv_version(void);
+
 FLOWKV_API const char* flowkv_status_string(flowkv_status s);
 FLOWKV_API const char* flowkv_last_error(void);          /* thread-local text of the last failure          */
 

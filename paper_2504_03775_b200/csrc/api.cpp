@@ -1423,6 +1423,9 @@ const char* flowkv_status_string(flowkv_status s) {
 const char* flowkv_last_error(void) {
   return impl::flowkv_last_error();
 }
+uint32_t flowkv_version(void) {
+  return FLOWKV_VERSION;
+}
 uint64_t flowkv_launch_count(void) {
   return impl::flowkv_launch_count();
 }

@@ -30,7 +30,9 @@ FLOWKV_VARIANT_AUTO, FLOWKV_VARIANT_LDST, FLOWKV_VARIANT_BULK = 0, 1, 2
 LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "strided": FLOWKV_LAYOUT_STRIDED,
            "blkthd": FLOWKV_LAYOUT_BLKTHD}
 
-EXPORTS = ["flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
+FLOWKV_VERSION = 4          # include/flowkv.h; the struct layouts below are this version's
+
+EXPORTS = ["flowkv_version", "flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
            "flowkv_launch_count", "flowkv_api_call_count", "flowkv_baseline_blockwise", "flowkv_baseline_segmentwise",
            "flowkv_transfer_layers", "flowkv_pack_layers", "flowkv_unpack_layers", "flowkv_transfer_via_host",
@@ -122,6 +124,15 @@ def _load() -> C.CDLL:
     lib.flowkv_plan_destroy.restype = None
     lib.flowkv_status_string.argtypes = [C.c_int]
     lib.flowkv_status_string.restype = C.c_char_p
+    try:                                             # a stale libflowkv.so next to a newer binding: fail loudly, never guess
+        lib.flowkv_version.argtypes = []
+        lib.flowkv_version.restype = C.c_uint32
+        have = lib.flowkv_version()
+    except AttributeError:
+        have = "< 4"
+    if have != FLOWKV_VERSION:
+        raise ImportError(f"{LIB_PATH} is FLOWKV_VERSION {have}, this binding needs {FLOWKV_VERSION} (struct layouts "
+                          "differ): rebuild it with `python -m paper_2504_03775_b200.build --force`")
     lib.flowkv_last_error.argtypes = []
     lib.flowkv_last_error.restype = C.c_char_p
     lib.flowkv_launch_count.argtypes = []
@@ -138,7 +149,7 @@ def _load() -> C.CDLL:
     lib.flowkv_alloc_destroy.argtypes = [C.c_void_p]
     lib.flowkv_alloc_destroy.restype = None
     for n in EXPORTS:
-        if n not in ("flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error", "flowkv_launch_count",
+        if n not in ("flowkv_version", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error", "flowkv_launch_count",
                      "flowkv_api_call_count",
                      "flowkv_alloc_destroy"):
             getattr(lib, n).restype = C.c_int

@@ -491,3 +491,11 @@ def test_alignment_properties_under_hypothesis():
         assert plan.stats["total_tokens"] == sum(lens)
 
     check()
+
+
+def test_library_version_matches_header_and_binding():
+    """flowkv_version() == FLOWKV_VERSION of include/flowkv.h == the version the ctypes struct layouts were written
+    for (the binding refuses to load a library of another version: flowkv_pool grew in version 4)."""
+    hdr = open(os.path.join(ROOT, "include", "flowkv.h")).read()
+    v = int(re.search(r"#define FLOWKV_VERSION (\d+)", hdr).group(1))
+    assert F._lib.flowkv_version() == v == F.FLOWKV_VERSION
