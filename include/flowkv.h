@@ -31,6 +31,9 @@
  *     and return without synchronising.  flowkv_transfer_via_host is the one composite call
  *     (2 kernels per layer chunk); it does not synchronise either.
  *   - A built plan's flowkv_transfer is capturable into a CUDA graph (it is one launch).
+ *   - Every kernel is launched with the programmatic-stream-serialization attribute: it lets the next kernel of the
+ *     stream become resident while it drains, and waits for the previous kernel's memory before touching any
+ *     (griddepcontrol), so stream order holds as usual.  FLOWKV_PDL=0 in the environment turns the attribute off.
  *   - There is no CPU fallback and no other backend: without a CUDA device every call that
  *     needs one returns FLOWKV_ERR_CUDA.
  *   - Thread safety: distinct plans may be used from distinct threads; one plan is run from one
