@@ -94,3 +94,29 @@ class DevicePools:
 
 def to_numpy(buf: torch.Tensor) -> np.ndarray:
     return buf.cpu().numpy()
+
+
+def pool_from_tensors(layers=None, k_layers=None, v_layers=None) -> F.flowkv_pool:
+    """Describe a cache that lives in per-layer torch tensors — the layout engines usually have and the one the paper
+    starts from — without copying anything.  Either
+
+      ``layers``               one tensor per layer shaped [2, num_blocks, block_size, num_kv_heads, head_dim]  (K|V stacked), or
+      ``k_layers, v_layers``   one K and one V tensor per layer, each [num_blocks, block_size, num_kv_heads, head_dim].
+
+    All tensors: same shape, dtype and CUDA device, contiguous.  The descriptor's base is the lowest data pointer and
+    ``plane_offsets`` the distances of the 2L planes from it; the caller keeps the tensors alive."""
+    if layers is not None:
+        assert k_layers is None and v_layers is None
+        ts = list(layers)
+        assert ts and all(t.dim() == 5 and t.shape[0] == 2 for t in ts), "layers: [2, NB, BS, H, D] each"
+        planes = [t[c] for t in ts for c in (0, 1)]
+    else:
+        assert k_layers is not None and v_layers is not None and len(k_layers) == len(v_layers) > 0
+        planes = [t for kv in zip(k_layers, v_layers) for t in kv]
+    p0 = planes[0]
+    assert all(t.shape == p0.shape and t.dtype == p0.dtype and t.device == p0.device and t.is_contiguous() for t in planes), \
+        "every plane: same shape, dtype, device; contiguous"
+    nb, bs, h, d = (int(x) for x in p0.shape)
+    base = min(t.data_ptr() for t in planes)
+    return F.make_pool(base, len(planes) // 2, h, d, p0.element_size(), nb, bs, "lkbthd",
+                       plane_offsets=[t.data_ptr() - base for t in planes])

@@ -1466,3 +1466,48 @@ def test_prefix_cache_hit_moves_only_the_suffix():
     assert np.array_equal(exp, exp2)
     G.assert_same(P.to_numpy(dst_buf), exp, "suffix after a prefix-cache hit")
     plan.destroy()
+
+
+@pytest.mark.parametrize("split_kv", [False, True])
+def test_pool_from_per_layer_torch_tensors(split_kv):
+    """`pools.pool_from_tensors`: a cache held as per-layer torch tensors ([2,NB,BS,H,D] each, or separate K and V tensors
+    per layer) is described in place (base = lowest pointer, plane offsets = pointer distances) and moved into one
+    (B,L,2,H) tensor — Eq. 5's migration — in one launch; checked against torch indexing per plane (test-only) and the
+    oracle run on each plane's own bytes."""
+    L, NB, BS, H, D, T = 5, 48, 16, 4, 64, 700
+    gen = torch.Generator(device="cuda").manual_seed(98)
+    mk = lambda *shape: torch.randn(*shape, device="cuda", dtype=torch.bfloat16, generator=gen)
+    if split_kv:
+        ks, vs = [mk(NB, BS, H, D) for _ in range(L)], [mk(NB, BS, H, D) for _ in range(L)]
+        src = P.pool_from_tensors(k_layers=ks, v_layers=vs)
+        planes = [t for kv in zip(ks, vs) for t in kv]
+    else:
+        layers = [mk(2, NB, BS, H, D) for _ in range(L)]
+        src = P.pool_from_tensors(layers=layers)
+        planes = [t[c] for t in layers for c in (0, 1)]
+    assert src.num_layers == L and src.elem_bytes == 2 and src.plane_offsets
+    dst_t = torch.full((NB, L, 2, BS, H, D), -1.0, device="cuda", dtype=torch.bfloat16)         # one (B,L,2,H) tensor
+    dst = F.make_pool(dst_t.data_ptr(), L, H, D, 2, NB, BS, "blkthd")
+    rng = np.random.default_rng(98)
+    stab, dtab = rng.permutation(NB)[:-(-T // BS)].astype(np.int32), rng.permutation(NB)[:-(-T // BS)].astype(np.int32)
+    n0 = F.flowkv_launch_count()
+    plan = F.flowkv_plan(src, dst, [F.Request(T, stab, dtab)], F.FLOWKV_CHECK_DST_ALIAS)
+    plan.transfer()
+    torch.cuda.synchronize()
+    assert F.flowkv_launch_count() - n0 == 1
+    full, rem = T // BS, T % BS
+    one = O.PoolGeom.lkbthd(1, H, D, 2, NB, BS)
+    gplane = O.PoolGeom(1, H, D, 2, NB, BS, one.s_layer, one.s_kv, one.s_block, one.s_token, one.s_head).with_plane_offsets([0, 0])
+    for p, t in enumerate(planes):
+        l, c = p // 2, p % 2
+        got = dst_t[:, l, c]                                             # [NB, BS, H, D]
+        exp = torch.full_like(got, -1.0)
+        exp[torch.from_numpy(dtab[:full]).long().cuda()] = t[torch.from_numpy(stab[:full]).long().cuda()]
+        exp[int(dtab[full]), :rem] = t[int(stab[full]), :rem]
+        assert torch.equal(got.view(torch.int16), exp.view(torch.int16)), f"plane {p}"
+        # the oracle on this plane alone: a one-layer pool whose K and V plane are both this tensor (offsets [0, 0])
+        o_src = t.contiguous().view(torch.uint8).cpu().numpy().reshape(-1)
+        o_dst = torch.full_like(t, -1.0).view(torch.uint8).cpu().numpy().reshape(-1).copy()
+        O.transfer(o_src, gplane, o_dst, gplane, stab, dtab, T)
+        assert np.array_equal(o_dst, got.contiguous().view(torch.uint8).cpu().numpy().reshape(-1)), f"plane {p} (oracle)"
+    plan.destroy()
