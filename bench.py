@@ -120,6 +120,11 @@ def build_workload(name: str, free_bytes: int):
         return (synth.config2_llama8b_13k(),
                 "configs[1] request and tables, src pool as 32 SEPARATE per-layer tensors of 1 GiB (the cache the paper "
                 "starts from, P:L98; flowkv_pool.plane_offsets), dst one contiguous pool")
+    if name == "cfg2mig":
+        w = synth.make_workload("cfg2_mig_13k", synth.SEED_BASE + 2000, synth.LLAMA3_8B, [13312],
+                                "lkbthd", 16, ("geometric", 4.0), 16384, "blkthd", 16, ("contiguous",), 1024)
+        return w, ("configs[1] request and src tables; src pool = 32 SEPARATE per-layer tensors (the cache the paper starts "
+                   "from, P:L98), dst = ONE (B,L,2,H) tensor: Eq. 5's re-layout fused into the move, one launch")
     if name in ("cfg2bm", "cfg2bm_ragged"):
         w = synth.config2_blockmajor("blkthd", tokens=13312 if name == "cfg2bm" else 13307)
         return w, ("configs[1] request and tables, both pools in the paper's (B,L,2,H) order (Eq. 5; BLKTHD): "
@@ -471,7 +476,7 @@ def run_ours(args) -> None:
         if args.same_device:
             free_b //= world
         w, desc = build_workload(args.config, free_b)
-        dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False, separate_src_layers=args.config == "cfg2sep")
+        dp = P.DevicePools(w, device=f"cuda:{local}", sentinel_dst=False, separate_src_layers=args.config in ("cfg2sep", "cfg2mig"))
         payload = w.payload_bytes
         # --peer: rank r's kernel stores into the dst pool that rank (r+1) % N owns, mapped through CUDA IPC — the paper's
         # single-machine "IPC" mode as a one-sided put; over NVLink when the ranks sit on different GPUs
@@ -519,7 +524,7 @@ def run_ours(args) -> None:
                 "latency_ms_call_to_done_min": m["latency_ms_call_to_done_min"],
                 "latency_ms_call_to_done_per_request": m["latency_ms_call_to_done"] / max(len(w.requests), 1),
                 "hbm_GBps": 2 * value, "pct_of_8TBps_nominal": 100 * 2 * value / world / 8000.0,
-                "roofline": roofline_of(m, payload, wkey, stats, K, args.device_tables, po=args.config == "cfg2sep"),
+                "roofline": roofline_of(m, payload, wkey, stats, K, args.device_tables, po=args.config in ("cfg2sep", "cfg2mig")),
                 "host": host_info(local),
             }
 
@@ -728,7 +733,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg2sep", "cfg2bm", "cfg2bm_ragged", "cfg3", "cfg4"])
+    ap.add_argument("--config", default="cfg2", choices=["cfg1", "cfg2", "cfg2sep", "cfg2mig", "cfg2bm", "cfg2bm_ragged", "cfg3", "cfg4"])
     ap.add_argument("--tuning", default=None, help="JSON dict of flowkv_tuning fields")
     ap.add_argument("--device-tables", action="store_true",
                     help="time flowkv_transfer_tables (block tables resident on the device, no plan) instead of plan+transfer")
@@ -751,7 +756,7 @@ def main() -> None:
     ap.add_argument("--same-device", action="store_true", help="all ranks on cuda:0 with a gloo control plane (a "
                     "functional check of the multi-rank path on a one-GPU box; not a scaling number)")
     args = ap.parse_args()
-    if args.config == "cfg2sep":     # the src pool is 32 separate tensors: no whole-pool probes, link legs or memcpy baselines
+    if args.config in ("cfg2sep", "cfg2mig"):     # the src pool is 32 separate tensors: no whole-pool probes, link legs or memcpy baselines
         args.no_e2e = args.no_baselines = True
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         spawn_ranks(args)          # does not return
