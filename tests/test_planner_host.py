@@ -499,3 +499,28 @@ def test_library_version_matches_header_and_binding():
     hdr = open(os.path.join(ROOT, "include", "flowkv.h")).read()
     v = int(re.search(r"#define FLOWKV_VERSION (\d+)", hdr).group(1))
     assert F._lib.flowkv_version() == v == F.FLOWKV_VERSION
+
+
+def test_pool_from_tensors_describes_per_layer_tensors_in_place():
+    """`pools.pool_from_tensors` (host part, CPU tensors stand in for device ones): base = the lowest data pointer,
+    plane offsets = pointer distances in plane order 2*l + c, shape and element size from the tensors; K|V stacked per
+    layer and separate K / V lists give the same kind of descriptor; the planner accepts it."""
+    import torch
+    from paper_2504_03775_b200 import pools as P
+    L, NB, BS, H, D = 3, 6, 4, 2, 8
+    layers = [torch.zeros(2, NB, BS, H, D, dtype=torch.bfloat16) for _ in range(L)]
+    p = P.pool_from_tensors(layers=layers)
+    base = min(t.data_ptr() for t in layers)
+    per = NB * BS * H * D * 2
+    assert (p.base, p.num_layers, p.num_kv_heads, p.head_dim, p.elem_bytes, p.num_blocks, p.block_size) == (base, L, H, D, 2, NB, BS)
+    assert list(p._plane_offsets_keep) == [t.data_ptr() - base + c * per for t in layers for c in (0, 1)]
+    ks = [torch.zeros(NB, BS, H, D, dtype=torch.float16) for _ in range(L)]
+    vs = [torch.zeros(NB, BS, H, D, dtype=torch.float16) for _ in range(L)]
+    q = P.pool_from_tensors(k_layers=ks, v_layers=vs)
+    b2 = min(t.data_ptr() for t in ks + vs)
+    assert list(q._plane_offsets_keep) == [t.data_ptr() - b2 for kv in zip(ks, vs) for t in kv]
+    req = [F.Request(18, [5, 0, 1, 2, 3], [0, 1, 2, 4, 5])]
+    st = F.flowkv_plan_host(q, _pool("lkbthd", L=L, H=H, D=D, NB=NB, BS=BS), req).stats
+    assert st["n_segments"] == O.count_segments([5, 0, 1, 2, 3], BS, [0, 1, 2, 4, 5], BS, 18) and st["mode_transfer"] == 1
+    with pytest.raises(AssertionError):
+        P.pool_from_tensors(layers=[layers[0], layers[1][:, :3]])          # shapes must agree
