@@ -358,6 +358,38 @@ FLOWKV_API flowkv_status flowkv_unpack_tables(const flowkv_pool* dst, const int3
                                               const void* window, uint64_t bytes, uint32_t layer_begin, uint32_t layer_end,
                                               uint32_t* error_flag, const flowkv_tuning* tuning, void* stream);
 
+/* Pool -> pool for callers that must not allocate device memory: same result as flowkv_transfer, and the call itself
+ * makes no cudaMalloc / cudaFree / pool allocation of any kind (no pinned host allocation either).
+ *
+ * Who needs it.  flowkv_plan() keeps a schedule of more than 512 entries in a device buffer it allocates per plan.
+ * That is unwelcome where the process may not touch the device allocator once it is serving: an engine that gave all
+ * of HBM to its own KV block pool at start-up (a later allocation can fail outright, or eat into memory the engine
+ * has already promised to requests), a latency-bound loop that cannot take the device-wide stall a cudaMalloc or
+ * cudaFree may bring, a tenant held to a fixed memory budget.  Such a caller plans on the host — flowkv_plan_host()
+ * makes no CUDA call — and runs the plan here.
+ *
+ * How.  The schedule goes into a fixed array inside the library's own device image,
+ * FLOWKV_STATIC_SCHEDULE_ENTRIES entries of 32 bytes = 1 MiB.  Every GPU that loads the library carries that 1 MiB
+ * until the process ends, whether or not this function is ever called.  Per call: one cudaMemcpyAsync of the
+ * schedule (from ordinary pageable host memory, which the runtime may hold back until earlier work on `stream` is
+ * done) and one kernel launch, both on `stream`; no host synchronisation beyond that.  The plan may be destroyed as
+ * soon as the call returns.
+ *   plan    built by flowkv_plan_host (or flowkv_plan) with both pools; the pools are the caller's inputs / outputs
+ *           as everywhere else.  Register path only: tuning.variant must be 0 or FLOWKV_VARIANT_LDST.
+ *   stream  cudaStream_t as void*.
+ * First call on a device: with that device current, the library looks up the array's device address once
+ * (cudaGetSymbolAddress) and the SM count, and remembers both.  Make that first call outside any stream capture.
+ * Sharing: all calls on a device use the one array, and it keeps the previous call's entries.  Nothing in it needs
+ * clearing — a launch reads only the entries its own call has just written — but two calls whose GPU work can
+ * overlap (different streams with no event between them, or two threads) race on the array and move garbage.
+ * Calls on a single stream are safe back to back.
+ * Errors (nothing is enqueued): INVALID_ARG plan NULL; UNSUPPORTED the plan has no pool->pool schedule, needs more
+ * than FLOWKV_STATIC_SCHEDULE_ENTRIES entries (flowkv_plan_stats.n_chunks_transfer tells beforehand; split the
+ * batch), asks for the bulk variant, or names a pool with plane_offsets (their device tables would have to be
+ * allocated); CUDA a runtime call failed.  An empty plan is FLOWKV_OK with nothing enqueued. */
+#define FLOWKV_STATIC_SCHEDULE_ENTRIES 32768u
+FLOWKV_API flowkv_status flowkv_transfer_static(const flowkv_plan_t* plan, void* stream);
+
 /* Frees the plan.  Its device buffer is released in stream order on the stream flowkv_plan() was
  * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,
  * synchronise that stream first.  NULL is ignored. */

@@ -1190,6 +1190,58 @@ flowkv_status flowkv_unpack_tables(const flowkv_pool* dst, const int32_t* dst_ta
                        bytes, layer_begin, layer_end, error_flag, tuning, stream);
 }
 
+// Pool -> pool with the schedule in the library's static device array (kernels.cu): for callers that must not
+// allocate device memory.  Works on host plans (flowkv_plan_host makes no CUDA call) as well as device plans; the
+// launch parameters are built here from the plan's host-side schedule, the ordinary run() path is not involved.
+flowkv_status flowkv_transfer_static(const flowkv_plan_t* pl, void* stream) {
+  if (!pl) return fail(FLOWKV_ERR_INVALID_ARG, "plan is NULL");
+  const Op& op = pl->transfer;
+  if (op.sched.mode == MODE_ABSENT)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "plan has no pool-to-pool schedule (needs both pools, no FLOWKV_PLAN_NO_TRANSFER)");
+  if (!pl->src_plane_off.empty() || !pl->dst_plane_off.empty())
+    return fail(FLOWKV_ERR_UNSUPPORTED, "flowkv_transfer_static: pools with plane_offsets need a device table of their own, "
+                                        "which this entry point will not allocate");
+  if (op.shape.variant != FLOWKV_VARIANT_LDST)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "flowkv_transfer_static runs the register path only: plan with tuning.variant 0 or FLOWKV_VARIANT_LDST");
+  // entries a whole-pool launch reads (a flat plan's third part serves layer ranges only)
+  const uint64_t n = op.sched.mode == MODE_FLAT ? (uint64_t)op.sched.n_flat + op.sched.n_ragged : op.sched.chunks.size();
+  if (n > kStaticChunks)
+    return fail(FLOWKV_ERR_UNSUPPORTED, "flowkv_transfer_static: the schedule has " + std::to_string(n) + " entries, the static "
+                "array holds " + std::to_string(kStaticChunks) + " (FLOWKV_STATIC_SCHEDULE_ENTRIES); split the batch");
+  if (n == 0) return FLOWKV_OK;            // A11: nothing to move, nothing enqueued
+  Chunk* d_sched = nullptr;
+  uint32_t sms = 0;
+  int rc = static_schedule_setup(&d_sched, &sms);
+  if (rc != 0) return fail_cuda((cudaError_t)rc, "cudaGetSymbolAddress(static schedule)");
+  KernelParams kp{};
+  kp.src = pool_side(pl->src);
+  kp.dst = pool_side(pl->dst);
+  kp.n_chunks = op.sched.n_per_plane();
+  kp.n_flat = op.sched.n_flat;
+  kp.flat_shift = op.sched.flat_shift;
+  kp.flat_tile = op.sched.flat_tile;
+  kp.n_planes = 2 * pl->g.L;
+  kp.plane0 = 0;
+  kp.n_tiles = (kp.n_flat << kp.flat_shift) + kp.n_chunks * kp.n_planes;
+  kp.row_bytes = pl->g.row_bytes;
+  kp.heads = pl->g.Hkv;
+  kp.tok_bytes = pl->g.tok_bytes;
+  kp.tile_order = op.tile_order;
+  LaunchShape ls = op.shape;
+  const uint32_t groups_per_cta = ls.threads / ls.group_threads;
+  const uint32_t use_sms = pl->tuning.max_sms ? std::min(pl->tuning.max_sms, sms) : sms;   // a host plan assumed 148 SMs
+  const uint64_t cap = (uint64_t)use_sms * (pl->tuning.ctas_per_sm ? pl->tuning.ctas_per_sm : 256);
+  ls.grid = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(cap, (kp.n_tiles + groups_per_cta - 1) / groups_per_cta));
+  kp.group_log2 = log2u(ls.group_threads);
+  kp.vpr_log2 = log2_or_none(kp.row_bytes / ls.vec_bytes);
+  kp.heads_log2 = log2_or_none(kp.heads);
+  rc = launch_copy_static(op.sched.mode, kp, op.sched.chunks.data(), (uint32_t)n, d_sched, ls, stream);
+  if (rc != 0) return fail_cuda((cudaError_t)rc, "flowkv_transfer_static: schedule copy / kernel launch");
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  g_api_calls.fetch_add(2, std::memory_order_relaxed);     // the schedule copy and the launch
+  return FLOWKV_OK;
+}
+
 void flowkv_plan_destroy(flowkv_plan_t* pl) {
   if (!pl) return;
   // via-host work on the helper streams was joined back into the caller's stream by an event, so the
@@ -1413,6 +1465,9 @@ flowkv_status flowkv_unpack_tables(
     uint32_t layer_begin, uint32_t layer_end, uint32_t* error_flag, const flowkv_tuning* tuning,
     void* stream) {
   return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_unpack_tables(dst, dst_tables, cu_tokens, n_reqs, max_dst_blocks, max_tokens, window, bytes, layer_begin, layer_end, error_flag, tuning, stream); });
+}
+flowkv_status flowkv_transfer_static(const flowkv_plan_t* plan, void* stream) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer_static(plan, stream); });
 }
 void flowkv_plan_destroy(flowkv_plan_t* plan) {
   try { impl::flowkv_plan_destroy(plan); } catch (...) {}

@@ -145,6 +145,16 @@ struct TablesParams {
 };
 int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream, const PlaneOffs* po = nullptr);
 
+// flowkv_transfer_static (kernels.cu): the schedule sits in a file-scope __device__ array of kStaticChunks entries.
+//   static_schedule_setup : address of that array on the CURRENT device + the device's SM count; the first call on a
+//                           device asks the runtime (cudaGetSymbolAddress), later calls return the remembered values.
+//   launch_copy_static    : copies `n` entries into the array on `stream`, then launches the one kernel (register path).
+// Neither allocates anything.  cudaError_t as int.
+constexpr uint32_t kStaticChunks = FLOWKV_STATIC_SCHEDULE_ENTRIES;
+int static_schedule_setup(Chunk** addr, uint32_t* num_sms);
+int launch_copy_static(Mode mode, const KernelParams& kp, const Chunk* host_chunks, uint32_t n, Chunk* device_addr,
+                       const LaunchShape& ls, void* stream);
+
 // Largest dynamic shared memory the bulk variant may use on the current device (0 on failure).
 uint32_t bulk_max_smem();
 

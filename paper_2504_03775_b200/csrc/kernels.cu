@@ -28,6 +28,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <utility>
 
@@ -810,6 +811,67 @@ int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream, c
   }
   if (ls.vec_bytes == 32) return (int)launch_kernel(fk_tables_ldst<32, 4, 2>, ls.grid, ls.threads, 0, st, tp);
   return (int)launch_kernel(fk_tables_ldst<16, 8, 2>, ls.grid, ls.threads, 0, st, tp);
+}
+
+// ------------------------------------------------------------------------------------------------
+// flowkv_transfer_static: the schedule-in-global-memory kernels with the schedule in memory nobody allocates.
+//
+// A schedule of more than kInlineChunks entries does not fit the kernel parameters, so the ordinary path
+// (flowkv_plan) puts it into a device buffer it allocates for the plan.  Some callers must not allocate on the
+// device after start-up: a serving engine that has handed all of HBM to its own block pool (a later cudaMalloc
+// can fail, or shrink what the engine believes it owns), a decode loop that cannot afford the device-wide
+// synchronisation cudaMalloc / cudaFree imply, a process held to a fixed memory budget by its operator.  For them
+// the schedule lives in the array below — part of the library's image, so every GPU that loads the library holds
+// these kStaticChunks * 32 bytes (1 MiB) until the process exits, used or not.
+//
+// Host code cannot use the name `g_static_schedule` as a pointer: on the host it is only a handle for the
+// runtime's symbol calls.  static_schedule_setup() asks the runtime for the array's address on the CURRENT device
+// (once per device, remembered) and that address is what the kernel receives.
+//
+// The array is shared by every call on a device and keeps whatever the last call wrote.  Nothing in it has to
+// start at zero: a launch reads entries [0, n) only, and the call has just written exactly those.  Two calls whose
+// GPU work overlaps (different streams, no event between them) race on it; calls on one stream are ordered.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) Chunk g_static_schedule[kStaticChunks];
+
+namespace {
+struct StaticSetup { Chunk* addr = nullptr; uint32_t num_sms = 0; };
+std::mutex g_static_mu;
+StaticSetup g_static_setup[64];
+}  // namespace
+
+int static_schedule_setup(Chunk** addr, uint32_t* num_sms) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return (int)e;
+  if (dev < 0 || dev >= 64) return (int)cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  StaticSetup& su = g_static_setup[dev];
+  if (!su.addr) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_schedule);       // the array's address on device `dev` (current)
+    if (e != cudaSuccess) return (int)e;
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return (int)e;
+    su.num_sms = (uint32_t)sms;
+    su.addr = (Chunk*)p;
+  }
+  *addr = su.addr;
+  *num_sms = su.num_sms;
+  return 0;
+}
+
+int launch_copy_static(Mode mode, const KernelParams& kp, const Chunk* host_chunks, uint32_t n, Chunk* device_addr,
+                       const LaunchShape& ls, void* stream) {
+  if (!host_chunks || !device_addr || n == 0 || n > kStaticChunks || ls.variant != FLOWKV_VARIANT_LDST)
+    return (int)cudaErrorInvalidValue;
+  cudaStream_t st = (cudaStream_t)stream;
+  // Pageable source: the runtime copies it into its own staging before it returns, so the caller may free the plan
+  // right after this call; the copy itself is ordered on `st` like any other, behind the previous call's kernel.
+  cudaError_t e = cudaMemcpyAsync(device_addr, host_chunks, (size_t)n * sizeof(Chunk), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return (int)e;
+  return launch_with(mode, kp, GlobalChunks{device_addr}, ls, st, nullptr);
 }
 
 }  // namespace flowkv

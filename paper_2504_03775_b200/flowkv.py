@@ -31,6 +31,7 @@ LAYOUTS = {"lkbthd": FLOWKV_LAYOUT_LKBTHD, "blkhtd": FLOWKV_LAYOUT_BLKHTD, "stri
            "blkthd": FLOWKV_LAYOUT_BLKTHD}
 
 FLOWKV_VERSION = 4          # include/flowkv.h; the struct layouts below are this version's
+FLOWKV_STATIC_SCHEDULE_ENTRIES = 32768      # include/flowkv.h: capacity of flowkv_transfer_static's fixed device array
 
 EXPORTS = ["flowkv_version", "flowkv_pool_strides", "flowkv_plan", "flowkv_plan_host", "flowkv_plan_info", "flowkv_transfer",
            "flowkv_pack", "flowkv_unpack", "flowkv_plan_destroy", "flowkv_status_string", "flowkv_last_error",
@@ -39,7 +40,7 @@ EXPORTS = ["flowkv_version", "flowkv_pool_strides", "flowkv_plan", "flowkv_plan_
            "flowkv_window_bytes", "flowkv_pack_window", "flowkv_unpack_window", "flowkv_via_host_scratch_bytes",
            "flowkv_transfer_tables", "flowkv_transfer_tables_layers", "flowkv_pack_tables", "flowkv_unpack_tables",
            "flowkv_alloc_create", "flowkv_alloc_allocate", "flowkv_alloc_free", "flowkv_alloc_stats",
-           "flowkv_alloc_destroy"]
+           "flowkv_alloc_destroy", "flowkv_transfer_static"]
 
 
 class flowkv_pool(C.Structure):
@@ -101,6 +102,7 @@ def _load() -> C.CDLL:
                                      P(flowkv_tuning), P(C.c_void_p)]
     lib.flowkv_plan_info.argtypes = [C.c_void_p, P(flowkv_plan_stats), P(P(flowkv_segment))]
     lib.flowkv_transfer.argtypes = [C.c_void_p, C.c_void_p]
+    lib.flowkv_transfer_static.argtypes = [C.c_void_p, C.c_void_p]
     lib.flowkv_pack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     lib.flowkv_unpack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     lib.flowkv_transfer_layers.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
@@ -384,6 +386,14 @@ def flowkv_plan_host(src: Optional[flowkv_pool], dst: Optional[flowkv_pool], req
 
 def flowkv_transfer(plan: Plan, stream: int = 0) -> None:
     _check(_lib.flowkv_transfer(plan.handle, C.c_void_p(stream)))
+
+
+def flowkv_transfer_static(plan: Plan, stream: int = 0) -> None:
+    """flowkv_transfer for callers that may not allocate device memory (an engine that owns all of HBM, a loop that
+    cannot take an allocator stall): the schedule rides in a fixed 1 MiB array inside the library instead of a
+    per-plan device buffer.  ``plan`` may come from :func:`flowkv_plan_host`.  At most
+    ``FLOWKV_STATIC_SCHEDULE_ENTRIES`` schedule entries; calls that overlap on the GPU race on the array."""
+    _check(_lib.flowkv_transfer_static(plan.handle, C.c_void_p(stream)))
 
 
 def flowkv_pack(plan: Plan, staging: int, nbytes: int, stream: int = 0) -> None:
