@@ -108,7 +108,7 @@ typedef struct {
                              * is plane_offsets[2l + c] = layer_offset[l] + c * s_kv.  The block, token and head strides
                              * describe one plane.  Such pools run the register / bulk-copy paths (no flat mode, no TMA
                              * tensor path) through kernels of their own; a schedule of <= 512 entries then always rides
-                             * in the largest (16 KiB) parameter form. */
+                             * in the 512-byte, 3 KiB or 16 KiB parameter form (16 / 96 / 512 entries). */
 } flowkv_pool;
 
 /* One request: its length and both sides' block-id lists.
@@ -204,7 +204,7 @@ FLOWKV_API flowkv_status flowkv_pool_strides(flowkv_pool* pool);
  *   out      : HOST pointer; receives the plan (caller destroys it).  Untouched on error.
  * The plan stays valid until destroyed; pools must stay alive while it is run.  The first plan (or table-driven call)
  * that names a new plane_offsets[] array copies it to the device once (16*L bytes on the library's own stream, waited
- * for; cached by content for the life of the process) — the one exception to "does not synchronise".  Inside a
+ * for; cached by content, at most 64 tables, see flowkv_trim) — the one exception to "does not synchronise".  Inside a
  * stream capture the table must already be cached: make one call (or build any plan) with the same offsets first.
  * Errors (nothing is allocated or enqueued when one is returned):
  *   INVALID_ARG  out NULL, both pools NULL, reqs NULL with n_reqs > 0, a table pointer NULL, unknown flag /
@@ -314,6 +314,8 @@ FLOWKV_API flowkv_status flowkv_transfer_via_host(const flowkv_plan_t* plan, voi
  *   max_tokens  upper bound of num_tokens[] known to the host (sizes the grid; tiles past a request's end exit)
  *   error_flag  DEVICE uint32 or NULL: OR-ed with 1 if a block id in use is outside its pool (that tile is
  *               skipped, nothing out of bounds is touched); the host cannot validate what it never sees.
+ *               OR-ed with 4 if a request's length on the device is above max_tokens: the grid was sized from
+ *               max_tokens, so that request's tokens from max_tokens (rounded up to a tile) on are NOT moved.
  *               The library only ever ORs bits into the flag and never clears or reads it: the CALLER zeroes it
  *               (cudaMemsetAsync on `stream` before the call, or once if it reads "any error since then") and
  *               reads it back after synchronising `stream`.
@@ -346,7 +348,8 @@ FLOWKV_API flowkv_status flowkv_transfer_tables_layers(const flowkv_pool* src, c
  *               — the "cumulative sequence lengths" array servers already keep on the device.
  *   window      DEVICE or mapped pinned HOST pointer, 16-B aligned; `bytes` = its capacity.  The host cannot see the
  *               total length, so the bound is enforced on the device: a request that would reach past `bytes` is
- *               skipped whole and error_flag is OR-ed with 2 (1 = a block id out of range, as above).
+ *               skipped whole and error_flag is OR-ed with 2 (1 = a block id out of range, 4 = a request longer
+ *               than max_tokens, as above).
  * One launch (zero if n_reqs, max_tokens or the layer range is empty).  Errors as flowkv_transfer_tables, plus
  * INVALID_ARG for a layer range outside [0, num_layers] or a NULL window / cu_tokens, ALIGN for the window. */
 FLOWKV_API flowkv_status flowkv_pack_tables(const flowkv_pool* src, const int32_t* src_tables, const uint64_t* cu_tokens,
@@ -394,6 +397,17 @@ FLOWKV_API flowkv_status flowkv_transfer_static(const flowkv_plan_t* plan, void*
  * given, so kernels already queued on THAT stream stay valid; if the plan was run on another stream,
  * synchronise that stream first.  NULL is ignored. */
 FLOWKV_API void flowkv_plan_destroy(flowkv_plan_t* plan);
+
+/* Process-lifetime caches, for long-lived servers.  The library keeps, per process: the device copies of
+ * plane_offsets[] tables (at most 64; beyond that the least recently used table that no plan holds is dropped, after a
+ * device-wide synchronisation), pinned host buffers that stage plan uploads (64 KiB and up each, at most 256, only
+ * as many as there were uploads in flight at once), and the helper streams / events of flowkv_transfer_via_host (at
+ * most 8 sets).  flowkv_trim() gives back everything that is idle right now: tables no plan references (it
+ * synchronises the device first — call it from a quiet moment, never inside a stream capture), staging buffers whose
+ * upload has finished, unused helper streams.  Plans stay valid.  flowkv_cache_counts() reports what is held
+ * (either pointer may be NULL). */
+FLOWKV_API flowkv_status flowkv_trim(void);
+FLOWKV_API flowkv_status flowkv_cache_counts(uint32_t* plane_offset_tables, uint32_t* pinned_buffers);
 
 /* FLOWKV_VERSION the library was built with.  The layout of flowkv_pool changed in version 4 (plane_offsets): a caller
  * compiled against another header must not pass structs to this library — compare before the first call. */

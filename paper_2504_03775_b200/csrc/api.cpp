@@ -111,6 +111,25 @@ class PinnedCache {
     std::lock_guard<std::mutex> lk(mu_);
     free_.push_back(b);
   }
+  // flowkv_trim(): give back every cached buffer whose last upload has finished (the others stay until a later trim).
+  void trim() {
+    std::vector<PinnedBuf> dead;
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      for (size_t i = 0; i < free_.size();) {
+        if (free_[i].pending && cudaEventQuery(free_[i].ev) != cudaSuccess) { ++i; continue; }
+        dead.push_back(free_[i]);
+        free_.erase(free_.begin() + i);
+        --n_alive_;
+      }
+    }
+    (void)cudaGetLastError();             // cudaErrorNotReady from the queries above is not an error
+    for (PinnedBuf& b : dead) { cudaEventDestroy(b.ev); cudaFreeHost(b.p); }
+  }
+  size_t alive() {
+    std::lock_guard<std::mutex> lk(mu_);
+    return n_alive_;
+  }
 
  private:
   static constexpr size_t kMaxBuffers = 256;
@@ -155,7 +174,11 @@ cudaError_t upload_stream(int device, cudaStream_t* out, cudaMemPool_t* pool) {
       int off = 0;
       e = cudaMemPoolSetAttribute(mp, cudaMemPoolReuseAllowInternalDependencies, &off);
     }
-    if (e != cudaSuccess) { cudaStreamDestroy(st); return e; }
+    if (e != cudaSuccess) {
+      if (mp) cudaMemPoolDestroy(mp);
+      cudaStreamDestroy(st);
+      return e;
+    }
     g_plan_pool[device] = mp;
     g_upload_stream[device] = st;
   }
@@ -165,21 +188,23 @@ cudaError_t upload_stream(int device, cudaStream_t* out, cudaMemPool_t* pool) {
 }
 
 // Per-plane offset tables (flowkv_pool.plane_offsets, reading A22) as the kernels read them: DEVICE arrays, uploaded
-// once per distinct content and device and kept for the life of the process (a server has a handful of pools).  The
-// upload rides the library's own stream and is waited for here — the first plan that names a new table pays for it.
+// once per distinct content and device and shared by every plan / call that names the same offsets.  The upload rides
+// the library's own stream and is waited for — outside the cache's mutex, so a first-use upload on one thread does not
+// stall planning on the others.  The cache is bounded: beyond kMaxEntries tables the least recently used one that no
+// plan or running call holds is dropped, after a device-wide synchronisation (a kernel launched by a call that has
+// already returned may still be reading it).  That costs a stall, but only a process that keeps re-allocating its
+// per-layer cache tensors ever gets there; a server with a handful of pools never evicts.
 class PlaneOffsetCache {
  public:
+  static constexpr size_t kMaxEntries = 64;
+  // Looks the table up (or uploads it) and takes a reference; the holder calls release() when it is done launching
+  // (table-driven calls: right after the launch; plans: when the plan dies).
   cudaError_t get(int device, const int64_t* host, uint32_t n, const int64_t** out) {
     uint64_t h = 1469598103934665603ull ^ (uint64_t)device;           // FNV-1a over the offsets
     for (uint32_t i = 0; i < n; ++i) { h ^= (uint64_t)host[i]; h *= 1099511628211ull; }
-    std::lock_guard<std::mutex> lk(mu_);
-    auto range = entries_.equal_range(h);
-    for (auto it = range.first; it != range.second; ++it) {
-      const Entry& e = it->second;
-      if (e.device == device && e.host.size() == n && memcmp(e.host.data(), host, n * sizeof(int64_t)) == 0) {
-        *out = e.dev;
-        return cudaSuccess;
-      }
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      if (Entry* e = find(h, device, host, n)) { ++e->refs; e->last_use = ++tick_; *out = e->dev; return cudaSuccess; }
     }
     cudaStream_t up = nullptr;
     cudaMemPool_t mp = nullptr;
@@ -193,15 +218,73 @@ class PlaneOffsetCache {
     e = cudaMemcpyAsync(en.dev, en.host.data(), n * sizeof(int64_t), cudaMemcpyHostToDevice, up);
     if (e == cudaSuccess) e = cudaStreamSynchronize(up);
     if (e != cudaSuccess) { cudaFree(en.dev); return e; }
-    *out = en.dev;
-    entries_.emplace(h, std::move(en));      // never evicted: a kernel in flight may still be reading the table
+    int64_t* spare = nullptr;             // ours, if another thread uploaded the same table meanwhile
+    Entry victim;                         // the least recently used unreferenced table, if the cache is full
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      if (Entry* hit = find(h, device, host, n)) {
+        spare = en.dev;
+        ++hit->refs; hit->last_use = ++tick_; *out = hit->dev;
+      } else {
+        en.refs = 1;
+        en.last_use = ++tick_;
+        *out = en.dev;
+        entries_.emplace(h, std::move(en));
+        if (entries_.size() > kMaxEntries) {
+          auto lru = entries_.end();
+          for (auto it = entries_.begin(); it != entries_.end(); ++it)
+            if (it->second.refs == 0 && (lru == entries_.end() || it->second.last_use < lru->second.last_use)) lru = it;
+          if (lru != entries_.end()) { victim = std::move(lru->second); entries_.erase(lru); }
+        }
+      }
+    }
+    if (spare) cudaFree(spare);           // never handed out
+    if (victim.dev) retire(victim);
     return cudaSuccess;
+  }
+  void release(const int64_t* dev) {
+    if (!dev) return;
+    std::lock_guard<std::mutex> lk(mu_);
+    for (auto& kv : entries_)
+      if (kv.second.dev == dev) { if (kv.second.refs) --kv.second.refs; return; }
+  }
+  // flowkv_trim(): drop every table nobody holds.
+  void trim() {
+    std::vector<Entry> dead;
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      for (auto it = entries_.begin(); it != entries_.end();)
+        if (it->second.refs == 0) { dead.push_back(std::move(it->second)); it = entries_.erase(it); } else ++it;
+    }
+    for (Entry& e : dead) retire(e);
+  }
+  size_t size() {
+    std::lock_guard<std::mutex> lk(mu_);
+    return entries_.size();
   }
 
  private:
-  struct Entry { int device = -1; std::vector<int64_t> host; int64_t* dev = nullptr; };
+  struct Entry { int device = -1; std::vector<int64_t> host; int64_t* dev = nullptr; uint32_t refs = 0; uint64_t last_use = 0; };
+  Entry* find(uint64_t h, int device, const int64_t* host, uint32_t n) {
+    auto range = entries_.equal_range(h);
+    for (auto it = range.first; it != range.second; ++it) {
+      Entry& e = it->second;
+      if (e.device == device && e.host.size() == n && memcmp(e.host.data(), host, n * sizeof(int64_t)) == 0) return &e;
+    }
+    return nullptr;
+  }
+  static void retire(Entry& e) {          // outside the mutex: wait for whatever may still read the table, then free it
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != e.device) cudaSetDevice(e.device);
+    cudaDeviceSynchronize();
+    cudaFree(e.dev);
+    if (cur >= 0 && cur != e.device) cudaSetDevice(cur);
+    e.dev = nullptr;
+  }
   std::mutex mu_;
   std::unordered_multimap<uint64_t, Entry> entries_;
+  uint64_t tick_ = 0;
 };
 PlaneOffsetCache g_plane_offsets;
 
@@ -240,6 +323,14 @@ class ViaHostCache {
     std::lock_guard<std::mutex> lk(mu_);
     if (free_.size() < 8) { free_.push_back(c); return; }
     destroy(c);
+  }
+  void trim() {                           // flowkv_trim(): helper streams and events no plan is using
+    std::vector<ViaHostCtx*> dead;
+    {
+      std::lock_guard<std::mutex> lk(mu_);
+      dead.swap(free_);
+    }
+    for (ViaHostCtx* c : dead) destroy(c);
   }
   static void destroy(ViaHostCtx* c) {
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
@@ -329,6 +420,8 @@ class VectorCache {
 VectorCache g_vectors;
 
 void drop_plan(flowkv_plan_t* pl) {       // every way a plan object dies goes through here
+  g_plane_offsets.release(pl->d_src_plane_off);
+  g_plane_offsets.release(pl->d_dst_plane_off);
   g_vectors.give(pl);
   delete pl;
 }
@@ -399,7 +492,7 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
     ls.grid = (uint32_t)std::min<uint64_t>((uint64_t)use_sms * ctas, std::max<uint64_t>(n_tiles, 1));
     return;
   }
-  // Defaults from the tuning sweeps on B200 (profiles/r01_ncu.md §4):
+  // Defaults from the tuning sweeps on B200 (round 1):
   //  * one CTA-wide round of 512 threads x 4 x 32 B covers a 64 KiB tile;
   //  * the grid is a grid-stride loop capped at 256 CTAs per SM.  Up to that cap every tile gets its
   //    own CTA and the hardware CTA scheduler hands tiles to whichever SM frees up first, which
@@ -597,9 +690,18 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       }
       pl->on_device = true;
     }
-  } catch (const std::bad_alloc&) {
+  } catch (...) {
+    // any exception (bad_alloc, length_error from a vector, ...) ends here once, with everything the plan took so far
+    // given back: the device buffer (stream-ordered, on the upload stream it came from), the pinned staging buffer,
+    // the plane-offset references (drop_plan); guarded() then turns the exception into a status code
+    if (pl->d_buf) {
+      cudaStream_t up = nullptr;
+      cudaMemPool_t mp = nullptr;
+      if (upload_stream(pl->device, &up, &mp) == cudaSuccess) FK_ENQ cudaFreeAsync(pl->d_buf, up);
+    }
+    g_pinned.release(pl->staging);
     drop_plan(pl);
-    return fail(FLOWKV_ERR_NOMEM, "out of host memory");
+    throw;
   }
   *out = pl;
   return FLOWKV_OK;
@@ -1109,7 +1211,7 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   const int64_t *d_slo = nullptr, *d_dlo = nullptr;      // device copies of the per-plane offsets (A22), cached
   if (src && src->plane_offsets) e = g_plane_offsets.get(dev, src->plane_offsets, 2 * src->num_layers, &d_slo);
   if (e == cudaSuccess && dst && dst->plane_offsets) e = g_plane_offsets.get(dev, dst->plane_offsets, 2 * dst->num_layers, &d_dlo);
-  if (e != cudaSuccess) return fail_cuda(e, "upload of plane_offsets");
+  if (e != cudaSuccess) { g_plane_offsets.release(d_slo); return fail_cuda(e, "upload of plane_offsets"); }
   TablesParams tp{};
   tp.kp.src = src ? pool_side(*src) : dense_side(dense, g, l0, l1);
   tp.kp.dst = dst ? pool_side(*dst) : dense_side(dense, g, l0, l1);
@@ -1128,8 +1230,13 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   tp.granule_log2 = src && dst ? std::min(tp.src_bs_log2, tp.dst_bs_log2) : (src ? tp.src_bs_log2 : tp.dst_bs_log2);
   tp.q_per_req = (uint32_t)(((uint64_t)max_tokens + (1u << tp.granule_log2) - 1) >> tp.granule_log2);
   const uint64_t n_tiles = (uint64_t)tp.kp.n_planes * n_reqs * tp.q_per_req;
-  if (n_tiles >= (1ull << 31)) return fail(FLOWKV_ERR_UNSUPPORTED, "more than 2^31 tiles in one batch; split the batch");
+  if (n_tiles >= (1ull << 31)) {
+    g_plane_offsets.release(d_slo);
+    g_plane_offsets.release(d_dlo);
+    return fail(FLOWKV_ERR_UNSUPPORTED, "more than 2^31 tiles in one batch; split the batch");
+  }
   tp.n_tiles = (uint32_t)n_tiles;
+  tp.max_tokens = max_tokens;
   LaunchShape ls{};
   ls.vec_bytes = pick_vec(src, dst, g);
   if (!(src && dst) && (uintptr_t)dense % 32) ls.vec_bytes = 16;
@@ -1146,6 +1253,8 @@ flowkv_status tables_common(const flowkv_pool* src, const flowkv_pool* dst, cons
   tp.kp.vpr_log2 = log2_or_none(g.row_bytes / ls.vec_bytes);
   tp.kp.heads_log2 = log2_or_none(g.Hkv);
   const int rc = launch_tables(tp, ls, stream, &po);
+  g_plane_offsets.release(d_slo);        // held only while launching; an eviction waits for the device before it frees
+  g_plane_offsets.release(d_dlo);
   if (rc != 0) return fail_cuda((cudaError_t)rc, "kernel launch");
   g_launches.fetch_add(1, std::memory_order_relaxed);
   g_api_calls.fetch_add(1, std::memory_order_relaxed);
@@ -1250,6 +1359,19 @@ void flowkv_plan_destroy(flowkv_plan_t* pl) {
   if (pl->d_buf) FK_ENQ cudaFreeAsync(pl->d_buf, pl->stream);   // ordered after everything queued on the plan's stream
   g_pinned.release(pl->staging);
   drop_plan(pl);
+}
+
+flowkv_status flowkv_trim(void) {
+  g_plane_offsets.trim();
+  g_pinned.trim();
+  g_via_host.trim();
+  return FLOWKV_OK;
+}
+
+flowkv_status flowkv_cache_counts(uint32_t* plane_offset_tables, uint32_t* pinned_buffers) {
+  if (plane_offset_tables) *plane_offset_tables = (uint32_t)g_plane_offsets.size();
+  if (pinned_buffers) *pinned_buffers = (uint32_t)g_pinned.alive();
+  return FLOWKV_OK;
 }
 
 const char* flowkv_status_string(flowkv_status s) {
@@ -1465,6 +1587,12 @@ flowkv_status flowkv_unpack_tables(
     uint32_t layer_begin, uint32_t layer_end, uint32_t* error_flag, const flowkv_tuning* tuning,
     void* stream) {
   return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_unpack_tables(dst, dst_tables, cu_tokens, n_reqs, max_dst_blocks, max_tokens, window, bytes, layer_begin, layer_end, error_flag, tuning, stream); });
+}
+flowkv_status flowkv_trim(void) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_trim(); });
+}
+flowkv_status flowkv_cache_counts(uint32_t* plane_offset_tables, uint32_t* pinned_buffers) {
+  return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_cache_counts(plane_offset_tables, pinned_buffers); });
 }
 flowkv_status flowkv_transfer_static(const flowkv_plan_t* plan, void* stream) {
   return flowkv::guarded([&]() -> flowkv_status { return impl::flowkv_transfer_static(plan, stream); });

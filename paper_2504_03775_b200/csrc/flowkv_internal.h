@@ -142,6 +142,7 @@ struct TablesParams {
   uint32_t        q_per_req;              // tiles per (request, plane) = ceil(max_tokens / granule)
   uint32_t        src_num_blocks, dst_num_blocks;
   uint32_t        n_tiles;                // n_planes * n_reqs * q_per_req
+  uint32_t        max_tokens;             // the host's bound on the lengths; a longer request sets error bit 4
 };
 int launch_tables(const TablesParams& tp, const LaunchShape& ls, void* stream, const PlaneOffs* po = nullptr);
 

@@ -666,8 +666,8 @@ static int launch_with(Mode mode, const KernelParams& kp, const CS& cs, const La
 }
 
 // Pools whose planes are separate allocations (reading A22): the *_po kernels take the per-plane offset tables as one
-// more parameter.  They exist for the uploaded schedule and for the largest parameter form only (a plan of <= 512
-// entries rides in the 16 KiB form whatever its size), in span and rows mode — such pools are never flat and never on
+// more parameter.  They exist for the uploaded schedule and for three parameter forms (16, 96 and 512 entries), in span
+// and rows mode — such pools are never flat and never on
 // the TMA tensor path — so the kernels of every other pool stay exactly what they were.
 template <class CS>
 static int launch_with_po(Mode mode, const KernelParams& kp, const CS& cs, const LaunchShape& ls, cudaStream_t st,
@@ -694,7 +694,14 @@ static int launch_with_po(Mode mode, const KernelParams& kp, const CS& cs, const
 #undef FK_LAUNCH_PO
 }
 
-// The parameter block of the larger forms (8-16 KiB) is built on the heap, not on the stack of every launch.
+// The parameter block of the larger forms (8-16 KiB) is not built on the stack of every launch, nor allocated and freed
+// per launch: each thread keeps one block per form for its lifetime (cudaLaunchKernelEx copies the arguments before it
+// returns, so the block is free again at once).
+template <uint32_t N>
+static ParamChunks<N>& param_scratch() {
+  static thread_local ParamChunks<N> pc;
+  return pc;
+}
 template <uint32_t N>
 static int launch_inline(Mode mode, const KernelParams& kp, const Chunk* host_chunks, uint32_t n, const LaunchShape& ls,
                          cudaStream_t st, const RowsTma* tma) {
@@ -703,12 +710,21 @@ static int launch_inline(Mode mode, const KernelParams& kp, const Chunk* host_ch
     memcpy(pc.c, host_chunks, (size_t)n * sizeof(Chunk));
     return launch_with(mode, kp, pc, ls, st, tma);
   }
-  ParamChunks<N>* pc = new (std::nothrow) ParamChunks<N>;
-  if (!pc) return (int)cudaErrorMemoryAllocation;
-  memcpy(pc->c, host_chunks, (size_t)n * sizeof(Chunk));
-  const int rc = launch_with(mode, kp, *pc, ls, st, tma);
-  delete pc;
-  return rc;
+  ParamChunks<N>& pc = param_scratch<N>();
+  memcpy(pc.c, host_chunks, (size_t)n * sizeof(Chunk));
+  return launch_with(mode, kp, pc, ls, st, tma);
+}
+template <uint32_t N>
+static int launch_inline_po(Mode mode, const KernelParams& kp, const Chunk* host_chunks, uint32_t n, const LaunchShape& ls,
+                            cudaStream_t st, const PlaneOffs& po) {
+  if (N <= 96) {
+    ParamChunks<N> pc;
+    memcpy(pc.c, host_chunks, (size_t)n * sizeof(Chunk));
+    return launch_with_po(mode, kp, pc, ls, st, po);
+  }
+  ParamChunks<N>& pc = param_scratch<N>();
+  memcpy(pc.c, host_chunks, (size_t)n * sizeof(Chunk));
+  return launch_with_po(mode, kp, pc, ls, st, po);
 }
 
 int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, const Chunk* host_chunks,
@@ -717,12 +733,11 @@ int launch_copy(Mode mode, const KernelParams& kp, const Chunk* device_chunks, c
   if (host_chunks && n_host_chunks > kInlineChunks) return (int)cudaErrorInvalidValue;
   if (po && (po->src || po->dst)) {        // planes of a side are separate allocations (A22)
     if (!host_chunks) return launch_with_po(mode, kp, GlobalChunks{device_chunks}, ls, st, *po);
-    ParamChunks<kInlineChunks>* pc = new (std::nothrow) ParamChunks<kInlineChunks>;
-    if (!pc) return (int)cudaErrorMemoryAllocation;
-    memcpy(pc->c, host_chunks, (size_t)n_host_chunks * sizeof(Chunk));
-    const int rc = launch_with_po(mode, kp, *pc, ls, st, *po);
-    delete pc;
-    return rc;
+    // small schedules take the 512-byte / 3 KiB parameter forms like every other pool (parameter bytes cost launch
+    // time); the larger ones share the 16 KiB form
+    if (n_host_chunks <= kInlineTiers[0]) return launch_inline_po<kInlineTiers[0]>(mode, kp, host_chunks, n_host_chunks, ls, st, *po);
+    if (n_host_chunks <= kInlineTiers[1]) return launch_inline_po<kInlineTiers[1]>(mode, kp, host_chunks, n_host_chunks, ls, st, *po);
+    return launch_inline_po<kInlineTiers[3]>(mode, kp, host_chunks, n_host_chunks, ls, st, *po);
   }
   if (host_chunks) {                       // small plan: the schedule rides in the kernel parameters
     if (n_host_chunks <= kInlineTiers[0]) return launch_inline<kInlineTiers[0]>(mode, kp, host_chunks, n_host_chunks, ls, st, tma);
@@ -776,6 +791,9 @@ __device__ __forceinline__ void tables_kernel(const TablesParams& tp, const int6
     uint64_t tok0 = 0;                                 // tokens of the requests before r (dense side only)
     if (tp.cu_tokens) { tok0 = __ldg(tp.cu_tokens + r); T = (uint32_t)(__ldg(tp.cu_tokens + r + 1) - tok0); }
     else              { T = __ldg(tp.num_tokens + r); }
+    // A length above the host's max_tokens breaks the call's contract: the grid was sized from max_tokens, so the
+    // tokens past it are never visited.  The host cannot see the lengths; the request's first tile reports it (bit 4).
+    if (T > tp.max_tokens && q == 0 && pl == 0 && tp.error && lane == 0) atomicOr(tp.error, 4u);
     const uint32_t t0 = q << tp.granule_log2;
     if (t0 >= T) continue;
     const uint32_t n = min(g, T - t0);

@@ -40,7 +40,7 @@ EXPORTS = ["flowkv_version", "flowkv_pool_strides", "flowkv_plan", "flowkv_plan_
            "flowkv_window_bytes", "flowkv_pack_window", "flowkv_unpack_window", "flowkv_via_host_scratch_bytes",
            "flowkv_transfer_tables", "flowkv_transfer_tables_layers", "flowkv_pack_tables", "flowkv_unpack_tables",
            "flowkv_alloc_create", "flowkv_alloc_allocate", "flowkv_alloc_free", "flowkv_alloc_stats",
-           "flowkv_alloc_destroy", "flowkv_transfer_static"]
+           "flowkv_alloc_destroy", "flowkv_transfer_static", "flowkv_trim", "flowkv_cache_counts"]
 
 
 class flowkv_pool(C.Structure):
@@ -103,6 +103,8 @@ def _load() -> C.CDLL:
     lib.flowkv_plan_info.argtypes = [C.c_void_p, P(flowkv_plan_stats), P(P(flowkv_segment))]
     lib.flowkv_transfer.argtypes = [C.c_void_p, C.c_void_p]
     lib.flowkv_transfer_static.argtypes = [C.c_void_p, C.c_void_p]
+    lib.flowkv_trim.argtypes = []
+    lib.flowkv_cache_counts.argtypes = [P(C.c_uint32), P(C.c_uint32)]
     lib.flowkv_pack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     lib.flowkv_unpack.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
     lib.flowkv_transfer_layers.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p]
@@ -486,6 +488,18 @@ def flowkv_unpack_tables(dst: flowkv_pool, dst_tables: int, cu_tokens: int, n_re
                          tuning=None, stream: int = 0) -> None:
     _tables_window(_lib.flowkv_unpack_tables, dst, dst_tables, cu_tokens, n_reqs, max_dst_blocks, max_tokens, window, nbytes,
                    layer_begin, layer_end, error_flag, tuning, stream)
+
+
+def flowkv_trim() -> None:
+    """Give back the library's idle caches (plane-offset tables no plan holds, finished staging buffers, unused helper
+    streams).  Synchronises the device when it drops a table."""
+    _check(_lib.flowkv_trim())
+
+
+def flowkv_cache_counts() -> dict:
+    a, b = C.c_uint32(), C.c_uint32()
+    _check(_lib.flowkv_cache_counts(C.byref(a), C.byref(b)))
+    return {"plane_offset_tables": int(a.value), "pinned_buffers": int(b.value)}
 
 
 def flowkv_plan_destroy(plan: Plan) -> None:

@@ -642,7 +642,8 @@ def test_transfer_is_cuda_graph_capturable(upload):
 @pytest.mark.parametrize("layouts", [("lkbthd", "lkbthd"), ("lkbthd", "blkhtd"), ("blkthd", "blkthd")])
 @pytest.mark.parametrize("tuning", [None, {"variant": "bulk"}, {"plan_in_params": 1, "tile_bytes": 4096}])
 def test_guard_bands_around_both_pools_stay_intact(layouts, tuning):
-    """Own bounds check (compute-sanitizer is not available on the pool): each pool sits between two 64 KiB guard
+    """Own bounds check (compute-sanitizer is installed but refused on the pool's boxes — exit code 86, "closed on this
+    pool and stays closed", profiles/r03_sanitizer.md): each pool sits between two 64 KiB guard
     bands inside one allocation, the request names the FIRST and the LAST block of both pools and ends in a partial
     block; after transfer, pack and unpack every guard byte still holds its sentinel and dst == oracle."""
     GUARD = 64 << 10
@@ -1036,6 +1037,12 @@ def test_bench_starts_its_own_ranks_and_peer_mode_runs_on_one_gpu():
     j = json.loads(lines[0])
     assert j["n_gpus"] == 2 and j["gpu_launches"] == 10 and j["launches_per_batch"] == 1.0
     assert "CUDA IPC" in j["run"]["dst"]
+    # one record per rank: two processes, each launched its 10 kernels, moved its payload, and what it stored through the
+    # IPC mapping reads back equal to its own src pool on sampled tokens
+    pr = j["per_rank"]
+    assert len(pr) == 2 and [r["rank"] for r in pr] == [0, 1] and pr[0]["pid"] != pr[1]["pid"]
+    assert all(r["gpu_launches"] == 10 and r["payload_bytes_moved"] == 10 * j["config"]["payload_bytes"] for r in pr)
+    assert all(r["peer_sample_matches_src"] is True for r in pr)
 
 
 def test_hand_worked_golden_example_on_the_gpu():
@@ -1511,3 +1518,101 @@ def test_pool_from_per_layer_torch_tensors(split_kv):
         O.transfer(o_src, gplane, o_dst, gplane, stab, dtab, T)
         assert np.array_equal(o_dst, got.contiguous().view(torch.uint8).cpu().numpy().reshape(-1)), f"plane {p} (oracle)"
     plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# round 3: contract violations the host cannot see, bounded caches, small parameter forms for separate-plane pools
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("separate", [False, True])
+def test_table_driven_length_above_max_tokens_is_reported(separate):
+    """A device-side length above the host's max_tokens: the grid was sized from max_tokens, so the tokens past it are
+    not moved — the kernel must say so (error bit 4) instead of truncating silently; everything below max_tokens
+    lands where the oracle puts it, nothing else is touched.  Both kernel forms (ordinary pool, per-plane offsets)."""
+    shape = synth.Shape(2, 2, 64, "fp16")
+    ssp, dsp = synth.PoolSpec("lkbthd", 16, 48), synth.PoolSpec("lkbthd", 16, 32)
+    src_buf, dst_buf = P.alloc_bytes(ssp.bytes(shape)), P.alloc_bytes(dsp.bytes(shape))
+    P.fill_values(src_buf, "bits", "fp16", 77)
+    P.fill_sentinel(dst_buf)
+    src_np = P.to_numpy(src_buf)
+    dst = P.describe(dsp, shape, dst_buf.data_ptr())
+    if separate:                                       # the same memory described plane by plane: the *_po kernel
+        plane = ssp.num_blocks * 16 * 2 * 64 * 2
+        src = F.make_pool(src_buf.data_ptr(), 2, 2, 64, 2, 48, 16, "lkbthd", plane_offsets=[p * plane for p in range(4)])
+    else:
+        src = P.describe(ssp, shape, src_buf.data_ptr())
+    rng = np.random.default_rng(5)
+    max_t, lens_h = 64, [64, 100, 17]                  # request 1 claims 100 tokens, the host said at most 64
+    ws = wd = 7                                        # the tables do hold 100 tokens' worth of ids
+    hs, hd = rng.permutation(48)[:21].astype(np.int32).reshape(3, 7), rng.permutation(32)[:21].astype(np.int32).reshape(3, 7)
+    st, dt = torch.from_numpy(hs).cuda(), torch.from_numpy(hd).cuda()
+    lens = torch.tensor(lens_h, dtype=torch.int32, device="cuda")
+    flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+    F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), 3, ws, wd, max_t, flag.data_ptr())
+    torch.cuda.synchronize()
+    assert int(flag.item()) == 4
+    gs, gd = G.geom(ssp, shape), G.geom(dsp, shape)
+    exp = np.full(dsp.bytes(shape), P.SENTINEL_BYTE, np.uint8)
+    for i, t in enumerate(lens_h):
+        t = min(t, max_t)
+        O.transfer(src_np, gs, exp, gd, hs[i, :-(-t // 16)], hd[i, :-(-t // 16)], t)
+    G.assert_same(P.to_numpy(dst_buf), exp, "tokens below max_tokens move, the rest is reported, not moved")
+    flag.zero_()                                       # within the bound: no bit
+    lens.copy_(torch.tensor([64, 64, 17], dtype=torch.int32))
+    F.flowkv_transfer_tables(src, dst, st.data_ptr(), dt.data_ptr(), lens.data_ptr(), 3, ws, wd, max_t, flag.data_ptr())
+    torch.cuda.synchronize()
+    assert int(flag.item()) == 0
+
+
+@pytest.mark.parametrize("tokens", [40, 600, 3000, 20000])
+def test_separate_plane_pools_in_every_parameter_form(tokens):
+    """Pools with plane_offsets and a schedule of 3 / 38 / 188 / 1250 entries: the 512-byte, 3 KiB and 16 KiB parameter
+    forms of the *_po kernels and the uploaded schedule, span and rows mode, against the oracle."""
+    shape = synth.Shape(2, 2, 64, "fp16")
+    for dst_layout, dst_bs in (("lkbthd", 16), ("blkhtd", 64)):
+        w = synth.make_workload(f"po_tiers_{tokens}_{dst_layout}", 8800 + tokens, shape, [tokens], "lkbthd", 16, ("fixed", 1), None,
+                                dst_layout, dst_bs, ("contiguous",), None, value_dist="bits")
+        dp = P.DevicePools(w, separate_src_layers=True)
+        src_np = np.concatenate([P.to_numpy(t) for t in dp.src_layers])
+        plan = dp.plan(F.FLOWKV_CHECK_DST_ALIAS)
+        n0 = F.flowkv_launch_count()
+        plan.transfer(torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert F.flowkv_launch_count() - n0 == 1
+        assert (plan.stats["plan_device_bytes"] == 0) == (plan.stats["n_chunks_transfer"] <= 512)
+        G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), w.name)
+
+
+def test_plane_offset_tables_stay_bounded_and_trim_gives_them_back():
+    """4,000 distinct plane_offsets tables (a server that keeps re-allocating its per-layer tensors): the library holds
+    at most 64 + those that live plans reference; a table an alive plan uses survives any number of evictions and the
+    plan still moves the right bytes; flowkv_trim() drops what nobody holds."""
+    shape = synth.Shape(2, 2, 64, "fp16")
+    w = synth.make_workload("po_cache", 8900, shape, [700], "lkbthd", 16, ("geometric", 2.0), None,
+                            "lkbthd", 16, ("contiguous",), None, value_dist="bits")
+    dp = P.DevicePools(w, separate_src_layers=True)
+    src_np = np.concatenate([P.to_numpy(t) for t in dp.src_layers])
+    s = torch.cuda.current_stream().cuda_stream
+    F.flowkv_trim()
+    base_tables = F.flowkv_cache_counts()["plane_offset_tables"]
+    keeper = dp.plan(F.FLOWKV_CHECK_DST_ALIAS, None, s)              # holds dp.src's table for the whole test
+    assert F.flowkv_cache_counts()["plane_offset_tables"] == base_tables + 1
+    plane = 64 * 16 * 2 * 64 * 2
+    big = P.alloc_bytes(4 * plane + 16 * 4000 + 4096)
+    for i in range(4000):                                             # 4,000 pools that differ in one plane offset
+        offs = [0, plane, 2 * plane, 3 * plane + 16 * (i + 1)]
+        pool = F.make_pool(big.data_ptr(), 2, 2, 64, 2, 64, 16, "lkbthd", plane_offsets=offs)
+        F.flowkv_plan(pool, None, [F.Request(16, np.array([i % 64], np.int32), None)], 0, None, s).destroy()
+        if i % 500 == 0:
+            assert F.flowkv_cache_counts()["plane_offset_tables"] <= 64 + 1 + base_tables
+    assert F.flowkv_cache_counts()["plane_offset_tables"] <= 64 + 1 + base_tables
+    keeper.transfer(s)                                                # its table was never evicted
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "plan that outlived 4,000 cache insertions")
+    F.flowkv_trim()
+    assert F.flowkv_cache_counts()["plane_offset_tables"] == base_tables + 1        # only the keeper's (and what earlier tests still hold)
+    keeper.destroy()
+    F.flowkv_trim()
+    assert F.flowkv_cache_counts()["plane_offset_tables"] == base_tables
+    dp.plan(F.FLOWKV_CHECK_DST_ALIAS, None, s).transfer(s)            # and everything still works afterwards
+    torch.cuda.synchronize()
+    G.assert_same(P.to_numpy(dp.dst_buf), G.oracle_transfer(w, src_np), "after trim")
