@@ -3,7 +3,6 @@
 length {1, 2, 8, 64, contiguous}, plus the device -> pinned-host pack path at 32,768 tokens.
 
     python bench_sweep.py [--out gpurun_out/sweep.json] [--reps 20] [--quick] [--tokens 1024,4096] [--runs 1,0]
-    python bench_sweep.py --tuning-grid [--tokens 128,512,1024,4096]     # A/B grid of launch shapes on the small points
     python bench_sweep.py --table3          # the paper's own request sizes (Table 3: 500 .. 12,000 tokens)
 
 Per point: payload, kernel time (CUDA events, mean and min over reps, L2 flushed between reps when
@@ -30,23 +29,23 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
-def main(argv=None) -> None:
+def main(argv=None, emit=None) -> list:
+    """Runs the sweep and returns its rows.  ``emit(row)`` is called per finished row (default: print the row as a
+    JSON line on stdout); bench.py passes its own so that its stdout stays ONE JSON line."""
+    if emit is None:
+        emit = lambda row: print(json.dumps(row), flush=True)
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(ROOT, "gpurun_out", "sweep.json"))
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--tuning", default=None)
     ap.add_argument("--no-baselines", action="store_true")
+    ap.add_argument("--no-pinned-pack", action="store_true", help="skip the device -> pinned host leg at 32,768 tokens")
     ap.add_argument("--tokens", default=None, help="comma-separated request lengths (default: the whole sweep)")
     ap.add_argument("--runs", default=None, help="comma-separated src run lengths, 0 = contiguous")
     ap.add_argument("--table3", action="store_true",
                     help="the paper's Table 3 request sizes (500 .. 12,000 tokens, src runs ~ Geometric(mean 4)); adds the "
                          "latency of the host route (flowkv_plan + flowkv_transfer_via_host: pool -> pinned host -> pool)")
-    ap.add_argument("--chunk-grid", action="store_true",
-                    help="with --table3: the host route's latency for n_chunks = 1 .. 64 per request size (what the "
-                         "library's default chunk rule was fitted to)")
-    ap.add_argument("--tuning-grid", action="store_true",
-                    help="time a grid of tile sizes / CTA shapes per point instead of the baselines (launch-shape A/B)")
     args = ap.parse_args(argv)
 
     import torch
@@ -69,8 +68,6 @@ def main(argv=None) -> None:
         tokens = [int(x) for x in args.tokens.split(",")]
     if args.runs and not args.table3:
         runs = [int(x) for x in args.runs.split(",")]
-    if args.tuning_grid:
-        args.no_baselines = True
     max_nb = (max(tokens) + 15) // 16
     src_spec_max = synth.PoolSpec("lkbthd", 16, max(16384, 2 * max_nb))
     src_buf = P.alloc_bytes(src_spec_max.bytes(shape))
@@ -146,24 +143,6 @@ def main(argv=None) -> None:
                 for _ in range(8):
                     plan.transfer(s)
             b2b = timed(eight, max(3, args.reps // 4), do_flush)[0] / 8
-            if args.tuning_grid:
-                grid_rows = []
-                for tb in (8192, 16384, 32768, 65536, 131072):
-                    for thr, grp in ((128, 64), (128, 128), (256, 64), (256, 128), (256, 256), (512, 64), (512, 128),
-                                     (512, 256), (512, 512)):
-                        if grp * 32 > tb:               # more threads than 32-byte vectors in a tile: idle lanes
-                            continue
-                        tn = dict(tuning or {}, tile_bytes=tb, threads=thr, group_threads=grp)
-                        p3 = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_PACK | F.FLOWKV_PLAN_NO_UNPACK, tn, s)
-                        p3.transfer(s); torch.cuda.synchronize()
-                        m3, n3 = timed(lambda: p3.transfer(s), args.reps, do_flush)
-                        grid_rows.append({"tile_bytes": tb, "threads": thr, "group_threads": grp, "grid": p3.stats["grid"],
-                                          "kernel_us_med": m3 * 1e3, "kernel_us_min": n3 * 1e3})
-                        p3.destroy()
-                best = min(grid_rows, key=lambda r: r["kernel_us_med"])
-                print(json.dumps({"tokens": T, "run": run or "contig", "default_us": med * 1e3, "plain_copy_us": pmed * 1e3,
-                                  "default_shape": {k: st[k] for k in ("tile_bytes", "threads", "group_threads", "grid")},
-                                  "best": best, "grid": grid_rows}), flush=True)
             row = {"tokens": T, "run": ("geometric(4)" if args.table3 else run or "contig"), "segments": st["n_segments"], "payload_bytes": payload,
                    "plain_copy_ms_med": pmed, "plain_copy_ms_min": pmn, "frac_of_plain_copy": pmed / med,
                    "graph_replay_ms_med": gmed, "back_to_back_ms_per_launch": b2b,
@@ -191,26 +170,6 @@ def main(argv=None) -> None:
                         hl.append((time.perf_counter() - t0) * 1e3)
                     pv.destroy()
                 del scratch
-                if args.chunk_grid:
-                    grid = {}
-                    for nc in (1, 2, 4, 8, 16, 32, 64):
-                        pv = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
-                        sbn = F.flowkv_via_host_scratch_bytes(pv, nc)
-                        pv.destroy()
-                        scr = P.alloc_bytes(sbn)
-                        gl = []
-                        for i in range(9):
-                            torch.cuda.synchronize()
-                            t0 = time.perf_counter()
-                            pv = F.flowkv_plan(src, dst, reqs, F.FLOWKV_PLAN_NO_TRANSFER, tuning, s)
-                            F.flowkv_transfer_via_host(pv, via_host.data_ptr(), payload, nc, 0, s, scr.data_ptr(), sbn)
-                            torch.cuda.synchronize()
-                            if i:
-                                gl.append((time.perf_counter() - t0) * 1e3)
-                            pv.destroy()
-                        del scr
-                        grid[nc] = float(np.median(gl))
-                    row["via_host_latency_ms_by_chunks"] = grid
                 row["via_host_latency_ms_plan_to_done"] = float(np.median(hl))
                 row["via_host_GBps_each_way"] = payload / (float(np.median(hl)) * 1e-3) / 1e9
             if not args.no_baselines:
@@ -225,11 +184,11 @@ def main(argv=None) -> None:
                     row["blockwise_memcpy"] = {"calls": calls, "ms": a.elapsed_time(b)}
             plan.destroy()
             rows.append(row)
-            print(json.dumps(row), flush=True)
+            emit(row)
 
     # ---- device -> pinned host pack at the 32k-token point ------------------------------------------------------
     T = 32768
-    if T in tokens and not args.table3:
+    if T in tokens and not args.table3 and not args.no_pinned_pack:
         nbytes = T * shape.bytes_per_token
         host = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
         dev_flat = dst_buf[:nbytes]
@@ -255,11 +214,13 @@ def main(argv=None) -> None:
                    "link_memcpy_d2h_GBps": link_d2h, "link_memcpy_h2d_GBps": link_h2d, "launches": 1}
             plan.destroy()
             rows.append(row)
-            print(json.dumps(row), flush=True)
+            emit(row)
         del host
 
-    os.makedirs(os.path.dirname(args.out), exist_ok=True)
-    json.dump(rows, open(args.out, "w"), indent=1)
+    if args.out:
+        os.makedirs(os.path.dirname(args.out), exist_ok=True)
+        json.dump(rows, open(args.out, "w"), indent=1)
+    return rows
 
 
 if __name__ == "__main__":
