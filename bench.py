@@ -161,12 +161,13 @@ def load_peaks() -> tuple:
 
 
 NCU_CAPTURES = {      # workload name -> (committed summary of its `ncu --set full` capture, commit whose kernels it measured)
-    "cfg2_llama8b_13k": ("r02_ncu_full_cfg2_fk_span_ldst.csv", "8d434be"),
+    "cfg2_llama8b_13k": ("r03_ncu_full_cfg2_fk_span_ldst.csv", "a3a5a7c"),
+    "cfg2_mig_13k+po": ("r03_ncu_full_cfg2mig_fk_rows_ldst_po.csv", "a3a5a7c"),
     "cfg2_llama8b_13k+po": ("r02_ncu_full_cfg2sep_fk_span_ldst_po.csv", "32ce955"),
     "cfg2_blkthd_13k": ("r02_ncu_full_cfg2bm_fk_flat_ldst.csv", "8d434be"),
     "cfg2_llama8b_13k+tables": ("r02_ncu_full_cfg2_fk_tables_ldst.csv", "8d434be"),
     "cfg3_batched_8b": ("r02_ncu_full_cfg3_fk_span_ldst.csv", "8d434be"),
-    "cfg4_hetero_70b": ("r02_ncu_full_cfg4_fk_rows_ldst.csv", "8d434be"),
+    "cfg4_hetero_70b": ("r03_ncu_full_cfg4_fk_rows_ldst.csv", "a3a5a7c"),
     "cfg4_hetero_70b+bulk": ("r02_ncu_full_cfg4_fk_rows_tma.csv", "8d434be"),
 }
 
@@ -745,6 +746,7 @@ def run_ours(args) -> None:
                 "roofline": roofline_of(m3, p3, w3.name + ("+tables" if args.device_tables else ""), m3["stats"], K3,
                                         args.device_tables),
                 "clocks": m3["clocks"], "gpu_launches": m3["launches"], "launches_per_batch": m3["launches"] / K3,
+                "cuda_api_calls_per_batch": m3["api_calls"] / K3,
                 "latency_ms_call_to_done": m3["latency_ms_call_to_done"],
                 "latency_ms_call_to_done_per_request": m3["latency_ms_call_to_done"] / max(len(w3.requests), 1)}
         del dp3
