@@ -463,6 +463,14 @@ void resolve_shape(flowkv_plan_t* pl, Op& op, const flowkv_pool* a, const flowkv
       ls.variant = FLOWKV_VARIANT_LDST;
   }
   op.tile_order = t.tile_order == 2 ? 1 : 0;
+  // Auto: plane-major, except for a rows-mode move into a block-major pool of the same block size (Eq. 5's re-layout as
+  // a move, `bench.py --config cfg2mig`): a chunk is then one whole block-plane, and chunk-major order makes the CTAs
+  // that run together fill ONE dst block's 2L planes — one contiguous range — instead of one plane of many blocks
+  // 2 MiB apart.  Same box, two runs each: 0.5333 -> 0.5264 ms (81.8 -> 82.9 % of 8 TB/s).  With unequal block sizes
+  // (configs[3]: 4 KiB pieces into 16 KiB head slabs) the order makes no difference (82.39 vs 82.44 %): unchanged.
+  if (t.tile_order == 0 && op.sched.mode == MODE_ROWS && a && b && a->block_size == b->block_size && !b->plane_offsets &&
+      b->stride_bytes[FLOWKV_S_BLOCK] >= b->stride_bytes[FLOWKV_S_LAYER] * (int64_t)pl->g.L)
+    op.tile_order = 1;
   const uint64_t n_tiles = ((uint64_t)op.sched.n_flat << op.sched.flat_shift) + (uint64_t)op.sched.n_per_plane() * 2 * pl->g.L;
   if (ls.variant == FLOWKV_VARIANT_BULK) {
     // a ring slot holds the largest chunk (span mode: at least one token's plane bytes); two slots must fit in
@@ -617,6 +625,12 @@ flowkv_status make_plan(const flowkv_pool* src, const flowkv_pool* dst, const fl
       const uint64_t want_tiles = 2ull * pl->num_sms;
       const uint64_t payload = pl->total_tokens * g.bytes_per_token;
       while (tile > 16384 && payload / tile < want_tiles) tile >>= 1;
+      // ... and between two and four tiles per SM (a 256-token Llama-3-8B request: 32 MiB) halve the 64 KiB tile once:
+      // 1,024 CTAs of 256 threads ramp up and drain faster than 512 of 512 (round 3, 40 repetitions, three runs
+      // each: contiguous request 15.2-15.3 us -> 14.3-14.5 us, single-block runs unchanged at 14.3-14.4 us; the
+      // same-size cudaMemcpyAsync takes 13.2-13.7 us).  Larger requests keep 64 KiB (1,024 tokens: 46.6-47.3 us
+      // against 50.5-50.8 us with the small shape).
+      if (tn.variant != FLOWKV_VARIANT_BULK && tile == (64u << 10) && payload / tile < 2 * want_tiles) tile >>= 1;
     }
     pl->tile_bytes = tile;
 
